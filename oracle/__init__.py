@@ -1,0 +1,151 @@
+"""ctypes shim over the CPU oracle (oracle/psync_oracle.cpp) -- TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this package.  It never imports the product package (paper_1702_05800_b200) and the
+product never imports it.  All arrays are numpy, host memory; bf16 gradients are uint16 bit
+patterns.  The arithmetic lives in the C++ file; this module only marshals arguments.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "psync_oracle.cpp"
+_LIB = _HERE / "libpsync_oracle.so"
+
+OK, EINVAL, ETOOFEW = 0, -1, -2
+F32, BF16 = 0, 1
+SGD, MOMENTUM, RMSPROP_MOM = 0, 1, 2
+EMA_POST, EMA_PRE, EMA_OFF = 0, 1, 2
+
+_lib = None
+
+
+def build(force: bool = False) -> Path:
+    """Compile the oracle with g++ (-O2, no fast-math, no FMA contraction, OpenMP)."""
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = _LIB.with_suffix(f".tmp{os.getpid()}.so")
+        cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+               "-Wall", "-Wextra", "-o", str(tmp), str(_SRC)]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def lib() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(str(_LIB))
+        i32, i64, f32, vp = ctypes.c_int32, ctypes.c_int64, ctypes.c_float, ctypes.c_void_p
+        L.oracle_select_first_n.argtypes = [vp, vp, i32, i32, i32, vp, vp]
+        L.oracle_select_first_n.restype = ctypes.c_int
+        L.oracle_aggregate_update.argtypes = [i64, i32, vp, i32, i32, vp, ctypes.c_int, vp, vp, vp, vp, vp,
+                                              ctypes.c_int, ctypes.c_int, f32, f32, f32, f32, f32]
+        L.oracle_aggregate_update.restype = ctypes.c_int
+        L.oracle_accumulate.argtypes = [vp, vp, ctypes.c_int, i64]
+        L.oracle_accumulate.restype = ctypes.c_int
+        L.oracle_apply_sum.argtypes = [i64, i32, vp, i32, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int,
+                                       f32, f32, f32, f32, f32]
+        L.oracle_apply_sum.restype = ctypes.c_int
+        L.oracle_ema.argtypes = [vp, vp, i64, f32]
+        L.oracle_ema.restype = ctypes.c_int
+        L.oracle_num_threads.restype = ctypes.c_int
+        L.oracle_set_num_threads.argtypes = [ctypes.c_int]
+        _lib = L
+    return _lib
+
+
+def _ptr(a):
+    return None if a is None else ctypes.c_void_p(a.ctypes.data)
+
+
+def _chk(a, dtype, name, n=None):
+    if a is None:
+        return
+    if not (isinstance(a, np.ndarray) and a.dtype == dtype and a.flags.c_contiguous):
+        raise TypeError(f"{name}: need a C-contiguous numpy array of {np.dtype(dtype)}")
+    if n is not None and a.size != n:
+        raise ValueError(f"{name}: need {n} elements, got {a.size}")
+
+
+def select_first_n(arrival, N, b, tags=None, t=0):
+    """-> (status, kept[int32 N] or None, t_nth or None).  PAPER.md:L130, L148-158."""
+    W = N + b
+    _chk(arrival, np.float32, "arrival", W)
+    _chk(tags, np.int32, "tags", W)
+    kept = np.full(max(N, 0), -1, dtype=np.int32)
+    t_nth = np.full(1, np.nan, dtype=np.float32)
+    st = lib().oracle_select_first_n(_ptr(arrival), _ptr(tags), t, N, b, _ptr(kept), _ptr(t_nth))
+    if st != OK:
+        return st, None, None
+    return st, kept, float(t_nth[0])
+
+
+def _grad_dtype(grads):
+    dt = grads[0].dtype
+    if dt == np.float32:
+        return F32
+    if dt == np.uint16:
+        return BF16
+    raise TypeError("gradients must be float32 or uint16 (bf16 bit patterns)")
+
+
+def aggregate_update(shard_off, N, grads, kept, theta, ema=None, state0=None, state1=None, opt=SGD,
+                     ema_mode=EMA_POST, gamma_t=0.0, alpha=0.0, mu=0.0, rho=0.0, eps=0.0):
+    """One step of Alg. 4 l.8-9 in place on theta / state / ema.  PAPER.md:L160-162."""
+    P = theta.size
+    shard_off = np.ascontiguousarray(shard_off, dtype=np.int64)
+    M = shard_off.size - 1
+    W = len(grads)
+    gd = _grad_dtype(grads)
+    for k, g in enumerate(grads):
+        _chk(g, grads[0].dtype, f"grads[{k}]", P)
+    _chk(kept, np.int32, "kept", N)
+    for nm, a in (("theta", theta), ("ema", ema), ("state0", state0), ("state1", state1)):
+        _chk(a, np.float32, nm, P)
+    ptrs = (ctypes.c_void_p * W)(*[g.ctypes.data for g in grads])
+    return lib().oracle_aggregate_update(P, M, _ptr(shard_off), N, W, ctypes.cast(ptrs, ctypes.c_void_p),
+                                         gd, _ptr(kept), _ptr(theta), _ptr(ema), _ptr(state0), _ptr(state1),
+                                         opt, ema_mode, gamma_t, alpha, mu, rho, eps)
+
+
+def accumulate(S, grad):
+    """S[i] += grad[i] in double (one kept worker); call in ascending kept order."""
+    _chk(S, np.float64, "S")
+    gd = _grad_dtype([grad])
+    _chk(grad, grad.dtype, "grad", S.size)
+    return lib().oracle_accumulate(_ptr(S), _ptr(grad), gd, S.size)
+
+
+def apply_sum(shard_off, N, S, theta, ema=None, state0=None, state1=None, opt=SGD, ema_mode=EMA_POST,
+              gamma_t=0.0, alpha=0.0, mu=0.0, rho=0.0, eps=0.0):
+    """Alg. 4 l.8-9 given the per-element sums S of the kept gradients."""
+    P = theta.size
+    shard_off = np.ascontiguousarray(shard_off, dtype=np.int64)
+    M = shard_off.size - 1
+    _chk(S, np.float64, "S", P)
+    for nm, a in (("theta", theta), ("ema", ema), ("state0", state0), ("state1", state1)):
+        _chk(a, np.float32, nm, P)
+    return lib().oracle_apply_sum(P, M, _ptr(shard_off), N, _ptr(S), _ptr(theta), _ptr(ema), _ptr(state0),
+                                  _ptr(state1), opt, ema_mode, gamma_t, alpha, mu, rho, eps)
+
+
+def ema_update(ema, theta, alpha):
+    """ema <- alpha ema + (1-alpha) theta in place.  PAPER.md:L40."""
+    _chk(ema, np.float32, "ema")
+    _chk(theta, np.float32, "theta", ema.size)
+    return lib().oracle_ema(_ptr(ema), _ptr(theta), ema.size, alpha)
+
+
+def num_threads() -> int:
+    return lib().oracle_num_threads()
+
+
+def set_num_threads(n: int) -> None:
+    lib().oracle_set_num_threads(n)

@@ -1,0 +1,274 @@
+// psync CPU oracle -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// A plain, slow, obviously-correct CPU statement of the parameter-server step of
+// "Revisiting Distributed Synchronous SGD" (arXiv 1702.05800), Algorithm 4
+// (de-interleaved in SURVEY.md section 2a):
+//
+//     G = {}; while |G| < N: wait for (G, t'); keep iff t' == t      (Alg. 4 l.2-6, L145-158)
+//     theta(t+1)[j] <- theta(t)[j] - (gamma_t / N) * sum_{G in G} G[j] (Alg. 4 l.8,  L160)
+//     ema(t)[j]     =  alpha * ema(t-1)[j] + (1 - alpha) * theta[j]    (Alg. 4 l.9,  L162; L40)
+//
+// with "the first N of N+b workers by arrival time are kept, the slowest b are
+// dropped" (section 3).  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may load this library.  It shares no code,
+// header, table or helper with the CUDA path (paper_1702_05800_b200/csrc) and
+// includes nothing but the C/C++ standard library.
+//
+// Arithmetic: every floating-point step is done in double on the fp32 (or bf16)
+// stored inputs, and each stored result is rounded once to fp32 by
+// static_cast<float>.  The scalar coefficients cross the interface as fp32 and the
+// derived coefficients (1/N, 1-alpha, 1-rho) are formed in fp32 first, then widened
+// (reading R8) -- the CUDA path does the same, so both sides multiply by
+// the same real numbers.
+//
+// Pins (tests/test_oracle_*.py, all `-m "not gpu"`): selection against
+// numpy's stable lexsort and exhaustive permutations; b=0 against numpy's mean;
+// N=1 against the arg-min worker; exact rational brute force (fractions.Fraction,
+// mpmath for the square root) for P <= 64; closed forms for constant gradients
+// (SGD, momentum, RMSProp second moment) and the constant-theta EMA; optimizer
+// reductions (mu=0, rho=1); a hand-worked dyadic example (tests/golden/).
+// Nothing here is "parity unpinned".
+//
+// Optional OpenMP (-fopenmp): the element loop is split over threads; per-element
+// arithmetic and order are untouched, so results are bit-identical to one thread.
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <utility>
+#include <vector>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+// Status codes (values fixed by the oracle's own contract; tests compare numbers).
+constexpr int ORACLE_OK = 0;
+constexpr int ORACLE_EINVAL = -1;
+constexpr int ORACLE_ETOOFEW = -2;
+
+// Gradient element types.
+constexpr int ORACLE_F32 = 0;
+constexpr int ORACLE_BF16 = 1;
+
+// Optimizers (a4 in SURVEY.md section 8a).
+constexpr int ORACLE_SGD = 0;
+constexpr int ORACLE_MOMENTUM = 1;
+constexpr int ORACLE_RMSPROP_MOM = 2;
+
+// EMA operand (reading R3).
+constexpr int ORACLE_EMA_POST = 0;  // ema uses the freshly updated theta(t+1)
+constexpr int ORACLE_EMA_PRE = 1;   // ema uses theta(t), the literal indexing of L162
+constexpr int ORACLE_EMA_OFF = 2;
+
+// bf16 -> double: a bf16 value is the upper 16 bits of an fp32 value; widening is exact.
+inline double widen_bf16(uint16_t h) {
+  uint32_t u = static_cast<uint32_t>(h) << 16;
+  float f;
+  std::memcpy(&f, &u, sizeof f);
+  return static_cast<double>(f);
+}
+
+inline double grad_at(const void* g, int dtype, int64_t i) {
+  if (dtype == ORACLE_F32) return static_cast<double>(static_cast<const float*>(g)[i]);
+  return widen_bf16(static_cast<const uint16_t*>(g)[i]);
+}
+
+struct Coeffs {
+  double gamma, alpha, one_minus_alpha, mu, rho, one_minus_rho, eps, inv_N;
+};
+
+// Derived coefficients formed in fp32, then widened (reading R8).
+inline Coeffs make_coeffs(int32_t N, float gamma_t, float alpha, float mu, float rho, float eps) {
+  Coeffs c;
+  c.gamma = static_cast<double>(gamma_t);
+  c.alpha = static_cast<double>(alpha);
+  c.one_minus_alpha = static_cast<double>(1.0f - alpha);
+  c.mu = static_cast<double>(mu);
+  c.rho = static_cast<double>(rho);
+  c.one_minus_rho = static_cast<double>(1.0f - rho);
+  c.eps = static_cast<double>(eps);
+  c.inv_N = static_cast<double>(1.0f / static_cast<float>(N));
+  return c;
+}
+
+// One element of Alg. 4 l.8-9 given S = sum of the kept gradients at this element.
+inline void apply_element(double S, const Coeffs& c, int opt, int ema_mode, float* theta, float* ema,
+                          float* state0, float* state1, int64_t i) {
+  const double G = S * c.inv_N;  // the mean gradient, (1/N) * sum   (L160)
+  const double th = static_cast<double>(theta[i]);
+  double th_new;
+  if (opt == ORACLE_SGD) {
+    // theta(t+1) = theta(t) - gamma_t * G                         (L40, L160)
+    th_new = th - c.gamma * G;
+  } else if (opt == ORACLE_MOMENTUM) {
+    // v <- mu v + G ; theta <- theta - gamma_t v                   (reading R6)
+    const double v = c.mu * static_cast<double>(state0[i]) + G;
+    state0[i] = static_cast<float>(v);
+    th_new = th - c.gamma * v;
+  } else {
+    // RMSProp with momentum, "decay" rho and "momentum" mu (L305, L315); the paper gives
+    // no equations -- DESIGN.md reading R5:
+    //   ms  <- rho ms + (1-rho) G^2
+    //   mom <- mu mom + gamma_t G / sqrt(ms + eps)
+    //   theta <- theta - mom
+    const double ms = c.rho * static_cast<double>(state0[i]) + c.one_minus_rho * (G * G);
+    const double mom = c.mu * static_cast<double>(state1[i]) + c.gamma * G / std::sqrt(ms + c.eps);
+    state0[i] = static_cast<float>(ms);
+    state1[i] = static_cast<float>(mom);
+    th_new = th - mom;
+  }
+  const float th_new_f = static_cast<float>(th_new);
+  theta[i] = th_new_f;
+  if (ema_mode != ORACLE_EMA_OFF) {
+    // ema = alpha * ema + (1 - alpha) * theta                      (L40, L162)
+    // POST uses the stored (fp32) theta(t+1); PRE uses the stored theta(t).
+    const double operand = (ema_mode == ORACLE_EMA_POST) ? static_cast<double>(th_new_f) : th;
+    ema[i] = static_cast<float>(c.alpha * static_cast<double>(ema[i]) + c.one_minus_alpha * operand);
+  }
+}
+
+bool args_ok(int64_t P, int32_t M, const int64_t* shard_off, int32_t N, int opt, int ema_mode,
+             const float* theta, const float* ema, const float* state0, const float* state1) {
+  if (P < 0 || M < 1 || N < 1 || !shard_off || !theta) return false;
+  if (shard_off[0] != 0 || shard_off[M] != P) return false;
+  for (int32_t j = 0; j < M; ++j)
+    if (shard_off[j + 1] < shard_off[j]) return false;
+  if (opt < ORACLE_SGD || opt > ORACLE_RMSPROP_MOM) return false;
+  if (ema_mode < ORACLE_EMA_POST || ema_mode > ORACLE_EMA_OFF) return false;
+  if (ema_mode != ORACLE_EMA_OFF && !ema) return false;
+  if (opt != ORACLE_SGD && !state0) return false;
+  if (opt == ORACLE_RMSPROP_MOM && !state1) return false;
+  return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+// ---------------------------------------------------------------------------------------------
+// Selection: the first N of W = N+b workers by arrival time (L130; Alg. 4 l.3-6, L148-158).
+//   arrival[W]  fp32 seconds; non-finite (NaN, +-inf) = never arrived (reading R13)
+//   tags[W]     or NULL; worker k is eligible iff tags[k] == t  (Alg. 4 l.5: "if t' == t")
+//   kept[N]     OUT ascending worker indices;  t_nth OUT (or NULL) the N-th smallest arrival
+// Ties on arrival time go to the lower worker index (reading R1).  Fewer than N eligible
+// workers -> ORACLE_ETOOFEW and kept / t_nth are left untouched.
+// ---------------------------------------------------------------------------------------------
+int oracle_select_first_n(const float* arrival, const int32_t* tags, int32_t t, int32_t N, int32_t b,
+                          int32_t* kept, float* t_nth) {
+  if (!arrival || !kept || N < 1 || b < 0) return ORACLE_EINVAL;
+  const int32_t W = N + b;
+  std::vector<std::pair<float, int32_t>> pairs;
+  for (int32_t k = 0; k < W; ++k) {
+    const bool eligible = std::isfinite(arrival[k]) && (tags == nullptr || tags[k] == t);
+    if (eligible) pairs.emplace_back(arrival[k], k);
+  }
+  if (static_cast<int32_t>(pairs.size()) < N) return ORACLE_ETOOFEW;
+  // Full sort by (time, worker index) with IEEE comparisons on the fp32 values (-0.0 == +0.0).
+  std::sort(pairs.begin(), pairs.end(), [](const std::pair<float, int32_t>& x, const std::pair<float, int32_t>& y) {
+    return x.first < y.first || (x.first == y.first && x.second < y.second);
+  });
+  std::vector<int32_t> first(N);
+  for (int32_t i = 0; i < N; ++i) first[i] = pairs[i].second;
+  std::sort(first.begin(), first.end());
+  for (int32_t i = 0; i < N; ++i) kept[i] = first[i];
+  if (t_nth) *t_nth = pairs[N - 1].first;
+  return ORACLE_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// One whole step, Alg. 4 l.8-9, written per shard j and per element as the definition reads.
+//   grads[W]     host pointers, each to P elements of grad_dtype laid out like theta
+//   kept[N]      worker indices to aggregate, summed in the order given (ascending from select)
+//   shard_off    [M+1], theta[j] = [shard_off[j], shard_off[j+1])
+// theta, ema, state0, state1 are updated in place (fp32 storage).
+// ---------------------------------------------------------------------------------------------
+int oracle_aggregate_update(int64_t P, int32_t M, const int64_t* shard_off, int32_t N, int32_t W,
+                            const void* const* grads, int grad_dtype, const int32_t* kept, float* theta,
+                            float* ema, float* state0, float* state1, int opt, int ema_mode, float gamma_t,
+                            float alpha, float mu, float rho, float eps) {
+  if (!args_ok(P, M, shard_off, N, opt, ema_mode, theta, ema, state0, state1)) return ORACLE_EINVAL;
+  if (!grads || !kept || W < N) return ORACLE_EINVAL;
+  if (grad_dtype != ORACLE_F32 && grad_dtype != ORACLE_BF16) return ORACLE_EINVAL;
+  for (int32_t n = 0; n < N; ++n)
+    if (kept[n] < 0 || kept[n] >= W || !grads[kept[n]]) return ORACLE_EINVAL;
+  const Coeffs c = make_coeffs(N, gamma_t, alpha, mu, rho, eps);
+  for (int32_t j = 0; j < M; ++j) {  // parameter server j owns theta[j]   (L42)
+    const int64_t lo = shard_off[j], hi = shard_off[j + 1];
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int64_t i = lo; i < hi; ++i) {
+      double S = 0.0;  // sum_{G in kept set} G[j]                  (L160)
+      for (int32_t n = 0; n < N; ++n) S += grad_at(grads[kept[n]], grad_dtype, i);
+      apply_element(S, c, opt, ema_mode, theta, ema, state0, state1, i);
+    }
+  }
+  return ORACLE_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// The same step split in two so that a caller can stream the kept buffers one at a time (the
+// paper-scale configs hold 10-20 GB of gradients): S[i] += G_k[i] for each kept k in ascending
+// order, then oracle_apply_sum.  Per element the additions happen in the same order as in
+// oracle_aggregate_update, so the two are bit-identical (tested).
+// ---------------------------------------------------------------------------------------------
+int oracle_accumulate(double* S, const void* grad, int grad_dtype, int64_t P) {
+  if (!S || !grad || P < 0) return ORACLE_EINVAL;
+  if (grad_dtype != ORACLE_F32 && grad_dtype != ORACLE_BF16) return ORACLE_EINVAL;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+  for (int64_t i = 0; i < P; ++i) S[i] += grad_at(grad, grad_dtype, i);
+  return ORACLE_OK;
+}
+
+int oracle_apply_sum(int64_t P, int32_t M, const int64_t* shard_off, int32_t N, const double* S, float* theta,
+                     float* ema, float* state0, float* state1, int opt, int ema_mode, float gamma_t, float alpha,
+                     float mu, float rho, float eps) {
+  if (!args_ok(P, M, shard_off, N, opt, ema_mode, theta, ema, state0, state1) || !S) return ORACLE_EINVAL;
+  const Coeffs c = make_coeffs(N, gamma_t, alpha, mu, rho, eps);
+  for (int32_t j = 0; j < M; ++j) {
+    const int64_t lo = shard_off[j], hi = shard_off[j + 1];
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int64_t i = lo; i < hi; ++i) apply_element(S[i], c, opt, ema_mode, theta, ema, state0, state1, i);
+  }
+  return ORACLE_OK;
+}
+
+// ema <- alpha * ema + (1 - alpha) * theta   (L40; Alg. 2 l.4 L87; Alg. 4 l.9 L162)
+int oracle_ema(float* ema, const float* theta, int64_t P, float alpha) {
+  if (!ema || !theta || P < 0) return ORACLE_EINVAL;
+  const double a = static_cast<double>(alpha);
+  const double oma = static_cast<double>(1.0f - alpha);
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+  for (int64_t i = 0; i < P; ++i)
+    ema[i] = static_cast<float>(a * static_cast<double>(ema[i]) + oma * static_cast<double>(theta[i]));
+  return ORACLE_OK;
+}
+
+// Threads the element loops use (1 without OpenMP); bench.py reports it as cpu_baseline.cores.
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+void oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+  if (n >= 1) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
+}  // extern "C"
