@@ -1,2 +1,13 @@
 """psync: the parameter-server step of synchronous SGD with backup workers (arXiv 1702.05800,
-Algorithm 4) as hand-written CUDA for sm_100a behind a C ABI (include/psync.h)."""
+Algorithm 4) as hand-written CUDA for sm_100a behind a C ABI (include/psync.h).
+
+`binding` mirrors the C entry points (argument marshalling only), `server` bundles the device
+buffers of one parameter server, `synth` draws the seeded synthetic workloads, `build` compiles
+libpsync.so in-tree.  Nothing in this package imports oracle/.
+"""
+from . import binding, synth  # noqa: F401
+from .binding import (PSYNC_BF16, PSYNC_ECUDA, PSYNC_EINVAL, PSYNC_EMA_OFF, PSYNC_EMA_POST, PSYNC_EMA_PRE,  # noqa: F401
+                      PSYNC_ETOOFEW, PSYNC_F32, PSYNC_MOMENTUM, PSYNC_OK, PSYNC_RMSPROP_MOM, PSYNC_SGD, PsyncError,
+                      make_grad_table, make_step, psync_aggregate_update, psync_ema, psync_launch_geometry,
+                      psync_select_first_n, psync_step_host, psync_step_host_workspace_bytes)
+from .server import ParameterServerStep  # noqa: F401

@@ -1,0 +1,259 @@
+"""Thin ctypes binding over libpsync.so (include/psync.h).  Argument marshalling ONLY: every step
+of the path (selection, aggregation, update, EMA) runs in the CUDA kernels behind the C ABI.
+
+torch is used for device memory and streams.  There is no CPU fallback: if the shared library is
+missing or a tensor is not on a CUDA device the call raises.  This module never imports oracle/.
+"""
+from __future__ import annotations
+
+import ctypes
+from dataclasses import dataclass
+from pathlib import Path
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+PKG = Path(__file__).resolve().parent
+LIB_PATH = PKG / "libpsync.so"
+
+PSYNC_OK, PSYNC_EINVAL, PSYNC_ETOOFEW, PSYNC_EUNSUPPORTED, PSYNC_ECUDA = 0, -1, -2, -3, -4
+PSYNC_F32, PSYNC_BF16 = 0, 1
+PSYNC_SGD, PSYNC_MOMENTUM, PSYNC_RMSPROP_MOM = 0, 1, 2
+PSYNC_EMA_POST, PSYNC_EMA_PRE, PSYNC_EMA_OFF = 0, 1, 2
+PSYNC_MAX_WORKERS = 1024
+
+EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_aggregate_update", "psync_ema",
+           "psync_step_host_workspace_bytes", "psync_step_host", "psync_launch_geometry", "psync_probe_read",
+           "psync_probe_copy")
+
+
+class PsyncError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {status_string(status)} ({status})")
+
+
+class psync_step(ctypes.Structure):
+    """Mirror of `struct psync_step` in include/psync.h (field order and types must match)."""
+    _fields_ = [
+        ("P", ctypes.c_int64), ("M", ctypes.c_int32), ("h_shard_off", ctypes.c_void_p),
+        ("N", ctypes.c_int32), ("W", ctypes.c_int32), ("d_grads", ctypes.c_void_p),
+        ("grad_dtype", ctypes.c_int32), ("d_kept", ctypes.c_void_p), ("d_status", ctypes.c_void_p),
+        ("d_theta", ctypes.c_void_p), ("d_ema", ctypes.c_void_p), ("d_state0", ctypes.c_void_p),
+        ("d_state1", ctypes.c_void_p), ("opt", ctypes.c_int32), ("ema_mode", ctypes.c_int32),
+        ("gamma_t", ctypes.c_float), ("alpha", ctypes.c_float), ("mu", ctypes.c_float), ("rho", ctypes.c_float),
+        ("eps", ctypes.c_float), ("grid_ctas", ctypes.c_int32), ("variant", ctypes.c_int32),
+    ]
+
+
+_lib: Optional[ctypes.CDLL] = None
+
+
+def lib() -> ctypes.CDLL:
+    """Loads libpsync.so; raises if it has not been built (run __graft_entry__.build())."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise FileNotFoundError(f"{LIB_PATH} is missing: build it with `python -m paper_1702_05800_b200.build` "
+                                    "(there is no CPU fallback)")
+        L = ctypes.CDLL(str(LIB_PATH))
+        vp, i32, i64, f32 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_float
+        L.psync_version.restype = ctypes.c_int
+        L.psync_status_string.argtypes = [ctypes.c_int]
+        L.psync_status_string.restype = ctypes.c_char_p
+        L.psync_select_first_n.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, vp]
+        L.psync_select_first_n.restype = ctypes.c_int
+        L.psync_aggregate_update.argtypes = [ctypes.POINTER(psync_step), vp]
+        L.psync_aggregate_update.restype = ctypes.c_int
+        L.psync_ema.argtypes = [vp, vp, i64, f32, vp]
+        L.psync_ema.restype = ctypes.c_int
+        L.psync_step_host_workspace_bytes.argtypes = [i32, i32, i32, i64]
+        L.psync_step_host_workspace_bytes.restype = ctypes.c_size_t
+        L.psync_step_host.argtypes = [ctypes.POINTER(psync_step), vp, vp, i32, vp, vp, vp, vp, vp, ctypes.c_size_t,
+                                      i64, vp]
+        L.psync_step_host.restype = ctypes.c_int
+        L.psync_launch_geometry.argtypes = [ctypes.POINTER(psync_step), vp, vp, vp, vp]
+        L.psync_launch_geometry.restype = ctypes.c_int
+        L.psync_probe_read.argtypes = [vp, i64, vp, vp]
+        L.psync_probe_read.restype = ctypes.c_int
+        L.psync_probe_copy.argtypes = [vp, vp, i64, vp]
+        L.psync_probe_copy.restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def status_string(status: int) -> str:
+    return lib().psync_status_string(status).decode()
+
+
+def psync_version() -> int:
+    return lib().psync_version()
+
+
+def _dptr(t: Optional[torch.Tensor], dtype=None, name="tensor") -> Optional[int]:
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"{name}: expected {dtype}, got {t.dtype}")
+    return t.data_ptr()
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def psync_select_first_n(d_arrival: torch.Tensor, N: int, b: int, d_kept: torch.Tensor, d_status: torch.Tensor,
+                         d_t_nth: Optional[torch.Tensor] = None, d_step_tag: Optional[torch.Tensor] = None,
+                         t: int = 0, stream=None, check: bool = True) -> int:
+    """Enqueues the selection kernel (include/psync.h: psync_select_first_n)."""
+    if d_arrival.numel() < N + b or d_kept.numel() < max(N, 0):
+        raise ValueError("d_arrival needs N+b elements and d_kept N elements")
+    if d_step_tag is not None and d_step_tag.numel() < N + b:
+        raise ValueError("d_step_tag needs N+b elements")
+    st = lib().psync_select_first_n(_dptr(d_arrival, torch.float32, "d_arrival"),
+                                    _dptr(d_step_tag, torch.int32, "d_step_tag"), t, N, b,
+                                    _dptr(d_kept, torch.int32, "d_kept"), _dptr(d_t_nth, torch.float32, "d_t_nth"),
+                                    _dptr(d_status, torch.int32, "d_status"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_select_first_n")
+    return st
+
+
+@dataclass
+class GradTable:
+    """Device array of W device pointers (worker k -> its gradient buffer) + the tensors kept alive."""
+    d_ptrs: torch.Tensor
+    buffers: Sequence[torch.Tensor]
+    grad_dtype: int
+
+    @property
+    def W(self) -> int:
+        return len(self.buffers)
+
+
+def make_grad_table(buffers: Sequence[torch.Tensor]) -> GradTable:
+    dt = buffers[0].dtype
+    if dt not in (torch.float32, torch.bfloat16):
+        raise TypeError("gradient buffers must be float32 or bfloat16")
+    for g in buffers:
+        if g.dtype != dt or not g.is_cuda or not g.is_contiguous():
+            raise ValueError("gradient buffers must be contiguous CUDA tensors of one dtype")
+    ptrs = torch.tensor([g.data_ptr() for g in buffers], dtype=torch.int64).to(buffers[0].device)
+    return GradTable(ptrs, list(buffers), PSYNC_F32 if dt == torch.float32 else PSYNC_BF16)
+
+
+def make_step(shard_off, N: int, W: int, grad_dtype: int, theta: torch.Tensor, ema: Optional[torch.Tensor] = None,
+              state0: Optional[torch.Tensor] = None, state1: Optional[torch.Tensor] = None, opt: int = PSYNC_SGD,
+              ema_mode: int = PSYNC_EMA_POST, gamma_t: float = 0.0, alpha: float = 0.0, mu: float = 0.0,
+              rho: float = 0.0, eps: float = 0.0, d_grads: Optional[torch.Tensor] = None,
+              d_kept: Optional[torch.Tensor] = None, d_status: Optional[torch.Tensor] = None, grid_ctas: int = 0,
+              variant: int = 0):
+    """Fills a psync_step.  Returns (struct, keepalive) -- hold on to both until the call returns."""
+    off = np.ascontiguousarray(shard_off, dtype=np.int64)
+    s = psync_step()
+    s.P = theta.numel()
+    s.M = off.size - 1
+    s.h_shard_off = off.ctypes.data
+    s.N, s.W = N, W
+    s.d_grads = _dptr(d_grads, torch.int64, "d_grads")
+    s.grad_dtype = grad_dtype
+    s.d_kept = _dptr(d_kept, torch.int32, "d_kept")
+    s.d_status = _dptr(d_status, torch.int32, "d_status")
+    s.d_theta = _dptr(theta, torch.float32, "theta")
+    s.d_ema = _dptr(ema, torch.float32, "ema")
+    s.d_state0 = _dptr(state0, torch.float32, "state0")
+    s.d_state1 = _dptr(state1, torch.float32, "state1")
+    for nm, a in (("ema", ema), ("state0", state0), ("state1", state1)):
+        if a is not None and a.numel() != theta.numel():
+            raise ValueError(f"{nm} must have P elements")
+    s.opt, s.ema_mode = opt, ema_mode
+    s.gamma_t, s.alpha, s.mu, s.rho, s.eps = gamma_t, alpha, mu, rho, eps
+    s.grid_ctas, s.variant = grid_ctas, variant
+    return s, (off, d_grads, d_kept, d_status, theta, ema, state0, state1)
+
+
+def psync_aggregate_update(step: psync_step, stream=None, check: bool = True) -> int:
+    """Enqueues the fused aggregate+update+EMA kernel (Alg. 4 l.8-9, L160-162)."""
+    st = lib().psync_aggregate_update(ctypes.byref(step), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_aggregate_update")
+    return st
+
+
+def psync_ema(d_ema: torch.Tensor, d_theta: torch.Tensor, alpha: float, stream=None, check: bool = True) -> int:
+    """ema <- alpha ema + (1-alpha) theta."""
+    if d_ema.numel() != d_theta.numel():
+        raise ValueError("ema and theta must have the same number of elements")
+    st = lib().psync_ema(_dptr(d_ema, torch.float32, "d_ema"), _dptr(d_theta, torch.float32, "d_theta"),
+                         d_ema.numel(), alpha, _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_ema")
+    return st
+
+
+def psync_launch_geometry(step: psync_step) -> dict:
+    g = [ctypes.c_int32() for _ in range(4)]
+    st = lib().psync_launch_geometry(ctypes.byref(step), *[ctypes.addressof(x) for x in g])
+    if st != PSYNC_OK:
+        raise PsyncError(st, "psync_launch_geometry")
+    return dict(grid=g[0].value, block=g[1].value, tile_elems=g[2].value, smem_bytes=g[3].value)
+
+
+def psync_step_host_workspace_bytes(N: int, W: int, grad_dtype: int, chunk_elems: int = 0) -> int:
+    return lib().psync_step_host_workspace_bytes(N, W, grad_dtype, chunk_elems)
+
+
+def psync_step_host(step: psync_step, h_arrival: np.ndarray, h_grads: Sequence[torch.Tensor],
+                    d_work: torch.Tensor, h_theta_out: Optional[torch.Tensor] = None,
+                    h_kept: Optional[np.ndarray] = None, h_step_tag: Optional[np.ndarray] = None, t: int = 0,
+                    chunk_elems: int = 0, stream=None, check: bool = True):
+    """The step with HOST gradient buffers (include/psync.h: psync_step_host).  h_grads are CPU tensors
+    (pinned for full PCIe rate); theta/ema/state stay on the device.  Returns (status, t_nth)."""
+    W = step.W
+    if len(h_grads) != W or h_arrival.size != W or h_arrival.dtype != np.float32:
+        raise ValueError("need W host gradient buffers and W fp32 arrival times")
+    for g in h_grads:
+        if g.is_cuda or not g.is_contiguous() or g.numel() != step.P:
+            raise ValueError("h_grads must be contiguous CPU tensors of P elements")
+    ptrs = (ctypes.c_void_p * W)(*[g.data_ptr() for g in h_grads])
+    t_nth = ctypes.c_float(float("nan"))
+    if h_theta_out is not None and (h_theta_out.is_cuda or h_theta_out.dtype != torch.float32
+                                    or h_theta_out.numel() != step.P):
+        raise ValueError("h_theta_out must be a CPU float32 tensor of P elements")
+    if h_kept is not None and (h_kept.dtype != np.int32 or h_kept.size != step.N):
+        raise ValueError("h_kept must be int32[N]")
+    if h_step_tag is not None and (h_step_tag.dtype != np.int32 or h_step_tag.size != W):
+        raise ValueError("h_step_tag must be int32[W]")
+    st = lib().psync_step_host(ctypes.byref(step), h_arrival.ctypes.data,
+                               None if h_step_tag is None else h_step_tag.ctypes.data, t,
+                               ctypes.cast(ptrs, ctypes.c_void_p),
+                               None if h_theta_out is None else h_theta_out.data_ptr(),
+                               None if h_kept is None else h_kept.ctypes.data, ctypes.addressof(t_nth),
+                               _dptr(d_work, None, "d_work"), d_work.numel() * d_work.element_size(), chunk_elems,
+                               _stream(stream))
+    if check and st not in (PSYNC_OK, PSYNC_ETOOFEW):
+        raise PsyncError(st, "psync_step_host")
+    return st, t_nth.value
+
+
+def psync_probe_read(d_src: torch.Tensor, d_sink: torch.Tensor, stream=None) -> int:
+    n = d_src.numel() * d_src.element_size() // 16
+    st = lib().psync_probe_read(_dptr(d_src), n, _dptr(d_sink, torch.float32), _stream(stream))
+    if st != PSYNC_OK:
+        raise PsyncError(st, "psync_probe_read")
+    return n * 16
+
+
+def psync_probe_copy(d_dst: torch.Tensor, d_src: torch.Tensor, stream=None) -> int:
+    n = d_src.numel() * d_src.element_size() // 16
+    st = lib().psync_probe_copy(_dptr(d_dst), _dptr(d_src), n, _stream(stream))
+    if st != PSYNC_OK:
+        raise PsyncError(st, "psync_probe_copy")
+    return n * 32

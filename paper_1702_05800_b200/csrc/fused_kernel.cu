@@ -1,0 +1,382 @@
+// K2: fused aggregate + update + EMA -- Alg. 4 l.8-9 in ONE pass over HBM.
+// K3: standalone EMA.
+//
+//   S[i]   = sum over the kept workers k, ascending k, of G_k[i]          (fp32, fixed order)
+//   G[i]   = S[i] * (1/N)
+//   theta, state <- optimizer(theta, state, G)      (SGD | momentum | RMSProp with momentum)
+//   ema    <- alpha ema + (1 - alpha) theta*        (theta* = new theta, or old theta for PRE)
+//
+// The path is a pure stream: N*sizeof(grad) + 8*(2 + n_state) bytes per parameter, ~0.25 flop/B,
+// so the HBM roofline bounds it and no tensor core is involved (there is no contraction).
+// B200 design:
+//   * only the N kept buffers are dereferenced, through a device pointer table indexed by the
+//     selection kernel's kept[] -- no host sync between K1 and K2, dropped buffers never touched;
+//   * 128-bit read-only streaming loads (ld.global.nc, L1 no-allocate), U independent loads in
+//     flight per thread per batch, accumulated strictly in worker order afterwards, so the result
+//     does not depend on the launch geometry;
+//   * persistent grid: SMs x resident CTAs, static tile striding (all tiles cost the same);
+//   * theta / state / ema are loaded after the gradient stream (its registers are dead by then),
+//     updated in registers and stored once.
+// The flat element space is processed without regard to shard cuts: the step is elementwise and
+// all arrays share one layout, so server j's slice gets exactly Alg. 4's result (DESIGN.md s.4).
+
+#include "psync_kernels.cuh"
+
+namespace psync {
+namespace {
+
+constexpr int OPT_SGD = 0, OPT_MOMENTUM = 1, OPT_RMSPROP_MOM = 2;
+constexpr int EMA_POST = 0, EMA_PRE = 1, EMA_OFF = 2;
+
+// ---- memory access helpers -------------------------------------------------------------------
+__device__ __forceinline__ uint4 ldg_stream16(const void* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ float ldg_stream_f32(const float* p) {
+  float r;
+  asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(r) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ uint16_t ldg_stream_u16(const uint16_t* p) {
+  uint16_t r;
+  asm volatile("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(r) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ float4 ld_state16(const float* p) {
+  float4 r;
+  asm volatile("ld.global.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];"
+               : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w)
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_state16(float* p, const float4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z),
+               "f"(v.w)
+               : "memory");
+}
+
+// ---- the per-element update, Alg. 4 l.8-9 ----------------------------------------------------
+template <int OPT, int EMA>
+__device__ __forceinline__ void update_element(float S, float& th, float& em, float& s0, float& s1,
+                                               const FusedParams& p) {
+  const float G = S * p.inv_N;  // mean of the kept gradients (L160)
+  const float th_old = th;
+  if (OPT == OPT_SGD) {
+    th = th - p.gamma * G;  // L40, L160
+  } else if (OPT == OPT_MOMENTUM) {
+    s0 = p.mu * s0 + G;  // v <- mu v + G          (reading R6)
+    th = th - p.gamma * s0;
+  } else {
+    s0 = p.rho * s0 + p.one_minus_rho * (G * G);            // ms  (reading R5)
+    s1 = p.mu * s1 + (p.gamma * G) / sqrtf(s0 + p.eps);     // mom
+    th = th - s1;
+  }
+  if (EMA != EMA_OFF) {
+    const float operand = (EMA == EMA_POST) ? th : th_old;  // reading R3
+    em = p.alpha * em + p.one_minus_alpha * operand;        // L40, L162
+  }
+}
+
+template <bool BF16>
+__device__ __forceinline__ void accumulate_unit(float* acc, const uint4& r) {
+  if (BF16) {  // 8 bf16 = 4 words; element 2i in the low half, 2i+1 in the high half; widening is exact
+    acc[0] += __uint_as_float(r.x << 16);
+    acc[1] += __uint_as_float(r.x & 0xFFFF0000u);
+    acc[2] += __uint_as_float(r.y << 16);
+    acc[3] += __uint_as_float(r.y & 0xFFFF0000u);
+    acc[4] += __uint_as_float(r.z << 16);
+    acc[5] += __uint_as_float(r.z & 0xFFFF0000u);
+    acc[6] += __uint_as_float(r.w << 16);
+    acc[7] += __uint_as_float(r.w & 0xFFFF0000u);
+  } else {
+    acc[0] += __uint_as_float(r.x);
+    acc[1] += __uint_as_float(r.y);
+    acc[2] += __uint_as_float(r.z);
+    acc[3] += __uint_as_float(r.w);
+  }
+}
+
+// ---- scalar path: any alignment, any range; also the < 8-element tail of the vector path ------
+template <bool BF16, int OPT, int EMA>
+__device__ void scalar_range(const FusedParams& p, const char* const* s_ptr, int64_t i0, int64_t i1, int64_t gtid,
+                             int64_t gthreads) {
+  for (int64_t i = i0 + gtid; i < i1; i += gthreads) {
+    float S = 0.f;
+#pragma unroll 4
+    for (int n = 0; n < p.N; ++n) {
+      float g;
+      if (BF16)
+        g = __uint_as_float(static_cast<uint32_t>(ldg_stream_u16(reinterpret_cast<const uint16_t*>(s_ptr[n]) + i))
+                            << 16);
+      else
+        g = ldg_stream_f32(reinterpret_cast<const float*>(s_ptr[n]) + i);
+      S += g;
+    }
+    float th = p.theta[i];
+    float em = (EMA != EMA_OFF) ? p.ema[i] : 0.f;
+    float s0 = (OPT != OPT_SGD) ? p.s0[i] : 0.f;
+    float s1 = (OPT == OPT_RMSPROP_MOM) ? p.s1[i] : 0.f;
+    update_element<OPT, EMA>(S, th, em, s0, s1, p);
+    p.theta[i] = th;
+    if (EMA != EMA_OFF) p.ema[i] = em;
+    if (OPT != OPT_SGD) p.s0[i] = s0;
+    if (OPT == OPT_RMSPROP_MOM) p.s1[i] = s1;
+  }
+}
+
+// ---- the fused kernel ------------------------------------------------------------------------
+// A "unit" is 16 bytes of one gradient buffer: E = 4 (fp32) or 8 (bf16) consecutive parameters.
+// A tile is THREADS x UPT units; slot j of thread tid is unit tile*THREADS*UPT + j*THREADS + tid, so
+// each warp-level load covers 512 contiguous bytes of one worker's buffer.
+template <int THREADS, int UPT, int U, int MINB, bool BF16, int OPT, int EMA>
+__global__ void __launch_bounds__(THREADS, MINB) fused_aggregate_update_ema(const FusedParams p) {
+  constexpr int E = BF16 ? 8 : 4;
+  constexpr int Q = E / 4;  // float4 groups of theta per unit
+  __shared__ const char* s_ptr[kMaxWorkers];
+
+  if (p.status != nullptr && *p.status != 0) return;  // selection failed: leave everything untouched
+
+  unsigned misalign = 0;
+  for (int n = threadIdx.x; n < p.N; n += THREADS) {
+    const char* g = static_cast<const char*>(p.grads[p.kept[n]]);
+    s_ptr[n] = g;
+    misalign |= static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 15u;
+  }
+  const bool vec_ok = (__syncthreads_or(static_cast<int>(misalign)) == 0) && (p.base_aligned != 0);
+
+  const int64_t gtid = static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x;
+  const int64_t gthreads = static_cast<int64_t>(gridDim.x) * THREADS;
+  if (!vec_ok) {
+    scalar_range<BF16, OPT, EMA>(p, s_ptr, 0, p.P, gtid, gthreads);
+    return;
+  }
+
+  const int64_t n_units = p.P / E;
+  constexpr int64_t TILE_UNITS = static_cast<int64_t>(THREADS) * UPT;
+  const int64_t n_tiles = (n_units + TILE_UNITS - 1) / TILE_UNITS;
+  const int N = p.N;
+
+  for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    int64_t unit[UPT];
+    bool live[UPT];
+#pragma unroll
+    for (int j = 0; j < UPT; ++j) {
+      const int64_t u = tile * TILE_UNITS + static_cast<int64_t>(j) * THREADS + threadIdx.x;
+      live[j] = u < n_units;
+      unit[j] = live[j] ? u : (n_units - 1);  // dead slots re-read a valid unit and store nothing
+    }
+
+    float acc[UPT][E];
+#pragma unroll
+    for (int j = 0; j < UPT; ++j)
+#pragma unroll
+      for (int e = 0; e < E; ++e) acc[j][e] = 0.f;
+
+    int n = 0;
+    for (; n + U <= N; n += U) {  // full batches: U x UPT independent 16-byte loads in flight
+      uint4 r[U][UPT];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const char* g = s_ptr[n + u];
+#pragma unroll
+        for (int j = 0; j < UPT; ++j) r[u][j] = ldg_stream16(g + unit[j] * 16);
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u)  // strictly ascending worker order per element
+#pragma unroll
+        for (int j = 0; j < UPT; ++j) accumulate_unit<BF16>(acc[j], r[u][j]);
+    }
+    if (n < N) {  // last, partial batch: same shape, predicated
+      uint4 r[U][UPT];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const bool on = (n + u) < N;
+        const char* g = s_ptr[on ? (n + u) : (N - 1)];
+#pragma unroll
+        for (int j = 0; j < UPT; ++j) r[u][j] = on ? ldg_stream16(g + unit[j] * 16) : make_uint4(0u, 0u, 0u, 0u);
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u)
+        if ((n + u) < N) {
+#pragma unroll
+          for (int j = 0; j < UPT; ++j) accumulate_unit<BF16>(acc[j], r[u][j]);
+        }
+    }
+
+    // theta / state / ema: loaded once the gradient registers are dead; other resident warps hide the latency
+    float4 th[UPT][Q], em[UPT][Q], a0[UPT][Q], a1[UPT][Q];
+#pragma unroll
+    for (int j = 0; j < UPT; ++j) {
+#pragma unroll
+      for (int q = 0; q < Q; ++q) {
+        const int64_t e = unit[j] * E + 4 * q;
+        th[j][q] = ld_state16(p.theta + e);
+        if (EMA != EMA_OFF) em[j][q] = ld_state16(p.ema + e);
+        if (OPT != OPT_SGD) a0[j][q] = ld_state16(p.s0 + e);
+        if (OPT == OPT_RMSPROP_MOM) a1[j][q] = ld_state16(p.s1 + e);
+      }
+    }
+
+#pragma unroll
+    for (int j = 0; j < UPT; ++j) {
+#pragma unroll
+      for (int q = 0; q < Q; ++q) {
+        float* t4 = reinterpret_cast<float*>(&th[j][q]);
+        float* e4 = reinterpret_cast<float*>(&em[j][q]);
+        float* x4 = reinterpret_cast<float*>(&a0[j][q]);
+        float* y4 = reinterpret_cast<float*>(&a1[j][q]);
+#pragma unroll
+        for (int l = 0; l < 4; ++l) update_element<OPT, EMA>(acc[j][4 * q + l], t4[l], e4[l], x4[l], y4[l], p);
+        if (live[j]) {
+          const int64_t e = unit[j] * E + 4 * q;
+          st_state16(p.theta + e, th[j][q]);
+          if (EMA != EMA_OFF) st_state16(p.ema + e, em[j][q]);
+          if (OPT != OPT_SGD) st_state16(p.s0 + e, a0[j][q]);
+          if (OPT == OPT_RMSPROP_MOM) st_state16(p.s1 + e, a1[j][q]);
+        }
+      }
+    }
+  }
+
+  // fewer than E trailing parameters
+  const int64_t tail0 = n_units * E;
+  if (tail0 < p.P && blockIdx.x == 0) scalar_range<BF16, OPT, EMA>(p, s_ptr, tail0, p.P, threadIdx.x, THREADS);
+}
+
+// ---- K3 ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) ema_kernel(float* __restrict__ ema, const float* __restrict__ theta, int64_t P,
+                                                  float alpha, float one_minus_alpha, int aligned) {
+  const int64_t gtid = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  const int64_t gthreads = static_cast<int64_t>(gridDim.x) * blockDim.x;
+  const int64_t n4 = aligned ? P / 4 : 0;
+  for (int64_t v = gtid; v < n4; v += gthreads) {
+    float4 e = ld_state16(ema + 4 * v);
+    const float4 t = ld_state16(theta + 4 * v);
+    e.x = alpha * e.x + one_minus_alpha * t.x;
+    e.y = alpha * e.y + one_minus_alpha * t.y;
+    e.z = alpha * e.z + one_minus_alpha * t.z;
+    e.w = alpha * e.w + one_minus_alpha * t.w;
+    st_state16(ema + 4 * v, e);
+  }
+  for (int64_t i = n4 * 4 + gtid; i < P; i += gthreads) ema[i] = alpha * ema[i] + one_minus_alpha * theta[i];
+}
+
+// ---- variants and dispatch ---------------------------------------------------------------------
+struct Variant {
+  int threads, upt, unroll, minb;
+};
+// variant ids are 1-based in the ABI (0 = default for the dtype)
+constexpr Variant kVariants[] = {
+    {256, 1, 8, 4},   // 1
+    {256, 2, 8, 2},   // 2
+    {256, 1, 16, 3},  // 3
+    {512, 1, 8, 2},   // 4
+    {256, 2, 4, 3},   // 5
+    {128, 1, 8, 8},   // 6
+};
+constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
+
+using KernelFn = void (*)(const FusedParams);
+
+template <int V, bool BF16, int OPT, int EMA>
+constexpr KernelFn kernel_for() {
+  return fused_aggregate_update_ema<kVariants[V].threads, kVariants[V].upt, kVariants[V].unroll, kVariants[V].minb,
+                                    BF16, OPT, EMA>;
+}
+
+template <int V, bool BF16, int OPT>
+KernelFn pick_ema(int ema) {
+  switch (ema) {
+    case EMA_POST: return kernel_for<V, BF16, OPT, EMA_POST>();
+    case EMA_PRE: return kernel_for<V, BF16, OPT, EMA_PRE>();
+    default: return kernel_for<V, BF16, OPT, EMA_OFF>();
+  }
+}
+template <int V, bool BF16>
+KernelFn pick_opt(int opt, int ema) {
+  switch (opt) {
+    case OPT_SGD: return pick_ema<V, BF16, OPT_SGD>(ema);
+    case OPT_MOMENTUM: return pick_ema<V, BF16, OPT_MOMENTUM>(ema);
+    default: return pick_ema<V, BF16, OPT_RMSPROP_MOM>(ema);
+  }
+}
+template <int V>
+KernelFn pick_dtype(int dtype, int opt, int ema) {
+  return dtype == 1 ? pick_opt<V, true>(opt, ema) : pick_opt<V, false>(opt, ema);
+}
+KernelFn pick_kernel(int v, int dtype, int opt, int ema) {
+  switch (v) {
+    case 0: return pick_dtype<0>(dtype, opt, ema);
+    case 1: return pick_dtype<1>(dtype, opt, ema);
+    case 2: return pick_dtype<2>(dtype, opt, ema);
+    case 3: return pick_dtype<3>(dtype, opt, ema);
+    case 4: return pick_dtype<4>(dtype, opt, ema);
+    default: return pick_dtype<5>(dtype, opt, ema);
+  }
+}
+
+int resolve_variant(int dtype, int variant) {
+  if (variant >= 1 && variant <= kNumVariants) return variant - 1;
+  return dtype == 1 ? 0 : 0;  // default: variant 1 (tuned on B200, see DESIGN.md s.6)
+}
+
+}  // namespace
+
+int fused_num_variants() { return kNumVariants; }
+
+int sm_count() {
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      sms <= 0) {
+    cudaGetLastError();
+    return 148;
+  }
+  return sms;
+}
+
+cudaError_t fused_geometry(int dtype, int opt, int ema, int variant, int grid_ctas, int64_t P, FusedGeometry* out) {
+  const int v = resolve_variant(dtype, variant);
+  const Variant& vr = kVariants[v];
+  const int E = dtype == 1 ? 8 : 4;
+  out->block = vr.threads;
+  out->tile_elems = vr.threads * vr.upt * E;
+  out->smem_bytes = static_cast<int>(sizeof(const char*)) * kMaxWorkers;
+  int per_sm = 0;
+  cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pick_kernel(v, dtype, opt, ema), vr.threads, 0);
+  if (err != cudaSuccess || per_sm <= 0) {
+    cudaGetLastError();
+    per_sm = vr.minb;  // no device to ask: the launch bound is the design occupancy
+  }
+  int64_t grid = grid_ctas > 0 ? grid_ctas : static_cast<int64_t>(sm_count()) * per_sm;
+  const int64_t n_tiles = (P / E + static_cast<int64_t>(vr.threads) * vr.upt - 1) / (static_cast<int64_t>(vr.threads) * vr.upt);
+  if (grid_ctas <= 0 && n_tiles < grid) grid = n_tiles;
+  if (grid < 1) grid = 1;
+  out->grid = static_cast<int>(grid);
+  return cudaSuccess;
+}
+
+cudaError_t launch_fused(const FusedParams& p, int dtype, int opt, int ema, int variant, int grid_ctas,
+                         cudaStream_t stream) {
+  FusedGeometry g;
+  cudaError_t err = fused_geometry(dtype, opt, ema, variant, grid_ctas, p.P, &g);
+  if (err != cudaSuccess) return err;
+  const int v = resolve_variant(dtype, variant);
+  pick_kernel(v, dtype, opt, ema)<<<g.grid, g.block, 0, stream>>>(p);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_ema(float* d_ema, const float* d_theta, int64_t P, float alpha, cudaStream_t stream) {
+  const int aligned = ((reinterpret_cast<uintptr_t>(d_ema) | reinterpret_cast<uintptr_t>(d_theta)) & 15u) == 0;
+  int64_t blocks = (P / 4 + 255) / 256;
+  const int64_t cap = static_cast<int64_t>(sm_count()) * 8;
+  if (blocks > cap) blocks = cap;
+  if (blocks < 1) blocks = 1;
+  ema_kernel<<<static_cast<int>(blocks), 256, 0, stream>>>(d_ema, d_theta, P, alpha, 1.0f - alpha, aligned);
+  return cudaGetLastError();
+}
+
+}  // namespace psync

@@ -1,0 +1,285 @@
+// The C ABI of include/psync.h: argument checks, dispatch to the sm_100a kernels, and the
+// host-buffer step (chunked, double-buffered H2D of the kept workers only).  No torch types, no
+// CPU arithmetic path: every step of Alg. 4 runs in the kernels of this directory.
+
+#include <cstring>
+#include <vector>
+
+#include "../../include/psync.h"
+#include "psync_kernels.cuh"
+
+namespace {
+
+using psync::FusedParams;
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+int check_step(const psync_step* s, bool need_device_tables) {
+  if (s == nullptr) return PSYNC_EINVAL;
+  if (s->P < 0 || s->M < 1 || s->h_shard_off == nullptr) return PSYNC_EINVAL;
+  if (s->h_shard_off[0] != 0 || s->h_shard_off[s->M] != s->P) return PSYNC_EINVAL;
+  for (int32_t j = 0; j < s->M; ++j)
+    if (s->h_shard_off[j + 1] < s->h_shard_off[j]) return PSYNC_EINVAL;
+  if (s->N < 1 || s->W < s->N || s->W > PSYNC_MAX_WORKERS) return PSYNC_EINVAL;
+  if (s->grad_dtype != PSYNC_F32 && s->grad_dtype != PSYNC_BF16) return PSYNC_EINVAL;
+  if (s->opt < PSYNC_SGD || s->opt > PSYNC_RMSPROP_MOM) return PSYNC_EINVAL;
+  if (s->ema_mode < PSYNC_EMA_POST || s->ema_mode > PSYNC_EMA_OFF) return PSYNC_EINVAL;
+  if (s->P > 0) {  // an empty parameter vector needs no buffers
+    if (s->d_theta == nullptr) return PSYNC_EINVAL;
+    if (s->ema_mode != PSYNC_EMA_OFF && s->d_ema == nullptr) return PSYNC_EINVAL;
+    if (s->opt != PSYNC_SGD && s->d_state0 == nullptr) return PSYNC_EINVAL;
+    if (s->opt == PSYNC_RMSPROP_MOM && s->d_state1 == nullptr) return PSYNC_EINVAL;
+  }
+  if (need_device_tables && (s->d_grads == nullptr || s->d_kept == nullptr)) return PSYNC_EINVAL;
+  if (s->grid_ctas < 0 || s->variant < 0 || s->variant > psync::fused_num_variants()) return PSYNC_EINVAL;
+  return PSYNC_OK;
+}
+
+// Coefficients formed in fp32 (reading R8); element range [first, first + count).
+FusedParams make_params(const psync_step* s, int64_t first, int64_t count, const void* const* d_grads,
+                        const int32_t* d_kept, const int32_t* d_status) {
+  FusedParams p;
+  p.P = count;
+  p.N = s->N;
+  p.grads = d_grads;
+  p.kept = d_kept;
+  p.status = d_status;
+  p.theta = s->d_theta + first;
+  p.ema = (s->ema_mode != PSYNC_EMA_OFF) ? s->d_ema + first : nullptr;
+  p.s0 = (s->opt != PSYNC_SGD) ? s->d_state0 + first : nullptr;
+  p.s1 = (s->opt == PSYNC_RMSPROP_MOM) ? s->d_state1 + first : nullptr;
+  p.gamma = s->gamma_t;
+  p.alpha = s->alpha;
+  p.one_minus_alpha = 1.0f - s->alpha;
+  p.mu = s->mu;
+  p.rho = s->rho;
+  p.one_minus_rho = 1.0f - s->rho;
+  p.eps = s->eps;
+  p.inv_N = 1.0f / static_cast<float>(s->N);
+  p.base_aligned = aligned16(p.theta) && (p.ema == nullptr || aligned16(p.ema)) && (p.s0 == nullptr || aligned16(p.s0)) &&
+                   (p.s1 == nullptr || aligned16(p.s1));
+  return p;
+}
+
+constexpr int64_t kDefaultChunkElems = int64_t{1} << 20;
+
+int64_t round_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+
+struct HostLayout {
+  int64_t chunk, stride_bytes;
+  size_t off_stage[2], off_ptrs[2], off_ident, off_arrival, off_tags, off_kept, off_tnth, off_status, total;
+};
+
+bool host_layout(int32_t N, int32_t W, int32_t dtype, int64_t chunk_elems, HostLayout* L) {
+  if (N < 1 || W < N || W > PSYNC_MAX_WORKERS) return false;
+  if (dtype != PSYNC_F32 && dtype != PSYNC_BF16) return false;
+  if (chunk_elems == 0) chunk_elems = kDefaultChunkElems;
+  if (chunk_elems < 64 || chunk_elems % 64 != 0) return false;
+  const int64_t esz = dtype == PSYNC_BF16 ? 2 : 4;
+  L->chunk = chunk_elems;
+  L->stride_bytes = round_up(chunk_elems * esz, 256);
+  size_t off = 0;
+  for (int i = 0; i < 2; ++i) {
+    L->off_stage[i] = off;
+    off += static_cast<size_t>(L->stride_bytes) * N;
+  }
+  for (int i = 0; i < 2; ++i) {
+    L->off_ptrs[i] = off;
+    off += static_cast<size_t>(round_up(int64_t{8} * N, 256));
+  }
+  L->off_ident = off;
+  off += static_cast<size_t>(round_up(int64_t{4} * N, 256));
+  L->off_arrival = off;
+  off += static_cast<size_t>(round_up(int64_t{4} * W, 256));
+  L->off_tags = off;
+  off += static_cast<size_t>(round_up(int64_t{4} * W, 256));
+  L->off_kept = off;
+  off += static_cast<size_t>(round_up(int64_t{4} * N, 256));
+  L->off_tnth = off;
+  off += 256;
+  L->off_status = off;
+  off += 256;
+  L->total = off;
+  return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+PSYNC_API int psync_version(void) { return PSYNC_VERSION; }
+
+PSYNC_API const char* psync_status_string(int status) {
+  switch (status) {
+    case PSYNC_OK: return "PSYNC_OK";
+    case PSYNC_EINVAL: return "PSYNC_EINVAL: invalid argument";
+    case PSYNC_ETOOFEW: return "PSYNC_ETOOFEW: fewer than N eligible workers";
+    case PSYNC_EUNSUPPORTED: return "PSYNC_EUNSUPPORTED";
+    case PSYNC_ECUDA: return "PSYNC_ECUDA: CUDA runtime error";
+    default: return "PSYNC: unknown status";
+  }
+}
+
+PSYNC_API int psync_select_first_n(const float* d_arrival, const int32_t* d_step_tag, int32_t t, int32_t N, int32_t b,
+                         int32_t* d_kept, float* d_t_nth, int32_t* d_status, void* stream) {
+  if (d_arrival == nullptr || d_kept == nullptr || d_status == nullptr) return PSYNC_EINVAL;
+  if (N < 1 || b < 0 || static_cast<int64_t>(N) + b > PSYNC_MAX_WORKERS) return PSYNC_EINVAL;
+  const cudaError_t err = psync::launch_select_first_n(d_arrival, d_step_tag, t, N, N + b, d_kept, d_t_nth, d_status,
+                                                       static_cast<cudaStream_t>(stream));
+  return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
+}
+
+PSYNC_API int psync_aggregate_update(const psync_step* step, void* stream) {
+  const int st = check_step(step, true);
+  if (st != PSYNC_OK) return st;
+  if (step->P == 0) return PSYNC_OK;
+  const FusedParams p = make_params(step, 0, step->P, step->d_grads, step->d_kept, step->d_status);
+  const cudaError_t err = psync::launch_fused(p, step->grad_dtype, step->opt, step->ema_mode, step->variant,
+                                              step->grid_ctas, static_cast<cudaStream_t>(stream));
+  return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
+}
+
+PSYNC_API int psync_ema(float* d_ema, const float* d_theta, int64_t P, float alpha, void* stream) {
+  if (d_ema == nullptr || d_theta == nullptr || P < 0) return PSYNC_EINVAL;
+  if (P == 0) return PSYNC_OK;
+  const cudaError_t err = psync::launch_ema(d_ema, d_theta, P, alpha, static_cast<cudaStream_t>(stream));
+  return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
+}
+
+PSYNC_API int psync_launch_geometry(const psync_step* step, int32_t* grid, int32_t* block, int32_t* tile_elems,
+                          int32_t* smem_bytes) {
+  const int st = check_step(step, false);
+  if (st != PSYNC_OK) return st;
+  psync::FusedGeometry g;
+  if (psync::fused_geometry(step->grad_dtype, step->opt, step->ema_mode, step->variant, step->grid_ctas, step->P, &g) !=
+      cudaSuccess)
+    return PSYNC_ECUDA;
+  if (grid) *grid = g.grid;
+  if (block) *block = g.block;
+  if (tile_elems) *tile_elems = g.tile_elems;
+  if (smem_bytes) *smem_bytes = g.smem_bytes;
+  return PSYNC_OK;
+}
+
+PSYNC_API int psync_probe_read(const void* d_src, int64_t n_vec16, float* d_sink, void* stream) {
+  if (d_src == nullptr || d_sink == nullptr || n_vec16 < 0 || !aligned16(d_src)) return PSYNC_EINVAL;
+  return psync::launch_probe_read(d_src, n_vec16, d_sink, static_cast<cudaStream_t>(stream)) == cudaSuccess ? PSYNC_OK
+                                                                                                             : PSYNC_ECUDA;
+}
+
+PSYNC_API int psync_probe_copy(void* d_dst, const void* d_src, int64_t n_vec16, void* stream) {
+  if (d_src == nullptr || d_dst == nullptr || n_vec16 < 0 || !aligned16(d_src) || !aligned16(d_dst)) return PSYNC_EINVAL;
+  return psync::launch_probe_copy(d_dst, d_src, n_vec16, static_cast<cudaStream_t>(stream)) == cudaSuccess ? PSYNC_OK
+                                                                                                            : PSYNC_ECUDA;
+}
+
+PSYNC_API size_t psync_step_host_workspace_bytes(int32_t N, int32_t W, int32_t grad_dtype, int64_t chunk_elems) {
+  HostLayout L;
+  if (!host_layout(N, W, grad_dtype, chunk_elems, &L)) return 0;
+  return L.total;
+}
+
+PSYNC_API int psync_step_host(const psync_step* st, const float* h_arrival, const int32_t* h_step_tag, int32_t t,
+                    const void* const* h_grads, float* h_theta_out, int32_t* h_kept, float* h_t_nth, void* d_work,
+                    size_t work_bytes, int64_t chunk_elems, void* stream) {
+  const int chk = check_step(st, false);
+  if (chk != PSYNC_OK) return chk;
+  if (h_arrival == nullptr || h_grads == nullptr || d_work == nullptr) return PSYNC_EINVAL;
+  HostLayout L;
+  if (!host_layout(st->N, st->W, st->grad_dtype, chunk_elems, &L)) return PSYNC_EINVAL;
+  if (work_bytes < L.total || (reinterpret_cast<uintptr_t>(d_work) & 255u) != 0) return PSYNC_EINVAL;
+  for (int32_t k = 0; k < st->W; ++k)
+    if (h_grads[k] == nullptr) return PSYNC_EINVAL;
+
+  const int32_t N = st->N, W = st->W;
+  const int64_t esz = st->grad_dtype == PSYNC_BF16 ? 2 : 4;
+  char* work = static_cast<char*>(d_work);
+  float* d_arrival = reinterpret_cast<float*>(work + L.off_arrival);
+  int32_t* d_tags = reinterpret_cast<int32_t*>(work + L.off_tags);
+  int32_t* d_kept = reinterpret_cast<int32_t*>(work + L.off_kept);
+  float* d_tnth = reinterpret_cast<float*>(work + L.off_tnth);
+  int32_t* d_status = reinterpret_cast<int32_t*>(work + L.off_status);
+  int32_t* d_ident = reinterpret_cast<int32_t*>(work + L.off_ident);
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t copied[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr};
+  int result = PSYNC_OK;
+  std::vector<int32_t> kept(N);
+  int32_t status = PSYNC_ECUDA;
+  float t_nth = 0.f;
+
+#define PSYNC_CU(call)              \
+  do {                              \
+    if ((call) != cudaSuccess) {    \
+      result = PSYNC_ECUDA;         \
+      goto cleanup;                 \
+    }                               \
+  } while (0)
+
+  // 1. selection on the device (Alg. 4 l.3-6): the only thing the host learns is kept[] / status
+  PSYNC_CU(cudaMemcpyAsync(d_arrival, h_arrival, sizeof(float) * W, cudaMemcpyHostToDevice, s));
+  if (h_step_tag != nullptr)
+    PSYNC_CU(cudaMemcpyAsync(d_tags, h_step_tag, sizeof(int32_t) * W, cudaMemcpyHostToDevice, s));
+  PSYNC_CU(psync::launch_select_first_n(d_arrival, h_step_tag ? d_tags : nullptr, t, N, W, d_kept, d_tnth, d_status, s));
+  PSYNC_CU(cudaMemcpyAsync(&status, d_status, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+  PSYNC_CU(cudaStreamSynchronize(s));
+  if (status != PSYNC_OK) {
+    result = status;
+    goto cleanup;
+  }
+  PSYNC_CU(cudaMemcpyAsync(kept.data(), d_kept, sizeof(int32_t) * N, cudaMemcpyDeviceToHost, s));
+  PSYNC_CU(cudaMemcpyAsync(&t_nth, d_tnth, sizeof(float), cudaMemcpyDeviceToHost, s));
+  for (int i = 0; i < 2; ++i)
+    PSYNC_CU(psync::launch_fill_stage_table(reinterpret_cast<const void**>(work + L.off_ptrs[i]), d_ident,
+                                            work + L.off_stage[i], L.stride_bytes, N, s));
+  PSYNC_CU(cudaStreamSynchronize(s));
+  if (h_kept != nullptr) std::memcpy(h_kept, kept.data(), sizeof(int32_t) * N);
+  if (h_t_nth != nullptr) *h_t_nth = t_nth;
+
+  // 2./3. stream the kept buffers chunk by chunk; copy stream runs one chunk ahead of the kernel
+  PSYNC_CU(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+  for (int i = 0; i < 2; ++i) {
+    PSYNC_CU(cudaEventCreateWithFlags(&copied[i], cudaEventDisableTiming));
+    PSYNC_CU(cudaEventCreateWithFlags(&consumed[i], cudaEventDisableTiming));
+  }
+  {
+    int64_t c = 0;
+    for (int64_t first = 0; first < st->P; first += L.chunk, ++c) {
+      const int buf = static_cast<int>(c & 1);
+      const int64_t count = (st->P - first < L.chunk) ? (st->P - first) : L.chunk;
+      if (c >= 2) PSYNC_CU(cudaStreamWaitEvent(copy_stream, consumed[buf], 0));
+      for (int32_t n = 0; n < N; ++n) {
+        const char* src = static_cast<const char*>(h_grads[kept[n]]) + first * esz;
+        PSYNC_CU(cudaMemcpyAsync(work + L.off_stage[buf] + static_cast<int64_t>(n) * L.stride_bytes, src,
+                                 static_cast<size_t>(count * esz), cudaMemcpyHostToDevice, copy_stream));
+      }
+      PSYNC_CU(cudaEventRecord(copied[buf], copy_stream));
+      PSYNC_CU(cudaStreamWaitEvent(s, copied[buf], 0));
+      const FusedParams p = make_params(st, first, count, reinterpret_cast<const void* const*>(work + L.off_ptrs[buf]),
+                                        d_ident, nullptr);
+      PSYNC_CU(psync::launch_fused(p, st->grad_dtype, st->opt, st->ema_mode, st->variant, st->grid_ctas, s));
+      PSYNC_CU(cudaEventRecord(consumed[buf], s));
+      if (h_theta_out != nullptr)
+        PSYNC_CU(cudaMemcpyAsync(h_theta_out + first, st->d_theta + first, sizeof(float) * static_cast<size_t>(count),
+                                 cudaMemcpyDeviceToHost, s));
+    }
+  }
+  PSYNC_CU(cudaStreamSynchronize(copy_stream));
+  PSYNC_CU(cudaStreamSynchronize(s));
+
+cleanup:
+#undef PSYNC_CU
+  if (result == PSYNC_ECUDA) cudaGetLastError();
+  if (copy_stream != nullptr) {
+    cudaStreamSynchronize(copy_stream);
+    cudaStreamDestroy(copy_stream);
+  }
+  for (int i = 0; i < 2; ++i) {
+    if (copied[i] != nullptr) cudaEventDestroy(copied[i]);
+    if (consumed[i] != nullptr) cudaEventDestroy(consumed[i]);
+  }
+  return result;
+}
+
+}  // extern "C"

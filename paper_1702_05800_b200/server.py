@@ -1,0 +1,67 @@
+"""ParameterServerStep: device buffers + the two calls of one step (plumbing only, no arithmetic).
+
+Holds theta / ema / optimizer state, the kept[] / status / t_Nth outputs of the selection kernel and
+the device pointer table of the W gradient buffers, and enqueues psync_select_first_n followed by
+psync_aggregate_update on one stream with no host synchronisation in between (Alg. 4).
+"""
+from __future__ import annotations
+
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+from . import binding as B
+
+
+class ParameterServerStep:
+    def __init__(self, shard_off, N: int, b: int, theta: torch.Tensor, ema: Optional[torch.Tensor],
+                 state0: Optional[torch.Tensor], state1: Optional[torch.Tensor], opt: int, ema_mode: int,
+                 alpha: float = 0.0, mu: float = 0.0, rho: float = 0.0, eps: float = 0.0, grid_ctas: int = 0,
+                 variant: int = 0):
+        dev = theta.device
+        self.shard_off = np.ascontiguousarray(shard_off, dtype=np.int64)
+        self.N, self.b, self.W = N, b, N + b
+        self.theta, self.ema, self.state0, self.state1 = theta, ema, state0, state1
+        self.opt, self.ema_mode = opt, ema_mode
+        self.alpha, self.mu, self.rho, self.eps = alpha, mu, rho, eps
+        self.grid_ctas, self.variant = grid_ctas, variant
+        self.d_kept = torch.full((N,), -1, dtype=torch.int32, device=dev)
+        self.d_status = torch.full((1,), B.PSYNC_ECUDA, dtype=torch.int32, device=dev)
+        self.d_t_nth = torch.zeros(1, dtype=torch.float32, device=dev)
+        self.table: Optional[B.GradTable] = None
+        self._step = None
+        self._keep = None
+
+    def set_gradients(self, buffers: Sequence[torch.Tensor]) -> None:
+        if len(buffers) != self.W:
+            raise ValueError(f"need W = {self.W} gradient buffers")
+        self.table = B.make_grad_table(buffers)
+        self._step = None
+
+    def _build(self, gamma_t: float):
+        self._step, self._keep = B.make_step(
+            self.shard_off, self.N, self.W, self.table.grad_dtype, self.theta, self.ema, self.state0, self.state1,
+            opt=self.opt, ema_mode=self.ema_mode, gamma_t=gamma_t, alpha=self.alpha, mu=self.mu, rho=self.rho,
+            eps=self.eps, d_grads=self.table.d_ptrs, d_kept=self.d_kept, d_status=self.d_status,
+            grid_ctas=self.grid_ctas, variant=self.variant)
+        return self._step
+
+    def geometry(self, gamma_t: float = 0.0) -> dict:
+        return B.psync_launch_geometry(self._build(gamma_t))
+
+    def step(self, d_arrival: torch.Tensor, gamma_t: float, d_step_tag: Optional[torch.Tensor] = None, t: int = 0,
+             stream=None) -> None:
+        """Enqueue selection + fused update for one iteration; returns without synchronising."""
+        if self.table is None:
+            raise RuntimeError("set_gradients() first")
+        if self._step is None or self._step.gamma_t != np.float32(gamma_t):
+            self._build(gamma_t)
+        B.psync_select_first_n(d_arrival, self.N, self.b, self.d_kept, self.d_status, self.d_t_nth, d_step_tag, t,
+                               stream)
+        B.psync_aggregate_update(self._step, stream)
+
+    def aggregate_only(self, gamma_t: float, stream=None) -> None:
+        if self._step is None or self._step.gamma_t != np.float32(gamma_t):
+            self._build(gamma_t)
+        B.psync_aggregate_update(self._step, stream)

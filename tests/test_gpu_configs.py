@@ -1,0 +1,153 @@
+"""GPU parity on the BASELINE.json configs: cfg1 in full; cfg2-4 at a reduced P the oracle finishes
+in seconds (several tiles + ragged tail, same N/b/M/optimizer/hyper-parameters) element by element;
+and at FULL size, in the launch configuration bench.py times, on sampled outputs the oracle
+computes one by one.  Also the host-buffer entry point psync_step_host."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1702_05800_b200 as psync
+from paper_1702_05800_b200 import synth
+
+from _harness import ATOL_STEP, RTOL_BF16, RTOL_FREE_100, RTOL_STEP, Pair, assert_close, to_np
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def test_cfg1_tiny_all_10_steps_lockstep_and_free_run():
+    Pair(synth.TINY).run(synth.TINY.steps, lockstep=True)
+    Pair(synth.TINY).run(synth.TINY.steps, lockstep=False, rtol=RTOL_FREE_100)
+
+
+@pytest.mark.parametrize("cfg", [synth.INCEPTION_SGD, synth.PAPER_RMSPROP, synth.MIXED_PRECISION],
+                         ids=lambda c: c.name)
+def test_cfg2_3_4_reduced_P_lockstep(cfg):
+    small = synth.scaled(cfg, 786_432 + 13)      # 768 Ki + ragged tail: hundreds of tiles, M ragged shards
+    rtol = RTOL_BF16 if cfg.grad_dtype == synth.BF16 else RTOL_STEP
+    Pair(small).run(3, lockstep=True, rtol=rtol, atol=ATOL_STEP)
+    if cfg.grad_dtype == synth.BF16:              # widening is exact, so the tight bound holds too
+        Pair(small).run(1, lockstep=True, rtol=RTOL_STEP, atol=ATOL_STEP)
+
+
+@pytest.mark.parametrize("cfg", [synth.INCEPTION_SGD, synth.PAPER_RMSPROP, synth.MIXED_PRECISION],
+                         ids=lambda c: c.name)
+def test_free_run_100_steps(cfg):
+    """north_star: 1e-4 relative after 100 steps of free running (2e-3 with bf16 gradients)."""
+    small = synth.scaled(cfg, 16_384 + 5)
+    rtol = RTOL_BF16 if cfg.grad_dtype == synth.BF16 else RTOL_FREE_100
+    Pair(small).run(100, lockstep=False, rtol=rtol, atol=ATOL_STEP, check_every=25)
+
+
+def test_cfg5_sweep_points_reduced():
+    for cfg in synth.sweep_configs():
+        if cfg.P != synth.SWEEP_P[0]:
+            continue
+        Pair(synth.scaled(cfg, 262_144 + 3)).run(2, lockstep=True)
+
+
+# ------------------------------------------------------------------ full size, bench launch config
+def _full_size_sampled(cfg, steps=2, n_sample=40_000):
+    """Run the real config on the GPU; check sampled elements against the oracle run on the gathered
+    columns (gathering by index moves data, it computes nothing)."""
+    free, _ = torch.cuda.mem_get_info()
+    if cfg.footprint_bytes * 1.15 > free:
+        pytest.skip("not enough free HBM for the full-size config")
+    pair = Pair(cfg)          # default variant / grid = what bench.py launches
+    rng = np.random.default_rng(cfg.cfg_id)
+    tile = 8192
+    idx = np.unique(np.concatenate([
+        np.arange(0, 2 * tile), np.arange(cfg.P - 2 * tile, cfg.P),           # first and last tiles
+        pair.shard_off[1:-1], np.maximum(pair.shard_off[1:-1] - 1, 0),                        # every shard cut
+        rng.integers(0, cfg.P, n_sample)])).astype(np.int64)
+    d_idx = torch.from_numpy(idx).to(DEV)
+    off_s = np.array([0, idx.size], dtype=np.int64)
+    host = {n: (None if getattr(pair.ps, n) is None else to_np(getattr(pair.ps, n)[d_idx]))
+            for n in ("theta", "ema", "state0", "state1")}
+    grads = [torch.empty(cfg.P, dtype=torch.float32 if cfg.grad_dtype == synth.F32 else torch.bfloat16, device=DEV)
+             for _ in range(cfg.W)]
+    for s in range(steps):
+        for k in range(cfg.W):
+            synth.gradient(cfg, s, k, DEV, out=grads[k])
+        arrival = synth.arrival_times(cfg, s)
+        st, kept, tn = pair.gpu_step(grads, arrival)
+        st_o, kept_o, tn_o = oracle.select_first_n(arrival, cfg.N, cfg.b)
+        assert st == st_o == 0 and np.array_equal(kept, kept_o) and tn == tn_o
+        g_s = [synth.as_numpy_grad(g[d_idx]) for g in grads]
+        rc = oracle.aggregate_update(off_s, cfg.N, g_s, kept_o, host["theta"], host["ema"], host["state0"],
+                                     host["state1"], opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma,
+                                     alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
+        assert rc == oracle.OK
+        rtol = RTOL_BF16 if cfg.grad_dtype == synth.BF16 else RTOL_STEP
+        for n in ("theta", "ema", "state0", "state1"):
+            if host[n] is not None:
+                got = to_np(getattr(pair.ps, n)[d_idx])
+                assert_close(got, host[n], rtol, ATOL_STEP, f"{cfg.name} step {s} {n} (sampled)")
+                host[n] = got                                               # lock-step
+        # property that holds at any size: nothing outside tolerance can hide as NaN/Inf
+        assert bool(torch.isfinite(pair.ps.theta).all())
+    geo = pair.ps.geometry(cfg.gamma)
+    assert geo["grid"] % 148 == 0 or torch.cuda.get_device_properties(0).multi_processor_count != 148
+
+
+def test_full_size_cfg3_paper_rmsprop_sampled():
+    _full_size_sampled(synth.PAPER_RMSPROP)
+
+
+def test_full_size_cfg2_inception_sgd_sampled():
+    _full_size_sampled(synth.INCEPTION_SGD)
+
+
+def test_full_size_cfg4_mixed_precision_sampled():
+    _full_size_sampled(synth.MIXED_PRECISION, steps=1)
+
+
+# ------------------------------------------------------------------ host-buffer entry point
+@pytest.mark.parametrize("cfg,chunk", [(synth.scaled(synth.PAPER_RMSPROP, 300_000 + 7), 65_536),
+                                       (synth.scaled(synth.MIXED_PRECISION, 200_000 + 3), 0),
+                                       (synth.TINY, 1024)], ids=["rmsprop_chunked", "bf16_default_chunk", "tiny"])
+def test_step_host_matches_oracle(cfg, chunk):
+    pair = Pair(cfg)
+    nbytes = psync.psync_step_host_workspace_bytes(cfg.N, cfg.W, cfg.grad_dtype, chunk)
+    assert nbytes > 0
+    d_work = torch.empty(nbytes, dtype=torch.uint8, device=DEV)
+    h_theta = torch.empty(cfg.P, dtype=torch.float32).pin_memory()
+    h_kept = np.full(cfg.N, -1, dtype=np.int32)
+    for s in range(2):
+        h_grads = [synth.gradient(cfg, s, k, "cpu").pin_memory() for k in range(cfg.W)]
+        arrival = synth.arrival_times(cfg, s)
+        step, keep = psync.make_step(pair.shard_off, cfg.N, cfg.W, cfg.grad_dtype, pair.ps.theta, pair.ps.ema,
+                                     pair.ps.state0, pair.ps.state1, opt=cfg.opt, ema_mode=cfg.ema_mode,
+                                     gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
+        st, t_nth = psync.psync_step_host(step, arrival, h_grads, d_work, h_theta_out=h_theta, h_kept=h_kept,
+                                          chunk_elems=chunk)
+        st_o, kept_o, tn_o = pair.oracle_step(h_grads, arrival)
+        assert st == st_o == 0 and np.array_equal(h_kept, kept_o) and t_nth == tn_o
+        rtol = RTOL_BF16 if cfg.grad_dtype == synth.BF16 else RTOL_STEP
+        pair.compare(rtol, ATOL_STEP, f"host step {s}")
+        assert np.array_equal(h_theta.numpy(), to_np(pair.ps.theta))       # theta(t+1) came back to the host
+        pair.sync_host_from_gpu()
+
+
+def test_step_host_too_few_and_bad_workspace():
+    cfg = synth.scaled(synth.TINY, 2048)
+    pair = Pair(cfg)
+    before = to_np(pair.ps.theta)
+    nbytes = psync.psync_step_host_workspace_bytes(cfg.N, cfg.W, cfg.grad_dtype, 0)
+    d_work = torch.empty(nbytes, dtype=torch.uint8, device=DEV)
+    h_grads = [synth.gradient(cfg, 0, k, "cpu") for k in range(cfg.W)]       # pageable memory is allowed
+    step, keep = psync.make_step(pair.shard_off, cfg.N, cfg.W, cfg.grad_dtype, pair.ps.theta, pair.ps.ema,
+                                 opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha)
+    arrival = np.array([0.1, np.nan, np.inf, 0.2, 0.3], dtype=np.float32)
+    st, _ = psync.psync_step_host(step, arrival, h_grads, d_work)
+    assert st == psync.PSYNC_ETOOFEW and np.array_equal(before, to_np(pair.ps.theta))
+    st, _ = psync.psync_step_host(step, synth.arrival_times(cfg, 0), h_grads, d_work[: nbytes // 2], check=False)
+    assert st == psync.PSYNC_EINVAL
+    assert psync.psync_step_host_workspace_bytes(cfg.N, cfg.W, cfg.grad_dtype, 100) == 0   # not a multiple of 64
+    st, _ = psync.psync_step_host(step, synth.arrival_times(cfg, 0), h_grads, d_work)
+    assert st == psync.PSYNC_OK
+    pair.oracle_step(h_grads, synth.arrival_times(cfg, 0))
+    pair.compare(RTOL_STEP, ATOL_STEP, "host pageable")

@@ -1,0 +1,285 @@
+"""GPU parity for K2 / K3 (psync_aggregate_update, psync_ema) against the CPU oracle, element by
+element, at sizes spanning several tiles and a ragged tail.  PAPER.md Alg. 4 l.8-9 (L160-162), L40."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1702_05800_b200 as psync
+from paper_1702_05800_b200 import synth
+
+from _harness import ATOL_STEP, RTOL_BF16, RTOL_FREE_100, RTOL_STEP, Pair, assert_close, to_np
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+BASE = synth.Config(name="unit", cfg_id=9, P=70_003, M=7, N=10, b=3, arrival_sigma=0.3, opt=synth.SGD, gamma=0.045,
+                    alpha=0.9999, mu=0.9, rho=0.9, eps=1.0, steps=3)
+
+
+def rtol_for(cfg):
+    return RTOL_BF16 if cfg.grad_dtype == synth.BF16 else RTOL_STEP
+
+
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+@pytest.mark.parametrize("opt", [synth.SGD, synth.MOMENTUM, synth.RMSPROP_MOM])
+@pytest.mark.parametrize("ema_mode", [synth.EMA_POST, synth.EMA_PRE, synth.EMA_OFF])
+def test_every_template_instance_lockstep(dtype, opt, ema_mode):
+    cfg = replace(BASE, grad_dtype=dtype, opt=opt, ema_mode=ema_mode, name=f"unit_d{dtype}_o{opt}_e{ema_mode}")
+    # fp32 gradients are held to the fp32 tolerance even here; bf16 inputs are widened exactly, so they too
+    # meet the tight bound -- the loose 2e-3 is only the ceiling north_star allows
+    Pair(cfg).run(3, lockstep=True, rtol=RTOL_STEP, atol=ATOL_STEP)
+
+
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+def test_every_variant(variant, dtype):
+    cfg = replace(BASE, grad_dtype=dtype, opt=synth.RMSPROP_MOM, N=21, b=2, P=200_001, name=f"variant{variant}")
+    Pair(cfg, variant=variant).run(2, lockstep=True)
+
+
+@pytest.mark.parametrize("P", [0, 1, 3, 4, 5, 7, 8, 9, 31, 1023, 1024, 1025, 4096 + 6])
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+def test_small_and_ragged_sizes(P, dtype):
+    cfg = replace(BASE, P=P, M=min(3, max(1, P)), grad_dtype=dtype, opt=synth.MOMENTUM, name=f"small{P}")
+    if P == 0:
+        th = torch.zeros(0, dtype=torch.float32, device=DEV)
+        step, keep = psync.make_step([0, 0], 2, 2, dtype, th, th.clone(), th.clone(), None, opt=synth.MOMENTUM,
+                                     d_grads=torch.zeros(2, dtype=torch.int64, device=DEV),
+                                     d_kept=torch.zeros(2, dtype=torch.int32, device=DEV))
+        assert psync.psync_aggregate_update(step) == psync.PSYNC_OK
+        return
+    Pair(cfg).run(2, lockstep=True)
+
+
+@pytest.mark.parametrize("N,b", [(1, 0), (1, 4), (2, 0), (7, 0), (8, 1), (9, 0), (16, 2), (17, 3), (100, 6)])
+def test_worker_counts_cross_unroll_boundaries(N, b):
+    cfg = replace(BASE, N=N, b=b, P=20_011, opt=synth.RMSPROP_MOM, name=f"N{N}b{b}")
+    Pair(cfg).run(2, lockstep=True)
+
+
+def test_max_workers_1024():
+    cfg = replace(BASE, N=1000, b=24, P=4099, opt=synth.SGD, name="W1024")
+    Pair(cfg).run(1, lockstep=True)
+
+
+def _views_with_offset(P, W, dtype, offset_elems):
+    """Buffers whose base is offset from the allocation by offset_elems elements (misaligned when odd)."""
+    tdt = torch.float32 if dtype == synth.F32 else torch.bfloat16
+    gen = torch.Generator(device=DEV)
+    gen.manual_seed(99)
+    out = []
+    for _ in range(W):
+        raw = torch.empty(P + 16, dtype=torch.float32, device=DEV).normal_(0, 1e-3, generator=gen).to(tdt)
+        out.append(raw[offset_elems:offset_elems + P])
+    return out
+
+
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+@pytest.mark.parametrize("which", ["grads", "theta", "one_grad"])
+def test_unaligned_pointers_take_the_scalar_path(dtype, which):
+    P, N, b = 10_007, 5, 2
+    W = N + b
+    cfg = replace(BASE, P=P, N=N, b=b, M=1, grad_dtype=dtype, opt=synth.RMSPROP_MOM, name="unaligned")
+    grads = _views_with_offset(P, W, dtype, 1 if which == "grads" else 0)
+    if which == "one_grad":
+        grads[3] = _views_with_offset(P, 1, dtype, 1)[0]
+    theta = None
+    if which == "theta":
+        theta = torch.empty(P + 4, dtype=torch.float32, device=DEV).normal_(0, 0.02)[1:P + 1]
+    pair = Pair(cfg, theta=theta)
+    arrival = np.array([0.1, 0.2, 9.0, 0.3, 0.4, 8.0, 0.5], dtype=np.float32)   # keeps 0,1,3,4,6
+    st, kept, _ = pair.gpu_step(grads, arrival)
+    st_o, kept_o, _ = pair.oracle_step(grads, arrival)
+    assert st == 0 and np.array_equal(kept, kept_o) and kept.tolist() == [0, 1, 3, 4, 6]
+    pair.compare(RTOL_STEP, ATOL_STEP, "unaligned")
+
+
+def test_exact_arithmetic_inputs_are_bit_identical():
+    """Dyadic gradients, N a power of two: every fp32 partial sum is exact, so the CUDA result must
+    equal the oracle bit for bit (any dropped term, wrong divisor or reordering shows)."""
+    P, N, b = 50_000 + 3, 8, 2
+    W = N + b
+    rng = np.random.default_rng(3)
+    grads = [torch.from_numpy((rng.integers(-64, 65, P) / 256.0).astype(np.float32)).to(DEV) for _ in range(W)]
+    theta = torch.from_numpy((rng.integers(-512, 513, P) / 1024.0).astype(np.float32)).to(DEV)
+    cfg = replace(BASE, P=P, N=N, b=b, M=3, opt=synth.SGD, gamma=0.5, alpha=0.5, name="exact")
+    pair = Pair(cfg, theta=theta)
+    arrival = synth.arrival_times(cfg, 0)
+    pair.gpu_step(grads, arrival)
+    pair.oracle_step(grads, arrival)
+    assert np.array_equal(to_np(pair.ps.theta), pair.host["theta"])
+    assert np.array_equal(to_np(pair.ps.ema), pair.host["ema"])
+
+
+def test_dropped_buffers_are_never_read_poison():
+    cfg = replace(BASE, P=30_001, N=6, b=3, opt=synth.RMSPROP_MOM, name="poison")
+    arrival = synth.arrival_times(cfg, 0)
+    _, kept, _ = oracle.select_first_n(arrival, cfg.N, cfg.b)
+    dropped = sorted(set(range(cfg.W)) - set(kept.tolist()))
+    outs = []
+    for poison in (False, True):
+        pair = Pair(cfg)
+        grads = pair.gradients(0)
+        if poison:
+            for k in dropped:
+                grads[k].fill_(float("nan"))
+        pair.gpu_step(grads, arrival)
+        outs.append([to_np(getattr(pair.ps, n)) for n in ("theta", "ema", "state0", "state1")])
+    for a, b_ in zip(*outs):
+        assert np.array_equal(a, b_) and np.isfinite(a).all()
+
+
+def test_null_pointer_for_dropped_worker_is_fine():
+    """A dropped worker's table entry may even be NULL: it is never dereferenced."""
+    cfg = replace(BASE, P=5_000, N=3, b=1, M=1, name="nullptr")
+    pair = Pair(cfg)
+    grads = pair.gradients(0)
+    arrival = np.array([0.3, 0.1, 50.0, 0.2], dtype=np.float32)
+    pair.ps.set_gradients(grads)
+    pair.ps.table.d_ptrs[2] = 0
+    pair.ps.step(torch.from_numpy(arrival).to(DEV), cfg.gamma)
+    torch.cuda.synchronize()
+    pair.oracle_step(grads, arrival)
+    pair.compare(RTOL_STEP, ATOL_STEP, "nullptr")
+
+
+def test_bitwise_invariance_shard_layout_grid_variant_and_rerun():
+    cfg = replace(BASE, P=123_457, N=13, b=2, opt=synth.RMSPROP_MOM, name="invariance")
+    arrival = synth.arrival_times(cfg, 0)
+    ref = None
+    P = cfg.P
+    layouts = [None, [0, P], [0, 1, 2, 77_777, 77_777, P]]
+    runs = [(lay, 0, 0) for lay in layouts] + [(None, 1, v) for v in range(1, 7)] + [(None, 37, 0), (None, 1000, 2)]
+    runs.append((None, 0, 0))   # the same launch again
+    for lay, grid, variant in runs:
+        pair = Pair(cfg, shard_off=lay, grid_ctas=grid, variant=variant)
+        pair.gpu_step(pair.gradients(0), arrival)
+        out = [to_np(getattr(pair.ps, n)) for n in ("theta", "ema", "state0", "state1")] + [pair.ps.d_kept.cpu().numpy()]
+        if ref is None:
+            ref = out
+        for a, b_ in zip(ref, out):
+            assert np.array_equal(a, b_), f"layout={lay} grid={grid} variant={variant}"
+
+
+def test_status_not_ok_leaves_state_untouched():
+    cfg = replace(BASE, P=9_001, N=4, b=1, opt=synth.RMSPROP_MOM, name="toofew")
+    pair = Pair(cfg)
+    before = [to_np(getattr(pair.ps, n)) for n in ("theta", "ema", "state0", "state1")]
+    arrival = np.array([0.1, np.inf, np.nan, 0.2, 0.3], dtype=np.float32)
+    st, _, _ = pair.gpu_step(pair.gradients(0), arrival)
+    assert st == psync.PSYNC_ETOOFEW
+    for a, n in zip(before, ("theta", "ema", "state0", "state1")):
+        assert np.array_equal(a, to_np(getattr(pair.ps, n)))
+    st_o, _, _ = pair.oracle_step(pair.gradients(0), arrival)
+    assert st_o == oracle.ETOOFEW
+
+
+def test_stale_tags_are_dropped():
+    """Alg. 4 l.5-6: a gradient tagged t' != t is dropped even if it arrived first."""
+    cfg = replace(BASE, P=6_001, N=3, b=2, name="tags")
+    pair = Pair(cfg)
+    grads = pair.gradients(0)
+    arrival = np.array([0.01, 0.5, 0.6, 0.7, 0.02], dtype=np.float32)
+    tags = np.array([6, 7, 7, 7, 7], dtype=np.int32)
+    st, kept, tn = pair.gpu_step(grads, arrival, tags=tags, t=7)
+    st_o, kept_o, tn_o = pair.oracle_step(grads, arrival, tags=tags, t=7)
+    assert st == 0 and kept.tolist() == [1, 2, 4] == kept_o.tolist() and tn == tn_o
+    pair.compare(RTOL_STEP, ATOL_STEP, "tags")
+
+
+def test_psync_ema_matches_oracle_and_fused_post():
+    rng = np.random.default_rng(4)
+    for P in (1, 5, 4096, 100_003):
+        theta = torch.from_numpy(rng.normal(0, 0.02, P).astype(np.float32)).to(DEV)
+        ema = torch.from_numpy(rng.normal(0, 0.02, P).astype(np.float32)).to(DEV)
+        want = to_np(ema)
+        oracle.ema_update(want, to_np(theta), 0.9999)
+        psync.psync_ema(ema, theta, 0.9999)
+        torch.cuda.synchronize()
+        assert_close(to_np(ema), want, RTOL_STEP, ATOL_STEP, f"psync_ema P={P}")
+    # EMA_OFF fused step + psync_ema == EMA_POST fused step, bit for bit
+    cfg = replace(BASE, P=40_001, opt=synth.MOMENTUM, name="ema_split")
+    arrival = synth.arrival_times(cfg, 0)
+    a = Pair(cfg)
+    a.gpu_step(a.gradients(0), arrival)
+    b_ = Pair(replace(cfg, ema_mode=synth.EMA_OFF))
+    ema_b = b_.ps.theta.clone()
+    b_.gpu_step(b_.gradients(0), arrival)
+    psync.psync_ema(ema_b, b_.ps.theta, cfg.alpha)
+    torch.cuda.synchronize()
+    assert np.array_equal(to_np(a.ps.theta), to_np(b_.ps.theta))
+    assert np.array_equal(to_np(a.ps.ema), to_np(ema_b))
+
+
+def test_ema_constant_theta_closed_form_on_gpu():
+    """gamma = 0: theta never moves and ema_T = alpha^T ema_0 + (1 - alpha^T) theta (north_star)."""
+    P, T, alpha = 2_000, 100, 0.999
+    cfg = replace(BASE, P=P, N=2, b=1, M=1, gamma=0.0, alpha=alpha, name="ema_closed")
+    pair = Pair(cfg)
+    theta0 = to_np(pair.ps.theta)
+    pair.ps.ema.copy_(torch.from_numpy(np.random.default_rng(6).uniform(-0.1, 0.1, P).astype(np.float32)))
+    ema0 = to_np(pair.ps.ema)
+    grads = pair.gradients(0)
+    for s in range(T):
+        pair.gpu_step(grads, synth.arrival_times(cfg, s))
+    assert np.array_equal(to_np(pair.ps.theta), theta0)
+    a = float(np.float32(alpha))
+    want = a ** T * ema0.astype(np.float64) + (1 - a ** T) * theta0.astype(np.float64)
+    assert_close(to_np(pair.ps.ema), want, 1e-4, 1e-6, "ema closed form")
+
+
+def test_b0_plain_mean_and_n1_earliest_on_gpu():
+    cfg = replace(BASE, P=12_345, N=16, b=0, M=1, gamma=0.25, ema_mode=synth.EMA_OFF, name="b0")
+    pair = Pair(cfg)
+    theta0 = to_np(pair.ps.theta).astype(np.float64)
+    grads = pair.gradients(0)
+    pair.gpu_step(grads, synth.arrival_times(cfg, 0))
+    mean = np.stack([to_np(g) for g in grads]).astype(np.float64).mean(axis=0)
+    assert_close(to_np(pair.ps.theta), theta0 - float(np.float32(0.25)) * mean, RTOL_STEP, ATOL_STEP, "b=0 mean")
+    cfg = replace(BASE, P=12_345, N=1, b=6, M=1, gamma=0.5, ema_mode=synth.EMA_OFF, name="n1")
+    pair = Pair(cfg)
+    theta0 = to_np(pair.ps.theta).astype(np.float64)
+    grads = pair.gradients(0)
+    arrival = synth.arrival_times(cfg, 0)
+    _, kept, _ = pair.gpu_step(grads, arrival)
+    k = int(np.argmin(arrival))
+    assert kept.tolist() == [k]
+    assert np.array_equal(to_np(pair.ps.theta), (theta0 - 0.5 * to_np(grads[k]).astype(np.float64)).astype(np.float32))
+
+
+def test_permutation_invariance_on_gpu():
+    cfg = replace(BASE, P=8_191, N=10, b=3, M=1, name="perm")
+    arrival = np.random.default_rng(8).permutation(np.linspace(0.5, 2.5, cfg.W)).astype(np.float32)
+    a = Pair(cfg)
+    grads = a.gradients(0)
+    _, kept_a, _ = a.gpu_step(grads, arrival)
+    pi = np.random.default_rng(9).permutation(cfg.W)
+    b_ = Pair(cfg)
+    _, kept_b, _ = b_.gpu_step([grads[p] for p in pi], arrival[pi].copy())
+    assert set(pi[kept_b].tolist()) == set(kept_a.tolist())
+    assert_close(to_np(b_.ps.theta), to_np(a.ps.theta), RTOL_STEP, ATOL_STEP, "permutation")
+
+
+def test_argument_errors_return_einval_and_touch_nothing():
+    cfg = replace(BASE, P=1_000, N=3, b=1, M=2, opt=synth.RMSPROP_MOM, name="einval")
+    pair = Pair(cfg)
+    pair.ps.set_gradients(pair.gradients(0))
+    before = to_np(pair.ps.theta)
+    good = dict(shard_off=pair.shard_off, N=3, W=4, grad_dtype=0, theta=pair.ps.theta, ema=pair.ps.ema,
+                state0=pair.ps.state0, state1=pair.ps.state1, opt=2, ema_mode=0, d_grads=pair.ps.table.d_ptrs,
+                d_kept=pair.ps.d_kept, d_status=pair.ps.d_status)
+    bad_cases = [dict(shard_off=[0, 600, 999]), dict(shard_off=[0, 700, 600, 1000]), dict(N=0), dict(W=2),
+                 dict(W=2000, N=1500), dict(grad_dtype=5), dict(opt=3), dict(ema_mode=-1), dict(ema=None),
+                 dict(state0=None), dict(state1=None), dict(d_grads=None), dict(d_kept=None), dict(variant=99),
+                 dict(grid_ctas=-1)]
+    for bad in bad_cases:
+        kw = dict(good)
+        kw.update(bad)
+        step, keep = psync.make_step(**kw)
+        assert psync.psync_aggregate_update(step, check=False) == psync.PSYNC_EINVAL, bad
+    torch.cuda.synchronize()
+    assert np.array_equal(before, to_np(pair.ps.theta))
+    assert psync.psync_ema(pair.ps.ema, pair.ps.theta, 0.9) == psync.PSYNC_OK
