@@ -71,6 +71,9 @@ class ClockSampler:
         self._stop = threading.Event()
         self._thr = None
         self.ok = False
+        if period_s < 0:
+            self.err = "disabled"
+            return
         try:
             import pynvml
             pynvml.nvmlInit()
@@ -134,7 +137,7 @@ def load_peaks():
 
 
 # ------------------------------------------------------------------------------------ CPU oracle legs
-def oracle_sample(cfg, seconds_budget=12.0, sample_elems=1 << 22, max_steps=200, warmup=0, fixed_steps=None,
+def oracle_sample(cfg, seconds_budget=12.0, sample_elems=1 << 22, max_steps=2000, warmup=0, fixed_steps=None,
                   wall_budget=60.0):
     """Times the oracle AS IT STANDS on the host cores on a bounded sample of the workload: the first
     `sample_elems` parameters of every buffer (same N, b, M-way ragged cut, optimizer, distributions).
@@ -216,12 +219,6 @@ def run_psync(args, cfg, rank, world, dist):
     dev = torch.device("cuda", local)
     K, Wm = args.steps, args.warmup
     off = synth.shard_offsets(cfg)
-    theta = synth.init_theta(cfg, dev)
-    s0, s1 = synth.init_state(cfg, dev)
-    ema = theta.clone()
-    ps = psync.ParameterServerStep(off, cfg.N, cfg.b, theta, ema, s0, s1, cfg.opt, cfg.ema_mode, alpha=cfg.alpha,
-                                   mu=cfg.mu, rho=cfg.rho, eps=cfg.eps, grid_ctas=args.grid_ctas, variant=args.variant)
-
     # resident gradient sets, rotated step by step: every step streams buffers it did not just touch
     set_bytes = cfg.W * cfg.P * cfg.grad_bytes
     free, _ = torch.cuda.mem_get_info()
@@ -233,6 +230,12 @@ def run_psync(args, cfg, rank, world, dist):
         for k in range(cfg.W):
             synth.gradient(cfg, r, k, dev, out=bufs[k])
         tables.append(psync.make_grad_table(bufs))
+    theta = synth.init_theta(cfg, dev)
+    s0, s1 = synth.init_state(cfg, dev)
+    ema = theta.clone()
+    ps = psync.ParameterServerStep(off, cfg.N, cfg.b, theta, ema, s0, s1, cfg.opt, cfg.ema_mode, alpha=cfg.alpha,
+                                   mu=cfg.mu, rho=cfg.rho, eps=cfg.eps, grid_ctas=args.grid_ctas, variant=args.variant)
+
     arrivals = torch.from_numpy(np.stack([synth.arrival_times(cfg, s) for s in range(K + Wm)])).to(dev)
     steps_struct = []
     for tb in tables:   # one psync_step per gradient set, built once (marshalling outside the timed region)
@@ -268,7 +271,7 @@ def run_psync(args, cfg, rank, world, dist):
 
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
     e_begin, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler = ClockSampler(local)
+    sampler = ClockSampler(local, period_s=args.clock_period_ms * 1e-3)
     barrier()
     torch.cuda.synchronize()
     sampler.start()
@@ -282,6 +285,8 @@ def run_psync(args, cfg, rank, world, dist):
     total_ms = e_begin.elapsed_time(e_end)
     fused_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
     select_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    if os.environ.get("PSYNC_BENCH_DEBUG"):
+        print("fused ms per step:", [round(e[1].elapsed_time(e[2]), 4) for e in evs], file=sys.stderr)
     assert int(ps.d_status.item()) == 0 and bool(torch.isfinite(theta[:4096]).all())
 
     units_local = float(cfg.N) * cfg.P * K
@@ -389,6 +394,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--clock-period-ms", type=float, default=2.0)
     ap.add_argument("--ref-sample-elems", type=int, default=0)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "psync":

@@ -90,7 +90,7 @@ def _full_size_sampled(cfg, steps=2, n_sample=40_000):
         # property that holds at any size: nothing outside tolerance can hide as NaN/Inf
         assert bool(torch.isfinite(pair.ps.theta).all())
     geo = pair.ps.geometry(cfg.gamma)
-    assert geo["grid"] % 148 == 0 or torch.cuda.get_device_properties(0).multi_processor_count != 148
+    assert geo["grid"] == -(-cfg.P // geo["tile_elems"])          # one tile per CTA, the bench's launch
 
 
 def test_full_size_cfg3_paper_rmsprop_sampled():
