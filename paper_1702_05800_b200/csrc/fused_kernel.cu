@@ -139,6 +139,12 @@ __global__ void __launch_bounds__(THREADS, MINB) fused_aggregate_update_ema(cons
   constexpr int Q = E / 4;  // float4 groups of theta per unit
   __shared__ const char* s_ptr[kMaxWorkers];
 
+  // Programmatic dependent launch: this CTA may be resident before the selection kernel (or the previous
+  // fused launch) has finished; nothing is read before the wait.  The successor is released at once --
+  // it, too, waits for this whole grid before touching memory.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+
   if (p.status != nullptr && *p.status != 0) return;  // selection failed: leave everything untouched
 
   unsigned misalign = 0;
@@ -365,8 +371,17 @@ cudaError_t launch_fused(const FusedParams& p, int dtype, int opt, int ema, int 
   cudaError_t err = fused_geometry(dtype, opt, ema, variant, grid_ctas, p.P, &g);
   if (err != cudaSuccess) return err;
   const int v = resolve_variant(dtype, variant);
-  pick_kernel(v, dtype, opt, ema)<<<g.grid, g.block, 0, stream>>>(p);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(static_cast<unsigned>(g.grid));
+  cfg.blockDim = dim3(static_cast<unsigned>(g.block));
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, pick_kernel(v, dtype, opt, ema), p);
 }
 
 cudaError_t launch_ema(float* d_ema, const float* d_theta, int64_t P, float alpha, cudaStream_t stream) {

@@ -8,12 +8,13 @@
 //   1. each fp32 arrival time becomes an order-preserving uint32 key (after -0.0 -> +0.0);
 //      ineligible workers (non-finite time or stale tag) get the key 0xFFFFFFFF, which no
 //      finite time maps to and which sorts last;
-//   2. the N-th smallest key tau is found by a 32-pass MSB-first radix select
-//      (per pass: count the still-matching keys whose current bit is 0, warp-reduce);
+//   2. the N-th smallest key tau is found by a 16-pass MSB-first radix select, two bits per pass
+//      (per pass: count the still-matching keys per digit value, warp-reduce);
 //   3. worker k is kept iff key_k < tau, or key_k == tau and k is among the first
 //      (N - #{key < tau}) such workers in index order (ties go to the lower index, reading R1).
 // Lanes own CONTIGUOUS index ranges, so a warp exclusive scan of the per-lane kept counts
 // gives every lane its output offset and the list comes out in ascending worker order.
+// The keys stay in registers (C per lane, templated), the select takes two bits per pass.
 
 #include "psync_kernels.cuh"
 
@@ -47,57 +48,86 @@ __device__ __forceinline__ int warp_exclusive_scan(int v, int lane, int* total) 
   return incl - v;
 }
 
+// Programmatic dependent launch (PDL): launched with programmatic stream serialization, this kernel
+// may become resident while its predecessor in the stream (typically the previous step's fused
+// kernel) drains, which hides its launch latency.  It touches no memory before griddepcontrol.wait
+// (which returns once the predecessor has completed and its writes are visible), so ordinary stream
+// semantics are preserved for any predecessor.  It releases its successor (the fused kernel, which
+// waits the same way before reading kept[]) immediately.
+__device__ __forceinline__ void pdl_wait_for_predecessor() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_release_successor() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// C = keys per lane (W <= 32*C); the keys live in registers, every loop is unrolled.
+template <int C>
 __global__ void __launch_bounds__(32) select_first_n_kernel(const float* __restrict__ arrival,
                                                             const int32_t* __restrict__ tags, int32_t t, int32_t N,
                                                             int32_t W, int32_t* __restrict__ kept,
                                                             float* __restrict__ t_nth, int32_t* __restrict__ status) {
-  // key of worker k lives at s_key[(k % c) * 32 + k / c]: lane k / c owns workers [lane*c, lane*c + c)
-  // and reads row i of its range at s_key[i * 32 + lane] -- conflict-free.
-  __shared__ uint32_t s_key[kMaxWorkers];
   const int lane = threadIdx.x;
-  const int c = (W + 31) >> 5;  // keys per lane, 1..32
+  const int base = lane * C;  // lane owns workers [base, base + C): ascending order falls out of the scan
+  pdl_release_successor();    // the fused kernel behind us may get resident; it waits before reading kept[]
+  pdl_wait_for_predecessor();
 
+  uint32_t key[C];
   int n_elig = 0;
-  for (int k = lane; k < c * 32; k += 32) {  // coalesced global reads
-    uint32_t key = kIneligible;
+#pragma unroll
+  for (int i = 0; i < C; ++i) {
+    const int k = base + i;
+    uint32_t v = kIneligible;
     if (k < W) {
-      key = arrival_key(arrival[k]);
-      if (tags != nullptr && tags[k] != t) key = kIneligible;  // Alg. 4 l.5-6: t' != t -> dropped
+      v = arrival_key(arrival[k]);
+      if (tags != nullptr && tags[k] != t) v = kIneligible;  // Alg. 4 l.5-6: t' != t -> dropped
     }
-    n_elig += (key != kIneligible);
-    s_key[(k % c) * 32 + (k / c)] = key;
+    key[i] = v;
+    n_elig += (v != kIneligible);
   }
   n_elig = __reduce_add_sync(0xFFFFFFFFu, n_elig);
-  __syncwarp();
   if (n_elig < N) {  // |G| can never reach N this step
     if (lane == 0) *status = kStatusTooFew;
     return;
   }
 
-  // radix select: tau = key of rank N-1 (0-based) among all keys (ineligible keys sort last)
+  // radix select, two bits per pass: tau = key of rank N-1 (0-based); ineligible keys sort last
   uint32_t prefix = 0u;
   int r = N - 1;
-  for (int bit = 31; bit >= 0; --bit) {
-    const uint32_t hi_mask = (bit == 31) ? 0u : (0xFFFFFFFFu << (bit + 1));
-    int zeros = 0;
-    for (int i = 0; i < c; ++i) {
-      const uint32_t key = s_key[i * 32 + lane];
-      zeros += (((key & hi_mask) == prefix) && (((key >> bit) & 1u) == 0u));
+#pragma unroll 1
+  for (int shift = 30; shift >= 0; shift -= 2) {
+    const uint32_t hi_mask = (shift == 30) ? 0u : (0xFFFFFFFFu << (shift + 2));
+    uint32_t c01 = 0u, c2 = 0u;  // counts of digit 0 (low half) and 1 (high half), and of digit 2
+#pragma unroll
+    for (int i = 0; i < C; ++i) {
+      const bool match = (key[i] & hi_mask) == prefix;
+      const uint32_t d = (key[i] >> shift) & 3u;
+      c01 += (match && d == 0u) ? 1u : 0u;
+      c01 += (match && d == 1u) ? 0x10000u : 0u;
+      c2 += (match && d == 2u) ? 1u : 0u;
     }
-    zeros = __reduce_add_sync(0xFFFFFFFFu, zeros);
-    if (r >= zeros) {
-      r -= zeros;
-      prefix |= (1u << bit);
+    c01 = __reduce_add_sync(0xFFFFFFFFu, c01);
+    c2 = __reduce_add_sync(0xFFFFFFFFu, c2);
+    const int n0 = static_cast<int>(c01 & 0xFFFFu), n1 = static_cast<int>(c01 >> 16), n2 = static_cast<int>(c2);
+    uint32_t digit;
+    if (r < n0) {
+      digit = 0u;
+    } else if (r < n0 + n1) {
+      digit = 1u;
+      r -= n0;
+    } else if (r < n0 + n1 + n2) {
+      digit = 2u;
+      r -= n0 + n1;
+    } else {
+      digit = 3u;
+      r -= n0 + n1 + n2;
     }
+    prefix |= digit << shift;
   }
   const uint32_t tau = prefix;
   const int eq_take = r + 1;  // how many of the workers tied at tau are kept, lowest indices first
 
   int n_less = 0, n_eq = 0;
-  for (int i = 0; i < c; ++i) {
-    const uint32_t key = s_key[i * 32 + lane];
-    n_less += (key < tau);
-    n_eq += (key == tau);
+#pragma unroll
+  for (int i = 0; i < C; ++i) {
+    n_less += (key[i] < tau);
+    n_eq += (key[i] == tau);
   }
   int total_eq, total_kept;
   const int eq_before = warp_exclusive_scan(n_eq, lane, &total_eq);
@@ -105,14 +135,14 @@ __global__ void __launch_bounds__(32) select_first_n_kernel(const float* __restr
   my_eq = my_eq < 0 ? 0 : (my_eq > n_eq ? n_eq : my_eq);
   int out = warp_exclusive_scan(n_less + my_eq, lane, &total_kept);  // total_kept == N
 
-  for (int i = 0; i < c; ++i) {  // ascending worker index within the lane's range
-    const uint32_t key = s_key[i * 32 + lane];
-    bool keep = key < tau;
-    if (key == tau && my_eq > 0) {
+#pragma unroll
+  for (int i = 0; i < C; ++i) {  // ascending worker index within the lane's range
+    bool keep = key[i] < tau;
+    if (key[i] == tau && my_eq > 0) {
       keep = true;
       --my_eq;
     }
-    if (keep) kept[out++] = lane * c + i;
+    if (keep) kept[out++] = base + i;
   }
   if (lane == 0) {
     *status = kStatusOk;
@@ -124,8 +154,24 @@ __global__ void __launch_bounds__(32) select_first_n_kernel(const float* __restr
 
 cudaError_t launch_select_first_n(const float* d_arrival, const int32_t* d_tags, int32_t t, int32_t N, int32_t W,
                                   int32_t* d_kept, float* d_t_nth, int32_t* d_status, cudaStream_t stream) {
-  select_first_n_kernel<<<1, 32, 0, stream>>>(d_arrival, d_tags, t, N, W, d_kept, d_t_nth, d_status);
-  return cudaGetLastError();
+  using Kernel = void (*)(const float*, const int32_t*, int32_t, int32_t, int32_t, int32_t*, float*, int32_t*);
+  Kernel kernel = select_first_n_kernel<32>;
+  if (W <= 32) kernel = select_first_n_kernel<1>;
+  else if (W <= 64) kernel = select_first_n_kernel<2>;
+  else if (W <= 128) kernel = select_first_n_kernel<4>;
+  else if (W <= 256) kernel = select_first_n_kernel<8>;
+  else if (W <= 512) kernel = select_first_n_kernel<16>;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(1);
+  cfg.blockDim = dim3(32);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, d_arrival, d_tags, t, N, W, d_kept, d_t_nth, d_status);
 }
 
 }  // namespace psync
