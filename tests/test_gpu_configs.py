@@ -151,3 +151,36 @@ def test_step_host_too_few_and_bad_workspace():
     assert st == psync.PSYNC_OK
     pair.oracle_step(h_grads, synth.arrival_times(cfg, 0))
     pair.compare(RTOL_STEP, ATOL_STEP, "host pageable")
+
+
+# ------------------------------------------------------------------ back-to-back launches (PDL ordering)
+@pytest.mark.parametrize("P", [4096, 300_000 + 5, 6_000_000 + 3])
+def test_back_to_back_steps_without_host_sync(P):
+    """Both kernels use programmatic dependent launch: the next step's selection may become resident
+    while this step's fused kernel drains.  Enqueue many steps with NO synchronisation in between
+    (shared kept[]/status buffers, fresh arrival times, rotating gradient sets) and compare the final
+    state with the oracle's free run: any early overwrite of kept[] or early read of theta would show."""
+    cfg = replace(synth.scaled(synth.PAPER_RMSPROP, P), N=12, b=4, M=5, name=f"b2b_{P}")
+    T, n_sets = 24, 3
+    pair = Pair(cfg)
+    sets = [[synth.gradient(cfg, r, k, DEV) for k in range(cfg.W)] for r in range(n_sets)]
+    tables = [psync.make_grad_table(s) for s in sets]
+    arrivals_h = [synth.arrival_times(cfg, s) for s in range(T)]
+    arrivals = torch.from_numpy(np.stack(arrivals_h)).to(DEV)
+    ps = pair.ps
+    steps = [psync.make_step(pair.shard_off, cfg.N, cfg.W, tb.grad_dtype, ps.theta, ps.ema, ps.state0, ps.state1,
+                             opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu,
+                             rho=cfg.rho, eps=cfg.eps, d_grads=tb.d_ptrs, d_kept=ps.d_kept, d_status=ps.d_status)
+             for tb in tables]
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    for s in range(T):
+        psync.psync_select_first_n(arrivals[s], cfg.N, cfg.b, ps.d_kept, ps.d_status, ps.d_t_nth, None, 0, stream)
+        psync.psync_aggregate_update(steps[s % n_sets][0], stream)
+    stream.synchronize()
+    for s in range(T):
+        st, _, _ = pair.oracle_step(sets[s % n_sets], arrivals_h[s])
+        assert st == 0
+    pair.compare(RTOL_FREE_100, ATOL_STEP, "back-to-back free run")
+    st, kept, tn = oracle.select_first_n(arrivals_h[T - 1], cfg.N, cfg.b)
+    assert np.array_equal(ps.d_kept.cpu().numpy(), kept) and float(ps.d_t_nth.item()) == tn

@@ -283,3 +283,44 @@ def test_argument_errors_return_einval_and_touch_nothing():
     torch.cuda.synchronize()
     assert np.array_equal(before, to_np(pair.ps.theta))
     assert psync.psync_ema(pair.ps.ema, pair.ps.theta, 0.9) == psync.PSYNC_OK
+
+
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+@pytest.mark.parametrize("P,pad", [(1, 4), (7, 8), (1021, 16), (4099, 64), (50_001, 8), (50_001, 3)])
+def test_guard_bands_no_out_of_bounds_access(dtype, P, pad):
+    """compute-sanitizer is closed on this GPU pool, so bounds are checked by hand: every array is a slice
+    of a larger allocation whose guard bands hold NaN (gradients: an out-of-bounds READ would poison the
+    result and fail parity) or a sentinel (theta/state/ema: an out-of-bounds WRITE would change it).
+    pad=3 makes every base pointer misaligned (scalar path); the others keep the 128-bit path."""
+    N, b = 6, 2
+    W = N + b
+    cfg = replace(BASE, P=P, N=N, b=b, M=1, grad_dtype=dtype, opt=synth.RMSPROP_MOM, name="guard")
+    tdt = torch.float32 if dtype == synth.F32 else torch.bfloat16
+    gen = torch.Generator(device=DEV)
+    gen.manual_seed(5)
+    SENT = 12345.0
+
+    def banded(fill, dt, draw_std):
+        raw = torch.full((P + 2 * pad,), fill, dtype=dt, device=DEV)
+        core = raw[pad:pad + P]
+        core.copy_(torch.empty(P, dtype=torch.float32, device=DEV).normal_(0, draw_std, generator=gen).to(dt))
+        return raw, core
+
+    grads_raw, grads = zip(*[banded(float("nan"), tdt, 1e-3) for _ in range(W)])
+    th_raw, th = banded(SENT, torch.float32, 0.02)
+    em_raw, em = banded(SENT, torch.float32, 0.02)
+    s0_raw, s0 = banded(SENT, torch.float32, 0.02)
+    s0.abs_()
+    s1_raw, s1 = banded(SENT, torch.float32, 1e-3)
+    pair = Pair(cfg, theta=th)
+    pair.ps.ema, pair.ps.state0, pair.ps.state1 = em, s0, s1
+    pair.sync_host_from_gpu()
+    arrival = synth.arrival_times(cfg, 0)
+    st, kept, _ = pair.gpu_step(list(grads), arrival)
+    st_o, kept_o, _ = pair.oracle_step(list(grads), arrival)
+    assert st == 0 and np.array_equal(kept, kept_o)
+    pair.compare(RTOL_STEP, ATOL_STEP, "guard bands")
+    for raw in (th_raw, em_raw, s0_raw, s1_raw):
+        assert bool((raw[:pad] == SENT).all()) and bool((raw[pad + P:] == SENT).all()), "write outside the array"
+    for raw in grads_raw:
+        assert bool(torch.isnan(raw[:pad].float()).all()) and bool(torch.isnan(raw[pad + P:].float()).all())
