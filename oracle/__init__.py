@@ -48,6 +48,14 @@ def lib() -> ctypes.CDLL:
         L.oracle_aggregate_update.argtypes = [i64, i32, vp, i32, i32, vp, ctypes.c_int, vp, vp, vp, vp, vp,
                                               ctypes.c_int, ctypes.c_int, f32, f32, f32, f32, f32]
         L.oracle_aggregate_update.restype = ctypes.c_int
+        L.oracle_select_first_n_sharded.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp]
+        L.oracle_select_first_n_sharded.restype = ctypes.c_int
+        L.oracle_select_timeout.argtypes = [vp, vp, i32, i32, f32, i32, vp, vp]
+        L.oracle_select_timeout.restype = ctypes.c_int
+        L.oracle_aggregate_update_rows.argtypes = [i64, i32, vp, i32, i32, vp, ctypes.c_int, ctypes.c_int, vp, i32,
+                                                   vp, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int,
+                                                   f32, f32, f32, f32, f32]
+        L.oracle_aggregate_update_rows.restype = ctypes.c_int
         L.oracle_accumulate.argtypes = [vp, vp, ctypes.c_int, i64]
         L.oracle_accumulate.restype = ctypes.c_int
         L.oracle_apply_sum.argtypes = [i64, i32, vp, i32, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int,
@@ -113,6 +121,65 @@ def aggregate_update(shard_off, N, grads, kept, theta, ema=None, state0=None, st
     return lib().oracle_aggregate_update(P, M, _ptr(shard_off), N, W, ctypes.cast(ptrs, ctypes.c_void_p),
                                          gd, _ptr(kept), _ptr(theta), _ptr(ema), _ptr(state0), _ptr(state1),
                                          opt, ema_mode, gamma_t, alpha, mu, rho, eps)
+
+
+def select_first_n_sharded(arrival, N, b, tags=None, t=0):
+    """Alg. 4 per parameter server j: arrival[M][W] -> (status[M], kept[M][N], t_nth[M]).
+    Rows of failed servers keep their fill values (kept -1, t_nth NaN)."""
+    W = N + b
+    if not (isinstance(arrival, np.ndarray) and arrival.ndim == 2 and arrival.shape[1] == W):
+        raise ValueError("arrival must be [M][N+b]")
+    M = arrival.shape[0]
+    _chk(arrival, np.float32, "arrival", M * W)
+    _chk(tags, np.int32, "tags", M * W)
+    kept = np.full((M, N), -1, dtype=np.int32)
+    t_nth = np.full(M, np.nan, dtype=np.float32)
+    status = np.full(M, EINVAL, dtype=np.int32)
+    rc = lib().oracle_select_first_n_sharded(_ptr(arrival), _ptr(tags), t, N, b, M, _ptr(kept), _ptr(t_nth),
+                                             _ptr(status))
+    if rc != OK:
+        raise ValueError("oracle_select_first_n_sharded: invalid arguments")
+    return status, kept, t_nth
+
+
+def select_timeout(arrival, timeout, min_keep=1, tags=None, t=0):
+    """Time-out rule (R19) -> (status, kept[int32 n_kept] or None)."""
+    W = arrival.size
+    _chk(arrival, np.float32, "arrival", W)
+    _chk(tags, np.int32, "tags", W)
+    kept = np.full(W, -1, dtype=np.int32)
+    n = np.zeros(1, dtype=np.int32)
+    st = lib().oracle_select_timeout(_ptr(arrival), _ptr(tags), t, W, timeout, min_keep, _ptr(kept), _ptr(n))
+    if st != OK:
+        return st, None
+    return st, kept[:int(n[0])].copy()
+
+
+def aggregate_update_rows(shard_off, N, grads, kept, theta, ema=None, state0=None, state1=None, per_shard=True,
+                          n_kept=None, status=None, opt=SGD, ema_mode=EMA_POST, gamma_t=0.0, alpha=0.0, mu=0.0,
+                          rho=0.0, eps=0.0):
+    """Alg. 4 l.8-9 with one kept row per server (per_shard) and/or a per-row count n_kept (time-out rule).
+    kept is int32 [rows][stride]; status int32 [rows] or None; rows = M if per_shard else 1."""
+    P = theta.size
+    shard_off = np.ascontiguousarray(shard_off, dtype=np.int64)
+    M = shard_off.size - 1
+    W = len(grads)
+    gd = _grad_dtype(grads)
+    for k, g in enumerate(grads):
+        _chk(g, grads[0].dtype, f"grads[{k}]", P)
+    rows = M if per_shard else 1
+    if not (isinstance(kept, np.ndarray) and kept.ndim == 2 and kept.shape[0] == rows):
+        raise ValueError("kept must be int32 [rows][stride]")
+    _chk(kept, np.int32, "kept")
+    _chk(n_kept, np.int32, "n_kept", rows)
+    _chk(status, np.int32, "status", rows)
+    for nm, a in (("theta", theta), ("ema", ema), ("state0", state0), ("state1", state1)):
+        _chk(a, np.float32, nm, P)
+    ptrs = (ctypes.c_void_p * W)(*[g.ctypes.data for g in grads])
+    return lib().oracle_aggregate_update_rows(P, M, _ptr(shard_off), N, W, ctypes.cast(ptrs, ctypes.c_void_p), gd,
+                                              1 if per_shard else 0, _ptr(kept), kept.shape[1], _ptr(n_kept),
+                                              _ptr(status), _ptr(theta), _ptr(ema), _ptr(state0), _ptr(state1),
+                                              opt, ema_mode, gamma_t, alpha, mu, rho, eps)
 
 
 def accumulate(S, grad):

@@ -254,6 +254,94 @@ int oracle_ema(float* ema, const float* theta, int64_t P, float alpha) {
   return ORACLE_OK;
 }
 
+// =============================================================================================
+// NEXT-1: Algorithm 4 run LITERALLY per parameter server j.  The listing is
+// titled "Sync-SGD Parameter Server j" (L134) and its wait loop (l.3-6, L148-158) runs on each
+// server separately, so server j keeps the first N gradients that reach *it*: arrival times are a
+// matrix arrival[M][W] (row j = the times at server j) and each server has its own kept set.
+//   arrival[M*W]  row-major; tags[M*W] or NULL; kept[M*N] row j = server j's kept workers ascending
+//   t_nth[M] or NULL; status[M]: ORACLE_OK or ORACLE_ETOOFEW per server (a failed server's kept
+//   row and t_nth entry are left untouched).  Returns ORACLE_EINVAL on bad arguments, else OK.
+// Each row is exactly oracle_select_first_n on that row.
+// =============================================================================================
+int oracle_select_first_n_sharded(const float* arrival, const int32_t* tags, int32_t t, int32_t N, int32_t b,
+                                  int32_t M, int32_t* kept, float* t_nth, int32_t* status) {
+  if (!arrival || !kept || !status || N < 1 || b < 0 || M < 1) return ORACLE_EINVAL;
+  const int64_t W = static_cast<int64_t>(N) + b;
+  for (int32_t j = 0; j < M; ++j)  // parameter server j waits for its own first N arrivals
+    status[j] = oracle_select_first_n(arrival + j * W, tags ? tags + j * W : nullptr, t, N, b,
+                                      kept + static_cast<int64_t>(j) * N, t_nth ? t_nth + j : nullptr);
+  return ORACLE_OK;
+}
+
+// =============================================================================================
+// NEXT-2: the time-out rule.  The paper only names it: "An alternative of
+// using time-outs instead of backup workers is also being explored" (section 6).  Reading
+// (R19): the server stops waiting at time `timeout`; every eligible worker (finite
+// arrival, tag == t) whose gradient arrived by then (arrival <= timeout, IEEE compare on fp32) is
+// kept, the rest are dropped; the update divides by the number actually kept, |G| (the mean of
+// the gradients in hand, as L160 divides by N = |G|).  Fewer than min_keep (>= 1) kept ->
+// ORACLE_ETOOFEW and nothing is written.
+//   kept[W] OUT: the first *n_kept entries are the kept workers ascending; the rest untouched.
+// =============================================================================================
+int oracle_select_timeout(const float* arrival, const int32_t* tags, int32_t t, int32_t W, float timeout,
+                          int32_t min_keep, int32_t* kept, int32_t* n_kept) {
+  if (!arrival || !kept || !n_kept || W < 1 || min_keep < 1 || std::isnan(timeout)) return ORACLE_EINVAL;
+  std::vector<int32_t> in_time;
+  for (int32_t k = 0; k < W; ++k) {
+    const bool eligible = std::isfinite(arrival[k]) && (tags == nullptr || tags[k] == t);
+    if (eligible && arrival[k] <= timeout) in_time.push_back(k);
+  }
+  if (static_cast<int32_t>(in_time.size()) < min_keep) return ORACLE_ETOOFEW;
+  for (size_t i = 0; i < in_time.size(); ++i) kept[i] = in_time[i];
+  *n_kept = static_cast<int32_t>(in_time.size());
+  return ORACLE_OK;
+}
+
+// =============================================================================================
+// Alg. 4 l.8-9 with one kept ROW per parameter server and a per-row count (NEXT-1, NEXT-2):
+//   row(j) = per_shard ? j : 0
+//   kept_j = kept[row * kept_stride .. + n_j),  n_j = n_kept ? n_kept[row] : N
+//   server j is skipped (theta[j], state[j], ema[j] untouched) when status && status[row] != OK
+//   theta(t+1)[j] = theta(t)[j] - (gamma_t / n_j) * sum_{k in kept_j} G_k[j]           (L160)
+// The divisor 1/n_j is formed in fp32 (reading R8), like 1/N.
+// =============================================================================================
+int oracle_aggregate_update_rows(int64_t P, int32_t M, const int64_t* shard_off, int32_t N, int32_t W,
+                                 const void* const* grads, int grad_dtype, int per_shard, const int32_t* kept,
+                                 int32_t kept_stride, const int32_t* n_kept, const int32_t* status, float* theta,
+                                 float* ema, float* state0, float* state1, int opt, int ema_mode, float gamma_t,
+                                 float alpha, float mu, float rho, float eps) {
+  if (!args_ok(P, M, shard_off, N, opt, ema_mode, theta, ema, state0, state1)) return ORACLE_EINVAL;
+  if (!grads || !kept || W < N || kept_stride < 1) return ORACLE_EINVAL;
+  if (grad_dtype != ORACLE_F32 && grad_dtype != ORACLE_BF16) return ORACLE_EINVAL;
+  for (int32_t j = 0; j < M; ++j) {  // validate every live row before anything is written
+    const int32_t row = per_shard ? j : 0;
+    if (status && status[row] != ORACLE_OK) continue;
+    const int32_t n_j = n_kept ? n_kept[row] : N;
+    if (n_j < 1 || n_j > kept_stride || n_j > W) return ORACLE_EINVAL;
+    const int32_t* kept_j = kept + static_cast<int64_t>(row) * kept_stride;
+    for (int32_t n = 0; n < n_j; ++n)
+      if (kept_j[n] < 0 || kept_j[n] >= W || !grads[kept_j[n]]) return ORACLE_EINVAL;
+  }
+  for (int32_t j = 0; j < M; ++j) {  // parameter server j owns theta[j]   (L42)
+    const int32_t row = per_shard ? j : 0;
+    if (status && status[row] != ORACLE_OK) continue;  // this server never collected its gradients
+    const int32_t n_j = n_kept ? n_kept[row] : N;
+    const int32_t* kept_j = kept + static_cast<int64_t>(row) * kept_stride;
+    const Coeffs c = make_coeffs(n_j, gamma_t, alpha, mu, rho, eps);
+    const int64_t lo = shard_off[j], hi = shard_off[j + 1];
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int64_t i = lo; i < hi; ++i) {
+      double S = 0.0;
+      for (int32_t n = 0; n < n_j; ++n) S += grad_at(grads[kept_j[n]], grad_dtype, i);
+      apply_element(S, c, opt, ema_mode, theta, ema, state0, state1, i);
+    }
+  }
+  return ORACLE_OK;
+}
+
 // Threads the element loops use (1 without OpenMP); bench.py reports it as cpu_baseline.cores.
 int oracle_num_threads(void) {
 #ifdef _OPENMP
