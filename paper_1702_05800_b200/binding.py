@@ -23,7 +23,8 @@ PSYNC_SGD, PSYNC_MOMENTUM, PSYNC_RMSPROP_MOM = 0, 1, 2
 PSYNC_EMA_POST, PSYNC_EMA_PRE, PSYNC_EMA_OFF = 0, 1, 2
 PSYNC_MAX_WORKERS = 1024
 
-EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_aggregate_update", "psync_ema",
+EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
+           "psync_select_timeout", "psync_aggregate_update", "psync_ema",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_launch_geometry", "psync_probe_read",
            "psync_probe_copy")
 
@@ -44,6 +45,8 @@ class psync_step(ctypes.Structure):
         ("d_state1", ctypes.c_void_p), ("opt", ctypes.c_int32), ("ema_mode", ctypes.c_int32),
         ("gamma_t", ctypes.c_float), ("alpha", ctypes.c_float), ("mu", ctypes.c_float), ("rho", ctypes.c_float),
         ("eps", ctypes.c_float), ("grid_ctas", ctypes.c_int32), ("variant", ctypes.c_int32),
+        ("per_shard", ctypes.c_int32), ("kept_stride", ctypes.c_int32), ("d_shard_off", ctypes.c_void_p),
+        ("d_n_kept", ctypes.c_void_p),
     ]
 
 
@@ -64,6 +67,10 @@ def lib() -> ctypes.CDLL:
         L.psync_status_string.restype = ctypes.c_char_p
         L.psync_select_first_n.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, vp]
         L.psync_select_first_n.restype = ctypes.c_int
+        L.psync_select_first_n_sharded.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp]
+        L.psync_select_first_n_sharded.restype = ctypes.c_int
+        L.psync_select_timeout.argtypes = [vp, vp, i32, i32, i32, f32, i32, vp, vp, vp, vp]
+        L.psync_select_timeout.restype = ctypes.c_int
         L.psync_aggregate_update.argtypes = [ctypes.POINTER(psync_step), vp]
         L.psync_aggregate_update.restype = ctypes.c_int
         L.psync_ema.argtypes = [vp, vp, i64, f32, vp]
@@ -126,6 +133,48 @@ def psync_select_first_n(d_arrival: torch.Tensor, N: int, b: int, d_kept: torch.
     return st
 
 
+def psync_select_first_n_sharded(d_arrival: torch.Tensor, N: int, b: int, M: int, d_kept: torch.Tensor,
+                                 d_status: torch.Tensor, d_t_nth: Optional[torch.Tensor] = None,
+                                 d_step_tag: Optional[torch.Tensor] = None, t: int = 0, stream=None,
+                                 check: bool = True) -> int:
+    """Alg. 4 per parameter server j (include/psync.h: psync_select_first_n_sharded):
+    d_arrival [M][N+b] -> d_kept [M][N], d_status [M], d_t_nth [M]."""
+    W = N + b
+    if d_arrival.numel() < M * W or d_kept.numel() < M * max(N, 0) or d_status.numel() < M:
+        raise ValueError("need d_arrival [M][N+b], d_kept [M][N], d_status [M]")
+    if d_step_tag is not None and d_step_tag.numel() < M * W:
+        raise ValueError("d_step_tag needs M*(N+b) elements")
+    if d_t_nth is not None and d_t_nth.numel() < M:
+        raise ValueError("d_t_nth needs M elements")
+    st = lib().psync_select_first_n_sharded(_dptr(d_arrival, torch.float32, "d_arrival"),
+                                            _dptr(d_step_tag, torch.int32, "d_step_tag"), t, N, b, M,
+                                            _dptr(d_kept, torch.int32, "d_kept"),
+                                            _dptr(d_t_nth, torch.float32, "d_t_nth"),
+                                            _dptr(d_status, torch.int32, "d_status"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_select_first_n_sharded")
+    return st
+
+
+def psync_select_timeout(d_arrival: torch.Tensor, W: int, timeout: float, d_kept: torch.Tensor,
+                         d_n_kept: torch.Tensor, d_status: torch.Tensor, rows: int = 1, min_keep: int = 1,
+                         d_step_tag: Optional[torch.Tensor] = None, t: int = 0, stream=None,
+                         check: bool = True) -> int:
+    """Time-out rule (include/psync.h: psync_select_timeout): d_arrival [rows][W] ->
+    d_kept [rows][W] (first d_n_kept[r] entries), d_n_kept [rows], d_status [rows]."""
+    if d_arrival.numel() < rows * W or d_kept.numel() < rows * W or d_n_kept.numel() < rows or d_status.numel() < rows:
+        raise ValueError("need d_arrival [rows][W], d_kept [rows][W], d_n_kept [rows], d_status [rows]")
+    if d_step_tag is not None and d_step_tag.numel() < rows * W:
+        raise ValueError("d_step_tag needs rows*W elements")
+    st = lib().psync_select_timeout(_dptr(d_arrival, torch.float32, "d_arrival"),
+                                    _dptr(d_step_tag, torch.int32, "d_step_tag"), t, W, rows, timeout, min_keep,
+                                    _dptr(d_kept, torch.int32, "d_kept"), _dptr(d_n_kept, torch.int32, "d_n_kept"),
+                                    _dptr(d_status, torch.int32, "d_status"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_select_timeout")
+    return st
+
+
 @dataclass
 class GradTable:
     """Device array of W device pointers (worker k -> its gradient buffer) + the tensors kept alive."""
@@ -154,7 +203,8 @@ def make_step(shard_off, N: int, W: int, grad_dtype: int, theta: torch.Tensor, e
               ema_mode: int = PSYNC_EMA_POST, gamma_t: float = 0.0, alpha: float = 0.0, mu: float = 0.0,
               rho: float = 0.0, eps: float = 0.0, d_grads: Optional[torch.Tensor] = None,
               d_kept: Optional[torch.Tensor] = None, d_status: Optional[torch.Tensor] = None, grid_ctas: int = 0,
-              variant: int = 0):
+              variant: int = 0, per_shard: bool = False, kept_stride: int = 0,
+              d_shard_off: Optional[torch.Tensor] = None, d_n_kept: Optional[torch.Tensor] = None):
     """Fills a psync_step.  Returns (struct, keepalive) -- hold on to both until the call returns."""
     off = np.ascontiguousarray(shard_off, dtype=np.int64)
     s = psync_step()
@@ -176,7 +226,17 @@ def make_step(shard_off, N: int, W: int, grad_dtype: int, theta: torch.Tensor, e
     s.opt, s.ema_mode = opt, ema_mode
     s.gamma_t, s.alpha, s.mu, s.rho, s.eps = gamma_t, alpha, mu, rho, eps
     s.grid_ctas, s.variant = grid_ctas, variant
-    return s, (off, d_grads, d_kept, d_status, theta, ema, state0, state1)
+    s.per_shard, s.kept_stride = int(per_shard), kept_stride
+    s.d_shard_off = _dptr(d_shard_off, torch.int64, "d_shard_off")
+    s.d_n_kept = _dptr(d_n_kept, torch.int32, "d_n_kept")
+    if d_shard_off is not None and d_shard_off.numel() != off.size:
+        raise ValueError("d_shard_off must have M+1 elements")
+    rows = s.M if per_shard else 1
+    stride = kept_stride if kept_stride > 0 else (W if d_n_kept is not None else N)
+    for nm, a, need in (("d_kept", d_kept, rows * stride), ("d_status", d_status, rows), ("d_n_kept", d_n_kept, rows)):
+        if a is not None and a.numel() < need:
+            raise ValueError(f"{nm} needs {need} elements")
+    return s, (off, d_grads, d_kept, d_status, theta, ema, state0, state1, d_shard_off, d_n_kept)
 
 
 def psync_aggregate_update(step: psync_step, stream=None, check: bool = True) -> int:

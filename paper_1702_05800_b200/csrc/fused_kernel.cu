@@ -62,9 +62,9 @@ __device__ __forceinline__ void st_state16(float* p, const float4& v) {
 
 // ---- the per-element update, Alg. 4 l.8-9 ----------------------------------------------------
 template <int OPT, int EMA>
-__device__ __forceinline__ void update_element(float S, float& th, float& em, float& s0, float& s1,
+__device__ __forceinline__ void update_element(float S, float inv_N, float& th, float& em, float& s0, float& s1,
                                                const FusedParams& p) {
-  const float G = S * p.inv_N;  // mean of the kept gradients (L160)
+  const float G = S * inv_N;  // mean of the kept gradients (L160)
   const float th_old = th;
   if (OPT == OPT_SGD) {
     th = th - p.gamma * G;  // L40, L160
@@ -102,30 +102,62 @@ __device__ __forceinline__ void accumulate_unit(float* acc, const uint4& r) {
 }
 
 // ---- scalar path: any alignment, any range; also the < 8-element tail of the vector path ------
+template <bool BF16>
+__device__ __forceinline__ float load_grad_scalar(const char* g, int64_t i) {
+  if (BF16)
+    return __uint_as_float(static_cast<uint32_t>(ldg_stream_u16(reinterpret_cast<const uint16_t*>(g) + i)) << 16);
+  return ldg_stream_f32(reinterpret_cast<const float*>(g) + i);
+}
+
+template <int OPT, int EMA>
+__device__ __forceinline__ void update_in_memory(const FusedParams& p, float S, float inv_N, int64_t i) {
+  float th = p.theta[i];
+  float em = (EMA != EMA_OFF) ? p.ema[i] : 0.f;
+  float s0 = (OPT != OPT_SGD) ? p.s0[i] : 0.f;
+  float s1 = (OPT == OPT_RMSPROP_MOM) ? p.s1[i] : 0.f;
+  update_element<OPT, EMA>(S, inv_N, th, em, s0, s1, p);
+  p.theta[i] = th;
+  if (EMA != EMA_OFF) p.ema[i] = em;
+  if (OPT != OPT_SGD) p.s0[i] = s0;
+  if (OPT == OPT_RMSPROP_MOM) p.s1[i] = s1;
+}
+
 template <bool BF16, int OPT, int EMA>
-__device__ void scalar_range(const FusedParams& p, const char* const* s_ptr, int64_t i0, int64_t i1, int64_t gtid,
-                             int64_t gthreads) {
+__device__ void scalar_range(const FusedParams& p, const char* const* s_ptr, int N, float inv_N, int64_t i0,
+                             int64_t i1, int64_t gtid, int64_t gthreads) {
   for (int64_t i = i0 + gtid; i < i1; i += gthreads) {
     float S = 0.f;
 #pragma unroll 4
-    for (int n = 0; n < p.N; ++n) {
-      float g;
-      if (BF16)
-        g = __uint_as_float(static_cast<uint32_t>(ldg_stream_u16(reinterpret_cast<const uint16_t*>(s_ptr[n]) + i))
-                            << 16);
-      else
-        g = ldg_stream_f32(reinterpret_cast<const float*>(s_ptr[n]) + i);
-      S += g;
-    }
-    float th = p.theta[i];
-    float em = (EMA != EMA_OFF) ? p.ema[i] : 0.f;
-    float s0 = (OPT != OPT_SGD) ? p.s0[i] : 0.f;
-    float s1 = (OPT == OPT_RMSPROP_MOM) ? p.s1[i] : 0.f;
-    update_element<OPT, EMA>(S, th, em, s0, s1, p);
-    p.theta[i] = th;
-    if (EMA != EMA_OFF) p.ema[i] = em;
-    if (OPT != OPT_SGD) p.s0[i] = s0;
-    if (OPT == OPT_RMSPROP_MOM) p.s1[i] = s1;
+    for (int n = 0; n < N; ++n) S += load_grad_scalar<BF16>(s_ptr[n], i);
+    update_in_memory<OPT, EMA>(p, S, inv_N, i);
+  }
+}
+
+// ---- per-server rows (Alg. 4 per parameter server j): which server owns element i ----------------
+// Smallest j with off[j+1] > i, i.e. off[j] <= i < off[j+1] (empty servers are skipped).  The table is
+// tiny and read by every CTA, so these loads hit L1/L2; all threads of a CTA search the same i.
+__device__ __forceinline__ int find_server(const int64_t* __restrict__ off, int M, int64_t i) {
+  int lo = 0, hi = M - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (__ldg(off + mid + 1) > i) hi = mid; else lo = mid + 1;
+  }
+  return lo;
+}
+
+// Elements [i0, i1) one at a time, each with its own server's kept row read from global memory: the slow,
+// always-correct path for tiles that straddle a server boundary, misaligned buffers and the tail.
+template <bool BF16, int OPT, int EMA>
+__device__ void rows_scalar_range(const FusedParams& p, int64_t i0, int64_t i1, int64_t tid, int64_t threads) {
+  for (int64_t i = i0 + tid; i < i1; i += threads) {
+    const int row = p.per_shard ? find_server(p.shard_off, p.M, i) : 0;
+    if (p.status != nullptr && p.status[row] != 0) continue;  // this server did not collect its gradients
+    const int N = p.n_kept ? p.n_kept[row] : p.N;
+    const float inv_N = p.n_kept ? 1.0f / static_cast<float>(N) : p.inv_N;
+    const int32_t* kept = p.kept + static_cast<int64_t>(row) * p.kept_stride;
+    float S = 0.f;
+    for (int n = 0; n < N; ++n) S += load_grad_scalar<BF16>(static_cast<const char*>(p.grads[kept[n]]), i);
+    update_in_memory<OPT, EMA>(p, S, inv_N, i);
   }
 }
 
@@ -133,10 +165,117 @@ __device__ void scalar_range(const FusedParams& p, const char* const* s_ptr, int
 // A "unit" is 16 bytes of one gradient buffer: E = 4 (fp32) or 8 (bf16) consecutive parameters.
 // A tile is THREADS x UPT units; slot j of thread tid is unit tile*THREADS*UPT + j*THREADS + tid, so
 // each warp-level load covers 512 contiguous bytes of one worker's buffer.
-template <int THREADS, int UPT, int U, int MINB, bool BF16, int OPT, int EMA>
-__global__ void __launch_bounds__(THREADS, MINB) fused_aggregate_update_ema(const FusedParams p) {
+//
+// One tile through the 128-bit path: sum the N buffers of s_ptr[] in ascending order, update, store.
+template <int THREADS, int UPT, int U, bool BF16, int OPT, int EMA>
+__device__ __forceinline__ void vector_tile(const FusedParams& p, const char* const* s_ptr, const int N,
+                                            const float inv_N, const int64_t tile, const int64_t n_units) {
   constexpr int E = BF16 ? 8 : 4;
   constexpr int Q = E / 4;  // float4 groups of theta per unit
+  constexpr int64_t TILE_UNITS = static_cast<int64_t>(THREADS) * UPT;
+  int64_t unit[UPT];
+  bool live[UPT];
+#pragma unroll
+  for (int j = 0; j < UPT; ++j) {
+    const int64_t u = tile * TILE_UNITS + static_cast<int64_t>(j) * THREADS + threadIdx.x;
+    live[j] = u < n_units;
+    unit[j] = live[j] ? u : (n_units - 1);  // dead slots re-read a valid unit and store nothing
+  }
+
+  float acc[UPT][E];
+#pragma unroll
+  for (int j = 0; j < UPT; ++j)
+#pragma unroll
+    for (int e = 0; e < E; ++e) acc[j][e] = 0.f;
+
+  int n = 0;
+  for (; n + U <= N; n += U) {  // full batches: U x UPT independent 16-byte loads in flight
+    uint4 r[U][UPT];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const char* g = s_ptr[n + u];
+#pragma unroll
+      for (int j = 0; j < UPT; ++j) r[u][j] = ldg_stream16(g + unit[j] * 16);
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u)  // strictly ascending worker order per element
+#pragma unroll
+      for (int j = 0; j < UPT; ++j) accumulate_unit<BF16>(acc[j], r[u][j]);
+  }
+  if (n < N) {  // last, partial batch: same shape, predicated
+    uint4 r[U][UPT];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const bool on = (n + u) < N;
+      const char* g = s_ptr[on ? (n + u) : (N - 1)];
+#pragma unroll
+      for (int j = 0; j < UPT; ++j) r[u][j] = on ? ldg_stream16(g + unit[j] * 16) : make_uint4(0u, 0u, 0u, 0u);
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+      if ((n + u) < N) {
+#pragma unroll
+        for (int j = 0; j < UPT; ++j) accumulate_unit<BF16>(acc[j], r[u][j]);
+      }
+  }
+
+  // theta / state / ema: loaded once the gradient registers are dead; other resident warps hide the latency
+  float4 th[UPT][Q], em[UPT][Q], a0[UPT][Q], a1[UPT][Q];
+#pragma unroll
+  for (int j = 0; j < UPT; ++j) {
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const int64_t e = unit[j] * E + 4 * q;
+      th[j][q] = ld_state16(p.theta + e);
+      if (EMA != EMA_OFF) em[j][q] = ld_state16(p.ema + e);
+      if (OPT != OPT_SGD) a0[j][q] = ld_state16(p.s0 + e);
+      if (OPT == OPT_RMSPROP_MOM) a1[j][q] = ld_state16(p.s1 + e);
+    }
+  }
+
+#pragma unroll
+  for (int j = 0; j < UPT; ++j) {
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      float* t4 = reinterpret_cast<float*>(&th[j][q]);
+      float* e4 = reinterpret_cast<float*>(&em[j][q]);
+      float* x4 = reinterpret_cast<float*>(&a0[j][q]);
+      float* y4 = reinterpret_cast<float*>(&a1[j][q]);
+#pragma unroll
+      for (int l = 0; l < 4; ++l) update_element<OPT, EMA>(acc[j][4 * q + l], inv_N, t4[l], e4[l], x4[l], y4[l], p);
+      if (live[j]) {
+        const int64_t e = unit[j] * E + 4 * q;
+        st_state16(p.theta + e, th[j][q]);
+        if (EMA != EMA_OFF) st_state16(p.ema + e, em[j][q]);
+        if (OPT != OPT_SGD) st_state16(p.s0 + e, a0[j][q]);
+        if (OPT == OPT_RMSPROP_MOM) st_state16(p.s1 + e, a1[j][q]);
+      }
+    }
+  }
+}
+
+// Stage kept row `row` as a table of N base pointers in shared memory; returns the OR of their low bits.
+template <int THREADS>
+__device__ __forceinline__ unsigned stage_row(const FusedParams& p, const char** s_ptr, int row, int N) {
+  const int32_t* kept = p.kept + static_cast<int64_t>(row) * p.kept_stride;
+  unsigned misalign = 0;
+  for (int n = threadIdx.x; n < N; n += THREADS) {
+    const char* g = static_cast<const char*>(p.grads[kept[n]]);
+    s_ptr[n] = g;
+    misalign |= static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 15u;
+  }
+  return misalign;
+}
+
+// ROWS = false: one kept row of exactly N workers for the whole parameter vector (reading R11).
+// ROWS = true : kept rows indexed on the device -- a device-side count (time-out rule, L259) and/or
+//               one kept row per parameter server j (Alg. 4 literally per server, L134-164): a tile that
+//               lies inside one server's slice stages that server's row and takes the same 128-bit path;
+//               the at most M-1 tiles that straddle a boundary go element by element.
+template <int THREADS, int UPT, int U, int MINB, bool BF16, int OPT, int EMA, bool ROWS>
+__global__ void __launch_bounds__(THREADS, MINB) fused_aggregate_update_ema(const FusedParams p) {
+  constexpr int E = BF16 ? 8 : 4;
+  constexpr int64_t TILE_UNITS = static_cast<int64_t>(THREADS) * UPT;
   __shared__ const char* s_ptr[kMaxWorkers];
 
   // Programmatic dependent launch: this CTA may be resident before the selection kernel (or the previous
@@ -145,113 +284,49 @@ __global__ void __launch_bounds__(THREADS, MINB) fused_aggregate_update_ema(cons
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
-  if (p.status != nullptr && *p.status != 0) return;  // selection failed: leave everything untouched
-
-  unsigned misalign = 0;
-  for (int n = threadIdx.x; n < p.N; n += THREADS) {
-    const char* g = static_cast<const char*>(p.grads[p.kept[n]]);
-    s_ptr[n] = g;
-    misalign |= static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 15u;
-  }
-  const bool vec_ok = (__syncthreads_or(static_cast<int>(misalign)) == 0) && (p.base_aligned != 0);
-
-  const int64_t gtid = static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x;
-  const int64_t gthreads = static_cast<int64_t>(gridDim.x) * THREADS;
-  if (!vec_ok) {
-    scalar_range<BF16, OPT, EMA>(p, s_ptr, 0, p.P, gtid, gthreads);
-    return;
-  }
-
   const int64_t n_units = p.P / E;
-  constexpr int64_t TILE_UNITS = static_cast<int64_t>(THREADS) * UPT;
   const int64_t n_tiles = (n_units + TILE_UNITS - 1) / TILE_UNITS;
-  const int N = p.N;
+  const int64_t tail0 = n_units * E;  // fewer than E trailing parameters
 
-  for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-    int64_t unit[UPT];
-    bool live[UPT];
-#pragma unroll
-    for (int j = 0; j < UPT; ++j) {
-      const int64_t u = tile * TILE_UNITS + static_cast<int64_t>(j) * THREADS + threadIdx.x;
-      live[j] = u < n_units;
-      unit[j] = live[j] ? u : (n_units - 1);  // dead slots re-read a valid unit and store nothing
+  if (!ROWS) {
+    if (p.status != nullptr && *p.status != 0) return;  // selection failed: leave everything untouched
+    const int N = p.N;  // both straight from the constant bank (a variable count takes the ROWS kernel)
+    const float inv_N = p.inv_N;
+    const unsigned misalign = stage_row<THREADS>(p, s_ptr, 0, N);
+    const bool vec_ok = (__syncthreads_or(static_cast<int>(misalign)) == 0) && (p.base_aligned != 0);
+    if (!vec_ok) {
+      scalar_range<BF16, OPT, EMA>(p, s_ptr, N, inv_N, 0, p.P, static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x,
+                                   static_cast<int64_t>(gridDim.x) * THREADS);
+      return;
     }
-
-    float acc[UPT][E];
-#pragma unroll
-    for (int j = 0; j < UPT; ++j)
-#pragma unroll
-      for (int e = 0; e < E; ++e) acc[j][e] = 0.f;
-
-    int n = 0;
-    for (; n + U <= N; n += U) {  // full batches: U x UPT independent 16-byte loads in flight
-      uint4 r[U][UPT];
-#pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const char* g = s_ptr[n + u];
-#pragma unroll
-        for (int j = 0; j < UPT; ++j) r[u][j] = ldg_stream16(g + unit[j] * 16);
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x)
+      vector_tile<THREADS, UPT, U, BF16, OPT, EMA>(p, s_ptr, N, inv_N, tile, n_units);
+    if (tail0 < p.P && blockIdx.x == 0) scalar_range<BF16, OPT, EMA>(p, s_ptr, N, inv_N, tail0, p.P, threadIdx.x, THREADS);
+  } else {
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      const int64_t e0 = tile * TILE_UNITS * E;
+      const int64_t e1 = (e0 + TILE_UNITS * E < tail0) ? e0 + TILE_UNITS * E : tail0;  // tile = elements [e0, e1)
+      // per_shard == 0 here means one row with a device-side count (time-out rule, L259): no lookup
+      const int row = p.per_shard ? find_server(p.shard_off, p.M, e0) : 0;
+      const bool one_server = p.per_shard ? (__ldg(p.shard_off + row + 1) >= e1) : true;  // CTA-uniform
+      bool fast = one_server && p.base_aligned != 0;
+      if (one_server && p.status != nullptr && p.status[row] != 0) continue;  // that server failed: skip its tile
+      __syncthreads();  // the previous tile's readers are done with s_ptr
+      int N = 0;
+      float inv_N = 0.f;
+      if (fast) {
+        N = p.n_kept ? p.n_kept[row] : p.N;
+        inv_N = p.n_kept ? 1.0f / static_cast<float>(N) : p.inv_N;
+        const unsigned misalign = stage_row<THREADS>(p, s_ptr, row, N);
+        fast = __syncthreads_or(static_cast<int>(misalign)) == 0;
       }
-#pragma unroll
-      for (int u = 0; u < U; ++u)  // strictly ascending worker order per element
-#pragma unroll
-        for (int j = 0; j < UPT; ++j) accumulate_unit<BF16>(acc[j], r[u][j]);
+      if (fast)
+        vector_tile<THREADS, UPT, U, BF16, OPT, EMA>(p, s_ptr, N, inv_N, tile, n_units);
+      else
+        rows_scalar_range<BF16, OPT, EMA>(p, e0, e1, threadIdx.x, THREADS);
     }
-    if (n < N) {  // last, partial batch: same shape, predicated
-      uint4 r[U][UPT];
-#pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const bool on = (n + u) < N;
-        const char* g = s_ptr[on ? (n + u) : (N - 1)];
-#pragma unroll
-        for (int j = 0; j < UPT; ++j) r[u][j] = on ? ldg_stream16(g + unit[j] * 16) : make_uint4(0u, 0u, 0u, 0u);
-      }
-#pragma unroll
-      for (int u = 0; u < U; ++u)
-        if ((n + u) < N) {
-#pragma unroll
-          for (int j = 0; j < UPT; ++j) accumulate_unit<BF16>(acc[j], r[u][j]);
-        }
-    }
-
-    // theta / state / ema: loaded once the gradient registers are dead; other resident warps hide the latency
-    float4 th[UPT][Q], em[UPT][Q], a0[UPT][Q], a1[UPT][Q];
-#pragma unroll
-    for (int j = 0; j < UPT; ++j) {
-#pragma unroll
-      for (int q = 0; q < Q; ++q) {
-        const int64_t e = unit[j] * E + 4 * q;
-        th[j][q] = ld_state16(p.theta + e);
-        if (EMA != EMA_OFF) em[j][q] = ld_state16(p.ema + e);
-        if (OPT != OPT_SGD) a0[j][q] = ld_state16(p.s0 + e);
-        if (OPT == OPT_RMSPROP_MOM) a1[j][q] = ld_state16(p.s1 + e);
-      }
-    }
-
-#pragma unroll
-    for (int j = 0; j < UPT; ++j) {
-#pragma unroll
-      for (int q = 0; q < Q; ++q) {
-        float* t4 = reinterpret_cast<float*>(&th[j][q]);
-        float* e4 = reinterpret_cast<float*>(&em[j][q]);
-        float* x4 = reinterpret_cast<float*>(&a0[j][q]);
-        float* y4 = reinterpret_cast<float*>(&a1[j][q]);
-#pragma unroll
-        for (int l = 0; l < 4; ++l) update_element<OPT, EMA>(acc[j][4 * q + l], t4[l], e4[l], x4[l], y4[l], p);
-        if (live[j]) {
-          const int64_t e = unit[j] * E + 4 * q;
-          st_state16(p.theta + e, th[j][q]);
-          if (EMA != EMA_OFF) st_state16(p.ema + e, em[j][q]);
-          if (OPT != OPT_SGD) st_state16(p.s0 + e, a0[j][q]);
-          if (OPT == OPT_RMSPROP_MOM) st_state16(p.s1 + e, a1[j][q]);
-        }
-      }
-    }
+    if (tail0 < p.P && blockIdx.x == 0) rows_scalar_range<BF16, OPT, EMA>(p, tail0, p.P, threadIdx.x, THREADS);
   }
-
-  // fewer than E trailing parameters
-  const int64_t tail0 = n_units * E;
-  if (tail0 < p.P && blockIdx.x == 0) scalar_range<BF16, OPT, EMA>(p, s_ptr, tail0, p.P, threadIdx.x, THREADS);
 }
 
 // ---- K3 ---------------------------------------------------------------------------------------
@@ -289,10 +364,31 @@ constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
 using KernelFn = void (*)(const FusedParams);
 
-template <int V, bool BF16, int OPT, int EMA>
+template <int V, bool BF16, int OPT, int EMA, bool ROWS = false>
 constexpr KernelFn kernel_for() {
   return fused_aggregate_update_ema<kVariants[V].threads, kVariants[V].upt, kVariants[V].unroll, kVariants[V].minb,
-                                    BF16, OPT, EMA>;
+                                    BF16, OPT, EMA, ROWS>;
+}
+
+// per-server rows: the default variant only (a forced variant > 1 is PSYNC_EUNSUPPORTED in the ABI)
+template <bool BF16, int OPT>
+KernelFn pick_rows_ema(int ema) {
+  switch (ema) {
+    case EMA_POST: return kernel_for<0, BF16, OPT, EMA_POST, true>();
+    case EMA_PRE: return kernel_for<0, BF16, OPT, EMA_PRE, true>();
+    default: return kernel_for<0, BF16, OPT, EMA_OFF, true>();
+  }
+}
+template <bool BF16>
+KernelFn pick_rows_opt(int opt, int ema) {
+  switch (opt) {
+    case OPT_SGD: return pick_rows_ema<BF16, OPT_SGD>(ema);
+    case OPT_MOMENTUM: return pick_rows_ema<BF16, OPT_MOMENTUM>(ema);
+    default: return pick_rows_ema<BF16, OPT_RMSPROP_MOM>(ema);
+  }
+}
+KernelFn pick_rows_kernel(int dtype, int opt, int ema) {
+  return dtype == 1 ? pick_rows_opt<true>(opt, ema) : pick_rows_opt<false>(opt, ema);
 }
 
 template <int V, bool BF16, int OPT>
@@ -381,7 +477,7 @@ cudaError_t launch_fused(const FusedParams& p, int dtype, int opt, int ema, int 
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, pick_kernel(v, dtype, opt, ema), p);
+  return cudaLaunchKernelEx(&cfg, (p.per_shard || p.n_kept != nullptr) ? pick_rows_kernel(dtype, opt, ema) : pick_kernel(v, dtype, opt, ema), p);
 }
 
 cudaError_t launch_ema(float* d_ema, const float* d_theta, int64_t P, float alpha, cudaStream_t stream) {

@@ -32,6 +32,11 @@ int check_step(const psync_step* s, bool need_device_tables) {
   }
   if (need_device_tables && (s->d_grads == nullptr || s->d_kept == nullptr)) return PSYNC_EINVAL;
   if (s->grid_ctas < 0 || s->variant < 0 || s->variant > psync::fused_num_variants()) return PSYNC_EINVAL;
+  if (s->per_shard != 0 && s->per_shard != 1) return PSYNC_EINVAL;
+  if (s->kept_stride < 0 || (s->kept_stride != 0 && s->kept_stride < s->N && s->d_n_kept == nullptr)) return PSYNC_EINVAL;
+  if (s->kept_stride > PSYNC_MAX_WORKERS) return PSYNC_EINVAL;
+  if (need_device_tables && s->per_shard && s->d_shard_off == nullptr) return PSYNC_EINVAL;
+  if ((s->per_shard || s->d_n_kept != nullptr) && s->variant > 1) return PSYNC_EUNSUPPORTED;  // rows kernel: default variant only
   return PSYNC_OK;
 }
 
@@ -56,6 +61,11 @@ FusedParams make_params(const psync_step* s, int64_t first, int64_t count, const
   p.one_minus_rho = 1.0f - s->rho;
   p.eps = s->eps;
   p.inv_N = 1.0f / static_cast<float>(s->N);
+  p.per_shard = s->per_shard;
+  p.kept_stride = s->kept_stride > 0 ? s->kept_stride : (s->d_n_kept != nullptr ? s->W : s->N);
+  p.M = s->M;
+  p.shard_off = s->d_shard_off;
+  p.n_kept = s->d_n_kept;
   p.base_aligned = aligned16(p.theta) && (p.ema == nullptr || aligned16(p.ema)) && (p.s0 == nullptr || aligned16(p.s0)) &&
                    (p.s1 == nullptr || aligned16(p.s1));
   return p;
@@ -124,8 +134,28 @@ PSYNC_API int psync_select_first_n(const float* d_arrival, const int32_t* d_step
                          int32_t* d_kept, float* d_t_nth, int32_t* d_status, void* stream) {
   if (d_arrival == nullptr || d_kept == nullptr || d_status == nullptr) return PSYNC_EINVAL;
   if (N < 1 || b < 0 || static_cast<int64_t>(N) + b > PSYNC_MAX_WORKERS) return PSYNC_EINVAL;
-  const cudaError_t err = psync::launch_select_first_n(d_arrival, d_step_tag, t, N, N + b, d_kept, d_t_nth, d_status,
+  const cudaError_t err = psync::launch_select_first_n(d_arrival, d_step_tag, t, N, N + b, 1, d_kept, d_t_nth, d_status,
                                                        static_cast<cudaStream_t>(stream));
+  return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
+}
+
+PSYNC_API int psync_select_first_n_sharded(const float* d_arrival, const int32_t* d_step_tag, int32_t t, int32_t N,
+                                 int32_t b, int32_t M, int32_t* d_kept, float* d_t_nth, int32_t* d_status,
+                                 void* stream) {
+  if (d_arrival == nullptr || d_kept == nullptr || d_status == nullptr) return PSYNC_EINVAL;
+  if (N < 1 || b < 0 || M < 1 || static_cast<int64_t>(N) + b > PSYNC_MAX_WORKERS) return PSYNC_EINVAL;
+  const cudaError_t err = psync::launch_select_first_n(d_arrival, d_step_tag, t, N, N + b, M, d_kept, d_t_nth, d_status,
+                                                       static_cast<cudaStream_t>(stream));
+  return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
+}
+
+PSYNC_API int psync_select_timeout(const float* d_arrival, const int32_t* d_step_tag, int32_t t, int32_t W,
+                         int32_t rows, float timeout, int32_t min_keep, int32_t* d_kept, int32_t* d_n_kept,
+                         int32_t* d_status, void* stream) {
+  if (d_arrival == nullptr || d_kept == nullptr || d_n_kept == nullptr || d_status == nullptr) return PSYNC_EINVAL;
+  if (W < 1 || W > PSYNC_MAX_WORKERS || rows < 1 || min_keep < 1 || timeout != timeout) return PSYNC_EINVAL;
+  const cudaError_t err = psync::launch_select_timeout(d_arrival, d_step_tag, t, W, rows, timeout, min_keep, d_kept,
+                                                       d_n_kept, d_status, static_cast<cudaStream_t>(stream));
   return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
 }
 
@@ -185,6 +215,7 @@ PSYNC_API int psync_step_host(const psync_step* st, const float* h_arrival, cons
   const int chk = check_step(st, false);
   if (chk != PSYNC_OK) return chk;
   if (h_arrival == nullptr || h_grads == nullptr || d_work == nullptr) return PSYNC_EINVAL;
+  if (st->per_shard != 0 || st->d_n_kept != nullptr) return PSYNC_EUNSUPPORTED;
   HostLayout L;
   if (!host_layout(st->N, st->W, st->grad_dtype, chunk_elems, &L)) return PSYNC_EINVAL;
   if (work_bytes < L.total || (reinterpret_cast<uintptr_t>(d_work) & 255u) != 0) return PSYNC_EINVAL;
@@ -221,7 +252,7 @@ PSYNC_API int psync_step_host(const psync_step* st, const float* h_arrival, cons
   PSYNC_CU(cudaMemcpyAsync(d_arrival, h_arrival, sizeof(float) * W, cudaMemcpyHostToDevice, s));
   if (h_step_tag != nullptr)
     PSYNC_CU(cudaMemcpyAsync(d_tags, h_step_tag, sizeof(int32_t) * W, cudaMemcpyHostToDevice, s));
-  PSYNC_CU(psync::launch_select_first_n(d_arrival, h_step_tag ? d_tags : nullptr, t, N, W, d_kept, d_tnth, d_status, s));
+  PSYNC_CU(psync::launch_select_first_n(d_arrival, h_step_tag ? d_tags : nullptr, t, N, W, 1, d_kept, d_tnth, d_status, s));
   PSYNC_CU(cudaMemcpyAsync(&status, d_status, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
   PSYNC_CU(cudaStreamSynchronize(s));
   if (status != PSYNC_OK) {

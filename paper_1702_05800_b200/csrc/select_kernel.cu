@@ -68,6 +68,14 @@ __global__ void __launch_bounds__(32) select_first_n_kernel(const float* __restr
   pdl_release_successor();    // the fused kernel behind us may get resident; it waits before reading kept[]
   pdl_wait_for_predecessor();
 
+  // one CTA (one warp) per row: row j = parameter server j's own arrival times (Alg. 4 per server, L134)
+  const int64_t row = blockIdx.x;
+  arrival += row * W;
+  if (tags != nullptr) tags += row * W;
+  kept += row * N;
+  if (t_nth != nullptr) t_nth += row;
+  status += row;
+
   uint32_t key[C];
   int n_elig = 0;
 #pragma unroll
@@ -150,10 +158,72 @@ __global__ void __launch_bounds__(32) select_first_n_kernel(const float* __restr
   }
 }
 
+// K1b: the time-out rule (reading R19).  Worker k is kept iff it is eligible
+// (finite arrival, tag == t) and arrival[k] <= timeout; kept[] comes out ascending because lanes own
+// contiguous index ranges; n_kept < min_keep -> ETOOFEW and nothing else is written.
+__global__ void __launch_bounds__(32) select_timeout_kernel(const float* __restrict__ arrival,
+                                                            const int32_t* __restrict__ tags, int32_t t, int32_t W,
+                                                            float timeout, int32_t min_keep,
+                                                            int32_t* __restrict__ kept, int32_t* __restrict__ n_kept,
+                                                            int32_t* __restrict__ status) {
+  const int lane = threadIdx.x;
+  pdl_release_successor();
+  pdl_wait_for_predecessor();
+  const int64_t row = blockIdx.x;
+  arrival += row * W;
+  if (tags != nullptr) tags += row * W;
+  kept += row * W;
+  const int C = (W + 31) / 32;  // workers per lane
+  const int base = lane * C;
+  int mine = 0;
+  for (int i = 0; i < C; ++i) {
+    const int k = base + i;
+    if (k < W) {
+      const float a = arrival[k];
+      const bool finite = (__float_as_uint(a) & 0x7F800000u) != 0x7F800000u;
+      mine += (finite && a <= timeout && (tags == nullptr || tags[k] == t)) ? 1 : 0;
+    }
+  }
+  int total;
+  int out = warp_exclusive_scan(mine, lane, &total);
+  if (total < min_keep) {
+    if (lane == 0) status[row] = kStatusTooFew;
+    return;
+  }
+  for (int i = 0; i < C; ++i) {
+    const int k = base + i;
+    if (k < W) {
+      const float a = arrival[k];
+      const bool finite = (__float_as_uint(a) & 0x7F800000u) != 0x7F800000u;
+      if (finite && a <= timeout && (tags == nullptr || tags[k] == t)) kept[out++] = k;
+    }
+  }
+  if (lane == 0) {
+    n_kept[row] = total;
+    status[row] = kStatusOk;
+  }
+}
+
+}  // namespace
+
+namespace {
+cudaLaunchConfig_t one_warp_per_row(int32_t rows, cudaStream_t stream, cudaLaunchAttribute* attr) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(static_cast<unsigned>(rows));
+  cfg.blockDim = dim3(32);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = stream;
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cfg;
+}
 }  // namespace
 
 cudaError_t launch_select_first_n(const float* d_arrival, const int32_t* d_tags, int32_t t, int32_t N, int32_t W,
-                                  int32_t* d_kept, float* d_t_nth, int32_t* d_status, cudaStream_t stream) {
+                                  int32_t rows, int32_t* d_kept, float* d_t_nth, int32_t* d_status,
+                                  cudaStream_t stream) {
   using Kernel = void (*)(const float*, const int32_t*, int32_t, int32_t, int32_t, int32_t*, float*, int32_t*);
   Kernel kernel = select_first_n_kernel<32>;
   if (W <= 32) kernel = select_first_n_kernel<1>;
@@ -161,17 +231,18 @@ cudaError_t launch_select_first_n(const float* d_arrival, const int32_t* d_tags,
   else if (W <= 128) kernel = select_first_n_kernel<4>;
   else if (W <= 256) kernel = select_first_n_kernel<8>;
   else if (W <= 512) kernel = select_first_n_kernel<16>;
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(1);
-  cfg.blockDim = dim3(32);
-  cfg.dynamicSmemBytes = 0;
-  cfg.stream = stream;
   cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr;
-  cfg.numAttrs = 1;
+  const cudaLaunchConfig_t cfg = one_warp_per_row(rows, stream, attr);
   return cudaLaunchKernelEx(&cfg, kernel, d_arrival, d_tags, t, N, W, d_kept, d_t_nth, d_status);
+}
+
+cudaError_t launch_select_timeout(const float* d_arrival, const int32_t* d_tags, int32_t t, int32_t W, int32_t rows,
+                                  float timeout, int32_t min_keep, int32_t* d_kept, int32_t* d_n_kept,
+                                  int32_t* d_status, cudaStream_t stream) {
+  cudaLaunchAttribute attr[1];
+  const cudaLaunchConfig_t cfg = one_warp_per_row(rows, stream, attr);
+  return cudaLaunchKernelEx(&cfg, select_timeout_kernel, d_arrival, d_tags, t, W, timeout, min_keep, d_kept,
+                            d_n_kept, d_status);
 }
 
 }  // namespace psync

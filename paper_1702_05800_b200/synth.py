@@ -194,6 +194,16 @@ def arrival_times(cfg: Config, step: int) -> np.ndarray:
     return t.astype(np.float32)
 
 
+def arrival_times_per_server(cfg: Config, step: int, server_sigma: float = 0.05) -> np.ndarray:
+    """fp32 [M][W]: the time worker k's gradient slice reaches parameter server j (Alg. 4 runs per server,
+    PAPER.md:L134).  Recipe: the worker's own time (arrival_times) times an independent per-(server, worker)
+    network jitter exp(server_sigma z_jk); computed in double, rounded once to fp32."""
+    base = arrival_times(cfg, step).astype(np.float64)
+    rng = np.random.default_rng(seed_for(cfg, step, STREAM_ARRIVAL) + 5)
+    z = rng.standard_normal((cfg.M, cfg.W))
+    return (base[None, :] * np.exp(server_sigma * z)).astype(np.float32)
+
+
 def as_numpy_grad(g: torch.Tensor) -> np.ndarray:
     """Host view for the oracle: float32 array, or uint16 bit patterns for bf16."""
     g = g.detach().cpu().contiguous()

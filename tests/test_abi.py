@@ -41,7 +41,7 @@ def test_every_declared_symbol_is_exported(B):
 
 
 def test_version_and_status_strings(B):
-    assert B.psync_version() == 100
+    assert B.psync_version() >= 110
     assert "ETOOFEW" in B.status_string(B.PSYNC_ETOOFEW) and "EINVAL" in B.status_string(B.PSYNC_EINVAL)
 
 
@@ -86,6 +86,25 @@ def test_einval_without_a_device(B):
         mutate()
         assert L.psync_aggregate_update(ctypes.byref(s), None) == B.PSYNC_EINVAL
         ctypes.memmove(ctypes.byref(s), saved, len(saved))
+    for mutate in (lambda: setattr(s, "per_shard", 2), lambda: setattr(s, "per_shard", 1),   # per_shard without d_shard_off
+                   lambda: setattr(s, "kept_stride", -1), lambda: setattr(s, "kept_stride", 1),  # stride < N, fixed count
+                   lambda: setattr(s, "kept_stride", 1025)):
+        saved = bytes(s)
+        mutate()
+        assert L.psync_aggregate_update(ctypes.byref(s), None) == B.PSYNC_EINVAL
+        ctypes.memmove(ctypes.byref(s), saved, len(saved))
+    s.per_shard, s.d_shard_off, s.variant = 1, 1024, 2
+    assert L.psync_aggregate_update(ctypes.byref(s), None) == B.PSYNC_EUNSUPPORTED
+    s.per_shard, s.d_shard_off, s.variant = 0, None, 0
+    assert L.psync_select_first_n_sharded(None, None, 0, 1, 0, 1, None, None, None, None) == B.PSYNC_EINVAL
+    assert L.psync_select_first_n_sharded(8, None, 0, 1, 0, 0, 8, None, 8, None) == B.PSYNC_EINVAL
+    assert L.psync_select_first_n_sharded(8, None, 0, 1000, 25, 2, 8, None, 8, None) == B.PSYNC_EINVAL
+    assert L.psync_select_timeout(None, None, 0, 4, 1, 1.0, 1, None, None, None, None) == B.PSYNC_EINVAL
+    assert L.psync_select_timeout(8, None, 0, 0, 1, 1.0, 1, 8, 8, 8, None) == B.PSYNC_EINVAL
+    assert L.psync_select_timeout(8, None, 0, 1025, 1, 1.0, 1, 8, 8, 8, None) == B.PSYNC_EINVAL
+    assert L.psync_select_timeout(8, None, 0, 4, 0, 1.0, 1, 8, 8, 8, None) == B.PSYNC_EINVAL
+    assert L.psync_select_timeout(8, None, 0, 4, 1, 1.0, 0, 8, 8, 8, None) == B.PSYNC_EINVAL
+    assert L.psync_select_timeout(8, None, 0, 4, 1, float("nan"), 1, 8, 8, 8, None) == B.PSYNC_EINVAL
     assert B.psync_step_host_workspace_bytes(0, 3, 0, 0) == 0
     assert B.psync_step_host_workspace_bytes(2, 3, 0, 100) == 0
     n = B.psync_step_host_workspace_bytes(100, 106, 0, 1 << 20)
