@@ -236,24 +236,47 @@ def run_psync(args, cfg, rank, world, dist):
     ps = psync.ParameterServerStep(off, cfg.N, cfg.b, theta, ema, s0, s1, cfg.opt, cfg.ema_mode, alpha=cfg.alpha,
                                    mu=cfg.mu, rho=cfg.rho, eps=cfg.eps, grid_ctas=args.grid_ctas, variant=args.variant)
 
-    arrivals = torch.from_numpy(np.stack([synth.arrival_times(cfg, s) for s in range(K + Wm)])).to(dev)
+    # --mode first_n (default, the headline): one kept set of N per step (reading R11).
+    # --mode per_server: Alg. 4 per server j, arrival [M][W] -> kept [M][N] (NEXT-1).
+    # --mode timeout: keep every worker that arrived by --timeout seconds, divide by the count (NEXT-2).
+    mode = args.mode
+    rows = cfg.M if mode == "per_server" else 1
+    if mode == "per_server":
+        arr_np = np.stack([synth.arrival_times_per_server(cfg, s) for s in range(K + Wm)])
+    else:
+        arr_np = np.stack([synth.arrival_times(cfg, s) for s in range(K + Wm)])
+    arrivals = torch.from_numpy(arr_np).to(dev)
+    stride = cfg.W if mode == "timeout" else cfg.N
+    d_kept = torch.full((rows, stride), -1, dtype=torch.int32, device=dev) if mode != "first_n" else ps.d_kept
+    d_status = torch.full((rows,), -9, dtype=torch.int32, device=dev) if mode != "first_n" else ps.d_status
+    d_n_kept = torch.zeros(rows, dtype=torch.int32, device=dev) if mode == "timeout" else None
+    d_off = torch.from_numpy(off).to(dev) if mode == "per_server" else None
     steps_struct = []
     for tb in tables:   # one psync_step per gradient set, built once (marshalling outside the timed region)
         st, keep = psync.make_step(off, cfg.N, cfg.W, tb.grad_dtype, theta, ema, s0, s1, opt=cfg.opt,
                                    ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho,
-                                   eps=cfg.eps, d_grads=tb.d_ptrs, d_kept=ps.d_kept, d_status=ps.d_status,
-                                   grid_ctas=args.grid_ctas, variant=args.variant)
+                                   eps=cfg.eps, d_grads=tb.d_ptrs, d_kept=d_kept, d_status=d_status,
+                                   grid_ctas=args.grid_ctas, variant=args.variant, per_shard=(mode == "per_server"),
+                                   d_shard_off=d_off, d_n_kept=d_n_kept)
         steps_struct.append((st, keep))
     geo = psync.psync_launch_geometry(steps_struct[0][0])
 
     stream = torch.cuda.Stream(device=dev)
     B = psync.binding
 
+    def select(i):
+        if mode == "first_n":
+            B.psync_select_first_n(arrivals[i], cfg.N, cfg.b, ps.d_kept, ps.d_status, ps.d_t_nth, None, i, stream)
+        elif mode == "per_server":
+            B.psync_select_first_n_sharded(arrivals[i], cfg.N, cfg.b, cfg.M, d_kept, d_status, None, None, i, stream)
+        else:
+            B.psync_select_timeout(arrivals[i], cfg.W, args.timeout, d_kept, d_n_kept, d_status, stream=stream)
+
     def one_step(i, ev=None):
         st = steps_struct[i % n_sets][0]
         if ev is not None:
             ev[0].record(stream)
-        B.psync_select_first_n(arrivals[i], cfg.N, cfg.b, ps.d_kept, ps.d_status, ps.d_t_nth, None, i, stream)
+        select(i)
         if ev is not None:
             ev[1].record(stream)
         B.psync_aggregate_update(st, stream)
@@ -267,7 +290,7 @@ def run_psync(args, cfg, rank, world, dist):
     for i in range(Wm):
         one_step(i)
     torch.cuda.synchronize()
-    assert int(ps.d_status.item()) == 0
+    assert bool((d_status == 0).all())
 
     # Per-kernel CUDA events are recorded on every `probe_every`-th timed step only: an event between
     # the two launches breaks their programmatic-dependent-launch pairing and costs ~10 us, so the
@@ -292,13 +315,19 @@ def run_psync(args, cfg, rank, world, dist):
     select_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs.values()]))
     if os.environ.get("PSYNC_BENCH_DEBUG"):
         print("fused ms per probed step:", [round(x, 4) for x in fused_list], file=sys.stderr)
-    assert int(ps.d_status.item()) == 0 and bool(torch.isfinite(theta[:4096]).all())
+    assert bool((d_status == 0).all()) and bool(torch.isfinite(theta[:4096]).all())
 
-    units_local = float(cfg.N) * cfg.P * K
+    # gradient elements aggregated per step: N*P, or (workers in time)*P for the time-out rule
+    if mode == "timeout":
+        n_eff = float(np.mean([(arr_np[Wm + k] <= args.timeout).sum() for k in range(K)]))
+    else:
+        n_eff = float(cfg.N)
+    bytes_per_step = cfg.bytes_per_step + (n_eff - cfg.N) * cfg.P * cfg.grad_bytes
+    units_local = n_eff * cfg.P * K
     units, max_ms = aggregate_over_ranks(units_local, total_ms, dist)
     value = units / (max_ms * 1e-3)
     peak, peak_src = load_peaks()
-    achieved = cfg.bytes_per_step / (fused_ms * 1e-3) / 1e9
+    achieved = bytes_per_step / (fused_ms * 1e-3) / 1e9
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": max_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -307,19 +336,20 @@ def run_psync(args, cfg, rank, world, dist):
         "config": workload_config(cfg, extra={
             "l2": f"no flush: each step streams {cfg.bytes_per_step / 1e9:.2f} GB (>> 126 MB L2) and gradient "
                   f"buffers rotate over {n_sets} resident sets",
-            "grad_sets": n_sets, "launch": geo, "variant": args.variant}),
-        "gbps_model": cfg.bytes_per_step * K * world / (max_ms * 1e-3) / 1e9,
+            "grad_sets": n_sets, "launch": geo, "variant": args.variant, "mode": mode,
+            "kept_per_step": n_eff}),
+        "gbps_model": bytes_per_step * K * world / (max_ms * 1e-3) / 1e9,
         "params_per_s": float(cfg.P) * K * world / (max_ms * 1e-3),
         "select_ms": select_ms, "fused_ms": fused_ms, "kernel_events_on_steps": len(fused_list),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": None, "peak_source": peak_src, "kernel": "fused_aggregate_update_ema",
-                     "algorithmic_bytes_per_launch": cfg.bytes_per_step,
+                     "algorithmic_bytes_per_launch": bytes_per_step,
                      "frac_of_nominal_8TBps": achieved / 8000.0},
         "clocks": clocks,
         "gpu_launches": 2 * K,
     }
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(traffic_file):   # dram bytes per launch from the committed ncu --set full capture
+    if os.path.exists(traffic_file) and mode == "first_n":   # dram bytes per launch from the committed ncu --set full capture
         try:
             with open(traffic_file) as fh:
                 out["roofline"]["traffic"] = json.load(fh).get(cfg.name)
@@ -329,7 +359,7 @@ def run_psync(args, cfg, rank, world, dist):
     # free the resident gradient sets before the host-buffer (e2e) leg
     del tables, steps_struct
     torch.cuda.empty_cache()
-    if not args.no_e2e:
+    if not args.no_e2e and mode == "first_n":
         out["e2e"] = run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         _, info = oracle_sample(cfg, seconds_budget=args.cpu_seconds, sample_elems=1 << 22)
@@ -391,6 +421,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="psync", choices=["psync", "reference"])
     ap.add_argument("--config", default="cfg3", choices=sorted(WORKLOADS))
+    ap.add_argument("--mode", default="first_n", choices=["first_n", "per_server", "timeout"],
+                    help="first_n: the headline (one kept set); per_server: Alg. 4 per server j; timeout: L259")
+    ap.add_argument("--timeout", type=float, default=1.5, help="seconds, for --mode timeout")
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--grid-ctas", type=int, default=0)
     ap.add_argument("--grad-sets", type=int, default=3)

@@ -123,13 +123,13 @@ __device__ __forceinline__ void update_in_memory(const FusedParams& p, float S, 
 }
 
 template <bool BF16, int OPT, int EMA>
-__device__ void scalar_range(const FusedParams& p, const char* const* s_ptr, int N, float inv_N, int64_t i0,
-                             int64_t i1, int64_t gtid, int64_t gthreads) {
+__device__ void scalar_range(const FusedParams& p, const char* const* s_ptr, int64_t i0, int64_t i1, int64_t gtid,
+                             int64_t gthreads) {
   for (int64_t i = i0 + gtid; i < i1; i += gthreads) {
     float S = 0.f;
 #pragma unroll 4
-    for (int n = 0; n < N; ++n) S += load_grad_scalar<BF16>(s_ptr[n], i);
-    update_in_memory<OPT, EMA>(p, S, inv_N, i);
+    for (int n = 0; n < p.N; ++n) S += load_grad_scalar<BF16>(s_ptr[n], i);
+    update_in_memory<OPT, EMA>(p, S, p.inv_N, i);
   }
 }
 
@@ -167,9 +167,12 @@ __device__ void rows_scalar_range(const FusedParams& p, int64_t i0, int64_t i1, 
 // each warp-level load covers 512 contiguous bytes of one worker's buffer.
 //
 // One tile through the 128-bit path: sum the N buffers of s_ptr[] in ascending order, update, store.
-template <int THREADS, int UPT, int U, bool BF16, int OPT, int EMA>
-__device__ __forceinline__ void vector_tile(const FusedParams& p, const char* const* s_ptr, const int N,
-                                            const float inv_N, const int64_t tile, const int64_t n_units) {
+// CONSTN: N and 1/N come straight from the kernel parameters (constant bank) instead of registers.
+template <int THREADS, int UPT, int U, bool BF16, int OPT, int EMA, bool CONSTN>
+__device__ __forceinline__ void vector_tile(const FusedParams& p, const char* const* s_ptr, const int N_arg,
+                                            const float inv_N_arg, const int64_t tile, const int64_t n_units) {
+  const int N = CONSTN ? p.N : N_arg;
+  const float inv_N = CONSTN ? p.inv_N : inv_N_arg;
   constexpr int E = BF16 ? 8 : 4;
   constexpr int Q = E / 4;  // float4 groups of theta per unit
   constexpr int64_t TILE_UNITS = static_cast<int64_t>(THREADS) * UPT;
@@ -290,18 +293,16 @@ __global__ void __launch_bounds__(THREADS, MINB) fused_aggregate_update_ema(cons
 
   if (!ROWS) {
     if (p.status != nullptr && *p.status != 0) return;  // selection failed: leave everything untouched
-    const int N = p.N;  // both straight from the constant bank (a variable count takes the ROWS kernel)
-    const float inv_N = p.inv_N;
-    const unsigned misalign = stage_row<THREADS>(p, s_ptr, 0, N);
+    const unsigned misalign = stage_row<THREADS>(p, s_ptr, 0, p.N);  // a variable count takes the ROWS kernel
     const bool vec_ok = (__syncthreads_or(static_cast<int>(misalign)) == 0) && (p.base_aligned != 0);
     if (!vec_ok) {
-      scalar_range<BF16, OPT, EMA>(p, s_ptr, N, inv_N, 0, p.P, static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x,
+      scalar_range<BF16, OPT, EMA>(p, s_ptr, 0, p.P, static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x,
                                    static_cast<int64_t>(gridDim.x) * THREADS);
       return;
     }
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x)
-      vector_tile<THREADS, UPT, U, BF16, OPT, EMA>(p, s_ptr, N, inv_N, tile, n_units);
-    if (tail0 < p.P && blockIdx.x == 0) scalar_range<BF16, OPT, EMA>(p, s_ptr, N, inv_N, tail0, p.P, threadIdx.x, THREADS);
+      vector_tile<THREADS, UPT, U, BF16, OPT, EMA, true>(p, s_ptr, 0, 0.f, tile, n_units);
+    if (tail0 < p.P && blockIdx.x == 0) scalar_range<BF16, OPT, EMA>(p, s_ptr, tail0, p.P, threadIdx.x, THREADS);
   } else {
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
       const int64_t e0 = tile * TILE_UNITS * E;
@@ -321,7 +322,7 @@ __global__ void __launch_bounds__(THREADS, MINB) fused_aggregate_update_ema(cons
         fast = __syncthreads_or(static_cast<int>(misalign)) == 0;
       }
       if (fast)
-        vector_tile<THREADS, UPT, U, BF16, OPT, EMA>(p, s_ptr, N, inv_N, tile, n_units);
+        vector_tile<THREADS, UPT, U, BF16, OPT, EMA, false>(p, s_ptr, N, inv_N, tile, n_units);
       else
         rows_scalar_range<BF16, OPT, EMA>(p, e0, e1, threadIdx.x, THREADS);
     }
