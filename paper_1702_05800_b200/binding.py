@@ -233,9 +233,11 @@ def make_step(shard_off, N: int, W: int, grad_dtype: int, theta: torch.Tensor, e
         raise ValueError("d_shard_off must have M+1 elements")
     rows = s.M if per_shard else 1
     stride = kept_stride if kept_stride > 0 else (W if d_n_kept is not None else N)
-    for nm, a, need in (("d_kept", d_kept, rows * stride), ("d_status", d_status, rows), ("d_n_kept", d_n_kept, rows)):
-        if a is not None and a.numel() < need:
-            raise ValueError(f"{nm} needs {need} elements")
+    if 1 <= N <= W <= PSYNC_MAX_WORKERS:       # out-of-range N / W are the C side's PSYNC_EINVAL to report
+        for nm, a, need in (("d_kept", d_kept, rows * stride), ("d_status", d_status, rows),
+                            ("d_n_kept", d_n_kept, rows)):
+            if a is not None and a.numel() < need:
+                raise ValueError(f"{nm} needs {need} elements")
     return s, (off, d_grads, d_kept, d_status, theta, ema, state0, state1, d_shard_off, d_n_kept)
 
 
