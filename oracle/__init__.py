@@ -56,6 +56,11 @@ def lib() -> ctypes.CDLL:
                                                    vp, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int,
                                                    f32, f32, f32, f32, f32]
         L.oracle_aggregate_update_rows.restype = ctypes.c_int
+        L.oracle_order_by_arrival.argtypes = [vp, i32, vp, vp]
+        L.oracle_order_by_arrival.restype = ctypes.c_int
+        L.oracle_async_apply.argtypes = [i64, i32, vp, i32, i32, vp, ctypes.c_int, vp, vp, vp, vp, vp, vp,
+                                         ctypes.c_int, ctypes.c_int, f32, f32, f32, f32, f32]
+        L.oracle_async_apply.restype = ctypes.c_int
         L.oracle_accumulate.argtypes = [vp, vp, ctypes.c_int, i64]
         L.oracle_accumulate.restype = ctypes.c_int
         L.oracle_apply_sum.argtypes = [i64, i32, vp, i32, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int,
@@ -180,6 +185,38 @@ def aggregate_update_rows(shard_off, N, grads, kept, theta, ema=None, state0=Non
                                               1 if per_shard else 0, _ptr(kept), kept.shape[1], _ptr(n_kept),
                                               _ptr(status), _ptr(theta), _ptr(ema), _ptr(state0), _ptr(state1),
                                               opt, ema_mode, gamma_t, alpha, mu, rho, eps)
+
+
+def order_by_arrival(arrival):
+    """Alg. 2's arrival order: worker indices by ascending (time, index), finite times only."""
+    W = arrival.size
+    _chk(arrival, np.float32, "arrival", W)
+    order = np.full(W, -1, dtype=np.int32)
+    n = np.zeros(1, dtype=np.int32)
+    st = lib().oracle_order_by_arrival(_ptr(arrival), W, _ptr(order), _ptr(n))
+    if st != OK:
+        raise ValueError("oracle_order_by_arrival: invalid arguments")
+    return order[:int(n[0])].copy()
+
+
+def async_apply(shard_off, grads, order, theta, ema=None, state0=None, state1=None, gammas=None, opt=SGD,
+                ema_mode=EMA_PRE, gamma_t=0.0, alpha=0.0, mu=0.0, rho=0.0, eps=0.0):
+    """len(order) iterations of Alg. 2, one gradient each, in place."""
+    P = theta.size
+    shard_off = np.ascontiguousarray(shard_off, dtype=np.int64)
+    M = shard_off.size - 1
+    W = len(grads)
+    gd = _grad_dtype(grads)
+    for k, g in enumerate(grads):
+        _chk(g, grads[0].dtype, f"grads[{k}]", P)
+    _chk(order, np.int32, "order")
+    _chk(gammas, np.float32, "gammas", order.size)
+    for nm, a in (("theta", theta), ("ema", ema), ("state0", state0), ("state1", state1)):
+        _chk(a, np.float32, nm, P)
+    ptrs = (ctypes.c_void_p * W)(*[g.ctypes.data for g in grads])
+    return lib().oracle_async_apply(P, M, _ptr(shard_off), order.size, W, ctypes.cast(ptrs, ctypes.c_void_p), gd,
+                                    _ptr(order), _ptr(gammas), _ptr(theta), _ptr(ema), _ptr(state0), _ptr(state1),
+                                    opt, ema_mode, gamma_t, alpha, mu, rho, eps)
 
 
 def accumulate(S, grad):

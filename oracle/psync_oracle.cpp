@@ -342,6 +342,63 @@ int oracle_aggregate_update_rows(int64_t P, int32_t M, const int64_t* shard_off,
   return ORACLE_OK;
 }
 
+// =============================================================================================
+// NEXT-3: Algorithm 2, "Async-SGD Parameter Server j" --
+// the paper's comparison method:
+//     for t = 0, 1, ...:  wait for gradient G from any worker               (L85)
+//                         theta(t+1)[j] <- theta(t)[j] - gamma_t G[j]       (L86)
+//                         ema(t)[j] = alpha ema(t-1)[j] + (1-alpha) theta(t)[j]   (L87)
+// Every arriving gradient is one iteration; nothing is dropped and no tag is checked.
+//
+// oracle_order_by_arrival: the order in which the W gradients reach the server = ascending
+// (arrival time, worker index) over the workers whose time is finite (reading R13: non-finite =
+// never arrived).  order[0..*n_arrived) OUT; the rest of order[] is left untouched.
+// =============================================================================================
+int oracle_order_by_arrival(const float* arrival, int32_t W, int32_t* order, int32_t* n_arrived) {
+  if (!arrival || !order || !n_arrived || W < 1) return ORACLE_EINVAL;
+  std::vector<std::pair<float, int32_t>> pairs;
+  for (int32_t k = 0; k < W; ++k)
+    if (std::isfinite(arrival[k])) pairs.emplace_back(arrival[k], k);
+  std::stable_sort(pairs.begin(), pairs.end(),
+                   [](const std::pair<float, int32_t>& x, const std::pair<float, int32_t>& y) {
+                     return x.first < y.first;  // stable: equal times keep ascending worker index
+                   });
+  for (size_t i = 0; i < pairs.size(); ++i) order[i] = pairs[i].second;
+  *n_arrived = static_cast<int32_t>(pairs.size());
+  return ORACLE_OK;
+}
+
+// oracle_async_apply: K iterations of Alg. 2, one per gradient, in the order given:
+//   for i = 0..K-1:  G = grads[order[i]];  gamma = gammas ? gammas[i] : gamma_t
+//                    every element: optimizer step with G (no averaging: the divisor is 1), then EMA
+// written as the paper's loop reads -- outer loop over arrivals, inner loop over the parameters of
+// each server j -- with theta / state / ema stored as fp32 after every iteration (they are the
+// server's stored state between arrivals).  The optimizer variants and the EMA operand are those of
+// the synchronous step (readings R3, R5, R6); EMA_PRE is the literal indexing of L87.
+int oracle_async_apply(int64_t P, int32_t M, const int64_t* shard_off, int32_t K, int32_t W,
+                       const void* const* grads, int grad_dtype, const int32_t* order, const float* gammas,
+                       float* theta, float* ema, float* state0, float* state1, int opt, int ema_mode,
+                       float gamma_t, float alpha, float mu, float rho, float eps) {
+  if (!args_ok(P, M, shard_off, 1, opt, ema_mode, theta, ema, state0, state1)) return ORACLE_EINVAL;
+  if (!grads || !order || K < 0 || K > W) return ORACLE_EINVAL;
+  if (grad_dtype != ORACLE_F32 && grad_dtype != ORACLE_BF16) return ORACLE_EINVAL;
+  for (int32_t i = 0; i < K; ++i)
+    if (order[i] < 0 || order[i] >= W || !grads[order[i]]) return ORACLE_EINVAL;
+  for (int32_t i = 0; i < K; ++i) {  // iteration t+i: "wait for gradient G from any worker"
+    const void* G = grads[order[i]];
+    const Coeffs c = make_coeffs(1, gammas ? gammas[i] : gamma_t, alpha, mu, rho, eps);
+    for (int32_t j = 0; j < M; ++j) {  // parameter server j
+      const int64_t lo = shard_off[j], hi = shard_off[j + 1];
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+      for (int64_t e = lo; e < hi; ++e)
+        apply_element(grad_at(G, grad_dtype, e), c, opt, ema_mode, theta, ema, state0, state1, e);
+    }
+  }
+  return ORACLE_OK;
+}
+
 // Threads the element loops use (1 without OpenMP); bench.py reports it as cpu_baseline.cores.
 int oracle_num_threads(void) {
 #ifdef _OPENMP
