@@ -24,7 +24,7 @@ PSYNC_EMA_POST, PSYNC_EMA_PRE, PSYNC_EMA_OFF = 0, 1, 2
 PSYNC_MAX_WORKERS = 1024
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
-           "psync_select_timeout", "psync_aggregate_update", "psync_ema",
+           "psync_select_timeout", "psync_aggregate_update", "psync_ema", "psync_order_by_arrival", "psync_async_apply",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_launch_geometry", "psync_probe_read",
            "psync_probe_copy")
 
@@ -73,6 +73,10 @@ def lib() -> ctypes.CDLL:
         L.psync_select_timeout.restype = ctypes.c_int
         L.psync_aggregate_update.argtypes = [ctypes.POINTER(psync_step), vp]
         L.psync_aggregate_update.restype = ctypes.c_int
+        L.psync_order_by_arrival.argtypes = [vp, i32, vp, vp, vp]
+        L.psync_order_by_arrival.restype = ctypes.c_int
+        L.psync_async_apply.argtypes = [ctypes.POINTER(psync_step), vp, vp]
+        L.psync_async_apply.restype = ctypes.c_int
         L.psync_ema.argtypes = [vp, vp, i64, f32, vp]
         L.psync_ema.restype = ctypes.c_int
         L.psync_step_host_workspace_bytes.argtypes = [i32, i32, i32, i64]
@@ -246,6 +250,28 @@ def psync_aggregate_update(step: psync_step, stream=None, check: bool = True) ->
     st = lib().psync_aggregate_update(ctypes.byref(step), _stream(stream))
     if check and st != PSYNC_OK:
         raise PsyncError(st, "psync_aggregate_update")
+    return st
+
+
+def psync_order_by_arrival(d_arrival: torch.Tensor, W: int, d_order: torch.Tensor, d_n_arrived: torch.Tensor,
+                           stream=None, check: bool = True) -> int:
+    """Arrival order of Alg. 2 (include/psync.h: psync_order_by_arrival)."""
+    if d_arrival.numel() < W or d_order.numel() < W or d_n_arrived.numel() < 1:
+        raise ValueError("need d_arrival [W], d_order [W], d_n_arrived [1]")
+    st = lib().psync_order_by_arrival(_dptr(d_arrival, torch.float32, "d_arrival"), W,
+                                      _dptr(d_order, torch.int32, "d_order"),
+                                      _dptr(d_n_arrived, torch.int32, "d_n_arrived"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_order_by_arrival")
+    return st
+
+
+def psync_async_apply(step: psync_step, d_gamma: Optional[torch.Tensor] = None, stream=None,
+                      check: bool = True) -> int:
+    """K iterations of Alg. 2 in one pass (include/psync.h: psync_async_apply)."""
+    st = lib().psync_async_apply(ctypes.byref(step), _dptr(d_gamma, torch.float32, "d_gamma"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_async_apply")
     return st
 
 

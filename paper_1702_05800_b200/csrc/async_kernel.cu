@@ -1,0 +1,224 @@
+// K4: the Async-SGD parameter server -- PAPER.md Algorithm 2 (L78-89), the paper's comparison method:
+//
+//     for t = 0, 1, ...:  wait for gradient G from any worker                       (L85)
+//                         theta(t+1)[j] <- theta(t)[j] - gamma_t G[j]               (L86)
+//                         ema(t)[j] = alpha ema(t-1)[j] + (1-alpha) theta(t)[j]     (L87)
+//
+// Every arriving gradient is one iteration.  K gradients that have arrived (K1c gives their order)
+// are applied ONE AT A TIME, in that order, but in ONE pass over HBM: a thread loads its 16-byte
+// unit of theta / state / ema once, walks the K gradient buffers in arrival order applying the
+// optimizer step and the EMA after each one in registers, and stores once.  Per element the
+// arithmetic is exactly K launches of the synchronous step with N=1, b=0 (bit-identical; tested),
+// but the traffic is K*sizeof(grad) + 8*(1 + n_state + [EMA]) bytes per parameter instead of
+// K*(sizeof(grad) + 8*(...)): 8.4x less for K=106 with RMSProp + EMA.
+// Unlike the synchronous step the chain of K dependent updates is real arithmetic: with RMSProp
+// (sqrt + divide per gradient element) the kernel is bound by the fp32/MUFU pipes, not by HBM;
+// with SGD / momentum it streams at the HBM roofline (DESIGN.md s.5).
+
+#include "psync_device.cuh"
+
+namespace psync {
+namespace {
+
+using namespace dev;
+
+template <bool BF16>
+__device__ __forceinline__ float unit_element(const uint4& r, int e) {
+  const uint32_t w = (&r.x)[BF16 ? (e >> 1) : e];
+  if (BF16) return __uint_as_float((e & 1) ? (w & 0xFFFF0000u) : (w << 16));
+  return __uint_as_float(w);
+}
+
+template <int THREADS, int U, int MINB, bool BF16, int OPT, int EMA>
+__global__ void __launch_bounds__(THREADS, MINB) async_apply_kernel(const FusedParams p) {
+  constexpr int E = BF16 ? 8 : 4;
+  constexpr int Q = E / 4;
+  __shared__ const char* s_ptr[kMaxWorkers];
+  __shared__ float s_gamma[kMaxWorkers];
+
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+
+  if (p.status != nullptr && *p.status != 0) return;
+  const int K = p.n_kept ? *p.n_kept : p.N;  // gradients that arrived
+  if (K <= 0) return;
+
+  unsigned misalign = 0;
+  for (int i = threadIdx.x; i < K; i += THREADS) {
+    const char* g = static_cast<const char*>(p.grads[p.kept[i]]);  // kept[] holds the arrival order
+    s_ptr[i] = g;
+    s_gamma[i] = p.gammas ? p.gammas[i] : p.gamma;  // gamma_t of iteration t+i
+    misalign |= static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 15u;
+  }
+  const bool vec_ok = (__syncthreads_or(static_cast<int>(misalign)) == 0) && (p.base_aligned != 0);
+
+  const int64_t n_units = vec_ok ? p.P / E : 0;
+  for (int64_t u = static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x; u < n_units;
+       u += static_cast<int64_t>(gridDim.x) * THREADS) {
+    float4 th4[Q], em4[Q], a04[Q], a14[Q];
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const int64_t e = u * E + 4 * q;
+      th4[q] = ld_state16(p.theta + e);
+      if (EMA != EMA_OFF) em4[q] = ld_state16(p.ema + e);
+      if (OPT != OPT_SGD) a04[q] = ld_state16(p.s0 + e);
+      if (OPT == OPT_RMSPROP_MOM) a14[q] = ld_state16(p.s1 + e);
+    }
+    float* th = reinterpret_cast<float*>(th4);
+    float* em = reinterpret_cast<float*>(em4);
+    float* a0 = reinterpret_cast<float*>(a04);
+    float* a1 = reinterpret_cast<float*>(a14);
+
+    int i = 0;
+    for (; i + U <= K; i += U) {  // U independent 16-byte loads in flight, then U dependent updates
+      uint4 r[U];
+#pragma unroll
+      for (int v = 0; v < U; ++v) r[v] = ldg_stream16(s_ptr[i + v] + u * 16);
+#pragma unroll
+      for (int v = 0; v < U; ++v) {
+        const float gamma = s_gamma[i + v];
+#pragma unroll
+        for (int e = 0; e < E; ++e)
+          update_element_g<OPT, EMA>(unit_element<BF16>(r[v], e), 1.0f, gamma, th[e], em[e], a0[e], a1[e], p);
+      }
+    }
+    for (; i < K; ++i) {
+      const uint4 r = ldg_stream16(s_ptr[i] + u * 16);
+      const float gamma = s_gamma[i];
+#pragma unroll
+      for (int e = 0; e < E; ++e)
+        update_element_g<OPT, EMA>(unit_element<BF16>(r, e), 1.0f, gamma, th[e], em[e], a0[e], a1[e], p);
+    }
+
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const int64_t e = u * E + 4 * q;
+      st_state16(p.theta + e, th4[q]);
+      if (EMA != EMA_OFF) st_state16(p.ema + e, em4[q]);
+      if (OPT != OPT_SGD) st_state16(p.s0 + e, a04[q]);
+      if (OPT == OPT_RMSPROP_MOM) st_state16(p.s1 + e, a14[q]);
+    }
+  }
+
+  // scalar path: the < E trailing parameters, or everything when a buffer is not 16-byte aligned
+  const int64_t tail0 = n_units * E;
+  const bool mine = vec_ok ? (blockIdx.x == 0) : true;
+  if (tail0 < p.P && mine) {
+    const int64_t first = vec_ok ? threadIdx.x : static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x;
+    const int64_t stride = vec_ok ? THREADS : static_cast<int64_t>(gridDim.x) * THREADS;
+    for (int64_t e = tail0 + first; e < p.P; e += stride) {
+      float th = p.theta[e];
+      float em = (EMA != EMA_OFF) ? p.ema[e] : 0.f;
+      float a0 = (OPT != OPT_SGD) ? p.s0[e] : 0.f;
+      float a1 = (OPT == OPT_RMSPROP_MOM) ? p.s1[e] : 0.f;
+      for (int i = 0; i < K; ++i)
+        update_element_g<OPT, EMA>(load_grad_scalar<BF16>(s_ptr[i], e), 1.0f, s_gamma[i], th, em, a0, a1, p);
+      p.theta[e] = th;
+      if (EMA != EMA_OFF) p.ema[e] = em;
+      if (OPT != OPT_SGD) p.s0[e] = a0;
+      if (OPT == OPT_RMSPROP_MOM) p.s1[e] = a1;
+    }
+  }
+}
+
+// K1c: rank sort of <= 1024 keys in one CTA.  Thread i owns worker i: its rank is the number of eligible
+// workers that come before it in (arrival, index) order; -0.0 == +0.0; non-finite = never arrived.
+__global__ void __launch_bounds__(1024) order_by_arrival_kernel(const float* __restrict__ arrival, int32_t W,
+                                                                int32_t* __restrict__ order,
+                                                                int32_t* __restrict__ n_arrived) {
+  __shared__ uint32_t s_key[kMaxWorkers];
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const int i = threadIdx.x;
+  uint32_t key = 0xFFFFFFFFu;
+  if (i < W) {
+    uint32_t u = __float_as_uint(arrival[i]);
+    if ((u & 0x7F800000u) != 0x7F800000u) {
+      if (u == 0x80000000u) u = 0u;
+      key = (u & 0x80000000u) ? ~u : (u | 0x80000000u);  // order-preserving; never 0xFFFFFFFF for finite input
+    }
+    s_key[i] = key;
+  }
+  const int n = __syncthreads_count(key != 0xFFFFFFFFu);
+  if (key != 0xFFFFFFFFu) {
+    int rank = 0;
+    for (int j = 0; j < W; ++j) {
+      const uint32_t kj = s_key[j];
+      rank += (kj < key || (kj == key && j < i)) ? 1 : 0;
+    }
+    order[rank] = i;
+  }
+  if (i == 0) *n_arrived = n;
+}
+
+struct AsyncShape {
+  int threads, unroll, minb;
+};
+constexpr AsyncShape kShapeF32 = {256, 8, 3};
+constexpr AsyncShape kShapeBF16 = {256, 8, 2};
+
+using KernelFn = void (*)(const FusedParams);
+
+template <bool BF16, int OPT>
+KernelFn pick_ema(int ema) {
+  constexpr AsyncShape S = BF16 ? kShapeBF16 : kShapeF32;
+  switch (ema) {
+    case EMA_POST: return async_apply_kernel<S.threads, S.unroll, S.minb, BF16, OPT, EMA_POST>;
+    case EMA_PRE: return async_apply_kernel<S.threads, S.unroll, S.minb, BF16, OPT, EMA_PRE>;
+    default: return async_apply_kernel<S.threads, S.unroll, S.minb, BF16, OPT, EMA_OFF>;
+  }
+}
+template <bool BF16>
+KernelFn pick_opt(int opt, int ema) {
+  switch (opt) {
+    case OPT_SGD: return pick_ema<BF16, OPT_SGD>(ema);
+    case OPT_MOMENTUM: return pick_ema<BF16, OPT_MOMENTUM>(ema);
+    default: return pick_ema<BF16, OPT_RMSPROP_MOM>(ema);
+  }
+}
+
+}  // namespace
+
+cudaError_t async_geometry(int dtype, int grid_ctas, int64_t P, FusedGeometry* out) {
+  const AsyncShape s = dtype == 1 ? kShapeBF16 : kShapeF32;
+  const int E = dtype == 1 ? 8 : 4;
+  out->block = s.threads;
+  out->tile_elems = s.threads * E;
+  out->smem_bytes = static_cast<int>((sizeof(const char*) + sizeof(float)) * kMaxWorkers);
+  int64_t grid = grid_ctas > 0 ? grid_ctas : (P / E + s.threads - 1) / s.threads;  // one unit per thread
+  if (grid > 0x7FFFFFFF) grid = 0x7FFFFFFF;
+  if (grid < 1) grid = 1;
+  out->grid = static_cast<int>(grid);
+  return cudaSuccess;
+}
+
+cudaError_t launch_async_apply(const FusedParams& p, int dtype, int opt, int ema, int grid_ctas, cudaStream_t stream) {
+  FusedGeometry g;
+  async_geometry(dtype, grid_ctas, p.P, &g);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(static_cast<unsigned>(g.grid));
+  cfg.blockDim = dim3(static_cast<unsigned>(g.block));
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, dtype == 1 ? pick_opt<true>(opt, ema) : pick_opt<false>(opt, ema), p);
+}
+
+cudaError_t launch_order_by_arrival(const float* d_arrival, int32_t W, int32_t* d_order, int32_t* d_n_arrived,
+                                    cudaStream_t stream) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(1);
+  cfg.blockDim = dim3(static_cast<unsigned>((W + 31) / 32 * 32));
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, order_by_arrival_kernel, d_arrival, W, d_order, d_n_arrived);
+}
+
+}  // namespace psync

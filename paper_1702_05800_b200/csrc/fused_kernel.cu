@@ -14,124 +14,19 @@
 //   * 128-bit read-only streaming loads (ld.global.nc, L1 no-allocate), U independent loads in
 //     flight per thread per batch, accumulated strictly in worker order afterwards, so the result
 //     does not depend on the launch geometry;
-//   * one tile per CTA (grid = number of tiles): the hardware CTA scheduler balances the tiles over
-//     the SMs dynamically; a forced smaller grid strides over the tiles (any grid is correct);
+//   * one tile per CTA (grid = number of tiles, no tile loop): the hardware CTA scheduler balances the
+//     tiles over the SMs dynamically;
 //   * theta / state / ema are loaded after the gradient stream (its registers are dead by then),
 //     updated in registers and stored once.
 // The flat element space is processed without regard to shard cuts: the step is elementwise and
 // all arrays share one layout, so server j's slice gets exactly Alg. 4's result (DESIGN.md s.4).
 
-#include "psync_kernels.cuh"
+#include "psync_device.cuh"
 
 namespace psync {
 namespace {
 
-constexpr int OPT_SGD = 0, OPT_MOMENTUM = 1, OPT_RMSPROP_MOM = 2;
-constexpr int EMA_POST = 0, EMA_PRE = 1, EMA_OFF = 2;
-
-// ---- memory access helpers -------------------------------------------------------------------
-__device__ __forceinline__ uint4 ldg_stream16(const void* p) {
-  uint4 r;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
-               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
-               : "l"(p));
-  return r;
-}
-__device__ __forceinline__ float ldg_stream_f32(const float* p) {
-  float r;
-  asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(r) : "l"(p));
-  return r;
-}
-__device__ __forceinline__ uint16_t ldg_stream_u16(const uint16_t* p) {
-  uint16_t r;
-  asm volatile("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(r) : "l"(p));
-  return r;
-}
-__device__ __forceinline__ float4 ld_state16(const float* p) {
-  float4 r;
-  asm volatile("ld.global.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];"
-               : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w)
-               : "l"(p));
-  return r;
-}
-__device__ __forceinline__ void st_state16(float* p, const float4& v) {
-  asm volatile("st.global.L1::no_allocate.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z),
-               "f"(v.w)
-               : "memory");
-}
-
-// ---- the per-element update, Alg. 4 l.8-9 ----------------------------------------------------
-template <int OPT, int EMA>
-__device__ __forceinline__ void update_element(float S, float inv_N, float& th, float& em, float& s0, float& s1,
-                                               const FusedParams& p) {
-  const float G = S * inv_N;  // mean of the kept gradients (L160)
-  const float th_old = th;
-  if (OPT == OPT_SGD) {
-    th = th - p.gamma * G;  // L40, L160
-  } else if (OPT == OPT_MOMENTUM) {
-    s0 = p.mu * s0 + G;  // v <- mu v + G          (reading R6)
-    th = th - p.gamma * s0;
-  } else {
-    s0 = p.rho * s0 + p.one_minus_rho * (G * G);            // ms  (reading R5)
-    s1 = p.mu * s1 + (p.gamma * G) / sqrtf(s0 + p.eps);     // mom
-    th = th - s1;
-  }
-  if (EMA != EMA_OFF) {
-    const float operand = (EMA == EMA_POST) ? th : th_old;  // reading R3
-    em = p.alpha * em + p.one_minus_alpha * operand;        // L40, L162
-  }
-}
-
-template <bool BF16>
-__device__ __forceinline__ void accumulate_unit(float* acc, const uint4& r) {
-  if (BF16) {  // 8 bf16 = 4 words; element 2i in the low half, 2i+1 in the high half; widening is exact
-    acc[0] += __uint_as_float(r.x << 16);
-    acc[1] += __uint_as_float(r.x & 0xFFFF0000u);
-    acc[2] += __uint_as_float(r.y << 16);
-    acc[3] += __uint_as_float(r.y & 0xFFFF0000u);
-    acc[4] += __uint_as_float(r.z << 16);
-    acc[5] += __uint_as_float(r.z & 0xFFFF0000u);
-    acc[6] += __uint_as_float(r.w << 16);
-    acc[7] += __uint_as_float(r.w & 0xFFFF0000u);
-  } else {
-    acc[0] += __uint_as_float(r.x);
-    acc[1] += __uint_as_float(r.y);
-    acc[2] += __uint_as_float(r.z);
-    acc[3] += __uint_as_float(r.w);
-  }
-}
-
-// ---- scalar path: any alignment, any range; also the < 8-element tail of the vector path ------
-template <bool BF16>
-__device__ __forceinline__ float load_grad_scalar(const char* g, int64_t i) {
-  if (BF16)
-    return __uint_as_float(static_cast<uint32_t>(ldg_stream_u16(reinterpret_cast<const uint16_t*>(g) + i)) << 16);
-  return ldg_stream_f32(reinterpret_cast<const float*>(g) + i);
-}
-
-template <int OPT, int EMA>
-__device__ __forceinline__ void update_in_memory(const FusedParams& p, float S, float inv_N, int64_t i) {
-  float th = p.theta[i];
-  float em = (EMA != EMA_OFF) ? p.ema[i] : 0.f;
-  float s0 = (OPT != OPT_SGD) ? p.s0[i] : 0.f;
-  float s1 = (OPT == OPT_RMSPROP_MOM) ? p.s1[i] : 0.f;
-  update_element<OPT, EMA>(S, inv_N, th, em, s0, s1, p);
-  p.theta[i] = th;
-  if (EMA != EMA_OFF) p.ema[i] = em;
-  if (OPT != OPT_SGD) p.s0[i] = s0;
-  if (OPT == OPT_RMSPROP_MOM) p.s1[i] = s1;
-}
-
-template <bool BF16, int OPT, int EMA>
-__device__ void scalar_range(const FusedParams& p, const char* const* s_ptr, int64_t i0, int64_t i1, int64_t gtid,
-                             int64_t gthreads) {
-  for (int64_t i = i0 + gtid; i < i1; i += gthreads) {
-    float S = 0.f;
-#pragma unroll 4
-    for (int n = 0; n < p.N; ++n) S += load_grad_scalar<BF16>(s_ptr[n], i);
-    update_in_memory<OPT, EMA>(p, S, p.inv_N, i);
-  }
-}
+using namespace dev;
 
 // ---- per-server rows (Alg. 4 per parameter server j): which server owns element i ----------------
 // Smallest j with off[j+1] > i, i.e. off[j] <= i < off[j+1] (empty servers are skipped).  The table is
@@ -300,31 +195,33 @@ __global__ void __launch_bounds__(THREADS, MINB) fused_aggregate_update_ema(cons
                                    static_cast<int64_t>(gridDim.x) * THREADS);
       return;
     }
-    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x)
-      vector_tile<THREADS, UPT, U, BF16, OPT, EMA, true>(p, s_ptr, 0, 0.f, tile, n_units);
+    if (blockIdx.x < n_tiles)  // one tile per CTA, no tile loop: its loop-carried registers cost a spill at 64
+      vector_tile<THREADS, UPT, U, BF16, OPT, EMA, true>(p, s_ptr, 0, 0.f, blockIdx.x, n_units);
     if (tail0 < p.P && blockIdx.x == 0) scalar_range<BF16, OPT, EMA>(p, s_ptr, tail0, p.P, threadIdx.x, THREADS);
   } else {
-    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const int64_t tile = blockIdx.x;
+    if (tile < n_tiles) {
       const int64_t e0 = tile * TILE_UNITS * E;
       const int64_t e1 = (e0 + TILE_UNITS * E < tail0) ? e0 + TILE_UNITS * E : tail0;  // tile = elements [e0, e1)
       // per_shard == 0 here means one row with a device-side count (time-out rule, L259): no lookup
       const int row = p.per_shard ? find_server(p.shard_off, p.M, e0) : 0;
       const bool one_server = p.per_shard ? (__ldg(p.shard_off + row + 1) >= e1) : true;  // CTA-uniform
-      bool fast = one_server && p.base_aligned != 0;
-      if (one_server && p.status != nullptr && p.status[row] != 0) continue;  // that server failed: skip its tile
-      __syncthreads();  // the previous tile's readers are done with s_ptr
-      int N = 0;
-      float inv_N = 0.f;
-      if (fast) {
-        N = p.n_kept ? p.n_kept[row] : p.N;
-        inv_N = p.n_kept ? 1.0f / static_cast<float>(N) : p.inv_N;
-        const unsigned misalign = stage_row<THREADS>(p, s_ptr, row, N);
-        fast = __syncthreads_or(static_cast<int>(misalign)) == 0;
+      const bool failed = one_server && p.status != nullptr && p.status[row] != 0;  // that server's tile is skipped
+      if (!failed) {
+        bool fast = one_server && p.base_aligned != 0;
+        int N = 0;
+        float inv_N = 0.f;
+        if (fast) {
+          N = p.n_kept ? p.n_kept[row] : p.N;
+          inv_N = p.n_kept ? 1.0f / static_cast<float>(N) : p.inv_N;
+          const unsigned misalign = stage_row<THREADS>(p, s_ptr, row, N);
+          fast = __syncthreads_or(static_cast<int>(misalign)) == 0;
+        }
+        if (fast)
+          vector_tile<THREADS, UPT, U, BF16, OPT, EMA, false>(p, s_ptr, N, inv_N, tile, n_units);
+        else
+          rows_scalar_range<BF16, OPT, EMA>(p, e0, e1, threadIdx.x, THREADS);
       }
-      if (fast)
-        vector_tile<THREADS, UPT, U, BF16, OPT, EMA, false>(p, s_ptr, N, inv_N, tile, n_units);
-      else
-        rows_scalar_range<BF16, OPT, EMA>(p, e0, e1, threadIdx.x, THREADS);
     }
     if (tail0 < p.P && blockIdx.x == 0) rows_scalar_range<BF16, OPT, EMA>(p, tail0, p.P, threadIdx.x, THREADS);
   }
@@ -339,13 +236,13 @@ __global__ void __launch_bounds__(256) ema_kernel(float* __restrict__ ema, const
   for (int64_t v = gtid; v < n4; v += gthreads) {
     float4 e = ld_state16(ema + 4 * v);
     const float4 t = ld_state16(theta + 4 * v);
-    e.x = alpha * e.x + one_minus_alpha * t.x;
-    e.y = alpha * e.y + one_minus_alpha * t.y;
-    e.z = alpha * e.z + one_minus_alpha * t.z;
-    e.w = alpha * e.w + one_minus_alpha * t.w;
+    e.x = __fmaf_rn(alpha, e.x, __fmul_rn(one_minus_alpha, t.x));
+    e.y = __fmaf_rn(alpha, e.y, __fmul_rn(one_minus_alpha, t.y));
+    e.z = __fmaf_rn(alpha, e.z, __fmul_rn(one_minus_alpha, t.z));
+    e.w = __fmaf_rn(alpha, e.w, __fmul_rn(one_minus_alpha, t.w));
     st_state16(ema + 4 * v, e);
   }
-  for (int64_t i = n4 * 4 + gtid; i < P; i += gthreads) ema[i] = alpha * ema[i] + one_minus_alpha * theta[i];
+  for (int64_t i = n4 * 4 + gtid; i < P; i += gthreads) ema[i] = __fmaf_rn(alpha, ema[i], __fmul_rn(one_minus_alpha, theta[i]));  // same form as the fused kernel
 }
 
 // ---- variants and dispatch ---------------------------------------------------------------------
@@ -358,17 +255,22 @@ constexpr Variant kVariants[] = {
     {256, 2, 8, 2},   // 2
     {256, 1, 16, 3},  // 3
     {512, 1, 8, 2},   // 4
-    {256, 2, 4, 3},   // 5
-    {256, 4, 2, 3},   // 6
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
 using KernelFn = void (*)(const FusedParams);
 
+// bf16 gradients with RMSProp hold 8 parameters x (acc, theta, ema, ms, mom) = 40 live values per thread:
+// at 4 CTAs/SM (64 registers) that spills, so this one combination runs at 3 CTAs/SM (85 registers).
+constexpr int minb_for(int v, bool bf16, int opt) {
+  const int cap = 768 / kVariants[v].threads;  // resident threads per SM that leave 85 registers each
+  return (bf16 && opt == OPT_RMSPROP_MOM && kVariants[v].minb > cap) ? cap : kVariants[v].minb;
+}
+
 template <int V, bool BF16, int OPT, int EMA, bool ROWS = false>
 constexpr KernelFn kernel_for() {
-  return fused_aggregate_update_ema<kVariants[V].threads, kVariants[V].upt, kVariants[V].unroll, kVariants[V].minb,
-                                    BF16, OPT, EMA, ROWS>;
+  return fused_aggregate_update_ema<kVariants[V].threads, kVariants[V].upt, kVariants[V].unroll,
+                                    minb_for(V, BF16, OPT), BF16, OPT, EMA, ROWS>;
 }
 
 // per-server rows: the default variant only (a forced variant > 1 is PSYNC_EUNSUPPORTED in the ABI)
@@ -417,9 +319,7 @@ KernelFn pick_kernel(int v, int dtype, int opt, int ema) {
     case 0: return pick_dtype<0>(dtype, opt, ema);
     case 1: return pick_dtype<1>(dtype, opt, ema);
     case 2: return pick_dtype<2>(dtype, opt, ema);
-    case 3: return pick_dtype<3>(dtype, opt, ema);
-    case 4: return pick_dtype<4>(dtype, opt, ema);
-    default: return pick_dtype<5>(dtype, opt, ema);
+    default: return pick_dtype<3>(dtype, opt, ema);
   }
 }
 
@@ -449,14 +349,15 @@ cudaError_t fused_geometry(int dtype, int opt, int ema, int variant, int grid_ct
   out->block = vr.threads;
   out->tile_elems = vr.threads * vr.upt * E;
   out->smem_bytes = static_cast<int>(sizeof(const char*)) * kMaxWorkers;
-  // One tile per CTA by default: the hardware CTA scheduler then balances tiles dynamically over the
-  // SMs, which measured 2-3 % faster on B200 than a persistent grid with static striding (DESIGN.md s.5).
-  // grid_ctas > 0 forces a grid; the kernel's tile loop strides by gridDim.x, so any grid is correct.
+  // One tile per CTA, always: the hardware CTA scheduler balances the tiles dynamically over the SMs, which
+  // measured 2-3 % faster on B200 than a persistent grid with static striding (DESIGN.md s.5), and a kernel
+  // without a tile loop stays inside 64 registers without spilling.  grid_ctas is accepted and ignored.
   (void)opt;
   (void)ema;
+  (void)grid_ctas;
   const int64_t n_tiles = (P / E + static_cast<int64_t>(vr.threads) * vr.upt - 1) / (static_cast<int64_t>(vr.threads) * vr.upt);
-  int64_t grid = grid_ctas > 0 ? grid_ctas : n_tiles;
-  if (grid > 0x7FFFFFFF) grid = 0x7FFFFFFF;
+  int64_t grid = n_tiles;
+  if (grid > 0x7FFFFFFF) return cudaErrorInvalidConfiguration;  // > 2^41 parameters: not addressable in HBM anyway
   if (grid < 1) grid = 1;
   out->grid = static_cast<int>(grid);
   return cudaSuccess;

@@ -66,6 +66,7 @@ FusedParams make_params(const psync_step* s, int64_t first, int64_t count, const
   p.M = s->M;
   p.shard_off = s->d_shard_off;
   p.n_kept = s->d_n_kept;
+  p.gammas = nullptr;
   p.base_aligned = aligned16(p.theta) && (p.ema == nullptr || aligned16(p.ema)) && (p.s0 == nullptr || aligned16(p.s0)) &&
                    (p.s1 == nullptr || aligned16(p.s1));
   return p;
@@ -166,6 +167,28 @@ PSYNC_API int psync_aggregate_update(const psync_step* step, void* stream) {
   const FusedParams p = make_params(step, 0, step->P, step->d_grads, step->d_kept, step->d_status);
   const cudaError_t err = psync::launch_fused(p, step->grad_dtype, step->opt, step->ema_mode, step->variant,
                                               step->grid_ctas, static_cast<cudaStream_t>(stream));
+  return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
+}
+
+PSYNC_API int psync_order_by_arrival(const float* d_arrival, int32_t W, int32_t* d_order, int32_t* d_n_arrived,
+                           void* stream) {
+  if (d_arrival == nullptr || d_order == nullptr || d_n_arrived == nullptr) return PSYNC_EINVAL;
+  if (W < 1 || W > PSYNC_MAX_WORKERS) return PSYNC_EINVAL;
+  return psync::launch_order_by_arrival(d_arrival, W, d_order, d_n_arrived, static_cast<cudaStream_t>(stream)) ==
+                 cudaSuccess
+             ? PSYNC_OK
+             : PSYNC_ECUDA;
+}
+
+PSYNC_API int psync_async_apply(const psync_step* step, const float* d_gamma, void* stream) {
+  const int st = check_step(step, true);
+  if (st != PSYNC_OK && !(st == PSYNC_EUNSUPPORTED && step->per_shard == 0)) return st;  // variant is ignored here
+  if (step->per_shard != 0) return PSYNC_EUNSUPPORTED;
+  if (step->P == 0) return PSYNC_OK;
+  FusedParams p = make_params(step, 0, step->P, step->d_grads, step->d_kept, step->d_status);
+  p.gammas = d_gamma;
+  const cudaError_t err = psync::launch_async_apply(p, step->grad_dtype, step->opt, step->ema_mode, step->grid_ctas,
+                                                    static_cast<cudaStream_t>(stream));
   return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
 }
 

@@ -1,0 +1,242 @@
+"""GPU parity for the Async-SGD parameter server (NEXT-3: Algorithm 2) against the CPU
+oracle through the C ABI: the arrival order bit-exactly, theta / state / ema within tolerance.
+
+Tolerance (R20): K async iterations are K dependent optimizer steps, so north_star's free-run
+budget applies -- rtol 1e-5 for K <= 10, growing linearly to 1e-4 at K = 100 (1e-6 * K), atol 1e-6."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1702_05800_b200 as psync
+from paper_1702_05800_b200 import synth
+
+from _harness import ATOL_STEP, STATE_NAMES, assert_close, to_np
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+BASE = synth.Config(name="async", cfg_id=12, P=70_003, M=7, N=13, b=0, arrival_sigma=0.3, opt=synth.SGD,
+                    gamma=0.045, alpha=0.9999, mu=0.9, rho=0.9, eps=1.0, ema_mode=synth.EMA_PRE, steps=3)
+
+
+def rtol_async(K):
+    return 1e-6 * max(10, K)
+
+
+class AsyncPair:
+    def __init__(self, cfg, misalign=0, grid_ctas=0):
+        self.cfg = cfg
+        self.off = synth.shard_offsets(cfg)
+
+        def place(t):
+            if t is None or not misalign:
+                return t
+            buf = torch.empty(t.numel() + 8, dtype=t.dtype, device=DEV)
+            view = buf[misalign:misalign + t.numel()]
+            view.copy_(t)
+            return view
+
+        self.theta = place(synth.init_theta(cfg, DEV))
+        s0, s1 = synth.init_state(cfg, DEV)
+        self.state0, self.state1 = place(s0), place(s1)
+        self.ema = place(self.theta.clone()) if cfg.ema_mode != synth.EMA_OFF else None
+        self.host = {n: to_np(getattr(self, n)) for n in STATE_NAMES}
+        self.d_order = torch.full((cfg.W,), -1, dtype=torch.int32, device=DEV)
+        self.d_n = torch.full((1,), -7, dtype=torch.int32, device=DEV)
+        self.grid_ctas = grid_ctas
+
+    def make_step(self, table, gamma=None, d_n=True, N=None):
+        cfg = self.cfg
+        return psync.make_step(self.off, cfg.W if N is None else N, cfg.W, table.grad_dtype, self.theta, self.ema,
+                               self.state0, self.state1, opt=cfg.opt, ema_mode=cfg.ema_mode,
+                               gamma_t=cfg.gamma if gamma is None else gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho,
+                               eps=cfg.eps, d_grads=table.d_ptrs, d_kept=self.d_order, grid_ctas=self.grid_ctas,
+                               d_n_kept=self.d_n if d_n else None, kept_stride=cfg.W)
+
+    def step(self, s, arrival, gammas=None):
+        cfg = self.cfg
+        grads = [synth.gradient(cfg, s, k, DEV) for k in range(cfg.W)]
+        table = psync.make_grad_table(grads)
+        psync.psync_order_by_arrival(torch.from_numpy(arrival).to(DEV), cfg.W, self.d_order, self.d_n)
+        st, keep = self.make_step(table)
+        d_gamma = None if gammas is None else torch.from_numpy(gammas).to(DEV)
+        psync.psync_async_apply(st, d_gamma)
+        torch.cuda.synchronize()
+        order = oracle.order_by_arrival(arrival)
+        K = order.size
+        assert int(self.d_n.item()) == K
+        assert np.array_equal(self.d_order.cpu().numpy()[:K], order)
+        h = self.host
+        rc = oracle.async_apply(self.off, [synth.as_numpy_grad(g) for g in grads], order, h["theta"], h["ema"],
+                                h["state0"], h["state1"], gammas=None if gammas is None else gammas[:K].copy(),
+                                opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu,
+                                rho=cfg.rho, eps=cfg.eps)
+        assert rc == oracle.OK
+        for n in STATE_NAMES:
+            g = getattr(self, n)
+            if g is not None:
+                assert_close(to_np(g), h[n], rtol_async(K), ATOL_STEP, f"{cfg.name} step {s} {n}")
+                h[n] = to_np(g)
+        return order
+
+
+# ------------------------------------------------------------------ K1c: arrival order
+@pytest.mark.parametrize("seed", range(6))
+def test_order_by_arrival_matches_oracle(seed):
+    rng = np.random.default_rng(1500 + seed)
+    W = int(rng.choice([1, 2, 31, 32, 33, 106, 212, 513, 1024]))
+    a = rng.lognormal(0, 0.3, W).astype(np.float32)
+    ties = rng.random(W) < 0.3
+    a[ties] = rng.choice(np.array([0.5, 1.0, 1.0, -0.0, 0.0, -2.0, 1e-42], np.float32), size=int(ties.sum()))
+    a[rng.random(W) < 0.08] = np.inf
+    a[rng.random(W) < 0.04] = np.nan
+    a[rng.random(W) < 0.04] = -np.inf
+    d_order = torch.full((W,), -1, dtype=torch.int32, device=DEV)
+    d_n = torch.full((1,), -7, dtype=torch.int32, device=DEV)
+    psync.psync_order_by_arrival(torch.from_numpy(a).to(DEV), W, d_order, d_n)
+    want = oracle.order_by_arrival(a)
+    got = d_order.cpu().numpy()
+    assert int(d_n.item()) == want.size and np.array_equal(got[:want.size], want) and (got[want.size:] == -1).all()
+
+
+def test_order_nobody_arrived_and_all_equal():
+    W = 40
+    d_order = torch.full((W,), -1, dtype=torch.int32, device=DEV)
+    d_n = torch.full((1,), -7, dtype=torch.int32, device=DEV)
+    psync.psync_order_by_arrival(torch.full((W,), float("nan"), device=DEV), W, d_order, d_n)
+    assert int(d_n.item()) == 0 and (d_order.cpu().numpy() == -1).all()
+    psync.psync_order_by_arrival(torch.full((W,), 1.25, device=DEV), W, d_order, d_n)
+    assert int(d_n.item()) == W and d_order.cpu().numpy().tolist() == list(range(W))
+
+
+# ------------------------------------------------------------------ K4: K iterations in one pass
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+@pytest.mark.parametrize("opt", [synth.SGD, synth.MOMENTUM, synth.RMSPROP_MOM])
+@pytest.mark.parametrize("ema_mode", [synth.EMA_PRE, synth.EMA_POST, synth.EMA_OFF])
+def test_async_every_template_instance_lockstep(dtype, opt, ema_mode):
+    cfg = replace(BASE, grad_dtype=dtype, opt=opt, ema_mode=ema_mode, name=f"async_d{dtype}_o{opt}_e{ema_mode}")
+    pair = AsyncPair(cfg)
+    rng = np.random.default_rng(7)
+    for s in range(2):
+        a = synth.arrival_times(cfg, s)
+        if s == 1:
+            a[[2, 9]] = np.inf                       # two workers never report: K = 11
+        gammas = rng.uniform(0.01, 0.09, cfg.W).astype(np.float32) if s == 1 else None
+        order = pair.step(s, a, gammas)
+        assert order.size == (13 if s == 0 else 11)
+
+
+@pytest.mark.parametrize("K", [1, 7, 8, 9, 16, 17, 106])
+def test_async_worker_counts_cross_unroll_boundaries(K):
+    cfg = replace(BASE, N=K, P=20_011, opt=synth.RMSPROP_MOM, name=f"async_K{K}")
+    AsyncPair(cfg).step(0, synth.arrival_times(cfg, 0))
+
+
+@pytest.mark.parametrize("P", [1, 3, 4, 5, 8, 9, 1023, 1025])
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+def test_async_small_and_ragged_sizes(P, dtype):
+    cfg = replace(BASE, P=P, M=1, grad_dtype=dtype, opt=synth.MOMENTUM, name=f"async_small{P}")
+    AsyncPair(cfg).step(0, synth.arrival_times(cfg, 0))
+
+
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+def test_async_unaligned_state_takes_the_scalar_path(dtype):
+    cfg = replace(BASE, P=9_001, grad_dtype=dtype, opt=synth.RMSPROP_MOM, name="async_unaligned")
+    AsyncPair(cfg, misalign=1).step(0, synth.arrival_times(cfg, 0))
+
+
+def test_async_forced_small_grid():
+    cfg = replace(BASE, P=300_007, opt=synth.MOMENTUM, name="async_grid")
+    for grid in (1, 148):
+        AsyncPair(cfg, grid_ctas=grid).step(0, synth.arrival_times(cfg, 0))
+
+
+@pytest.mark.parametrize("dtype,opt", [(synth.F32, synth.RMSPROP_MOM), (synth.BF16, synth.MOMENTUM), (synth.F32, synth.SGD)])
+def test_async_is_bit_identical_to_k_sequential_n1_steps_on_the_gpu(dtype, opt):
+    """Property at any size: one K-iteration pass == K launches of the synchronous kernel with N=1, b=0."""
+    cfg = replace(BASE, P=200_003, N=9, grad_dtype=dtype, opt=opt, ema_mode=synth.EMA_PRE, name="async_vs_seq")
+    a = synth.arrival_times(cfg, 0)
+    order = oracle.order_by_arrival(a)
+    grads = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    table = psync.make_grad_table(grads)
+    one = AsyncPair(cfg)
+    psync.psync_order_by_arrival(torch.from_numpy(a).to(DEV), cfg.W, one.d_order, one.d_n)
+    st, keep = one.make_step(table)
+    psync.psync_async_apply(st)
+    seq = AsyncPair(cfg)
+    d_k = torch.zeros(1, dtype=torch.int32, device=DEV)
+    for k in order:
+        d_k.fill_(int(k))
+        st2, keep2 = psync.make_step(seq.off, 1, cfg.W, table.grad_dtype, seq.theta, seq.ema, seq.state0, seq.state1,
+                                     opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu,
+                                     rho=cfg.rho, eps=cfg.eps, d_grads=table.d_ptrs, d_kept=d_k)
+        psync.psync_aggregate_update(st2)
+        torch.cuda.synchronize()
+    for n in STATE_NAMES:
+        if getattr(one, n) is not None:
+            assert np.array_equal(to_np(getattr(one, n)), to_np(getattr(seq, n))), n
+
+
+def test_async_k0_status_and_argument_errors_touch_nothing():
+    cfg = replace(BASE, P=5_000, opt=synth.RMSPROP_MOM, name="async_noop")
+    pair = AsyncPair(cfg)
+    grads = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    table = psync.make_grad_table(grads)
+    before = {n: to_np(getattr(pair, n)) for n in STATE_NAMES}
+    psync.psync_order_by_arrival(torch.full((cfg.W,), float("inf"), device=DEV), cfg.W, pair.d_order, pair.d_n)
+    st, keep = pair.make_step(table)
+    assert psync.psync_async_apply(st) == psync.PSYNC_OK                     # K = 0: a no-op
+    bad_status = torch.full((1,), psync.PSYNC_ETOOFEW, dtype=torch.int32, device=DEV)
+    pair.d_n.fill_(3)
+    pair.d_order[:3] = torch.tensor([0, 1, 2], dtype=torch.int32, device=DEV)
+    st.d_status = bad_status.data_ptr()
+    assert psync.psync_async_apply(st) == psync.PSYNC_OK                     # status != OK: a no-op
+    st.d_status = None
+    st.per_shard = 1
+    st.d_shard_off = pair.d_n.data_ptr()
+    assert psync.psync_async_apply(st, check=False) == psync.PSYNC_EUNSUPPORTED
+    st.per_shard, st.d_shard_off, st.N = 0, None, 0
+    assert psync.psync_async_apply(st, check=False) == psync.PSYNC_EINVAL
+    torch.cuda.synchronize()
+    for n in STATE_NAMES:
+        assert np.array_equal(to_np(getattr(pair, n)), before[n]), n
+    L = psync.binding.lib()
+    assert L.psync_order_by_arrival(None, 4, None, None, None) == psync.PSYNC_EINVAL
+    assert L.psync_order_by_arrival(8, 0, 8, 8, None) == psync.PSYNC_EINVAL
+    assert L.psync_order_by_arrival(8, 1025, 8, 8, None) == psync.PSYNC_EINVAL
+
+
+def test_full_size_async_cfg3_shape_sampled():
+    """cfg3's shape (P = 25,165,824, W = 106, RMSProp + EMA) through Alg. 2: all 106 gradients applied one at a
+    time in one pass; sampled elements against the oracle on the gathered columns."""
+    cfg = replace(synth.PAPER_RMSPROP, N=106, b=0, ema_mode=synth.EMA_PRE, name="async_cfg3")
+    free, _ = torch.cuda.mem_get_info()
+    if cfg.footprint_bytes * 1.15 > free:
+        pytest.skip("not enough free HBM")
+    pair = AsyncPair(cfg)
+    rng = np.random.default_rng(3)
+    idx = np.unique(np.concatenate([np.arange(0, 2048), np.arange(cfg.P - 2048, cfg.P),
+                                    rng.integers(0, cfg.P, 20_000)])).astype(np.int64)
+    d_idx = torch.from_numpy(idx).to(DEV)
+    host = {n: to_np(getattr(pair, n)[d_idx]) for n in STATE_NAMES}
+    grads = [torch.empty(cfg.P, dtype=torch.float32, device=DEV) for _ in range(cfg.W)]
+    for k in range(cfg.W):
+        synth.gradient(cfg, 0, k, DEV, out=grads[k])
+    table = psync.make_grad_table(grads)
+    a = synth.arrival_times(cfg, 0)
+    psync.psync_order_by_arrival(torch.from_numpy(a).to(DEV), cfg.W, pair.d_order, pair.d_n)
+    st, keep = pair.make_step(table)
+    psync.psync_async_apply(st)
+    torch.cuda.synchronize()
+    order = oracle.order_by_arrival(a)
+    assert order.size == 106 and np.array_equal(pair.d_order.cpu().numpy(), order)
+    rc = oracle.async_apply([0, idx.size], [synth.as_numpy_grad(g[d_idx]) for g in grads], order, host["theta"],
+                            host["ema"], host["state0"], host["state1"], opt=cfg.opt, ema_mode=cfg.ema_mode,
+                            gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
+    assert rc == oracle.OK
+    for n in STATE_NAMES:
+        assert_close(to_np(getattr(pair, n)[d_idx]), host[n], rtol_async(106), ATOL_STEP, f"async cfg3 {n} (sampled)")
+    assert bool(torch.isfinite(pair.theta).all())

@@ -33,7 +33,7 @@ def test_every_template_instance_lockstep(dtype, opt, ema_mode):
     Pair(cfg).run(3, lockstep=True, rtol=RTOL_STEP, atol=ATOL_STEP)
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
 @pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
 def test_every_variant(variant, dtype):
     cfg = replace(BASE, grad_dtype=dtype, opt=synth.RMSPROP_MOM, N=21, b=2, P=200_001, name=f"variant{variant}")
@@ -152,7 +152,7 @@ def test_bitwise_invariance_shard_layout_grid_variant_and_rerun():
     ref = None
     P = cfg.P
     layouts = [None, [0, P], [0, 1, 2, 77_777, 77_777, P]]
-    runs = [(lay, 0, 0) for lay in layouts] + [(None, 1, v) for v in range(1, 7)] + [(None, 37, 0), (None, 1000, 2)]
+    runs = [(lay, 0, 0) for lay in layouts] + [(None, 1, v) for v in range(1, 5)] + [(None, 37, 0), (None, 1000, 2)]
     runs.append((None, 0, 0))   # the same launch again
     for lay, grid, variant in runs:
         pair = Pair(cfg, shard_off=lay, grid_ctas=grid, variant=variant)
