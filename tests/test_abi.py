@@ -118,8 +118,9 @@ def test_launch_geometry_without_a_device(B):
     s.d_theta, s.d_ema, s.d_state0, s.d_state1, s.opt = 256, 512, 1024, 2048, B.PSYNC_RMSPROP_MOM
     g = B.psync_launch_geometry(s)
     assert g["block"] in (128, 256, 512) and g["grid"] >= 148 and g["tile_elems"] >= 512
-    s.grid_ctas = 37
-    assert B.psync_launch_geometry(s)["grid"] == 37
+    assert g["grid"] == -(-25_165_824 // g["tile_elems"])            # one tile per CTA, always
+    s.grid_ctas = 37                                                 # accepted and ignored
+    assert B.psync_launch_geometry(s)["grid"] == g["grid"]
 
 
 def test_binding_refuses_cpu_tensors(B):
