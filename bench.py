@@ -246,10 +246,12 @@ def run_psync(args, cfg, rank, world, dist):
     else:
         arr_np = np.stack([synth.arrival_times(cfg, s) for s in range(K + Wm)])
     arrivals = torch.from_numpy(arr_np).to(dev)
-    stride = cfg.W if mode == "timeout" else cfg.N
+    # --mode async: Alg. 2 -- all W gradients applied one at a time in arrival order, one pass (NEXT-3).
+    stride = cfg.W if mode in ("timeout", "async") else cfg.N
     d_kept = torch.full((rows, stride), -1, dtype=torch.int32, device=dev) if mode != "first_n" else ps.d_kept
-    d_status = torch.full((rows,), -9, dtype=torch.int32, device=dev) if mode != "first_n" else ps.d_status
-    d_n_kept = torch.zeros(rows, dtype=torch.int32, device=dev) if mode == "timeout" else None
+    d_status = torch.full((rows,), 0 if mode == "async" else -9, dtype=torch.int32,
+                          device=dev) if mode != "first_n" else ps.d_status
+    d_n_kept = torch.zeros(rows, dtype=torch.int32, device=dev) if mode in ("timeout", "async") else None
     d_off = torch.from_numpy(off).to(dev) if mode == "per_server" else None
     steps_struct = []
     for tb in tables:   # one psync_step per gradient set, built once (marshalling outside the timed region)
@@ -269,8 +271,10 @@ def run_psync(args, cfg, rank, world, dist):
             B.psync_select_first_n(arrivals[i], cfg.N, cfg.b, ps.d_kept, ps.d_status, ps.d_t_nth, None, i, stream)
         elif mode == "per_server":
             B.psync_select_first_n_sharded(arrivals[i], cfg.N, cfg.b, cfg.M, d_kept, d_status, None, None, i, stream)
-        else:
+        elif mode == "timeout":
             B.psync_select_timeout(arrivals[i], cfg.W, args.timeout, d_kept, d_n_kept, d_status, stream=stream)
+        else:
+            B.psync_order_by_arrival(arrivals[i], cfg.W, d_kept, d_n_kept, stream)
 
     def one_step(i, ev=None):
         st = steps_struct[i % n_sets][0]
@@ -279,7 +283,10 @@ def run_psync(args, cfg, rank, world, dist):
         select(i)
         if ev is not None:
             ev[1].record(stream)
-        B.psync_aggregate_update(st, stream)
+        if mode == "async":
+            B.psync_async_apply(st, None, stream)
+        else:
+            B.psync_aggregate_update(st, stream)
         if ev is not None:
             ev[2].record(stream)
 
@@ -318,7 +325,9 @@ def run_psync(args, cfg, rank, world, dist):
     assert bool((d_status == 0).all()) and bool(torch.isfinite(theta[:4096]).all())
 
     # gradient elements aggregated per step: N*P, or (workers in time)*P for the time-out rule
-    if mode == "timeout":
+    if mode == "async":
+        n_eff = float(cfg.W)                 # every gradient is applied (nothing is dropped in Alg. 2)
+    elif mode == "timeout":
         n_eff = float(np.mean([(arr_np[Wm + k] <= args.timeout).sum() for k in range(K)]))
     else:
         n_eff = float(cfg.N)
@@ -342,7 +351,7 @@ def run_psync(args, cfg, rank, world, dist):
         "params_per_s": float(cfg.P) * K * world / (max_ms * 1e-3),
         "select_ms": select_ms, "fused_ms": fused_ms, "kernel_events_on_steps": len(fused_list),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "peak_source": peak_src, "kernel": "fused_aggregate_update_ema",
+                     "traffic": None, "peak_source": peak_src, "kernel": "async_apply_kernel" if mode == "async" else "fused_aggregate_update_ema",
                      "algorithmic_bytes_per_launch": bytes_per_step,
                      "frac_of_nominal_8TBps": achieved / 8000.0},
         "clocks": clocks,
@@ -421,8 +430,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="psync", choices=["psync", "reference"])
     ap.add_argument("--config", default="cfg3", choices=sorted(WORKLOADS))
-    ap.add_argument("--mode", default="first_n", choices=["first_n", "per_server", "timeout"],
-                    help="first_n: the headline (one kept set); per_server: Alg. 4 per server j; timeout: L259")
+    ap.add_argument("--mode", default="first_n", choices=["first_n", "per_server", "timeout", "async"],
+                    help="first_n: the headline (one kept set); per_server: Alg. 4 per server j; timeout: L259; "
+                         "async: Alg. 2, all W gradients one at a time in one pass")
     ap.add_argument("--timeout", type=float, default=1.5, help="seconds, for --mode timeout")
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--grid-ctas", type=int, default=0)
