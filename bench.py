@@ -278,6 +278,9 @@ def run_psync(args, cfg, rank, world, dist):
 
     def one_step(i, ev=None):
         st = steps_struct[i % n_sets][0]
+        if ev is None and mode in ("first_n", "per_server"):     # the user's call: selection + fused update
+            B.psync_step_device(st, arrivals[i], None, None, i, stream)
+            return
         if ev is not None:
             ev[0].record(stream)
         select(i)

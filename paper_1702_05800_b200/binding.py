@@ -24,7 +24,7 @@ PSYNC_EMA_POST, PSYNC_EMA_PRE, PSYNC_EMA_OFF = 0, 1, 2
 PSYNC_MAX_WORKERS = 1024
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
-           "psync_select_timeout", "psync_aggregate_update", "psync_ema", "psync_order_by_arrival", "psync_async_apply",
+           "psync_select_timeout", "psync_aggregate_update", "psync_ema", "psync_order_by_arrival", "psync_async_apply", "psync_step_device",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_launch_geometry", "psync_probe_read",
            "psync_probe_copy")
 
@@ -73,6 +73,8 @@ def lib() -> ctypes.CDLL:
         L.psync_select_timeout.restype = ctypes.c_int
         L.psync_aggregate_update.argtypes = [ctypes.POINTER(psync_step), vp]
         L.psync_aggregate_update.restype = ctypes.c_int
+        L.psync_step_device.argtypes = [ctypes.POINTER(psync_step), vp, vp, i32, vp, vp]
+        L.psync_step_device.restype = ctypes.c_int
         L.psync_order_by_arrival.argtypes = [vp, i32, vp, vp, vp]
         L.psync_order_by_arrival.restype = ctypes.c_int
         L.psync_async_apply.argtypes = [ctypes.POINTER(psync_step), vp, vp]
@@ -250,6 +252,24 @@ def psync_aggregate_update(step: psync_step, stream=None, check: bool = True) ->
     st = lib().psync_aggregate_update(ctypes.byref(step), _stream(stream))
     if check and st != PSYNC_OK:
         raise PsyncError(st, "psync_aggregate_update")
+    return st
+
+
+def psync_step_device(step: psync_step, d_arrival: torch.Tensor, d_t_nth: Optional[torch.Tensor] = None,
+                      d_step_tag: Optional[torch.Tensor] = None, t: int = 0, stream=None, check: bool = True) -> int:
+    """Selection + fused update in one call (include/psync.h: psync_step_device; Alg. 4)."""
+    rows = step.M if step.per_shard else 1
+    if d_arrival.numel() < rows * step.W:
+        raise ValueError("d_arrival needs rows*W elements")
+    if d_step_tag is not None and d_step_tag.numel() < rows * step.W:
+        raise ValueError("d_step_tag needs rows*W elements")
+    if d_t_nth is not None and d_t_nth.numel() < rows:
+        raise ValueError("d_t_nth needs one element per row")
+    st = lib().psync_step_device(ctypes.byref(step), _dptr(d_arrival, torch.float32, "d_arrival"),
+                                 _dptr(d_step_tag, torch.int32, "d_step_tag"), t,
+                                 _dptr(d_t_nth, torch.float32, "d_t_nth"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_step_device")
     return st
 
 

@@ -170,6 +170,25 @@ PSYNC_API int psync_aggregate_update(const psync_step* step, void* stream) {
   return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
 }
 
+PSYNC_API int psync_step_device(const psync_step* step, const float* d_arrival, const int32_t* d_step_tag, int32_t t,
+                      float* d_t_nth, void* stream) {
+  const int st = check_step(step, true);
+  if (st != PSYNC_OK) return st;
+  if (d_arrival == nullptr || step->d_status == nullptr || step->d_n_kept != nullptr) return PSYNC_EINVAL;
+  if (step->kept_stride != 0 && step->kept_stride != step->N) return PSYNC_EINVAL;  // the selection writes rows of N
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const int32_t rows = step->per_shard ? step->M : 1;
+  if (psync::launch_select_first_n(d_arrival, d_step_tag, t, step->N, step->W, rows, const_cast<int32_t*>(step->d_kept),
+                                   d_t_nth, const_cast<int32_t*>(step->d_status), s) != cudaSuccess)
+    return PSYNC_ECUDA;
+  if (step->P == 0) return PSYNC_OK;
+  const FusedParams p = make_params(step, 0, step->P, step->d_grads, step->d_kept, step->d_status);
+  return psync::launch_fused(p, step->grad_dtype, step->opt, step->ema_mode, step->variant, step->grid_ctas, s) ==
+                 cudaSuccess
+             ? PSYNC_OK
+             : PSYNC_ECUDA;
+}
+
 PSYNC_API int psync_order_by_arrival(const float* d_arrival, int32_t W, int32_t* d_order, int32_t* d_n_arrived,
                            void* stream) {
   if (d_arrival == nullptr || d_order == nullptr || d_n_arrived == nullptr) return PSYNC_EINVAL;

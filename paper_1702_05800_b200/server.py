@@ -1,8 +1,8 @@
 """ParameterServerStep: device buffers + the two calls of one step (plumbing only, no arithmetic).
 
 Holds theta / ema / optimizer state, the kept[] / status / t_Nth outputs of the selection kernel and
-the device pointer table of the W gradient buffers, and enqueues psync_select_first_n followed by
-psync_aggregate_update on one stream with no host synchronisation in between (Alg. 4).
+the device pointer table of the W gradient buffers, and enqueues the selection followed by the fused update
+(psync_step_device) on one stream with no host synchronisation in between (Alg. 4).
 """
 from __future__ import annotations
 
@@ -57,9 +57,7 @@ class ParameterServerStep:
             raise RuntimeError("set_gradients() first")
         if self._step is None or self._step.gamma_t != np.float32(gamma_t):
             self._build(gamma_t)
-        B.psync_select_first_n(d_arrival, self.N, self.b, self.d_kept, self.d_status, self.d_t_nth, d_step_tag, t,
-                               stream)
-        B.psync_aggregate_update(self._step, stream)
+        B.psync_step_device(self._step, d_arrival, self.d_t_nth, d_step_tag, t, stream)   # K1 + K2, one C call
 
     def aggregate_only(self, gamma_t: float, stream=None) -> None:
         if self._step is None or self._step.gamma_t != np.float32(gamma_t):

@@ -184,3 +184,64 @@ def test_back_to_back_steps_without_host_sync(P):
     pair.compare(RTOL_FREE_100, ATOL_STEP, "back-to-back free run")
     st, kept, tn = oracle.select_first_n(arrivals_h[T - 1], cfg.N, cfg.b)
     assert np.array_equal(ps.d_kept.cpu().numpy(), kept) and float(ps.d_t_nth.item()) == tn
+
+
+# ------------------------------------------------------------------ one-call step and CUDA graph capture
+def test_step_device_equals_the_two_calls_bitwise():
+    cfg = synth.scaled(synth.PAPER_RMSPROP, 150_001)
+    arrival = synth.arrival_times(cfg, 0)
+    out = []
+    for one_call in (True, False):
+        pair = Pair(cfg)
+        grads = pair.gradients(0)
+        pair.ps.set_gradients(grads)
+        d_arr = torch.from_numpy(arrival).to(DEV)
+        if one_call:
+            pair.ps.step(d_arr, cfg.gamma)
+        else:
+            psync.psync_select_first_n(d_arr, cfg.N, cfg.b, pair.ps.d_kept, pair.ps.d_status, pair.ps.d_t_nth)
+            pair.ps.aggregate_only(cfg.gamma)
+        torch.cuda.synchronize()
+        out.append([to_np(getattr(pair.ps, n)) for n in ("theta", "ema", "state0", "state1", "d_kept", "d_t_nth")])
+    for a, b_ in zip(*out):
+        assert np.array_equal(a, b_)
+
+
+@pytest.mark.parametrize("cfg", [synth.TINY, synth.scaled(synth.PAPER_RMSPROP, 40_003)])
+def test_cuda_graph_capture_and_replay_matches_oracle(cfg):
+    """The step is capturable (no synchronising call inside): capture 3 steps reading a fixed arrival buffer,
+    replay twice with fresh arrival times, compare with the oracle after every replay."""
+    pair = Pair(cfg)
+    grads = pair.gradients(0)
+    pair.ps.set_gradients(grads)
+    steps_per_graph = 3
+    d_arr = torch.zeros(steps_per_graph, cfg.W, dtype=torch.float32, device=DEV)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        d_arr.copy_(torch.from_numpy(np.stack([synth.arrival_times(cfg, 100 + i) for i in range(steps_per_graph)])))
+        snapshot = {n: (None if getattr(pair.ps, n) is None else getattr(pair.ps, n).clone())
+                    for n in ("theta", "ema", "state0", "state1")}
+        pair.ps.step(d_arr[0], cfg.gamma, stream=side)                     # warm-up outside capture
+        side.synchronize()
+        for n, v in snapshot.items():                                      # undo the warm-up step
+            if v is not None:
+                getattr(pair.ps, n).copy_(v)
+        with torch.cuda.graph(graph, stream=side):
+            for i in range(steps_per_graph):
+                pair.ps.step(d_arr[i], cfg.gamma, stream=side)
+    torch.cuda.synchronize()
+    s = 0
+    for replay in range(2):
+        arr = np.stack([synth.arrival_times(cfg, s + i) for i in range(steps_per_graph)])
+        d_arr.copy_(torch.from_numpy(arr))
+        graph.replay()
+        torch.cuda.synchronize()
+        for i in range(steps_per_graph):
+            st, kept, _ = pair.oracle_step(grads, arr[i])
+            assert st == 0
+        assert np.array_equal(pair.ps.d_kept.cpu().numpy(), kept)
+        pair.compare(RTOL_STEP * steps_per_graph, ATOL_STEP, f"graph replay {replay}")
+        pair.sync_host_from_gpu()
+        s += steps_per_graph
