@@ -58,8 +58,12 @@ def lib() -> ctypes.CDLL:
         L.oracle_aggregate_update_rows.restype = ctypes.c_int
         L.oracle_order_by_arrival.argtypes = [vp, i32, vp, vp]
         L.oracle_order_by_arrival.restype = ctypes.c_int
-        L.oracle_async_apply.argtypes = [i64, i32, vp, i32, i32, vp, ctypes.c_int, vp, vp, vp, vp, vp, vp,
+        L.oracle_async_apply.argtypes = [i64, i32, vp, i32, i32, vp, ctypes.c_int, vp, vp, vp, vp, vp, vp, vp,
                                          ctypes.c_int, ctypes.c_int, f32, f32, f32, f32, f32]
+        L.oracle_lr_schedule.argtypes = [f32, f32, i64, i32, ctypes.c_double, vp]
+        L.oracle_lr_schedule.restype = ctypes.c_int
+        L.oracle_clip_scales.argtypes = [vp, i32, i64, ctypes.c_int, f32, vp]
+        L.oracle_clip_scales.restype = ctypes.c_int
         L.oracle_async_apply.restype = ctypes.c_int
         L.oracle_accumulate.argtypes = [vp, vp, ctypes.c_int, i64]
         L.oracle_accumulate.restype = ctypes.c_int
@@ -199,7 +203,28 @@ def order_by_arrival(arrival):
     return order[:int(n[0])].copy()
 
 
-def async_apply(shard_off, grads, order, theta, ema=None, state0=None, state1=None, gammas=None, opt=SGD,
+def lr_schedule(gamma0, beta, t0, K, s):
+    """gamma_0 beta^(t s) for t = t0 .. t0+K-1 -> float32 [K]."""
+    out = np.zeros(K, dtype=np.float32)
+    if lib().oracle_lr_schedule(gamma0, beta, t0, K, s, _ptr(out)) != OK:
+        raise ValueError("oracle_lr_schedule: invalid arguments")
+    return out
+
+
+def clip_scales(grads, clip):
+    """Global-norm clip factor clip / max(||G_k||, clip) of every worker's buffer -> float32 [W]."""
+    W = len(grads)
+    gd = _grad_dtype(grads)
+    for k, g in enumerate(grads):
+        _chk(g, grads[0].dtype, f"grads[{k}]", grads[0].size)
+    ptrs = (ctypes.c_void_p * W)(*[g.ctypes.data for g in grads])
+    out = np.zeros(W, dtype=np.float32)
+    if lib().oracle_clip_scales(ctypes.cast(ptrs, ctypes.c_void_p), W, grads[0].size, gd, clip, _ptr(out)) != OK:
+        raise ValueError("oracle_clip_scales: invalid arguments")
+    return out
+
+
+def async_apply(shard_off, grads, order, theta, ema=None, state0=None, state1=None, gammas=None, gscales=None, opt=SGD,
                 ema_mode=EMA_PRE, gamma_t=0.0, alpha=0.0, mu=0.0, rho=0.0, eps=0.0):
     """len(order) iterations of Alg. 2, one gradient each, in place."""
     P = theta.size
@@ -211,11 +236,13 @@ def async_apply(shard_off, grads, order, theta, ema=None, state0=None, state1=No
         _chk(g, grads[0].dtype, f"grads[{k}]", P)
     _chk(order, np.int32, "order")
     _chk(gammas, np.float32, "gammas", order.size)
+    _chk(gscales, np.float32, "gscales", order.size)
     for nm, a in (("theta", theta), ("ema", ema), ("state0", state0), ("state1", state1)):
         _chk(a, np.float32, nm, P)
     ptrs = (ctypes.c_void_p * W)(*[g.ctypes.data for g in grads])
     return lib().oracle_async_apply(P, M, _ptr(shard_off), order.size, W, ctypes.cast(ptrs, ctypes.c_void_p), gd,
-                                    _ptr(order), _ptr(gammas), _ptr(theta), _ptr(ema), _ptr(state0), _ptr(state1),
+                                    _ptr(order), _ptr(gammas), _ptr(gscales), _ptr(theta), _ptr(ema), _ptr(state0),
+                                    _ptr(state1),
                                     opt, ema_mode, gamma_t, alpha, mu, rho, eps)
 
 

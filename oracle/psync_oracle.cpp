@@ -369,7 +369,7 @@ int oracle_order_by_arrival(const float* arrival, int32_t W, int32_t* order, int
 }
 
 // oracle_async_apply: K iterations of Alg. 2, one per gradient, in the order given:
-//   for i = 0..K-1:  G = grads[order[i]];  gamma = gammas ? gammas[i] : gamma_t
+//   for i = 0..K-1:  G = grads[order[i]] (times gscales[i] if given);  gamma = gammas ? gammas[i] : gamma_t
 //                    every element: optimizer step with G (no averaging: the divisor is 1), then EMA
 // written as the paper's loop reads -- outer loop over arrivals, inner loop over the parameters of
 // each server j -- with theta / state / ema stored as fp32 after every iteration (they are the
@@ -377,8 +377,8 @@ int oracle_order_by_arrival(const float* arrival, int32_t W, int32_t* order, int
 // the synchronous step (readings R3, R5, R6); EMA_PRE is the literal indexing of L87.
 int oracle_async_apply(int64_t P, int32_t M, const int64_t* shard_off, int32_t K, int32_t W,
                        const void* const* grads, int grad_dtype, const int32_t* order, const float* gammas,
-                       float* theta, float* ema, float* state0, float* state1, int opt, int ema_mode,
-                       float gamma_t, float alpha, float mu, float rho, float eps) {
+                       const float* gscales, float* theta, float* ema, float* state0, float* state1, int opt,
+                       int ema_mode, float gamma_t, float alpha, float mu, float rho, float eps) {
   if (!args_ok(P, M, shard_off, 1, opt, ema_mode, theta, ema, state0, state1)) return ORACLE_EINVAL;
   if (!grads || !order || K < 0 || K > W) return ORACLE_EINVAL;
   if (grad_dtype != ORACLE_F32 && grad_dtype != ORACLE_BF16) return ORACLE_EINVAL;
@@ -386,7 +386,10 @@ int oracle_async_apply(int64_t P, int32_t M, const int64_t* shard_off, int32_t K
     if (order[i] < 0 || order[i] >= W || !grads[order[i]]) return ORACLE_EINVAL;
   for (int32_t i = 0; i < K; ++i) {  // iteration t+i: "wait for gradient G from any worker"
     const void* G = grads[order[i]];
-    const Coeffs c = make_coeffs(1, gammas ? gammas[i] : gamma_t, alpha, mu, rho, eps);
+    Coeffs c = make_coeffs(1, gammas ? gammas[i] : gamma_t, alpha, mu, rho, eps);
+    // global-norm clipping (L313; R22): the i-th gradient is scaled by gscales[i] before the update.
+    // apply_element multiplies the gradient by c.inv_N, which is 1 here, so the clip factor takes its place.
+    if (gscales) c.inv_N = static_cast<double>(gscales[i]);
     for (int32_t j = 0; j < M; ++j) {  // parameter server j
       const int64_t lo = shard_off[j], hi = shard_off[j + 1];
 #ifdef _OPENMP
@@ -395,6 +398,45 @@ int oracle_async_apply(int64_t P, int32_t M, const int64_t* shard_off, int32_t K
       for (int64_t e = lo; e < hi; ++e)
         apply_element(grad_at(G, grad_dtype, e), c, opt, ema_mode, theta, ema, state0, state1, e);
     }
+  }
+  return ORACLE_OK;
+}
+
+// =============================================================================================
+// NEXT-4 helpers.
+//
+// Learning-rate schedule of A.2 / A.3 (L305, L315): gamma_t = gamma_0 * beta^(t * s) with
+// s = N/(2T) for Sync-Opt and s = 1/(2T) for Async-Opt, T = |X|/B mini-batches per epoch
+// ("exponentially decreased with decay rate beta = 0.94 as gamma_0 beta^(tN/(2T))").  out[i] is the
+// rate of iteration t0 + i, computed in double and rounded once to fp32.
+// =============================================================================================
+int oracle_lr_schedule(float gamma0, float beta, int64_t t0, int32_t K, double s, float* out) {
+  if (!out || K < 0 || t0 < 0 || !(beta > 0.0f)) return ORACLE_EINVAL;
+  for (int32_t i = 0; i < K; ++i)
+    out[i] = static_cast<float>(static_cast<double>(gamma0) *
+                                std::pow(static_cast<double>(beta), static_cast<double>(t0 + i) * s));
+  return ORACLE_OK;
+}
+
+// Global-norm clipping of Async-Opt (A.3, L313: "collect the gradient across all layers of the deep
+// model, compute the global norm ||G|| and then clip all gradient accordingly").  The paper gives no
+// formula; reading R22 (the TensorFlow operation it ran on, L197): G <- G * clip / max(||G||, clip),
+// ||G|| the Euclidean norm over ALL P elements of one worker's gradient.  scales[k] is that factor for
+// worker k's buffer, computed in double and rounded once to fp32 (1 when the norm is within the bound;
+// a non-finite norm gives a NaN/0 factor per IEEE, as the definition reads).
+int oracle_clip_scales(const void* const* grads, int32_t W, int64_t P, int grad_dtype, float clip, float* scales) {
+  if (!grads || !scales || W < 1 || P < 0 || !(clip > 0.0f)) return ORACLE_EINVAL;
+  if (grad_dtype != ORACLE_F32 && grad_dtype != ORACLE_BF16) return ORACLE_EINVAL;
+  for (int32_t k = 0; k < W; ++k) {
+    if (!grads[k]) return ORACLE_EINVAL;
+    double sumsq = 0.0;
+    for (int64_t i = 0; i < P; ++i) {
+      const double g = grad_at(grads[k], grad_dtype, i);
+      sumsq += g * g;
+    }
+    const double norm = std::sqrt(sumsq);
+    const double c = static_cast<double>(clip);
+    scales[k] = static_cast<float>(c / std::max(norm, c));
   }
   return ORACLE_OK;
 }
