@@ -24,7 +24,8 @@ PSYNC_EMA_POST, PSYNC_EMA_PRE, PSYNC_EMA_OFF = 0, 1, 2
 PSYNC_MAX_WORKERS = 1024
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
-           "psync_select_timeout", "psync_aggregate_update", "psync_ema", "psync_order_by_arrival", "psync_async_apply", "psync_step_device",
+           "psync_select_timeout", "psync_aggregate_update", "psync_ema", "psync_order_by_arrival", "psync_async_apply", "psync_step_device", "psync_clip_workspace_bytes",
+           "psync_clip_scales", "psync_lr_schedule",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_launch_geometry", "psync_probe_read",
            "psync_probe_copy")
 
@@ -77,7 +78,13 @@ def lib() -> ctypes.CDLL:
         L.psync_step_device.restype = ctypes.c_int
         L.psync_order_by_arrival.argtypes = [vp, i32, vp, vp, vp]
         L.psync_order_by_arrival.restype = ctypes.c_int
-        L.psync_async_apply.argtypes = [ctypes.POINTER(psync_step), vp, vp]
+        L.psync_async_apply.argtypes = [ctypes.POINTER(psync_step), vp, vp, vp]
+        L.psync_clip_workspace_bytes.argtypes = [i32, i64, i32]
+        L.psync_clip_workspace_bytes.restype = ctypes.c_size_t
+        L.psync_clip_scales.argtypes = [vp, i32, i64, i32, f32, vp, vp, ctypes.c_size_t, vp]
+        L.psync_clip_scales.restype = ctypes.c_int
+        L.psync_lr_schedule.argtypes = [f32, f32, i64, i32, ctypes.c_double, vp, vp]
+        L.psync_lr_schedule.restype = ctypes.c_int
         L.psync_async_apply.restype = ctypes.c_int
         L.psync_ema.argtypes = [vp, vp, i64, f32, vp]
         L.psync_ema.restype = ctypes.c_int
@@ -286,10 +293,42 @@ def psync_order_by_arrival(d_arrival: torch.Tensor, W: int, d_order: torch.Tenso
     return st
 
 
-def psync_async_apply(step: psync_step, d_gamma: Optional[torch.Tensor] = None, stream=None,
+def psync_clip_workspace_bytes(W: int, P: int, grad_dtype: int) -> int:
+    return lib().psync_clip_workspace_bytes(W, P, grad_dtype)
+
+
+def psync_clip_scales(table: "GradTable", clip: float, d_scales: torch.Tensor, d_work: torch.Tensor, stream=None,
                       check: bool = True) -> int:
+    """Global-norm clip factors of the W buffers (include/psync.h: psync_clip_scales)."""
+    if d_scales.numel() < table.W:
+        raise ValueError("d_scales needs W elements")
+    st = lib().psync_clip_scales(_dptr(table.d_ptrs, torch.int64, "d_grads"), table.W, table.buffers[0].numel(),
+                                 table.grad_dtype, clip, _dptr(d_scales, torch.float32, "d_scales"),
+                                 _dptr(d_work, None, "d_work"), d_work.numel() * d_work.element_size(),
+                                 _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_clip_scales")
+    return st
+
+
+def psync_lr_schedule(gamma0: float, beta: float, t0: int, K: int, s: float, d_gamma: torch.Tensor, stream=None,
+                      check: bool = True) -> int:
+    """gamma_0 beta^((t0+i) s), i < K (include/psync.h: psync_lr_schedule)."""
+    if d_gamma.numel() < K:
+        raise ValueError("d_gamma needs K elements")
+    st = lib().psync_lr_schedule(gamma0, beta, t0, K, s, _dptr(d_gamma, torch.float32, "d_gamma"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_lr_schedule")
+    return st
+
+
+def psync_async_apply(step: psync_step, d_gamma: Optional[torch.Tensor] = None, stream=None, check: bool = True,
+                      d_gscale: Optional[torch.Tensor] = None) -> int:
     """K iterations of Alg. 2 in one pass (include/psync.h: psync_async_apply)."""
-    st = lib().psync_async_apply(ctypes.byref(step), _dptr(d_gamma, torch.float32, "d_gamma"), _stream(stream))
+    if d_gscale is not None and d_gscale.numel() < step.W:
+        raise ValueError("d_gscale needs W elements (indexed by worker)")
+    st = lib().psync_async_apply(ctypes.byref(step), _dptr(d_gamma, torch.float32, "d_gamma"),
+                                 _dptr(d_gscale, torch.float32, "d_gscale"), _stream(stream))
     if check and st != PSYNC_OK:
         raise PsyncError(st, "psync_async_apply")
     return st

@@ -35,6 +35,7 @@ __global__ void __launch_bounds__(THREADS, MINB) async_apply_kernel(const FusedP
   constexpr int Q = E / 4;
   __shared__ const char* s_ptr[kMaxWorkers];
   __shared__ float s_gamma[kMaxWorkers];
+  __shared__ float s_scale[kMaxWorkers];  // global-norm clip factor of the i-th gradient (1 without clipping)
 
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -45,8 +46,10 @@ __global__ void __launch_bounds__(THREADS, MINB) async_apply_kernel(const FusedP
 
   unsigned misalign = 0;
   for (int i = threadIdx.x; i < K; i += THREADS) {
-    const char* g = static_cast<const char*>(p.grads[p.kept[i]]);  // kept[] holds the arrival order
+    const int k = p.kept[i];  // kept[] holds the arrival order
+    const char* g = static_cast<const char*>(p.grads[k]);
     s_ptr[i] = g;
+    s_scale[i] = p.gscales ? p.gscales[k] : 1.0f;  // indexed by WORKER (L313: each worker clips its own gradient)
     s_gamma[i] = p.gammas ? p.gammas[i] : p.gamma;  // gamma_t of iteration t+i
     misalign |= static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 15u;
   }
@@ -76,18 +79,18 @@ __global__ void __launch_bounds__(THREADS, MINB) async_apply_kernel(const FusedP
       for (int v = 0; v < U; ++v) r[v] = ldg_stream16(s_ptr[i + v] + u * 16);
 #pragma unroll
       for (int v = 0; v < U; ++v) {
-        const float gamma = s_gamma[i + v];
+        const float gamma = s_gamma[i + v], scale = s_scale[i + v];
 #pragma unroll
         for (int e = 0; e < E; ++e)
-          update_element_g<OPT, EMA>(unit_element<BF16>(r[v], e), 1.0f, gamma, th[e], em[e], a0[e], a1[e], p);
+          update_element_g<OPT, EMA>(unit_element<BF16>(r[v], e), scale, gamma, th[e], em[e], a0[e], a1[e], p);
       }
     }
     for (; i < K; ++i) {
       const uint4 r = ldg_stream16(s_ptr[i] + u * 16);
-      const float gamma = s_gamma[i];
+      const float gamma = s_gamma[i], scale = s_scale[i];
 #pragma unroll
       for (int e = 0; e < E; ++e)
-        update_element_g<OPT, EMA>(unit_element<BF16>(r, e), 1.0f, gamma, th[e], em[e], a0[e], a1[e], p);
+        update_element_g<OPT, EMA>(unit_element<BF16>(r, e), scale, gamma, th[e], em[e], a0[e], a1[e], p);
     }
 
 #pragma unroll
@@ -112,7 +115,7 @@ __global__ void __launch_bounds__(THREADS, MINB) async_apply_kernel(const FusedP
       float a0 = (OPT != OPT_SGD) ? p.s0[e] : 0.f;
       float a1 = (OPT == OPT_RMSPROP_MOM) ? p.s1[e] : 0.f;
       for (int i = 0; i < K; ++i)
-        update_element_g<OPT, EMA>(load_grad_scalar<BF16>(s_ptr[i], e), 1.0f, s_gamma[i], th, em, a0, a1, p);
+        update_element_g<OPT, EMA>(load_grad_scalar<BF16>(s_ptr[i], e), s_scale[i], s_gamma[i], th, em, a0, a1, p);
       p.theta[e] = th;
       if (EMA != EMA_OFF) p.ema[e] = em;
       if (OPT != OPT_SGD) p.s0[e] = a0;
@@ -184,7 +187,7 @@ cudaError_t async_geometry(int dtype, int grid_ctas, int64_t P, FusedGeometry* o
   const int E = dtype == 1 ? 8 : 4;
   out->block = s.threads;
   out->tile_elems = s.threads * E;
-  out->smem_bytes = static_cast<int>((sizeof(const char*) + sizeof(float)) * kMaxWorkers);
+  out->smem_bytes = static_cast<int>((sizeof(const char*) + 2 * sizeof(float)) * kMaxWorkers);
   int64_t grid = grid_ctas > 0 ? grid_ctas : (P / E + s.threads - 1) / s.threads;  // one unit per thread
   if (grid > 0x7FFFFFFF) grid = 0x7FFFFFFF;
   if (grid < 1) grid = 1;

@@ -1,0 +1,163 @@
+// K5 / K6: the two helpers the asynchronous baseline of the paper needs around K4.
+//
+// K5 -- global-norm clipping (PAPER.md A.3, L313: "gradient clipping is also needed for stabilization, which
+// requires each worker to collect the gradient across all layers of the deep model, compute the global norm ||G||
+// and then clip all gradient accordingly").  Reading R22: G <- G * clip / max(||G||_2, clip).  Only the FACTOR is
+// computed here; K4 applies it while it streams the gradient (it takes the place of the 1/N multiplier), so the
+// clipped gradient is never written.  The norm needs one extra pass over the W buffers (W*P*sizeof(grad) bytes, an
+// HBM-bound stream) -- the paper's point that clipping serialises the update behind the whole gradient.
+// Deterministic: fixed chunking, fixed-order tree reductions, no atomics.
+//
+// K6 -- gamma_t = gamma_0 * beta^(t s) (A.2 L305, A.3 L315) for K consecutive iterations, for K4's d_gamma table.
+
+#include "psync_device.cuh"
+
+namespace psync {
+namespace {
+
+using namespace dev;
+
+constexpr int kClipThreads = 256;
+constexpr int kClipUnitsPerThread = 32;                                   // 16-byte units per thread per chunk
+constexpr int64_t kClipChunkUnits = int64_t{kClipThreads} * kClipUnitsPerThread;  // 8192 units = 128 KB per CTA
+
+__device__ __forceinline__ double block_sum(double v, double* s_warp) {
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) v += __shfl_down_sync(0xFFFFFFFFu, v, d);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) s_warp[warp] = v;
+  __syncthreads();
+  double total = 0.0;
+  if (threadIdx.x == 0)
+    for (int w = 0; w < (blockDim.x + 31) / 32; ++w) total += s_warp[w];  // fixed order
+  return total;  // valid in thread 0
+}
+
+template <bool BF16>
+__device__ __forceinline__ float unit_sumsq(const uint4& r) {
+  float s = 0.f;
+  if (BF16) {
+    const uint32_t w[4] = {r.x, r.y, r.z, r.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float lo = __uint_as_float(w[i] << 16), hi = __uint_as_float(w[i] & 0xFFFF0000u);
+      s = __fmaf_rn(lo, lo, s);
+      s = __fmaf_rn(hi, hi, s);
+    }
+  } else {
+    const float x = __uint_as_float(r.x), y = __uint_as_float(r.y), z = __uint_as_float(r.z), w = __uint_as_float(r.w);
+    s = __fmaf_rn(x, x, s);
+    s = __fmaf_rn(y, y, s);
+    s = __fmaf_rn(z, z, s);
+    s = __fmaf_rn(w, w, s);
+  }
+  return s;
+}
+
+// grid (chunks, W): CTA (c, k) writes the sum of squares of chunk c of worker k's buffer to work[k * chunks + c].
+template <bool BF16>
+__global__ void __launch_bounds__(kClipThreads) sumsq_chunks_kernel(const void* const* __restrict__ grads, int64_t P,
+                                                                    double* __restrict__ work) {
+  constexpr int E = BF16 ? 8 : 4;
+  __shared__ double s_warp[kClipThreads / 32];
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const char* g = static_cast<const char*>(grads[blockIdx.y]);
+  const int64_t n_units = ((reinterpret_cast<uintptr_t>(g) & 15u) == 0) ? P / E : 0;  // misaligned: all scalar
+  const int64_t u0 = static_cast<int64_t>(blockIdx.x) * kClipChunkUnits;
+  double acc = 0.0;
+  constexpr int U = 8;
+  for (int b = 0; b < kClipUnitsPerThread; b += U) {
+    uint4 r[U];
+    bool on[U];
+#pragma unroll
+    for (int v = 0; v < U; ++v) {
+      const int64_t u = u0 + static_cast<int64_t>(b + v) * kClipThreads + threadIdx.x;
+      on[v] = u < n_units;
+      r[v] = on[v] ? ldg_stream16(g + u * 16) : make_uint4(0u, 0u, 0u, 0u);
+    }
+#pragma unroll
+    for (int v = 0; v < U; ++v)
+      if (on[v]) acc += static_cast<double>(unit_sumsq<BF16>(r[v]));  // fp32 inside a 16-byte unit, double across
+  }
+  // elements the vector path does not cover (tail, or everything if misaligned): chunk 0 takes them
+  if (blockIdx.x == 0)
+    for (int64_t i = n_units * E + threadIdx.x; i < P; i += kClipThreads) {
+      const float x = load_grad_scalar<BF16>(g, i);
+      acc += static_cast<double>(x) * static_cast<double>(x);
+    }
+  const double total = block_sum(acc, s_warp);
+  if (threadIdx.x == 0) work[static_cast<int64_t>(blockIdx.y) * gridDim.x + blockIdx.x] = total;
+}
+
+// one CTA per worker: fixed-order sum of its chunk partials, then the clip factor
+__global__ void __launch_bounds__(kClipThreads) clip_finalize_kernel(const double* __restrict__ work, int chunks,
+                                                                     float clip, float* __restrict__ scales) {
+  __shared__ double s_warp[kClipThreads / 32];
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const double* row = work + static_cast<int64_t>(blockIdx.x) * chunks;
+  double acc = 0.0;
+  for (int c = threadIdx.x; c < chunks; c += kClipThreads) acc += row[c];
+  const double total = block_sum(acc, s_warp);
+  if (threadIdx.x == 0) {
+    const double c = static_cast<double>(clip);
+    scales[blockIdx.x] = static_cast<float>(c / fmax(sqrt(total), c));
+  }
+}
+
+__global__ void lr_schedule_kernel(float gamma0, float beta, int64_t t0, int32_t K, double s, float* __restrict__ out) {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < K)
+    out[i] = static_cast<float>(static_cast<double>(gamma0) *
+                                pow(static_cast<double>(beta), static_cast<double>(t0 + i) * s));
+}
+
+int clip_chunks(int64_t P, int dtype) {
+  const int E = dtype == 1 ? 8 : 4;
+  const int64_t c = (P / E + kClipChunkUnits - 1) / kClipChunkUnits;
+  return static_cast<int>(c < 1 ? 1 : c);
+}
+
+void pdl_config(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* attr, dim3 grid, dim3 block, cudaStream_t stream) {
+  *cfg = {};
+  cfg->gridDim = grid;
+  cfg->blockDim = block;
+  cfg->stream = stream;
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg->attrs = attr;
+  cfg->numAttrs = 1;
+}
+
+}  // namespace
+
+size_t clip_workspace_bytes(int32_t W, int64_t P, int dtype) {
+  return sizeof(double) * static_cast<size_t>(W) * static_cast<size_t>(clip_chunks(P, dtype));
+}
+
+cudaError_t launch_clip_scales(const void* const* d_grads, int32_t W, int64_t P, int dtype, float clip, float* d_scales,
+                               void* d_work, cudaStream_t stream) {
+  const int chunks = clip_chunks(P, dtype);
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute attr[1];
+  pdl_config(&cfg, attr, dim3(static_cast<unsigned>(chunks), static_cast<unsigned>(W)), dim3(kClipThreads), stream);
+  double* work = static_cast<double*>(d_work);
+  cudaError_t err = dtype == 1 ? cudaLaunchKernelEx(&cfg, sumsq_chunks_kernel<true>, d_grads, P, work)
+                               : cudaLaunchKernelEx(&cfg, sumsq_chunks_kernel<false>, d_grads, P, work);
+  if (err != cudaSuccess) return err;
+  pdl_config(&cfg, attr, dim3(static_cast<unsigned>(W)), dim3(kClipThreads), stream);
+  return cudaLaunchKernelEx(&cfg, clip_finalize_kernel, static_cast<const double*>(work), chunks, clip, d_scales);
+}
+
+cudaError_t launch_lr_schedule(float gamma0, float beta, int64_t t0, int32_t K, double s, float* d_gamma,
+                               cudaStream_t stream) {
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute attr[1];
+  pdl_config(&cfg, attr, dim3(static_cast<unsigned>((K + 127) / 128)), dim3(128), stream);
+  return cudaLaunchKernelEx(&cfg, lr_schedule_kernel, gamma0, beta, t0, K, s, d_gamma);
+}
+
+}  // namespace psync

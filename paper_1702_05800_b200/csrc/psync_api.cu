@@ -67,6 +67,7 @@ FusedParams make_params(const psync_step* s, int64_t first, int64_t count, const
   p.shard_off = s->d_shard_off;
   p.n_kept = s->d_n_kept;
   p.gammas = nullptr;
+  p.gscales = nullptr;
   p.base_aligned = aligned16(p.theta) && (p.ema == nullptr || aligned16(p.ema)) && (p.s0 == nullptr || aligned16(p.s0)) &&
                    (p.s1 == nullptr || aligned16(p.s1));
   return p;
@@ -199,16 +200,43 @@ PSYNC_API int psync_order_by_arrival(const float* d_arrival, int32_t W, int32_t*
              : PSYNC_ECUDA;
 }
 
-PSYNC_API int psync_async_apply(const psync_step* step, const float* d_gamma, void* stream) {
+PSYNC_API int psync_async_apply(const psync_step* step, const float* d_gamma, const float* d_gscale, void* stream) {
   const int st = check_step(step, true);
   if (st != PSYNC_OK && !(st == PSYNC_EUNSUPPORTED && step->per_shard == 0)) return st;  // variant is ignored here
   if (step->per_shard != 0) return PSYNC_EUNSUPPORTED;
   if (step->P == 0) return PSYNC_OK;
   FusedParams p = make_params(step, 0, step->P, step->d_grads, step->d_kept, step->d_status);
   p.gammas = d_gamma;
+  p.gscales = d_gscale;
   const cudaError_t err = psync::launch_async_apply(p, step->grad_dtype, step->opt, step->ema_mode, step->grid_ctas,
                                                     static_cast<cudaStream_t>(stream));
   return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
+}
+
+PSYNC_API size_t psync_clip_workspace_bytes(int32_t W, int64_t P, int32_t grad_dtype) {
+  if (W < 1 || W > PSYNC_MAX_WORKERS || P < 0 || (grad_dtype != PSYNC_F32 && grad_dtype != PSYNC_BF16)) return 0;
+  return psync::clip_workspace_bytes(W, P, grad_dtype);
+}
+
+PSYNC_API int psync_clip_scales(const void* const* d_grads, int32_t W, int64_t P, int32_t grad_dtype, float clip,
+                      float* d_scales, void* d_work, size_t work_bytes, void* stream) {
+  if (d_grads == nullptr || d_scales == nullptr || d_work == nullptr) return PSYNC_EINVAL;
+  if (W < 1 || W > PSYNC_MAX_WORKERS || P < 0 || !(clip > 0.0f)) return PSYNC_EINVAL;
+  if (grad_dtype != PSYNC_F32 && grad_dtype != PSYNC_BF16) return PSYNC_EINVAL;
+  if (work_bytes < psync::clip_workspace_bytes(W, P, grad_dtype) || (reinterpret_cast<uintptr_t>(d_work) & 7u) != 0)
+    return PSYNC_EINVAL;
+  return psync::launch_clip_scales(d_grads, W, P, grad_dtype, clip, d_scales, d_work, static_cast<cudaStream_t>(stream)) ==
+                 cudaSuccess
+             ? PSYNC_OK
+             : PSYNC_ECUDA;
+}
+
+PSYNC_API int psync_lr_schedule(float gamma0, float beta, int64_t t0, int32_t K, double s, float* d_gamma, void* stream) {
+  if (K < 0 || t0 < 0 || !(beta > 0.0f) || (K > 0 && d_gamma == nullptr)) return PSYNC_EINVAL;
+  if (K == 0) return PSYNC_OK;
+  return psync::launch_lr_schedule(gamma0, beta, t0, K, s, d_gamma, static_cast<cudaStream_t>(stream)) == cudaSuccess
+             ? PSYNC_OK
+             : PSYNC_ECUDA;
 }
 
 PSYNC_API int psync_ema(float* d_ema, const float* d_theta, int64_t P, float alpha, void* stream) {

@@ -1,0 +1,150 @@
+"""GPU parity for the NEXT-4 helpers through the C ABI: learning-rate schedule, global-norm
+clip factors and the clipped asynchronous update, against the CPU oracle."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1702_05800_b200 as psync
+from paper_1702_05800_b200 import synth
+
+from _harness import ATOL_STEP, STATE_NAMES, assert_close, to_np
+from test_gpu_async import BASE, AsyncPair, rtol_async
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def ulp_diff(a, b):
+    ia = np.asarray(a, np.float32).view(np.int32).astype(np.int64)
+    ib = np.asarray(b, np.float32).view(np.int32).astype(np.int64)
+    return np.abs(ia - ib)
+
+
+@pytest.mark.parametrize("gamma0,beta,t0,K,s", [(4.5, 0.94, 0, 200, 100 / (2 * 40037.0)), (0.045, 0.94, 10**6, 1024, 1 / 80074.0),
+                                                (0.1, 0.5, 3, 2, 1.0), (2.25, 0.94, 12345, 1, 50 / 80074.0), (1.0, 1.0, 0, 33, 9.0)])
+def test_lr_schedule_matches_oracle(gamma0, beta, t0, K, s):
+    d = torch.full((K + 2,), -1.0, dtype=torch.float32, device=DEV)
+    psync.psync_lr_schedule(gamma0, beta, t0, K, s, d)
+    want = oracle.lr_schedule(gamma0, beta, t0, K, s)
+    got = d.cpu().numpy()
+    assert ulp_diff(got[:K], want).max() <= 1          # double pow on both sides, one rounding to fp32
+    assert (got[K:] == -1.0).all()
+    assert psync.psync_lr_schedule(gamma0, beta, t0, 0, s, d) == psync.PSYNC_OK
+    L = psync.binding.lib()
+    assert L.psync_lr_schedule(0.1, 0.0, 0, 1, 1.0, d.data_ptr(), None) == psync.PSYNC_EINVAL
+    assert L.psync_lr_schedule(0.1, 0.5, -1, 1, 1.0, d.data_ptr(), None) == psync.PSYNC_EINVAL
+    assert L.psync_lr_schedule(0.1, 0.5, 0, 1, 1.0, None, None) == psync.PSYNC_EINVAL
+
+
+def _clip_gpu(grads, clip):
+    table = psync.make_grad_table(grads)
+    nbytes = psync.psync_clip_workspace_bytes(table.W, grads[0].numel(), table.grad_dtype)
+    assert nbytes >= 8 * table.W
+    d_work = torch.empty(nbytes // 8, dtype=torch.float64, device=DEV)
+    d_scales = torch.full((table.W,), -1.0, dtype=torch.float32, device=DEV)
+    psync.psync_clip_scales(table, clip, d_scales, d_work)
+    torch.cuda.synchronize()
+    return d_scales
+
+
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+@pytest.mark.parametrize("P", [1, 7, 8, 9, 1000, 32_768, 32_769, 300_001])
+def test_clip_scales_match_oracle(dtype, P):
+    rng = np.random.default_rng(P + dtype)
+    W = 6
+    grads = []
+    for k in range(W):
+        g = torch.randn(P, device=DEV) * float(10.0 ** rng.integers(-4, 1))
+        grads.append(g.to(torch.bfloat16) if dtype == synth.BF16 else g)
+    clip = 0.05
+    got = _clip_gpu(grads, clip).cpu().numpy()
+    want = oracle.clip_scales([synth.as_numpy_grad(g) for g in grads], clip)
+    assert np.abs(got - want).max() <= 1e-6 * np.abs(want).max() + 1e-12
+    assert ((want == 1.0) == (got == 1.0)).all() or np.abs(got - want).max() < 2e-7
+
+
+def test_clip_scales_3_4_5_and_determinism_and_unaligned():
+    g = [torch.tensor([3.0, 4.0], device=DEV), torch.zeros(2, device=DEV), torch.tensor([-6.0, 8.0], device=DEV)]
+    assert _clip_gpu(g, 2.5).cpu().tolist() == [0.5, 1.0, 0.25]
+    big = [torch.randn(1_000_003, device=DEV) for _ in range(3)]
+    a, b = _clip_gpu(big, 1.0).cpu().numpy(), _clip_gpu(big, 1.0).cpu().numpy()
+    assert np.array_equal(a, b)                                              # no atomics: run-to-run identical
+    buf = torch.randn(50_010, device=DEV)
+    shifted = [buf[1:50_001], buf[2:50_002], buf[3:50_003]]                   # 4-, 8-, 12-byte offsets
+    got = _clip_gpu([s for s in shifted], 1.0).cpu().numpy()
+    want = oracle.clip_scales([s.cpu().numpy().copy() for s in shifted], 1.0)
+    assert np.abs(got - want).max() <= 1e-6
+
+
+def test_clip_invalid_arguments():
+    L = psync.binding.lib()
+    assert L.psync_clip_scales(None, 1, 4, 0, 1.0, None, None, 0, None) == psync.PSYNC_EINVAL
+    assert L.psync_clip_scales(8, 0, 4, 0, 1.0, 8, 8, 64, None) == psync.PSYNC_EINVAL
+    assert L.psync_clip_scales(8, 1, 4, 0, 0.0, 8, 8, 64, None) == psync.PSYNC_EINVAL
+    assert L.psync_clip_scales(8, 1, 4, 2, 1.0, 8, 8, 64, None) == psync.PSYNC_EINVAL
+    assert L.psync_clip_scales(8, 1, 4, 0, 1.0, 8, 8, 4, None) == psync.PSYNC_EINVAL      # workspace too small
+    assert psync.psync_clip_workspace_bytes(0, 4, 0) == 0
+
+
+@pytest.mark.parametrize("dtype,opt", [(synth.F32, synth.RMSPROP_MOM), (synth.BF16, synth.MOMENTUM), (synth.F32, synth.SGD)])
+def test_async_with_clipping_and_schedule_matches_oracle(dtype, opt):
+    """The paper's Async-Opt recipe end to end (A.3): arrival order, global-norm clipping of every gradient, a
+    decaying learning rate per iteration, RMSProp / momentum / SGD, EMA."""
+    cfg = replace(BASE, grad_dtype=dtype, opt=opt, P=90_001, grad_dist=("normal", 1e-2), name=f"async_clip_{dtype}_{opt}")
+    pair = AsyncPair(cfg)
+    clip = 2.0                                          # ||G|| ~ 1e-2 * sqrt(90001) = 3: every gradient is clipped
+    for s in range(2):
+        grads = [synth.gradient(cfg, s, k, DEV) for k in range(cfg.W)]
+        if s == 1:
+            grads[5] = grads[5] * 0.1                   # one gradient inside the bound: factor exactly 1
+        table = psync.make_grad_table(grads)
+        arrival = synth.arrival_times(cfg, s)
+        psync.psync_order_by_arrival(torch.from_numpy(arrival).to(DEV), cfg.W, pair.d_order, pair.d_n)
+        d_work = torch.empty(psync.psync_clip_workspace_bytes(cfg.W, cfg.P, table.grad_dtype) // 8, dtype=torch.float64,
+                             device=DEV)
+        d_scales = torch.empty(cfg.W, dtype=torch.float32, device=DEV)
+        psync.psync_clip_scales(table, clip, d_scales, d_work)
+        d_gamma = torch.empty(cfg.W, dtype=torch.float32, device=DEV)
+        psync.psync_lr_schedule(0.045, 0.94, 1000 * s, cfg.W, 0.01, d_gamma)
+        st, keep = pair.make_step(table)
+        psync.psync_async_apply(st, d_gamma, d_gscale=d_scales)
+        torch.cuda.synchronize()
+        # oracle, fed the GPU's clip factors and rates (each checked against its own oracle first): lock-step
+        order = oracle.order_by_arrival(arrival)
+        np_grads = [synth.as_numpy_grad(g) for g in grads]
+        sc_o = oracle.clip_scales(np_grads, clip)
+        sc_g = d_scales.cpu().numpy()
+        assert np.abs(sc_g - sc_o).max() <= 1e-6 and (s == 0 or sc_g[5] == 1.0) and (np.delete(sc_g, 5) < 1.0).all()
+        gm_o = oracle.lr_schedule(0.045, 0.94, 1000 * s, cfg.W, 0.01)
+        gm_g = d_gamma.cpu().numpy()
+        assert ulp_diff(gm_g, gm_o).max() <= 1
+        h = pair.host
+        rc = oracle.async_apply(pair.off, np_grads, order, h["theta"], h["ema"], h["state0"], h["state1"],
+                                gammas=gm_g[:order.size].copy(), gscales=sc_g[order].copy(), opt=cfg.opt,
+                                ema_mode=cfg.ema_mode, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
+        assert rc == oracle.OK
+        for n in STATE_NAMES:
+            g = getattr(pair, n)
+            if g is not None:
+                assert_close(to_np(g), h[n], rtol_async(order.size), ATOL_STEP, f"{cfg.name} step {s} {n}")
+                h[n] = to_np(g)
+
+
+def test_unit_scale_is_bit_identical_to_no_scale():
+    cfg = replace(BASE, P=50_003, opt=synth.RMSPROP_MOM, name="async_unit_scale")
+    arrival = synth.arrival_times(cfg, 0)
+    grads = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    table = psync.make_grad_table(grads)
+    out = []
+    for scaled in (False, True):
+        pair = AsyncPair(cfg)
+        psync.psync_order_by_arrival(torch.from_numpy(arrival).to(DEV), cfg.W, pair.d_order, pair.d_n)
+        st, keep = pair.make_step(table)
+        psync.psync_async_apply(st, d_gscale=torch.ones(cfg.W, device=DEV) if scaled else None)
+        torch.cuda.synchronize()
+        out.append({n: to_np(getattr(pair, n)) for n in STATE_NAMES})
+    for n in STATE_NAMES:
+        assert np.array_equal(out[0][n], out[1][n])
