@@ -262,6 +262,11 @@ def run_psync(args, cfg, rank, world, dist):
                                    d_shard_off=d_off, d_n_kept=d_n_kept)
         steps_struct.append((st, keep))
     geo = psync.psync_launch_geometry(steps_struct[0][0])
+    d_scales = d_clip_work = None
+    if mode == "async" and args.clip > 0:
+        d_scales = torch.ones(cfg.W, dtype=torch.float32, device=dev)
+        d_clip_work = torch.empty(psync.psync_clip_workspace_bytes(cfg.W, cfg.P, cfg.grad_dtype) // 8,
+                                  dtype=torch.float64, device=dev)
 
     stream = torch.cuda.Stream(device=dev)
     B = psync.binding
@@ -287,7 +292,9 @@ def run_psync(args, cfg, rank, world, dist):
         if ev is not None:
             ev[1].record(stream)
         if mode == "async":
-            B.psync_async_apply(st, None, stream)
+            if args.clip > 0:            # A.3 (L313): global-norm clipping = one more pass over the W buffers
+                B.psync_clip_scales(tables[i % n_sets], args.clip, d_scales, d_clip_work, stream)
+            B.psync_async_apply(st, None, stream, d_gscale=d_scales if args.clip > 0 else None)
         else:
             B.psync_aggregate_update(st, stream)
         if ev is not None:
@@ -335,6 +342,8 @@ def run_psync(args, cfg, rank, world, dist):
     else:
         n_eff = float(cfg.N)
     bytes_per_step = cfg.bytes_per_step + (n_eff - cfg.N) * cfg.P * cfg.grad_bytes
+    if mode == "async" and args.clip > 0:
+        bytes_per_step += cfg.W * cfg.P * cfg.grad_bytes      # the norm pass reads every buffer once more
     units_local = n_eff * cfg.P * K
     units, max_ms = aggregate_over_ranks(units_local, total_ms, dist)
     value = units / (max_ms * 1e-3)
@@ -437,6 +446,7 @@ def main():
                     help="first_n: the headline (one kept set); per_server: Alg. 4 per server j; timeout: L259; "
                          "async: Alg. 2, all W gradients one at a time in one pass")
     ap.add_argument("--timeout", type=float, default=1.5, help="seconds, for --mode timeout")
+    ap.add_argument("--clip", type=float, default=0.0, help="--mode async: global-norm clip bound (0 = off)")
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--grid-ctas", type=int, default=0)
     ap.add_argument("--grad-sets", type=int, default=3)
