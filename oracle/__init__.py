@@ -60,6 +60,8 @@ def lib() -> ctypes.CDLL:
         L.oracle_order_by_arrival.restype = ctypes.c_int
         L.oracle_async_apply.argtypes = [i64, i32, vp, i32, i32, vp, ctypes.c_int, vp, vp, vp, vp, vp, vp, vp,
                                          ctypes.c_int, ctypes.c_int, f32, f32, f32, f32, f32]
+        L.oracle_kth_arrival_stats.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp]
+        L.oracle_kth_arrival_stats.restype = ctypes.c_int
         L.oracle_lr_schedule.argtypes = [f32, f32, i64, i32, ctypes.c_double, vp]
         L.oracle_lr_schedule.restype = ctypes.c_int
         L.oracle_clip_scales.argtypes = [vp, i32, i64, ctypes.c_int, f32, vp]
@@ -201,6 +203,25 @@ def order_by_arrival(arrival):
     if st != OK:
         raise ValueError("oracle_order_by_arrival: invalid arguments")
     return order[:int(n[0])].copy()
+
+
+def kth_arrival_stats(arrival, iters=None):
+    """Section 3.1's procedure on arrival[T][W] -> dict(sorted, count, mean, median[, est_time])."""
+    if not (isinstance(arrival, np.ndarray) and arrival.ndim == 2):
+        raise ValueError("arrival must be [T][W]")
+    T, W = arrival.shape
+    _chk(arrival, np.float32, "arrival", T * W)
+    _chk(iters, np.float64, "iters", W)
+    out = dict(sorted=np.zeros((T, W), np.float32), count=np.zeros(W, np.int32), mean=np.zeros(W, np.float64),
+               median=np.zeros(W, np.float64))
+    est = None if iters is None else np.zeros(W, np.float64)
+    rc = lib().oracle_kth_arrival_stats(_ptr(arrival), T, W, _ptr(out["sorted"]), _ptr(out["count"]), _ptr(out["mean"]),
+                                        _ptr(out["median"]), _ptr(iters), _ptr(est))
+    if rc != OK:
+        raise ValueError("oracle_kth_arrival_stats: invalid arguments")
+    if est is not None:
+        out["est_time"] = est
+    return out
 
 
 def lr_schedule(gamma0, beta, t0, K, s):

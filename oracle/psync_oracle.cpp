@@ -36,6 +36,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstring>
+#include <limits>
 #include <utility>
 #include <vector>
 
@@ -437,6 +438,55 @@ int oracle_clip_scales(const void* const* grads, int32_t W, int64_t P, int grad_
     const double norm = std::sqrt(sumsq);
     const double c = static_cast<double>(clip);
     scales[k] = static_cast<float>(c / std::max(norm, c));
+  }
+  return ORACLE_OK;
+}
+
+// =============================================================================================
+// Straggler statistics -- the PROCEDURE of section 3.1 (L171-193), on whatever arrival times are
+// supplied: "we collected for each iteration both the start time of the iteration and the time when
+// the kth gradient ... arrived at the parameter server" (L171; Fig. 3 is the CDF of these per k),
+// "Mean and median times, across all iterations, to collect k gradients" (Fig. 4), and "We can
+// multiply this with the mean iteration times (Figure 4) to obtain the running time required to
+// converge for each setting of N and b" (Fig. 6).
+//   arrival[T][W]  times since each iteration's start; non-finite = never arrived
+//   sorted[T][W]   OUT: row t ascending; entry k = time the (k+1)-th gradient arrived; missing = +inf
+//   count[W], mean[W], median[W]  OUT over the iterations in which a (k+1)-th gradient arrived
+//                  (mean/median are NaN where count is 0; median of an even count = mean of the two
+//                  middle values)
+//   iters[W] or NULL, est_time[W] OUT or NULL: est_time[k] = mean[k] * iters[k], iters[k] = iterations
+//                  to converge when aggregating k+1 gradients (Fig. 5, supplied by the caller)
+// =============================================================================================
+int oracle_kth_arrival_stats(const float* arrival, int32_t T, int32_t W, float* sorted, int32_t* count,
+                             double* mean, double* median, const double* iters, double* est_time) {
+  if (!arrival || !sorted || !count || !mean || !median || T < 1 || W < 1) return ORACLE_EINVAL;
+  if ((iters == nullptr) != (est_time == nullptr)) return ORACLE_EINVAL;
+  const float inf = std::numeric_limits<float>::infinity();
+  for (int32_t t = 0; t < T; ++t) {
+    std::vector<float> row;
+    for (int32_t k = 0; k < W; ++k)
+      if (std::isfinite(arrival[static_cast<int64_t>(t) * W + k])) row.push_back(arrival[static_cast<int64_t>(t) * W + k]);
+    std::sort(row.begin(), row.end());
+    for (int32_t k = 0; k < W; ++k)
+      sorted[static_cast<int64_t>(t) * W + k] = k < static_cast<int32_t>(row.size()) ? row[k] : inf;
+  }
+  for (int32_t k = 0; k < W; ++k) {
+    std::vector<float> col;
+    for (int32_t t = 0; t < T; ++t)
+      if (std::isfinite(sorted[static_cast<int64_t>(t) * W + k])) col.push_back(sorted[static_cast<int64_t>(t) * W + k]);
+    count[k] = static_cast<int32_t>(col.size());
+    if (col.empty()) {
+      mean[k] = median[k] = std::numeric_limits<double>::quiet_NaN();
+    } else {
+      double sum = 0.0;
+      for (float v : col) sum += static_cast<double>(v);
+      mean[k] = sum / static_cast<double>(col.size());
+      std::sort(col.begin(), col.end());
+      const size_t n = col.size();
+      median[k] = (n % 2) ? static_cast<double>(col[n / 2])
+                          : 0.5 * (static_cast<double>(col[n / 2 - 1]) + static_cast<double>(col[n / 2]));
+    }
+    if (est_time) est_time[k] = mean[k] * iters[k];
   }
   return ORACLE_OK;
 }

@@ -245,3 +245,37 @@ def test_cuda_graph_capture_and_replay_matches_oracle(cfg):
         pair.compare(RTOL_STEP * steps_per_graph, ATOL_STEP, f"graph replay {replay}")
         pair.sync_host_from_gpu()
         s += steps_per_graph
+
+
+# ------------------------------------------------------------------ stale gradients across steps (Alg. 4 l.5-6)
+def test_stale_gradients_of_dropped_workers_carry_into_the_next_step_and_are_dropped():
+    """NEXT-2: the b workers dropped at step t-1 deliver that old gradient, tagged t-1, EARLY in step t (before
+    anyone else).  Alg. 4 l.5-6 drops it by its tag; the server then keeps the first N of the
+    remaining workers.  The stale buffers hold NaN, so any use of them would poison theta."""
+    cfg = replace(synth.scaled(synth.PAPER_RMSPROP, 60_001), N=20, b=6, M=5, name="stale_carry")
+    pair = Pair(cfg)
+    stale = np.array([], dtype=np.int64)
+    for t in range(5):
+        grads = pair.gradients(t)
+        arrival = synth.arrival_times(cfg, t)
+        tags = np.full(cfg.W, t, dtype=np.int32)
+        if stale.size:
+            tags[stale] = t - 1
+            arrival[stale] = np.float32(1e-3) * (1 + np.arange(stale.size, dtype=np.float32))   # first to arrive
+            for k in stale:
+                grads[k].fill_(float("nan"))
+        st_g, kept_g, tn_g = pair.gpu_step(grads, arrival, tags=tags, t=t)
+        st_o, kept_o, tn_o = pair.oracle_step(grads, arrival, tags=tags, t=t)
+        assert st_g == st_o == 0 and np.array_equal(kept_g, kept_o) and tn_g == tn_o
+        assert not set(kept_g.tolist()) & set(stale.tolist())
+        assert tn_g > 0.1                                        # the server waited for fresh gradients
+        pair.compare(RTOL_STEP, ATOL_STEP, f"stale carry step {t}")
+        pair.sync_host_from_gpu()
+        assert bool(torch.isfinite(pair.ps.theta).all())
+        stale = np.setdiff1d(np.arange(cfg.W), kept_g)[:cfg.b]   # this step's dropped workers are next step's stale
+    # more stale workers than backups: the server can never collect N fresh gradients
+    tags = np.full(cfg.W, 9, dtype=np.int32)
+    tags[:cfg.b + 1] = 8
+    before = to_np(pair.ps.theta)
+    st_g, _, _ = pair.gpu_step(pair.gradients(9), synth.arrival_times(cfg, 9), tags=tags, t=9)
+    assert st_g == psync.PSYNC_ETOOFEW and np.array_equal(before, to_np(pair.ps.theta))
