@@ -25,7 +25,7 @@ PSYNC_MAX_WORKERS = 1024
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
            "psync_select_timeout", "psync_aggregate_update", "psync_ema", "psync_order_by_arrival", "psync_async_apply", "psync_step_device", "psync_clip_workspace_bytes",
-           "psync_clip_scales", "psync_lr_schedule",
+           "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_launch_geometry", "psync_probe_read",
            "psync_probe_copy")
 
@@ -83,6 +83,8 @@ def lib() -> ctypes.CDLL:
         L.psync_clip_workspace_bytes.restype = ctypes.c_size_t
         L.psync_clip_scales.argtypes = [vp, i32, i64, i32, f32, vp, vp, ctypes.c_size_t, vp]
         L.psync_clip_scales.restype = ctypes.c_int
+        L.psync_kth_arrival_stats.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+        L.psync_kth_arrival_stats.restype = ctypes.c_int
         L.psync_lr_schedule.argtypes = [f32, f32, i64, i32, ctypes.c_double, vp, vp]
         L.psync_lr_schedule.restype = ctypes.c_int
         L.psync_async_apply.restype = ctypes.c_int
@@ -308,6 +310,29 @@ def psync_clip_scales(table: "GradTable", clip: float, d_scales: torch.Tensor, d
                                  _stream(stream))
     if check and st != PSYNC_OK:
         raise PsyncError(st, "psync_clip_scales")
+    return st
+
+
+def psync_kth_arrival_stats(d_arrival: torch.Tensor, d_sorted: torch.Tensor, d_count: torch.Tensor,
+                            d_mean: torch.Tensor, d_median: torch.Tensor, d_iters: Optional[torch.Tensor] = None,
+                            d_est_time: Optional[torch.Tensor] = None, stream=None, check: bool = True) -> int:
+    """Section 3.1's straggler statistics (include/psync.h: psync_kth_arrival_stats)."""
+    if d_arrival.dim() != 2:
+        raise ValueError("d_arrival must be [T][W]")
+    T, W = d_arrival.shape
+    if d_sorted.numel() < T * W:
+        raise ValueError("d_sorted needs T*W elements")
+    for nm, a in (("d_count", d_count), ("d_mean", d_mean), ("d_median", d_median), ("d_iters", d_iters),
+                  ("d_est_time", d_est_time)):
+        if a is not None and a.numel() < W:
+            raise ValueError(f"{nm} needs W elements")
+    st = lib().psync_kth_arrival_stats(_dptr(d_arrival, torch.float32, "d_arrival"), T, W,
+                                       _dptr(d_sorted, torch.float32, "d_sorted"), _dptr(d_count, torch.int32, "d_count"),
+                                       _dptr(d_mean, torch.float64, "d_mean"), _dptr(d_median, torch.float64, "d_median"),
+                                       _dptr(d_iters, torch.float64, "d_iters"),
+                                       _dptr(d_est_time, torch.float64, "d_est_time"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_kth_arrival_stats")
     return st
 
 

@@ -115,6 +115,120 @@ __global__ void lr_schedule_kernel(float gamma0, float beta, int64_t t0, int32_t
                                 pow(static_cast<double>(beta), static_cast<double>(t0 + i) * s));
 }
 
+// ---- K7: straggler statistics, the procedure of section 3.1 -----------------------------
+__device__ __forceinline__ uint32_t time_key(float a) {  // order-preserving; 0xFFFFFFFF = never arrived
+  uint32_t u = __float_as_uint(a);
+  if ((u & 0x7F800000u) == 0x7F800000u) return 0xFFFFFFFFu;
+  if (u == 0x80000000u) u = 0u;
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float key_time(uint32_t key) {
+  return __uint_as_float((key & 0x80000000u) ? (key & 0x7FFFFFFFu) : ~key);
+}
+
+// K7a: one CTA per iteration: rank-sort its W arrival times; entry k of the row = when the (k+1)-th gradient arrived
+__global__ void __launch_bounds__(1024) sort_rows_kernel(const float* __restrict__ arrival, int32_t W,
+                                                         float* __restrict__ sorted) {
+  __shared__ uint32_t s_key[kMaxWorkers];
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const int i = threadIdx.x;
+  const int64_t row = static_cast<int64_t>(blockIdx.x) * W;
+  uint32_t key = 0xFFFFFFFFu;
+  if (i < W) {
+    key = time_key(arrival[row + i]);
+    s_key[i] = key;
+  }
+  const int n = __syncthreads_count(key != 0xFFFFFFFFu);
+  if (i < W && i >= n) sorted[row + i] = __int_as_float(0x7F800000);  // no (i+1)-th arrival this iteration: +inf
+  if (key != 0xFFFFFFFFu) {
+    int rank = 0;
+    for (int j = 0; j < W; ++j) {
+      const uint32_t kj = s_key[j];
+      rank += (kj < key || (kj == key && j < i)) ? 1 : 0;
+    }
+    sorted[row + rank] = key_time(key);
+  }
+}
+
+// K7b: one CTA per k: count / mean (fixed-order double sum) / median (radix select over the T keys of column k)
+__global__ void __launch_bounds__(256) column_stats_kernel(const float* __restrict__ sorted, int32_t T, int32_t W,
+                                                           int32_t* __restrict__ count, double* __restrict__ mean,
+                                                           double* __restrict__ median, const double* __restrict__ iters,
+                                                           double* __restrict__ est_time) {
+  __shared__ double s_warp[8];
+  __shared__ int s_cnt[4];
+  __shared__ int s_n;
+  __shared__ double s_sum;
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const int k = blockIdx.x;
+  double acc = 0.0;
+  int mine = 0;
+  for (int t = threadIdx.x; t < T; t += 256) {
+    const float v = sorted[static_cast<int64_t>(t) * W + k];
+    if (time_key(v) != 0xFFFFFFFFu) {
+      acc += static_cast<double>(v);
+      ++mine;
+    }
+  }
+  const double total = block_sum(acc, s_warp);
+  if (threadIdx.x == 0) {
+    s_sum = total;
+    s_n = 0;
+  }
+  __syncthreads();
+  atomicAdd(&s_n, mine);  // integer: the result does not depend on the order
+  __syncthreads();
+  const int c = s_n;
+  double med = __longlong_as_double(0x7FF8000000000000LL);  // NaN when nobody ever delivered a (k+1)-th gradient
+  if (c > 0) {
+    double v[2];
+    for (int which = 0; which < 2; ++which) {
+      int r = which == 0 ? (c - 1) / 2 : c / 2;
+      uint32_t prefix = 0u;
+      for (int shift = 30; shift >= 0; shift -= 2) {
+        const uint32_t hi_mask = (shift == 30) ? 0u : (0xFFFFFFFFu << (shift + 2));
+        if (threadIdx.x < 4) s_cnt[threadIdx.x] = 0;
+        __syncthreads();
+        int c0 = 0, c1 = 0, c2 = 0, c3 = 0;
+        for (int t = threadIdx.x; t < T; t += 256) {
+          const uint32_t key = time_key(sorted[static_cast<int64_t>(t) * W + k]);
+          if (key != 0xFFFFFFFFu && (key & hi_mask) == prefix) {
+            const uint32_t d = (key >> shift) & 3u;
+            c0 += d == 0u;
+            c1 += d == 1u;
+            c2 += d == 2u;
+            c3 += d == 3u;
+          }
+        }
+        if (c0) atomicAdd(&s_cnt[0], c0);
+        if (c1) atomicAdd(&s_cnt[1], c1);
+        if (c2) atomicAdd(&s_cnt[2], c2);
+        if (c3) atomicAdd(&s_cnt[3], c3);
+        __syncthreads();
+        const int n0 = s_cnt[0], n1 = s_cnt[1], n2 = s_cnt[2];
+        uint32_t digit;
+        if (r < n0) digit = 0u;
+        else if (r < n0 + n1) { digit = 1u; r -= n0; }
+        else if (r < n0 + n1 + n2) { digit = 2u; r -= n0 + n1; }
+        else { digit = 3u; r -= n0 + n1 + n2; }
+        prefix |= digit << shift;
+        __syncthreads();
+      }
+      v[which] = static_cast<double>(key_time(prefix));
+    }
+    med = (c & 1) ? v[0] : 0.5 * (v[0] + v[1]);
+  }
+  if (threadIdx.x == 0) {
+    const double m = c > 0 ? s_sum / static_cast<double>(c) : __longlong_as_double(0x7FF8000000000000LL);
+    count[k] = c;
+    mean[k] = m;
+    median[k] = med;
+    if (est_time != nullptr) est_time[k] = m * iters[k];
+  }
+}
+
 int clip_chunks(int64_t P, int dtype) {
   const int E = dtype == 1 ? 8 : 4;
   const int64_t c = (P / E + kClipChunkUnits - 1) / kClipChunkUnits;
@@ -150,6 +264,19 @@ cudaError_t launch_clip_scales(const void* const* d_grads, int32_t W, int64_t P,
   if (err != cudaSuccess) return err;
   pdl_config(&cfg, attr, dim3(static_cast<unsigned>(W)), dim3(kClipThreads), stream);
   return cudaLaunchKernelEx(&cfg, clip_finalize_kernel, static_cast<const double*>(work), chunks, clip, d_scales);
+}
+
+cudaError_t launch_kth_arrival_stats(const float* d_arrival, int32_t T, int32_t W, float* d_sorted, int32_t* d_count,
+                                     double* d_mean, double* d_median, const double* d_iters, double* d_est_time,
+                                     cudaStream_t stream) {
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute attr[1];
+  pdl_config(&cfg, attr, dim3(static_cast<unsigned>(T)), dim3(static_cast<unsigned>((W + 31) / 32 * 32)), stream);
+  cudaError_t err = cudaLaunchKernelEx(&cfg, sort_rows_kernel, d_arrival, W, d_sorted);
+  if (err != cudaSuccess) return err;
+  pdl_config(&cfg, attr, dim3(static_cast<unsigned>(W)), dim3(256), stream);
+  return cudaLaunchKernelEx(&cfg, column_stats_kernel, static_cast<const float*>(d_sorted), T, W, d_count, d_mean,
+                            d_median, d_iters, d_est_time);
 }
 
 cudaError_t launch_lr_schedule(float gamma0, float beta, int64_t t0, int32_t K, double s, float* d_gamma,

@@ -231,6 +231,17 @@ PSYNC_API int psync_clip_scales(const void* const* d_grads, int32_t W, int64_t P
              : PSYNC_ECUDA;
 }
 
+PSYNC_API int psync_kth_arrival_stats(const float* d_arrival, int32_t T, int32_t W, float* d_sorted, int32_t* d_count,
+                            double* d_mean, double* d_median, const double* d_iters, double* d_est_time, void* stream) {
+  if (d_arrival == nullptr || d_sorted == nullptr || d_count == nullptr || d_mean == nullptr || d_median == nullptr)
+    return PSYNC_EINVAL;
+  if (T < 1 || W < 1 || W > PSYNC_MAX_WORKERS || (d_iters == nullptr) != (d_est_time == nullptr)) return PSYNC_EINVAL;
+  return psync::launch_kth_arrival_stats(d_arrival, T, W, d_sorted, d_count, d_mean, d_median, d_iters, d_est_time,
+                                         static_cast<cudaStream_t>(stream)) == cudaSuccess
+             ? PSYNC_OK
+             : PSYNC_ECUDA;
+}
+
 PSYNC_API int psync_lr_schedule(float gamma0, float beta, int64_t t0, int32_t K, double s, float* d_gamma, void* stream) {
   if (K < 0 || t0 < 0 || !(beta > 0.0f) || (K > 0 && d_gamma == nullptr)) return PSYNC_EINVAL;
   if (K == 0) return PSYNC_OK;

@@ -148,3 +148,67 @@ def test_unit_scale_is_bit_identical_to_no_scale():
         out.append({n: to_np(getattr(pair, n)) for n in STATE_NAMES})
     for n in STATE_NAMES:
         assert np.array_equal(out[0][n], out[1][n])
+
+
+# ------------------------------------------------------------------ straggler statistics (section 3.1)
+def _stats_gpu(a, iters=None):
+    T, W = a.shape
+    d_sorted = torch.full((T, W), -1.0, dtype=torch.float32, device=DEV)
+    d_count = torch.full((W,), -1, dtype=torch.int32, device=DEV)
+    d_mean = torch.zeros(W, dtype=torch.float64, device=DEV)
+    d_median = torch.zeros(W, dtype=torch.float64, device=DEV)
+    d_iters = None if iters is None else torch.from_numpy(iters).to(DEV)
+    d_est = None if iters is None else torch.zeros(W, dtype=torch.float64, device=DEV)
+    psync.psync_kth_arrival_stats(torch.from_numpy(a).to(DEV), d_sorted, d_count, d_mean, d_median, d_iters, d_est)
+    torch.cuda.synchronize()
+    out = dict(sorted=d_sorted.cpu().numpy(), count=d_count.cpu().numpy(), mean=d_mean.cpu().numpy(),
+               median=d_median.cpu().numpy())
+    if iters is not None:
+        out["est_time"] = d_est.cpu().numpy()
+    return out
+
+
+@pytest.mark.parametrize("T,W", [(1, 1), (3, 3), (7, 33), (50, 106), (1000, 106), (257, 1024), (4001, 12)])
+def test_kth_arrival_stats_match_oracle(T, W):
+    rng = np.random.default_rng(T * 1000 + W)
+    a = rng.lognormal(0, 0.25, (T, W)).astype(np.float32)
+    a[rng.random((T, W)) < 0.02] *= 5
+    ties = rng.random((T, W)) < 0.1
+    a[ties] = rng.choice(np.array([1.0, 1.5, 0.0, -0.0, -1.0], np.float32), size=int(ties.sum()))
+    a[rng.random((T, W)) < 0.05] = np.inf
+    a[rng.random((T, W)) < 0.02] = np.nan
+    if W > 2:
+        a[:, -1] = np.inf                                     # a worker that never reports: last column count 0
+    iters = rng.uniform(7e4, 1.4e5, W)
+    got, want = _stats_gpu(a, iters), oracle.kth_arrival_stats(a, iters)
+    assert np.array_equal(got["sorted"], want["sorted"])                         # bit-exact (0.0 == -0.0)
+    assert np.array_equal(got["count"], want["count"])
+    assert np.array_equal(got["median"], want["median"], equal_nan=True)         # exact selection
+    ok = want["count"] > 0
+    assert np.isnan(got["mean"][~ok]).all() and np.isnan(got["est_time"][~ok]).all()
+    assert np.allclose(got["mean"][ok], want["mean"][ok], rtol=1e-13, atol=0)    # double sums, different order
+    assert np.allclose(got["est_time"][ok], want["est_time"][ok], rtol=1e-13, atol=0)
+
+
+def test_kth_arrival_stats_paper_shape_and_link_to_selection():
+    """cfg3's arrival recipe, N+b = 106, 500 iterations: column N-1 of the sorted matrix is the time the
+    synchronous server waits (t_Nth of the selection kernel), and the tail grows as in Fig. 4."""
+    cfg = synth.PAPER_RMSPROP
+    a = np.stack([synth.arrival_times(cfg, s) for s in range(500)])
+    got = _stats_gpu(a)
+    assert (np.diff(got["mean"]) >= 0).all() and (got["count"] == 500).all()
+    assert got["mean"][-1] - got["mean"][-7] > got["mean"][60] - got["mean"][54]      # the last few are the slow ones
+    d_kept = torch.zeros(cfg.N, dtype=torch.int32, device=DEV)
+    d_status = torch.zeros(1, dtype=torch.int32, device=DEV)
+    d_tn = torch.zeros(1, dtype=torch.float32, device=DEV)
+    for t in (0, 17, 499):
+        psync.psync_select_first_n(torch.from_numpy(a[t]).to(DEV), cfg.N, cfg.b, d_kept, d_status, d_tn)
+        assert float(d_tn.item()) == got["sorted"][t, cfg.N - 1]
+
+
+def test_kth_arrival_stats_invalid_arguments():
+    L = psync.binding.lib()
+    assert L.psync_kth_arrival_stats(None, 1, 1, None, None, None, None, None, None, None) == psync.PSYNC_EINVAL
+    assert L.psync_kth_arrival_stats(8, 0, 1, 8, 8, 8, 8, None, None, None) == psync.PSYNC_EINVAL
+    assert L.psync_kth_arrival_stats(8, 1, 1025, 8, 8, 8, 8, None, None, None) == psync.PSYNC_EINVAL
+    assert L.psync_kth_arrival_stats(8, 1, 4, 8, 8, 8, 8, 8, None, None) == psync.PSYNC_EINVAL   # iters without est_time
