@@ -157,14 +157,19 @@ __global__ void __launch_bounds__(1024) order_by_arrival_kernel(const float* __r
 struct AsyncShape {
   int threads, unroll, minb;
 };
-constexpr AsyncShape kShapeF32 = {256, 8, 3};
-constexpr AsyncShape kShapeBF16 = {256, 8, 2};
+// {threads, loads in flight per thread, CTAs per SM}, measured on B200 over 12 shapes (DESIGN.md s.5): the K
+// dependent updates want occupancy more than deep load batches -- 4 CTAs/SM for fp32 (64 registers), and for RMSProp
+// (issue-bound) 4 loads in flight instead of 8; bf16 holds 8 parameters per thread, so 3 CTAs/SM (2 with RMSProp).
+constexpr AsyncShape shape_for(bool bf16, int opt) {
+  return bf16 ? (opt == OPT_RMSPROP_MOM ? AsyncShape{256, 8, 2} : AsyncShape{256, 8, 3})
+              : (opt == OPT_RMSPROP_MOM ? AsyncShape{256, 4, 4} : AsyncShape{256, 8, 4});
+}
 
 using KernelFn = void (*)(const FusedParams);
 
 template <bool BF16, int OPT>
 KernelFn pick_ema(int ema) {
-  constexpr AsyncShape S = BF16 ? kShapeBF16 : kShapeF32;
+  constexpr AsyncShape S = shape_for(BF16, OPT);
   switch (ema) {
     case EMA_POST: return async_apply_kernel<S.threads, S.unroll, S.minb, BF16, OPT, EMA_POST>;
     case EMA_PRE: return async_apply_kernel<S.threads, S.unroll, S.minb, BF16, OPT, EMA_PRE>;
@@ -183,7 +188,7 @@ KernelFn pick_opt(int opt, int ema) {
 }  // namespace
 
 cudaError_t async_geometry(int dtype, int grid_ctas, int64_t P, FusedGeometry* out) {
-  const AsyncShape s = dtype == 1 ? kShapeBF16 : kShapeF32;
+  const AsyncShape s = shape_for(dtype == 1, OPT_SGD);  // every shape has 256 threads: the grid does not depend on opt
   const int E = dtype == 1 ? 8 : 4;
   out->block = s.threads;
   out->tile_elems = s.threads * E;
