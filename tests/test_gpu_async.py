@@ -240,3 +240,11 @@ def test_full_size_async_cfg3_shape_sampled():
     for n in STATE_NAMES:
         assert_close(to_np(getattr(pair, n)[d_idx]), host[n], rtol_async(106), ATOL_STEP, f"async cfg3 {n} (sampled)")
     assert bool(torch.isfinite(pair.theta).all())
+
+
+def test_async_max_workers_1024():
+    """W = PSYNC_MAX_WORKERS: the shared-memory pointer / gamma / scale tables are full."""
+    cfg = replace(BASE, N=1024, P=3_001, opt=synth.MOMENTUM, grad_dist=("normal", 1e-4), name="async_K1024")
+    pair = AsyncPair(cfg)
+    order = pair.step(0, synth.arrival_times(cfg, 0))
+    assert order.size == 1024

@@ -391,3 +391,14 @@ def test_full_size_cfg3_per_server_sampled():
             assert_close(got, host[n], RTOL_STEP, ATOL_STEP, f"cfg3 per-server step {s} {n} (sampled)")
             host[n] = got
         assert bool(torch.isfinite(pair.theta).all())
+
+
+def test_per_server_many_tiny_servers_every_tile_straddles():
+    """M = 1000 servers of ~100 parameters: every 1024-parameter tile spans ~10 servers, so the whole vector goes
+    through the element-wise path, each element with its own server's kept row."""
+    cfg = per_server_cfg(P=100_003, M=1000, N=5, b=2, opt=synth.RMSPROP_MOM, name="ps_tiny_servers")
+    pair = RowsPair(cfg)
+    a = synth.arrival_times_per_server(cfg, 0, server_sigma=0.3)
+    a[::7, :4] = np.inf                       # every 7th server fails (3 < N eligible)
+    status, kept = pair.step_first_n(0, a)
+    assert (status[::7] == oracle.ETOOFEW).all() and (np.delete(status, np.s_[::7]) == 0).all()
