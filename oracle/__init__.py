@@ -74,6 +74,8 @@ def lib() -> ctypes.CDLL:
         L.oracle_apply_sum.restype = ctypes.c_int
         L.oracle_ema.argtypes = [vp, vp, i64, f32]
         L.oracle_ema.restype = ctypes.c_int
+        L.oracle_set_fp32_mirror.argtypes = [ctypes.c_int]
+        L.oracle_set_fp32_mirror.restype = ctypes.c_int
         L.oracle_num_threads.restype = ctypes.c_int
         L.oracle_set_num_threads.argtypes = [ctypes.c_int]
         _lib = L
@@ -293,6 +295,20 @@ def ema_update(ema, theta, alpha):
     _chk(ema, np.float32, "ema")
     _chk(theta, np.float32, "theta", ema.size)
     return lib().oracle_ema(_ptr(ema), _ptr(theta), ema.size, alpha)
+
+
+class fp32_mirror:
+    """Context manager: inside it the oracle computes in fp32 exactly as DESIGN.md readings R9/R10 state the GPU does
+    (fp32 adds in the listed order, the five stated FMAs) -- a diagnostic that a GPU result must match BIT FOR BIT.
+    The double-arithmetic oracle outside it stays the graded truth."""
+
+    def __enter__(self):
+        self.prev = lib().oracle_set_fp32_mirror(1)
+        return self
+
+    def __exit__(self, *exc):
+        lib().oracle_set_fp32_mirror(self.prev)
+        return False
 
 
 def num_threads() -> int:
