@@ -377,6 +377,27 @@ def run_psync(args, cfg, rank, world, dist):
         except Exception:  # noqa: BLE001
             pass
 
+    # What this box's HBM gives a plain stream right now (K0 probes of the library, same process, same clocks):
+    # a read-only pass over the gradient buffers of one set and a copy between two of them.  MEASURED_PEAKS's
+    # number is a copy; the fused kernel is 96 % reads, so the read-only probe is the closer ceiling.
+    if not args.no_probe and torch.cuda.mem_get_info()[0] > 12e9:
+        src = torch.zeros(1 << 30, dtype=torch.float32, device=dev)          # 4 GiB >> L2
+        dst = torch.empty_like(src)
+        sink = torch.zeros(4, dtype=torch.float32, device=dev)
+        pe = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        for rep in range(3):                               # the first repetitions are the warm-up
+            pe[0].record(stream)
+            rbytes = B.psync_probe_read(src, sink, stream)
+            pe[1].record(stream)
+            cbytes = B.psync_probe_copy(dst, src, stream)
+            pe[2].record(stream)
+            torch.cuda.synchronize()
+        read_gbs = rbytes / (pe[0].elapsed_time(pe[1]) * 1e-3) / 1e9
+        out["roofline"]["probe_read_gbs"] = read_gbs
+        out["roofline"]["frac_of_probe_read"] = achieved / read_gbs
+        out["roofline"]["probe_copy_gbs"] = cbytes / (pe[1].elapsed_time(pe[2]) * 1e-3) / 1e9
+        del src, dst
+
     # free the resident gradient sets before the host-buffer (e2e) leg
     del tables, steps_struct
     torch.cuda.empty_cache()
@@ -456,6 +477,7 @@ def main():
                          "PCIe on this box against 52 GB/s with the library default of 2^20)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-probe", action="store_true", help="skip the live HBM stream probes")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--clock-period-ms", type=float, default=2.0)
     ap.add_argument("--probe-every", type=int, default=4)
