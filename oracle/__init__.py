@@ -62,6 +62,8 @@ def lib() -> ctypes.CDLL:
                                          ctypes.c_int, ctypes.c_int, f32, f32, f32, f32, f32]
         L.oracle_kth_arrival_stats.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp]
         L.oracle_kth_arrival_stats.restype = ctypes.c_int
+        L.oracle_interp_iterations.argtypes = [vp, vp, i32, i32, vp]
+        L.oracle_interp_iterations.restype = ctypes.c_int
         L.oracle_lr_schedule.argtypes = [f32, f32, i64, i32, ctypes.c_double, vp]
         L.oracle_lr_schedule.restype = ctypes.c_int
         L.oracle_clip_scales.argtypes = [vp, i32, i64, ctypes.c_int, f32, vp]
@@ -223,6 +225,18 @@ def kth_arrival_stats(arrival, iters=None):
         raise ValueError("oracle_kth_arrival_stats: invalid arguments")
     if est is not None:
         out["est_time"] = est
+    return out
+
+
+def interp_iterations(N_pts, iters_pts, W):
+    """Fig. 5's measured points linearly interpolated to every N = 1..W -> float64 [W]."""
+    N_pts = np.ascontiguousarray(N_pts, dtype=np.int32)
+    iters_pts = np.ascontiguousarray(iters_pts, dtype=np.float64)
+    if N_pts.size != iters_pts.size:
+        raise ValueError("one iteration count per N")
+    out = np.zeros(max(W, 0), dtype=np.float64)
+    if lib().oracle_interp_iterations(_ptr(N_pts), _ptr(iters_pts), N_pts.size, W, _ptr(out)) != OK:
+        raise ValueError("oracle_interp_iterations: invalid arguments")
     return out
 
 

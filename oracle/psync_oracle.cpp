@@ -576,6 +576,31 @@ int oracle_kth_arrival_stats(const float* arrival, int32_t T, int32_t W, float* 
   return ORACLE_OK;
 }
 
+// Iterations to converge as a function of N, for Fig. 6's estimate: "we can estimate the iterations required
+// from Figure 5 (linearly interpolating for values of N for which we did not collect data)" (L193).
+//   N_pts[n_pts] strictly ascending worker counts with measured iterations iters_pts[n_pts]
+//   iters[W] OUT: entry k is the value for N = k+1 gradients; below the first / above the last measured N the
+//   nearest measured value is held (the paper interpolates only; reading R23).
+int oracle_interp_iterations(const int32_t* N_pts, const double* iters_pts, int32_t n_pts, int32_t W, double* iters) {
+  if (!N_pts || !iters_pts || !iters || n_pts < 1 || W < 1) return ORACLE_EINVAL;
+  for (int32_t p = 1; p < n_pts; ++p)
+    if (N_pts[p] <= N_pts[p - 1]) return ORACLE_EINVAL;
+  for (int32_t k = 0; k < W; ++k) {
+    const int32_t N = k + 1;
+    if (N <= N_pts[0]) {
+      iters[k] = iters_pts[0];
+    } else if (N >= N_pts[n_pts - 1]) {
+      iters[k] = iters_pts[n_pts - 1];
+    } else {
+      int32_t p = 0;
+      while (N_pts[p + 1] < N) ++p;  // N_pts[p] < N <= N_pts[p+1]
+      const double num = (iters_pts[p + 1] - iters_pts[p]) * static_cast<double>(N - N_pts[p]);
+      iters[k] = iters_pts[p] + num / static_cast<double>(N_pts[p + 1] - N_pts[p]);
+    }
+  }
+  return ORACLE_OK;
+}
+
 // fp32 mirror switch (diagnostic, see above); returns the previous setting.
 int oracle_set_fp32_mirror(int on) {
   const int prev = g_fp32_mirror;

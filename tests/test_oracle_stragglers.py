@@ -82,3 +82,34 @@ def test_invalid_arguments():
         oracle.kth_arrival_stats(np.zeros((0, 3), np.float32))
     with pytest.raises(ValueError):
         oracle.kth_arrival_stats(np.zeros(3, np.float32))
+
+
+# ------------------------------------------------------------------ Fig. 5 -> Fig. 6: iterations(N), interpolated
+def test_interp_iterations_paper_points():
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_fig5_points.json")) as fh:
+        g = json.load(fh)
+    it = oracle.interp_iterations(g["N"], g["iterations"], 106)
+    for n, want in g["interpolated"].items():
+        assert abs(it[int(n) - 1] - want) <= 1e-9 * want
+    assert 0.55 < it[99] / it[49] < 0.56                       # "nearly halves" (L181)
+    assert (it[:50] == 137500.0).all() and (it[99:] == 76200.0).all()      # held outside the measured range (R23)
+    assert (np.diff(it[49:100]) < 0).all()
+
+
+def test_interp_iterations_against_numpy_interp_and_fig6_product():
+    rng = np.random.default_rng(11)
+    N_pts = np.array([50, 70, 80, 90, 100], np.int32)
+    iters = np.sort(rng.uniform(7e4, 1.4e5, 5))[::-1].copy()
+    W = 106
+    got = oracle.interp_iterations(N_pts, iters, W)
+    want = np.interp(np.arange(1, W + 1), N_pts, iters)        # numpy holds the end values too
+    assert np.allclose(got, want, rtol=1e-15, atol=0)
+    a = rng.lognormal(0, 0.25, (40, W)).astype(np.float32)
+    r = oracle.kth_arrival_stats(a, got)
+    assert np.allclose(r["est_time"], r["mean"] * want, rtol=1e-14)
+    best = int(np.argmin(r["est_time"][49:100])) + 50          # Fig. 6: the N in 50..100 with the least estimated time
+    assert 50 <= best <= 100
+    with pytest.raises(ValueError):
+        oracle.interp_iterations([50, 50], [1.0, 2.0], 10)
+    with pytest.raises(ValueError):
+        oracle.interp_iterations([], [], 10)
