@@ -25,7 +25,7 @@ PSYNC_MAX_WORKERS = 1024
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
            "psync_select_timeout", "psync_aggregate_update", "psync_ema", "psync_order_by_arrival", "psync_async_apply", "psync_step_device", "psync_clip_workspace_bytes",
-           "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats",
+           "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_launch_geometry", "psync_probe_read",
            "psync_probe_copy")
 
@@ -85,6 +85,8 @@ def lib() -> ctypes.CDLL:
         L.psync_clip_scales.restype = ctypes.c_int
         L.psync_kth_arrival_stats.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, vp]
         L.psync_kth_arrival_stats.restype = ctypes.c_int
+        L.psync_interp_iterations.argtypes = [vp, vp, i32, i32, vp, vp]
+        L.psync_interp_iterations.restype = ctypes.c_int
         L.psync_lr_schedule.argtypes = [f32, f32, i64, i32, ctypes.c_double, vp, vp]
         L.psync_lr_schedule.restype = ctypes.c_int
         L.psync_async_apply.restype = ctypes.c_int
@@ -333,6 +335,21 @@ def psync_kth_arrival_stats(d_arrival: torch.Tensor, d_sorted: torch.Tensor, d_c
                                        _dptr(d_est_time, torch.float64, "d_est_time"), _stream(stream))
     if check and st != PSYNC_OK:
         raise PsyncError(st, "psync_kth_arrival_stats")
+    return st
+
+
+def psync_interp_iterations(N_pts, iters_pts, W: int, d_iters: torch.Tensor, stream=None, check: bool = True) -> int:
+    """iterations(N), N = 1..W, from measured points (include/psync.h: psync_interp_iterations)."""
+    n = np.ascontiguousarray(N_pts, dtype=np.int32)
+    it = np.ascontiguousarray(iters_pts, dtype=np.float64)
+    if n.size != it.size:
+        raise ValueError("one iteration count per N")
+    if d_iters.numel() < W:
+        raise ValueError("d_iters needs W elements")
+    st = lib().psync_interp_iterations(n.ctypes.data, it.ctypes.data, n.size, W,
+                                       _dptr(d_iters, torch.float64, "d_iters"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_interp_iterations")
     return st
 
 

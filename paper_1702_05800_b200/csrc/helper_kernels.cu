@@ -229,6 +229,28 @@ __global__ void __launch_bounds__(256) column_stats_kernel(const float* __restri
   }
 }
 
+// K7c: iterations(N) for N = 1..W by linear interpolation of measured points (Fig. 5 -> Fig. 6);
+// the nearest measured value is held outside the measured range.  Explicitly rounded double operations.
+__global__ void interp_iterations_kernel(const InterpPoints pts, int32_t W, double* __restrict__ iters) {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= W) return;
+  const int N = k + 1;
+  double v;
+  if (N <= pts.N[0]) {
+    v = pts.iters[0];
+  } else if (N >= pts.N[pts.n - 1]) {
+    v = pts.iters[pts.n - 1];
+  } else {
+    int p = 0;
+    while (pts.N[p + 1] < N) ++p;
+    const double num = __dmul_rn(__dsub_rn(pts.iters[p + 1], pts.iters[p]), static_cast<double>(N - pts.N[p]));
+    v = __dadd_rn(pts.iters[p], __ddiv_rn(num, static_cast<double>(pts.N[p + 1] - pts.N[p])));
+  }
+  iters[k] = v;
+}
+
 int clip_chunks(int64_t P, int dtype) {
   const int E = dtype == 1 ? 8 : 4;
   const int64_t c = (P / E + kClipChunkUnits - 1) / kClipChunkUnits;
@@ -277,6 +299,13 @@ cudaError_t launch_kth_arrival_stats(const float* d_arrival, int32_t T, int32_t 
   pdl_config(&cfg, attr, dim3(static_cast<unsigned>(W)), dim3(256), stream);
   return cudaLaunchKernelEx(&cfg, column_stats_kernel, static_cast<const float*>(d_sorted), T, W, d_count, d_mean,
                             d_median, d_iters, d_est_time);
+}
+
+cudaError_t launch_interp_iterations(const InterpPoints& pts, int32_t W, double* d_iters, cudaStream_t stream) {
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute attr[1];
+  pdl_config(&cfg, attr, dim3(static_cast<unsigned>((W + 127) / 128)), dim3(128), stream);
+  return cudaLaunchKernelEx(&cfg, interp_iterations_kernel, pts, W, d_iters);
 }
 
 cudaError_t launch_lr_schedule(float gamma0, float beta, int64_t t0, int32_t K, double s, float* d_gamma,

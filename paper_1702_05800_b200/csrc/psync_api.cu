@@ -242,6 +242,21 @@ PSYNC_API int psync_kth_arrival_stats(const float* d_arrival, int32_t T, int32_t
              : PSYNC_ECUDA;
 }
 
+PSYNC_API int psync_interp_iterations(const int32_t* h_N, const double* h_iters, int32_t n_pts, int32_t W,
+                            double* d_iters, void* stream) {
+  if (h_N == nullptr || h_iters == nullptr || d_iters == nullptr) return PSYNC_EINVAL;
+  if (n_pts < 1 || n_pts > psync::kMaxInterpPoints || W < 1 || W > PSYNC_MAX_WORKERS) return PSYNC_EINVAL;
+  psync::InterpPoints pts;
+  pts.n = n_pts;
+  for (int32_t p = 0; p < psync::kMaxInterpPoints; ++p) {
+    pts.N[p] = p < n_pts ? h_N[p] : 0;
+    pts.iters[p] = p < n_pts ? h_iters[p] : 0.0;
+    if (p > 0 && p < n_pts && h_N[p] <= h_N[p - 1]) return PSYNC_EINVAL;
+  }
+  return psync::launch_interp_iterations(pts, W, d_iters, static_cast<cudaStream_t>(stream)) == cudaSuccess ? PSYNC_OK
+                                                                                                          : PSYNC_ECUDA;
+}
+
 PSYNC_API int psync_lr_schedule(float gamma0, float beta, int64_t t0, int32_t K, double s, float* d_gamma, void* stream) {
   if (K < 0 || t0 < 0 || !(beta > 0.0f) || (K > 0 && d_gamma == nullptr)) return PSYNC_EINVAL;
   if (K == 0) return PSYNC_OK;

@@ -212,3 +212,35 @@ def test_kth_arrival_stats_invalid_arguments():
     assert L.psync_kth_arrival_stats(8, 0, 1, 8, 8, 8, 8, None, None, None) == psync.PSYNC_EINVAL
     assert L.psync_kth_arrival_stats(8, 1, 1025, 8, 8, 8, 8, None, None, None) == psync.PSYNC_EINVAL
     assert L.psync_kth_arrival_stats(8, 1, 4, 8, 8, 8, 8, 8, None, None) == psync.PSYNC_EINVAL   # iters without est_time
+
+
+def test_interp_iterations_and_fig6_estimate_on_the_gpu():
+    """Fig. 5 -> Fig. 6: the paper's two printed points interpolated to every N, then mean time to
+    collect N gradients x iterations(N) on cfg3's synthetic arrival times; bit-equal to the oracle."""
+    W = 106
+    d_iters = torch.full((W + 1,), -1.0, dtype=torch.float64, device=DEV)
+    for N_pts, iters in (([50, 100], [137.5e3, 76.2e3]), ([50, 70, 80, 90, 100], [137.5e3, 111e3, 98.7e3, 85.1e3, 76.2e3]),
+                         ([7], [5.0])):
+        psync.psync_interp_iterations(N_pts, iters, W, d_iters)
+        got = d_iters.cpu().numpy()
+        assert np.array_equal(got[:W], oracle.interp_iterations(N_pts, iters, W)) and got[W] == -1.0
+    psync.psync_interp_iterations([50, 100], [137.5e3, 76.2e3], W, d_iters)
+    assert abs(float(d_iters[95]) - 81104.0) < 1e-6 and float(d_iters[74]) == 106850.0
+    cfg = synth.PAPER_RMSPROP
+    a = np.stack([synth.arrival_times(cfg, s) for s in range(300)])
+    it = d_iters[:W].clone()
+    d_sorted = torch.empty((300, W), dtype=torch.float32, device=DEV)
+    d_count = torch.empty(W, dtype=torch.int32, device=DEV)
+    d_mean = torch.empty(W, dtype=torch.float64, device=DEV)
+    d_median = torch.empty(W, dtype=torch.float64, device=DEV)
+    d_est = torch.empty(W, dtype=torch.float64, device=DEV)
+    psync.psync_kth_arrival_stats(torch.from_numpy(a).to(DEV), d_sorted, d_count, d_mean, d_median, it, d_est)
+    want = oracle.kth_arrival_stats(a, oracle.interp_iterations([50, 100], [137.5e3, 76.2e3], W))
+    assert np.allclose(d_est.cpu().numpy(), want["est_time"], rtol=1e-13)
+    best = int(np.argmin(d_est.cpu().numpy()[49:100])) + 50
+    assert best == int(np.argmin(want["est_time"][49:100])) + 50 and 90 <= best <= 100   # a few backups win, as in Fig. 6
+    L = psync.binding.lib()
+    n2 = np.array([50, 50], np.int32); i2 = np.array([1.0, 2.0])
+    assert L.psync_interp_iterations(n2.ctypes.data, i2.ctypes.data, 2, W, d_iters.data_ptr(), None) == psync.PSYNC_EINVAL
+    assert L.psync_interp_iterations(n2.ctypes.data, i2.ctypes.data, 0, W, d_iters.data_ptr(), None) == psync.PSYNC_EINVAL
+    assert L.psync_interp_iterations(None, i2.ctypes.data, 1, W, d_iters.data_ptr(), None) == psync.PSYNC_EINVAL
