@@ -362,6 +362,7 @@ def run_psync(args, cfg, rank, world, dist):
         "gbps_model": bytes_per_step * K * world / (max_ms * 1e-3) / 1e9,
         "params_per_s": float(cfg.P) * K * world / (max_ms * 1e-3),
         "select_ms": select_ms, "fused_ms": fused_ms, "kernel_events_on_steps": len(fused_list),
+        "fused_ms_min_median_max": [float(np.min(fused_list)), float(np.median(fused_list)), float(np.max(fused_list))],
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": None, "peak_source": peak_src, "kernel": "async_apply_kernel" if mode == "async" else "fused_aggregate_update_ema",
                      "algorithmic_bytes_per_launch": bytes_per_step,
@@ -406,6 +407,17 @@ def run_psync(args, cfg, rank, world, dist):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         _, info = oracle_sample(cfg, seconds_budget=args.cpu_seconds, sample_elems=1 << 22)
         out["cpu_baseline"] = {k: info[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        if args.cpu_seconds_1thread > 0:       # the oracle single-threaded as well (a short sample)
+            import oracle
+            threads = oracle.num_threads()
+            oracle.set_num_threads(1)
+            try:
+                v1, info1 = oracle_sample(cfg, seconds_budget=args.cpu_seconds_1thread, sample_elems=1 << 20,
+                                          wall_budget=20.0)
+            finally:
+                oracle.set_num_threads(threads)
+            out["cpu_baseline"]["value_1thread"] = v1
+            out["cpu_baseline"]["sample_1thread"] = info1["sample"]
     return out
 
 
@@ -479,6 +491,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-probe", action="store_true", help="skip the live HBM stream probes")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--cpu-seconds-1thread", type=float, default=3.0)
     ap.add_argument("--clock-period-ms", type=float, default=2.0)
     ap.add_argument("--probe-every", type=int, default=4)
     ap.add_argument("--ref-sample-elems", type=int, default=0)
