@@ -279,3 +279,62 @@ def test_stale_gradients_of_dropped_workers_carry_into_the_next_step_and_are_dro
     before = to_np(pair.ps.theta)
     st_g, _, _ = pair.gpu_step(pair.gradients(9), synth.arrival_times(cfg, 9), tags=tags, t=9)
     assert st_g == psync.PSYNC_ETOOFEW and np.array_equal(before, to_np(pair.ps.theta))
+
+
+# ------------------------------------------------------------------ re-entrancy and 64-bit indexing
+def test_two_servers_on_two_streams_are_independent():
+    """The library keeps no state: two servers stepping concurrently on two streams give, bit for bit, what each
+    gives alone."""
+    cfg = synth.scaled(synth.PAPER_RMSPROP, 2_000_003)
+    results = []
+    for concurrent in (False, True):
+        pairs = [Pair(cfg), Pair(replace(cfg, cfg_id=33))]
+        grads = [p.gradients(0) for p in pairs]
+        for p, g in zip(pairs, grads):
+            p.ps.set_gradients(g)
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()] if concurrent else [torch.cuda.current_stream()] * 2
+        torch.cuda.synchronize()
+        for s in range(6):
+            for p, st in zip(pairs, streams):
+                d_arr = torch.from_numpy(synth.arrival_times(p.cfg, s)).to(DEV)
+                st.wait_stream(torch.cuda.current_stream())
+                p.ps.step(d_arr, cfg.gamma, stream=st)
+                d_arr.record_stream(st)
+        torch.cuda.synchronize()
+        results.append([[to_np(getattr(p.ps, n)) for n in ("theta", "ema", "state0", "state1", "d_kept")]
+                        for p in pairs])
+    for alone, together in zip(results[0], results[1]):
+        for a, b_ in zip(alone, together):
+            assert np.array_equal(a, b_)
+
+
+def test_more_than_2_to_31_parameters_sampled():
+    """P = 2^31 + 2^20 + 5: element indices and byte offsets need 64 bits (the last tile starts beyond 8 GiB).
+    SGD + EMA, N=2, b=1; sampled elements (first and last tiles, around 2^31, random) against the oracle."""
+    P = (1 << 31) + (1 << 20) + 5
+    cfg = replace(synth.INCEPTION_SGD, P=P, M=3, N=2, b=1, name="huge_P")
+    free, _ = torch.cuda.mem_get_info()
+    if cfg.footprint_bytes * 1.3 > free:
+        pytest.skip("not enough free HBM for 2^31 parameters")
+    pair = Pair(cfg)
+    rng = np.random.default_rng(2)
+    idx = np.unique(np.concatenate([np.arange(0, 2048), np.arange(P - 2048, P),
+                                    np.arange((1 << 31) - 1500, (1 << 31) + 1500),
+                                    pair.shard_off[1:-1], rng.integers(0, P, 20_000)])).astype(np.int64)
+    d_idx = torch.from_numpy(idx).to(DEV)
+    off_s = np.array([0, idx.size], dtype=np.int64)
+    host = {n: to_np(getattr(pair.ps, n)[d_idx]) for n in ("theta", "ema")}
+    grads = [torch.empty(P, dtype=torch.float32, device=DEV) for _ in range(cfg.W)]
+    for k in range(cfg.W):
+        synth.gradient(cfg, 0, k, DEV, out=grads[k])
+    arrival = synth.arrival_times(cfg, 0)
+    st, kept, _ = pair.gpu_step(grads, arrival)
+    st_o, kept_o, _ = oracle.select_first_n(arrival, cfg.N, cfg.b)
+    assert st == st_o == 0 and np.array_equal(kept, kept_o)
+    rc = oracle.aggregate_update(off_s, cfg.N, [synth.as_numpy_grad(g[d_idx]) for g in grads], kept_o, host["theta"],
+                                 host["ema"], opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha)
+    assert rc == oracle.OK
+    for n in ("theta", "ema"):
+        assert_close(to_np(getattr(pair.ps, n)[d_idx]), host[n], RTOL_STEP, ATOL_STEP, f"huge P {n} (sampled)")
+    geo = pair.ps.geometry(cfg.gamma)
+    assert geo["grid"] == -(-P // geo["tile_elems"]) and geo["grid"] > (1 << 21)
