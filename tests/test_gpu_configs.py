@@ -338,3 +338,14 @@ def test_more_than_2_to_31_parameters_sampled():
         assert_close(to_np(getattr(pair.ps, n)[d_idx]), host[n], RTOL_STEP, ATOL_STEP, f"huge P {n} (sampled)")
     geo = pair.ps.geometry(cfg.gamma)
     assert geo["grid"] == -(-P // geo["tile_elems"]) and geo["grid"] > (1 << 21)
+
+
+def test_full_size_largest_sweep_point_sampled():
+    """cfg5's largest point at full size: P = 256 Mi, N = 100, b = 10, M = 64 ragged (120.3 GB resident)."""
+    cfg = [c for c in synth.sweep_configs() if c.P == synth.SWEEP_P[-1] and c.M == 64 and c.N == 100][0]
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    if cfg.footprint_bytes * 1.1 > free:
+        pytest.skip("not enough free HBM for the 120 GB sweep point")
+    _full_size_sampled(cfg, steps=1, n_sample=20_000)
+    torch.cuda.empty_cache()
