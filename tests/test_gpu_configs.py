@@ -349,3 +349,21 @@ def test_full_size_largest_sweep_point_sampled():
         pytest.skip("not enough free HBM for the 120 GB sweep point")
     _full_size_sampled(cfg, steps=1, n_sample=20_000)
     torch.cuda.empty_cache()
+
+
+def test_plain_c_client_of_the_abi(tmp_path):
+    """A C program (gcc, no Python, no torch) includes include/psync.h, links libpsync.so and runs one hand-checkable
+    step: the boundary really is a C ABI with plain pointers."""
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cuda = os.environ.get("CUDA_HOME", "/usr/local/cuda")
+    exe = tmp_path / "abi_smoke"
+    pkg = os.path.join(root, "paper_1702_05800_b200")
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-O1", os.path.join(root, "tests", "c", "abi_smoke.c"),
+                    "-I", os.path.join(root, "include"), "-I", os.path.join(cuda, "include"), "-L", pkg, "-lpsync",
+                    "-L", os.path.join(cuda, "lib64"), "-lcudart", "-lm", f"-Wl,-rpath,{pkg}",
+                    f"-Wl,-rpath,{os.path.join(cuda, 'lib64')}", "-o", str(exe)], check=True)
+    out = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert out.returncode == 0, out.stderr
+    assert "abi_smoke ok" in out.stdout
