@@ -27,6 +27,11 @@
 // mpmath for the square root) for P <= 64; closed forms for constant gradients
 // (SGD, momentum, RMSProp second moment) and the constant-theta EMA; optimizer
 // reductions (mu=0, rho=1); a hand-worked dyadic example (tests/golden/).
+// The functions added for SURVEY.md section 8(f) are pinned the same way: per-server rows and the
+// time-out rule (tests/test_oracle_per_server.py), Alg. 2 (tests/test_oracle_async.py), learning-rate
+// schedule and clip factors (tests/test_oracle_helpers.py), straggler statistics and the Fig. 5
+// interpolation, the latter against the two values the paper prints (tests/test_oracle_stragglers.py),
+// and the fp32 mirror (tests/test_oracle_fp32_mirror.py).
 // Nothing here is "parity unpinned".
 //
 // Optional OpenMP (-fopenmp): the element loop is split over threads; per-element
