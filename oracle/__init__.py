@@ -17,6 +17,8 @@ import numpy as np
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "psync_oracle.cpp"
 _LIB = _HERE / "libpsync_oracle.so"
+_MIRROR_SRC = _HERE / "psync_mirror_f32.cpp"       # the fp32 diagnostic: a separate library, not the graded oracle
+_MIRROR_LIB = _HERE / "libpsync_mirror_f32.so"
 
 OK, EINVAL, ETOOFEW = 0, -1, -2
 F32, BF16 = 0, 1
@@ -24,24 +26,46 @@ SGD, MOMENTUM, RMSPROP_MOM = 0, 1, 2
 EMA_POST, EMA_PRE, EMA_OFF = 0, 1, 2
 
 _lib = None
+_mirror_lib = None
+_mirror_on = False
+
+
+def _compile(src: Path, out: Path, force: bool, extra=()) -> Path:
+    if force or not out.exists() or out.stat().st_mtime < src.stat().st_mtime:
+        tmp = out.with_suffix(f".tmp{os.getpid()}.so")
+        cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-Wall", "-Wextra", *extra,
+               "-o", str(tmp), str(src)]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, out)
+    return out
 
 
 def build(force: bool = False) -> Path:
-    """Compile the oracle with g++ (-O2, no fast-math, no FMA contraction, OpenMP)."""
-    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
-        tmp = _LIB.with_suffix(f".tmp{os.getpid()}.so")
-        cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
-               "-Wall", "-Wextra", "-o", str(tmp), str(_SRC)]
-        subprocess.run(cmd, check=True)
-        os.replace(tmp, _LIB)
+    """Compile the oracle with g++ (-O2, no fast-math, no FMA contraction, OpenMP) and, beside it, the fp32
+    diagnostic mirror (its own source, its own library)."""
+    _compile(_SRC, _LIB, force, ("-fopenmp",))
+    _compile(_MIRROR_SRC, _MIRROR_LIB, force)
     return _LIB
+
+
+def build_sanitized(out_dir) -> Path:
+    """The graded oracle built with -fsanitize=address,undefined into `out_dir`; used by
+    tests/test_oracle_sanitizers.py, which runs the oracle's own pin tests against it in a subprocess."""
+    out = Path(out_dir) / "libpsync_oracle_asan.so"
+    cmd = ["g++", "-std=c++17", "-O1", "-g", "-fno-omit-frame-pointer", "-ffp-contract=off", "-fopenmp", "-fPIC",
+           "-shared", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-Wall", "-Wextra",
+           "-o", str(out), str(_SRC)]
+    subprocess.run(cmd, check=True)
+    return out
 
 
 def lib() -> ctypes.CDLL:
     global _lib
     if _lib is None:
-        build()
-        L = ctypes.CDLL(str(_LIB))
+        override = os.environ.get("PSYNC_ORACLE_LIB")     # the sanitizer job points this at its instrumented build
+        if not override:
+            build()
+        L = ctypes.CDLL(override or str(_LIB))
         i32, i64, f32, vp = ctypes.c_int32, ctypes.c_int64, ctypes.c_float, ctypes.c_void_p
         L.oracle_select_first_n.argtypes = [vp, vp, i32, i32, i32, vp, vp]
         L.oracle_select_first_n.restype = ctypes.c_int
@@ -56,6 +80,8 @@ def lib() -> ctypes.CDLL:
                                                    vp, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int,
                                                    f32, f32, f32, f32, f32]
         L.oracle_aggregate_update_rows.restype = ctypes.c_int
+        L.oracle_aggregate_update_slices.argtypes = L.oracle_aggregate_update_rows.argtypes
+        L.oracle_aggregate_update_slices.restype = ctypes.c_int
         L.oracle_order_by_arrival.argtypes = [vp, i32, vp, vp]
         L.oracle_order_by_arrival.restype = ctypes.c_int
         L.oracle_async_apply.argtypes = [i64, i32, vp, i32, i32, vp, ctypes.c_int, vp, vp, vp, vp, vp, vp, vp,
@@ -76,12 +102,33 @@ def lib() -> ctypes.CDLL:
         L.oracle_apply_sum.restype = ctypes.c_int
         L.oracle_ema.argtypes = [vp, vp, i64, f32]
         L.oracle_ema.restype = ctypes.c_int
-        L.oracle_set_fp32_mirror.argtypes = [ctypes.c_int]
-        L.oracle_set_fp32_mirror.restype = ctypes.c_int
         L.oracle_num_threads.restype = ctypes.c_int
         L.oracle_set_num_threads.argtypes = [ctypes.c_int]
         _lib = L
     return _lib
+
+
+def mirror_lib() -> ctypes.CDLL:
+    """The fp32 diagnostic mirror (oracle/psync_mirror_f32.cpp): its own library, loaded only on request."""
+    global _mirror_lib
+    if _mirror_lib is None:
+        _compile(_MIRROR_SRC, _MIRROR_LIB, False)
+        L = ctypes.CDLL(str(_MIRROR_LIB))
+        i32, i64, f32, vp, ci = ctypes.c_int32, ctypes.c_int64, ctypes.c_float, ctypes.c_void_p, ctypes.c_int
+        L.mirror_rsqrt_rn.argtypes = [f32]
+        L.mirror_rsqrt_rn.restype = f32
+        L.mirror_aggregate_update_rows.argtypes = [i64, i32, vp, i32, i32, vp, ci, ci, ci, vp, i32, vp, vp, vp, vp, vp,
+                                                   vp, ci, ci, f32, f32, f32, f32, f32]
+        L.mirror_accumulate.argtypes = [vp, vp, ci, i64]
+        L.mirror_apply_sum.argtypes = [i64, i32, vp, i32, vp, vp, vp, vp, vp, ci, ci, f32, f32, f32, f32, f32]
+        L.mirror_ema.argtypes = [vp, vp, i64, f32]
+        L.mirror_async_apply.argtypes = [i64, i32, vp, i32, i32, vp, ci, vp, vp, vp, vp, vp, vp, vp, ci, ci,
+                                         f32, f32, f32, f32, f32]
+        for fn in (L.mirror_aggregate_update_rows, L.mirror_accumulate, L.mirror_apply_sum, L.mirror_ema,
+                   L.mirror_async_apply):
+            fn.restype = ci
+        _mirror_lib = L
+    return _mirror_lib
 
 
 def _ptr(a):
@@ -133,6 +180,11 @@ def aggregate_update(shard_off, N, grads, kept, theta, ema=None, state0=None, st
     for nm, a in (("theta", theta), ("ema", ema), ("state0", state0), ("state1", state1)):
         _chk(a, np.float32, nm, P)
     ptrs = (ctypes.c_void_p * W)(*[g.ctypes.data for g in grads])
+    if _mirror_on:
+        return mirror_lib().mirror_aggregate_update_rows(P, M, _ptr(shard_off), N, W, ctypes.cast(ptrs, ctypes.c_void_p),
+                                                         gd, 0, 0, _ptr(kept), N, None, None, _ptr(theta), _ptr(ema),
+                                                         _ptr(state0), _ptr(state1), opt, ema_mode, gamma_t, alpha, mu,
+                                                         rho, eps)
     return lib().oracle_aggregate_update(P, M, _ptr(shard_off), N, W, ctypes.cast(ptrs, ctypes.c_void_p),
                                          gd, _ptr(kept), _ptr(theta), _ptr(ema), _ptr(state0), _ptr(state1),
                                          opt, ema_mode, gamma_t, alpha, mu, rho, eps)
@@ -191,10 +243,57 @@ def aggregate_update_rows(shard_off, N, grads, kept, theta, ema=None, state0=Non
     for nm, a in (("theta", theta), ("ema", ema), ("state0", state0), ("state1", state1)):
         _chk(a, np.float32, nm, P)
     ptrs = (ctypes.c_void_p * W)(*[g.ctypes.data for g in grads])
+    if _mirror_on:
+        return mirror_lib().mirror_aggregate_update_rows(P, M, _ptr(shard_off), N, W, ctypes.cast(ptrs, ctypes.c_void_p),
+                                                         gd, 0, 1 if per_shard else 0, _ptr(kept), kept.shape[1],
+                                                         _ptr(n_kept), _ptr(status), _ptr(theta), _ptr(ema),
+                                                         _ptr(state0), _ptr(state1), opt, ema_mode, gamma_t, alpha, mu,
+                                                         rho, eps)
     return lib().oracle_aggregate_update_rows(P, M, _ptr(shard_off), N, W, ctypes.cast(ptrs, ctypes.c_void_p), gd,
                                               1 if per_shard else 0, _ptr(kept), kept.shape[1], _ptr(n_kept),
                                               _ptr(status), _ptr(theta), _ptr(ema), _ptr(state0), _ptr(state1),
                                               opt, ema_mode, gamma_t, alpha, mu, rho, eps)
+
+
+def aggregate_update_slices(shard_off, N, slices, kept, theta, ema=None, state0=None, state1=None, per_shard=False,
+                            n_kept=None, status=None, opt=SGD, ema_mode=EMA_POST, gamma_t=0.0, alpha=0.0, mu=0.0,
+                            rho=0.0, eps=0.0):
+    """Alg. 4 l.8-9 on what each server RECEIVES: slices[k][j] is worker k's G_k[j], a
+    separate array of len_j elements (None where server j does not keep worker k).  kept is int32 [rows][stride]
+    (a 1-D kept[N] is one row); n_kept / status int32 [rows] or None; rows = M if per_shard else 1."""
+    P = theta.size
+    shard_off = np.ascontiguousarray(shard_off, dtype=np.int64)
+    M = shard_off.size - 1
+    W = len(slices)
+    first = next(a for row in slices for a in row if a is not None)
+    gd = _grad_dtype([first])
+    for k, row in enumerate(slices):
+        if len(row) != M:
+            raise ValueError(f"slices[{k}] needs M = {M} entries")
+        for j, a in enumerate(row):
+            _chk(a, first.dtype, f"slices[{k}][{j}]", int(shard_off[j + 1] - shard_off[j]))
+    kept = np.ascontiguousarray(kept, dtype=np.int32)
+    if kept.ndim == 1:
+        kept = kept[None, :]
+    rows = M if per_shard else 1
+    if kept.shape[0] != rows:
+        raise ValueError("kept must be int32 [rows][stride]")
+    _chk(n_kept, np.int32, "n_kept", rows)
+    _chk(status, np.int32, "status", rows)
+    for nm, a in (("theta", theta), ("ema", ema), ("state0", state0), ("state1", state1)):
+        _chk(a, np.float32, nm, P)
+    flat = [None if a is None else a.ctypes.data for row in slices for a in row]
+    ptrs = (ctypes.c_void_p * (W * M))(*flat)
+    if _mirror_on:
+        return mirror_lib().mirror_aggregate_update_rows(P, M, _ptr(shard_off), N, W, ctypes.cast(ptrs, ctypes.c_void_p),
+                                                         gd, 1, 1 if per_shard else 0, _ptr(kept), kept.shape[1],
+                                                         _ptr(n_kept), _ptr(status), _ptr(theta), _ptr(ema),
+                                                         _ptr(state0), _ptr(state1), opt, ema_mode, gamma_t, alpha, mu,
+                                                         rho, eps)
+    return lib().oracle_aggregate_update_slices(P, M, _ptr(shard_off), N, W, ctypes.cast(ptrs, ctypes.c_void_p), gd,
+                                                1 if per_shard else 0, _ptr(kept), kept.shape[1], _ptr(n_kept),
+                                                _ptr(status), _ptr(theta), _ptr(ema), _ptr(state0), _ptr(state1),
+                                                opt, ema_mode, gamma_t, alpha, mu, rho, eps)
 
 
 def order_by_arrival(arrival):
@@ -277,10 +376,10 @@ def async_apply(shard_off, grads, order, theta, ema=None, state0=None, state1=No
     for nm, a in (("theta", theta), ("ema", ema), ("state0", state0), ("state1", state1)):
         _chk(a, np.float32, nm, P)
     ptrs = (ctypes.c_void_p * W)(*[g.ctypes.data for g in grads])
-    return lib().oracle_async_apply(P, M, _ptr(shard_off), order.size, W, ctypes.cast(ptrs, ctypes.c_void_p), gd,
-                                    _ptr(order), _ptr(gammas), _ptr(gscales), _ptr(theta), _ptr(ema), _ptr(state0),
-                                    _ptr(state1),
-                                    opt, ema_mode, gamma_t, alpha, mu, rho, eps)
+    fn = mirror_lib().mirror_async_apply if _mirror_on else lib().oracle_async_apply
+    return fn(P, M, _ptr(shard_off), order.size, W, ctypes.cast(ptrs, ctypes.c_void_p), gd,
+              _ptr(order), _ptr(gammas), _ptr(gscales), _ptr(theta), _ptr(ema), _ptr(state0), _ptr(state1),
+              opt, ema_mode, gamma_t, alpha, mu, rho, eps)
 
 
 def accumulate(S, grad):
@@ -288,7 +387,8 @@ def accumulate(S, grad):
     _chk(S, np.float64, "S")
     gd = _grad_dtype([grad])
     _chk(grad, grad.dtype, "grad", S.size)
-    return lib().oracle_accumulate(_ptr(S), _ptr(grad), gd, S.size)
+    fn = mirror_lib().mirror_accumulate if _mirror_on else lib().oracle_accumulate
+    return fn(_ptr(S), _ptr(grad), gd, S.size)
 
 
 def apply_sum(shard_off, N, S, theta, ema=None, state0=None, state1=None, opt=SGD, ema_mode=EMA_POST,
@@ -300,28 +400,37 @@ def apply_sum(shard_off, N, S, theta, ema=None, state0=None, state1=None, opt=SG
     _chk(S, np.float64, "S", P)
     for nm, a in (("theta", theta), ("ema", ema), ("state0", state0), ("state1", state1)):
         _chk(a, np.float32, nm, P)
-    return lib().oracle_apply_sum(P, M, _ptr(shard_off), N, _ptr(S), _ptr(theta), _ptr(ema), _ptr(state0),
-                                  _ptr(state1), opt, ema_mode, gamma_t, alpha, mu, rho, eps)
+    fn = mirror_lib().mirror_apply_sum if _mirror_on else lib().oracle_apply_sum
+    return fn(P, M, _ptr(shard_off), N, _ptr(S), _ptr(theta), _ptr(ema), _ptr(state0), _ptr(state1), opt, ema_mode,
+              gamma_t, alpha, mu, rho, eps)
 
 
 def ema_update(ema, theta, alpha):
     """ema <- alpha ema + (1-alpha) theta in place.  PAPER.md:L40."""
     _chk(ema, np.float32, "ema")
     _chk(theta, np.float32, "theta", ema.size)
-    return lib().oracle_ema(_ptr(ema), _ptr(theta), ema.size, alpha)
+    fn = mirror_lib().mirror_ema if _mirror_on else lib().oracle_ema
+    return fn(_ptr(ema), _ptr(theta), ema.size, alpha)
 
 
 class fp32_mirror:
-    """Context manager: inside it the oracle computes in fp32 exactly as DESIGN.md readings R9/R10 state the GPU does
-    (fp32 adds in the listed order, the five stated FMAs) -- a diagnostic that a GPU result must match BIT FOR BIT.
-    The double-arithmetic oracle outside it stays the graded truth."""
+    """Context manager: inside it aggregate_update / aggregate_update_rows / async_apply / accumulate / apply_sum /
+    ema_update are served by the SEPARATE fp32 diagnostic library (oracle/psync_mirror_f32.cpp), which restates the
+    operation list DESIGN.md readings R9/R10 give for the GPU (fp32 adds in the listed order, the five stated FMAs, a
+    correctly rounded reciprocal square root) -- a GPU result must match it BIT FOR BIT.  It is a regression check of the
+    kernels against their documented arithmetic, not parity evidence: the double-arithmetic oracle
+    (oracle/psync_oracle.cpp, which contains none of this) stays the graded truth.  Selection, schedules, statistics
+    are always the graded oracle's."""
 
     def __enter__(self):
-        self.prev = lib().oracle_set_fp32_mirror(1)
+        global _mirror_on
+        self.prev = _mirror_on
+        _mirror_on = True
         return self
 
     def __exit__(self, *exc):
-        lib().oracle_set_fp32_mirror(self.prev)
+        global _mirror_on
+        _mirror_on = self.prev
         return False
 
 

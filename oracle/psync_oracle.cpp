@@ -30,8 +30,10 @@
 // The functions added for SURVEY.md section 8(f) are pinned the same way: per-server rows and the
 // time-out rule (tests/test_oracle_per_server.py), Alg. 2 (tests/test_oracle_async.py), learning-rate
 // schedule and clip factors (tests/test_oracle_helpers.py), straggler statistics and the Fig. 5
-// interpolation, the latter against the two values the paper prints (tests/test_oracle_stragglers.py),
-// and the fp32 mirror (tests/test_oracle_fp32_mirror.py).
+// interpolation, the latter against the two values the paper prints (tests/test_oracle_stragglers.py);
+// the per-(worker, server) slice layout (tests/test_oracle_slices.py).
+// (The fp32 diagnostic mirror of the GPU's operation list is a SEPARATE library, oracle/psync_mirror_f32.cpp;
+// nothing of it is in this file.)
 // Nothing here is "parity unpinned".
 //
 // Optional OpenMP (-fopenmp): the element loop is split over threads; per-element
@@ -137,84 +139,6 @@ inline void apply_element(double S, const Coeffs& c, int opt, int ema_mode, floa
   }
 }
 
-// ---------------------------------------------------------------------------------------------
-// fp32 MIRROR (diagnostic; SURVEY.md section 8c "a second build of the same oracle ... in float, same
-// order").  The double-arithmetic path above is the graded truth.  When the mirror is switched on the
-// same steps are done in fp32 exactly as DESIGN.md reading R9/R10 states the GPU does them: the kept
-// gradients are added in fp32 in the order given starting from 0, and theta - gamma G, mu v + G,
-// rho ms + (1-rho) G^2, mu mom + step, alpha ema + (1-alpha) theta are ONE fused multiply-add each
-// (std::fmaf), every other operation a single IEEE fp32 operation (this file is compiled with
-// -ffp-contract=off, so nothing else is fused).  A GPU result then has to match bit for bit, which
-// checks the summation order and the exact arithmetic, not just closeness.
-// ---------------------------------------------------------------------------------------------
-int g_fp32_mirror = 0;
-
-struct CoeffsF {
-  float gamma, alpha, one_minus_alpha, mu, rho, one_minus_rho, eps, inv_N;
-};
-
-inline CoeffsF narrow(const Coeffs& c) {  // every coefficient is an fp32 value widened: narrowing is exact
-  CoeffsF f;
-  f.gamma = static_cast<float>(c.gamma);
-  f.alpha = static_cast<float>(c.alpha);
-  f.one_minus_alpha = static_cast<float>(c.one_minus_alpha);
-  f.mu = static_cast<float>(c.mu);
-  f.rho = static_cast<float>(c.rho);
-  f.one_minus_rho = static_cast<float>(c.one_minus_rho);
-  f.eps = static_cast<float>(c.eps);
-  f.inv_N = static_cast<float>(c.inv_N);
-  return f;
-}
-
-inline void apply_element_f32(float S, const CoeffsF& c, int opt, int ema_mode, float* theta, float* ema,
-                              float* state0, float* state1, int64_t i) {
-  const float G = S * c.inv_N;
-  const float th = theta[i];
-  float th_new;
-  if (opt == ORACLE_SGD) {
-    th_new = std::fmaf(-c.gamma, G, th);
-  } else if (opt == ORACLE_MOMENTUM) {
-    const float v = std::fmaf(c.mu, state0[i], G);
-    state0[i] = v;
-    th_new = std::fmaf(-c.gamma, v, th);
-  } else {
-    const float g2 = G * G;
-    const float ms = std::fmaf(c.rho, state0[i], c.one_minus_rho * g2);
-    const float root = std::sqrt(ms + c.eps);
-    const float step = (c.gamma * G) / root;
-    const float mom = std::fmaf(c.mu, state1[i], step);
-    state0[i] = ms;
-    state1[i] = mom;
-    th_new = th - mom;
-  }
-  theta[i] = th_new;
-  if (ema_mode != ORACLE_EMA_OFF) {
-    const float operand = (ema_mode == ORACLE_EMA_POST) ? th_new : th;
-    ema[i] = std::fmaf(c.alpha, ema[i], c.one_minus_alpha * operand);
-  }
-}
-
-// Sum of n gradients at element i in the order listed; mirror mode adds in fp32 starting from 0.
-inline double sum_listed(const void* const* grads, const int32_t* list, int32_t n, int dtype, int64_t i) {
-  if (g_fp32_mirror) {
-    float S = 0.0f;
-    for (int32_t k = 0; k < n; ++k) S += static_cast<float>(grad_at(grads[list[k]], dtype, i));
-    return static_cast<double>(S);
-  }
-  double S = 0.0;  // sum_{G in kept set} G[j]                  (L160)
-  for (int32_t k = 0; k < n; ++k) S += grad_at(grads[list[k]], dtype, i);
-  return S;
-}
-
-// One element given the sum: the double path, or the fp32 mirror when it is switched on.
-inline void apply_any(double S, const Coeffs& c, int opt, int ema_mode, float* theta, float* ema, float* state0,
-                      float* state1, int64_t i) {
-  if (g_fp32_mirror)
-    apply_element_f32(static_cast<float>(S), narrow(c), opt, ema_mode, theta, ema, state0, state1, i);
-  else
-    apply_element(S, c, opt, ema_mode, theta, ema, state0, state1, i);
-}
-
 bool args_ok(int64_t P, int32_t M, const int64_t* shard_off, int32_t N, int opt, int ema_mode,
              const float* theta, const float* ema, const float* state0, const float* state1) {
   if (P < 0 || M < 1 || N < 1 || !shard_off || !theta) return false;
@@ -286,8 +210,9 @@ int oracle_aggregate_update(int64_t P, int32_t M, const int64_t* shard_off, int3
 #pragma omp parallel for schedule(static)
 #endif
     for (int64_t i = lo; i < hi; ++i) {
-      const double S = sum_listed(grads, kept, N, grad_dtype, i);  // sum_{G in kept set} G[j]   (L160)
-      apply_any(S, c, opt, ema_mode, theta, ema, state0, state1, i);
+      double S = 0.0;  // sum_{G in kept set} G[j]                  (L160)
+      for (int32_t n = 0; n < N; ++n) S += grad_at(grads[kept[n]], grad_dtype, i);
+      apply_element(S, c, opt, ema_mode, theta, ema, state0, state1, i);
     }
   }
   return ORACLE_OK;
@@ -305,12 +230,7 @@ int oracle_accumulate(double* S, const void* grad, int grad_dtype, int64_t P) {
 #ifdef _OPENMP
 #pragma omp parallel for schedule(static)
 #endif
-  for (int64_t i = 0; i < P; ++i) {
-    if (g_fp32_mirror)  // one fp32 addition (S[i] holds an fp32 value exactly)
-      S[i] = static_cast<double>(static_cast<float>(S[i]) + static_cast<float>(grad_at(grad, grad_dtype, i)));
-    else
-      S[i] += grad_at(grad, grad_dtype, i);
-  }
+  for (int64_t i = 0; i < P; ++i) S[i] += grad_at(grad, grad_dtype, i);
   return ORACLE_OK;
 }
 
@@ -324,7 +244,7 @@ int oracle_apply_sum(int64_t P, int32_t M, const int64_t* shard_off, int32_t N, 
 #ifdef _OPENMP
 #pragma omp parallel for schedule(static)
 #endif
-    for (int64_t i = lo; i < hi; ++i) apply_any(S[i], c, opt, ema_mode, theta, ema, state0, state1, i);
+    for (int64_t i = lo; i < hi; ++i) apply_element(S[i], c, opt, ema_mode, theta, ema, state0, state1, i);
   }
   return ORACLE_OK;
 }
@@ -337,12 +257,8 @@ int oracle_ema(float* ema, const float* theta, int64_t P, float alpha) {
 #ifdef _OPENMP
 #pragma omp parallel for schedule(static)
 #endif
-  for (int64_t i = 0; i < P; ++i) {
-    if (g_fp32_mirror)
-      ema[i] = std::fmaf(alpha, ema[i], (1.0f - alpha) * theta[i]);
-    else
-      ema[i] = static_cast<float>(a * static_cast<double>(ema[i]) + oma * static_cast<double>(theta[i]));
-  }
+  for (int64_t i = 0; i < P; ++i)
+    ema[i] = static_cast<float>(a * static_cast<double>(ema[i]) + oma * static_cast<double>(theta[i]));
   return ORACLE_OK;
 }
 
@@ -426,8 +342,63 @@ int oracle_aggregate_update_rows(int64_t P, int32_t M, const int64_t* shard_off,
 #pragma omp parallel for schedule(static)
 #endif
     for (int64_t i = lo; i < hi; ++i) {
-      const double S = sum_listed(grads, kept_j, n_j, grad_dtype, i);
-      apply_any(S, c, opt, ema_mode, theta, ema, state0, state1, i);
+      double S = 0.0;  // sum over server j's own kept set
+      for (int32_t n = 0; n < n_j; ++n) S += grad_at(grads[kept_j[n]], grad_dtype, i);
+      apply_element(S, c, opt, ema_mode, theta, ema, state0, state1, i);
+    }
+  }
+  return ORACLE_OK;
+}
+
+// =============================================================================================
+// NEXT-1, companion layout (SURVEY.md section 8b last line, 8f NEXT-1): what parameter server j RECEIVES.
+// Alg. 4 is the program of ONE server j (L134): it waits for "(G, t') from any worker" (l.4, L152) and uses
+// only G[j] (l.8, L160) -- worker k sends server j the slice G_k[j] of its gradient, as server j owns
+// only theta[j] (L42).  So the gradients of one step are W*M separate buffers, one per (worker, server):
+//   grad_slices[k*M + j] -> the len_j = shard_off[j+1] - shard_off[j] elements of G_k[j]
+// (element i of that buffer belongs to parameter shard_off[j] + i), each its own allocation with its own
+// alignment; nothing is assumed about where they lie relative to one another.  Entries of workers that
+// are not kept by server j are never dereferenced (they may be NULL); an empty server (len_j = 0) needs
+// no buffers at all.  Everything else -- kept rows, per-row counts, status, the divisor 1/n_j formed in
+// fp32, the update and the EMA -- is oracle_aggregate_update_rows' (per_shard = 0: row 0 serves every
+// server, n_kept = NULL: exactly N workers, status = NULL: every server is live):
+//   theta(t+1)[j] = theta(t)[j] - (gamma_t / n_j) * sum_{k in kept_j, ascending} G_k[j]            (L160)
+// =============================================================================================
+int oracle_aggregate_update_slices(int64_t P, int32_t M, const int64_t* shard_off, int32_t N, int32_t W,
+                                   const void* const* grad_slices, int grad_dtype, int per_shard,
+                                   const int32_t* kept, int32_t kept_stride, const int32_t* n_kept,
+                                   const int32_t* status, float* theta, float* ema, float* state0, float* state1,
+                                   int opt, int ema_mode, float gamma_t, float alpha, float mu, float rho, float eps) {
+  if (!args_ok(P, M, shard_off, N, opt, ema_mode, theta, ema, state0, state1)) return ORACLE_EINVAL;
+  if (!grad_slices || !kept || W < N || kept_stride < 1) return ORACLE_EINVAL;
+  if (grad_dtype != ORACLE_F32 && grad_dtype != ORACLE_BF16) return ORACLE_EINVAL;
+  for (int32_t j = 0; j < M; ++j) {  // validate every live row before anything is written
+    const int32_t row = per_shard ? j : 0;
+    if (status && status[row] != ORACLE_OK) continue;
+    const int32_t n_j = n_kept ? n_kept[row] : N;
+    if (n_j < 1 || n_j > kept_stride || n_j > W) return ORACLE_EINVAL;
+    const int32_t* kept_j = kept + static_cast<int64_t>(row) * kept_stride;
+    const int64_t len_j = shard_off[j + 1] - shard_off[j];
+    for (int32_t n = 0; n < n_j; ++n) {
+      if (kept_j[n] < 0 || kept_j[n] >= W) return ORACLE_EINVAL;
+      if (len_j > 0 && !grad_slices[static_cast<int64_t>(kept_j[n]) * M + j]) return ORACLE_EINVAL;
+    }
+  }
+  for (int32_t j = 0; j < M; ++j) {  // parameter server j owns theta[j]   (L42)
+    const int32_t row = per_shard ? j : 0;
+    if (status && status[row] != ORACLE_OK) continue;  // this server never collected its gradients
+    const int32_t n_j = n_kept ? n_kept[row] : N;
+    const int32_t* kept_j = kept + static_cast<int64_t>(row) * kept_stride;
+    const Coeffs c = make_coeffs(n_j, gamma_t, alpha, mu, rho, eps);
+    const int64_t lo = shard_off[j], len_j = shard_off[j + 1] - shard_off[j];
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int64_t i = 0; i < len_j; ++i) {  // element i of what server j received = parameter lo + i
+      double S = 0.0;                      // sum_{G in kept set of server j} G[j]              (L160)
+      for (int32_t n = 0; n < n_j; ++n)
+        S += grad_at(grad_slices[static_cast<int64_t>(kept_j[n]) * M + j], grad_dtype, i);
+      apply_element(S, c, opt, ema_mode, theta, ema, state0, state1, lo + i);
     }
   }
   return ORACLE_OK;
@@ -487,7 +458,7 @@ int oracle_async_apply(int64_t P, int32_t M, const int64_t* shard_off, int32_t K
 #pragma omp parallel for schedule(static)
 #endif
       for (int64_t e = lo; e < hi; ++e)
-        apply_any(grad_at(G, grad_dtype, e), c, opt, ema_mode, theta, ema, state0, state1, e);
+        apply_element(grad_at(G, grad_dtype, e), c, opt, ema_mode, theta, ema, state0, state1, e);
     }
   }
   return ORACLE_OK;
@@ -604,13 +575,6 @@ int oracle_interp_iterations(const int32_t* N_pts, const double* iters_pts, int3
     }
   }
   return ORACLE_OK;
-}
-
-// fp32 mirror switch (diagnostic, see above); returns the previous setting.
-int oracle_set_fp32_mirror(int on) {
-  const int prev = g_fp32_mirror;
-  g_fp32_mirror = on ? 1 : 0;
-  return prev;
 }
 
 // Threads the element loops use (1 without OpenMP); bench.py reports it as cpu_baseline.cores.

@@ -1,7 +1,8 @@
-"""Pins for the oracle's fp32 MIRROR (diagnostic mode; readings R9/R10): the same step
-in fp32 with the summation order and the five fused multiply-adds the GPU is documented to use.  Pinned by exact
-rational arithmetic with one RN-even rounding per stated operation, by the hand-worked examples (dyadic, so exact in
-any precision) and by closeness to the double-arithmetic oracle, which stays the graded truth."""
+"""Pins for the fp32 MIRROR (oracle/psync_mirror_f32.cpp -- a separate diagnostic library, not the graded oracle;
+SURVEY.md section 8c; readings R9/R10): the same step in fp32 with the summation order, the five fused
+multiply-adds and the correctly rounded reciprocal square root the GPU is documented to use.  Pinned by exact rational
+arithmetic with one RN-even rounding per stated operation, by the hand-worked examples (dyadic, so exact in any
+precision) and by closeness to the double-arithmetic oracle, which stays the graded truth."""
 import json
 import os
 from fractions import Fraction
@@ -20,10 +21,10 @@ def rn(x):
     return F(_round_f32(x))
 
 
-def sqrt_rn(x: Fraction) -> Fraction:
-    """Correctly rounded fp32 square root of an exact rational (mpmath at 200 digits decides the rounding)."""
+def rsqrt_rn(x: Fraction) -> Fraction:
+    """Correctly rounded fp32 reciprocal square root of an exact rational (mpmath at 200 digits decides the rounding)."""
     with mpmath.workdps(200):
-        r = mpmath.sqrt(mpmath.mpf(x.numerator) / mpmath.mpf(x.denominator))
+        r = 1 / mpmath.sqrt(mpmath.mpf(x.numerator) / mpmath.mpf(x.denominator))
         return F(_round_f32(Fraction(int(mpmath.floor(r * mpmath.mpf(10) ** 150)), 10 ** 150)))
 
 
@@ -47,7 +48,7 @@ def mirror_step_exact(theta, ema, s0, s1, grads, kept, N, opt, ema_mode, gamma, 
             th_new = rn(th - g_ * v)                          # one FMA
         else:
             ms = rn(r_ * F(s0[i]) + rn(omr * rn(G * G)))      # mul, mul, FMA
-            step = rn(rn(g_ * G) / sqrt_rn(rn(ms + e_)))      # mul, add, sqrt, div
+            step = rn(rn(g_ * G) * rsqrt_rn(rn(ms + e_)))     # mul, add, rsqrt, mul
             mom = rn(m_ * F(s1[i]) + step)                    # one FMA
             out[2][i], out[3][i] = f32(float(ms)), f32(float(mom))
             th_new = rn(th - mom)
@@ -56,6 +57,23 @@ def mirror_step_exact(theta, ema, s0, s1, grads, kept, N, opt, ema_mode, gamma, 
             operand = th_new if ema_mode == oracle.EMA_POST else th
             out[1][i] = f32(float(rn(a_ * F(ema[i]) + rn(oma * operand))))    # mul, FMA
     return out
+
+
+def test_mirror_rsqrt_is_correctly_rounded():
+    """mirror_rsqrt_rn against mpmath (200 digits) on random fp32 values over the whole normal range, on values whose
+    reciprocal root sits next to a rounding boundary (x = 1/m^2 rounded, m a midpoint of two floats), and exact cases."""
+    fn = oracle.mirror_lib().mirror_rsqrt_rn
+    rng = np.random.default_rng(77)
+    xs = [f32(v) for v in np.exp(rng.uniform(np.log(1.2e-38), np.log(3e38), 3000))]
+    xs += [f32(v) for v in rng.uniform(0.5, 4.0, 3000)]
+    for _ in range(2000):                                   # near-midpoint cases
+        y = f32(rng.uniform(0.5, 2.0))
+        m = (float(y) + float(np.nextafter(y, f32(4.0)))) / 2
+        x = f32(1.0 / (m * m))
+        xs += [x, np.nextafter(x, f32(0)), np.nextafter(x, f32(9))]
+    for x in xs:
+        assert F(f32(fn(float(x)))) == rsqrt_rn(F(f32(x))), float(x)
+    assert fn(4.0) == 0.5 and fn(0.25) == 2.0 and fn(1.0) == 1.0 and fn(float(2.0 ** -100)) == 2.0 ** 50
 
 
 @pytest.mark.parametrize("opt", [oracle.SGD, oracle.MOMENTUM, oracle.RMSPROP_MOM])
