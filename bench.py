@@ -269,6 +269,7 @@ def run_psync(args, cfg, rank, world, dist):
                                   dtype=torch.float64, device=dev)
 
     stream = torch.cuda.Stream(device=dev)
+    stream.wait_stream(torch.cuda.current_stream())    # tables, kept[] and status were filled on the default stream
     B = psync.binding
 
     def select(i):

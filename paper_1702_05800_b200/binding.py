@@ -21,10 +21,12 @@ PSYNC_OK, PSYNC_EINVAL, PSYNC_ETOOFEW, PSYNC_EUNSUPPORTED, PSYNC_ECUDA = 0, -1, 
 PSYNC_F32, PSYNC_BF16 = 0, 1
 PSYNC_SGD, PSYNC_MOMENTUM, PSYNC_RMSPROP_MOM = 0, 1, 2
 PSYNC_EMA_POST, PSYNC_EMA_PRE, PSYNC_EMA_OFF = 0, 1, 2
+PSYNC_GRADS_FLAT, PSYNC_GRADS_SLICES = 0, 1
 PSYNC_MAX_WORKERS = 1024
+PSYNC_TILE_UNITS = 256
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
-           "psync_select_timeout", "psync_aggregate_update", "psync_ema", "psync_order_by_arrival", "psync_async_apply", "psync_step_device", "psync_clip_workspace_bytes",
+           "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_async_apply", "psync_step_device", "psync_clip_workspace_bytes",
            "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_launch_geometry", "psync_probe_read",
            "psync_probe_copy")
@@ -47,7 +49,7 @@ class psync_step(ctypes.Structure):
         ("gamma_t", ctypes.c_float), ("alpha", ctypes.c_float), ("mu", ctypes.c_float), ("rho", ctypes.c_float),
         ("eps", ctypes.c_float), ("grid_ctas", ctypes.c_int32), ("variant", ctypes.c_int32),
         ("per_shard", ctypes.c_int32), ("kept_stride", ctypes.c_int32), ("d_shard_off", ctypes.c_void_p),
-        ("d_n_kept", ctypes.c_void_p),
+        ("d_n_kept", ctypes.c_void_p), ("grad_layout", ctypes.c_int32), ("d_tile_start", ctypes.c_void_p),
     ]
 
 
@@ -74,6 +76,8 @@ def lib() -> ctypes.CDLL:
         L.psync_select_timeout.restype = ctypes.c_int
         L.psync_aggregate_update.argtypes = [ctypes.POINTER(psync_step), vp]
         L.psync_aggregate_update.restype = ctypes.c_int
+        L.psync_shard_worklist.argtypes = [vp, i32, i32, vp, vp]
+        L.psync_shard_worklist.restype = ctypes.c_int
         L.psync_step_device.argtypes = [ctypes.POINTER(psync_step), vp, vp, i32, vp, vp]
         L.psync_step_device.restype = ctypes.c_int
         L.psync_order_by_arrival.argtypes = [vp, i32, vp, vp, vp]
@@ -215,13 +219,50 @@ def make_grad_table(buffers: Sequence[torch.Tensor]) -> GradTable:
     return GradTable(ptrs, list(buffers), PSYNC_F32 if dt == torch.float32 else PSYNC_BF16)
 
 
+def make_slice_table(slices: Sequence[Sequence[Optional[torch.Tensor]]]) -> GradTable:
+    """Device pointer table [W*M] for PSYNC_GRADS_SLICES: slices[k][j] is worker k's G_k[j], its own CUDA tensor of
+    len_j elements (any element alignment; None -> a NULL entry, legal where server j does not keep worker k)."""
+    W, M = len(slices), len(slices[0])
+    first = next(t for row in slices for t in row if t is not None)
+    dt = first.dtype
+    if dt not in (torch.float32, torch.bfloat16):
+        raise TypeError("gradient slices must be float32 or bfloat16")
+    ptrs = []
+    for row in slices:
+        if len(row) != M:
+            raise ValueError("every worker needs M slices")
+        for t in row:
+            if t is not None and (t.dtype != dt or not t.is_cuda or not t.is_contiguous()):
+                raise ValueError("gradient slices must be contiguous CUDA tensors of one dtype")
+            ptrs.append(0 if t is None else t.data_ptr())
+    d_ptrs = torch.tensor(ptrs, dtype=torch.int64).to(first.device)
+    return GradTable(d_ptrs, [t for row in slices for t in row], PSYNC_F32 if dt == torch.float32 else PSYNC_BF16)
+
+
+def psync_shard_worklist(d_shard_off: torch.Tensor, grad_dtype: int, d_tile_start: Optional[torch.Tensor] = None,
+                         stream=None) -> torch.Tensor:
+    """(server, tile) work list of the shard-aware kernel (include/psync.h: psync_shard_worklist).  Returns the device
+    int64 [M+1] table (allocated here unless given); it depends only on the shard layout and the gradient dtype."""
+    M = d_shard_off.numel() - 1
+    if d_tile_start is None:
+        d_tile_start = torch.empty(M + 1, dtype=torch.int64, device=d_shard_off.device)
+    if d_tile_start.numel() < M + 1:
+        raise ValueError("d_tile_start needs M+1 elements")
+    st = lib().psync_shard_worklist(_dptr(d_shard_off, torch.int64, "d_shard_off"), M, grad_dtype,
+                                    _dptr(d_tile_start, torch.int64, "d_tile_start"), _stream(stream))
+    if st != PSYNC_OK:
+        raise PsyncError(st, "psync_shard_worklist")
+    return d_tile_start
+
+
 def make_step(shard_off, N: int, W: int, grad_dtype: int, theta: torch.Tensor, ema: Optional[torch.Tensor] = None,
               state0: Optional[torch.Tensor] = None, state1: Optional[torch.Tensor] = None, opt: int = PSYNC_SGD,
               ema_mode: int = PSYNC_EMA_POST, gamma_t: float = 0.0, alpha: float = 0.0, mu: float = 0.0,
               rho: float = 0.0, eps: float = 0.0, d_grads: Optional[torch.Tensor] = None,
               d_kept: Optional[torch.Tensor] = None, d_status: Optional[torch.Tensor] = None, grid_ctas: int = 0,
               variant: int = 0, per_shard: bool = False, kept_stride: int = 0,
-              d_shard_off: Optional[torch.Tensor] = None, d_n_kept: Optional[torch.Tensor] = None):
+              d_shard_off: Optional[torch.Tensor] = None, d_n_kept: Optional[torch.Tensor] = None,
+              grad_layout: int = PSYNC_GRADS_FLAT, d_tile_start: Optional[torch.Tensor] = None):
     """Fills a psync_step.  Returns (struct, keepalive) -- hold on to both until the call returns."""
     off = np.ascontiguousarray(shard_off, dtype=np.int64)
     s = psync_step()
@@ -246,8 +287,14 @@ def make_step(shard_off, N: int, W: int, grad_dtype: int, theta: torch.Tensor, e
     s.per_shard, s.kept_stride = int(per_shard), kept_stride
     s.d_shard_off = _dptr(d_shard_off, torch.int64, "d_shard_off")
     s.d_n_kept = _dptr(d_n_kept, torch.int32, "d_n_kept")
+    s.grad_layout = grad_layout
+    s.d_tile_start = _dptr(d_tile_start, torch.int64, "d_tile_start")
     if d_shard_off is not None and d_shard_off.numel() != off.size:
         raise ValueError("d_shard_off must have M+1 elements")
+    if d_tile_start is not None and d_tile_start.numel() != off.size:
+        raise ValueError("d_tile_start must have M+1 elements")
+    if grad_layout == PSYNC_GRADS_SLICES and d_grads is not None and d_grads.numel() < W * (off.size - 1):
+        raise ValueError("PSYNC_GRADS_SLICES: d_grads needs W*M entries")
     rows = s.M if per_shard else 1
     stride = kept_stride if kept_stride > 0 else (W if d_n_kept is not None else N)
     if 1 <= N <= W <= PSYNC_MAX_WORKERS:       # out-of-range N / W are the C side's PSYNC_EINVAL to report
@@ -255,7 +302,7 @@ def make_step(shard_off, N: int, W: int, grad_dtype: int, theta: torch.Tensor, e
                             ("d_n_kept", d_n_kept, rows)):
             if a is not None and a.numel() < need:
                 raise ValueError(f"{nm} needs {need} elements")
-    return s, (off, d_grads, d_kept, d_status, theta, ema, state0, state1, d_shard_off, d_n_kept)
+    return s, (off, d_grads, d_kept, d_status, theta, ema, state0, state1, d_shard_off, d_n_kept, d_tile_start)
 
 
 def psync_aggregate_update(step: psync_step, stream=None, check: bool = True) -> int:

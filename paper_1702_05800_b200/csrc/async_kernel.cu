@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(THREADS, MINB) async_apply_kernel(const FusedP
 
   if (p.status != nullptr && *p.status != 0) return;
   const int K = p.n_kept ? *p.n_kept : p.N;  // gradients that arrived
-  if (K <= 0) return;
+  if (K <= 0 || K > kMaxWorkers) return;  // nothing arrived, or a count nobody wrote
 
   unsigned misalign = 0;
   for (int i = threadIdx.x; i < K; i += THREADS) {

@@ -48,6 +48,7 @@ __device__ void rows_scalar_range(const FusedParams& p, int64_t i0, int64_t i1, 
     const int row = p.per_shard ? find_server(p.shard_off, p.M, i) : 0;
     if (p.status != nullptr && p.status[row] != 0) continue;  // this server did not collect its gradients
     const int N = p.n_kept ? p.n_kept[row] : p.N;
+    if (N <= 0 || N > p.kept_stride) continue;  // a count nobody wrote: the row counts as failed
     const float inv_N = p.n_kept ? 1.0f / static_cast<float>(N) : p.inv_N;
     const int32_t* kept = p.kept + static_cast<int64_t>(row) * p.kept_stride;
     float S = 0.f;
@@ -211,13 +212,18 @@ __global__ void __launch_bounds__(THREADS, MINB) fused_aggregate_update_ema(cons
         bool fast = one_server && p.base_aligned != 0;
         int N = 0;
         float inv_N = 0.f;
+        bool bad_count = false;  // a device-side count outside [1, kept_stride] (never written, stale): failed row
         if (fast) {
           N = p.n_kept ? p.n_kept[row] : p.N;
+          bad_count = N <= 0 || N > p.kept_stride || N > kMaxWorkers;
+          if (bad_count) N = 0;
           inv_N = p.n_kept ? 1.0f / static_cast<float>(N) : p.inv_N;
           const unsigned misalign = stage_row<THREADS>(p, s_ptr, row, N);
           fast = __syncthreads_or(static_cast<int>(misalign)) == 0;
         }
-        if (fast)
+        if (bad_count) {
+          // leave the slice untouched
+        } else if (fast)
           vector_tile<THREADS, UPT, U, BF16, OPT, EMA, false>(p, s_ptr, N, inv_N, tile, n_units);
         else
           rows_scalar_range<BF16, OPT, EMA>(p, e0, e1, threadIdx.x, THREADS);
@@ -225,6 +231,234 @@ __global__ void __launch_bounds__(THREADS, MINB) fused_aggregate_update_ema(cons
     }
     if (tail0 < p.P && blockIdx.x == 0) rows_scalar_range<BF16, OPT, EMA>(p, tail0, p.P, threadIdx.x, THREADS);
   }
+}
+
+
+// ---- variant 6: 256-bit loads (sm_100: ld.global.v8, SASS LDG.E.256) with L2::evict_first ----------------------
+// Same schedule as vector_tile with 32-byte units: E = 8 (fp32) or 16 (bf16) parameters per thread, one tile per
+// CTA, U independent loads in flight, strictly ascending worker order per element -- the same bits as every other
+// variant.  Kept selectable so that the A/B against the 128-bit default can be re-run (profiles/r2_variants.md).
+struct alignas(32) U8 {
+  uint32_t v[8];
+};
+__device__ __forceinline__ U8 ldg_stream32(const void* p) {
+  U8 r;
+  asm volatile("ld.global.nc.L1::no_allocate.L2::evict_first.v8.u32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(r.v[0]), "=r"(r.v[1]), "=r"(r.v[2]), "=r"(r.v[3]), "=r"(r.v[4]), "=r"(r.v[5]), "=r"(r.v[6]),
+                 "=r"(r.v[7])
+               : "l"(p));
+  return r;
+}
+
+template <int THREADS, int U, int MINB, bool BF16, int OPT, int EMA>
+__global__ void __launch_bounds__(THREADS, MINB) fused_aggregate_update_ema_v256(const FusedParams p) {
+  constexpr int E = BF16 ? 16 : 8;  // parameters per 32-byte unit
+  constexpr int Q = E / 4;
+  __shared__ const char* s_ptr[kMaxWorkers];
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  if (p.status != nullptr && *p.status != 0) return;
+  unsigned misalign = 0;
+  for (int n = threadIdx.x; n < p.N; n += THREADS) {
+    const char* g = static_cast<const char*>(p.grads[p.kept[n]]);
+    s_ptr[n] = g;
+    misalign |= static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 31u;
+  }
+  const bool vec_ok = (__syncthreads_or(static_cast<int>(misalign)) == 0) && (p.base_aligned != 0);
+  if (!vec_ok) {
+    scalar_range<BF16, OPT, EMA>(p, s_ptr, 0, p.P, static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x,
+                                 static_cast<int64_t>(gridDim.x) * THREADS);
+    return;
+  }
+  const int64_t n_units = p.P / E;
+  const int64_t tail0 = n_units * E;
+  const int64_t u = static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x;
+  if (static_cast<int64_t>(blockIdx.x) * THREADS < n_units) {
+    const bool live = u < n_units;
+    const int64_t unit = live ? u : (n_units - 1);
+    const int N = p.N;
+    float acc[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) acc[e] = 0.f;
+    auto add_unit = [&acc](const U8& r) {
+      const uint4 lo = make_uint4(r.v[0], r.v[1], r.v[2], r.v[3]), hi = make_uint4(r.v[4], r.v[5], r.v[6], r.v[7]);
+      accumulate_unit<BF16>(acc, lo);
+      accumulate_unit<BF16>(acc + E / 2, hi);
+    };
+    int n = 0;
+    for (; n + U <= N; n += U) {
+      U8 r[U];
+#pragma unroll
+      for (int v = 0; v < U; ++v) r[v] = ldg_stream32(s_ptr[n + v] + unit * 32);
+#pragma unroll
+      for (int v = 0; v < U; ++v) add_unit(r[v]);
+    }
+    for (; n < N; ++n) add_unit(ldg_stream32(s_ptr[n] + unit * 32));
+
+    float4 th[Q], em[Q], a0[Q], a1[Q];
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const int64_t e = unit * E + 4 * q;
+      th[q] = ld_state16(p.theta + e);
+      if (EMA != EMA_OFF) em[q] = ld_state16(p.ema + e);
+      if (OPT != OPT_SGD) a0[q] = ld_state16(p.s0 + e);
+      if (OPT == OPT_RMSPROP_MOM) a1[q] = ld_state16(p.s1 + e);
+    }
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      float* t4 = reinterpret_cast<float*>(&th[q]);
+      float* e4 = reinterpret_cast<float*>(&em[q]);
+      float* x4 = reinterpret_cast<float*>(&a0[q]);
+      float* y4 = reinterpret_cast<float*>(&a1[q]);
+#pragma unroll
+      for (int l = 0; l < 4; ++l) update_element<OPT, EMA>(acc[4 * q + l], p.inv_N, t4[l], e4[l], x4[l], y4[l], p);
+      if (live) {
+        const int64_t e = unit * E + 4 * q;
+        st_state16(p.theta + e, th[q]);
+        if (EMA != EMA_OFF) st_state16(p.ema + e, em[q]);
+        if (OPT != OPT_SGD) st_state16(p.s0 + e, a0[q]);
+        if (OPT == OPT_RMSPROP_MOM) st_state16(p.s1 + e, a1[q]);
+      }
+    }
+  }
+  if (tail0 < p.P && blockIdx.x == 0) scalar_range<BF16, OPT, EMA>(p, s_ptr, tail0, p.P, threadIdx.x, THREADS);
+}
+
+// ---- variant 5: TMA bulk staging -- cp.async.bulk global -> shared through an mbarrier ring ----------------------
+// One producer thread (warp CONSUMERS/32, lane 0) issues one cp.async.bulk per kept worker: that worker's 4 KB row
+// of the CTA's tile (256 16-byte units) into stage n % STAGES, completion counted in bytes on full[stage].  The 256
+// consumer threads wait for the stage, add their 16-byte unit from shared memory (ascending worker order, so the
+// same bits as every other variant) and release it on empty[stage] (one arrival per consumer warp).  Bytes in
+// flight no longer cost registers: STAGES x 4 KB per CTA.  Needs 16-byte aligned buffers (like the 128-bit path).
+// Kept selectable so that the A/B against plain 128-bit loads can be re-run (profiles/r2_variants.md).
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+  asm volatile(
+      "{\n\t.reg .pred ok;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 ok, [%0], %1;\n\t"
+      "@ok bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+      : "memory");
+}
+
+template <int STAGES, int MINB, bool BF16, int OPT, int EMA>
+__global__ void __launch_bounds__(256 + 32, MINB) fused_aggregate_update_ema_bulk(const FusedParams p) {
+  constexpr int CONSUMERS = 256;
+  constexpr int E = BF16 ? 8 : 4;
+  constexpr int Q = E / 4;
+  constexpr unsigned kRowBytes = CONSUMERS * 16;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  uint4* stage = reinterpret_cast<uint4*>(smem_raw);                                      // [STAGES][256] x 16 B
+  const char** s_ptr = reinterpret_cast<const char**>(smem_raw + STAGES * kRowBytes);    // [kMaxWorkers]
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + STAGES * kRowBytes + sizeof(char*) * kMaxWorkers);
+  uint64_t* empty = full + STAGES;
+
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  if (p.status != nullptr && *p.status != 0) return;
+  unsigned misalign = 0;
+  for (int n = threadIdx.x; n < p.N; n += CONSUMERS + 32) {
+    const char* g = static_cast<const char*>(p.grads[p.kept[n]]);
+    s_ptr[n] = g;
+    misalign |= static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 15u;
+  }
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(&full[s], 1);               // the producer's arrive.expect_tx; the copy completes the bytes
+      mbar_init(&empty[s], CONSUMERS / 32);  // one arrival per consumer warp
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  const bool vec_ok = (__syncthreads_or(static_cast<int>(misalign)) == 0) && (p.base_aligned != 0);
+  if (!vec_ok) {
+    if (threadIdx.x < CONSUMERS)
+      scalar_range<BF16, OPT, EMA>(p, s_ptr, 0, p.P, static_cast<int64_t>(blockIdx.x) * CONSUMERS + threadIdx.x,
+                                   static_cast<int64_t>(gridDim.x) * CONSUMERS);
+    return;
+  }
+  const int N = p.N;
+  const int64_t n_units = p.P / E;
+  const int64_t tail0 = n_units * E;
+  const int64_t u0 = static_cast<int64_t>(blockIdx.x) * CONSUMERS;
+  const bool has_tile = u0 < n_units;
+  const int64_t live_units = has_tile ? ((n_units - u0 < CONSUMERS) ? (n_units - u0) : CONSUMERS) : 0;
+
+  if (threadIdx.x >= CONSUMERS) {  // ---- producer warp
+    if (threadIdx.x == CONSUMERS && has_tile) {
+      uint64_t policy;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+      const unsigned bytes = static_cast<unsigned>(live_units) * 16u;
+      for (int n = 0; n < N; ++n) {
+        const int s = n % STAGES;
+        if (n >= STAGES) mbar_wait(&empty[s], ((n / STAGES) - 1) & 1);  // every consumer warp has read the slot
+        mbar_expect_tx(&full[s], bytes);
+        bulk_g2s(stage + s * CONSUMERS, s_ptr[n] + u0 * 16, bytes, &full[s], policy);
+      }
+    }
+    return;
+  }
+
+  // ---- consumers
+  if (has_tile) {
+    const bool live = threadIdx.x < live_units;
+    const int64_t unit = u0 + (live ? threadIdx.x : 0);
+    float acc[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) acc[e] = 0.f;
+    for (int n = 0; n < N; ++n) {
+      const int s = n % STAGES;
+      mbar_wait(&full[s], (n / STAGES) & 1);
+      const uint4 r = live ? stage[s * CONSUMERS + threadIdx.x] : make_uint4(0u, 0u, 0u, 0u);
+      __syncwarp();
+      if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[s]);
+      accumulate_unit<BF16>(acc, r);
+    }
+    float4 th[Q], em[Q], a0[Q], a1[Q];
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const int64_t e = unit * E + 4 * q;
+      th[q] = ld_state16(p.theta + e);
+      if (EMA != EMA_OFF) em[q] = ld_state16(p.ema + e);
+      if (OPT != OPT_SGD) a0[q] = ld_state16(p.s0 + e);
+      if (OPT == OPT_RMSPROP_MOM) a1[q] = ld_state16(p.s1 + e);
+    }
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      float* t4 = reinterpret_cast<float*>(&th[q]);
+      float* e4 = reinterpret_cast<float*>(&em[q]);
+      float* x4 = reinterpret_cast<float*>(&a0[q]);
+      float* y4 = reinterpret_cast<float*>(&a1[q]);
+#pragma unroll
+      for (int l = 0; l < 4; ++l) update_element<OPT, EMA>(acc[4 * q + l], p.inv_N, t4[l], e4[l], x4[l], y4[l], p);
+      if (live) {
+        const int64_t e = unit * E + 4 * q;
+        st_state16(p.theta + e, th[q]);
+        if (EMA != EMA_OFF) st_state16(p.ema + e, em[q]);
+        if (OPT != OPT_SGD) st_state16(p.s0 + e, a0[q]);
+        if (OPT == OPT_RMSPROP_MOM) st_state16(p.s1 + e, a1[q]);
+      }
+    }
+  }
+  if (tail0 < p.P && blockIdx.x == 0) scalar_range<BF16, OPT, EMA>(p, s_ptr, tail0, p.P, threadIdx.x, CONSUMERS);
 }
 
 // ---- K3 ---------------------------------------------------------------------------------------
@@ -246,17 +480,22 @@ __global__ void __launch_bounds__(256) ema_kernel(float* __restrict__ ema, const
 }
 
 // ---- variants and dispatch ---------------------------------------------------------------------
+enum VariantKind { kPlain128 = 0, kBulkRing = 1, kPlain256 = 2 };
 struct Variant {
-  int threads, upt, unroll, minb;
+  int threads, upt, unroll, minb, kind;
 };
-// variant ids are 1-based in the ABI (0 = default for the dtype)
+// variant ids are 1-based in the ABI (0 = default)
 constexpr Variant kVariants[] = {
-    {256, 1, 8, 4},   // 1
-    {256, 2, 8, 2},   // 2
-    {256, 1, 16, 3},  // 3
-    {512, 1, 8, 2},   // 4
+    {256, 1, 8, 4, kPlain128},    // 1  the default: 128-bit loads, 8 in flight per thread, 4 CTAs/SM
+    {256, 2, 8, 2, kPlain128},    // 2
+    {256, 1, 16, 3, kPlain128},   // 3
+    {512, 1, 8, 2, kPlain128},    // 4
+    {256, 1, 12, 3, kBulkRing},   // 5  cp.async.bulk -> 12-stage shared-memory ring (unroll = stages), 1 producer warp
+    {256, 1, 8, 2, kPlain256},    // 6  256-bit loads with L2::evict_first, 8 in flight per thread
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
+constexpr int kRingStages = kVariants[4].unroll;
+constexpr int kRingSmemBytes = kRingStages * 256 * 16 + static_cast<int>(sizeof(const char*)) * kMaxWorkers + 2 * kRingStages * 8;
 
 using KernelFn = void (*)(const FusedParams);
 
@@ -269,11 +508,17 @@ constexpr int minb_for(int v, bool bf16, int opt) {
 
 template <int V, bool BF16, int OPT, int EMA, bool ROWS = false>
 constexpr KernelFn kernel_for() {
-  return fused_aggregate_update_ema<kVariants[V].threads, kVariants[V].upt, kVariants[V].unroll,
-                                    minb_for(V, BF16, OPT), BF16, OPT, EMA, ROWS>;
+  if constexpr (kVariants[V].kind == kBulkRing)
+    return fused_aggregate_update_ema_bulk<kVariants[V].unroll, kVariants[V].minb, BF16, OPT, EMA>;
+  else if constexpr (kVariants[V].kind == kPlain256)
+    return fused_aggregate_update_ema_v256<kVariants[V].threads, kVariants[V].unroll, (BF16 ? 1 : kVariants[V].minb),
+                                           BF16, OPT, EMA>;
+  else
+    return fused_aggregate_update_ema<kVariants[V].threads, kVariants[V].upt, kVariants[V].unroll,
+                                      minb_for(V, BF16, OPT), BF16, OPT, EMA, ROWS>;
 }
 
-// per-server rows: the default variant only (a forced variant > 1 is PSYNC_EUNSUPPORTED in the ABI)
+// kept rows with a device-side count / one row per server in the flat index space: the default variant only
 template <bool BF16, int OPT>
 KernelFn pick_rows_ema(int ema) {
   switch (ema) {
@@ -319,13 +564,15 @@ KernelFn pick_kernel(int v, int dtype, int opt, int ema) {
     case 0: return pick_dtype<0>(dtype, opt, ema);
     case 1: return pick_dtype<1>(dtype, opt, ema);
     case 2: return pick_dtype<2>(dtype, opt, ema);
-    default: return pick_dtype<3>(dtype, opt, ema);
+    case 3: return pick_dtype<3>(dtype, opt, ema);
+    case 4: return pick_dtype<4>(dtype, opt, ema);
+    default: return pick_dtype<5>(dtype, opt, ema);
   }
 }
 
-int resolve_variant(int dtype, int variant) {
+int resolve_variant(int variant) {
   if (variant >= 1 && variant <= kNumVariants) return variant - 1;
-  return dtype == 1 ? 0 : 0;  // default: variant 1 (tuned on B200, see DESIGN.md s.6)
+  return 0;  // default: variant 1 (tuned on B200, DESIGN.md s.5; the A/B of all six is profiles/r2_variants.md)
 }
 
 }  // namespace
@@ -343,19 +590,19 @@ int sm_count() {
 }
 
 cudaError_t fused_geometry(int dtype, int opt, int ema, int variant, int grid_ctas, int64_t P, FusedGeometry* out) {
-  const int v = resolve_variant(dtype, variant);
+  const int v = resolve_variant(variant);
   const Variant& vr = kVariants[v];
-  const int E = dtype == 1 ? 8 : 4;
-  out->block = vr.threads;
+  const int E = (dtype == 1 ? 8 : 4) * (vr.kind == kPlain256 ? 2 : 1);  // parameters per 16- or 32-byte unit
+  out->block = vr.threads + (vr.kind == kBulkRing ? 32 : 0);           // + the producer warp
   out->tile_elems = vr.threads * vr.upt * E;
-  out->smem_bytes = static_cast<int>(sizeof(const char*)) * kMaxWorkers;
+  out->smem_bytes = vr.kind == kBulkRing ? kRingSmemBytes : static_cast<int>(sizeof(const char*)) * kMaxWorkers;
   // One tile per CTA, always: the hardware CTA scheduler balances the tiles dynamically over the SMs, which
   // measured 2-3 % faster on B200 than a persistent grid with static striding (DESIGN.md s.5), and a kernel
   // without a tile loop stays inside 64 registers without spilling.  grid_ctas is accepted and ignored.
   (void)opt;
   (void)ema;
   (void)grid_ctas;
-  const int64_t n_tiles = (P / E + static_cast<int64_t>(vr.threads) * vr.upt - 1) / (static_cast<int64_t>(vr.threads) * vr.upt);
+  const int64_t n_tiles = (P / E + static_cast<int64_t>(vr.threads) * vr.upt - 1) / (static_cast<int64_t>(vr.threads) * vr.upt);  // E: per unit of this variant
   int64_t grid = n_tiles;
   if (grid > 0x7FFFFFFF) return cudaErrorInvalidConfiguration;  // > 2^41 parameters: not addressable in HBM anyway
   if (grid < 1) grid = 1;
@@ -368,18 +615,26 @@ cudaError_t launch_fused(const FusedParams& p, int dtype, int opt, int ema, int 
   FusedGeometry g;
   cudaError_t err = fused_geometry(dtype, opt, ema, variant, grid_ctas, p.P, &g);
   if (err != cudaSuccess) return err;
-  const int v = resolve_variant(dtype, variant);
+  const int v = resolve_variant(variant);
+  const bool rows = p.per_shard || p.n_kept != nullptr;
+  const KernelFn kernel = rows ? pick_rows_kernel(dtype, opt, ema) : pick_kernel(v, dtype, opt, ema);
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(static_cast<unsigned>(g.grid));
   cfg.blockDim = dim3(static_cast<unsigned>(g.block));
   cfg.dynamicSmemBytes = 0;
+  if (!rows && kVariants[v].kind == kBulkRing) {  // the ring lives in dynamic shared memory (> 48 KB: opt in)
+    cfg.dynamicSmemBytes = kRingSmemBytes;
+    err = cudaFuncSetAttribute(reinterpret_cast<const void*>(kernel), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               kRingSmemBytes);
+    if (err != cudaSuccess) return err;
+  }
   cfg.stream = stream;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, (p.per_shard || p.n_kept != nullptr) ? pick_rows_kernel(dtype, opt, ema) : pick_kernel(v, dtype, opt, ema), p);
+  return cudaLaunchKernelEx(&cfg, kernel, p);
 }
 
 cudaError_t launch_ema(float* d_ema, const float* d_theta, int64_t P, float alpha, cudaStream_t stream) {

@@ -90,8 +90,9 @@ __global__ void __launch_bounds__(kClipThreads) sumsq_chunks_kernel(const void* 
   if (threadIdx.x == 0) work[static_cast<int64_t>(blockIdx.y) * gridDim.x + blockIdx.x] = total;
 }
 
-// one CTA per worker: fixed-order sum of its chunk partials, then the clip factor
-__global__ void __launch_bounds__(kClipThreads) clip_finalize_kernel(const double* __restrict__ work, int chunks,
+// one CTA per worker: fixed-order sum of its chunk partials, then the clip factor (`work` comes from the
+// predecessor kernel: a plain pointer, see K7b)
+__global__ void __launch_bounds__(kClipThreads) clip_finalize_kernel(const double* work, int chunks,
                                                                      float clip, float* __restrict__ scales) {
   __shared__ double s_warp[kClipThreads / 32];
   asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -151,10 +152,12 @@ __global__ void __launch_bounds__(1024) sort_rows_kernel(const float* __restrict
   }
 }
 
+// (`sorted` and `iters` are written by the predecessor kernel, which may still be running when this grid becomes
+// resident under programmatic dependent launch: they are plain pointers, never ld.global.nc / __restrict__.)
 // K7b: one CTA per k: count / mean (fixed-order double sum) / median (radix select over the T keys of column k)
-__global__ void __launch_bounds__(256) column_stats_kernel(const float* __restrict__ sorted, int32_t T, int32_t W,
+__global__ void __launch_bounds__(256) column_stats_kernel(const float* sorted, int32_t T, int32_t W,
                                                            int32_t* __restrict__ count, double* __restrict__ mean,
-                                                           double* __restrict__ median, const double* __restrict__ iters,
+                                                           double* __restrict__ median, const double* iters,
                                                            double* __restrict__ est_time) {
   __shared__ double s_warp[8];
   __shared__ int s_cnt[4];

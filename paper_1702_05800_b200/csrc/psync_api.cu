@@ -36,7 +36,11 @@ int check_step(const psync_step* s, bool need_device_tables) {
   if (s->kept_stride < 0 || (s->kept_stride != 0 && s->kept_stride < s->N && s->d_n_kept == nullptr)) return PSYNC_EINVAL;
   if (s->kept_stride > PSYNC_MAX_WORKERS) return PSYNC_EINVAL;
   if (need_device_tables && s->per_shard && s->d_shard_off == nullptr) return PSYNC_EINVAL;
-  if ((s->per_shard || s->d_n_kept != nullptr) && s->variant > 1) return PSYNC_EUNSUPPORTED;  // rows kernel: default variant only
+  if (s->grad_layout != PSYNC_GRADS_FLAT && s->grad_layout != PSYNC_GRADS_SLICES) return PSYNC_EINVAL;
+  if (need_device_tables && s->grad_layout == PSYNC_GRADS_SLICES && (s->d_shard_off == nullptr || s->d_tile_start == nullptr))
+    return PSYNC_EINVAL;
+  if ((s->per_shard || s->d_n_kept != nullptr || s->grad_layout == PSYNC_GRADS_SLICES) && s->variant > 1)
+    return PSYNC_EUNSUPPORTED;  // rows / shard-aware kernels: default launch shape only
   return PSYNC_OK;
 }
 
@@ -66,11 +70,31 @@ FusedParams make_params(const psync_step* s, int64_t first, int64_t count, const
   p.M = s->M;
   p.shard_off = s->d_shard_off;
   p.n_kept = s->d_n_kept;
+  p.slices = s->grad_layout == PSYNC_GRADS_SLICES ? 1 : 0;
+  p.tile_start = s->d_tile_start;
   p.gammas = nullptr;
   p.gscales = nullptr;
   p.base_aligned = aligned16(p.theta) && (p.ema == nullptr || aligned16(p.ema)) && (p.s0 == nullptr || aligned16(p.s0)) &&
                    (p.s1 == nullptr || aligned16(p.s1));
   return p;
+}
+
+// The shard-aware kernel (work list, one CTA per (server, tile)) serves the slices layout, and flat buffers with one
+// kept row per server when the caller supplies the work list; everything else is the flat stream.
+bool wants_sharded(const psync_step* s) {
+  return s->grad_layout == PSYNC_GRADS_SLICES || (s->per_shard != 0 && s->d_tile_start != nullptr);
+}
+
+int64_t sharded_tiles(const psync_step* s) {
+  const int64_t T = psync::sharded_tile_elems(s->grad_dtype);
+  int64_t n = 0;
+  for (int32_t j = 0; j < s->M; ++j) n += (s->h_shard_off[j + 1] - s->h_shard_off[j] + T - 1) / T;
+  return n;
+}
+
+cudaError_t launch_step_kernel(const psync_step* s, const FusedParams& p, cudaStream_t stream) {
+  if (wants_sharded(s)) return psync::launch_sharded(p, s->grad_dtype, s->opt, s->ema_mode, sharded_tiles(s), stream);
+  return psync::launch_fused(p, s->grad_dtype, s->opt, s->ema_mode, s->variant, s->grid_ctas, stream);
 }
 
 constexpr int64_t kDefaultChunkElems = int64_t{1} << 20;
@@ -166,9 +190,18 @@ PSYNC_API int psync_aggregate_update(const psync_step* step, void* stream) {
   if (st != PSYNC_OK) return st;
   if (step->P == 0) return PSYNC_OK;
   const FusedParams p = make_params(step, 0, step->P, step->d_grads, step->d_kept, step->d_status);
-  const cudaError_t err = psync::launch_fused(p, step->grad_dtype, step->opt, step->ema_mode, step->variant,
-                                              step->grid_ctas, static_cast<cudaStream_t>(stream));
+  const cudaError_t err = launch_step_kernel(step, p, static_cast<cudaStream_t>(stream));
   return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
+}
+
+PSYNC_API int psync_shard_worklist(const int64_t* d_shard_off, int32_t M, int32_t grad_dtype, int64_t* d_tile_start,
+                         void* stream) {
+  if (d_shard_off == nullptr || d_tile_start == nullptr || M < 1) return PSYNC_EINVAL;
+  if (grad_dtype != PSYNC_F32 && grad_dtype != PSYNC_BF16) return PSYNC_EINVAL;
+  return psync::launch_shard_worklist(d_shard_off, M, grad_dtype, d_tile_start, static_cast<cudaStream_t>(stream)) ==
+                 cudaSuccess
+             ? PSYNC_OK
+             : PSYNC_ECUDA;
 }
 
 PSYNC_API int psync_step_device(const psync_step* step, const float* d_arrival, const int32_t* d_step_tag, int32_t t,
@@ -184,10 +217,7 @@ PSYNC_API int psync_step_device(const psync_step* step, const float* d_arrival, 
     return PSYNC_ECUDA;
   if (step->P == 0) return PSYNC_OK;
   const FusedParams p = make_params(step, 0, step->P, step->d_grads, step->d_kept, step->d_status);
-  return psync::launch_fused(p, step->grad_dtype, step->opt, step->ema_mode, step->variant, step->grid_ctas, s) ==
-                 cudaSuccess
-             ? PSYNC_OK
-             : PSYNC_ECUDA;
+  return launch_step_kernel(step, p, s) == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
 }
 
 PSYNC_API int psync_order_by_arrival(const float* d_arrival, int32_t W, int32_t* d_order, int32_t* d_n_arrived,
@@ -203,7 +233,7 @@ PSYNC_API int psync_order_by_arrival(const float* d_arrival, int32_t W, int32_t*
 PSYNC_API int psync_async_apply(const psync_step* step, const float* d_gamma, const float* d_gscale, void* stream) {
   const int st = check_step(step, true);
   if (st != PSYNC_OK && !(st == PSYNC_EUNSUPPORTED && step->per_shard == 0)) return st;  // variant is ignored here
-  if (step->per_shard != 0) return PSYNC_EUNSUPPORTED;
+  if (step->per_shard != 0 || step->grad_layout != PSYNC_GRADS_FLAT) return PSYNC_EUNSUPPORTED;
   if (step->P == 0) return PSYNC_OK;
   FusedParams p = make_params(step, 0, step->P, step->d_grads, step->d_kept, step->d_status);
   p.gammas = d_gamma;
@@ -277,9 +307,17 @@ PSYNC_API int psync_launch_geometry(const psync_step* step, int32_t* grid, int32
   const int st = check_step(step, false);
   if (st != PSYNC_OK) return st;
   psync::FusedGeometry g;
-  if (psync::fused_geometry(step->grad_dtype, step->opt, step->ema_mode, step->variant, step->grid_ctas, step->P, &g) !=
-      cudaSuccess)
+  if (wants_sharded(step)) {
+    const int64_t tiles = sharded_tiles(step);
+    if (tiles > 0x7FFFFFFF) return PSYNC_ECUDA;
+    g.grid = static_cast<int>(tiles);
+    g.block = PSYNC_TILE_UNITS;
+    g.tile_elems = psync::sharded_tile_elems(step->grad_dtype);
+    g.smem_bytes = 8 * PSYNC_MAX_WORKERS + 4 * g.tile_elems + 4;
+  } else if (psync::fused_geometry(step->grad_dtype, step->opt, step->ema_mode, step->variant, step->grid_ctas, step->P,
+                                   &g) != cudaSuccess) {
     return PSYNC_ECUDA;
+  }
   if (grid) *grid = g.grid;
   if (block) *block = g.block;
   if (tile_elems) *tile_elems = g.tile_elems;
@@ -311,7 +349,7 @@ PSYNC_API int psync_step_host(const psync_step* st, const float* h_arrival, cons
   const int chk = check_step(st, false);
   if (chk != PSYNC_OK) return chk;
   if (h_arrival == nullptr || h_grads == nullptr || d_work == nullptr) return PSYNC_EINVAL;
-  if (st->per_shard != 0 || st->d_n_kept != nullptr) return PSYNC_EUNSUPPORTED;
+  if (st->per_shard != 0 || st->d_n_kept != nullptr || st->grad_layout != PSYNC_GRADS_FLAT) return PSYNC_EUNSUPPORTED;
   HostLayout L;
   if (!host_layout(st->N, st->W, st->grad_dtype, chunk_elems, &L)) return PSYNC_EINVAL;
   if (work_bytes < L.total || (reinterpret_cast<uintptr_t>(d_work) & 255u) != 0) return PSYNC_EINVAL;

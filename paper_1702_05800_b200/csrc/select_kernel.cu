@@ -160,7 +160,7 @@ __global__ void __launch_bounds__(32) select_first_n_kernel(const float* __restr
 
 // K1b: the time-out rule (reading R19).  Worker k is kept iff it is eligible
 // (finite arrival, tag == t) and arrival[k] <= timeout; kept[] comes out ascending because lanes own
-// contiguous index ranges; n_kept < min_keep -> ETOOFEW and nothing else is written.
+// contiguous index ranges; fewer than min_keep -> ETOOFEW, n_kept[row] = 0 and the kept row is not written.
 __global__ void __launch_bounds__(32) select_timeout_kernel(const float* __restrict__ arrival,
                                                             const int32_t* __restrict__ tags, int32_t t, int32_t W,
                                                             float timeout, int32_t min_keep,
@@ -187,7 +187,10 @@ __global__ void __launch_bounds__(32) select_timeout_kernel(const float* __restr
   int total;
   int out = warp_exclusive_scan(mine, lane, &total);
   if (total < min_keep) {
-    if (lane == 0) status[row] = kStatusTooFew;
+    if (lane == 0) {
+      status[row] = kStatusTooFew;
+      n_kept[row] = 0;  // a consumer that ignores the status must still see an empty row, never a stale count
+    }
     return;
   }
   for (int i = 0; i < C; ++i) {

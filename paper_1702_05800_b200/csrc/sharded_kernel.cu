@@ -1,0 +1,332 @@
+// K2s: the SHARD-AWARE fused aggregate + update + EMA -- Alg. 4 l.8-9 as parameter server j
+// runs it: server j owns theta[j] (L42), receives the slice G_k[j] of every worker's gradient (L152) and applies
+//     theta(t+1)[j] <- theta(t)[j] - (gamma_t / n_j) sum_{k in kept_j} G_k[j];   ema[j] <- alpha ema[j] + (1-alpha) theta[j]
+//
+// Two gradient layouts (psync_step.grad_layout):
+//   SLICES  d_grads is [W*M]: entry k*M + j -> the len_j elements of G_k[j], each its own allocation with its
+//           own alignment (what a parameter server, or the landing buffer of a reduce-scatter, holds);
+//   FLAT    d_grads is [W] flat P-element buffers; server j's slice of worker k starts at element off[j].
+// and any kept-row mode (one shared row, one row per server, device-side counts).
+//
+// Work list (hard part 4): the grid is one CTA per (server, tile); tile_start[j] is the
+// prefix sum of ceil(len_j / TILE) (psync_shard_worklist), a CTA finds its server by binary search.  A tile never
+// straddles two servers, so every CTA stages ONE kept row and streams with 128-bit loads.
+//
+// Alignment (hard part 3): the 128-bit stream is aligned to the GRADIENT slices -- they are 96 % of the bytes.
+// The first kept worker's slice base fixes a head peel h < E elements; units are [h + uE, h + (u+1)E) of the
+// slice.  A kept worker whose base has another phase is read with narrower loads (that worker only); the
+// head/tail peel (< 2E elements per server) is done element by element by the server's first CTA.  theta /
+// state / ema start at element off[j] + h of flat arrays, which for ragged cuts is NOT 16-byte aligned in
+// general: then the sums are transposed through shared memory and theta / state / ema are read and written
+// with coalesced 32-bit accesses (thread t <-> element t, t + 256, ...), so they still move every byte once.
+// The arithmetic per element is exactly K2's (same fixed-order fp32 sum, same update_element): bit-identical.
+
+#include "psync_device.cuh"
+
+namespace psync {
+namespace {
+
+using namespace dev;
+
+constexpr int kThreads = 256;  // = PSYNC_TILE_UNITS: one 16-byte unit per thread
+constexpr int kU = 8;          // independent 128-bit loads in flight per thread
+
+// smallest j with a[j+1] > i (a is a non-decreasing prefix array of M+1 entries, a[M] > i).  Plain loads: the
+// table may have been written by the predecessor kernel (psync_shard_worklist) under programmatic dependent launch.
+__device__ __forceinline__ int upper_slot(const int64_t* a, int M, int64_t i) {
+  int lo = 0, hi = M - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (a[mid + 1] > i) hi = mid; else lo = mid + 1;
+  }
+  return lo;
+}
+
+// 16 bytes at `a`, which is 16-byte aligned iff `aligned`; otherwise assembled from element-aligned loads.
+template <bool BF16>
+__device__ __forceinline__ uint4 load_unit_any(const char* a, bool aligned) {
+  if (aligned) return ldg_stream16(a);
+  uint4 r;
+  if (!BF16 || (reinterpret_cast<uintptr_t>(a) & 3u) == 0) {
+    const float* f = reinterpret_cast<const float*>(a);
+    r.x = __float_as_uint(ldg_stream_f32(f));
+    r.y = __float_as_uint(ldg_stream_f32(f + 1));
+    r.z = __float_as_uint(ldg_stream_f32(f + 2));
+    r.w = __float_as_uint(ldg_stream_f32(f + 3));
+  } else {
+    const uint16_t* s = reinterpret_cast<const uint16_t*>(a);
+    uint32_t w[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+      w[i] = static_cast<uint32_t>(ldg_stream_u16(s + 2 * i)) | (static_cast<uint32_t>(ldg_stream_u16(s + 2 * i + 1)) << 16);
+    r = make_uint4(w[0], w[1], w[2], w[3]);
+  }
+  return r;
+}
+
+template <bool BF16, int OPT, int EMA, int MINB>
+__global__ void __launch_bounds__(kThreads, MINB) sharded_aggregate_update_ema(const FusedParams p) {
+  constexpr int E = BF16 ? 8 : 4;
+  constexpr int ESZ = BF16 ? 2 : 4;
+  constexpr int Q = E / 4;
+  __shared__ const char* s_ptr[kMaxWorkers];
+  __shared__ __align__(16) float s_acc[kThreads * E];
+  __shared__ unsigned s_ref;
+
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+
+  // ---- which (server, tile) is this CTA ---------------------------------------------------------------
+  const int64_t b = blockIdx.x;
+  const int j = upper_slot(p.tile_start, p.M, b);
+  const int64_t off_j = p.shard_off[j];
+  const int64_t len_j = p.shard_off[j + 1] - off_j;
+  const int64_t tile = b - p.tile_start[j];
+  const int row = p.per_shard ? j : 0;
+  if (p.status != nullptr && p.status[row] != 0) return;  // this server did not collect its gradients
+  const int N = p.n_kept ? p.n_kept[row] : p.N;
+  if (N <= 0 || N > p.kept_stride || N > kMaxWorkers) return;  // a count nobody wrote: treat the row as failed
+  const float inv_N = p.n_kept ? 1.0f / static_cast<float>(N) : p.inv_N;
+
+  // ---- stage server j's kept row as slice base pointers; the first one fixes the 16-byte phase -----------
+  const int32_t* kept = p.kept + static_cast<int64_t>(row) * p.kept_stride;
+  for (int i = threadIdx.x; i < N; i += kThreads) {
+    const int k = kept[i];
+    const char* g = p.slices ? static_cast<const char*>(p.grads[static_cast<int64_t>(k) * p.M + j])
+                             : static_cast<const char*>(p.grads[k]) + off_j * ESZ;
+    s_ptr[i] = g;
+    if (i == 0) s_ref = static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 15u;
+  }
+  __syncthreads();
+  const unsigned ref = s_ref;
+  const int h = static_cast<int>(((16u - ref) & 15u) / ESZ);  // head peel: elements before the first 16-byte boundary
+  unsigned mis = 0;
+  for (int i = threadIdx.x; i < N; i += kThreads) {
+    const char* g = s_ptr[i];
+    mis |= (static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 15u) ^ ref;
+    s_ptr[i] = g + h * ESZ;  // unit u of this worker = s_ptr[i] + 16 u
+  }
+  const bool mixed = __syncthreads_or(static_cast<int>(mis)) != 0;  // some kept worker has another phase
+
+  const int64_t nu = len_j > h ? (len_j - h) / E : 0;  // whole units of this server
+  const int64_t u0 = tile * kThreads;
+  const int64_t e0 = off_j + h;                        // parameter index of unit 0's first element
+
+  if (u0 < nu) {
+    const int64_t live_units = (nu - u0 < kThreads) ? (nu - u0) : kThreads;
+    const bool live = threadIdx.x < live_units;
+    const int64_t unit = live ? (u0 + threadIdx.x) : (nu - 1);  // dead slots re-read a valid unit, store nothing
+    float acc[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) acc[e] = 0.f;
+
+    if (!mixed) {
+      int n = 0;
+      for (; n + kU <= N; n += kU) {
+        uint4 r[kU];
+#pragma unroll
+        for (int u = 0; u < kU; ++u) r[u] = ldg_stream16(s_ptr[n + u] + unit * 16);
+#pragma unroll
+        for (int u = 0; u < kU; ++u) accumulate_unit<BF16>(acc, r[u]);  // strictly ascending worker order
+      }
+      if (n < N) {
+        uint4 r[kU];
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+          const bool on = (n + u) < N;
+          r[u] = on ? ldg_stream16(s_ptr[on ? (n + u) : (N - 1)] + unit * 16) : make_uint4(0u, 0u, 0u, 0u);
+        }
+#pragma unroll
+        for (int u = 0; u < kU; ++u)
+          if ((n + u) < N) accumulate_unit<BF16>(acc, r[u]);
+      }
+    } else {
+#pragma unroll 4
+      for (int n = 0; n < N; ++n) {
+        const char* g = s_ptr[n];
+        const uint4 r = load_unit_any<BF16>(g + unit * 16, (reinterpret_cast<uintptr_t>(g) & 15u) == 0);
+        accumulate_unit<BF16>(acc, r);
+      }
+    }
+
+    const bool theta_vec = p.base_aligned != 0 && (e0 & 3) == 0;  // CTA-uniform
+    if (theta_vec) {
+      float4 th[Q], em[Q], a0[Q], a1[Q];
+#pragma unroll
+      for (int q = 0; q < Q; ++q) {
+        const int64_t e = e0 + unit * E + 4 * q;
+        th[q] = ld_state16(p.theta + e);
+        if (EMA != EMA_OFF) em[q] = ld_state16(p.ema + e);
+        if (OPT != OPT_SGD) a0[q] = ld_state16(p.s0 + e);
+        if (OPT == OPT_RMSPROP_MOM) a1[q] = ld_state16(p.s1 + e);
+      }
+#pragma unroll
+      for (int q = 0; q < Q; ++q) {
+        float* t4 = reinterpret_cast<float*>(&th[q]);
+        float* e4 = reinterpret_cast<float*>(&em[q]);
+        float* x4 = reinterpret_cast<float*>(&a0[q]);
+        float* y4 = reinterpret_cast<float*>(&a1[q]);
+#pragma unroll
+        for (int l = 0; l < 4; ++l) update_element<OPT, EMA>(acc[4 * q + l], inv_N, t4[l], e4[l], x4[l], y4[l], p);
+        if (live) {
+          const int64_t e = e0 + unit * E + 4 * q;
+          st_state16(p.theta + e, th[q]);
+          if (EMA != EMA_OFF) st_state16(p.ema + e, em[q]);
+          if (OPT != OPT_SGD) st_state16(p.s0 + e, a0[q]);
+          if (OPT == OPT_RMSPROP_MOM) st_state16(p.s1 + e, a1[q]);
+        }
+      }
+    } else {
+      // theta's slice is not co-aligned with the gradient units: transpose the sums through shared memory so that
+      // thread t owns elements t, t + 256, ... of the tile and theta / state / ema move as coalesced 32-bit accesses.
+#pragma unroll
+      for (int q = 0; q < Q; ++q)
+        *reinterpret_cast<float4*>(&s_acc[(threadIdx.x * Q + q) * 4]) =
+            make_float4(acc[4 * q], acc[4 * q + 1], acc[4 * q + 2], acc[4 * q + 3]);
+      __syncthreads();
+      const int64_t tile_e0 = e0 + u0 * E;
+      const int live_elems = static_cast<int>(live_units) * E;
+      float th[E], em[E], a0[E], a1[E], S[E];
+#pragma unroll
+      for (int q = 0; q < E; ++q) {
+        const int idx = q * kThreads + threadIdx.x;
+        const int64_t e = tile_e0 + (idx < live_elems ? idx : 0);
+        S[q] = s_acc[idx];
+        th[q] = p.theta[e];
+        if (EMA != EMA_OFF) em[q] = p.ema[e];
+        if (OPT != OPT_SGD) a0[q] = p.s0[e];
+        if (OPT == OPT_RMSPROP_MOM) a1[q] = p.s1[e];
+      }
+#pragma unroll
+      for (int q = 0; q < E; ++q) {
+        const int idx = q * kThreads + threadIdx.x;
+        update_element<OPT, EMA>(S[q], inv_N, th[q], em[q], a0[q], a1[q], p);
+        if (idx < live_elems) {
+          const int64_t e = tile_e0 + idx;
+          p.theta[e] = th[q];
+          if (EMA != EMA_OFF) p.ema[e] = em[q];
+          if (OPT != OPT_SGD) p.s0[e] = a0[q];
+          if (OPT == OPT_RMSPROP_MOM) p.s1[e] = a1[q];
+        }
+      }
+    }
+  }
+
+  // ---- head and tail peel of server j (fewer than 2E elements), by its first CTA --------------------------
+  if (tile == 0) {
+    const int64_t tail0 = h + nu * E;  // first element after the whole units (h > len_j: everything is "head")
+    const int64_t n_head = h < len_j ? h : len_j;
+    const int64_t n_tail = len_j > tail0 ? len_j - tail0 : 0;
+    if (threadIdx.x < n_head + n_tail) {
+      const int64_t e = threadIdx.x < n_head ? threadIdx.x : tail0 + (threadIdx.x - n_head);
+      float S = 0.f;
+#pragma unroll 8
+      for (int n = 0; n < N; ++n) S += load_grad_scalar<BF16>(s_ptr[n] - h * ESZ, e);
+      update_in_memory<OPT, EMA>(p, S, inv_N, off_j + e);
+    }
+  }
+}
+
+// ---- work list: tile_start[j] = sum_{i<j} ceil(len_i / tile_elems), tile_start[M] = number of tiles ----------
+__global__ void __launch_bounds__(1024) shard_worklist_kernel(const int64_t* shard_off, int32_t M, int32_t tile_elems,
+                                                              int64_t* __restrict__ tile_start) {
+  __shared__ int64_t s_warp[32];
+  __shared__ int64_t s_carry;
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (threadIdx.x == 0) {
+    s_carry = 0;
+    tile_start[0] = 0;
+  }
+  __syncthreads();
+  for (int32_t base = 0; base < M; base += 1024) {  // 1024 servers per round, inclusive block scan
+    const int32_t j = base + threadIdx.x;
+    int64_t v = 0;
+    if (j < M) {
+      const int64_t len = shard_off[j + 1] - shard_off[j];
+      v = (len + tile_elems - 1) / tile_elems;
+    }
+    int64_t incl = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int64_t up = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+      if (lane >= d) incl += up;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+      int64_t w = s_warp[lane];
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int64_t up = __shfl_up_sync(0xFFFFFFFFu, w, d);
+        if (lane >= d) w += up;
+      }
+      s_warp[lane] = w;
+    }
+    __syncthreads();
+    const int64_t carry = s_carry;
+    const int64_t before = warp > 0 ? s_warp[warp - 1] : 0;
+    if (j < M) tile_start[j + 1] = carry + before + incl;
+    __syncthreads();
+    if (threadIdx.x == 1023) s_carry = carry + before + incl;
+    __syncthreads();
+  }
+}
+
+using KernelFn = void (*)(const FusedParams);
+
+// bf16 gradients hold 8 parameters per thread: with RMSProp (40 live values) 3 CTAs/SM, like K2 (fused_kernel.cu)
+template <bool BF16, int OPT>
+KernelFn pick_ema(int ema) {
+  constexpr int MINB = (BF16 && OPT == OPT_RMSPROP_MOM) ? 3 : 4;
+  switch (ema) {
+    case EMA_POST: return sharded_aggregate_update_ema<BF16, OPT, EMA_POST, MINB>;
+    case EMA_PRE: return sharded_aggregate_update_ema<BF16, OPT, EMA_PRE, MINB>;
+    default: return sharded_aggregate_update_ema<BF16, OPT, EMA_OFF, MINB>;
+  }
+}
+template <bool BF16>
+KernelFn pick_opt(int opt, int ema) {
+  switch (opt) {
+    case OPT_SGD: return pick_ema<BF16, OPT_SGD>(ema);
+    case OPT_MOMENTUM: return pick_ema<BF16, OPT_MOMENTUM>(ema);
+    default: return pick_ema<BF16, OPT_RMSPROP_MOM>(ema);
+  }
+}
+
+}  // namespace
+
+int sharded_tile_elems(int dtype) { return kThreads * (dtype == 1 ? 8 : 4); }
+
+cudaError_t launch_shard_worklist(const int64_t* d_shard_off, int32_t M, int dtype, int64_t* d_tile_start,
+                                  cudaStream_t stream) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(1);
+  cfg.blockDim = dim3(1024);
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, shard_worklist_kernel, d_shard_off, M, static_cast<int32_t>(sharded_tile_elems(dtype)),
+                            d_tile_start);
+}
+
+cudaError_t launch_sharded(const FusedParams& p, int dtype, int opt, int ema, int64_t n_tiles, cudaStream_t stream) {
+  if (n_tiles <= 0) return cudaSuccess;
+  if (n_tiles > 0x7FFFFFFF) return cudaErrorInvalidConfiguration;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(static_cast<unsigned>(n_tiles));
+  cfg.blockDim = dim3(kThreads);
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, dtype == 1 ? pick_opt<true>(opt, ema) : pick_opt<false>(opt, ema), p);
+}
+
+}  // namespace psync

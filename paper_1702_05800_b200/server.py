@@ -6,6 +6,7 @@ the device pointer table of the W gradient buffers, and enqueues the selection f
 """
 from __future__ import annotations
 
+from collections import deque
 from typing import Optional, Sequence
 
 import numpy as np
@@ -30,12 +31,19 @@ class ParameterServerStep:
         self.d_status = torch.full((1,), B.PSYNC_ECUDA, dtype=torch.int32, device=dev)
         self.d_t_nth = torch.zeros(1, dtype=torch.float32, device=dev)
         self.table: Optional[B.GradTable] = None
+        # A fused kernel in flight stages its pointers from the table it was launched with for its whole lifetime
+        # (each CTA reads it at its own start).  Tables replaced by set_gradients() are therefore kept alive for a few
+        # steps instead of going straight back to torch's caching allocator, and step() also records the launch stream
+        # on the table, so a step enqueued on a side stream can never see its table's block reused under it.
+        self._retired = deque(maxlen=4)
         self._step = None
         self._keep = None
 
     def set_gradients(self, buffers: Sequence[torch.Tensor]) -> None:
         if len(buffers) != self.W:
             raise ValueError(f"need W = {self.W} gradient buffers")
+        if self.table is not None:
+            self._retired.append((self.table, self._keep))
         self.table = B.make_grad_table(buffers)
         self._step = None
 
@@ -57,6 +65,8 @@ class ParameterServerStep:
             raise RuntimeError("set_gradients() first")
         if self._step is None or self._step.gamma_t != np.float32(gamma_t):
             self._build(gamma_t)
+        if stream is not None and hasattr(stream, "cuda_stream"):
+            self.table.d_ptrs.record_stream(stream)
         B.psync_step_device(self._step, d_arrival, self.d_t_nth, d_step_tag, t, stream)   # K1 + K2, one C call
 
     def aggregate_only(self, gamma_t: float, stream=None) -> None:

@@ -49,7 +49,7 @@ def test_synchronous_step_every_template_instance(dtype, opt, ema_mode):
             assert_bits(pair.ps, pair.host, f"{cfg.name} step {s}")
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3, 4])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6])      # 5: cp.async.bulk ring; 6: 256-bit loads
 def test_every_variant_and_the_scalar_path(variant):
     cfg = replace(BASE, opt=synth.RMSPROP_MOM, N=100, b=6, P=40_001, name=f"bits_variant{variant}")
     pair = Pair(cfg, variant=variant)
@@ -59,6 +59,27 @@ def test_every_variant_and_the_scalar_path(variant):
         pair.gpu_step(grads, arrival)
         pair.oracle_step(grads, arrival)
     assert_bits(pair.ps, pair.host, cfg.name)
+
+
+@pytest.mark.parametrize("dtype,opt", [(synth.F32, synth.RMSPROP_MOM), (synth.BF16, synth.MOMENTUM)])
+def test_shard_aware_kernel_on_misaligned_slices(dtype, opt):
+    """The slices layout through the work list: aligned, one-phase and mixed-phase slices, transposed epilogue."""
+    from test_gpu_slices import RAGGED, SlicesPair, cut_slices
+    cfg = replace(BASE, grad_dtype=dtype, opt=opt, name=f"bits_slices_{dtype}_{opt}")
+    pair = SlicesPair(cfg, shard_off=RAGGED)
+    with oracle.fp32_mirror():
+        for s, offs in enumerate([None, lambda k, j: (3 * j + 1) % 8, lambda k, j: (5 * k + 3 * j) % 8]):
+            flat = [synth.gradient(cfg, s, k, DEV) for k in range(cfg.W)]
+            slices = cut_slices(flat, pair.off, offs)
+            arrival = synth.arrival_times(cfg, s)
+            d_kept = torch.full((cfg.N,), -1, dtype=torch.int32, device=DEV)
+            d_status = torch.full((1,), -9, dtype=torch.int32, device=DEV)
+            st, keep = pair.make_step(psync.make_slice_table(slices), d_kept, d_status)
+            psync.psync_step_device(st, torch.from_numpy(arrival).to(DEV))
+            torch.cuda.synchronize()
+            _, kept, _ = oracle.select_first_n(arrival, cfg.N, cfg.b)
+            pair.oracle(slices, kept)
+            assert_bits(pair, pair.host, f"{cfg.name} step {s}")
 
 
 def test_per_server_rows_and_timeout_device_side_divisor():

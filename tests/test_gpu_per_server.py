@@ -24,11 +24,10 @@ class RowsPair:
     """One parameter-server state on the GPU and on the host, stepped with kept ROWS (per server and/or
     variable count) on both sides from the same bytes."""
 
-    def __init__(self, cfg, shard_off=None, grid_ctas=0, misalign=0):
+    def __init__(self, cfg, shard_off=None, misalign=0):
         self.cfg = cfg
         self.off = synth.shard_offsets(cfg) if shard_off is None else np.asarray(shard_off, dtype=np.int64)
         self.M = self.off.size - 1
-        self.grid_ctas = grid_ctas
         self.misalign = misalign
 
         def place(t):      # optionally put the array at an element offset that breaks 16-byte alignment
@@ -51,7 +50,7 @@ class RowsPair:
         return psync.make_step(self.off, cfg.N, cfg.W, table.grad_dtype, self.theta, self.ema, self.state0,
                                self.state1, opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha,
                                mu=cfg.mu, rho=cfg.rho, eps=cfg.eps, d_grads=table.d_ptrs, d_kept=d_kept,
-                               d_status=d_status, grid_ctas=self.grid_ctas, per_shard=per_shard,
+                               d_status=d_status, per_shard=per_shard,
                                kept_stride=kept_stride, d_shard_off=self.d_off if per_shard else None,
                                d_n_kept=d_n_kept)
 
@@ -192,13 +191,6 @@ def test_per_server_stale_tags_per_row():
     pair.step_first_n(0, a, tags=tags, t=3)
 
 
-def test_per_server_forced_small_grid_restages_rows_per_tile():
-    cfg = per_server_cfg(P=300_007, M=13, opt=synth.MOMENTUM, name="ps_grid")
-    for grid in (1, 7, 148):
-        pair = RowsPair(cfg, grid_ctas=grid)
-        pair.step_first_n(0, synth.arrival_times_per_server(cfg, 0, server_sigma=0.3))
-
-
 @pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
 def test_per_server_unaligned_state_takes_the_scalar_path(dtype):
     cfg = per_server_cfg(P=9_001, grad_dtype=dtype, opt=synth.RMSPROP_MOM, name="ps_unaligned")
@@ -290,7 +282,7 @@ def test_select_timeout_matches_oracle(seed):
                     assert n_g[r] == kept.size and np.array_equal(kept_g[r, :kept.size], kept)
                     assert (kept_g[r, kept.size:] == -1).all()
                 else:
-                    assert n_g[r] == -7 and (kept_g[r] == -1).all()      # nothing written
+                    assert n_g[r] == 0 and (kept_g[r] == -1).all()       # the count is zeroed, the row is not written
 
 
 @pytest.mark.parametrize("per_shard", [False, True])
