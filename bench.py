@@ -1,7 +1,12 @@
 #!/usr/bin/env python
 """bench.py -- whole-job throughput of the parameter-server step (Alg. 4) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg3] [--impl psync|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg1..cfg5] [--impl psync|reference]
+                    [--mode first_n|per_server|timeout|async] [--layout flat|slices] [--variant 1..6] [--servers M]
+
+The default run is the headline (cfg3, first_n, flat buffers); its JSON line also carries `also`: short
+measurements of cfg2, cfg4, every other mode, the slices layout, many-server cuts and launch variants 5 / 6.
+`--config cfg5` runs BASELINE.json's bandwidth sweep (one JSON line with every point, `--sweep-md` for the table).
 
 A "step" is one pass of the whole hot path -- psync_select_first_n then the fused
 psync_aggregate_update (sum of the N kept gradients, optimizer update, EMA) -- over one batch of
@@ -12,7 +17,7 @@ N*P*sizeof(grad) + P*8*(1 + n_state + 1).
 
 Multi-GPU (--gpus N under torchrun): the step does not shard across GPUs (north_star: no
 collectives) -> N independent replicas, weak scaling; value = units of all ranks / max-over-ranks
-time.  `--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded sample.
+time.  `--impl reference` times the CPU oracle (oracle/) as it stands on the host cores on the full workload.
 """
 from __future__ import annotations
 
@@ -137,34 +142,31 @@ def load_peaks():
 
 
 # ------------------------------------------------------------------------------------ CPU oracle legs
-def oracle_sample(cfg, seconds_budget=12.0, sample_elems=1 << 22, max_steps=2000, warmup=0, fixed_steps=None,
-                  wall_budget=60.0):
-    """Times the oracle AS IT STANDS on the host cores on a bounded sample of the workload: the first
-    `sample_elems` parameters of every buffer (same N, b, M-way ragged cut, optimizer, distributions).
-    The W gradient buffers of the sample are drawn once (not timed); every step has fresh arrival
-    times, hence a fresh kept set, and continues from the previous step's theta / state / ema.
-    Runs `fixed_steps` steps, else until `seconds_budget` seconds of oracle time (or `wall_budget`
-    seconds of wall clock).  Returns (grad-elements/s, info)."""
+def oracle_full(cfg, host_grads, seconds_budget=12.0, max_steps=2000, warmup=0, fixed_steps=None, wall_budget=90.0,
+                first_step=0):
+    """Times the oracle AS IT STANDS (oracle.select_first_n + oracle.aggregate_update, all host cores) on the FULL
+    workload: all P parameters of the W gradient buffers in `host_grads` (numpy, host RAM; for the cpu_baseline leg the
+    exact bytes of the GPU's gradient set 0, copied D2H before timing), fresh arrival times every step, continuing from
+    the previous step's theta / state / ema.  Runs `fixed_steps` steps, else until `seconds_budget` seconds of oracle
+    time (or `wall_budget` seconds of wall clock).  Returns (grad-elements/s, info)."""
     import oracle  # the one place bench.py executes oracle/ (cpu_baseline / --impl reference)
 
-    Ps = int(min(sample_elems, cfg.P))
-    sub = synth.scaled(cfg, Ps, name=cfg.name + "_sample")
-    off = synth.shard_offsets(sub)
-    theta = synth.init_theta(sub).numpy().copy()
-    s0, s1 = synth.init_state(sub)
+    off = synth.shard_offsets(cfg)
+    theta = synth.init_theta(cfg).numpy().copy()
+    s0, s1 = synth.init_state(cfg)
     s0 = None if s0 is None else s0.numpy().copy()
     s1 = None if s1 is None else s1.numpy().copy()
     ema = theta.copy()
     t_begin = time.perf_counter()
-    grads = [synth.as_numpy_grad(synth.gradient(sub, 0, k)) for k in range(sub.W)]   # not timed
     times = []
     total_steps = (fixed_steps + warmup) if fixed_steps is not None else max_steps
     for s in range(total_steps):
-        arrival = synth.arrival_times(sub, s)
+        arrival = synth.arrival_times(cfg, first_step + s)
         t0 = time.perf_counter()
-        st, kept, _ = oracle.select_first_n(arrival, sub.N, sub.b)
-        rc = oracle.aggregate_update(off, sub.N, grads, kept, theta, ema, s0, s1, opt=sub.opt, ema_mode=sub.ema_mode,
-                                     gamma_t=sub.gamma, alpha=sub.alpha, mu=sub.mu, rho=sub.rho, eps=sub.eps)
+        st, kept, _ = oracle.select_first_n(arrival, cfg.N, cfg.b)
+        rc = oracle.aggregate_update(off, cfg.N, host_grads, kept, theta, ema, s0, s1, opt=cfg.opt,
+                                     ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho,
+                                     eps=cfg.eps)
         t1 = time.perf_counter()
         assert st == 0 and rc == 0
         if s >= warmup:
@@ -172,109 +174,213 @@ def oracle_sample(cfg, seconds_budget=12.0, sample_elems=1 << 22, max_steps=2000
         if fixed_steps is None and times and (sum(times) > seconds_budget or t1 - t_begin > wall_budget):
             break
     sec = float(np.sum(times))
-    value = sub.N * Ps * len(times) / sec
+    value = cfg.N * cfg.P * len(times) / sec
     info = {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"first {Ps} of P={cfg.P} parameters of every buffer, N={cfg.N} b={cfg.b}, "
-                      f"{len(times)} steps, {sec:.2f} s of oracle time (select + aggregate/update/EMA; "
-                      f"input generation excluded)",
-            "ms_per_step_sample": 1e3 * sec / len(times),
-            "gbps": sub.bytes_per_step * len(times) / sec / 1e9}
+            "note": "the oracle as it stands, never tuned: double arithmetic, element-major over the N kept streams",
+            "sample": f"the FULL workload: all P={cfg.P} parameters of the W={cfg.W} gradient buffers of one resident "
+                      f"gradient set held in host RAM, N={cfg.N} b={cfg.b}, fresh arrival times per step, "
+                      f"{len(times)} steps, {sec:.2f} s of oracle time (select + aggregate/update/EMA; input "
+                      f"generation and device-to-host copies excluded)",
+            "ms_per_step": 1e3 * sec / len(times),
+            "gbps": cfg.bytes_per_step * len(times) / sec / 1e9}
     return value, info
 
 
+def host_gradient_set(cfg, device="cpu", set_id=0):
+    """The W gradient buffers of one set in host RAM (numpy): drawn on `device` with the workload's seeds."""
+    out = []
+    for k in range(cfg.W):
+        out.append(synth.as_numpy_grad(synth.gradient(cfg, set_id, k, device)).copy())
+    return out
+
+
+def host_ram_ok(cfg) -> bool:
+    need = cfg.W * cfg.P * cfg.grad_bytes + 6 * 4 * cfg.P + (2 << 30)
+    try:
+        import psutil
+        return psutil.virtual_memory().available > need
+    except Exception:  # noqa: BLE001
+        return True
+
+
 def run_reference(args, cfg, rank):
-    """--impl reference: the oracle on the host cores, K steps of a bounded sample, same metric."""
+    """--impl reference: the oracle on the host cores, K steps of the FULL workload (no GPU is touched: the
+    gradient set is drawn by torch's CPU generator with the workload's seeds and distribution), same metric."""
     if rank != 0:
         return None
-    value, info = oracle_sample(cfg, sample_elems=args.ref_sample_elems, warmup=args.warmup, fixed_steps=args.steps)
+    run_cfg = cfg if args.ref_sample_elems <= 0 else synth.scaled(cfg, int(min(args.ref_sample_elems, cfg.P)),
+                                                                   name=cfg.name)
+    if run_cfg is cfg and not host_ram_ok(cfg):        # a host without room for one gradient set: bounded sample
+        run_cfg = synth.scaled(cfg, 1 << 22, name=cfg.name)
+    grads = host_gradient_set(run_cfg)
+    value, info = oracle_full(run_cfg, grads, warmup=args.warmup, fixed_steps=args.steps)
+    if run_cfg is not cfg:
+        info["sample"] = f"first {run_cfg.P} of P={cfg.P} parameters of every buffer; " + info["sample"]
     return {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": info["ms_per_step_sample"],
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": info["ms_per_step"],
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64 arithmetic on f32 storage", "data": "synthetic",
-            "config": workload_config(cfg, extra={"sample": info["sample"]}),
-            "cpu_baseline": {k: info[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "config": workload_config(cfg, "first_n", "flat"),
+            "cpu_baseline": {k: info[k] for k in ("value", "unit", "cores", "kind", "sample", "note")},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
 
 
-def workload_config(cfg, extra=None):
-    c = {"workload": f"{cfg.name}: P={cfg.P} fp32 params in M={cfg.M} ragged shards, N={cfg.N}, b={cfg.b}, "
-                     f"{'bf16' if cfg.grad_dtype == synth.BF16 else 'fp32'} gradients, {OPT_NAME[cfg.opt]}, EMA",
-         "P": cfg.P, "M": cfg.M, "N": cfg.N, "b": cfg.b, "optimizer": OPT_NAME[cfg.opt],
-         "grad_dtype": "bf16" if cfg.grad_dtype == synth.BF16 else "fp32", "gamma": cfg.gamma, "alpha": cfg.alpha,
-         "bytes_per_step_model": cfg.bytes_per_step, "parallelism": "replicas only (no sharding across GPUs)"}
-    if extra:
-        c.update(extra)
-    return c
+def workload_config(cfg, mode="first_n", layout="flat"):
+    """The `config` object: names the workload; identical for the CUDA arm and the reference arm."""
+    return {"workload": f"{cfg.name}: P={cfg.P} fp32 params in M={cfg.M} ragged shards, N={cfg.N}, b={cfg.b}, "
+                        f"{'bf16' if cfg.grad_dtype == synth.BF16 else 'fp32'} gradients, {OPT_NAME[cfg.opt]}, EMA",
+            "P": cfg.P, "M": cfg.M, "N": cfg.N, "b": cfg.b, "optimizer": OPT_NAME[cfg.opt],
+            "grad_dtype": "bf16" if cfg.grad_dtype == synth.BF16 else "fp32", "gamma": cfg.gamma, "alpha": cfg.alpha,
+            "bytes_per_step_model": cfg.bytes_per_step, "parallelism": "replicas only (no sharding across GPUs)",
+            "mode": mode, "grad_layout": layout,
+            "l2": f"no flush: each step streams {cfg.bytes_per_step / 1e9:.2f} GB (>> 126 MB L2) and the gradient "
+                  f"buffers rotate over several resident sets"}
 
 
 # ------------------------------------------------------------------------------------ the CUDA arm
-def run_psync(args, cfg, rank, world, dist):
-    import paper_1702_05800_b200 as psync
+L2_BYTES = 126 * 10**6
 
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU path")
-    local = env_int("LOCAL_RANK", 0)
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    K, Wm = args.steps, args.warmup
-    off = synth.shard_offsets(cfg)
-    # resident gradient sets, rotated step by step: every step streams buffers it did not just touch
-    set_bytes = cfg.W * cfg.P * cfg.grad_bytes
-    free, _ = torch.cuda.mem_get_info()
-    n_sets = int(max(1, min(args.grad_sets, (0.7 * free) // max(set_bytes, 1))))
-    tdt = torch.float32 if cfg.grad_dtype == synth.F32 else torch.bfloat16
-    tables = []
-    for r in range(n_sets):
-        bufs = [torch.empty(cfg.P, dtype=tdt, device=dev) for _ in range(cfg.W)]
-        for k in range(cfg.W):
-            synth.gradient(cfg, r, k, dev, out=bufs[k])
-        tables.append(psync.make_grad_table(bufs))
-    theta = synth.init_theta(cfg, dev)
-    s0, s1 = synth.init_state(cfg, dev)
-    ema = theta.clone()
-    ps = psync.ParameterServerStep(off, cfg.N, cfg.b, theta, ema, s0, s1, cfg.opt, cfg.ema_mode, alpha=cfg.alpha,
-                                   mu=cfg.mu, rho=cfg.rho, eps=cfg.eps, grid_ctas=args.grid_ctas, variant=args.variant)
 
-    # --mode first_n (default, the headline): one kept set of N per step (reading R11).
-    # --mode per_server: Alg. 4 per server j, arrival [M][W] -> kept [M][N] (NEXT-1).
-    # --mode timeout: keep every worker that arrived by --timeout seconds, divide by the count (NEXT-2).
-    mode = args.mode
+class Workload:
+    """Device-resident data of one config: `n_sets` gradient sets (flat buffers or per-(worker, server) slices), the
+    pointer tables, theta / state / ema, the shard table and the (server, tile) work list."""
+
+    def __init__(self, psync, cfg, dev, n_sets, layout="flat", state_first=False):
+        self.cfg, self.dev, self.layout = cfg, dev, layout
+        self.off = synth.shard_offsets(cfg)
+        tdt = torch.float32 if cfg.grad_dtype == synth.F32 else torch.bfloat16
+        set_bytes = cfg.W * cfg.P * cfg.grad_bytes
+        free, _ = torch.cuda.mem_get_info()
+        self.n_sets = int(max(1, min(n_sets, (0.7 * free) // max(set_bytes, 1))))
+        self.tables, self.sets = [], []
+        if layout == "flat":
+            for r in range(self.n_sets):     # gradient sets are allocated before theta / state (DESIGN.md s.5)
+                bufs = [torch.empty(cfg.P, dtype=tdt, device=dev) for _ in range(cfg.W)]
+                for k in range(cfg.W):
+                    synth.gradient(cfg, r, k, dev, out=bufs[k])
+                self.sets.append(bufs)
+                self.tables.append(psync.make_grad_table(bufs))
+        elif cfg.M <= 64:                    # every (worker, server) slice is its own allocation
+            tmp = torch.empty(cfg.P, dtype=tdt, device=dev)
+            for r in range(self.n_sets):
+                slices = []
+                for k in range(cfg.W):
+                    synth.gradient(cfg, r, k, dev, out=tmp)
+                    row = []
+                    for j in range(cfg.M):
+                        lo, hi = int(self.off[j]), int(self.off[j + 1])
+                        t = torch.empty(hi - lo, dtype=tdt, device=dev)
+                        t.copy_(tmp[lo:hi])
+                        row.append(t)
+                    slices.append(row)
+                self.sets.append(slices)
+                self.tables.append(psync.make_slice_table(slices))
+            del tmp
+            self.slices_how = "every slice its own torch allocation"
+        else:
+            # Thousands of servers: W*M separate tensors cost minutes of Python, so each worker's slices are carved
+            # from one arena at 256-byte boundaries (the alignment a separate cudaMalloc would give each of them);
+            # the kernel sees the same thing either way -- W*M unrelated base pointers in a table.
+            lens = np.diff(self.off)
+            esz = cfg.grad_bytes
+            starts = np.zeros(cfg.M, dtype=np.int64)      # arena offset of slice j, in elements
+            pos = 0
+            for j in range(cfg.M):
+                starts[j] = pos
+                pos = -(-(pos + int(lens[j])) * esz // 256) * 256 // esz
+            arena_elems = max(pos, 1)
+            pad = torch.from_numpy(starts - self.off[:-1]).to(dev)
+            dst = torch.arange(cfg.P, dtype=torch.int64, device=dev) + torch.repeat_interleave(
+                pad, torch.from_numpy(lens).to(dev))
+            tmp = torch.empty(cfg.P, dtype=tdt, device=dev)
+            for r in range(self.n_sets):
+                arenas = []
+                ptrs = np.empty((cfg.W, cfg.M), dtype=np.int64)
+                for k in range(cfg.W):
+                    synth.gradient(cfg, r, k, dev, out=tmp)
+                    arena = torch.zeros(arena_elems, dtype=tdt, device=dev)
+                    arena.index_copy_(0, dst, tmp)
+                    arenas.append(arena)
+                    ptrs[k] = arena.data_ptr() + starts * esz
+                self.sets.append(arenas)
+                self.tables.append(psync.binding.GradTable(torch.from_numpy(ptrs.reshape(-1)).to(dev), arenas,
+                                                           psync.PSYNC_F32 if esz == 4 else psync.PSYNC_BF16))
+            del tmp, dst
+            self.slices_how = "slices carved at 256-byte boundaries from one arena per worker"
+        self.theta = synth.init_theta(cfg, dev)
+        self.s0, self.s1 = synth.init_state(cfg, dev)
+        self.ema = self.theta.clone()
+        self.d_off = torch.from_numpy(self.off).to(dev)
+        self.d_tiles = psync.psync_shard_worklist(self.d_off, cfg.grad_dtype)
+
+    def with_servers(self, psync, M):
+        """The same resident flat gradient sets and state cut into M ragged servers (only the tables change)."""
+        from dataclasses import replace
+        other = object.__new__(Workload)
+        other.__dict__.update(self.__dict__)
+        other.cfg = replace(self.cfg, M=M, name=f"{self.cfg.name}_M{M}")
+        other.off = synth.shard_offsets(other.cfg)
+        other.d_off = torch.from_numpy(other.off).to(self.dev)
+        other.d_tiles = psync.psync_shard_worklist(other.d_off, other.cfg.grad_dtype)
+        return other
+
+    def reset_state(self):
+        cfg = self.cfg
+        self.theta.copy_(synth.init_theta(cfg, self.dev))
+        self.ema.copy_(self.theta)
+        s0, s1 = synth.init_state(cfg, self.dev)
+        if s0 is not None:
+            self.s0.copy_(s0)
+        if s1 is not None:
+            self.s1.copy_(s1)
+
+
+def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist=True, clip=0.0, probe_every=4):
+    """W warm-up + K timed steps of one (workload, mode) on `stream`; returns the per-step numbers, the fused kernel's
+    own CUDA-event duration (every `probe_every`-th timed step) and the clocks sampled during the timed region.
+      first_n     one kept set of N per step (the headline; reading R11)
+      per_server  Alg. 4 per server j: arrival [M][W] -> kept [M][N] (NEXT-1)
+      timeout     keep every worker that arrived by --timeout seconds, divide by the count (NEXT-2)
+      async       Alg. 2: all W gradients one at a time in arrival order, one pass (NEXT-3)"""
+    cfg, dev = wl.cfg, wl.dev
+    B = psync.binding
+    slices = wl.layout == "slices"
     rows = cfg.M if mode == "per_server" else 1
     if mode == "per_server":
         arr_np = np.stack([synth.arrival_times_per_server(cfg, s) for s in range(K + Wm)])
     else:
         arr_np = np.stack([synth.arrival_times(cfg, s) for s in range(K + Wm)])
     arrivals = torch.from_numpy(arr_np).to(dev)
-    # --mode async: Alg. 2 -- all W gradients applied one at a time in arrival order, one pass (NEXT-3).
     stride = cfg.W if mode in ("timeout", "async") else cfg.N
-    d_kept = torch.full((rows, stride), -1, dtype=torch.int32, device=dev) if mode != "first_n" else ps.d_kept
-    d_status = torch.full((rows,), 0 if mode == "async" else -9, dtype=torch.int32,
-                          device=dev) if mode != "first_n" else ps.d_status
+    d_kept = torch.full((rows, stride), -1, dtype=torch.int32, device=dev)
+    d_status = torch.full((rows,), 0 if mode == "async" else -9, dtype=torch.int32, device=dev)
+    d_t_nth = torch.zeros(rows, dtype=torch.float32, device=dev)
     d_n_kept = torch.zeros(rows, dtype=torch.int32, device=dev) if mode in ("timeout", "async") else None
-    d_off = torch.from_numpy(off).to(dev) if mode == "per_server" else None
+    use_tiles = slices or (mode == "per_server" and worklist)
     steps_struct = []
-    for tb in tables:   # one psync_step per gradient set, built once (marshalling outside the timed region)
-        st, keep = psync.make_step(off, cfg.N, cfg.W, tb.grad_dtype, theta, ema, s0, s1, opt=cfg.opt,
+    for tb in wl.tables:   # one psync_step per gradient set, built once (marshalling outside the timed region)
+        st, keep = psync.make_step(wl.off, cfg.N, cfg.W, tb.grad_dtype, wl.theta, wl.ema, wl.s0, wl.s1, opt=cfg.opt,
                                    ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho,
                                    eps=cfg.eps, d_grads=tb.d_ptrs, d_kept=d_kept, d_status=d_status,
-                                   grid_ctas=args.grid_ctas, variant=args.variant, per_shard=(mode == "per_server"),
-                                   d_shard_off=d_off, d_n_kept=d_n_kept)
+                                   grid_ctas=args.grid_ctas, variant=variant, per_shard=(mode == "per_server"),
+                                   d_shard_off=wl.d_off if (mode == "per_server" or slices) else None,
+                                   d_n_kept=d_n_kept,
+                                   grad_layout=psync.PSYNC_GRADS_SLICES if slices else psync.PSYNC_GRADS_FLAT,
+                                   d_tile_start=wl.d_tiles if use_tiles else None)
         steps_struct.append((st, keep))
     geo = psync.psync_launch_geometry(steps_struct[0][0])
     d_scales = d_clip_work = None
-    if mode == "async" and args.clip > 0:
+    if mode == "async" and clip > 0:
         d_scales = torch.ones(cfg.W, dtype=torch.float32, device=dev)
         d_clip_work = torch.empty(psync.psync_clip_workspace_bytes(cfg.W, cfg.P, cfg.grad_dtype) // 8,
                                   dtype=torch.float64, device=dev)
-
-    stream = torch.cuda.Stream(device=dev)
-    stream.wait_stream(torch.cuda.current_stream())    # tables, kept[] and status were filled on the default stream
-    B = psync.binding
+    n_sets = len(wl.tables)
+    stream.wait_stream(torch.cuda.current_stream())    # everything above was filled on the default stream
 
     def select(i):
         if mode == "first_n":
-            B.psync_select_first_n(arrivals[i], cfg.N, cfg.b, ps.d_kept, ps.d_status, ps.d_t_nth, None, i, stream)
+            B.psync_select_first_n(arrivals[i], cfg.N, cfg.b, d_kept, d_status, d_t_nth, None, i, stream)
         elif mode == "per_server":
             B.psync_select_first_n_sharded(arrivals[i], cfg.N, cfg.b, cfg.M, d_kept, d_status, None, None, i, stream)
         elif mode == "timeout":
@@ -293,9 +399,9 @@ def run_psync(args, cfg, rank, world, dist):
         if ev is not None:
             ev[1].record(stream)
         if mode == "async":
-            if args.clip > 0:            # A.3 (L313): global-norm clipping = one more pass over the W buffers
-                B.psync_clip_scales(tables[i % n_sets], args.clip, d_scales, d_clip_work, stream)
-            B.psync_async_apply(st, None, stream, d_gscale=d_scales if args.clip > 0 else None)
+            if clip > 0:                 # A.3 (L313): global-norm clipping = one more pass over the W buffers
+                B.psync_clip_scales(wl.tables[i % n_sets], clip, d_scales, d_clip_work, stream)
+            B.psync_async_apply(st, None, stream, d_gscale=d_scales if clip > 0 else None)
         else:
             B.psync_aggregate_update(st, stream)
         if ev is not None:
@@ -313,10 +419,10 @@ def run_psync(args, cfg, rank, world, dist):
     # Per-kernel CUDA events are recorded on every `probe_every`-th timed step only: an event between
     # the two launches breaks their programmatic-dependent-launch pairing and costs ~10 us, so the
     # other steps run exactly as a user's loop would.  All of it is inside the one timed region.
-    probe_every = max(1, args.probe_every)
+    probe_every = max(1, probe_every)
     evs = {k: [torch.cuda.Event(enable_timing=True) for _ in range(3)] for k in range(0, K, probe_every)}
     e_begin, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler = ClockSampler(local, period_s=args.clock_period_ms * 1e-3)
+    sampler = ClockSampler(env_int("LOCAL_RANK", 0), period_s=args.clock_period_ms * 1e-3)
     barrier()
     torch.cuda.synchronize()
     sampler.start()
@@ -333,7 +439,7 @@ def run_psync(args, cfg, rank, world, dist):
     select_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs.values()]))
     if os.environ.get("PSYNC_BENCH_DEBUG"):
         print("fused ms per probed step:", [round(x, 4) for x in fused_list], file=sys.stderr)
-    assert bool((d_status == 0).all()) and bool(torch.isfinite(theta[:4096]).all())
+    assert bool((d_status == 0).all()) and bool(torch.isfinite(wl.theta[:4096]).all())
 
     # gradient elements aggregated per step: N*P, or (workers in time)*P for the time-out rule
     if mode == "async":
@@ -343,39 +449,136 @@ def run_psync(args, cfg, rank, world, dist):
     else:
         n_eff = float(cfg.N)
     bytes_per_step = cfg.bytes_per_step + (n_eff - cfg.N) * cfg.P * cfg.grad_bytes
-    if mode == "async" and args.clip > 0:
+    launches_per_step = 2                    # selection (or arrival order) + the fused pass
+    if mode == "async" and clip > 0:
         bytes_per_step += cfg.W * cfg.P * cfg.grad_bytes      # the norm pass reads every buffer once more
-    units_local = n_eff * cfg.P * K
-    units, max_ms = aggregate_over_ranks(units_local, total_ms, dist)
+        launches_per_step = 4                # + sum-of-squares chunks + clip factors
+    return {"total_ms": total_ms, "ms_per_step": total_ms / K, "fused_ms": fused_ms, "select_ms": select_ms,
+            "fused_list": fused_list, "n_eff": n_eff, "bytes_per_step": bytes_per_step, "units": n_eff * cfg.P * K,
+            "clocks": clocks, "geo": geo, "launches_per_step": launches_per_step,
+            "kernel": "async_apply_kernel" if mode == "async" else
+                      ("sharded_aggregate_update_ema" if use_tiles else "fused_aggregate_update_ema")}
+
+
+def short_entry(cfg, mode, layout, m, peak, note=None):
+    """One entry of the `also` object: kernel ms, GB/s of algorithmic bytes, fractions, its own clocks."""
+    gbs = m["bytes_per_step"] / (m["fused_ms"] * 1e-3) / 1e9
+    e = {"workload": cfg.name, "mode": mode, "grad_layout": layout, "P": cfg.P, "M": cfg.M, "N": cfg.N, "b": cfg.b,
+         "kernel": m["kernel"], "kernel_ms": m["fused_ms"], "step_ms": m["ms_per_step"], "kept_per_step": m["n_eff"],
+         "algorithmic_bytes_per_launch": m["bytes_per_step"], "gbps": gbs, "frac": gbs / peak,
+         "frac_of_nominal_8TBps": gbs / 8000.0,
+         "value": m["units"] / (m["total_ms"] * 1e-3), "unit": UNIT, "launch": m["geo"],
+         "clocks": {k: m["clocks"].get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons")}}
+    if note:
+        e["note"] = note
+    return e
+
+
+def run_also(psync, args, wl3, stream, peak):
+    """Short (5-step) measurements of the other configs and modes, so that the driver's BENCH record carries them:
+    cfg3 in every mode and layout (reusing the headline's resident gradient sets), then cfg2 and cfg4."""
+    from dataclasses import replace
+    K, Wm = args.also_steps, 3
+    out = []
+    dev = wl3.dev
+    cfg3 = wl3.cfg
+    for mode in ("per_server", "timeout", "async"):
+        wl3.reset_state()
+        m = measure(psync, args, wl3, mode, K, Wm, stream, probe_every=1)
+        note = None
+        if mode == "async":
+            note = "Alg. 2, all W gradients one at a time in one pass; RMSProp: bound by instruction issue as well as HBM"
+        out.append(short_entry(cfg3, mode, "flat", m, peak, note))
+    for M in (1000, 20000):              # one kept row per server, many small ragged servers, flat buffers + work list
+        wlm = wl3.with_servers(psync, M)
+        wlm.reset_state()
+        m = measure(psync, args, wlm, "per_server", K, Wm, stream, probe_every=1)
+        out.append(short_entry(wlm.cfg, "per_server", "flat", m, peak, "flat buffers through the (server, tile) work list"))
+    for v in (5, 6):                     # the two rejected designs, re-measured every run (DESIGN.md s.5)
+        wl3.reset_state()
+        m = measure(psync, args, wl3, "first_n", K, Wm, stream, variant=v, probe_every=1)
+        out.append(short_entry(cfg3, "first_n", "flat", m, peak,
+                               "variant 5: cp.async.bulk + mbarrier ring" if v == 5 else "variant 6: 256-bit loads"))
+        out[-1]["variant"] = v
+    sets3 = len(wl3.tables)
+    del wl3.tables[1:], wl3.sets[1:]     # keep one flat set for the cpu_baseline leg; make room
+    torch.cuda.empty_cache()
+    # per-(worker, server) slices of cfg3, one shared kept set and one kept row per server; many small servers
+    for M, modes in ((cfg3.M, ("first_n", "per_server")), (1000, ("per_server",)), (20000, ("per_server",))):
+        cfg = cfg3 if M == cfg3.M else replace(cfg3, M=M, name=f"{cfg3.name}_M{M}")
+        wl = Workload(psync, cfg, dev, 2, layout="slices")
+        for mode in modes:
+            wl.reset_state()
+            m = measure(psync, args, wl, mode, K, Wm, stream, probe_every=1)
+            out.append(short_entry(cfg, mode, "slices", m, peak,
+                                   f"{cfg.W * cfg.M} slices per set ({wl.slices_how}), {wl.n_sets} sets"))
+        del wl
+        torch.cuda.empty_cache()
+    for cfg in (synth.INCEPTION_SGD, synth.MIXED_PRECISION):
+        wl = Workload(psync, cfg, dev, 3)
+        m = measure(psync, args, wl, "first_n", K, Wm, stream, probe_every=1)
+        out.append(short_entry(cfg, "first_n", "flat", m, peak))
+        if cfg is synth.MIXED_PRECISION:
+            wl.reset_state()
+            m = measure(psync, args, wl, "async", K, Wm, stream, probe_every=1)
+            out.append(short_entry(cfg, "async", "flat", m, peak))
+        del wl
+        torch.cuda.empty_cache()
+    return out, sets3
+
+
+def run_psync(args, cfg, rank, world, dist):
+    import paper_1702_05800_b200 as psync
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU path")
+    local = env_int("LOCAL_RANK", 0)
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    K, Wm = args.steps, args.warmup
+    mode = args.mode
+    if args.servers > 0 and args.servers != cfg.M:
+        from dataclasses import replace
+        cfg = replace(cfg, M=args.servers, name=f"{cfg.name}_M{args.servers}")
+    wl = Workload(psync, cfg, dev, args.grad_sets, layout=args.layout)
+    stream = torch.cuda.Stream(device=dev)
+    B = psync.binding
+    m = measure(psync, args, wl, mode, K, Wm, stream, dist, variant=args.variant, worklist=not args.no_worklist,
+                clip=args.clip, probe_every=args.probe_every)
+
+    units, max_ms = aggregate_over_ranks(m["units"], m["total_ms"], dist)
     value = units / (max_ms * 1e-3)
     peak, peak_src = load_peaks()
+    bytes_per_step, fused_ms, fused_list = m["bytes_per_step"], m["fused_ms"], m["fused_list"]
     achieved = bytes_per_step / (fused_ms * 1e-3) / 1e9
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": max_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if cfg.grad_dtype == synth.F32 else "f32 (bf16 gradients widened exactly)",
         "data": "synthetic",
-        "config": workload_config(cfg, extra={
-            "l2": f"no flush: each step streams {cfg.bytes_per_step / 1e9:.2f} GB (>> 126 MB L2) and gradient "
-                  f"buffers rotate over {n_sets} resident sets",
-            "grad_sets": n_sets, "launch": geo, "variant": args.variant, "mode": mode,
-            "kept_per_step": n_eff}),
+        "config": workload_config(cfg, mode, args.layout),
+        "launch": {"geometry": m["geo"], "variant": args.variant, "grad_sets": wl.n_sets,
+                   "kept_per_step": m["n_eff"], "work_list": bool(args.layout == "slices" or
+                                                                   (mode == "per_server" and not args.no_worklist))},
         "gbps_model": bytes_per_step * K * world / (max_ms * 1e-3) / 1e9,
         "params_per_s": float(cfg.P) * K * world / (max_ms * 1e-3),
-        "select_ms": select_ms, "fused_ms": fused_ms, "kernel_events_on_steps": len(fused_list),
+        "select_ms": m["select_ms"], "fused_ms": fused_ms, "kernel_events_on_steps": len(fused_list),
         "fused_ms_min_median_max": [float(np.min(fused_list)), float(np.median(fused_list)), float(np.max(fused_list))],
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "peak_source": peak_src, "kernel": "async_apply_kernel" if mode == "async" else "fused_aggregate_update_ema",
+                     "traffic": None, "peak_source": peak_src, "kernel": m["kernel"],
                      "algorithmic_bytes_per_launch": bytes_per_step,
                      "frac_of_nominal_8TBps": achieved / 8000.0},
-        "clocks": clocks,
-        "gpu_launches": 2 * K,
+        "clocks": m["clocks"],
+        "gpu_launches": m["launches_per_step"] * K,
     }
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(traffic_file) and mode == "first_n":   # dram bytes per launch from the committed ncu --set full capture
-        try:
+    if os.path.exists(traffic_file) and mode == "first_n" and args.layout == "flat" and args.variant in (0, 1):
+        try:                                  # dram bytes per launch from the committed ncu --set full capture
             with open(traffic_file) as fh:
                 out["roofline"]["traffic"] = json.load(fh).get(cfg.name)
+            out["roofline"]["traffic_source"] = ("ncu --set full capture committed in profiles/traffic.json "
+                                                 "(dram__bytes_read.sum + dram__bytes_write.sum per launch; not "
+                                                 "measured in this run)")
         except Exception:  # noqa: BLE001
             pass
 
@@ -387,6 +590,7 @@ def run_psync(args, cfg, rank, world, dist):
         dst = torch.empty_like(src)
         sink = torch.zeros(4, dtype=torch.float32, device=dev)
         pe = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        stream.wait_stream(torch.cuda.current_stream())
         for rep in range(3):                               # the first repetitions are the warm-up
             pe[0].record(stream)
             rbytes = B.psync_probe_read(src, sink, stream)
@@ -400,26 +604,114 @@ def run_psync(args, cfg, rank, world, dist):
         out["roofline"]["probe_copy_gbs"] = cbytes / (pe[1].elapsed_time(pe[2]) * 1e-3) / 1e9
         del src, dst
 
-    # free the resident gradient sets before the host-buffer (e2e) leg
-    del tables, steps_struct
+    headline = (rank == 0 and world == 1 and args.config == "cfg3" and mode == "first_n" and args.layout == "flat"
+                and args.servers <= 0)
+    if headline and not args.no_also:
+        out["also"], _ = run_also(psync, args, wl, stream, peak)
+
+    # the CPU baseline leg: the exact bytes of gradient set 0, copied D2H before any oracle timing
+    host_grads = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and args.layout == "flat":
+        if host_ram_ok(cfg):
+            host_grads = [synth.as_numpy_grad(g).copy() for g in wl.sets[0]]
+    theta, ema, s0, s1, off = wl.theta, wl.ema, wl.s0, wl.s1, wl.off
+    del wl.tables, wl.sets
     torch.cuda.empty_cache()
-    if not args.no_e2e and mode == "first_n":
+    if not args.no_e2e and mode == "first_n" and args.layout == "flat":
         out["e2e"] = run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        _, info = oracle_sample(cfg, seconds_budget=args.cpu_seconds, sample_elems=1 << 22)
-        out["cpu_baseline"] = {k: info[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        import oracle
+        if host_grads is None:               # no room in host RAM for one gradient set: bounded sample
+            sub = synth.scaled(cfg, 1 << 22, name=cfg.name)
+            _, info = oracle_full(sub, host_gradient_set(sub), seconds_budget=args.cpu_seconds)
+            info["sample"] = f"first {sub.P} of P={cfg.P} parameters of every buffer; " + info["sample"]
+        else:
+            _, info = oracle_full(cfg, host_grads, seconds_budget=args.cpu_seconds, first_step=Wm)
+            info["sample"] += "; the buffers are the GPU arm's gradient set 0, byte for byte"
+        out["cpu_baseline"] = {k: info[k] for k in ("value", "unit", "cores", "kind", "sample", "note")}
         if args.cpu_seconds_1thread > 0:       # the oracle single-threaded as well (a short sample)
-            import oracle
             threads = oracle.num_threads()
             oracle.set_num_threads(1)
             try:
-                v1, info1 = oracle_sample(cfg, seconds_budget=args.cpu_seconds_1thread, sample_elems=1 << 20,
-                                          wall_budget=20.0)
+                sub = synth.scaled(cfg, 1 << 20, name=cfg.name)
+                sub_grads = [g[:sub.P] for g in host_grads] if host_grads is not None else host_gradient_set(sub)
+                v1, info1 = oracle_full(sub, sub_grads, seconds_budget=args.cpu_seconds_1thread, wall_budget=20.0)
             finally:
                 oracle.set_num_threads(threads)
             out["cpu_baseline"]["value_1thread"] = v1
-            out["cpu_baseline"]["sample_1thread"] = info1["sample"]
+            out["cpu_baseline"]["sample_1thread"] = f"first {sub.P} parameters of every buffer; " + info1["sample"]
     return out
+
+
+def run_sweep(args, rank, world, dist):
+    """--config cfg5: BASELINE.json's bandwidth sweep -- P in {1,4,16,64,256} Mi, M in {1, 64 ragged}, (N,b) in
+    {(8,0),(16,2),(50,5),(100,10)}, fp32 gradients ~U[-1,1], SGD + EMA, 5 timed steps each after 3 warm-up steps,
+    fresh arrival times per step, gradient sets rotated whenever two fit.  One JSON line with every point; --sweep-md
+    writes the GB/s-vs-P-and-(N+b) table as markdown.  A point whose gradient set is smaller than 4x the 126 MB L2 is
+    flagged: part of it is served from L2, so it is not an HBM number."""
+    import paper_1702_05800_b200 as psync
+
+    local = env_int("LOCAL_RANK", 0)
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.Stream(device=dev)
+    peak, peak_src = load_peaks()
+    points = []
+    K, Wm = args.sweep_steps, 3
+    for cfg in synth.sweep_configs():
+        if args.sweep_filter and args.sweep_filter not in cfg.name:
+            continue
+        set_bytes = cfg.W * cfg.P * cfg.grad_bytes
+        wl = Workload(psync, cfg, dev, 3 if set_bytes < 20e9 else 2, layout=args.layout)
+        m = measure(psync, args, wl, "first_n", K, Wm, stream, dist, variant=args.variant, probe_every=1)
+        e = short_entry(cfg, "first_n", args.layout, m, peak)
+        e["grad_sets"] = wl.n_sets
+        e["gradient_set_bytes"] = set_bytes
+        e["l2"] = ("L2-resident: the whole footprint fits the 126 MB L2" if cfg.footprint_bytes <= L2_BYTES else
+                   ("partly L2-served: one gradient set is smaller than 4 x L2" if set_bytes < 4 * L2_BYTES else "HBM"))
+        points.append(e)
+        del wl
+        torch.cuda.empty_cache()
+    big = max(points, key=lambda e: e["algorithmic_bytes_per_launch"])
+    units, max_ms = aggregate_over_ranks(big["value"] * big["step_ms"] * 1e-3 * K, big["step_ms"] * K, dist)
+    out = {"metric": METRIC, "value": units / (max_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+           "ms_per_step": big["step_ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f32", "data": "synthetic",
+           "config": {"workload": f"cfg5 bandwidth sweep, {len(points)} points; value = the largest point "
+                                  f"({big['workload']})", "grad_layout": args.layout,
+                      "l2": "every point flagged: HBM / partly L2-served / L2-resident"},
+           "roofline": {"bound": "hbm", "achieved": big["gbps"], "peak": peak, "unit": "GB/s", "frac": big["frac"],
+                        "traffic": None, "peak_source": peak_src, "kernel": big["kernel"],
+                        "algorithmic_bytes_per_launch": big["algorithmic_bytes_per_launch"]},
+           "clocks": big["clocks"], "gpu_launches": 2 * K * len(points), "points": points}
+    if args.sweep_md and rank == 0:
+        write_sweep_md(args.sweep_md, points, peak, peak_src)
+    return out
+
+
+def write_sweep_md(path, points, peak, peak_src):
+    lines = ["# cfg5 bandwidth sweep: GB/s of algorithmic bytes (fused kernel, CUDA events) vs P and N+b", "",
+             "Command: `python bench.py --config cfg5 --sweep-md <this file>`; 3 warm-up + 5 timed steps per point, "
+             "gradient sets rotated.  Flags: `L2` = whole footprint fits the 126 MB L2, `~L2` = one gradient set is "
+             f"smaller than 4 x L2 (partly L2-served); unflagged points stream from HBM.  Peak: {peak} GB/s, {peak_src}.",
+             ""]
+    for M in sorted({e["M"] for e in points}):
+        lines += [f"## M = {M} {'shard' if M == 1 else 'ragged shards'}", "",
+                  "| P | " + " | ".join(f"N={N}, b={b} (N+b={N + b})" for N, b in synth.SWEEP_NB) + " |",
+                  "|---|" + "---|" * len(synth.SWEEP_NB)]
+        for P in synth.SWEEP_P:
+            row = [f"{P >> 20} Mi"]
+            for N, b in synth.SWEEP_NB:
+                e = next((x for x in points if x["M"] == M and x["P"] == P and x["N"] == N and x["b"] == b), None)
+                if e is None:
+                    row.append("—")
+                    continue
+                flag = {"L": " `L2`", "p": " `~L2`", "H": ""}[e["l2"][0]]
+                row.append(f"{e['gbps']:.0f} ({e['kernel_ms'] * 1e3:.1f} us, {100 * e['frac_of_nominal_8TBps']:.0f} %){flag}")
+            lines.append("| " + " | ".join(row) + " |")
+        lines.append("")
+    with open(path, "w") as fh:
+        fh.write("\n".join(lines))
 
 
 def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist):
@@ -475,7 +767,18 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="psync", choices=["psync", "reference"])
-    ap.add_argument("--config", default="cfg3", choices=sorted(WORKLOADS))
+    ap.add_argument("--config", default="cfg3", choices=sorted(WORKLOADS) + ["cfg5"],
+                    help="cfg5 = the bandwidth sweep (one JSON line with every point)")
+    ap.add_argument("--layout", default="flat", choices=["flat", "slices"],
+                    help="flat: W flat gradient buffers; slices: W*M separately allocated per-(worker, server) slices")
+    ap.add_argument("--servers", type=int, default=0, help="override M (ragged cut into that many servers)")
+    ap.add_argument("--no-worklist", action="store_true",
+                    help="--mode per_server with flat buffers: tiles of the flat index space instead of the work list")
+    ap.add_argument("--no-also", action="store_true", help="skip the short measurements of the other configs / modes")
+    ap.add_argument("--also-steps", type=int, default=5)
+    ap.add_argument("--sweep-steps", type=int, default=5)
+    ap.add_argument("--sweep-md", default="", help="--config cfg5: also write the table as markdown to this path")
+    ap.add_argument("--sweep-filter", default="", help="--config cfg5: only points whose name contains this")
     ap.add_argument("--mode", default="first_n", choices=["first_n", "per_server", "timeout", "async"],
                     help="first_n: the headline (one kept set); per_server: Alg. 4 per server j; timeout: L259; "
                          "async: Alg. 2, all W gradients one at a time in one pass")
@@ -495,19 +798,19 @@ def main():
     ap.add_argument("--cpu-seconds-1thread", type=float, default=3.0)
     ap.add_argument("--clock-period-ms", type=float, default=2.0)
     ap.add_argument("--probe-every", type=int, default=4)
-    ap.add_argument("--ref-sample-elems", type=int, default=0)
+    ap.add_argument("--ref-sample-elems", type=int, default=0,
+                    help="--impl reference: run on the first this-many parameters only (0 = the full workload)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "psync":
         args.warmup = 3                     # timing rule: at least 3 warm-up steps
-    cfg = WORKLOADS[args.config]
+    cfg = WORKLOADS.get(args.config, synth.PAPER_RMSPROP)
     rank, world = env_int("RANK", 0), env_int("WORLD_SIZE", 1)
 
     if args.impl == "reference":
         if rank != 0:
             return 0                        # the oracle runs on rank 0 alone
-        if args.ref_sample_elems <= 0:      # bounded sample: K steps stay within a few minutes of host time
-            elems = int((1 << 22) * min(1.0, 60.0 / max(1, args.steps + args.warmup)))
-            args.ref_sample_elems = max(1 << 14, (elems >> 14) << 14)
+        if args.ref_sample_elems <= 0 and args.steps + args.warmup > 400:
+            args.ref_sample_elems = 1 << 22  # an unusually long run: keep it within a few minutes of host time
         print(json.dumps(run_reference(args, cfg, rank)), flush=True)
         return 0
 
@@ -518,7 +821,7 @@ def main():
         dist_mod.init_process_group(backend="nccl")
         dist = dist_mod
     try:
-        out = run_psync(args, cfg, rank, world, dist)
+        out = run_sweep(args, rank, world, dist) if args.config == "cfg5" else run_psync(args, cfg, rank, world, dist)
         if rank == 0:
             print(json.dumps(out), flush=True)
     finally:

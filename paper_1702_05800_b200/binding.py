@@ -29,7 +29,7 @@ EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psyn
            "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_async_apply", "psync_step_device", "psync_clip_workspace_bytes",
            "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_launch_geometry", "psync_probe_read",
-           "psync_probe_copy")
+           "psync_probe_copy", "psync_selftest_rsqrt")
 
 
 class PsyncError(RuntimeError):
@@ -107,6 +107,8 @@ def lib() -> ctypes.CDLL:
         L.psync_probe_read.restype = ctypes.c_int
         L.psync_probe_copy.argtypes = [vp, vp, i64, vp]
         L.psync_probe_copy.restype = ctypes.c_int
+        L.psync_selftest_rsqrt.argtypes = [vp, ctypes.c_uint32, i64, vp, vp, vp]
+        L.psync_selftest_rsqrt.restype = ctypes.c_int
         _lib = L
     return _lib
 
@@ -491,5 +493,15 @@ def psync_probe_copy(d_dst: torch.Tensor, d_src: torch.Tensor, stream=None) -> i
     n = d_src.numel() * d_src.element_size() // 16
     st = lib().psync_probe_copy(_dptr(d_dst), _dptr(d_src), n, _stream(stream))
     if st != PSYNC_OK:
-        raise PsyncError(st, "psync_probe_copy")
+        raise PsyncError(st, "psync_probe_copy", "psync_selftest_rsqrt")
     return n * 32
+
+
+def psync_selftest_rsqrt(d_mismatch: torch.Tensor, n: int, first_bits: int = 0, d_x: Optional[torch.Tensor] = None,
+                         d_y: Optional[torch.Tensor] = None, stream=None) -> int:
+    """Device rsqrt_rn against __frsqrt_rn on d_x[i] or on the bit patterns first_bits + i (include/psync.h)."""
+    st = lib().psync_selftest_rsqrt(_dptr(d_x, torch.float32, "d_x"), first_bits, n, _dptr(d_y, torch.float32, "d_y"),
+                                    _dptr(d_mismatch, torch.int64, "d_mismatch"), _stream(stream))
+    if st != PSYNC_OK:
+        raise PsyncError(st, "psync_selftest_rsqrt")
+    return st

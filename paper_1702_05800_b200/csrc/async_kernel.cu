@@ -11,9 +11,14 @@
 // arithmetic is exactly K launches of the synchronous step with N=1, b=0 (bit-identical; tested),
 // but the traffic is K*sizeof(grad) + 8*(1 + n_state + [EMA]) bytes per parameter instead of
 // K*(sizeof(grad) + 8*(...)): 8.4x less for K=106 with RMSProp + EMA.
-// Unlike the synchronous step the chain of K dependent updates is real arithmetic: with RMSProp
-// (sqrt + divide per gradient element) the kernel is bound by the fp32/MUFU pipes, not by HBM;
-// with SGD / momentum it streams at the HBM roofline (DESIGN.md s.5).
+// Unlike the synchronous step the chain of K dependent updates is real arithmetic -- one optimizer
+// update per gradient LOAD.  With SGD / momentum the kernel streams at the HBM roofline; with RMSProp
+// it is bound by the FMA pipe (19 fp32 operations per element update at 128 lanes per clock per SM)
+// about as much as by HBM.  What keeps it near both limits on B200: the update runs on PAIRS of
+// elements with the packed fp32x2 instructions (FFMA2 / FMUL2: half the issue slots, same bits), the
+// step is (gamma G) * rsqrt(ms + eps) with the correctly rounded rsqrt computed by an 8-operation
+// refinement of MUFU.RSQ whose range check is a sticky flag outside the inner loop (psync_device.cuh),
+// and the loads of the next batch of gradients are in flight while the current batch is applied.
 
 #include "psync_device.cuh"
 
@@ -29,7 +34,29 @@ __device__ __forceinline__ float unit_element(const uint4& r, int e) {
   return __uint_as_float(w);
 }
 
-template <int THREADS, int U, int MINB, bool BF16, int OPT, int EMA>
+// elements 2i and 2i+1 of a 16-byte unit as one fp32x2 operand
+template <bool BF16>
+__device__ __forceinline__ float2 unit_pair(const uint4& r, int i) {
+  if (BF16) {
+    const uint32_t w = (&r.x)[i];
+    return make_float2(__uint_as_float(w << 16), __uint_as_float(w & 0xFFFF0000u));
+  }
+  return make_float2(__uint_as_float((&r.x)[2 * i]), __uint_as_float((&r.x)[2 * i + 1]));
+}
+
+// one arriving gradient (its 16-byte unit r) applied to the E parameters a thread holds, two at a time
+template <bool BF16, int OPT, int EMA, bool SCALED>
+__device__ __forceinline__ void apply_unit(const uint4& r, float scale, float gamma, float2* th, float2* em, float2* a0,
+                                           float2* a1, const PairCoeffs& c, unsigned& bad) {
+  constexpr int E = BF16 ? 8 : 4;
+  const float2 scale2 = dup2(scale), gamma2 = dup2(gamma);
+#pragma unroll
+  for (int i = 0; i < E / 2; ++i)
+    update_pair_g<OPT, EMA, SCALED>(unit_pair<BF16>(r, i), scale2, gamma2, th[i], em[i], a0[i], a1[i], c, bad);
+}
+
+// PIPE: software-pipelined batches (below); SCALED: per-worker clip factors are applied (else they are all 1)
+template <int THREADS, int U, int MINB, bool PIPE, bool BF16, int OPT, int EMA, bool SCALED>
 __global__ void __launch_bounds__(THREADS, MINB) async_apply_kernel(const FusedParams p) {
   constexpr int E = BF16 ? 8 : 4;
   constexpr int Q = E / 4;
@@ -55,6 +82,7 @@ __global__ void __launch_bounds__(THREADS, MINB) async_apply_kernel(const FusedP
   }
   const bool vec_ok = (__syncthreads_or(static_cast<int>(misalign)) == 0) && (p.base_aligned != 0);
 
+  const PairCoeffs pc = make_pair_coeffs(p);
   const int64_t n_units = vec_ok ? p.P / E : 0;
   for (int64_t u = static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x; u < n_units;
        u += static_cast<int64_t>(gridDim.x) * THREADS) {
@@ -67,30 +95,74 @@ __global__ void __launch_bounds__(THREADS, MINB) async_apply_kernel(const FusedP
       if (OPT != OPT_SGD) a04[q] = ld_state16(p.s0 + e);
       if (OPT == OPT_RMSPROP_MOM) a14[q] = ld_state16(p.s1 + e);
     }
-    float* th = reinterpret_cast<float*>(th4);
-    float* em = reinterpret_cast<float*>(em4);
-    float* a0 = reinterpret_cast<float*>(a04);
-    float* a1 = reinterpret_cast<float*>(a14);
+    float2* th = reinterpret_cast<float2*>(th4);
+    float2* em = reinterpret_cast<float2*>(em4);
+    float2* a0 = reinterpret_cast<float2*>(a04);
+    float2* a1 = reinterpret_cast<float2*>(a14);
 
-    int i = 0;
-    for (; i + U <= K; i += U) {  // U independent 16-byte loads in flight, then U dependent updates
-      uint4 r[U];
+    unsigned bad = 0;  // RMSProp: did any ms + eps leave the range of the unchecked packed rsqrt?
+    if (PIPE) {
+      // Software-pipelined over batches of U gradients: the loads of batch b+1 are in flight while the U dependent
+      // updates of batch b run (the updates are real arithmetic here -- with RMSProp the FMA pipe, not HBM, is the
+      // limit -- so a warp that only started its next loads after its updates left both idle in turn).
+      const int n_batches = K / U;
+      uint4 cur[U], nxt[U];
+      if (n_batches > 0) {
 #pragma unroll
-      for (int v = 0; v < U; ++v) r[v] = ldg_stream16(s_ptr[i + v] + u * 16);
+        for (int v = 0; v < U; ++v) cur[v] = ldg_stream16(s_ptr[v] + u * 16);
+      }
+      for (int b = 0; b < n_batches; ++b) {
+        const int i = b * U;
+        if (b + 1 < n_batches) {
 #pragma unroll
-      for (int v = 0; v < U; ++v) {
-        const float gamma = s_gamma[i + v], scale = s_scale[i + v];
+          for (int v = 0; v < U; ++v) nxt[v] = ldg_stream16(s_ptr[i + U + v] + u * 16);
+        }
 #pragma unroll
-        for (int e = 0; e < E; ++e)
-          update_element_g<OPT, EMA>(unit_element<BF16>(r[v], e), scale, gamma, th[e], em[e], a0[e], a1[e], p);
+        for (int v = 0; v < U; ++v)
+          apply_unit<BF16, OPT, EMA, SCALED>(cur[v], s_scale[i + v], s_gamma[i + v], th, em, a0, a1, pc, bad);
+#pragma unroll
+        for (int v = 0; v < U; ++v) cur[v] = nxt[v];
+      }
+      for (int i = n_batches * U; i < K; ++i) {
+        const uint4 r = ldg_stream16(s_ptr[i] + u * 16);
+        apply_unit<BF16, OPT, EMA, SCALED>(r, s_scale[i], s_gamma[i], th, em, a0, a1, pc, bad);
+      }
+    } else {
+      int i = 0;
+      for (; i + U <= K; i += U) {  // U independent 16-byte loads in flight, then U dependent updates
+        uint4 r[U];
+#pragma unroll
+        for (int v = 0; v < U; ++v) r[v] = ldg_stream16(s_ptr[i + v] + u * 16);
+#pragma unroll
+        for (int v = 0; v < U; ++v)
+          apply_unit<BF16, OPT, EMA, SCALED>(r[v], s_scale[i + v], s_gamma[i + v], th, em, a0, a1, pc, bad);
+      }
+      for (; i < K; ++i) {
+        const uint4 r = ldg_stream16(s_ptr[i] + u * 16);
+        apply_unit<BF16, OPT, EMA, SCALED>(r, s_scale[i], s_gamma[i], th, em, a0, a1, pc, bad);
       }
     }
-    for (; i < K; ++i) {
-      const uint4 r = ldg_stream16(s_ptr[i] + u * 16);
-      const float gamma = s_gamma[i], scale = s_scale[i];
+    if (OPT == OPT_RMSPROP_MOM && rsqrt_pair_left_range(bad)) {
+      // Never on sane data: a non-finite or absurd second moment.  Nothing has been stored yet, so redo this unit from
+      // memory with the checked scalar update (IEEE special values propagate as the definition says).
 #pragma unroll
-      for (int e = 0; e < E; ++e)
-        update_element_g<OPT, EMA>(unit_element<BF16>(r, e), scale, gamma, th[e], em[e], a0[e], a1[e], p);
+      for (int q = 0; q < Q; ++q) {
+        const int64_t e = u * E + 4 * q;
+        th4[q] = ld_state16(p.theta + e);
+        if (EMA != EMA_OFF) em4[q] = ld_state16(p.ema + e);
+        a04[q] = ld_state16(p.s0 + e);
+        a14[q] = ld_state16(p.s1 + e);
+      }
+      float* ths = reinterpret_cast<float*>(th4);
+      float* ems = reinterpret_cast<float*>(em4);
+      float* a0s = reinterpret_cast<float*>(a04);
+      float* a1s = reinterpret_cast<float*>(a14);
+      for (int n = 0; n < K; ++n) {
+        const uint4 r = ldg_stream16(s_ptr[n] + u * 16);
+#pragma unroll
+        for (int e = 0; e < E; ++e)
+          update_element_g<OPT, EMA>(unit_element<BF16>(r, e), s_scale[n], s_gamma[n], ths[e], ems[e], a0s[e], a1s[e], p);
+      }
     }
 
 #pragma unroll
@@ -156,32 +228,39 @@ __global__ void __launch_bounds__(1024) order_by_arrival_kernel(const float* __r
 
 struct AsyncShape {
   int threads, unroll, minb;
+  bool pipe;
 };
-// {threads, loads in flight per thread, CTAs per SM}, measured on B200 over 12 shapes (DESIGN.md s.5): the K
-// dependent updates want occupancy more than deep load batches -- 4 CTAs/SM for fp32 (64 registers), and for RMSProp
-// (issue-bound) 4 loads in flight instead of 8; bf16 holds 8 parameters per thread, so 3 CTAs/SM (2 with RMSProp).
+// {threads, gradients per batch, CTAs per SM, software-pipelined}, measured on B200 (profiles/r2_async.md).  fp32: two
+// batches live (one applied, one in flight), 64 registers, 4 CTAs/SM; for RMSProp (FMA-pipe-bound) batches of 3 were the
+// best of nine shapes (cfg3 shape: 1.83 ms; batches of 2: 1.95, 4 at 3 CTAs/SM: 2.13, 8 unpipelined: 2.23).  bf16 holds
+// 8 parameters per thread: one batch of 8 loads, 3 CTAs/SM (RMSProp: pipelined short batches, 2 CTAs/SM).
 constexpr AsyncShape shape_for(bool bf16, int opt) {
-  return bf16 ? (opt == OPT_RMSPROP_MOM ? AsyncShape{256, 8, 2} : AsyncShape{256, 8, 3})
-              : (opt == OPT_RMSPROP_MOM ? AsyncShape{256, 4, 4} : AsyncShape{256, 8, 4});
+  return bf16 ? (opt == OPT_RMSPROP_MOM ? AsyncShape{256, 2, 2, true} : AsyncShape{256, 8, 3, false})
+              : (opt == OPT_RMSPROP_MOM ? AsyncShape{256, 3, 4, true} : AsyncShape{256, 4, 4, true});
 }
 
 using KernelFn = void (*)(const FusedParams);
 
-template <bool BF16, int OPT>
-KernelFn pick_ema(int ema) {
+template <bool BF16, int OPT, int EMA>
+KernelFn pick_scaled(bool scaled) {
   constexpr AsyncShape S = shape_for(BF16, OPT);
+  return scaled ? async_apply_kernel<S.threads, S.unroll, S.minb, S.pipe, BF16, OPT, EMA, true>
+                : async_apply_kernel<S.threads, S.unroll, S.minb, S.pipe, BF16, OPT, EMA, false>;
+}
+template <bool BF16, int OPT>
+KernelFn pick_ema(int ema, bool scaled) {
   switch (ema) {
-    case EMA_POST: return async_apply_kernel<S.threads, S.unroll, S.minb, BF16, OPT, EMA_POST>;
-    case EMA_PRE: return async_apply_kernel<S.threads, S.unroll, S.minb, BF16, OPT, EMA_PRE>;
-    default: return async_apply_kernel<S.threads, S.unroll, S.minb, BF16, OPT, EMA_OFF>;
+    case EMA_POST: return pick_scaled<BF16, OPT, EMA_POST>(scaled);
+    case EMA_PRE: return pick_scaled<BF16, OPT, EMA_PRE>(scaled);
+    default: return pick_scaled<BF16, OPT, EMA_OFF>(scaled);
   }
 }
 template <bool BF16>
-KernelFn pick_opt(int opt, int ema) {
+KernelFn pick_opt(int opt, int ema, bool scaled) {
   switch (opt) {
-    case OPT_SGD: return pick_ema<BF16, OPT_SGD>(ema);
-    case OPT_MOMENTUM: return pick_ema<BF16, OPT_MOMENTUM>(ema);
-    default: return pick_ema<BF16, OPT_RMSPROP_MOM>(ema);
+    case OPT_SGD: return pick_ema<BF16, OPT_SGD>(ema, scaled);
+    case OPT_MOMENTUM: return pick_ema<BF16, OPT_MOMENTUM>(ema, scaled);
+    default: return pick_ema<BF16, OPT_RMSPROP_MOM>(ema, scaled);
   }
 }
 
@@ -212,7 +291,8 @@ cudaError_t launch_async_apply(const FusedParams& p, int dtype, int opt, int ema
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, dtype == 1 ? pick_opt<true>(opt, ema) : pick_opt<false>(opt, ema), p);
+  const bool scaled = p.gscales != nullptr;
+  return cudaLaunchKernelEx(&cfg, dtype == 1 ? pick_opt<true>(opt, ema, scaled) : pick_opt<false>(opt, ema, scaled), p);
 }
 
 cudaError_t launch_order_by_arrival(const float* d_arrival, int32_t W, int32_t* d_order, int32_t* d_n_arrived,

@@ -337,6 +337,15 @@ PSYNC_API int psync_probe_copy(void* d_dst, const void* d_src, int64_t n_vec16, 
                                                                                                             : PSYNC_ECUDA;
 }
 
+PSYNC_API int psync_selftest_rsqrt(const float* d_x, uint32_t first_bits, int64_t n, float* d_y,
+                         unsigned long long* d_mismatch, void* stream) {
+  if (n < 0 || d_mismatch == nullptr) return PSYNC_EINVAL;
+  return psync::launch_selftest_rsqrt(d_x, first_bits, n, d_y, d_mismatch, static_cast<cudaStream_t>(stream)) ==
+                 cudaSuccess
+             ? PSYNC_OK
+             : PSYNC_ECUDA;
+}
+
 PSYNC_API size_t psync_step_host_workspace_bytes(int32_t N, int32_t W, int32_t grad_dtype, int64_t chunk_elems) {
   HostLayout L;
   if (!host_layout(N, W, grad_dtype, chunk_elems, &L)) return 0;

@@ -13,12 +13,16 @@
 // straddles two servers, so every CTA stages ONE kept row and streams with 128-bit loads.
 //
 // Alignment (hard part 3): the 128-bit stream is aligned to the GRADIENT slices -- they are 96 % of the bytes.
-// The first kept worker's slice base fixes a head peel h < E elements; units are [h + uE, h + (u+1)E) of the
-// slice.  A kept worker whose base has another phase is read with narrower loads (that worker only); the
-// head/tail peel (< 2E elements per server) is done element by element by the server's first CTA.  theta /
-// state / ema start at element off[j] + h of flat arrays, which for ragged cuts is NOT 16-byte aligned in
-// general: then the sums are transposed through shared memory and theta / state / ema are read and written
-// with coalesced 32-bit accesses (thread t <-> element t, t + 256, ...), so they still move every byte once.
+// The first kept worker's slice base fixes a head peel h: the elements before its first 128-byte boundary
+// (< 32 fp32 / < 64 bf16), so that every warp-level 512-byte request covers exactly four 128-byte lines (a tile that
+// starts on a 16-byte but not a 128-byte boundary costs 12 % more L2 sector traffic and 1.5 % of the kernel: ncu,
+// profiles/r2_sharded.md); units are [h + uE, h + (u+1)E) of the slice.  A kept worker whose base has another
+// 16-byte phase is read with narrower loads (that worker only); the head/tail peel is done element by element by the
+// server's first CTA.  theta / state / ema start at element off[j] + h of flat arrays, which for ragged cuts is NOT
+// 16-byte aligned in general: then each WARP transposes its 32 sums through shared memory (no CTA barrier: a
+// __syncthreads here cost 3 % -- every warp waited for the CTA's slowest gradient load) and theta / state / ema are
+// read and written as coalesced 32-bit accesses (lane l <-> elements l, l + 32, ... of the warp's 128- or 256-element
+// segment), so they still move every byte once.
 // The arithmetic per element is exactly K2's (same fixed-order fp32 sum, same update_element): bit-identical.
 
 #include "psync_device.cuh"
@@ -95,15 +99,15 @@ __global__ void __launch_bounds__(kThreads, MINB) sharded_aggregate_update_ema(c
     const char* g = p.slices ? static_cast<const char*>(p.grads[static_cast<int64_t>(k) * p.M + j])
                              : static_cast<const char*>(p.grads[k]) + off_j * ESZ;
     s_ptr[i] = g;
-    if (i == 0) s_ref = static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 15u;
+    if (i == 0) s_ref = static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 127u;
   }
   __syncthreads();
   const unsigned ref = s_ref;
-  const int h = static_cast<int>(((16u - ref) & 15u) / ESZ);  // head peel: elements before the first 16-byte boundary
+  const int h = static_cast<int>(((128u - ref) & 127u) / ESZ);  // head peel: elements before the first 128-byte line
   unsigned mis = 0;
   for (int i = threadIdx.x; i < N; i += kThreads) {
     const char* g = s_ptr[i];
-    mis |= (static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 15u) ^ ref;
+    mis |= ((static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) ^ ref) & 15u);  // another 16-byte phase
     s_ptr[i] = g + h * ESZ;  // unit u of this worker = s_ptr[i] + 16 u
   }
   const bool mixed = __syncthreads_or(static_cast<int>(mis)) != 0;  // some kept worker has another phase
@@ -177,36 +181,41 @@ __global__ void __launch_bounds__(kThreads, MINB) sharded_aggregate_update_ema(c
         }
       }
     } else {
-      // theta's slice is not co-aligned with the gradient units: transpose the sums through shared memory so that
-      // thread t owns elements t, t + 256, ... of the tile and theta / state / ema move as coalesced 32-bit accesses.
+      // theta's slice is not co-aligned with the gradient units: every warp transposes its own 32 units through
+      // shared memory (__syncwarp only), so that lane l owns elements l, l + 32, ... of the warp's segment and
+      // theta / state / ema move as coalesced 32-bit accesses.
+      constexpr int SEG = 32 * E;  // elements per warp
+      const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+      float* seg = s_acc + warp * SEG;
 #pragma unroll
       for (int q = 0; q < Q; ++q)
-        *reinterpret_cast<float4*>(&s_acc[(threadIdx.x * Q + q) * 4]) =
+        *reinterpret_cast<float4*>(&seg[(lane * Q + q) * 4]) =
             make_float4(acc[4 * q], acc[4 * q + 1], acc[4 * q + 2], acc[4 * q + 3]);
-      __syncthreads();
-      const int64_t tile_e0 = e0 + u0 * E;
-      const int live_elems = static_cast<int>(live_units) * E;
+      __syncwarp();
+      const int64_t seg_e0 = e0 + (u0 + warp * 32) * E;                       // parameter index of the segment
+      const int64_t live_in_seg = (live_units - warp * 32) * E;               // may be <= 0 (dead warp) or > SEG
       float th[E], em[E], a0[E], a1[E], S[E];
 #pragma unroll
       for (int q = 0; q < E; ++q) {
-        const int idx = q * kThreads + threadIdx.x;
-        const int64_t e = tile_e0 + (idx < live_elems ? idx : 0);
-        S[q] = s_acc[idx];
-        th[q] = p.theta[e];
-        if (EMA != EMA_OFF) em[q] = p.ema[e];
-        if (OPT != OPT_SGD) a0[q] = p.s0[e];
-        if (OPT == OPT_RMSPROP_MOM) a1[q] = p.s1[e];
+        const int idx = q * 32 + lane;
+        const int64_t e = seg_e0 + (idx < live_in_seg ? idx : 0);
+        const bool on = live_in_seg > 0;                                     // a dead warp must not touch memory
+        S[q] = seg[idx];
+        th[q] = on ? ld_state32(p.theta + e) : 0.f;
+        if (EMA != EMA_OFF) em[q] = on ? ld_state32(p.ema + e) : 0.f;
+        if (OPT != OPT_SGD) a0[q] = on ? ld_state32(p.s0 + e) : 1.f;
+        if (OPT == OPT_RMSPROP_MOM) a1[q] = on ? ld_state32(p.s1 + e) : 0.f;
       }
 #pragma unroll
       for (int q = 0; q < E; ++q) {
-        const int idx = q * kThreads + threadIdx.x;
+        const int idx = q * 32 + lane;
         update_element<OPT, EMA>(S[q], inv_N, th[q], em[q], a0[q], a1[q], p);
-        if (idx < live_elems) {
-          const int64_t e = tile_e0 + idx;
-          p.theta[e] = th[q];
-          if (EMA != EMA_OFF) p.ema[e] = em[q];
-          if (OPT != OPT_SGD) p.s0[e] = a0[q];
-          if (OPT == OPT_RMSPROP_MOM) p.s1[e] = a1[q];
+        if (idx < live_in_seg) {
+          const int64_t e = seg_e0 + idx;
+          st_state32(p.theta + e, th[q]);
+          if (EMA != EMA_OFF) st_state32(p.ema + e, em[q]);
+          if (OPT != OPT_SGD) st_state32(p.s0 + e, a0[q]);
+          if (OPT == OPT_RMSPROP_MOM) st_state32(p.s1 + e, a1[q]);
         }
       }
     }

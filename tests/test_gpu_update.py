@@ -327,3 +327,30 @@ def test_guard_bands_no_out_of_bounds_access(dtype, P, pad):
         assert bool((raw[:pad] == SENT).all()) and bool((raw[pad + P:] == SENT).all()), "write outside the array"
     for raw in grads_raw:
         assert bool(torch.isnan(raw[:pad].float()).all()) and bool(torch.isnan(raw[pad + P:].float()).all())
+
+
+def test_device_rsqrt_rn_equals_frsqrt_rn_exhaustively_and_the_mirror_on_a_sample():
+    """The RMSProp step's RN(1/sqrt(x)) (reading R10): the device routine (refinement of __frsqrt_rn without range
+    reduction inside [2^-60, 2^60), __frsqrt_rn outside) against __frsqrt_rn on EVERY fp32 bit pattern of the fast range
+    and on the rest of the positive floats by stride, and against the CPU mirror's correctly rounded rsqrt (pinned by
+    exact arithmetic in tests/test_oracle_fp32_mirror.py) on a random sample."""
+    from paper_1702_05800_b200 import binding as B
+    bad = torch.zeros(1, dtype=torch.int64, device=DEV)
+    lo, hi = 0x21800000, 0x5D800000                      # 2^-60 ... 2^60: every bit pattern (1.0e9 inputs)
+    B.psync_selftest_rsqrt(bad, hi - lo, first_bits=lo)
+    B.psync_selftest_rsqrt(bad, 1 << 16, first_bits=lo - (1 << 15))          # across the lower edge
+    B.psync_selftest_rsqrt(bad, 1 << 16, first_bits=hi - (1 << 15))          # across the upper edge
+    B.psync_selftest_rsqrt(bad, 1 << 24, first_bits=0)                       # zero, denormals, tiny normals
+    B.psync_selftest_rsqrt(bad, 1 << 24, first_bits=0x7F000000)              # huge, +inf, NaNs
+    B.psync_selftest_rsqrt(bad, 1 << 20, first_bits=0x80000000)              # -0 and negatives
+    torch.cuda.synchronize()
+    assert int(bad.item()) == 0
+    rng = np.random.default_rng(9)
+    x = np.concatenate([np.exp(rng.uniform(np.log(1e-30), np.log(1e30), 200_000)),
+                        rng.uniform(0.9, 1.2, 100_000)]).astype(np.float32)
+    d_y = torch.empty(x.size, dtype=torch.float32, device=DEV)
+    B.psync_selftest_rsqrt(bad, x.size, d_x=torch.from_numpy(x).to(DEV), d_y=d_y)
+    torch.cuda.synchronize()
+    fn = oracle.mirror_lib().mirror_rsqrt_rn
+    want = np.array([fn(float(v)) for v in x], dtype=np.float32)
+    assert int(bad.item()) == 0 and np.array_equal(d_y.cpu().numpy().view(np.uint32), want.view(np.uint32))
