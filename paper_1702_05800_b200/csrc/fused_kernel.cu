@@ -87,8 +87,32 @@ __device__ __forceinline__ void vector_tile(const FusedParams& p, const char* co
 #pragma unroll
     for (int e = 0; e < E; ++e) acc[j][e] = 0.f;
 
+  // HOIST: with at most two fp32 state arrays (SGD, or momentum without EMA) the theta / ema loads fit in registers
+  // next to the last batch of gradient loads, so they are issued WITH it instead of after it: one memory round trip
+  // less per CTA.  Nothing for N = 100 (other CTAs cover it), but a CTA with N = 8 lives for four round trips
+  // (kept -> pointers -> gradients -> theta) and the small sweep points are latency-bound: a small gain there (P = 1 Mi,
+  // N = 8: 3072 -> 3283 GB/s; 4 Mi, N = 8: 6133 -> 6190; profiles/r2_small_points.md).  Same loads, same adds in the same
+  // order: same bits.
+  constexpr int kStateArrays = 1 + (EMA != EMA_OFF ? 1 : 0) + (OPT != OPT_SGD ? 1 : 0) + (OPT == OPT_RMSPROP_MOM ? 1 : 0);
+  constexpr bool HOIST = !BF16 && UPT == 1 && kStateArrays <= 2;
+  float4 th[UPT][Q], em[UPT][Q], a0[UPT][Q], a1[UPT][Q];
+  auto load_state = [&]() {
+#pragma unroll
+    for (int j = 0; j < UPT; ++j) {
+#pragma unroll
+      for (int q = 0; q < Q; ++q) {
+        const int64_t e = unit[j] * E + 4 * q;
+        th[j][q] = ld_state16(p.theta + e);
+        if (EMA != EMA_OFF) em[j][q] = ld_state16(p.ema + e);
+        if (OPT != OPT_SGD) a0[j][q] = ld_state16(p.s0 + e);
+        if (OPT == OPT_RMSPROP_MOM) a1[j][q] = ld_state16(p.s1 + e);
+      }
+    }
+  };
+
   int n = 0;
-  for (; n + U <= N; n += U) {  // full batches: U x UPT independent 16-byte loads in flight
+  const int n_loop = HOIST ? ((N - 1) / U) * U : (N / U) * U;  // HOIST keeps 1..U gradients for the final batch
+  for (; n < n_loop; n += U) {  // full batches: U x UPT independent 16-byte loads in flight
     uint4 r[U][UPT];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
@@ -101,7 +125,7 @@ __device__ __forceinline__ void vector_tile(const FusedParams& p, const char* co
 #pragma unroll
       for (int j = 0; j < UPT; ++j) accumulate_unit<BF16>(acc[j], r[u][j]);
   }
-  if (n < N) {  // last, partial batch: same shape, predicated
+  if (HOIST || n < N) {  // last batch (partial unless HOIST and U divides N): same shape, predicated
     uint4 r[U][UPT];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
@@ -110,6 +134,7 @@ __device__ __forceinline__ void vector_tile(const FusedParams& p, const char* co
 #pragma unroll
       for (int j = 0; j < UPT; ++j) r[u][j] = on ? ldg_stream16(g + unit[j] * 16) : make_uint4(0u, 0u, 0u, 0u);
     }
+    if (HOIST) load_state();
 #pragma unroll
     for (int u = 0; u < U; ++u)
       if ((n + u) < N) {
@@ -119,18 +144,7 @@ __device__ __forceinline__ void vector_tile(const FusedParams& p, const char* co
   }
 
   // theta / state / ema: loaded once the gradient registers are dead; other resident warps hide the latency
-  float4 th[UPT][Q], em[UPT][Q], a0[UPT][Q], a1[UPT][Q];
-#pragma unroll
-  for (int j = 0; j < UPT; ++j) {
-#pragma unroll
-    for (int q = 0; q < Q; ++q) {
-      const int64_t e = unit[j] * E + 4 * q;
-      th[j][q] = ld_state16(p.theta + e);
-      if (EMA != EMA_OFF) em[j][q] = ld_state16(p.ema + e);
-      if (OPT != OPT_SGD) a0[j][q] = ld_state16(p.s0 + e);
-      if (OPT == OPT_RMSPROP_MOM) a1[j][q] = ld_state16(p.s1 + e);
-    }
-  }
+  if (!HOIST) load_state();
 
 #pragma unroll
   for (int j = 0; j < UPT; ++j) {
