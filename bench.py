@@ -738,15 +738,16 @@ def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist):
                                  ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho,
                                  eps=cfg.eps, grid_ctas=args.grid_ctas, variant=args.variant)
     arrivals = [synth.arrival_times(cfg, 2000 + s) for s in range(K + 1)]
+    ctx = psync.HostCtx()               # the copy stream and events, created once for the loop
     psync.psync_step_host(step, arrivals[K], h_grads, d_work, h_theta_out=h_theta, h_kept=h_kept, chunk_elems=chunk,
-                          stream=stream)                                   # warm-up
+                          stream=stream, ctx=ctx)                          # warm-up
     if dist is not None and dist.is_initialized():
         dist.barrier()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for s in range(K):
         st, _ = psync.psync_step_host(step, arrivals[s], h_grads, d_work, h_theta_out=h_theta, h_kept=h_kept,
-                                      chunk_elems=chunk, stream=stream)
+                                      chunk_elems=chunk, stream=stream, ctx=ctx)
         assert st == 0
     torch.cuda.synchronize()
     ms = (time.perf_counter() - t0) * 1e3

@@ -82,6 +82,8 @@ def lib() -> ctypes.CDLL:
         L.oracle_aggregate_update_rows.restype = ctypes.c_int
         L.oracle_aggregate_update_slices.argtypes = L.oracle_aggregate_update_rows.argtypes
         L.oracle_aggregate_update_slices.restype = ctypes.c_int
+        L.oracle_staleness.argtypes = [vp, i32, vp, i32, i64, i32, vp, vp, vp]
+        L.oracle_staleness.restype = ctypes.c_int
         L.oracle_order_by_arrival.argtypes = [vp, i32, vp, vp]
         L.oracle_order_by_arrival.restype = ctypes.c_int
         L.oracle_async_apply.argtypes = [i64, i32, vp, i32, i32, vp, ctypes.c_int, vp, vp, vp, vp, vp, vp, vp,
@@ -306,6 +308,21 @@ def order_by_arrival(arrival):
     if st != OK:
         raise ValueError("oracle_order_by_arrival: invalid arguments")
     return order[:int(n[0])].copy()
+
+
+def staleness(read_iter, order, t0, lag=0):
+    """Staleness of the gradients Alg. 2 applies (Table 1) -> (status, staleness int64 [K],
+    read_iter_out int64 [W], stats float64 [6] = min, mean, median, max, std, count)."""
+    W, K = read_iter.size, order.size
+    _chk(read_iter, np.int64, "read_iter", W)
+    _chk(order, np.int32, "order", K)
+    st = np.zeros(K, np.int64)
+    nxt = np.zeros(W, np.int64)
+    stats = np.zeros(6, np.float64)
+    rc = lib().oracle_staleness(_ptr(read_iter), W, _ptr(order), K, t0, lag, _ptr(st), _ptr(nxt), _ptr(stats))
+    if rc != OK:
+        return rc, None, None, None
+    return rc, st, nxt, stats
 
 
 def kth_arrival_stats(arrival, iters=None):

@@ -31,7 +31,8 @@
 // time-out rule (tests/test_oracle_per_server.py), Alg. 2 (tests/test_oracle_async.py), learning-rate
 // schedule and clip factors (tests/test_oracle_helpers.py), straggler statistics and the Fig. 5
 // interpolation, the latter against the two values the paper prints (tests/test_oracle_stragglers.py);
-// the per-(worker, server) slice layout (tests/test_oracle_slices.py).
+// the per-(worker, server) slice layout (tests/test_oracle_slices.py); the staleness bookkeeping of Alg. 2
+// (tests/test_oracle_staleness.py).
 // (The fp32 diagnostic mirror of the GPU's operation list is a SEPARATE library, oracle/psync_mirror_f32.cpp;
 // nothing of it is in this file.)
 // Nothing here is "parity unpinned".
@@ -461,6 +462,65 @@ int oracle_async_apply(int64_t P, int32_t M, const int64_t* shard_off, int32_t K
         apply_element(grad_at(G, grad_dtype, e), c, opt, ema_mode, theta, ema, state0, state1, e);
     }
   }
+  return ORACLE_OK;
+}
+
+// =============================================================================================
+// Staleness of the gradients Alg. 2 applies (NEXT-3, remainder): "Staleness of a gradient is measured as the
+// number of updates that have occurred between its corresponding read and update operations" (Table 1,
+// PAPER.md:L103-110).  The server counts its updates t = 0, 1, ... (Alg. 2's loop variable, L84).  Worker k
+// read theta when the counter stood at read_iter[k] (Alg. 1 l.2, L64); the gradient it computed from that
+// copy is the i-th one the server applies in this batch, as update number t0 + lag + i, so
+//     staleness_i = (t0 + lag + i) - read_iter[order[i]]
+// updates were applied in between.  `lag` >= 0 is the fixed-lag simulation of section 2.1 (L114: "simulated
+// staleness by using old gradients for the parameter updates"): every gradient waits `lag` further updates
+// before it is applied, which adds exactly `lag` to its staleness.  After its gradient has been applied the
+// worker reads again (Alg. 1 is a loop: send, then read, L62-75): read_iter_out[k] = t0 + lag + i + 1, the counter
+// right after its own update; workers not in `order` keep their value.
+//   read_iter[W] int64 (>= 0, <= the update index it is compared with, else EINVAL: a gradient cannot be
+//   computed from parameters that do not exist yet);  order[K] distinct worker indices;  t0 >= 0
+//   staleness[K] int64 OUT;  read_iter_out[W] int64 OUT (may alias read_iter);
+//   stats[6] double OUT: min, mean, median, max, standard deviation (population: divide by K), count --
+//   the columns of Table 1.  K = 0: stats = NaN, NaN, NaN, NaN, NaN, 0.
+// =============================================================================================
+int oracle_staleness(const int64_t* read_iter, int32_t W, const int32_t* order, int32_t K, int64_t t0, int32_t lag,
+                     int64_t* staleness, int64_t* read_iter_out, double* stats) {
+  if (!read_iter || !order || !staleness || !read_iter_out || !stats || W < 1 || K < 0 || K > W || t0 < 0 || lag < 0)
+    return ORACLE_EINVAL;
+  std::vector<char> seen(W, 0);
+  for (int32_t i = 0; i < K; ++i) {
+    const int32_t k = order[i];
+    if (k < 0 || k >= W || seen[k]) return ORACLE_EINVAL;
+    seen[k] = 1;
+    if (read_iter[k] < 0 || read_iter[k] > t0 + lag + i) return ORACLE_EINVAL;
+  }
+  std::vector<int64_t> next(read_iter, read_iter + W);
+  for (int32_t i = 0; i < K; ++i) {  // the i-th gradient to arrive is update number t0 + lag + i
+    const int64_t applied_as = t0 + lag + i;
+    staleness[i] = applied_as - read_iter[order[i]];
+    next[order[i]] = applied_as + 1;  // the worker's next read sees its own update
+  }
+  for (int32_t k = 0; k < W; ++k) read_iter_out[k] = next[k];
+  const double nan = std::numeric_limits<double>::quiet_NaN();
+  if (K == 0) {
+    stats[0] = stats[1] = stats[2] = stats[3] = stats[4] = nan;
+    stats[5] = 0.0;
+    return ORACLE_OK;
+  }
+  std::vector<int64_t> sorted(staleness, staleness + K);
+  std::sort(sorted.begin(), sorted.end());
+  double sum = 0.0;
+  for (int32_t i = 0; i < K; ++i) sum += static_cast<double>(staleness[i]);
+  const double mean = sum / K;
+  double ss = 0.0;
+  for (int32_t i = 0; i < K; ++i) ss += (static_cast<double>(staleness[i]) - mean) * (static_cast<double>(staleness[i]) - mean);
+  stats[0] = static_cast<double>(sorted.front());
+  stats[1] = mean;
+  stats[2] = (K % 2) ? static_cast<double>(sorted[K / 2])
+                     : 0.5 * (static_cast<double>(sorted[K / 2 - 1]) + static_cast<double>(sorted[K / 2]));
+  stats[3] = static_cast<double>(sorted.back());
+  stats[4] = std::sqrt(ss / K);
+  stats[5] = static_cast<double>(K);
   return ORACLE_OK;
 }
 

@@ -28,7 +28,8 @@ PSYNC_TILE_UNITS = 256
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
            "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_async_apply", "psync_step_device", "psync_clip_workspace_bytes",
            "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
-           "psync_step_host_workspace_bytes", "psync_step_host", "psync_launch_geometry", "psync_probe_read",
+           "psync_step_host_workspace_bytes", "psync_step_host", "psync_host_ctx_create", "psync_host_ctx_destroy",
+           "psync_step_host_ctx", "psync_launch_geometry", "psync_probe_read",
            "psync_probe_copy", "psync_selftest_rsqrt")
 
 
@@ -101,6 +102,13 @@ def lib() -> ctypes.CDLL:
         L.psync_step_host.argtypes = [ctypes.POINTER(psync_step), vp, vp, i32, vp, vp, vp, vp, vp, ctypes.c_size_t,
                                       i64, vp]
         L.psync_step_host.restype = ctypes.c_int
+        L.psync_host_ctx_create.argtypes = [ctypes.POINTER(ctypes.c_void_p)]
+        L.psync_host_ctx_create.restype = ctypes.c_int
+        L.psync_host_ctx_destroy.argtypes = [vp]
+        L.psync_host_ctx_destroy.restype = ctypes.c_int
+        L.psync_step_host_ctx.argtypes = [vp, ctypes.POINTER(psync_step), vp, vp, i32, vp, vp, vp, vp, vp,
+                                          ctypes.c_size_t, i64, vp]
+        L.psync_step_host_ctx.restype = ctypes.c_int
         L.psync_launch_geometry.argtypes = [ctypes.POINTER(psync_step), vp, vp, vp, vp]
         L.psync_launch_geometry.restype = ctypes.c_int
         L.psync_probe_read.argtypes = [vp, i64, vp, vp]
@@ -448,10 +456,32 @@ def psync_step_host_workspace_bytes(N: int, W: int, grad_dtype: int, chunk_elems
     return lib().psync_step_host_workspace_bytes(N, W, grad_dtype, chunk_elems)
 
 
+class HostCtx:
+    """Copy stream + events of the host-buffer step, created once (include/psync.h: psync_host_ctx_create)."""
+
+    def __init__(self):
+        h = ctypes.c_void_p()
+        st = lib().psync_host_ctx_create(ctypes.byref(h))
+        if st != PSYNC_OK:
+            raise PsyncError(st, "psync_host_ctx_create")
+        self.handle = h
+
+    def close(self):
+        if self.handle is not None:
+            lib().psync_host_ctx_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:  # noqa: BLE001
+            pass
+
+
 def psync_step_host(step: psync_step, h_arrival: np.ndarray, h_grads: Sequence[torch.Tensor],
                     d_work: torch.Tensor, h_theta_out: Optional[torch.Tensor] = None,
                     h_kept: Optional[np.ndarray] = None, h_step_tag: Optional[np.ndarray] = None, t: int = 0,
-                    chunk_elems: int = 0, stream=None, check: bool = True):
+                    chunk_elems: int = 0, stream=None, check: bool = True, ctx: Optional[HostCtx] = None):
     """The step with HOST gradient buffers (include/psync.h: psync_step_host).  h_grads are CPU tensors
     (pinned for full PCIe rate); theta/ema/state stay on the device.  Returns (status, t_nth)."""
     W = step.W
@@ -469,7 +499,7 @@ def psync_step_host(step: psync_step, h_arrival: np.ndarray, h_grads: Sequence[t
         raise ValueError("h_kept must be int32[N]")
     if h_step_tag is not None and (h_step_tag.dtype != np.int32 or h_step_tag.size != W):
         raise ValueError("h_step_tag must be int32[W]")
-    st = lib().psync_step_host(ctypes.byref(step), h_arrival.ctypes.data,
+    st = lib().psync_step_host_ctx(None if ctx is None else ctx.handle, ctypes.byref(step), h_arrival.ctypes.data,
                                None if h_step_tag is None else h_step_tag.ctypes.data, t,
                                ctypes.cast(ptrs, ctypes.c_void_p),
                                None if h_theta_out is None else h_theta_out.data_ptr(),

@@ -99,6 +99,35 @@ cudaError_t launch_step_kernel(const psync_step* s, const FusedParams& p, cudaSt
 
 constexpr int64_t kDefaultChunkElems = int64_t{1} << 20;
 
+// The copy stream and the four events psync_step_host needs; created per call, or once by psync_host_ctx_create.
+struct HostCtx {
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t copied[2] = {nullptr, nullptr};
+  cudaEvent_t consumed[2] = {nullptr, nullptr};
+};
+
+void host_ctx_release(HostCtx* c) {
+  if (c->copy_stream != nullptr) {
+    cudaStreamSynchronize(c->copy_stream);
+    cudaStreamDestroy(c->copy_stream);
+    c->copy_stream = nullptr;
+  }
+  for (int i = 0; i < 2; ++i) {
+    if (c->copied[i] != nullptr) cudaEventDestroy(c->copied[i]);
+    if (c->consumed[i] != nullptr) cudaEventDestroy(c->consumed[i]);
+    c->copied[i] = c->consumed[i] = nullptr;
+  }
+}
+
+bool host_ctx_init(HostCtx* c) {
+  if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return false;
+  for (int i = 0; i < 2; ++i) {
+    if (cudaEventCreateWithFlags(&c->copied[i], cudaEventDisableTiming) != cudaSuccess) return false;
+    if (cudaEventCreateWithFlags(&c->consumed[i], cudaEventDisableTiming) != cudaSuccess) return false;
+  }
+  return true;
+}
+
 int64_t round_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
 struct HostLayout {
@@ -352,9 +381,38 @@ PSYNC_API size_t psync_step_host_workspace_bytes(int32_t N, int32_t W, int32_t g
   return L.total;
 }
 
+PSYNC_API int psync_host_ctx_create(void** ctx) {
+  if (ctx == nullptr) return PSYNC_EINVAL;
+  HostCtx* c = new HostCtx();
+  if (!host_ctx_init(c)) {
+    host_ctx_release(c);
+    delete c;
+    cudaGetLastError();
+    *ctx = nullptr;
+    return PSYNC_ECUDA;
+  }
+  *ctx = c;
+  return PSYNC_OK;
+}
+
+PSYNC_API int psync_host_ctx_destroy(void* ctx) {
+  if (ctx == nullptr) return PSYNC_EINVAL;
+  HostCtx* c = static_cast<HostCtx*>(ctx);
+  host_ctx_release(c);
+  delete c;
+  return PSYNC_OK;
+}
+
 PSYNC_API int psync_step_host(const psync_step* st, const float* h_arrival, const int32_t* h_step_tag, int32_t t,
                     const void* const* h_grads, float* h_theta_out, int32_t* h_kept, float* h_t_nth, void* d_work,
                     size_t work_bytes, int64_t chunk_elems, void* stream) {
+  return psync_step_host_ctx(nullptr, st, h_arrival, h_step_tag, t, h_grads, h_theta_out, h_kept, h_t_nth, d_work,
+                             work_bytes, chunk_elems, stream);
+}
+
+PSYNC_API int psync_step_host_ctx(void* ctx, const psync_step* st, const float* h_arrival, const int32_t* h_step_tag,
+                        int32_t t, const void* const* h_grads, float* h_theta_out, int32_t* h_kept, float* h_t_nth,
+                        void* d_work, size_t work_bytes, int64_t chunk_elems, void* stream) {
   const int chk = check_step(st, false);
   if (chk != PSYNC_OK) return chk;
   if (h_arrival == nullptr || h_grads == nullptr || d_work == nullptr) return PSYNC_EINVAL;
@@ -376,8 +434,8 @@ PSYNC_API int psync_step_host(const psync_step* st, const float* h_arrival, cons
   int32_t* d_ident = reinterpret_cast<int32_t*>(work + L.off_ident);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
 
-  cudaStream_t copy_stream = nullptr;
-  cudaEvent_t copied[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr};
+  HostCtx local;                                   // used when the caller brought no context
+  HostCtx* hc = ctx != nullptr ? static_cast<HostCtx*>(ctx) : &local;
   int result = PSYNC_OK;
   std::vector<int32_t> kept(N);
   int32_t status = PSYNC_ECUDA;
@@ -412,12 +470,15 @@ PSYNC_API int psync_step_host(const psync_step* st, const float* h_arrival, cons
   if (h_t_nth != nullptr) *h_t_nth = t_nth;
 
   // 2./3. stream the kept buffers chunk by chunk; copy stream runs one chunk ahead of the kernel
-  PSYNC_CU(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
-  for (int i = 0; i < 2; ++i) {
-    PSYNC_CU(cudaEventCreateWithFlags(&copied[i], cudaEventDisableTiming));
-    PSYNC_CU(cudaEventCreateWithFlags(&consumed[i], cudaEventDisableTiming));
+  if (ctx == nullptr && !host_ctx_init(&local)) {
+    result = PSYNC_ECUDA;
+    goto cleanup;
   }
   {
+    cudaStream_t copy_stream = hc->copy_stream;
+    cudaEvent_t* copied = hc->copied;
+    cudaEvent_t* consumed = hc->consumed;
+    // both streams are idle here: `s` was synchronised above and every call ends with both streams drained
     int64_t c = 0;
     for (int64_t first = 0; first < st->P; first += L.chunk, ++c) {
       const int buf = static_cast<int>(c & 1);
@@ -439,20 +500,14 @@ PSYNC_API int psync_step_host(const psync_step* st, const float* h_arrival, cons
                                  cudaMemcpyDeviceToHost, s));
     }
   }
-  PSYNC_CU(cudaStreamSynchronize(copy_stream));
+  PSYNC_CU(cudaStreamSynchronize(hc->copy_stream));
   PSYNC_CU(cudaStreamSynchronize(s));
 
 cleanup:
 #undef PSYNC_CU
   if (result == PSYNC_ECUDA) cudaGetLastError();
-  if (copy_stream != nullptr) {
-    cudaStreamSynchronize(copy_stream);
-    cudaStreamDestroy(copy_stream);
-  }
-  for (int i = 0; i < 2; ++i) {
-    if (copied[i] != nullptr) cudaEventDestroy(copied[i]);
-    if (consumed[i] != nullptr) cudaEventDestroy(consumed[i]);
-  }
+  if (hc->copy_stream != nullptr) cudaStreamSynchronize(hc->copy_stream);
+  if (ctx == nullptr) host_ctx_release(&local);
   return result;
 }
 

@@ -29,7 +29,7 @@ int main(void) {
   int32_t *d_kept, *d_status, kept[N], status = -99;
   const void** d_table;
   float tnth = 0.f;
-  CHECK(psync_version() >= 130);
+  CHECK(psync_version() >= 200);
   CHECK(cudaMalloc((void**)&d_theta, sizeof(float) * P) == cudaSuccess);
   CHECK(cudaMalloc((void**)&d_ema, sizeof(float) * P) == cudaSuccess);
   CHECK(cudaMalloc((void**)&d_arrival, sizeof(arrival)) == cudaSuccess);
@@ -94,6 +94,49 @@ int main(void) {
     CHECK(status == PSYNC_ETOOFEW);
     CHECK(cudaMemcpy(h, d_theta, sizeof(float) * P, cudaMemcpyDeviceToHost) == cudaSuccess);
     for (int i = 0; i < P; ++i) CHECK(h[i] == 0.375f);
+  }
+  /* the slices layout: what each server RECEIVES -- one cudaMalloc per (worker, server) slice, the slices of worker 1 placed
+   * 4 bytes after the allocation boundary; theta = 1 again; same kept set {0,1,2,3} => theta' = 0.6875, ema' = 0.5*ema + 0.34375 */
+  {
+    enum { M = 2 };
+    float* slice[W][M];
+    const void* h_table[W * M];
+    const void** d_slices;
+    int64_t *d_off, *d_tiles, tiles[M + 1];
+    for (int k = 0; k < W; ++k)
+      for (int j = 0; j < M; ++j) {
+        const int64_t len = shard_off[j + 1] - shard_off[j];
+        float* base;
+        CHECK(cudaMalloc((void**)&base, sizeof(float) * (size_t)(len + 1)) == cudaSuccess);
+        slice[k][j] = base + (k == 1 ? 1 : 0);
+        for (int64_t i = 0; i < len; ++i) h[i] = (k == 4) ? NAN : 0.25f * (float)(k + 1);
+        CHECK(cudaMemcpy(slice[k][j], h, sizeof(float) * (size_t)len, cudaMemcpyHostToDevice) == cudaSuccess);
+        h_table[k * M + j] = (k == 4) ? NULL : slice[k][j];          /* the straggler's slices are not even there */
+      }
+    CHECK(cudaMalloc((void**)&d_slices, sizeof(h_table)) == cudaSuccess);
+    CHECK(cudaMemcpy(d_slices, h_table, sizeof(h_table), cudaMemcpyHostToDevice) == cudaSuccess);
+    CHECK(cudaMalloc((void**)&d_off, sizeof(shard_off)) == cudaSuccess);
+    CHECK(cudaMalloc((void**)&d_tiles, sizeof(tiles)) == cudaSuccess);
+    CHECK(cudaMemcpy(d_off, shard_off, sizeof(shard_off), cudaMemcpyHostToDevice) == cudaSuccess);
+    CHECK(psync_shard_worklist(d_off, M, PSYNC_F32, d_tiles, NULL) == PSYNC_OK);
+    CHECK(cudaMemcpy(tiles, d_tiles, sizeof(tiles), cudaMemcpyDeviceToHost) == cudaSuccess);
+    CHECK(tiles[0] == 0 && tiles[1] == 1 && tiles[2] == 1 + 4);      /* ceil(1000/1024), ceil(3099/1024) */
+    for (int i = 0; i < P; ++i) h[i] = 1.0f;
+    CHECK(cudaMemcpy(d_theta, h, sizeof(float) * P, cudaMemcpyHostToDevice) == cudaSuccess);
+    CHECK(cudaMemcpy(d_arrival, arrival, sizeof(arrival), cudaMemcpyHostToDevice) == cudaSuccess);
+    st.d_grads = (const void* const*)d_slices; st.grad_layout = PSYNC_GRADS_SLICES;
+    st.d_shard_off = d_off; st.d_tile_start = d_tiles; st.ema_mode = PSYNC_EMA_POST;
+    st.d_tile_start = NULL;
+    CHECK(psync_step_device(&st, d_arrival, NULL, 0, d_tnth, NULL) == PSYNC_EINVAL);   /* slices need the work list */
+    st.d_tile_start = d_tiles;
+    CHECK(psync_step_device(&st, d_arrival, NULL, 0, d_tnth, NULL) == PSYNC_OK);
+    CHECK(cudaDeviceSynchronize() == cudaSuccess);
+    CHECK(cudaMemcpy(&status, d_status, sizeof(status), cudaMemcpyDeviceToHost) == cudaSuccess);
+    CHECK(status == PSYNC_OK);
+    CHECK(cudaMemcpy(h, d_theta, sizeof(float) * P, cudaMemcpyDeviceToHost) == cudaSuccess);
+    for (int i = 0; i < P; ++i) CHECK(h[i] == 0.6875f);
+    CHECK(cudaMemcpy(h, d_ema, sizeof(float) * P, cudaMemcpyDeviceToHost) == cudaSuccess);
+    for (int i = 0; i < P; ++i) CHECK(h[i] == 0.5f * 0.359375f + 0.34375f);
   }
   printf("abi_smoke ok: %s\n", psync_status_string(PSYNC_OK));
   return 0;

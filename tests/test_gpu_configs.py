@@ -93,6 +93,45 @@ def _full_size_sampled(cfg, steps=2, n_sample=40_000):
     assert geo["grid"] == -(-cfg.P // geo["tile_elems"])          # one tile per CTA, the bench's launch
 
 
+def _full_size_every_element(cfg, steps=2):
+    """The real config in bench.py's launch configuration, ALL P elements of theta / state / ema compared after every
+    step (lock-step) with the oracle's streamed form: oracle.accumulate over the kept workers' buffers in ascending
+    order (one buffer D2H at a time), then oracle.apply_sum -- bit-identical to the whole-step oracle (pinned in
+    tests/test_oracle_update.py::test_shard_layout_invariance_and_streamed_form)."""
+    free, _ = torch.cuda.mem_get_info()
+    if cfg.footprint_bytes * 1.15 > free:
+        pytest.skip("not enough free HBM for the full-size config")
+    pair = Pair(cfg)
+    grads = [torch.empty(cfg.P, dtype=torch.float32 if cfg.grad_dtype == synth.F32 else torch.bfloat16, device=DEV)
+             for _ in range(cfg.W)]
+    S = np.zeros(cfg.P, np.float64)
+    h = pair.host
+    rtol = RTOL_BF16 if cfg.grad_dtype == synth.BF16 else RTOL_STEP
+    for s in range(steps):
+        for k in range(cfg.W):
+            synth.gradient(cfg, s, k, DEV, out=grads[k])
+        arrival = synth.arrival_times(cfg, s)
+        st, kept, tn = pair.gpu_step(grads, arrival)
+        st_o, kept_o, tn_o = oracle.select_first_n(arrival, cfg.N, cfg.b)
+        assert st == st_o == 0 and np.array_equal(kept, kept_o) and tn == tn_o
+        S[:] = 0.0
+        for k in kept_o:
+            assert oracle.accumulate(S, synth.as_numpy_grad(grads[k])) == oracle.OK
+        assert oracle.apply_sum(pair.shard_off, cfg.N, S, h["theta"], h["ema"], h["state0"], h["state1"], opt=cfg.opt,
+                                ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho,
+                                eps=cfg.eps) == oracle.OK
+        pair.compare(rtol, ATOL_STEP, f"{cfg.name} full size, every element, step {s}")
+        pair.sync_host_from_gpu()
+
+
+def test_full_size_cfg3_paper_rmsprop_every_element():
+    _full_size_every_element(synth.PAPER_RMSPROP)
+
+
+def test_full_size_cfg2_inception_sgd_every_element():
+    _full_size_every_element(synth.INCEPTION_SGD)
+
+
 def test_full_size_cfg3_paper_rmsprop_sampled():
     _full_size_sampled(synth.PAPER_RMSPROP)
 
