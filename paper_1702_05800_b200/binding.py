@@ -26,7 +26,7 @@ PSYNC_MAX_WORKERS = 1024
 PSYNC_TILE_UNITS = 256
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
-           "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_async_apply", "psync_step_device", "psync_clip_workspace_bytes",
+           "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_async_apply", "psync_staleness", "psync_step_device", "psync_clip_workspace_bytes",
            "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_host_ctx_create", "psync_host_ctx_destroy",
            "psync_step_host_ctx", "psync_launch_geometry", "psync_probe_read",
@@ -83,6 +83,8 @@ def lib() -> ctypes.CDLL:
         L.psync_step_device.restype = ctypes.c_int
         L.psync_order_by_arrival.argtypes = [vp, i32, vp, vp, vp]
         L.psync_order_by_arrival.restype = ctypes.c_int
+        L.psync_staleness.argtypes = [vp, i32, vp, vp, i32, vp, i32, vp, vp, vp, vp]
+        L.psync_staleness.restype = ctypes.c_int
         L.psync_async_apply.argtypes = [ctypes.POINTER(psync_step), vp, vp, vp]
         L.psync_clip_workspace_bytes.argtypes = [i32, i64, i32]
         L.psync_clip_workspace_bytes.restype = ctypes.c_size_t
@@ -534,4 +536,20 @@ def psync_selftest_rsqrt(d_mismatch: torch.Tensor, n: int, first_bits: int = 0, 
                                     _dptr(d_mismatch, torch.int64, "d_mismatch"), _stream(stream))
     if st != PSYNC_OK:
         raise PsyncError(st, "psync_selftest_rsqrt")
+    return st
+
+
+def psync_staleness(d_read_iter: torch.Tensor, d_order: torch.Tensor, d_t: torch.Tensor, d_staleness: torch.Tensor,
+                    d_stats: torch.Tensor, d_status: torch.Tensor, K: int = 0, d_n_arrived: Optional[torch.Tensor] = None,
+                    lag: int = 0, stream=None, check: bool = True) -> int:
+    """Staleness of the gradients Alg. 2 applies (include/psync.h: psync_staleness)."""
+    W = d_read_iter.numel()
+    if d_staleness.numel() < W or d_stats.numel() < 6 or d_order.numel() < (W if d_n_arrived is not None else K):
+        raise ValueError("need d_staleness [W], d_stats [6], d_order [K]")
+    st = lib().psync_staleness(_dptr(d_read_iter, torch.int64, "d_read_iter"), W, _dptr(d_order, torch.int32, "d_order"),
+                               _dptr(d_n_arrived, torch.int32, "d_n_arrived"), K, _dptr(d_t, torch.int64, "d_t"), lag,
+                               _dptr(d_staleness, torch.int64, "d_staleness"), _dptr(d_stats, torch.float64, "d_stats"),
+                               _dptr(d_status, torch.int32, "d_status"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_staleness")
     return st

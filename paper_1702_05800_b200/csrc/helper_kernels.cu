@@ -271,6 +271,87 @@ void pdl_config(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* attr, dim3 grid, d
   cfg->numAttrs = 1;
 }
 
+// ---- K8: staleness of the gradients Alg. 2 applies (Table 1; fixed lag: section 2.1) -------
+// One CTA, thread i owns the i-th applied gradient: staleness_i = (t + lag + i) - read_iter[order[i]]; the worker's next
+// read sees t + lag + i + 1.  Validation (a worker twice in one batch, a read from the future) happens before anything
+// is written.  Statistics: min / max by reduction, mean = sum / K (integer sum, exact), the population standard
+// deviation summed by one thread in index order (the order the oracle uses), the median from a rank sort.
+__global__ void __launch_bounds__(1024) staleness_kernel(int64_t* read_iter, int32_t W, const int32_t* order,
+                                                         const int32_t* n_arrived, int32_t K_arg, int64_t* t_counter,
+                                                         int32_t lag, int64_t* staleness, double* stats, int32_t* status) {
+  __shared__ int s_seen[kMaxWorkers];
+  __shared__ long long s_val[kMaxWorkers];
+  __shared__ long long s_sorted[kMaxWorkers];
+  __shared__ int s_bad;
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const int i = threadIdx.x;
+  const int K = n_arrived ? *n_arrived : K_arg;
+  if (i < W) s_seen[i] = 0;
+  if (i == 0) s_bad = (K < 0 || K > W) ? 1 : 0;
+  __syncthreads();
+  const long long t0 = *t_counter;
+  int k = -1;
+  long long st = 0;
+  if (s_bad == 0 && i < K) {
+    k = order[i];
+    if (k < 0 || k >= W) {
+      atomicExch(&s_bad, 1);
+    } else {
+      if (atomicAdd(&s_seen[k], 1) != 0) atomicExch(&s_bad, 1);  // the same worker twice in one batch
+      const long long r = read_iter[k];
+      st = t0 + lag + i - r;
+      if (r < 0 || st < 0) atomicExch(&s_bad, 1);  // computed from parameters that did not exist yet
+    }
+  }
+  if (t0 < 0 || lag < 0) s_bad = 1;
+  __syncthreads();
+  if (s_bad != 0) {
+    if (i == 0) *status = -1;  // PSYNC_EINVAL; nothing else is written
+    return;
+  }
+  if (i < K) {
+    staleness[i] = st;
+    read_iter[k] = t0 + lag + i + 1;
+    s_val[i] = st;
+  }
+  __syncthreads();
+  if (i < K) {  // rank sort (ties by index)
+    int rank = 0;
+    for (int j = 0; j < K; ++j) {
+      const long long v = s_val[j];
+      rank += (v < st || (v == st && j < i)) ? 1 : 0;
+    }
+    s_sorted[rank] = st;
+  }
+  __syncthreads();
+  if (i == 0) {
+    *status = 0;
+    *t_counter = t0 + K;
+    if (K == 0) {
+      const double nan = __longlong_as_double(0x7FF8000000000000LL);
+      stats[0] = stats[1] = stats[2] = stats[3] = stats[4] = nan;
+      stats[5] = 0.0;
+    } else {
+      double sum = 0.0;
+      for (int j = 0; j < K; ++j) sum = __dadd_rn(sum, static_cast<double>(s_val[j]));
+      const double mean = __ddiv_rn(sum, static_cast<double>(K));
+      double ss = 0.0;
+      for (int j = 0; j < K; ++j) {
+        const double d = __dsub_rn(static_cast<double>(s_val[j]), mean);
+        ss = __dadd_rn(ss, __dmul_rn(d, d));
+      }
+      stats[0] = static_cast<double>(s_sorted[0]);
+      stats[1] = mean;
+      stats[2] = (K & 1) ? static_cast<double>(s_sorted[K / 2])
+                         : __dmul_rn(0.5, __dadd_rn(static_cast<double>(s_sorted[K / 2 - 1]), static_cast<double>(s_sorted[K / 2])));
+      stats[3] = static_cast<double>(s_sorted[K - 1]);
+      stats[4] = __dsqrt_rn(__ddiv_rn(ss, static_cast<double>(K)));
+      stats[5] = static_cast<double>(K);
+    }
+  }
+}
+
 }  // namespace
 
 size_t clip_workspace_bytes(int32_t W, int64_t P, int dtype) {
@@ -317,6 +398,22 @@ cudaError_t launch_lr_schedule(float gamma0, float beta, int64_t t0, int32_t K, 
   cudaLaunchAttribute attr[1];
   pdl_config(&cfg, attr, dim3(static_cast<unsigned>((K + 127) / 128)), dim3(128), stream);
   return cudaLaunchKernelEx(&cfg, lr_schedule_kernel, gamma0, beta, t0, K, s, d_gamma);
+}
+
+cudaError_t launch_staleness(int64_t* d_read_iter, int32_t W, const int32_t* d_order, const int32_t* d_n_arrived,
+                             int32_t K, int64_t* d_t, int32_t lag, int64_t* d_staleness, double* d_stats,
+                             int32_t* d_status, cudaStream_t stream) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(1);
+  cfg.blockDim = dim3(static_cast<unsigned>((W + 31) / 32 * 32));
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, staleness_kernel, d_read_iter, W, d_order, d_n_arrived, K, d_t, lag, d_staleness,
+                            d_stats, d_status);
 }
 
 }  // namespace psync

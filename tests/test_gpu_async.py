@@ -248,3 +248,62 @@ def test_async_max_workers_1024():
     pair = AsyncPair(cfg)
     order = pair.step(0, synth.arrival_times(cfg, 0))
     assert order.size == 1024
+
+
+# ------------------------------------------------------------------ staleness bookkeeping (Table 1)
+def _staleness_gpu(read, order_dev, n_dev, t_dev, lag=0, K=0):
+    W = read.numel()
+    d_st = torch.full((W,), -7, dtype=torch.int64, device=DEV)
+    d_stats = torch.full((6,), -7.0, dtype=torch.float64, device=DEV)
+    d_status = torch.full((1,), -9, dtype=torch.int32, device=DEV)
+    psync.psync_staleness(read, order_dev, t_dev, d_st, d_stats, d_status, K=K, d_n_arrived=n_dev, lag=lag)
+    torch.cuda.synchronize()
+    return d_st.cpu().numpy(), d_stats.cpu().numpy(), int(d_status.item())
+
+
+@pytest.mark.parametrize("W,lag", [(1, 0), (5, 0), (40, 0), (106, 3), (1024, 1)])
+def test_staleness_chained_batches_match_the_oracle_bit_for_bit(W, lag):
+    """Several Alg. 2 batches chained on the device (order from psync_order_by_arrival, the update counter and the read
+    iterations stay on the GPU): staleness, next reads, the counter and all six statistics equal the oracle's."""
+    rng = np.random.default_rng(W)
+    d_read = torch.zeros(W, dtype=torch.int64, device=DEV)
+    d_t = torch.zeros(1, dtype=torch.int64, device=DEV)
+    h_read = np.zeros(W, np.int64)
+    t0 = 0
+    d_order = torch.full((W,), -1, dtype=torch.int32, device=DEV)
+    d_n = torch.zeros(1, dtype=torch.int32, device=DEV)
+    for batch in range(5):
+        arrival = rng.lognormal(0, 0.4, W).astype(np.float32)
+        arrival[rng.random(W) < 0.2] = np.inf                    # some workers send nothing this time
+        psync.psync_order_by_arrival(torch.from_numpy(arrival).to(DEV), W, d_order, d_n)
+        st, stats, status = _staleness_gpu(d_read, d_order, d_n, d_t, lag=lag)
+        order = oracle.order_by_arrival(arrival)
+        rc, want, h_read, want_stats = oracle.staleness(h_read, order, t0, lag=lag)
+        assert rc == oracle.OK and status == psync.PSYNC_OK
+        K = order.size
+        assert np.array_equal(st[:K], want) and (st[K:] == -7).all()
+        assert np.array_equal(d_read.cpu().numpy(), h_read)
+        t0 += K
+        assert int(d_t.item()) == t0
+        assert np.array_equal(stats, want_stats, equal_nan=True)
+
+
+def test_staleness_round_robin_is_W_minus_1_and_bad_batches_write_nothing():
+    W = 40
+    d_read = torch.zeros(W, dtype=torch.int64, device=DEV)
+    d_t = torch.zeros(1, dtype=torch.int64, device=DEV)
+    d_order = torch.arange(W, dtype=torch.int32, device=DEV)
+    for rnd in range(3):
+        st, stats, status = _staleness_gpu(d_read, d_order, None, d_t, K=W)
+        assert status == 0
+        assert (st == W - 1).all() if rnd else st.tolist() == list(range(W))
+    before = d_read.clone()
+    dup = d_order.clone()
+    dup[3] = 2                                                     # worker 2 twice in one batch
+    st, stats, status = _staleness_gpu(d_read, dup, None, d_t, K=W)
+    assert status == psync.PSYNC_EINVAL and (st == -7).all() and (stats == -7).all()
+    assert torch.equal(d_read, before) and int(d_t.item()) == 3 * W
+    future = before.clone()
+    future[0] = 10_000                                             # a read from the future
+    st, stats, status = _staleness_gpu(future, d_order, None, d_t, K=W)
+    assert status == psync.PSYNC_EINVAL and int(d_t.item()) == 3 * W

@@ -105,9 +105,9 @@ def _full_size_every_element(cfg, steps=2):
     grads = [torch.empty(cfg.P, dtype=torch.float32 if cfg.grad_dtype == synth.F32 else torch.bfloat16, device=DEV)
              for _ in range(cfg.W)]
     S = np.zeros(cfg.P, np.float64)
-    h = pair.host
     rtol = RTOL_BF16 if cfg.grad_dtype == synth.BF16 else RTOL_STEP
     for s in range(steps):
+        h = pair.host                                                # lock-step: re-synchronised after every step
         for k in range(cfg.W):
             synth.gradient(cfg, s, k, DEV, out=grads[k])
         arrival = synth.arrival_times(cfg, s)
