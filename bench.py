@@ -143,12 +143,16 @@ def load_peaks():
 
 # ------------------------------------------------------------------------------------ CPU oracle legs
 def oracle_full(cfg, host_grads, seconds_budget=12.0, max_steps=2000, warmup=0, fixed_steps=None, wall_budget=90.0,
-                first_step=0):
-    """Times the oracle AS IT STANDS (oracle.select_first_n + oracle.aggregate_update, all host cores) on the FULL
-    workload: all P parameters of the W gradient buffers in `host_grads` (numpy, host RAM; for the cpu_baseline leg the
-    exact bytes of the GPU's gradient set 0, copied D2H before timing), fresh arrival times every step, continuing from
-    the previous step's theta / state / ema.  Runs `fixed_steps` steps, else until `seconds_budget` seconds of oracle
-    time (or `wall_budget` seconds of wall clock).  Returns (grad-elements/s, info)."""
+                first_step=0, form="streamed"):
+    """Times the oracle AS IT STANDS (all host cores) on the FULL workload: all P parameters of the W gradient buffers in
+    `host_grads` (numpy, host RAM; for the cpu_baseline leg the exact bytes of the GPU's gradient set 0, copied D2H before
+    timing), fresh arrival times every step, continuing from the previous step's theta / state / ema.
+      form = "streamed": oracle.select_first_n, then oracle.accumulate over the kept buffers one at
+             a time in ascending worker order, then oracle.apply_sum;
+      form = "whole"  : oracle.select_first_n + oracle.aggregate_update (element-major over the N kept streams).
+    The two are the same arithmetic in the same order (bit-identical, pinned in tests/test_oracle_update.py).  Runs
+    `fixed_steps` steps, else until `seconds_budget` seconds of oracle time (or `wall_budget` seconds of wall clock).
+    Returns (grad-elements/s, info)."""
     import oracle  # the one place bench.py executes oracle/ (cpu_baseline / --impl reference)
 
     off = synth.shard_offsets(cfg)
@@ -157,6 +161,8 @@ def oracle_full(cfg, host_grads, seconds_budget=12.0, max_steps=2000, warmup=0, 
     s0 = None if s0 is None else s0.numpy().copy()
     s1 = None if s1 is None else s1.numpy().copy()
     ema = theta.copy()
+    S = np.zeros(cfg.P, np.float64) if form == "streamed" else None
+    hp = dict(opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
     t_begin = time.perf_counter()
     times = []
     total_steps = (fixed_steps + warmup) if fixed_steps is not None else max_steps
@@ -164,9 +170,13 @@ def oracle_full(cfg, host_grads, seconds_budget=12.0, max_steps=2000, warmup=0, 
         arrival = synth.arrival_times(cfg, first_step + s)
         t0 = time.perf_counter()
         st, kept, _ = oracle.select_first_n(arrival, cfg.N, cfg.b)
-        rc = oracle.aggregate_update(off, cfg.N, host_grads, kept, theta, ema, s0, s1, opt=cfg.opt,
-                                     ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho,
-                                     eps=cfg.eps)
+        if form == "streamed":
+            S[:] = 0.0
+            for k in kept:
+                rc = oracle.accumulate(S, host_grads[k])
+            rc = rc or oracle.apply_sum(off, cfg.N, S, theta, ema, s0, s1, **hp)
+        else:
+            rc = oracle.aggregate_update(off, cfg.N, host_grads, kept, theta, ema, s0, s1, **hp)
         t1 = time.perf_counter()
         assert st == 0 and rc == 0
         if s >= warmup:
@@ -175,8 +185,10 @@ def oracle_full(cfg, host_grads, seconds_budget=12.0, max_steps=2000, warmup=0, 
             break
     sec = float(np.sum(times))
     value = cfg.N * cfg.P * len(times) / sec
+    how = ("kept buffers accumulated one at a time in ascending worker order (oracle.accumulate), then oracle.apply_sum"
+           if form == "streamed" else "oracle.aggregate_update, element-major over the N kept streams")
     info = {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "note": "the oracle as it stands, never tuned: double arithmetic, element-major over the N kept streams",
+            "note": "the oracle as it stands, never tuned: double arithmetic, " + how,
             "sample": f"the FULL workload: all P={cfg.P} parameters of the W={cfg.W} gradient buffers of one resident "
                       f"gradient set held in host RAM, N={cfg.N} b={cfg.b}, fresh arrival times per step, "
                       f"{len(times)} steps, {sec:.2f} s of oracle time (select + aggregate/update/EMA; input "
@@ -638,6 +650,10 @@ def run_psync(args, cfg, rank, world, dist):
             _, info = oracle_full(cfg, host_grads, seconds_budget=args.cpu_seconds, first_step=Wm)
             info["sample"] += "; the buffers are the GPU arm's gradient set 0, byte for byte"
         out["cpu_baseline"] = {k: info[k] for k in ("value", "unit", "cores", "kind", "sample", "note")}
+        if host_grads is not None:            # the same arithmetic through the whole-step entry point (element-major)
+            vw, infow = oracle_full(cfg, host_grads, fixed_steps=2, first_step=Wm, form="whole")
+            out["cpu_baseline"]["value_whole_step_form"] = vw
+            out["cpu_baseline"]["note_whole_step_form"] = infow["note"] + "; 2 steps"
         if args.cpu_seconds_1thread > 0:       # the oracle single-threaded as well (a short sample)
             threads = oracle.num_threads()
             oracle.set_num_threads(1)
