@@ -394,3 +394,35 @@ def test_per_server_many_tiny_servers_every_tile_straddles():
     a[::7, :4] = np.inf                       # every 7th server fails (3 < N eligible)
     status, kept = pair.step_first_n(0, a)
     assert (status[::7] == oracle.ETOOFEW).all() and (np.delete(status, np.s_[::7]) == 0).all()
+
+
+def test_flat_rows_kernel_status_null_zero_count_and_garbage_count_are_failed_rows():
+    """The flat-index rows kernel (no work list) with status = NULL: a row whose time-out selection failed carries a
+    zero count and is skipped; a count nobody wrote (out of range) is skipped too -- never a loop over a stale count, a
+    wild pointer or 0 * inf = NaN in theta."""
+    cfg = per_server_cfg(opt=synth.RMSPROP_MOM, P=50_003, name="rows_null_status")
+    pair = RowsPair(cfg)
+    W, M = cfg.W, pair.M
+    a = synth.arrival_times_per_server(cfg, 0, server_sigma=0.3)
+    a[3, :] = 9.0
+    d_kept, d_n, d_status = _timeout_gpu(a, 1.1, M, W)
+    torch.cuda.synchronize()
+    assert int(d_status[3].item()) == oracle.ETOOFEW and int(d_n[3].item()) == 0
+    d_n[5] = 1_000_000                                             # garbage
+    grads = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    table = psync.make_grad_table(grads)
+    st, keep = pair.make_step(table, d_kept, None, per_shard=True, d_n_kept=d_n)
+    st.d_status = None
+    psync.psync_aggregate_update(st)
+    torch.cuda.synchronize()
+    kept = np.full((M, W), -1, np.int32)
+    n_kept = np.ones(M, np.int32)
+    status = np.zeros(M, np.int32)
+    for r in range(M):
+        status[r], k = oracle.select_timeout(a[r], 1.1)
+        if status[r] == oracle.OK:
+            kept[r, :k.size], n_kept[r] = k, k.size
+    status[5] = oracle.ETOOFEW                                     # the garbage row must behave like a failed one
+    pair.oracle_rows(grads, kept, True, n_kept=n_kept, status=status)
+    pair.compare_and_sync("rows kernel, status NULL")
+    assert bool(torch.isfinite(pair.theta).all())

@@ -364,3 +364,50 @@ def test_cfg3_full_size_separately_allocated_slices_some_misaligned_every_elemen
                                 ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho,
                                 eps=cfg.eps) == oracle.OK
         pair.compare_and_sync(f"cfg3 full size, slices, step {s}")
+
+
+def test_cfg3_full_size_1000_servers_one_kept_row_each_through_the_work_list_sampled():
+    """cfg3's P, N, b and optimizer cut into M = 1000 ragged servers (25 k parameters each), every server with its own
+    kept row (per-server arrival times), flat buffers through the work list -- the launch `bench.py --mode per_server
+    --servers 1000` times.  Sampled columns (every server boundary, the first and last tiles, 40 k random elements)
+    against the oracle's per-server rows on the gathered columns; two lock-step steps."""
+    cfg = replace(synth.PAPER_RMSPROP, M=1000, name="cfg3_M1000")
+    free, _ = torch.cuda.mem_get_info()
+    if cfg.footprint_bytes * 1.15 > free:
+        pytest.skip("not enough free HBM for the full-size config")
+    pair = SlicesPair(cfg)
+    off = pair.off
+    rng = np.random.default_rng(1000)
+    idx = np.unique(np.concatenate([np.arange(0, 4096), np.arange(cfg.P - 4096, cfg.P), off[1:-1], off[1:-1] - 1,
+                                    off[1:-1] + 1, rng.integers(0, cfg.P, 40_000)])).astype(np.int64)
+    idx = idx[(idx >= 0) & (idx < cfg.P)]
+    d_idx = torch.from_numpy(idx).to(DEV)
+    off_s = np.searchsorted(idx, off).astype(np.int64)             # the same servers, cut in the sampled index space
+    host = {n: to_np(getattr(pair, n)[d_idx]) for n in STATE_NAMES}
+    grads = [torch.empty(cfg.P, dtype=torch.float32, device=DEV) for _ in range(cfg.W)]
+    table = psync.make_grad_table(grads)
+    d_kept = torch.full((cfg.M, cfg.N), -1, dtype=torch.int32, device=DEV)
+    d_status = torch.full((cfg.M,), -9, dtype=torch.int32, device=DEV)
+    st, keep = pair.make_step(table, d_kept, d_status, per_shard=True, layout=psync.PSYNC_GRADS_FLAT)
+    geo = psync.psync_launch_geometry(st)
+    assert geo["grid"] == int(np.sum(-(-np.diff(off) // 1024))) and geo["block"] == 256      # the work list's grid
+    for s in range(2):
+        for k in range(cfg.W):
+            synth.gradient(cfg, s, k, DEV, out=grads[k])
+        a = synth.arrival_times_per_server(cfg, s, server_sigma=0.3)
+        a[7, :20] = np.inf                                          # server 7 cannot collect N gradients
+        psync.psync_step_device(st, torch.from_numpy(a).to(DEV), t=s)
+        torch.cuda.synchronize()
+        status, kept, _ = oracle.select_first_n_sharded(a, cfg.N, cfg.b)
+        assert status[7] == oracle.ETOOFEW and np.array_equal(d_status.cpu().numpy(), status)
+        assert np.array_equal(d_kept.cpu().numpy()[status == 0], kept[status == 0])
+        g_s = [synth.as_numpy_grad(g[d_idx]) for g in grads]
+        assert oracle.aggregate_update_rows(off_s, cfg.N, g_s, kept, host["theta"], host["ema"], host["state0"],
+                                            host["state1"], per_shard=True, status=status, opt=cfg.opt,
+                                            ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu,
+                                            rho=cfg.rho, eps=cfg.eps) == oracle.OK
+        for n in STATE_NAMES:
+            got = to_np(getattr(pair, n)[d_idx])
+            assert_close(got, host[n], RTOL_STEP, ATOL_STEP, f"cfg3 M=1000 step {s} {n} (sampled)")
+            host[n] = got
+        assert bool(torch.isfinite(pair.theta).all())
