@@ -75,7 +75,6 @@ __global__ void __launch_bounds__(kThreads, MINB) sharded_aggregate_update_ema(c
   constexpr int Q = E / 4;
   __shared__ const char* s_ptr[kMaxWorkers];
   __shared__ __align__(16) float s_acc[kThreads * E];
-  __shared__ unsigned s_ref;
 
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -92,21 +91,19 @@ __global__ void __launch_bounds__(kThreads, MINB) sharded_aggregate_update_ema(c
   if (N <= 0 || N > p.kept_stride || N > kMaxWorkers) return;  // a count nobody wrote: treat the row as failed
   const float inv_N = p.n_kept ? 1.0f / static_cast<float>(N) : p.inv_N;
 
-  // ---- stage server j's kept row as slice base pointers; the first one fixes the 16-byte phase -----------
+  // ---- stage server j's kept row as slice base pointers; the first one fixes the phase ---------------------
+  // Every thread reads the row's first pointer itself (one address for the whole CTA: a broadcast), so the head peel
+  // is known before the staging pass and one barrier is enough.
   const int32_t* kept = p.kept + static_cast<int64_t>(row) * p.kept_stride;
-  for (int i = threadIdx.x; i < N; i += kThreads) {
-    const int k = kept[i];
-    const char* g = p.slices ? static_cast<const char*>(p.grads[static_cast<int64_t>(k) * p.M + j])
-                             : static_cast<const char*>(p.grads[k]) + off_j * ESZ;
-    s_ptr[i] = g;
-    if (i == 0) s_ref = static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 127u;
-  }
-  __syncthreads();
-  const unsigned ref = s_ref;
+  auto slice_ptr = [&](int k) -> const char* {
+    return p.slices ? static_cast<const char*>(p.grads[static_cast<int64_t>(k) * p.M + j])
+                    : static_cast<const char*>(p.grads[k]) + off_j * ESZ;
+  };
+  const unsigned ref = static_cast<unsigned>(reinterpret_cast<uintptr_t>(slice_ptr(kept[0]))) & 127u;
   const int h = static_cast<int>(((128u - ref) & 127u) / ESZ);  // head peel: elements before the first 128-byte line
   unsigned mis = 0;
   for (int i = threadIdx.x; i < N; i += kThreads) {
-    const char* g = s_ptr[i];
+    const char* g = slice_ptr(kept[i]);
     mis |= ((static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) ^ ref) & 15u);  // another 16-byte phase
     s_ptr[i] = g + h * ESZ;  // unit u of this worker = s_ptr[i] + 16 u
   }
@@ -120,30 +117,70 @@ __global__ void __launch_bounds__(kThreads, MINB) sharded_aggregate_update_ema(c
     const int64_t live_units = (nu - u0 < kThreads) ? (nu - u0) : kThreads;
     const bool live = threadIdx.x < live_units;
     const int64_t unit = live ? (u0 + threadIdx.x) : (nu - 1);  // dead slots re-read a valid unit, store nothing
+    const bool theta_vec = p.base_aligned != 0 && (e0 & 3) == 0;  // CTA-uniform: theta co-aligned with the units
+    // transposed epilogue: lane l of a warp owns elements l, l + 32, ... of the warp's segment of 32 units
+    constexpr int SEG = 32 * E;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t seg_e0 = e0 + (u0 + warp * 32) * E;              // parameter index of the segment
+    const int64_t live_in_seg = (live_units - warp * 32) * E;      // may be <= 0 (dead warp) or > SEG
+
+    // theta / state / ema in registers: float4 per unit (co-aligned) or E scalars (transposed); both are E values
+    float th[E], em[E], a0[E], a1[E];
+    auto load_state = [&]() {
+      if (theta_vec) {
+#pragma unroll
+        for (int q = 0; q < Q; ++q) {
+          const int64_t e = e0 + unit * E + 4 * q;
+          *reinterpret_cast<float4*>(&th[4 * q]) = ld_state16(p.theta + e);
+          if (EMA != EMA_OFF) *reinterpret_cast<float4*>(&em[4 * q]) = ld_state16(p.ema + e);
+          if (OPT != OPT_SGD) *reinterpret_cast<float4*>(&a0[4 * q]) = ld_state16(p.s0 + e);
+          if (OPT == OPT_RMSPROP_MOM) *reinterpret_cast<float4*>(&a1[4 * q]) = ld_state16(p.s1 + e);
+        }
+      } else {
+        const bool on = live_in_seg > 0;  // a dead warp must not touch memory
+#pragma unroll
+        for (int q = 0; q < E; ++q) {
+          const int idx = q * 32 + lane;
+          const int64_t e = seg_e0 + (idx < live_in_seg ? idx : 0);
+          th[q] = on ? ld_state32(p.theta + e) : 0.f;
+          if (EMA != EMA_OFF) em[q] = on ? ld_state32(p.ema + e) : 0.f;
+          if (OPT != OPT_SGD) a0[q] = on ? ld_state32(p.s0 + e) : 1.f;
+          if (OPT == OPT_RMSPROP_MOM) a1[q] = on ? ld_state32(p.s1 + e) : 0.f;
+        }
+      }
+    };
+    // HOIST (as in K2): with at most two fp32 state arrays their loads are issued WITH the last batch of gradient
+    // loads -- one dependent memory round trip less per CTA, which is what small N is bound by.
+    constexpr int kStateArrays = 1 + (EMA != EMA_OFF ? 1 : 0) + (OPT != OPT_SGD ? 1 : 0) + (OPT == OPT_RMSPROP_MOM ? 1 : 0);
+    constexpr bool HOIST = !BF16 && kStateArrays <= 2;
+
     float acc[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) acc[e] = 0.f;
 
     if (!mixed) {
       int n = 0;
-      for (; n + kU <= N; n += kU) {
+      const int n_loop = HOIST ? ((N - 1) / kU) * kU : (N / kU) * kU;  // HOIST keeps 1..kU gradients for the last batch
+      for (; n < n_loop; n += kU) {
         uint4 r[kU];
 #pragma unroll
         for (int u = 0; u < kU; ++u) r[u] = ldg_stream16(s_ptr[n + u] + unit * 16);
 #pragma unroll
         for (int u = 0; u < kU; ++u) accumulate_unit<BF16>(acc, r[u]);  // strictly ascending worker order
       }
-      if (n < N) {
+      if (HOIST || n < N) {
         uint4 r[kU];
 #pragma unroll
         for (int u = 0; u < kU; ++u) {
           const bool on = (n + u) < N;
           r[u] = on ? ldg_stream16(s_ptr[on ? (n + u) : (N - 1)] + unit * 16) : make_uint4(0u, 0u, 0u, 0u);
         }
+        if (HOIST) load_state();
 #pragma unroll
         for (int u = 0; u < kU; ++u)
           if ((n + u) < N) accumulate_unit<BF16>(acc, r[u]);
       }
+      if (!HOIST) load_state();
     } else {
 #pragma unroll 4
       for (int n = 0; n < N; ++n) {
@@ -151,65 +188,35 @@ __global__ void __launch_bounds__(kThreads, MINB) sharded_aggregate_update_ema(c
         const uint4 r = load_unit_any<BF16>(g + unit * 16, (reinterpret_cast<uintptr_t>(g) & 15u) == 0);
         accumulate_unit<BF16>(acc, r);
       }
+      load_state();
     }
 
-    const bool theta_vec = p.base_aligned != 0 && (e0 & 3) == 0;  // CTA-uniform
     if (theta_vec) {
-      float4 th[Q], em[Q], a0[Q], a1[Q];
 #pragma unroll
-      for (int q = 0; q < Q; ++q) {
-        const int64_t e = e0 + unit * E + 4 * q;
-        th[q] = ld_state16(p.theta + e);
-        if (EMA != EMA_OFF) em[q] = ld_state16(p.ema + e);
-        if (OPT != OPT_SGD) a0[q] = ld_state16(p.s0 + e);
-        if (OPT == OPT_RMSPROP_MOM) a1[q] = ld_state16(p.s1 + e);
-      }
+      for (int l = 0; l < E; ++l) update_element<OPT, EMA>(acc[l], inv_N, th[l], em[l], a0[l], a1[l], p);
+      if (live) {
 #pragma unroll
-      for (int q = 0; q < Q; ++q) {
-        float* t4 = reinterpret_cast<float*>(&th[q]);
-        float* e4 = reinterpret_cast<float*>(&em[q]);
-        float* x4 = reinterpret_cast<float*>(&a0[q]);
-        float* y4 = reinterpret_cast<float*>(&a1[q]);
-#pragma unroll
-        for (int l = 0; l < 4; ++l) update_element<OPT, EMA>(acc[4 * q + l], inv_N, t4[l], e4[l], x4[l], y4[l], p);
-        if (live) {
+        for (int q = 0; q < Q; ++q) {
           const int64_t e = e0 + unit * E + 4 * q;
-          st_state16(p.theta + e, th[q]);
-          if (EMA != EMA_OFF) st_state16(p.ema + e, em[q]);
-          if (OPT != OPT_SGD) st_state16(p.s0 + e, a0[q]);
-          if (OPT == OPT_RMSPROP_MOM) st_state16(p.s1 + e, a1[q]);
+          st_state16(p.theta + e, *reinterpret_cast<float4*>(&th[4 * q]));
+          if (EMA != EMA_OFF) st_state16(p.ema + e, *reinterpret_cast<float4*>(&em[4 * q]));
+          if (OPT != OPT_SGD) st_state16(p.s0 + e, *reinterpret_cast<float4*>(&a0[4 * q]));
+          if (OPT == OPT_RMSPROP_MOM) st_state16(p.s1 + e, *reinterpret_cast<float4*>(&a1[4 * q]));
         }
       }
     } else {
-      // theta's slice is not co-aligned with the gradient units: every warp transposes its own 32 units through
-      // shared memory (__syncwarp only), so that lane l owns elements l, l + 32, ... of the warp's segment and
-      // theta / state / ema move as coalesced 32-bit accesses.
-      constexpr int SEG = 32 * E;  // elements per warp
-      const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+      // theta's slice is not co-aligned with the gradient units: every warp transposes its own 32 sums through
+      // shared memory (__syncwarp only) and theta / state / ema move as coalesced 32-bit accesses.
       float* seg = s_acc + warp * SEG;
 #pragma unroll
       for (int q = 0; q < Q; ++q)
         *reinterpret_cast<float4*>(&seg[(lane * Q + q) * 4]) =
             make_float4(acc[4 * q], acc[4 * q + 1], acc[4 * q + 2], acc[4 * q + 3]);
       __syncwarp();
-      const int64_t seg_e0 = e0 + (u0 + warp * 32) * E;                       // parameter index of the segment
-      const int64_t live_in_seg = (live_units - warp * 32) * E;               // may be <= 0 (dead warp) or > SEG
-      float th[E], em[E], a0[E], a1[E], S[E];
 #pragma unroll
       for (int q = 0; q < E; ++q) {
         const int idx = q * 32 + lane;
-        const int64_t e = seg_e0 + (idx < live_in_seg ? idx : 0);
-        const bool on = live_in_seg > 0;                                     // a dead warp must not touch memory
-        S[q] = seg[idx];
-        th[q] = on ? ld_state32(p.theta + e) : 0.f;
-        if (EMA != EMA_OFF) em[q] = on ? ld_state32(p.ema + e) : 0.f;
-        if (OPT != OPT_SGD) a0[q] = on ? ld_state32(p.s0 + e) : 1.f;
-        if (OPT == OPT_RMSPROP_MOM) a1[q] = on ? ld_state32(p.s1 + e) : 0.f;
-      }
-#pragma unroll
-      for (int q = 0; q < E; ++q) {
-        const int idx = q * 32 + lane;
-        update_element<OPT, EMA>(S[q], inv_N, th[q], em[q], a0[q], a1[q], p);
+        update_element<OPT, EMA>(seg[idx], inv_N, th[q], em[q], a0[q], a1[q], p);
         if (idx < live_in_seg) {
           const int64_t e = seg_e0 + idx;
           st_state32(p.theta + e, th[q]);
