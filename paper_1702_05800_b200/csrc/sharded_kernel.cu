@@ -81,6 +81,9 @@ __global__ void __launch_bounds__(kThreads, MINB) sharded_aggregate_update_ema(c
 
   // ---- which (server, tile) is this CTA ---------------------------------------------------------------
   const int64_t b = blockIdx.x;
+  // The grid is the work list's total, computed by the host from the shard table; a table built for another gradient
+  // dtype (another tile size) has another total: then nothing is touched, instead of a partial update.
+  if (p.tile_start[p.M] != static_cast<int64_t>(gridDim.x)) return;
   const int j = upper_slot(p.tile_start, p.M, b);
   const int64_t off_j = p.shard_off[j];
   const int64_t len_j = p.shard_off[j + 1] - off_j;

@@ -296,6 +296,42 @@ def test_many_tiny_servers_through_the_work_list_match_the_oracle_and_the_flat_r
         assert x is None or np.array_equal(x, y)
 
 
+def test_slices_step_is_capturable_in_a_cuda_graph_and_replays_bit_identically():
+    """psync_step_device on the slices layout makes no synchronising call: capture three steps, replay, compare with the
+    same three steps enqueued directly."""
+    cfg = replace(BASE, opt=synth.MOMENTUM, name="slices_graph")
+    flat = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+
+    def run(use_graph):
+        pair = SlicesPair(cfg, shard_off=RAGGED)
+        table = psync.make_slice_table(cut_slices(flat, pair.off, lambda k, j: (k + j) % 3))
+        d_kept = torch.full((cfg.N,), -1, dtype=torch.int32, device=DEV)
+        d_status = torch.full((1,), -9, dtype=torch.int32, device=DEV)
+        st, keep = pair.make_step(table, d_kept, d_status)
+        arr = [torch.from_numpy(synth.arrival_times(cfg, s)).to(DEV) for s in range(3)]
+        stream = torch.cuda.Stream()
+        stream.wait_stream(torch.cuda.current_stream())
+        if use_graph:
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                for s in range(3):
+                    psync.psync_step_device(st, arr[s], t=s, stream=torch.cuda.current_stream())
+            before = [to_np(getattr(pair, n)) for n in STATE_NAMES]
+            g.replay()
+            torch.cuda.synchronize()
+            assert not np.array_equal(before[0], to_np(pair.theta))          # capture did not run the kernels, replay did
+        else:
+            for s in range(3):
+                psync.psync_step_device(st, arr[s], t=s, stream=stream)
+            torch.cuda.synchronize()
+        return [to_np(getattr(pair, n)) for n in STATE_NAMES], keep, table
+
+    a, _, _ = run(False)
+    b_, _, _ = run(True)
+    for x, y in zip(a, b_):
+        assert x is None or np.array_equal(x, y)
+
+
 def test_abi_validation_of_the_slices_layout():
     cfg = replace(BASE, P=4096, M=2, N=3, b=1, ragged=False, name="slices_abi")
     pair = SlicesPair(cfg)
@@ -320,6 +356,12 @@ def test_abi_validation_of_the_slices_layout():
     assert np.array_equal(to_np(pair.theta), before)
     geo = psync.psync_launch_geometry(pair.make_step(table, d_kept)[0])
     assert geo["grid"] == 4 and geo["block"] == 256 and geo["tile_elems"] == 1024
+    # a work list built for the other gradient dtype (2048-parameter tiles): detected on the device, nothing is touched
+    pair.d_tiles = psync.psync_shard_worklist(pair.d_off, synth.BF16)
+    st, keep = pair.make_step(table, d_kept)
+    assert psync.psync_aggregate_update(st, check=False) == psync.PSYNC_OK
+    torch.cuda.synchronize()
+    assert np.array_equal(to_np(pair.theta), before)
 
 
 # ------------------------------------------------------------------ the headline config at FULL size, every element
