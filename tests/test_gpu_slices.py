@@ -453,3 +453,35 @@ def test_cfg3_full_size_1000_servers_one_kept_row_each_through_the_work_list_sam
             assert_close(got, host[n], RTOL_STEP, ATOL_STEP, f"cfg3 M=1000 step {s} {n} (sampled)")
             host[n] = got
         assert bool(torch.isfinite(pair.theta).all())
+
+
+def test_parameter_server_step_class_drives_slices_and_per_server_rows():
+    """The convenience class (plumbing only): per-(worker, server) slices + Alg. 4 per server j in one call per step."""
+    cfg = replace(BASE, opt=synth.RMSPROP_MOM, name="slices_class")
+    off = np.asarray(RAGGED, dtype=np.int64)
+    theta = synth.init_theta(cfg, DEV)
+    s0, s1 = synth.init_state(cfg, DEV)
+    ema = theta.clone()
+    ps = psync.ParameterServerStep(off, cfg.N, cfg.b, theta, ema, s0, s1, cfg.opt, cfg.ema_mode, alpha=cfg.alpha,
+                                   mu=cfg.mu, rho=cfg.rho, eps=cfg.eps, per_server=True)
+    host = {"theta": to_np(theta), "ema": to_np(ema), "state0": to_np(s0), "state1": to_np(s1)}
+    for s in range(2):
+        flat = [synth.gradient(cfg, s, k, DEV) for k in range(cfg.W)]
+        a = synth.arrival_times_per_server(replace(cfg, M=off.size - 1), s, server_sigma=0.3)
+        if s == 0:
+            slices = cut_slices(flat, off, lambda k, j: (k + 2 * j) % 4)
+            ps.set_gradient_slices(slices)
+        else:
+            ps.set_gradients(flat)                                  # flat buffers through the same work list
+        ps.step(torch.from_numpy(a).to(DEV), cfg.gamma, t=s)
+        torch.cuda.synchronize()
+        status, kept, t_nth = oracle.select_first_n_sharded(a, cfg.N, cfg.b)
+        assert np.array_equal(ps.d_status.cpu().numpy(), status) and np.array_equal(ps.d_kept.cpu().numpy(), kept)
+        assert np.array_equal(ps.d_t_nth.cpu().numpy(), t_nth)
+        assert oracle.aggregate_update_rows(off, cfg.N, [synth.as_numpy_grad(g) for g in flat], kept, host["theta"],
+                                            host["ema"], host["state0"], host["state1"], per_shard=True, status=status,
+                                            opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha,
+                                            mu=cfg.mu, rho=cfg.rho, eps=cfg.eps) == oracle.OK
+        for n, t in (("theta", theta), ("ema", ema), ("state0", s0), ("state1", s1)):
+            assert_close(to_np(t), host[n], RTOL_STEP, ATOL_STEP, f"class step {s} {n}")
+            host[n] = to_np(t)
