@@ -132,6 +132,10 @@ def test_full_size_cfg2_inception_sgd_every_element():
     _full_size_every_element(synth.INCEPTION_SGD)
 
 
+def test_full_size_cfg4_mixed_precision_every_element():
+    _full_size_every_element(synth.MIXED_PRECISION, steps=1)
+
+
 def test_full_size_cfg3_paper_rmsprop_sampled():
     _full_size_sampled(synth.PAPER_RMSPROP)
 
