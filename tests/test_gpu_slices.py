@@ -485,3 +485,52 @@ def test_parameter_server_step_class_drives_slices_and_per_server_rows():
         for n, t in (("theta", theta), ("ema", ema), ("state0", s0), ("state1", s1)):
             assert_close(to_np(t), host[n], RTOL_STEP, ATOL_STEP, f"class step {s} {n}")
             host[n] = to_np(t)
+
+
+# ------------------------------------------------------------------ seeded random cases: shapes nobody thought of
+@pytest.mark.parametrize("seed", range(24))
+def test_random_shard_layouts_alignments_rows_and_counts(seed):
+    """Random M, shard lengths (many empty / shorter than the head peel / around one tile), slice offsets (0-7 elements,
+    per worker and server), N, b, dtype, optimizer, EMA mode, kept-row mode (shared / per server / per-row counts) and
+    failed rows; gradients chosen directly (no selection kernel), lock-step against oracle.aggregate_update_slices."""
+    rng = np.random.default_rng(4000 + seed)
+    M = int(rng.choice([1, 2, 3, 5, 17, 60]))
+    lens = rng.choice([0, 1, 2, 3, 5, 31, 33, 100, 1023, 1024, 1025, 2049, 5000], size=M,
+                      p=[.08, .06, .06, .06, .06, .06, .06, .1, .08, .08, .1, .1, .1])
+    if lens.sum() == 0:
+        lens[0] = 7
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    P = int(off[-1])
+    W = int(rng.integers(1, 40))
+    N = int(rng.integers(1, W + 1))
+    dtype = int(rng.integers(0, 2))
+    opt = int(rng.integers(0, 3))
+    ema_mode = int(rng.integers(0, 3))
+    cfg = replace(BASE, P=P, M=M, N=N, b=W - N, grad_dtype=dtype, opt=opt, ema_mode=ema_mode, ragged=False,
+                  name=f"fuzz{seed}")
+    pair = SlicesPair(cfg, shard_off=off, state_misalign=int(rng.choice([0, 0, 1, 2])))
+    mode = int(rng.integers(0, 3))                  # 0: one shared row; 1: one row per server; 2: rows with counts
+    per_shard = mode > 0
+    rows = M if per_shard else 1
+    stride = W if mode == 2 else N
+    kept = np.full((rows, stride), -1, np.int32)
+    n_kept = np.full(rows, N, np.int32)
+    for r in range(rows):
+        n_kept[r] = int(rng.integers(1, W + 1)) if mode == 2 else N
+        kept[r, :n_kept[r]] = np.sort(rng.permutation(W)[:n_kept[r]])
+    status = np.zeros(rows, np.int32)
+    if per_shard and M > 1:
+        status[int(rng.integers(0, M))] = oracle.ETOOFEW
+    same_phase = bool(rng.integers(0, 2))
+    phase = rng.integers(0, 8, size=M)
+    tdt = torch.float32 if dtype == synth.F32 else torch.bfloat16
+    flat = [(torch.randn(P, device=DEV) * 1e-3).to(tdt) for _ in range(W)]
+    slices = cut_slices(flat, off, (lambda k, j: int(phase[j])) if same_phase else (lambda k, j: int((phase[j] + 3 * k) % 8)))
+    table = psync.make_slice_table(slices)
+    st, keep = pair.make_step(table, torch.from_numpy(kept).to(DEV), torch.from_numpy(status).to(DEV),
+                              per_shard=per_shard, d_n_kept=torch.from_numpy(n_kept).to(DEV) if mode == 2 else None)
+    psync.psync_aggregate_update(st)
+    torch.cuda.synchronize()
+    pair.oracle(slices, kept, per_shard=per_shard, n_kept=n_kept if mode == 2 else None, status=status)
+    pair.compare_and_sync(f"fuzz {seed}: M={M} P={P} W={W} N={N} dtype={dtype} opt={opt} ema={ema_mode} mode={mode}",
+                          RTOL_BF16 if dtype == synth.BF16 else RTOL_STEP)
