@@ -82,6 +82,10 @@ def lib() -> ctypes.CDLL:
         L.oracle_aggregate_update_rows.restype = ctypes.c_int
         L.oracle_aggregate_update_slices.argtypes = L.oracle_aggregate_update_rows.argtypes
         L.oracle_aggregate_update_slices.restype = ctypes.c_int
+        L.oracle_async_apply_rows.argtypes = [i64, i32, vp, i32, i32, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, i32,
+                                              vp, vp, vp, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int,
+                                              f32, f32, f32, f32, f32]
+        L.oracle_async_apply_rows.restype = ctypes.c_int
         L.oracle_staleness.argtypes = [vp, i32, vp, i32, i64, i32, vp, vp, vp]
         L.oracle_staleness.restype = ctypes.c_int
         L.oracle_order_by_arrival.argtypes = [vp, i32, vp, vp]
@@ -397,6 +401,50 @@ def async_apply(shard_off, grads, order, theta, ema=None, state0=None, state1=No
     return fn(P, M, _ptr(shard_off), order.size, W, ctypes.cast(ptrs, ctypes.c_void_p), gd,
               _ptr(order), _ptr(gammas), _ptr(gscales), _ptr(theta), _ptr(ema), _ptr(state0), _ptr(state1),
               opt, ema_mode, gamma_t, alpha, mu, rho, eps)
+
+
+def async_apply_rows(shard_off, grads, order, theta, ema=None, state0=None, state1=None, slices=False, per_shard=True,
+                     n_arrived=None, status=None, gammas=None, gscales=None, opt=SGD, ema_mode=EMA_PRE, gamma_t=0.0,
+                     alpha=0.0, mu=0.0, rho=0.0, eps=0.0):
+    """Alg. 2 per parameter server j: order is int32 [rows][stride] (rows = M if per_shard else 1),
+    n_arrived int32 [rows] or None (= stride), gscales float32 [W] indexed by WORKER.  grads: W flat arrays, or with
+    slices=True a list of W lists of M arrays (None where not needed)."""
+    P = theta.size
+    shard_off = np.ascontiguousarray(shard_off, dtype=np.int64)
+    M = shard_off.size - 1
+    W = len(grads)
+    if slices:
+        first = next(a for row in grads for a in row if a is not None)
+        gd = _grad_dtype([first])
+        for k, row in enumerate(grads):
+            for j, a in enumerate(row):
+                _chk(a, first.dtype, f"grads[{k}][{j}]", int(shard_off[j + 1] - shard_off[j]))
+        flat = [None if a is None else a.ctypes.data for row in grads for a in row]
+        ptrs = (ctypes.c_void_p * (W * M))(*flat)
+    else:
+        gd = _grad_dtype(grads)
+        for k, g in enumerate(grads):
+            _chk(g, grads[0].dtype, f"grads[{k}]", P)
+        ptrs = (ctypes.c_void_p * W)(*[g.ctypes.data for g in grads])
+    order = np.ascontiguousarray(order, dtype=np.int32)
+    if order.ndim == 1:
+        order = order[None, :]
+    rows = M if per_shard else 1
+    if order.shape[0] != rows:
+        raise ValueError("order must be int32 [rows][stride]")
+    _chk(n_arrived, np.int32, "n_arrived", rows)
+    _chk(status, np.int32, "status", rows)
+    _chk(gammas, np.float32, "gammas")
+    _chk(gscales, np.float32, "gscales", W)
+    for nm, a in (("theta", theta), ("ema", ema), ("state0", state0), ("state1", state1)):
+        _chk(a, np.float32, nm, P)
+    if _mirror_on:
+        raise NotImplementedError("the fp32 mirror has no per-server Alg. 2; compare rows one server at a time")
+    return lib().oracle_async_apply_rows(P, M, _ptr(shard_off), order.shape[1], W, ctypes.cast(ptrs, ctypes.c_void_p), gd,
+                                         1 if slices else 0, 1 if per_shard else 0, _ptr(order), order.shape[1],
+                                         _ptr(n_arrived), _ptr(status), _ptr(gammas), _ptr(gscales), _ptr(theta),
+                                         _ptr(ema), _ptr(state0), _ptr(state1), opt, ema_mode, gamma_t, alpha, mu, rho,
+                                         eps)
 
 
 def accumulate(S, grad):

@@ -32,7 +32,7 @@
 // schedule and clip factors (tests/test_oracle_helpers.py), straggler statistics and the Fig. 5
 // interpolation, the latter against the two values the paper prints (tests/test_oracle_stragglers.py);
 // the per-(worker, server) slice layout (tests/test_oracle_slices.py); the staleness bookkeeping of Alg. 2
-// (tests/test_oracle_staleness.py).
+// (tests/test_oracle_staleness.py) and Alg. 2 per server (tests/test_oracle_async.py).
 // (The fp32 diagnostic mirror of the GPU's operation list is a SEPARATE library, oracle/psync_mirror_f32.cpp;
 // nothing of it is in this file.)
 // Nothing here is "parity unpinned".
@@ -460,6 +460,61 @@ int oracle_async_apply(int64_t P, int32_t M, const int64_t* shard_off, int32_t K
 #endif
       for (int64_t e = lo; e < hi; ++e)
         apply_element(grad_at(G, grad_dtype, e), c, opt, ema_mode, theta, ema, state0, state1, e);
+    }
+  }
+  return ORACLE_OK;
+}
+
+// =============================================================================================
+// Alg. 2 run LITERALLY per parameter server j on what it receives.  The listing is "Async-SGD Parameter Server j"
+// (L78): each server has its own loop "wait for gradient G from any worker" (L85) and applies G[j] (L86), so the
+// order in which the gradients are applied, and how many have arrived, may differ from server to server (the
+// same remark as for Alg. 4).  Row r(j) = per_shard ? j : 0 of `order` (stride order_stride) lists the
+// workers in the order server j applies them, K_j = n_arrived ? n_arrived[r] : K of them.
+//   slices != 0: grads is [W*M], entry k*M + j -> the len_j elements of worker k's G_k[j] (element i = parameter
+//                shard_off[j] + i); else grads is [W] flat buffers.
+//   gammas[i]  learning rate of the server's i-th iteration of this batch (or NULL: gamma_t for all);
+//   gscales[k] global-norm clip factor of WORKER k's gradient (L313), or NULL (= 1);
+//   status[r]  != OK: server j applies nothing (its slice is untouched).
+// Per server the arithmetic is oracle_async_apply's: outer loop over the arrivals, inner loop over the server's
+// parameters, one optimizer step (divisor 1) and one EMA per arrival, stored as fp32 after every iteration.
+// =============================================================================================
+int oracle_async_apply_rows(int64_t P, int32_t M, const int64_t* shard_off, int32_t K, int32_t W,
+                            const void* const* grads, int grad_dtype, int slices, int per_shard, const int32_t* order,
+                            int32_t order_stride, const int32_t* n_arrived, const int32_t* status, const float* gammas,
+                            const float* gscales, float* theta, float* ema, float* state0, float* state1, int opt,
+                            int ema_mode, float gamma_t, float alpha, float mu, float rho, float eps) {
+  if (!args_ok(P, M, shard_off, 1, opt, ema_mode, theta, ema, state0, state1)) return ORACLE_EINVAL;
+  if (!grads || !order || K < 0 || K > W || order_stride < 1) return ORACLE_EINVAL;
+  if (grad_dtype != ORACLE_F32 && grad_dtype != ORACLE_BF16) return ORACLE_EINVAL;
+  for (int32_t j = 0; j < M; ++j) {  // validate every live row before anything is written
+    const int32_t row = per_shard ? j : 0;
+    if (status && status[row] != ORACLE_OK) continue;
+    const int32_t K_j = n_arrived ? n_arrived[row] : K;
+    if (K_j < 0 || K_j > order_stride || K_j > W) return ORACLE_EINVAL;
+    const int64_t len_j = shard_off[j + 1] - shard_off[j];
+    for (int32_t i = 0; i < K_j; ++i) {
+      const int32_t k = order[static_cast<int64_t>(row) * order_stride + i];
+      if (k < 0 || k >= W) return ORACLE_EINVAL;
+      if (len_j > 0 && !grads[slices ? static_cast<int64_t>(k) * M + j : k]) return ORACLE_EINVAL;
+    }
+  }
+  for (int32_t j = 0; j < M; ++j) {  // parameter server j
+    const int32_t row = per_shard ? j : 0;
+    if (status && status[row] != ORACLE_OK) continue;
+    const int32_t K_j = n_arrived ? n_arrived[row] : K;
+    const int64_t lo = shard_off[j], len_j = shard_off[j + 1] - shard_off[j];
+    for (int32_t i = 0; i < K_j; ++i) {  // its i-th iteration: "wait for gradient G from any worker"   (L85)
+      const int32_t k = order[static_cast<int64_t>(row) * order_stride + i];
+      Coeffs c = make_coeffs(1, gammas ? gammas[i] : gamma_t, alpha, mu, rho, eps);
+      if (gscales) c.inv_N = static_cast<double>(gscales[k]);  // the clip factor takes the place of 1/N = 1
+      const void* G = slices ? grads[static_cast<int64_t>(k) * M + j] : grads[k];
+      const int64_t g0 = slices ? 0 : lo;  // where server j's part starts in that buffer
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+      for (int64_t e = 0; e < len_j; ++e)  // theta(t+1)[j] <- theta(t)[j] - gamma_t G[j]; then the EMA   (L86-87)
+        apply_element(grad_at(G, grad_dtype, g0 + e), c, opt, ema_mode, theta, ema, state0, state1, lo + e);
     }
   }
   return ORACLE_OK;

@@ -174,3 +174,106 @@ def test_async_k0_is_a_no_op_and_invalid_arguments():
     assert oracle.async_apply([0, 4], grads, np.array([1], np.int32), theta, ema_mode=oracle.EMA_OFF) == oracle.EINVAL
     assert oracle.async_apply([0, 4], grads, np.array([0, 0], np.int32), theta, ema_mode=oracle.EMA_OFF) == oracle.EINVAL
     assert oracle.async_apply([0, 3], grads, np.array([0], np.int32), theta, ema_mode=oracle.EMA_OFF) == oracle.EINVAL
+
+
+# ------------------------------------------------------------------ Alg. 2 per parameter server j (rows, slices)
+def _g():
+    with open(os.path.join(os.path.dirname(__file__), "golden", "hand_worked_async.json")) as fh:
+        return json.load(fh)
+
+
+def test_golden_per_server_orders_counts_rates_clip_factors_and_a_failed_server():
+    g = _g()
+    ps = g["per_server"]
+    arr = lambda x: np.array(x, dtype=np.float32)                            # noqa: E731
+    flat = [arr(x) for x in g["grads"]]
+    sl = [[x[0:1].copy(), x[1:2].copy()] for x in flat]                       # what each server receives
+    order = np.array(ps["order"], np.int32)
+    n = np.array(ps["n_arrived"], np.int32)
+    for grads, slices in ((flat, False), (sl, True)):
+        for mode, key in ((oracle.EMA_PRE, "ema_pre"), (oracle.EMA_POST, "ema_post")):
+            th, em = arr(g["theta"]), arr(g["ema"])
+            assert oracle.async_apply_rows(ps["shard_off"], grads, order, th, em, slices=slices, n_arrived=n,
+                                           ema_mode=mode, gamma_t=g["gamma"], alpha=g["alpha"]) == oracle.OK
+            assert th.tolist() == ps["theta_out"] and em.tolist() == ps[key]
+        th = arr(g["theta"])
+        assert oracle.async_apply_rows(ps["shard_off"], grads, order, th, None, slices=slices, n_arrived=n,
+                                       gammas=arr(g["gammas"]), ema_mode=oracle.EMA_OFF) == oracle.OK
+        assert th.tolist() == ps["theta_out_gammas"]
+        th = arr(g["theta"])
+        assert oracle.async_apply_rows(ps["shard_off"], grads, order, th, None, slices=slices, n_arrived=n,
+                                       gscales=arr(ps["gscales"]), ema_mode=oracle.EMA_OFF, gamma_t=g["gamma"]) == oracle.OK
+        assert th.tolist() == ps["theta_out_scaled"]
+        th, em = arr(g["theta"]), arr(g["ema"])
+        assert oracle.async_apply_rows(ps["shard_off"], grads, order, th, em, slices=slices, n_arrived=n,
+                                       status=np.array(ps["failed_status"], np.int32), gamma_t=g["gamma"],
+                                       alpha=g["alpha"]) == oracle.OK
+        assert th.tolist() == ps["failed_theta_out"] and em.tolist() == ps["failed_ema_pre"]
+
+
+@pytest.mark.parametrize("opt", [oracle.SGD, oracle.MOMENTUM, oracle.RMSPROP_MOM])
+@pytest.mark.parametrize("bf16", [False, True])
+def test_per_server_rows_reduce_to_the_pinned_single_order_oracle_server_by_server(opt, bf16):
+    """Each server's slice must equal what the already pinned oracle_async_apply computes when it is given that
+    server's parameters alone, its own order, count, rates and (per-arrival) clip factors -- flat and sliced."""
+    from test_oracle_update import to_bf16_bits
+    rng = np.random.default_rng(810 + 2 * opt + bf16)
+    P, M, W = 1501, 6, 9
+    cuts = np.sort(rng.integers(0, P + 1, M - 1))
+    off = np.concatenate([[0], cuts, [P]]).astype(np.int64)
+    off[3] = off[2]                                                            # an empty server
+    off = np.sort(off)
+    theta = rng.normal(0, 0.02, P).astype(np.float32)
+    grads = [rng.normal(0, 1e-3, P).astype(np.float32) for _ in range(W)]
+    if bf16:
+        grads = [to_bf16_bits(x) for x in grads]
+    order = np.full((M, W), -1, np.int32)
+    n = rng.integers(0, W + 1, M).astype(np.int32)
+    for j in range(M):
+        order[j, :n[j]] = rng.permutation(W)[:n[j]]
+    status = np.zeros(M, np.int32)
+    status[4] = oracle.ETOOFEW
+    gammas = rng.uniform(0.01, 0.09, W).astype(np.float32)
+    gscales = rng.uniform(0.3, 1.0, W).astype(np.float32)
+    hp = dict(opt=opt, ema_mode=oracle.EMA_PRE, alpha=0.9999, mu=0.9, rho=0.9, eps=1.0)
+
+    def state():
+        return [theta.copy(), theta.copy(), np.ones(P, np.float32) if opt else None,
+                np.zeros(P, np.float32) if opt == oracle.RMSPROP_MOM else None]
+
+    want = state()
+    for j in range(M):
+        lo, hi = int(off[j]), int(off[j + 1])
+        if status[j] != 0 or hi == lo or n[j] == 0:
+            continue
+        sub = [None if a is None else a[lo:hi].copy() for a in want]
+        o = order[j, :n[j]].copy()
+        assert oracle.async_apply([0, hi - lo], [x[lo:hi].copy() for x in grads], o, *sub, gammas=gammas[:n[j]].copy(),
+                                  gscales=gscales[o].copy(), **hp) == oracle.OK
+        for a, b_ in zip(want, sub):
+            if a is not None:
+                a[lo:hi] = b_
+    got = state()
+    assert oracle.async_apply_rows(off, grads, order, *got, n_arrived=n, status=status, gammas=gammas, gscales=gscales,
+                                   **hp) == oracle.OK
+    sl = [[x[off[j]:off[j + 1]].copy() for j in range(M)] for x in grads]
+    got_s = state()
+    assert oracle.async_apply_rows(off, sl, order, *got_s, slices=True, n_arrived=n, status=status, gammas=gammas,
+                                   gscales=gscales, **hp) == oracle.OK
+    for a, b_, c in zip(want, got, got_s):
+        if a is not None:
+            assert np.array_equal(a, b_) and np.array_equal(a, c)
+    assert np.array_equal(got[0][off[4]:off[5]], theta[off[4]:off[5]])         # the failed server is untouched
+
+
+def test_per_server_rows_invalid_arguments():
+    g = _g()
+    arr = lambda x: np.array(x, dtype=np.float32)                            # noqa: E731
+    flat = [arr(x) for x in g["grads"]]
+    th = arr(g["theta"])
+    bad = np.array([[0, 3, 1], [1, 0, -1]], np.int32)
+    assert oracle.async_apply_rows([0, 1, 2], flat, bad, th, None, ema_mode=oracle.EMA_OFF) == oracle.EINVAL
+    ok = np.array([[0, 2, 1], [1, 0, 2]], np.int32)
+    assert oracle.async_apply_rows([0, 1, 2], flat, ok, th, None, n_arrived=np.array([3, 4], np.int32),
+                                   ema_mode=oracle.EMA_OFF) == oracle.EINVAL
+    assert th.tolist() == g["theta"]
