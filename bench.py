@@ -354,36 +354,39 @@ def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist
       first_n     one kept set of N per step (the headline; reading R11)
       per_server  Alg. 4 per server j: arrival [M][W] -> kept [M][N] (NEXT-1)
       timeout     keep every worker that arrived by --timeout seconds, divide by the count (NEXT-2)
-      async       Alg. 2: all W gradients one at a time in arrival order, one pass (NEXT-3)"""
+      async       Alg. 2: all W gradients one at a time in arrival order, one pass (NEXT-3)
+      async_per_server  Alg. 2 per server j: arrival [M][W] -> one order per server, over the work list"""
     cfg, dev = wl.cfg, wl.dev
     B = psync.binding
     slices = wl.layout == "slices"
-    rows = cfg.M if mode == "per_server" else 1
-    if mode == "per_server":
+    per_server = mode in ("per_server", "async_per_server")
+    is_async = mode in ("async", "async_per_server")
+    rows = cfg.M if per_server else 1
+    if per_server:
         arr_np = np.stack([synth.arrival_times_per_server(cfg, s) for s in range(K + Wm)])
     else:
         arr_np = np.stack([synth.arrival_times(cfg, s) for s in range(K + Wm)])
     arrivals = torch.from_numpy(arr_np).to(dev)
-    stride = cfg.W if mode in ("timeout", "async") else cfg.N
+    stride = cfg.W if (mode == "timeout" or is_async) else cfg.N
     d_kept = torch.full((rows, stride), -1, dtype=torch.int32, device=dev)
-    d_status = torch.full((rows,), 0 if mode == "async" else -9, dtype=torch.int32, device=dev)
+    d_status = torch.full((rows,), 0 if is_async else -9, dtype=torch.int32, device=dev)
     d_t_nth = torch.zeros(rows, dtype=torch.float32, device=dev)
-    d_n_kept = torch.zeros(rows, dtype=torch.int32, device=dev) if mode in ("timeout", "async") else None
-    use_tiles = slices or (mode == "per_server" and worklist)
+    d_n_kept = torch.zeros(rows, dtype=torch.int32, device=dev) if (mode == "timeout" or is_async) else None
+    use_tiles = slices or (mode == "per_server" and worklist) or mode == "async_per_server"
     steps_struct = []
     for tb in wl.tables:   # one psync_step per gradient set, built once (marshalling outside the timed region)
         st, keep = psync.make_step(wl.off, cfg.N, cfg.W, tb.grad_dtype, wl.theta, wl.ema, wl.s0, wl.s1, opt=cfg.opt,
                                    ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho,
                                    eps=cfg.eps, d_grads=tb.d_ptrs, d_kept=d_kept, d_status=d_status,
-                                   grid_ctas=args.grid_ctas, variant=variant, per_shard=(mode == "per_server"),
-                                   d_shard_off=wl.d_off if (mode == "per_server" or slices) else None,
+                                   grid_ctas=args.grid_ctas, variant=variant, per_shard=per_server,
+                                   d_shard_off=wl.d_off if (per_server or slices) else None,
                                    d_n_kept=d_n_kept,
                                    grad_layout=psync.PSYNC_GRADS_SLICES if slices else psync.PSYNC_GRADS_FLAT,
                                    d_tile_start=wl.d_tiles if use_tiles else None)
         steps_struct.append((st, keep))
     geo = psync.psync_launch_geometry(steps_struct[0][0])
     d_scales = d_clip_work = None
-    if mode == "async" and clip > 0:
+    if is_async and clip > 0:
         d_scales = torch.ones(cfg.W, dtype=torch.float32, device=dev)
         d_clip_work = torch.empty(psync.psync_clip_workspace_bytes(cfg.W, cfg.P, cfg.grad_dtype) // 8,
                                   dtype=torch.float64, device=dev)
@@ -406,6 +409,8 @@ def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist
             B.psync_select_first_n_sharded(arrivals[i], cfg.N, cfg.b, cfg.M, d_kept, d_status, None, None, i, stream)
         elif mode == "timeout":
             B.psync_select_timeout(arrivals[i], cfg.W, args.timeout, d_kept, d_n_kept, d_status, stream=stream)
+        elif mode == "async_per_server":
+            B.psync_order_by_arrival_sharded(arrivals[i], cfg.W, cfg.M, d_kept, d_n_kept, stream)
         else:
             B.psync_order_by_arrival(arrivals[i], cfg.W, d_kept, d_n_kept, stream)
 
@@ -419,7 +424,7 @@ def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist
         select(i)
         if ev is not None:
             ev[1].record(stream)
-        if mode == "async":
+        if is_async:
             if clip > 0:                 # A.3 (L313): global-norm clipping = one more pass over the W buffers
                 B.psync_clip_scales(wl.tables[i % n_sets], clip, d_scales, d_clip_work, stream)
             B.psync_async_apply(st, None, stream, d_gscale=d_scales if clip > 0 else None)
@@ -463,7 +468,7 @@ def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist
     assert bool((d_status == 0).all()) and bool(torch.isfinite(wl.theta[:4096]).all())
 
     # gradient elements aggregated per step: N*P, or (workers in time)*P for the time-out rule
-    if mode == "async":
+    if is_async:
         n_eff = float(cfg.W)                 # every gradient is applied (nothing is dropped in Alg. 2)
     elif mode == "timeout":
         n_eff = float(np.mean([(arr_np[Wm + k] <= args.timeout).sum() for k in range(K)]))
@@ -471,13 +476,13 @@ def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist
         n_eff = float(cfg.N)
     bytes_per_step = cfg.bytes_per_step + (n_eff - cfg.N) * cfg.P * cfg.grad_bytes
     launches_per_step = 2                    # selection (or arrival order) + the fused pass
-    if mode == "async" and clip > 0:
+    if is_async and clip > 0:
         bytes_per_step += cfg.W * cfg.P * cfg.grad_bytes      # the norm pass reads every buffer once more
         launches_per_step = 4                # + sum-of-squares chunks + clip factors
     return {"total_ms": total_ms, "ms_per_step": total_ms / K, "fused_ms": fused_ms, "select_ms": select_ms,
             "fused_list": fused_list, "n_eff": n_eff, "bytes_per_step": bytes_per_step, "units": n_eff * cfg.P * K,
             "clocks": clocks, "geo": geo, "launches_per_step": launches_per_step,
-            "kernel": "async_apply_kernel" if mode == "async" else
+            "kernel": ("async_sharded_kernel" if use_tiles else "async_apply_kernel") if is_async else
                       ("sharded_aggregate_update_ema" if use_tiles else "fused_aggregate_update_ema")}
 
 
@@ -503,10 +508,12 @@ def run_also(psync, args, wl3, stream, peak):
     out = []
     dev = wl3.dev
     cfg3 = wl3.cfg
-    for mode in ("per_server", "timeout", "async"):
+    for mode in ("per_server", "timeout", "async", "async_per_server"):
         wl3.reset_state()
         m = measure(psync, args, wl3, mode, K, Wm, stream, probe_every=2)
         note = None
+        if mode == "async_per_server":
+            note = "Alg. 2 per server j: one arrival order per server, flat buffers through the (server, tile) work list"
         if mode == "async":
             note = "Alg. 2, all W gradients one at a time in one pass; RMSProp: bound by instruction issue as well as HBM"
         out.append(short_entry(cfg3, mode, "flat", m, peak, note))
@@ -525,7 +532,7 @@ def run_also(psync, args, wl3, stream, peak):
     del wl3.tables[1:], wl3.sets[1:]     # keep one flat set for the cpu_baseline leg; make room
     torch.cuda.empty_cache()
     # per-(worker, server) slices of cfg3, one shared kept set and one kept row per server; many small servers
-    for M, modes in ((cfg3.M, ("first_n", "per_server")), (1000, ("per_server",)), (20000, ("per_server",))):
+    for M, modes in ((cfg3.M, ("first_n", "per_server", "async", "async_per_server")), (1000, ("per_server",)), (20000, ("per_server",))):
         cfg = cfg3 if M == cfg3.M else replace(cfg3, M=M, name=f"{cfg3.name}_M{M}")
         wl = Workload(psync, cfg, dev, 2, layout="slices")
         for mode in modes:
@@ -807,7 +814,7 @@ def main():
     ap.add_argument("--sweep-steps", type=int, default=5)
     ap.add_argument("--sweep-md", default="", help="--config cfg5: also write the table as markdown to this path")
     ap.add_argument("--sweep-filter", default="", help="--config cfg5: only points whose name contains this")
-    ap.add_argument("--mode", default="first_n", choices=["first_n", "per_server", "timeout", "async"],
+    ap.add_argument("--mode", default="first_n", choices=["first_n", "per_server", "timeout", "async", "async_per_server"],
                     help="first_n: the headline (one kept set); per_server: Alg. 4 per server j; timeout: L259; "
                          "async: Alg. 2, all W gradients one at a time in one pass")
     ap.add_argument("--timeout", type=float, default=1.5, help="seconds, for --mode timeout")

@@ -26,7 +26,7 @@ PSYNC_MAX_WORKERS = 1024
 PSYNC_TILE_UNITS = 256
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
-           "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_async_apply", "psync_staleness", "psync_step_device", "psync_clip_workspace_bytes",
+           "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_order_by_arrival_sharded", "psync_async_apply", "psync_staleness", "psync_step_device", "psync_clip_workspace_bytes",
            "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_host_ctx_create", "psync_host_ctx_destroy",
            "psync_step_host_ctx", "psync_launch_geometry", "psync_probe_read",
@@ -83,6 +83,8 @@ def lib() -> ctypes.CDLL:
         L.psync_step_device.restype = ctypes.c_int
         L.psync_order_by_arrival.argtypes = [vp, i32, vp, vp, vp]
         L.psync_order_by_arrival.restype = ctypes.c_int
+        L.psync_order_by_arrival_sharded.argtypes = [vp, i32, i32, vp, vp, vp]
+        L.psync_order_by_arrival_sharded.restype = ctypes.c_int
         L.psync_staleness.argtypes = [vp, i32, vp, vp, i32, vp, i32, vp, vp, vp, vp]
         L.psync_staleness.restype = ctypes.c_int
         L.psync_async_apply.argtypes = [ctypes.POINTER(psync_step), vp, vp, vp]
@@ -353,6 +355,19 @@ def psync_order_by_arrival(d_arrival: torch.Tensor, W: int, d_order: torch.Tenso
                                       _dptr(d_n_arrived, torch.int32, "d_n_arrived"), _stream(stream))
     if check and st != PSYNC_OK:
         raise PsyncError(st, "psync_order_by_arrival")
+    return st
+
+
+def psync_order_by_arrival_sharded(d_arrival: torch.Tensor, W: int, M: int, d_order: torch.Tensor,
+                                   d_n_arrived: torch.Tensor, stream=None, check: bool = True) -> int:
+    """Arrival order of Alg. 2 per parameter server j (include/psync.h: psync_order_by_arrival_sharded)."""
+    if d_arrival.numel() < M * W or d_order.numel() < M * W or d_n_arrived.numel() < M:
+        raise ValueError("need d_arrival [M][W], d_order [M][W], d_n_arrived [M]")
+    st = lib().psync_order_by_arrival_sharded(_dptr(d_arrival, torch.float32, "d_arrival"), W, M,
+                                              _dptr(d_order, torch.int32, "d_order"),
+                                              _dptr(d_n_arrived, torch.int32, "d_n_arrived"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_order_by_arrival_sharded")
     return st
 
 

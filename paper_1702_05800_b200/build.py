@@ -9,7 +9,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libpsync.so"
-SOURCES = ["psync_api.cu", "select_kernel.cu", "fused_kernel.cu", "sharded_kernel.cu", "async_kernel.cu", "helper_kernels.cu", "probe_kernels.cu"]
+SOURCES = ["psync_api.cu", "select_kernel.cu", "fused_kernel.cu", "sharded_kernel.cu", "async_kernel.cu", "async_sharded_kernel.cu", "helper_kernels.cu", "probe_kernels.cu"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-cudart", "static"]
 

@@ -20,40 +20,12 @@
 // refinement of MUFU.RSQ whose range check is a sticky flag outside the inner loop (psync_device.cuh),
 // and the loads of the next batch of gradients are in flight while the current batch is applied.
 
-#include "psync_device.cuh"
+#include "async_common.cuh"
 
 namespace psync {
 namespace {
 
 using namespace dev;
-
-template <bool BF16>
-__device__ __forceinline__ float unit_element(const uint4& r, int e) {
-  const uint32_t w = (&r.x)[BF16 ? (e >> 1) : e];
-  if (BF16) return __uint_as_float((e & 1) ? (w & 0xFFFF0000u) : (w << 16));
-  return __uint_as_float(w);
-}
-
-// elements 2i and 2i+1 of a 16-byte unit as one fp32x2 operand
-template <bool BF16>
-__device__ __forceinline__ float2 unit_pair(const uint4& r, int i) {
-  if (BF16) {
-    const uint32_t w = (&r.x)[i];
-    return make_float2(__uint_as_float(w << 16), __uint_as_float(w & 0xFFFF0000u));
-  }
-  return make_float2(__uint_as_float((&r.x)[2 * i]), __uint_as_float((&r.x)[2 * i + 1]));
-}
-
-// one arriving gradient (its 16-byte unit r) applied to the E parameters a thread holds, two at a time
-template <bool BF16, int OPT, int EMA, bool SCALED>
-__device__ __forceinline__ void apply_unit(const uint4& r, float scale, float gamma, float2* th, float2* em, float2* a0,
-                                           float2* a1, const PairCoeffs& c, unsigned& bad) {
-  constexpr int E = BF16 ? 8 : 4;
-  const float2 scale2 = dup2(scale), gamma2 = dup2(gamma);
-#pragma unroll
-  for (int i = 0; i < E / 2; ++i)
-    update_pair_g<OPT, EMA, SCALED>(unit_pair<BF16>(r, i), scale2, gamma2, th[i], em[i], a0[i], a1[i], c, bad);
-}
 
 // PIPE: software-pipelined batches (below); SCALED: per-worker clip factors are applied (else they are all 1)
 template <int THREADS, int U, int MINB, bool PIPE, bool BF16, int OPT, int EMA, bool SCALED>
@@ -198,12 +170,16 @@ __global__ void __launch_bounds__(THREADS, MINB) async_apply_kernel(const FusedP
 
 // K1c: rank sort of <= 1024 keys in one CTA.  Thread i owns worker i: its rank is the number of eligible
 // workers that come before it in (arrival, index) order; -0.0 == +0.0; non-finite = never arrived.
-__global__ void __launch_bounds__(1024) order_by_arrival_kernel(const float* __restrict__ arrival, int32_t W,
-                                                                int32_t* __restrict__ order,
-                                                                int32_t* __restrict__ n_arrived) {
+// One CTA per row: row r of arrival [rows][W] is what parameter server r saw (Alg. 2 is the program of one server j).
+__global__ void __launch_bounds__(1024) order_by_arrival_kernel(const float* __restrict__ arrival_rows, int32_t W,
+                                                                int32_t* __restrict__ order_rows,
+                                                                int32_t* __restrict__ n_arrived_rows) {
   __shared__ uint32_t s_key[kMaxWorkers];
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const float* arrival = arrival_rows + static_cast<int64_t>(blockIdx.x) * W;
+  int32_t* order = order_rows + static_cast<int64_t>(blockIdx.x) * W;
+  int32_t* n_arrived = n_arrived_rows + blockIdx.x;
   const int i = threadIdx.x;
   uint32_t key = 0xFFFFFFFFu;
   if (i < W) {
@@ -295,10 +271,10 @@ cudaError_t launch_async_apply(const FusedParams& p, int dtype, int opt, int ema
   return cudaLaunchKernelEx(&cfg, dtype == 1 ? pick_opt<true>(opt, ema, scaled) : pick_opt<false>(opt, ema, scaled), p);
 }
 
-cudaError_t launch_order_by_arrival(const float* d_arrival, int32_t W, int32_t* d_order, int32_t* d_n_arrived,
-                                    cudaStream_t stream) {
+cudaError_t launch_order_by_arrival(const float* d_arrival, int32_t W, int32_t rows, int32_t* d_order,
+                                    int32_t* d_n_arrived, cudaStream_t stream) {
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(1);
+  cfg.gridDim = dim3(static_cast<unsigned>(rows));
   cfg.blockDim = dim3(static_cast<unsigned>((W + 31) / 32 * 32));
   cfg.stream = stream;
   cudaLaunchAttribute attr[1];

@@ -1,0 +1,277 @@
+// K4s: Alg. 2 run LITERALLY PER PARAMETER SERVER j -- "Async-SGD Parameter Server j":
+//
+//     for t = 0, 1, ...:  wait for gradient G from any worker                       (L85)
+//                         theta(t+1)[j] <- theta(t)[j] - gamma_t G[j]               (L86)
+//                         ema(t)[j] = alpha ema(t-1)[j] + (1-alpha) theta(t)[j]     (L87)
+//
+// Every server runs this loop on its own: the order in which the gradients reach server j, and how many have
+// arrived, is server j's (the same remark as for Alg. 4), and what it receives is G[j] -- with
+// PSYNC_GRADS_SLICES one buffer per (worker, server), each its own allocation with its own alignment; with flat
+// buffers the range [off[j], off[j+1]) of each.  Row r(j) = per_shard ? j : 0 of the order table lists the workers
+// in the order server j applies them, K_j = n_kept ? n_kept[r] : N of them; gammas[i] is the rate of the server's
+// i-th iteration of this batch, gscales[k] worker k's clip factor (L313).
+//
+// Same CTA <-> data mapping as the synchronous shard-aware kernel K2s (sharded_kernel.cu): one CTA per (server,
+// tile) of the work list, the 128-bit gradient stream aligned to the server's first slice (head peel to its first
+// 128-byte line), narrower loads for a slice with another 16-byte phase, head / tail elements done one by one by the
+// server's first CTA.  Same arithmetic per element as K4 (async_kernel.cu: K dependent optimizer steps + EMAs in
+// registers, packed fp32x2, software-pipelined gradient batches): bit-identical to it and to K launches of the
+// synchronous step with N = 1 (tested).
+// What differs from K2s: the state cannot wait for the end of the gradient stream -- every arriving gradient is
+// applied to it -- so when theta's slice is not co-aligned with the gradient units (ragged cuts: off[j] + h is not a
+// multiple of 4) each warp moves theta / state / ema as coalesced 32-bit accesses and transposes them through shared
+// memory ONCE on the way in and once on the way out (K-independent; the gradient stream stays 128-bit).
+
+#include "async_common.cuh"
+
+namespace psync {
+namespace {
+
+using namespace dev;
+
+constexpr int kThreads = 256;  // = PSYNC_TILE_UNITS: one 16-byte unit per thread
+
+template <bool BF16, int OPT, int EMA, bool SCALED, int U, int MINB>
+__global__ void __launch_bounds__(kThreads, MINB) async_sharded_kernel(const FusedParams p) {
+  constexpr int E = BF16 ? 8 : 4;
+  constexpr int ESZ = BF16 ? 2 : 4;
+  constexpr int Q = E / 4;
+  constexpr int SEG = 32 * E;  // parameters of one warp's 32 units
+  __shared__ const char* s_ptr[kMaxWorkers];
+  __shared__ float s_gamma[kMaxWorkers];
+  __shared__ float s_scale[kMaxWorkers];
+  __shared__ __align__(16) float s_seg[kThreads * E];
+
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+
+  // ---- which (server, tile) is this CTA (as K2s) ---------------------------------------------------------
+  const int64_t b = blockIdx.x;
+  if (p.tile_start[p.M] != static_cast<int64_t>(gridDim.x)) return;  // a work list of another layout: touch nothing
+  const int j = upper_slot(p.tile_start, p.M, b);
+  const int64_t off_j = p.shard_off[j];
+  const int64_t len_j = p.shard_off[j + 1] - off_j;
+  const int64_t tile = b - p.tile_start[j];
+  const int row = p.per_shard ? j : 0;
+  if (p.status != nullptr && p.status[row] != 0) return;
+  const int K = p.n_kept ? p.n_kept[row] : p.N;  // gradients that have reached server j
+  if (K <= 0 || K > p.kept_stride || K > kMaxWorkers) return;  // nothing arrived, or a count nobody wrote
+
+  // ---- stage server j's arrivals: slice base pointers, rates, clip factors; the first slice fixes the phase ---
+  const int32_t* order = p.kept + static_cast<int64_t>(row) * p.kept_stride;
+  auto slice_ptr = [&](int k) -> const char* {
+    return p.slices ? static_cast<const char*>(p.grads[static_cast<int64_t>(k) * p.M + j])
+                    : static_cast<const char*>(p.grads[k]) + off_j * ESZ;
+  };
+  const unsigned ref = static_cast<unsigned>(reinterpret_cast<uintptr_t>(slice_ptr(order[0]))) & 127u;
+  const int h = static_cast<int>(((128u - ref) & 127u) / ESZ);  // head peel: elements before the first 128-byte line
+  unsigned mis = 0;
+  for (int i = threadIdx.x; i < K; i += kThreads) {
+    const int k = order[i];
+    const char* g = slice_ptr(k);
+    mis |= ((static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) ^ ref) & 15u);
+    s_ptr[i] = g + h * ESZ;  // unit u of this arrival = s_ptr[i] + 16 u
+    s_scale[i] = p.gscales ? p.gscales[k] : 1.0f;   // indexed by WORKER
+    s_gamma[i] = p.gammas ? p.gammas[i] : p.gamma;  // rate of the server's i-th iteration of this batch
+  }
+  const bool mixed = __syncthreads_or(static_cast<int>(mis)) != 0;
+
+  const int64_t nu = len_j > h ? (len_j - h) / E : 0;  // whole units of this server
+  const int64_t u0 = tile * kThreads;
+  const int64_t e0 = off_j + h;                        // parameter index of unit 0's first element
+
+  if (u0 < nu) {
+    const int64_t live_units = (nu - u0 < kThreads) ? (nu - u0) : kThreads;
+    const bool live = threadIdx.x < live_units;
+    const int64_t unit = live ? (u0 + threadIdx.x) : (nu - 1);  // dead slots re-read a valid unit, store nothing
+    const bool theta_vec = p.base_aligned != 0 && (e0 & 3) == 0;  // CTA-uniform: theta co-aligned with the units
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t seg_e0 = e0 + (u0 + warp * 32) * E;
+    const int64_t live_in_seg = (live_units - warp * 32) * E;  // <= 0 for a dead warp: it touches no memory
+    float* seg = s_seg + warp * SEG;
+
+    // one array's E values of this thread's unit: 128-bit when co-aligned, else coalesced 32-bit + warp transpose
+    auto load_arr = [&](const float* arr, float4* dst, float fill) {
+      if (theta_vec) {
+#pragma unroll
+        for (int q = 0; q < Q; ++q) dst[q] = ld_state16(arr + e0 + unit * E + 4 * q);
+      } else {
+#pragma unroll
+        for (int q = 0; q < E; ++q) {
+          const int idx = q * 32 + lane;
+          seg[idx] = idx < live_in_seg ? ld_state32(arr + seg_e0 + idx) : fill;
+        }
+        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < Q; ++q) dst[q] = *reinterpret_cast<const float4*>(&seg[(lane * Q + q) * 4]);
+        __syncwarp();
+      }
+    };
+    auto store_arr = [&](float* arr, const float4* src) {
+      if (theta_vec) {
+        if (live) {
+#pragma unroll
+          for (int q = 0; q < Q; ++q) st_state16(arr + e0 + unit * E + 4 * q, src[q]);
+        }
+      } else {
+#pragma unroll
+        for (int q = 0; q < Q; ++q) *reinterpret_cast<float4*>(&seg[(lane * Q + q) * 4]) = src[q];
+        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < E; ++q) {
+          const int idx = q * 32 + lane;
+          if (idx < live_in_seg) st_state32(arr + seg_e0 + idx, seg[idx]);
+        }
+        __syncwarp();
+      }
+    };
+
+    float4 th4[Q], em4[Q], a04[Q], a14[Q];
+    auto load_state = [&]() {
+      load_arr(p.theta, th4, 0.f);
+      if (EMA != EMA_OFF) load_arr(p.ema, em4, 0.f);
+      if (OPT != OPT_SGD) load_arr(p.s0, a04, 1.f);
+      if (OPT == OPT_RMSPROP_MOM) load_arr(p.s1, a14, 0.f);
+    };
+    load_state();
+    float2* th = reinterpret_cast<float2*>(th4);
+    float2* em = reinterpret_cast<float2*>(em4);
+    float2* a0 = reinterpret_cast<float2*>(a04);
+    float2* a1 = reinterpret_cast<float2*>(a14);
+    const PairCoeffs pc = make_pair_coeffs(p);
+
+    unsigned bad = 0;  // RMSProp: did any ms + eps leave the range of the unchecked packed rsqrt?
+    if (!mixed) {
+      // software-pipelined batches of U arrivals, as K4: the loads of batch b+1 fly while batch b is applied
+      const int n_batches = K / U;
+      uint4 cur[U], nxt[U];
+      if (n_batches > 0) {
+#pragma unroll
+        for (int v = 0; v < U; ++v) cur[v] = ldg_stream16(s_ptr[v] + unit * 16);
+      }
+      for (int bt = 0; bt < n_batches; ++bt) {
+        const int i = bt * U;
+        if (bt + 1 < n_batches) {
+#pragma unroll
+          for (int v = 0; v < U; ++v) nxt[v] = ldg_stream16(s_ptr[i + U + v] + unit * 16);
+        }
+#pragma unroll
+        for (int v = 0; v < U; ++v)
+          apply_unit<BF16, OPT, EMA, SCALED>(cur[v], s_scale[i + v], s_gamma[i + v], th, em, a0, a1, pc, bad);
+#pragma unroll
+        for (int v = 0; v < U; ++v) cur[v] = nxt[v];
+      }
+      for (int i = n_batches * U; i < K; ++i) {
+        const uint4 r = ldg_stream16(s_ptr[i] + unit * 16);
+        apply_unit<BF16, OPT, EMA, SCALED>(r, s_scale[i], s_gamma[i], th, em, a0, a1, pc, bad);
+      }
+    } else {
+#pragma unroll 2
+      for (int i = 0; i < K; ++i) {
+        const char* g = s_ptr[i];
+        const uint4 r = load_unit_any<BF16>(g + unit * 16, (reinterpret_cast<uintptr_t>(g) & 15u) == 0);
+        apply_unit<BF16, OPT, EMA, SCALED>(r, s_scale[i], s_gamma[i], th, em, a0, a1, pc, bad);
+      }
+    }
+    if (OPT == OPT_RMSPROP_MOM && __any_sync(0xFFFFFFFFu, rsqrt_pair_left_range(bad))) {
+      // Never on sane data: a non-finite or absurd second moment somewhere in this warp.  Nothing has been stored
+      // yet: the whole warp (the transposed loads are warp-collective) redoes its units from memory with the checked
+      // scalar update, which gives the same bits wherever the packed form was in range.
+      load_state();
+      float* ths = reinterpret_cast<float*>(th4);
+      float* ems = reinterpret_cast<float*>(em4);
+      float* a0s = reinterpret_cast<float*>(a04);
+      float* a1s = reinterpret_cast<float*>(a14);
+      for (int n = 0; n < K; ++n) {
+        const char* g = s_ptr[n];
+        const uint4 r = load_unit_any<BF16>(g + unit * 16, (reinterpret_cast<uintptr_t>(g) & 15u) == 0);
+#pragma unroll
+        for (int e = 0; e < E; ++e)
+          update_element_g<OPT, EMA>(unit_element<BF16>(r, e), s_scale[n], s_gamma[n], ths[e], ems[e], a0s[e], a1s[e], p);
+      }
+    }
+
+    store_arr(p.theta, th4);
+    if (EMA != EMA_OFF) store_arr(p.ema, em4);
+    if (OPT != OPT_SGD) store_arr(p.s0, a04);
+    if (OPT == OPT_RMSPROP_MOM) store_arr(p.s1, a14);
+  }
+
+  // ---- head and tail peel of server j, by its first CTA: K dependent updates per element, in registers --------
+  if (tile == 0) {
+    const int64_t tail0 = h + nu * E;
+    const int64_t n_head = h < len_j ? h : len_j;
+    const int64_t n_tail = len_j > tail0 ? len_j - tail0 : 0;
+    if (threadIdx.x < n_head + n_tail) {
+      const int64_t e = threadIdx.x < n_head ? threadIdx.x : tail0 + (threadIdx.x - n_head);
+      const int64_t i = off_j + e;
+      float th = p.theta[i];
+      float em = (EMA != EMA_OFF) ? p.ema[i] : 0.f;
+      float a0 = (OPT != OPT_SGD) ? p.s0[i] : 0.f;
+      float a1 = (OPT == OPT_RMSPROP_MOM) ? p.s1[i] : 0.f;
+      for (int n = 0; n < K; ++n)
+        update_element_g<OPT, EMA>(load_grad_scalar<BF16>(s_ptr[n] - h * ESZ, e), s_scale[n], s_gamma[n], th, em, a0, a1, p);
+      p.theta[i] = th;
+      if (EMA != EMA_OFF) p.ema[i] = em;
+      if (OPT != OPT_SGD) p.s0[i] = a0;
+      if (OPT == OPT_RMSPROP_MOM) p.s1[i] = a1;
+    }
+  }
+}
+
+// arrivals per batch and CTAs per SM: K4's shapes (async_kernel.cu), measured there
+struct Shape {
+  int unroll, minb;
+};
+constexpr Shape shape_for(bool bf16, int opt) {
+  return bf16 ? (opt == OPT_RMSPROP_MOM ? Shape{2, 2} : Shape{4, 3}) : (opt == OPT_RMSPROP_MOM ? Shape{3, 4} : Shape{4, 4});
+}
+
+using KernelFn = void (*)(const FusedParams);
+
+template <bool BF16, int OPT, int EMA>
+KernelFn pick_scaled(bool scaled) {
+  constexpr Shape S = shape_for(BF16, OPT);
+  return scaled ? async_sharded_kernel<BF16, OPT, EMA, true, S.unroll, S.minb>
+                : async_sharded_kernel<BF16, OPT, EMA, false, S.unroll, S.minb>;
+}
+template <bool BF16, int OPT>
+KernelFn pick_ema(int ema, bool scaled) {
+  switch (ema) {
+    case EMA_POST: return pick_scaled<BF16, OPT, EMA_POST>(scaled);
+    case EMA_PRE: return pick_scaled<BF16, OPT, EMA_PRE>(scaled);
+    default: return pick_scaled<BF16, OPT, EMA_OFF>(scaled);
+  }
+}
+template <bool BF16>
+KernelFn pick_opt(int opt, int ema, bool scaled) {
+  switch (opt) {
+    case OPT_SGD: return pick_ema<BF16, OPT_SGD>(ema, scaled);
+    case OPT_MOMENTUM: return pick_ema<BF16, OPT_MOMENTUM>(ema, scaled);
+    default: return pick_ema<BF16, OPT_RMSPROP_MOM>(ema, scaled);
+  }
+}
+
+}  // namespace
+
+int async_sharded_smem_bytes(int dtype) {
+  return static_cast<int>((sizeof(const char*) + 2 * sizeof(float)) * kMaxWorkers) + 4 * kThreads * (dtype == 1 ? 8 : 4);
+}
+
+cudaError_t launch_async_sharded(const FusedParams& p, int dtype, int opt, int ema, int64_t n_tiles, cudaStream_t stream) {
+  if (n_tiles <= 0) return cudaSuccess;
+  if (n_tiles > 0x7FFFFFFF) return cudaErrorInvalidConfiguration;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(static_cast<unsigned>(n_tiles));
+  cfg.blockDim = dim3(kThreads);
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  const bool scaled = p.gscales != nullptr;
+  return cudaLaunchKernelEx(&cfg, dtype == 1 ? pick_opt<true>(opt, ema, scaled) : pick_opt<false>(opt, ema, scaled), p);
+}
+
+}  // namespace psync

@@ -253,21 +253,38 @@ PSYNC_API int psync_order_by_arrival(const float* d_arrival, int32_t W, int32_t*
                            void* stream) {
   if (d_arrival == nullptr || d_order == nullptr || d_n_arrived == nullptr) return PSYNC_EINVAL;
   if (W < 1 || W > PSYNC_MAX_WORKERS) return PSYNC_EINVAL;
-  return psync::launch_order_by_arrival(d_arrival, W, d_order, d_n_arrived, static_cast<cudaStream_t>(stream)) ==
+  return psync::launch_order_by_arrival(d_arrival, W, 1, d_order, d_n_arrived, static_cast<cudaStream_t>(stream)) ==
+                 cudaSuccess
+             ? PSYNC_OK
+             : PSYNC_ECUDA;
+}
+
+PSYNC_API int psync_order_by_arrival_sharded(const float* d_arrival, int32_t W, int32_t M, int32_t* d_order,
+                                   int32_t* d_n_arrived, void* stream) {
+  if (d_arrival == nullptr || d_order == nullptr || d_n_arrived == nullptr) return PSYNC_EINVAL;
+  if (W < 1 || W > PSYNC_MAX_WORKERS || M < 1) return PSYNC_EINVAL;
+  return psync::launch_order_by_arrival(d_arrival, W, M, d_order, d_n_arrived, static_cast<cudaStream_t>(stream)) ==
                  cudaSuccess
              ? PSYNC_OK
              : PSYNC_ECUDA;
 }
 
 PSYNC_API int psync_async_apply(const psync_step* step, const float* d_gamma, const float* d_gscale, void* stream) {
-  const int st = check_step(step, true);
-  if (st != PSYNC_OK && !(st == PSYNC_EUNSUPPORTED && step->per_shard == 0)) return st;  // variant is ignored here
-  if (step->per_shard != 0 || step->grad_layout != PSYNC_GRADS_FLAT) return PSYNC_EUNSUPPORTED;
-  if (step->P == 0) return PSYNC_OK;
-  FusedParams p = make_params(step, 0, step->P, step->d_grads, step->d_kept, step->d_status);
+  if (step == nullptr) return PSYNC_EINVAL;
+  psync_step s = *step;
+  s.variant = 0;  // ignored here: Alg. 2's kernels have one launch shape per instance
+  const int st = check_step(&s, true);
+  if (st != PSYNC_OK) return st;
+  // Alg. 2 per server (one order row per server) walks the (server, tile) work list like the slices layout does
+  if (s.per_shard != 0 && s.d_tile_start == nullptr) return PSYNC_EUNSUPPORTED;  // no flat-index rows form of Alg. 2
+  if (s.P == 0) return PSYNC_OK;
+  FusedParams p = make_params(&s, 0, s.P, s.d_grads, s.d_kept, s.d_status);
   p.gammas = d_gamma;
   p.gscales = d_gscale;
-  const cudaError_t err = psync::launch_async_apply(p, step->grad_dtype, step->opt, step->ema_mode, step->grid_ctas,
+  const cudaError_t err =
+      wants_sharded(&s) ? psync::launch_async_sharded(p, s.grad_dtype, s.opt, s.ema_mode, sharded_tiles(&s),
+                                                      static_cast<cudaStream_t>(stream))
+                        : psync::launch_async_apply(p, s.grad_dtype, s.opt, s.ema_mode, s.grid_ctas,
                                                     static_cast<cudaStream_t>(stream));
   return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
 }

@@ -1,0 +1,350 @@
+"""GPU parity for Alg. 2 run PER PARAMETER SERVER j (K4s, "Async-SGD Parameter Server j"): one
+arrival order per server, the gradients as per-(worker, server) slices or flat buffers, over the (server, tile) work
+list -- against oracle.async_apply_rows through the C ABI.  Orders bit-exact; theta / state / ema within Alg. 2's
+tolerance (R21: rtol 1e-6 * max(10, K), atol 1e-6); bit-identity with the flat single-order kernel K4 is a
+property checked at any size."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1702_05800_b200 as psync
+from paper_1702_05800_b200 import synth
+
+from _harness import ATOL_STEP, STATE_NAMES, assert_close, to_np
+from test_gpu_slices import RAGGED, cut_slices, np_slices
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+BASE = synth.Config(name="async_rows", cfg_id=16, P=70_003, M=7, N=13, b=0, arrival_sigma=0.3, opt=synth.SGD,
+                    gamma=0.045, alpha=0.9999, mu=0.9, rho=0.9, eps=1.0, ema_mode=synth.EMA_PRE, steps=3)
+
+
+def rtol_async(K):
+    return 1e-6 * max(10, K)
+
+
+class RowsPair:
+    """One parameter-server state on the GPU and on the host, stepped by Alg. 2 server by server."""
+
+    def __init__(self, cfg, shard_off=None, state_misalign=0):
+        self.cfg = cfg
+        self.off = synth.shard_offsets(cfg) if shard_off is None else np.asarray(shard_off, dtype=np.int64)
+        self.M = self.off.size - 1
+
+        def place(t):
+            if t is None or not state_misalign:
+                return t
+            buf = torch.empty(t.numel() + 8, dtype=t.dtype, device=DEV)
+            view = buf[state_misalign:state_misalign + t.numel()]
+            view.copy_(t)
+            return view
+
+        self.theta = place(synth.init_theta(cfg, DEV))
+        s0, s1 = synth.init_state(cfg, DEV)
+        self.state0, self.state1 = place(s0), place(s1)
+        self.ema = place(self.theta.clone()) if cfg.ema_mode != synth.EMA_OFF else None
+        self.d_off = torch.from_numpy(self.off).to(DEV)
+        self.d_tiles = psync.psync_shard_worklist(self.d_off, cfg.grad_dtype)
+        self.host = {n: to_np(getattr(self, n)) for n in STATE_NAMES}
+        self.d_order = torch.full((self.M, cfg.W), -1, dtype=torch.int32, device=DEV)
+        self.d_n = torch.full((self.M,), -7, dtype=torch.int32, device=DEV)
+
+    def make_step(self, table, per_shard=True, slices=True, d_status=None, d_n=True, N=None):
+        cfg = self.cfg
+        return psync.make_step(self.off, cfg.W if N is None else N, cfg.W, table.grad_dtype, self.theta, self.ema,
+                               self.state0, self.state1, opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma,
+                               alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho, eps=cfg.eps, d_grads=table.d_ptrs,
+                               d_kept=self.d_order, d_status=d_status, per_shard=per_shard, d_shard_off=self.d_off,
+                               d_n_kept=self.d_n if d_n else None, kept_stride=cfg.W,
+                               grad_layout=psync.PSYNC_GRADS_SLICES if slices else psync.PSYNC_GRADS_FLAT,
+                               d_tile_start=self.d_tiles)
+
+    def compare_and_sync(self, what, K):
+        for n in STATE_NAMES:
+            g = getattr(self, n)
+            if g is not None:
+                assert_close(to_np(g), self.host[n], rtol_async(K), ATOL_STEP, f"{what} {n}")
+                self.host[n] = to_np(g)
+
+    def step(self, s, arrival_rows, slices=True, offset_of=None, gammas=None, gscales=None, status=None):
+        """arrival_rows fp32 [M][W]: order per server on the device, one K4s pass, the oracle server by server."""
+        cfg = self.cfg
+        flat = [synth.gradient(cfg, s, k, DEV) for k in range(cfg.W)]
+        sl = cut_slices(flat, self.off, offset_of) if slices else None
+        table = psync.make_slice_table(sl) if slices else psync.make_grad_table(flat)
+        psync.psync_order_by_arrival_sharded(torch.from_numpy(arrival_rows).to(DEV), cfg.W, self.M, self.d_order, self.d_n)
+        d_status = None if status is None else torch.from_numpy(status).to(DEV)
+        st, keep = self.make_step(table, slices=slices, d_status=d_status)
+        d_gamma = None if gammas is None else torch.from_numpy(gammas).to(DEV)
+        d_gscale = None if gscales is None else torch.from_numpy(gscales).to(DEV)
+        psync.psync_async_apply(st, d_gamma, d_gscale=d_gscale)
+        torch.cuda.synchronize()
+        order = np.full((self.M, cfg.W), -1, dtype=np.int32)
+        n_arr = np.zeros(self.M, dtype=np.int32)
+        for j in range(self.M):
+            o = oracle.order_by_arrival(arrival_rows[j])
+            order[j, :o.size], n_arr[j] = o, o.size
+        assert np.array_equal(self.d_n.cpu().numpy(), n_arr)
+        got = self.d_order.cpu().numpy()
+        for j in range(self.M):                      # entries past the count are not written
+            assert np.array_equal(got[j, :n_arr[j]], order[j, :n_arr[j]]), f"server {j}: arrival order differs"
+        h = self.host
+        safe = np.where(order < 0, 0, order)
+        rc = oracle.async_apply_rows(self.off, np_slices(sl) if slices else [synth.as_numpy_grad(g) for g in flat], safe,
+                                     h["theta"], h["ema"], h["state0"], h["state1"], slices=slices, per_shard=True,
+                                     n_arrived=n_arr, status=status, gammas=gammas, gscales=gscales, opt=cfg.opt,
+                                     ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho,
+                                     eps=cfg.eps)
+        assert rc == oracle.OK
+        self.compare_and_sync(f"{cfg.name} step {s}", int(n_arr.max(initial=1)))
+        return order, n_arr
+
+
+# ------------------------------------------------------------------ K1c per server
+def test_order_by_arrival_sharded_matches_the_oracle_row_by_row():
+    rng = np.random.default_rng(1600)
+    M, W = 37, 106
+    a = rng.lognormal(0, 0.3, (M, W)).astype(np.float32)
+    a[rng.random((M, W)) < 0.2] = 1.0
+    a[rng.random((M, W)) < 0.05] = np.inf
+    a[rng.random((M, W)) < 0.03] = np.nan
+    a[5] = np.nan                                    # nothing reached server 5
+    d_order = torch.full((M, W), -1, dtype=torch.int32, device=DEV)
+    d_n = torch.full((M,), -7, dtype=torch.int32, device=DEV)
+    psync.psync_order_by_arrival_sharded(torch.from_numpy(a).to(DEV), W, M, d_order, d_n)
+    got, n = d_order.cpu().numpy(), d_n.cpu().numpy()
+    for j in range(M):
+        want = oracle.order_by_arrival(a[j])
+        assert n[j] == want.size and np.array_equal(got[j, :want.size], want) and (got[j, want.size:] == -1).all()
+    assert n[5] == 0
+    L = psync.binding.lib()
+    assert L.psync_order_by_arrival_sharded(None, 4, 2, None, None, None) == psync.PSYNC_EINVAL
+    assert L.psync_order_by_arrival_sharded(8, 4, 0, 8, 8, None) == psync.PSYNC_EINVAL
+    assert L.psync_order_by_arrival_sharded(8, 1025, 1, 8, 8, None) == psync.PSYNC_EINVAL
+
+
+# ------------------------------------------------------------------ every template instance, lock-step
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+@pytest.mark.parametrize("opt", [synth.SGD, synth.MOMENTUM, synth.RMSPROP_MOM])
+@pytest.mark.parametrize("ema_mode", [synth.EMA_PRE, synth.EMA_POST, synth.EMA_OFF])
+def test_every_template_instance_lockstep_on_ragged_slices(dtype, opt, ema_mode):
+    cfg = replace(BASE, grad_dtype=dtype, opt=opt, ema_mode=ema_mode, name=f"arows_d{dtype}_o{opt}_e{ema_mode}")
+    pair = RowsPair(cfg, shard_off=RAGGED)
+    rng = np.random.default_rng(11)
+    for s in range(3):
+        # step 0: allocator-aligned slices (theta's slices are not co-aligned: transposed state); step 1: one odd
+        # phase per server (head peel), per-iteration rates, two workers never reach some servers; step 2: phases
+        # differ between workers (narrow loads), clip factors per worker
+        offs = [None, lambda k, j: (3 * j + 1) % 8, lambda k, j: (5 * k + 3 * j) % 8][s]
+        a = synth.arrival_times_per_server(cfg, s, server_sigma=0.3)
+        gammas = gscales = None
+        if s == 1:
+            a[1::2, 2] = np.inf
+            a[4:, 9] = np.nan
+            gammas = rng.uniform(0.01, 0.09, cfg.W).astype(np.float32)
+        if s == 2:
+            gscales = rng.uniform(0.25, 1.0, cfg.W).astype(np.float32)
+        order, n = pair.step(s, a, offset_of=offs, gammas=gammas, gscales=gscales)
+        assert len({tuple(r) for r in order.tolist()}) > 1, "the servers should not all see the same order"
+
+
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+@pytest.mark.parametrize("opt", [synth.MOMENTUM, synth.RMSPROP_MOM])
+def test_flat_buffers_with_one_order_row_per_server(dtype, opt):
+    cfg = replace(BASE, grad_dtype=dtype, opt=opt, name=f"arows_flat_d{dtype}_o{opt}")
+    pair = RowsPair(cfg, shard_off=RAGGED)
+    for s in range(2):
+        pair.step(s, synth.arrival_times_per_server(cfg, s, server_sigma=0.3), slices=False)
+
+
+@pytest.mark.parametrize("K", [1, 2, 3, 4, 5, 7, 8, 9, 12, 33])
+def test_arrival_counts_cross_the_batch_boundaries(K):
+    cfg = replace(BASE, N=K, P=20_011, M=3, opt=synth.RMSPROP_MOM, name=f"arows_K{K}")
+    RowsPair(cfg).step(0, synth.arrival_times_per_server(cfg, 0, server_sigma=0.3))
+
+
+def test_aligned_cuts_take_the_128_bit_state_path_and_misaligned_state_does_not():
+    cfg = replace(BASE, P=65_536, M=4, ragged=False, opt=synth.RMSPROP_MOM, name="arows_aligned")
+    RowsPair(cfg).step(0, synth.arrival_times_per_server(cfg, 0, server_sigma=0.3))
+    RowsPair(cfg, state_misalign=1).step(0, synth.arrival_times_per_server(cfg, 0, server_sigma=0.3))
+
+
+def test_failed_and_empty_servers_are_left_untouched():
+    cfg = replace(BASE, opt=synth.MOMENTUM, name="arows_failed")
+    pair = RowsPair(cfg, shard_off=RAGGED)
+    a = synth.arrival_times_per_server(cfg, 0, server_sigma=0.3)
+    a[3] = np.inf                                                    # nothing reached server 3: K_3 = 0
+    status = np.zeros(pair.M, dtype=np.int32)
+    status[5] = psync.PSYNC_ETOOFEW                                  # server 5 is marked failed
+    before = {n: to_np(getattr(pair, n)) for n in STATE_NAMES}
+    order, n = pair.step(0, a, status=status)
+    assert n[3] == 0
+    for j in (3, 5):
+        lo, hi = int(pair.off[j]), int(pair.off[j + 1])
+        for nm in STATE_NAMES:
+            if before[nm] is not None:
+                assert np.array_equal(to_np(getattr(pair, nm))[lo:hi], before[nm][lo:hi]), (j, nm)
+    lo, hi = int(pair.off[4]), int(pair.off[5])
+    assert not np.array_equal(to_np(pair.theta)[lo:hi], before["theta"][lo:hi])
+
+
+def test_one_shared_order_on_slices_equals_the_flat_single_order_kernel_bit_for_bit():
+    """per_shard = 0 with the slices layout: every server applies row 0.  K4s must give the bits of K4."""
+    for dtype, opt in ((synth.F32, synth.RMSPROP_MOM), (synth.BF16, synth.MOMENTUM), (synth.F32, synth.SGD)):
+        cfg = replace(BASE, P=200_003, M=9, N=11, grad_dtype=dtype, opt=opt, name="arows_vs_k4")
+        a = synth.arrival_times(cfg, 0)
+        flat = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+        rng = np.random.default_rng(5)
+        gam = torch.from_numpy(rng.uniform(0.01, 0.09, cfg.W).astype(np.float32)).to(DEV)
+        gsc = torch.from_numpy(rng.uniform(0.25, 1.0, cfg.W).astype(np.float32)).to(DEV)
+        one = RowsPair(cfg)
+        d_order = torch.full((cfg.W,), -1, dtype=torch.int32, device=DEV)
+        d_n = torch.full((1,), -7, dtype=torch.int32, device=DEV)
+        psync.psync_order_by_arrival(torch.from_numpy(a).to(DEV), cfg.W, d_order, d_n)
+        t_flat = psync.make_grad_table(flat)
+        st, keep = psync.make_step(one.off, cfg.W, cfg.W, t_flat.grad_dtype, one.theta, one.ema, one.state0, one.state1,
+                                   opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu,
+                                   rho=cfg.rho, eps=cfg.eps, d_grads=t_flat.d_ptrs, d_kept=d_order, d_n_kept=d_n,
+                                   kept_stride=cfg.W)
+        psync.psync_async_apply(st, gam, d_gscale=gsc)
+        two = RowsPair(cfg)
+        sl = cut_slices(flat, two.off, lambda k, j: (k + j) % 4)
+        t_sl = psync.make_slice_table(sl)
+        two.d_order[0].copy_(d_order)
+        two.d_n[:1].copy_(d_n)
+        st2, keep2 = two.make_step(t_sl, per_shard=False)
+        psync.psync_async_apply(st2, gam, d_gscale=gsc)
+        torch.cuda.synchronize()
+        for n in STATE_NAMES:
+            if getattr(one, n) is not None:
+                assert np.array_equal(to_np(getattr(one, n)), to_np(getattr(two, n))), (dtype, opt, n)
+
+
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+@pytest.mark.parametrize("side", ["low", "high"])
+def test_second_moment_outside_the_packed_rsqrt_range_is_redone_with_the_checked_routine(dtype, side):
+    """RMSProp: on a sparse set of elements ms + eps stays below 2^-63 (ms_0 = eps = 1e-30, gradients ~1e-12) or above
+    2^65 (ms_0 = 1e30) for the whole pass: outside the range of the unchecked packed rsqrt, so the warp redoes its units
+    from memory with the checked scalar routine.  Both K4s and K4."""
+    if side == "low":
+        cfg = replace(BASE, grad_dtype=dtype, opt=synth.RMSPROP_MOM, eps=1e-30, gamma=1e-4, grad_dist=("normal", 1e-12),
+                      name=f"arows_range_low_d{dtype}")
+        ms0 = 1e-30
+    else:
+        cfg = replace(BASE, grad_dtype=dtype, opt=synth.RMSPROP_MOM, name=f"arows_range_high_d{dtype}")
+        ms0 = 1e30
+    rng = np.random.default_rng(21)
+    tiny = torch.from_numpy(np.unique(rng.integers(0, cfg.P, 400))).to(DEV)
+    pair = RowsPair(cfg, shard_off=RAGGED)
+    pair.state0[tiny] = ms0
+    pair.host["state0"] = to_np(pair.state0)
+    pair.step(0, synth.arrival_times_per_server(cfg, 0, server_sigma=0.3))
+    assert bool(torch.isfinite(pair.theta).all()) and bool(torch.isfinite(pair.state1).all())
+    # the flat single-order kernel on the same data
+    one = RowsPair(cfg, shard_off=[0, cfg.P])
+    one.state0[tiny] = ms0
+    one.host["state0"] = to_np(one.state0)
+    a = synth.arrival_times(cfg, 0)
+    flat = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    table = psync.make_grad_table(flat)
+    d_order = torch.full((cfg.W,), -1, dtype=torch.int32, device=DEV)
+    d_n = torch.full((1,), -7, dtype=torch.int32, device=DEV)
+    psync.psync_order_by_arrival(torch.from_numpy(a).to(DEV), cfg.W, d_order, d_n)
+    st, keep = psync.make_step(one.off, cfg.W, cfg.W, table.grad_dtype, one.theta, one.ema, one.state0, one.state1,
+                               opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu,
+                               rho=cfg.rho, eps=cfg.eps, d_grads=table.d_ptrs, d_kept=d_order, d_n_kept=d_n,
+                               kept_stride=cfg.W)
+    psync.psync_async_apply(st)
+    torch.cuda.synchronize()
+    h = one.host
+    order = oracle.order_by_arrival(a)
+    rc = oracle.async_apply(one.off, [synth.as_numpy_grad(g) for g in flat], order, h["theta"], h["ema"], h["state0"],
+                            h["state1"], opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha,
+                            mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
+    assert rc == oracle.OK
+    one.compare_and_sync("K4 range", order.size)
+
+
+def test_many_tiny_servers_and_the_maximum_worker_count():
+    """M = 600 ragged servers of ~50 parameters (every tile mostly empty, most of every server is head / tail peel);
+    then W = 1024 arrivals on a small vector (the shared tables are full)."""
+    cfg = replace(BASE, P=30_011, M=600, opt=synth.MOMENTUM, name="arows_tiny_servers")
+    RowsPair(cfg).step(0, synth.arrival_times_per_server(cfg, 0, server_sigma=0.3))
+    cfg = replace(BASE, N=1024, P=3_001, M=3, opt=synth.MOMENTUM, grad_dist=("normal", 1e-4), name="arows_K1024")
+    order, n = RowsPair(cfg).step(0, synth.arrival_times_per_server(cfg, 0, server_sigma=0.3))
+    assert (n == 1024).all()
+
+
+def test_abi_validation_and_a_foreign_work_list_touch_nothing():
+    cfg = replace(BASE, P=4096, M=2, N=3, ragged=False, name="arows_abi")
+    pair = RowsPair(cfg)
+    flat = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    table = psync.make_slice_table(cut_slices(flat, pair.off))
+    pair.d_order[:] = torch.arange(3, dtype=torch.int32, device=DEV)
+    pair.d_n.fill_(3)
+    before = to_np(pair.theta)
+    st, keep = pair.make_step(table)
+    st.d_tile_start = None
+    assert psync.psync_async_apply(st, check=False) == psync.PSYNC_EINVAL          # slices need the work list
+    st, keep = pair.make_step(psync.make_grad_table(flat), slices=False)
+    st.d_tile_start = None
+    assert psync.psync_async_apply(st, check=False) == psync.PSYNC_EUNSUPPORTED    # rows without a work list
+    st, keep = pair.make_step(table)
+    st.d_shard_off = None
+    assert psync.psync_async_apply(st, check=False) == psync.PSYNC_EINVAL
+    # a work list built for the other gradient dtype: detected on the device
+    pair.d_tiles = psync.psync_shard_worklist(torch.from_numpy(np.array([0, 2048, 8192], np.int64)).to(DEV), synth.F32)
+    st, keep = pair.make_step(table)
+    assert psync.psync_async_apply(st) == psync.PSYNC_OK
+    # a count nobody wrote
+    pair.d_tiles = psync.psync_shard_worklist(pair.d_off, synth.F32)
+    pair.d_n.fill_(-7)
+    st, keep = pair.make_step(table)
+    assert psync.psync_async_apply(st) == psync.PSYNC_OK
+    pair.d_n.fill_(4)                                                               # > kept_stride = W = 3
+    assert psync.psync_async_apply(st) == psync.PSYNC_OK
+    torch.cuda.synchronize()
+    assert np.array_equal(to_np(pair.theta), before)
+    pair.d_n.fill_(3)
+    assert psync.psync_async_apply(st) == psync.PSYNC_OK
+    torch.cuda.synchronize()
+    assert not np.array_equal(to_np(pair.theta), before)
+
+
+def test_full_size_cfg3_shape_every_element_on_separately_allocated_slices():
+    """cfg3's shape (P = 25,165,824, M = 20 ragged, W = 106, RMSProp + EMA) through Alg. 2 per server: 2,120 separately
+    allocated slices (every third one placed 1-3 elements off its allocation), 20 different arrival orders, EVERY
+    element against the oracle."""
+    cfg = replace(synth.PAPER_RMSPROP, N=106, b=0, ema_mode=synth.EMA_PRE, name="arows_cfg3")
+    free, _ = torch.cuda.mem_get_info()
+    if cfg.footprint_bytes * 1.25 > free:
+        pytest.skip("not enough free HBM")
+    pair = RowsPair(cfg)
+    sl = []
+    for k in range(cfg.W):
+        g = synth.gradient(cfg, 0, k, DEV)
+        sl.append(cut_slices([g], pair.off, lambda _k, j, k=k: ((k + j) % 4) if (k + j) % 3 == 0 else 0)[0])
+        del g
+    table = psync.make_slice_table(sl)
+    a = synth.arrival_times_per_server(cfg, 0)
+    a[7, 13] = np.inf                                                 # worker 13's slice never reaches server 7
+    psync.psync_order_by_arrival_sharded(torch.from_numpy(a).to(DEV), cfg.W, pair.M, pair.d_order, pair.d_n)
+    st, keep = pair.make_step(table)
+    psync.psync_async_apply(st)
+    torch.cuda.synchronize()
+    order = np.zeros((pair.M, cfg.W), dtype=np.int32)
+    n_arr = np.zeros(pair.M, dtype=np.int32)
+    for j in range(pair.M):
+        o = oracle.order_by_arrival(a[j])
+        order[j, :o.size], n_arr[j] = o, o.size
+    assert n_arr[7] == 105 and np.array_equal(pair.d_n.cpu().numpy(), n_arr)
+    h = pair.host
+    rc = oracle.async_apply_rows(pair.off, np_slices(sl), order, h["theta"], h["ema"], h["state0"], h["state1"],
+                                 slices=True, per_shard=True, n_arrived=n_arr, opt=cfg.opt, ema_mode=cfg.ema_mode,
+                                 gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
+    assert rc == oracle.OK
+    pair.compare_and_sync("async rows cfg3 (every element)", 106)
