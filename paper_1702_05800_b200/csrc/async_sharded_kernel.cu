@@ -31,109 +31,173 @@ using namespace dev;
 
 constexpr int kThreads = 256;  // = PSYNC_TILE_UNITS: one 16-byte unit per thread
 
-template <bool BF16, int OPT, int EMA, bool SCALED, int U, int MINB>
+// Where this thread's unit and its warp's segment lie, derived from four CTA-uniform numbers.  The kernel derives it
+// twice: before the gradient loop from registers, and after it from a copy of the four numbers in shared memory read
+// through a volatile pointer -- so that none of these addresses stays live across the loop.  (With them live, ptxas
+// ran out of the 64 registers that 4 CTAs/SM allow, merged the loop's two gradient buffers into one and loaded the
+// next batch only after the current one was consumed: the warp then waited for every batch, 48 % of all stall
+// samples and 8 % of the kernel; ncu, profiles/r2_async.md.)
+template <int E>
+struct Geom {
+  int64_t nu, u0, e0, unit, seg_e0, live_in_seg;
+  bool live, theta_vec;
+  int lane;
+  float* seg;
+};
+template <int E>
+__device__ __forceinline__ Geom<E> make_geom(int64_t off_j, int64_t len_j, int h, int64_t tile, int base_aligned,
+                                             float* s_seg) {
+  Geom<E> g;
+  g.nu = len_j > h ? (len_j - h) / E : 0;  // whole units of this server
+  g.u0 = tile * kThreads;
+  g.e0 = off_j + h;                        // parameter index of unit 0's first element
+  const int64_t live_units = (g.nu - g.u0 < kThreads) ? (g.nu - g.u0) : kThreads;
+  g.live = threadIdx.x < live_units;
+  g.unit = g.live ? (g.u0 + threadIdx.x) : (g.nu - 1);  // dead slots re-read a valid unit, store nothing
+  g.theta_vec = base_aligned != 0 && (g.e0 & 3) == 0;   // CTA-uniform: theta co-aligned with the units
+  const int warp = threadIdx.x >> 5;
+  g.lane = threadIdx.x & 31;
+  g.seg_e0 = g.e0 + (g.u0 + warp * 32) * E;
+  g.live_in_seg = (live_units - warp * 32) * E;  // <= 0 for a dead warp: it touches no memory
+  g.seg = s_seg + warp * (32 * E);
+  return g;
+}
+
+// one array's E values of this thread's unit: 128-bit when co-aligned, else coalesced 32-bit + warp transpose
+template <int E>
+__device__ __forceinline__ void load_arr(const Geom<E>& g, const float* arr, float4* dst, float fill) {
+  constexpr int Q = E / 4;
+  if (g.theta_vec) {
+#pragma unroll
+    for (int q = 0; q < Q; ++q) dst[q] = ld_state16(arr + g.e0 + g.unit * E + 4 * q);
+  } else {
+#pragma unroll
+    for (int q = 0; q < E; ++q) {
+      const int idx = q * 32 + g.lane;
+      g.seg[idx] = idx < g.live_in_seg ? ld_state32(arr + g.seg_e0 + idx) : fill;
+    }
+    __syncwarp();
+#pragma unroll
+    for (int q = 0; q < Q; ++q) dst[q] = *reinterpret_cast<const float4*>(&g.seg[(g.lane * Q + q) * 4]);
+    __syncwarp();
+  }
+}
+template <int E>
+__device__ __forceinline__ void store_arr(const Geom<E>& g, float* arr, const float4* src) {
+  constexpr int Q = E / 4;
+  if (g.theta_vec) {
+    if (g.live) {
+#pragma unroll
+      for (int q = 0; q < Q; ++q) st_state16(arr + g.e0 + g.unit * E + 4 * q, src[q]);
+    }
+  } else {
+#pragma unroll
+    for (int q = 0; q < Q; ++q) *reinterpret_cast<float4*>(&g.seg[(g.lane * Q + q) * 4]) = src[q];
+    __syncwarp();
+#pragma unroll
+    for (int q = 0; q < E; ++q) {
+      const int idx = q * 32 + g.lane;
+      if (idx < g.live_in_seg) st_state32(arr + g.seg_e0 + idx, g.seg[idx]);
+    }
+    __syncwarp();
+  }
+}
+template <int E, int OPT, int EMA>
+__device__ __forceinline__ void load_state(const Geom<E>& g, const FusedParams& p, float4* th4, float4* em4, float4* a04,
+                                           float4* a14) {
+  load_arr<E>(g, p.theta, th4, 0.f);
+  if (EMA != EMA_OFF) load_arr<E>(g, p.ema, em4, 0.f);
+  if (OPT != OPT_SGD) load_arr<E>(g, p.s0, a04, 1.f);
+  if (OPT == OPT_RMSPROP_MOM) load_arr<E>(g, p.s1, a14, 0.f);
+}
+
+template <bool BF16, int OPT, int EMA, bool SCALED, int U, int MINB, bool PIPE>
 __global__ void __launch_bounds__(kThreads, MINB) async_sharded_kernel(const FusedParams p) {
   constexpr int E = BF16 ? 8 : 4;
   constexpr int ESZ = BF16 ? 2 : 4;
   constexpr int Q = E / 4;
-  constexpr int SEG = 32 * E;  // parameters of one warp's 32 units
   __shared__ const char* s_ptr[kMaxWorkers];
   __shared__ float s_gamma[kMaxWorkers];
   __shared__ float s_scale[kMaxWorkers];
   __shared__ __align__(16) float s_seg[kThreads * E];
+  __shared__ int64_t s_meta[4];  // off_j, len_j, h, tile: what Geom is derived from, re-read after the gradient loop
 
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
-  // ---- which (server, tile) is this CTA (as K2s) ---------------------------------------------------------
-  const int64_t b = blockIdx.x;
-  if (p.tile_start[p.M] != static_cast<int64_t>(gridDim.x)) return;  // a work list of another layout: touch nothing
-  const int j = upper_slot(p.tile_start, p.M, b);
-  const int64_t off_j = p.shard_off[j];
-  const int64_t len_j = p.shard_off[j + 1] - off_j;
-  const int64_t tile = b - p.tile_start[j];
-  const int row = p.per_shard ? j : 0;
-  if (p.status != nullptr && p.status[row] != 0) return;
-  const int K = p.n_kept ? p.n_kept[row] : p.N;  // gradients that have reached server j
-  if (K <= 0 || K > p.kept_stride || K > kMaxWorkers) return;  // nothing arrived, or a count nobody wrote
+  int K;
+  bool mixed;
+  {
+    // ---- which (server, tile) is this CTA; its row of the order table ---------------------------------------
+    // The prologue is a chain of dependent loads that every CTA pays before its first gradient byte moves, so it is
+    // kept SHORT: the server by a warp-wide search (1-2 levels), then everything that only needs j in ONE level --
+    // shard bounds, tile origin, status, count, this thread's entry of the order row and the row's first entry --
+    // loaded before any of it is checked (all of these addresses are valid whatever the values turn out to be),
+    // then the slice pointers in one more level.
+    const int64_t b = blockIdx.x;
+    const int64_t total = p.tile_start[p.M];
+    const int j = upper_slot_warp(p.tile_start, p.M, b);
+    const int row = p.per_shard ? j : 0;
+    const int32_t* order = p.kept + static_cast<int64_t>(row) * p.kept_stride;
+    const int64_t off_j = p.shard_off[j];
+    const int64_t off_j1 = p.shard_off[j + 1];
+    const int64_t tile0 = p.tile_start[j];
+    const int st = p.status != nullptr ? p.status[row] : 0;
+    K = p.n_kept != nullptr ? p.n_kept[row] : p.N;  // gradients that have reached server j
+    const int k_first = order[0];
+    const int i_mine = static_cast<int>(threadIdx.x) < p.kept_stride ? static_cast<int>(threadIdx.x) : p.kept_stride - 1;
+    const int k_mine = order[i_mine];
+    if (total != static_cast<int64_t>(gridDim.x)) return;  // a work list of another layout: touch nothing
+    if (st != 0) return;                                   // this server applies nothing
+    if (K <= 0 || K > p.kept_stride || K > kMaxWorkers) return;  // nothing arrived, or a count nobody wrote
+    const int64_t len_j = off_j1 - off_j;
+    const int64_t tile = b - tile0;
 
-  // ---- stage server j's arrivals: slice base pointers, rates, clip factors; the first slice fixes the phase ---
-  const int32_t* order = p.kept + static_cast<int64_t>(row) * p.kept_stride;
-  auto slice_ptr = [&](int k) -> const char* {
-    return p.slices ? static_cast<const char*>(p.grads[static_cast<int64_t>(k) * p.M + j])
-                    : static_cast<const char*>(p.grads[k]) + off_j * ESZ;
-  };
-  const unsigned ref = static_cast<unsigned>(reinterpret_cast<uintptr_t>(slice_ptr(order[0]))) & 127u;
-  const int h = static_cast<int>(((128u - ref) & 127u) / ESZ);  // head peel: elements before the first 128-byte line
-  unsigned mis = 0;
-  for (int i = threadIdx.x; i < K; i += kThreads) {
-    const int k = order[i];
-    const char* g = slice_ptr(k);
-    mis |= ((static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) ^ ref) & 15u);
-    s_ptr[i] = g + h * ESZ;  // unit u of this arrival = s_ptr[i] + 16 u
-    s_scale[i] = p.gscales ? p.gscales[k] : 1.0f;   // indexed by WORKER
-    s_gamma[i] = p.gammas ? p.gammas[i] : p.gamma;  // rate of the server's i-th iteration of this batch
+    // ---- stage server j's arrivals: slice base pointers, rates, clip factors; the first slice fixes the phase -
+    auto slice_ptr = [&](int k) -> const char* {
+      return p.slices ? static_cast<const char*>(p.grads[static_cast<int64_t>(k) * p.M + j])
+                      : static_cast<const char*>(p.grads[k]) + off_j * ESZ;
+    };
+    const char* g_first = slice_ptr(k_first);
+    const char* g_mine = static_cast<int>(threadIdx.x) < K ? slice_ptr(k_mine) : g_first;
+    const unsigned ref = static_cast<unsigned>(reinterpret_cast<uintptr_t>(g_first)) & 127u;
+    const int h = static_cast<int>(((128u - ref) & 127u) / ESZ);  // head peel: elements before the first 128-byte line
+    unsigned mis = 0;
+    for (int i = threadIdx.x; i < K; i += kThreads) {
+      const int k = i < kThreads ? k_mine : order[i];
+      const char* g = i < kThreads ? g_mine : slice_ptr(k);
+      mis |= ((static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) ^ ref) & 15u);
+      s_ptr[i] = g + h * ESZ;  // unit u of this arrival = s_ptr[i] + 16 u
+      s_scale[i] = p.gscales ? p.gscales[k] : 1.0f;   // indexed by WORKER
+      s_gamma[i] = p.gammas ? p.gammas[i] : p.gamma;  // rate of the server's i-th iteration of this batch
+    }
+    if (threadIdx.x == 0) {
+      s_meta[0] = off_j;
+      s_meta[1] = len_j;
+      s_meta[2] = h;
+      s_meta[3] = tile;
+    }
+    mixed = __syncthreads_or(static_cast<int>(mis)) != 0;
   }
-  const bool mixed = __syncthreads_or(static_cast<int>(mis)) != 0;
+  const volatile int64_t* meta = s_meta;
 
-  const int64_t nu = len_j > h ? (len_j - h) / E : 0;  // whole units of this server
-  const int64_t u0 = tile * kThreads;
-  const int64_t e0 = off_j + h;                        // parameter index of unit 0's first element
-
-  if (u0 < nu) {
-    const int64_t live_units = (nu - u0 < kThreads) ? (nu - u0) : kThreads;
-    const bool live = threadIdx.x < live_units;
-    const int64_t unit = live ? (u0 + threadIdx.x) : (nu - 1);  // dead slots re-read a valid unit, store nothing
-    const bool theta_vec = p.base_aligned != 0 && (e0 & 3) == 0;  // CTA-uniform: theta co-aligned with the units
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int64_t seg_e0 = e0 + (u0 + warp * 32) * E;
-    const int64_t live_in_seg = (live_units - warp * 32) * E;  // <= 0 for a dead warp: it touches no memory
-    float* seg = s_seg + warp * SEG;
-
-    // one array's E values of this thread's unit: 128-bit when co-aligned, else coalesced 32-bit + warp transpose
-    auto load_arr = [&](const float* arr, float4* dst, float fill) {
-      if (theta_vec) {
+  float4 th4[Q], em4[Q], a04[Q], a14[Q];
+  int64_t goff;  // byte offset of this thread's unit in every arrival's slice
+  const int n_batches = mixed ? 0 : K / U;  // mixed phases: everything goes through the narrow-load loop below
+  uint4 cur[U], nxt[U];
+  {
+    const Geom<E> g = make_geom<E>(meta[0], meta[1], static_cast<int>(meta[2]), meta[3], p.base_aligned, s_seg);
+    if (g.u0 >= g.nu) goto peel;  // CTA-uniform: this tile holds no whole unit (a server shorter than its head)
+    goff = g.unit * 16;
+    // the first batch of gradients is requested BEFORE the state: when theta is not co-aligned its loads are followed
+    // by a trip through shared memory, and the gradient stream should not wait for that
+    if (n_batches > 0) {
 #pragma unroll
-        for (int q = 0; q < Q; ++q) dst[q] = ld_state16(arr + e0 + unit * E + 4 * q);
-      } else {
-#pragma unroll
-        for (int q = 0; q < E; ++q) {
-          const int idx = q * 32 + lane;
-          seg[idx] = idx < live_in_seg ? ld_state32(arr + seg_e0 + idx) : fill;
-        }
-        __syncwarp();
-#pragma unroll
-        for (int q = 0; q < Q; ++q) dst[q] = *reinterpret_cast<const float4*>(&seg[(lane * Q + q) * 4]);
-        __syncwarp();
-      }
-    };
-    auto store_arr = [&](float* arr, const float4* src) {
-      if (theta_vec) {
-        if (live) {
-#pragma unroll
-          for (int q = 0; q < Q; ++q) st_state16(arr + e0 + unit * E + 4 * q, src[q]);
-        }
-      } else {
-#pragma unroll
-        for (int q = 0; q < Q; ++q) *reinterpret_cast<float4*>(&seg[(lane * Q + q) * 4]) = src[q];
-        __syncwarp();
-#pragma unroll
-        for (int q = 0; q < E; ++q) {
-          const int idx = q * 32 + lane;
-          if (idx < live_in_seg) st_state32(arr + seg_e0 + idx, seg[idx]);
-        }
-        __syncwarp();
-      }
-    };
-
-    float4 th4[Q], em4[Q], a04[Q], a14[Q];
-    auto load_state = [&]() {
-      load_arr(p.theta, th4, 0.f);
-      if (EMA != EMA_OFF) load_arr(p.ema, em4, 0.f);
-      if (OPT != OPT_SGD) load_arr(p.s0, a04, 1.f);
-      if (OPT == OPT_RMSPROP_MOM) load_arr(p.s1, a14, 0.f);
-    };
-    load_state();
+      for (int v = 0; v < U; ++v) cur[v] = ldg_stream16(s_ptr[v] + goff);
+    }
+    load_state<E, OPT, EMA>(g, p, th4, em4, a04, a14);
+  }
+  {
     float2* th = reinterpret_cast<float2*>(th4);
     float2* em = reinterpret_cast<float2*>(em4);
     float2* a0 = reinterpret_cast<float2*>(a04);
@@ -142,63 +206,74 @@ __global__ void __launch_bounds__(kThreads, MINB) async_sharded_kernel(const Fus
 
     unsigned bad = 0;  // RMSProp: did any ms + eps leave the range of the unchecked packed rsqrt?
     if (!mixed) {
-      // software-pipelined batches of U arrivals, as K4: the loads of batch b+1 fly while batch b is applied
-      const int n_batches = K / U;
-      uint4 cur[U], nxt[U];
-      if (n_batches > 0) {
-#pragma unroll
-        for (int v = 0; v < U; ++v) cur[v] = ldg_stream16(s_ptr[v] + unit * 16);
-      }
+      // software-pipelined batches of U arrivals, exactly K4's loop: the loads of batch b+1 fly while batch b is applied
       for (int bt = 0; bt < n_batches; ++bt) {
         const int i = bt * U;
-        if (bt + 1 < n_batches) {
+        if (PIPE) {
+          if (bt + 1 < n_batches) {
 #pragma unroll
-          for (int v = 0; v < U; ++v) nxt[v] = ldg_stream16(s_ptr[i + U + v] + unit * 16);
+            for (int v = 0; v < U; ++v) nxt[v] = ldg_stream16(s_ptr[i + U + v] + goff);
+          }
+          // Scheduling fence.  Without it ptxas predicates the loads above and sinks them below the updates (or, with
+          // the last batch peeled, merges the two buffers): the next batch is then in flight for a few instructions
+          // only and the warp waits for every batch -- 48 % of all stall samples, +8 % kernel time (ncu, r2_async.md).
+          __syncwarp();
         }
 #pragma unroll
         for (int v = 0; v < U; ++v)
           apply_unit<BF16, OPT, EMA, SCALED>(cur[v], s_scale[i + v], s_gamma[i + v], th, em, a0, a1, pc, bad);
+        if (PIPE) {
 #pragma unroll
-        for (int v = 0; v < U; ++v) cur[v] = nxt[v];
+          for (int v = 0; v < U; ++v) cur[v] = nxt[v];
+        } else if (bt + 1 < n_batches) {  // one buffer: U independent loads in flight, then U dependent updates
+#pragma unroll
+          for (int v = 0; v < U; ++v) cur[v] = ldg_stream16(s_ptr[i + U + v] + goff);
+        }
       }
       for (int i = n_batches * U; i < K; ++i) {
-        const uint4 r = ldg_stream16(s_ptr[i] + unit * 16);
+        const uint4 r = ldg_stream16(s_ptr[i] + goff);
         apply_unit<BF16, OPT, EMA, SCALED>(r, s_scale[i], s_gamma[i], th, em, a0, a1, pc, bad);
       }
     } else {
 #pragma unroll 2
       for (int i = 0; i < K; ++i) {
         const char* g = s_ptr[i];
-        const uint4 r = load_unit_any<BF16>(g + unit * 16, (reinterpret_cast<uintptr_t>(g) & 15u) == 0);
+        const uint4 r = load_unit_any<BF16>(g + goff, (reinterpret_cast<uintptr_t>(g) & 15u) == 0);
         apply_unit<BF16, OPT, EMA, SCALED>(r, s_scale[i], s_gamma[i], th, em, a0, a1, pc, bad);
       }
     }
+
+    // ---- epilogue: the addresses are derived again (Geom's comment) -----------------------------------------
+    const Geom<E> g = make_geom<E>(meta[0], meta[1], static_cast<int>(meta[2]), meta[3], p.base_aligned, s_seg);
     if (OPT == OPT_RMSPROP_MOM && __any_sync(0xFFFFFFFFu, rsqrt_pair_left_range(bad))) {
       // Never on sane data: a non-finite or absurd second moment somewhere in this warp.  Nothing has been stored
       // yet: the whole warp (the transposed loads are warp-collective) redoes its units from memory with the checked
       // scalar update, which gives the same bits wherever the packed form was in range.
-      load_state();
+      load_state<E, OPT, EMA>(g, p, th4, em4, a04, a14);
       float* ths = reinterpret_cast<float*>(th4);
       float* ems = reinterpret_cast<float*>(em4);
       float* a0s = reinterpret_cast<float*>(a04);
       float* a1s = reinterpret_cast<float*>(a14);
       for (int n = 0; n < K; ++n) {
-        const char* g = s_ptr[n];
-        const uint4 r = load_unit_any<BF16>(g + unit * 16, (reinterpret_cast<uintptr_t>(g) & 15u) == 0);
+        const char* gp = s_ptr[n];
+        const uint4 r = load_unit_any<BF16>(gp + g.unit * 16, (reinterpret_cast<uintptr_t>(gp) & 15u) == 0);
 #pragma unroll
         for (int e = 0; e < E; ++e)
           update_element_g<OPT, EMA>(unit_element<BF16>(r, e), s_scale[n], s_gamma[n], ths[e], ems[e], a0s[e], a1s[e], p);
       }
     }
-
-    store_arr(p.theta, th4);
-    if (EMA != EMA_OFF) store_arr(p.ema, em4);
-    if (OPT != OPT_SGD) store_arr(p.s0, a04);
-    if (OPT == OPT_RMSPROP_MOM) store_arr(p.s1, a14);
+    store_arr<E>(g, p.theta, th4);
+    if (EMA != EMA_OFF) store_arr<E>(g, p.ema, em4);
+    if (OPT != OPT_SGD) store_arr<E>(g, p.s0, a04);
+    if (OPT == OPT_RMSPROP_MOM) store_arr<E>(g, p.s1, a14);
   }
 
+peel:
   // ---- head and tail peel of server j, by its first CTA: K dependent updates per element, in registers --------
-  if (tile == 0) {
+  if (meta[3] == 0) {
+    const int64_t off_j = meta[0], len_j = meta[1];
+    const int h = static_cast<int>(meta[2]);
+    const int64_t nu = len_j > h ? (len_j - h) / E : 0;
     const int64_t tail0 = h + nu * E;
     const int64_t n_head = h < len_j ? h : len_j;
     const int64_t n_tail = len_j > tail0 ? len_j - tail0 : 0;
@@ -219,12 +294,14 @@ __global__ void __launch_bounds__(kThreads, MINB) async_sharded_kernel(const Fus
   }
 }
 
-// arrivals per batch and CTAs per SM: K4's shapes (async_kernel.cu), measured there
+// arrivals per batch, CTAs per SM, software-pipelined or not: K4's shapes (async_kernel.cu), measured there
 struct Shape {
   int unroll, minb;
+  bool pipe;
 };
 constexpr Shape shape_for(bool bf16, int opt) {
-  return bf16 ? (opt == OPT_RMSPROP_MOM ? Shape{2, 2} : Shape{4, 3}) : (opt == OPT_RMSPROP_MOM ? Shape{3, 4} : Shape{4, 4});
+  return bf16 ? (opt == OPT_RMSPROP_MOM ? Shape{2, 2, true} : Shape{8, 3, false})
+              : (opt == OPT_RMSPROP_MOM ? Shape{3, 4, true} : Shape{4, 4, true});
 }
 
 using KernelFn = void (*)(const FusedParams);
@@ -232,8 +309,8 @@ using KernelFn = void (*)(const FusedParams);
 template <bool BF16, int OPT, int EMA>
 KernelFn pick_scaled(bool scaled) {
   constexpr Shape S = shape_for(BF16, OPT);
-  return scaled ? async_sharded_kernel<BF16, OPT, EMA, true, S.unroll, S.minb>
-                : async_sharded_kernel<BF16, OPT, EMA, false, S.unroll, S.minb>;
+  return scaled ? async_sharded_kernel<BF16, OPT, EMA, true, S.unroll, S.minb, S.pipe>
+                : async_sharded_kernel<BF16, OPT, EMA, false, S.unroll, S.minb, S.pipe>;
 }
 template <bool BF16, int OPT>
 KernelFn pick_ema(int ema, bool scaled) {
