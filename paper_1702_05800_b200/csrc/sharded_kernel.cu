@@ -46,34 +46,48 @@ __global__ void __launch_bounds__(kThreads, MINB) sharded_aggregate_update_ema(c
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
-  // ---- which (server, tile) is this CTA ---------------------------------------------------------------
+  // ---- which (server, tile) is this CTA; its kept row ---------------------------------------------------------
+  // The prologue is a chain of dependent loads that every CTA pays before its first gradient byte moves, so it is kept
+  // SHORT: the server by a warp-wide search (1-2 levels), then everything that only needs j in ONE level -- shard
+  // bounds, tile origin, status, count, this thread's entry of the kept row and the row's first entry -- loaded before
+  // any of it is checked (all of these addresses are valid whatever the values turn out to be), then the slice
+  // pointers in one more level.
   const int64_t b = blockIdx.x;
   // The grid is the work list's total, computed by the host from the shard table; a table built for another gradient
   // dtype (another tile size) has another total: then nothing is touched, instead of a partial update.
-  if (p.tile_start[p.M] != static_cast<int64_t>(gridDim.x)) return;
-  const int j = upper_slot(p.tile_start, p.M, b);
-  const int64_t off_j = p.shard_off[j];
-  const int64_t len_j = p.shard_off[j + 1] - off_j;
-  const int64_t tile = b - p.tile_start[j];
+  const int64_t total = p.tile_start[p.M];
+  const int j = upper_slot_warp(p.tile_start, p.M, b);
   const int row = p.per_shard ? j : 0;
-  if (p.status != nullptr && p.status[row] != 0) return;  // this server did not collect its gradients
-  const int N = p.n_kept ? p.n_kept[row] : p.N;
+  const int32_t* kept = p.kept + static_cast<int64_t>(row) * p.kept_stride;
+  const int64_t off_j = p.shard_off[j];
+  const int64_t off_j1 = p.shard_off[j + 1];
+  const int64_t tile0 = p.tile_start[j];
+  const int st = p.status != nullptr ? p.status[row] : 0;
+  const int N = p.n_kept != nullptr ? p.n_kept[row] : p.N;
+  const int k_first = kept[0];
+  const int i_mine = static_cast<int>(threadIdx.x) < p.kept_stride ? static_cast<int>(threadIdx.x) : p.kept_stride - 1;
+  const int k_mine = kept[i_mine];
+  if (total != static_cast<int64_t>(gridDim.x)) return;
+  if (st != 0) return;  // this server did not collect its gradients
   if (N <= 0 || N > p.kept_stride || N > kMaxWorkers) return;  // a count nobody wrote: treat the row as failed
+  const int64_t len_j = off_j1 - off_j;
+  const int64_t tile = b - tile0;
   const float inv_N = p.n_kept ? 1.0f / static_cast<float>(N) : p.inv_N;
 
   // ---- stage server j's kept row as slice base pointers; the first one fixes the phase ---------------------
   // Every thread reads the row's first pointer itself (one address for the whole CTA: a broadcast), so the head peel
   // is known before the staging pass and one barrier is enough.
-  const int32_t* kept = p.kept + static_cast<int64_t>(row) * p.kept_stride;
   auto slice_ptr = [&](int k) -> const char* {
     return p.slices ? static_cast<const char*>(p.grads[static_cast<int64_t>(k) * p.M + j])
                     : static_cast<const char*>(p.grads[k]) + off_j * ESZ;
   };
-  const unsigned ref = static_cast<unsigned>(reinterpret_cast<uintptr_t>(slice_ptr(kept[0]))) & 127u;
+  const char* g_first = slice_ptr(k_first);
+  const char* g_mine = static_cast<int>(threadIdx.x) < N ? slice_ptr(k_mine) : g_first;
+  const unsigned ref = static_cast<unsigned>(reinterpret_cast<uintptr_t>(g_first)) & 127u;
   const int h = static_cast<int>(((128u - ref) & 127u) / ESZ);  // head peel: elements before the first 128-byte line
   unsigned mis = 0;
   for (int i = threadIdx.x; i < N; i += kThreads) {
-    const char* g = slice_ptr(kept[i]);
+    const char* g = i < kThreads ? g_mine : slice_ptr(kept[i]);
     mis |= ((static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) ^ ref) & 15u);  // another 16-byte phase
     s_ptr[i] = g + h * ESZ;  // unit u of this worker = s_ptr[i] + 16 u
   }
