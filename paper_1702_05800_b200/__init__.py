@@ -13,4 +13,4 @@ from .binding import (psync_staleness, HostCtx, PSYNC_GRADS_FLAT, PSYNC_GRADS_SL
                       psync_lr_schedule, psync_kth_arrival_stats, psync_interp_iterations, psync_launch_geometry,
                       psync_select_first_n, psync_select_first_n_sharded, psync_select_timeout, psync_step_host,
                       psync_step_host_workspace_bytes)
-from .server import ParameterServerStep  # noqa: F401
+from .server import AsyncServerStep, ParameterServerStep  # noqa: F401

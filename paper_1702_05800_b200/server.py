@@ -103,3 +103,103 @@ class ParameterServerStep:
         if self._step is None or self._step.gamma_t != np.float32(gamma_t):
             self._build(gamma_t)
         B.psync_aggregate_update(self._step, stream)
+
+
+class AsyncServerStep:
+    """The Async-SGD parameter server (Alg. 2, L78-89): device buffers + the calls of one batch of arrivals.
+
+    apply(d_arrival) enqueues, with no host synchronisation: the arrival order (per server with per_server=True,
+    d_arrival [M][W]), optionally the global-norm clip factors (clip > 0; flat buffers only: the norm is over the whole
+    gradient of a worker, L313), optionally the learning rates of this batch's iterations (lr = (gamma0, beta, s):
+    gamma0 * beta^((t0 + i) s), L315), the one-pass application of the arrivals, and with track_staleness=True (one
+    order only) Table 1's bookkeeping.  Plumbing only, no arithmetic."""
+
+    def __init__(self, shard_off, W: int, theta: torch.Tensor, ema: Optional[torch.Tensor],
+                 state0: Optional[torch.Tensor], state1: Optional[torch.Tensor], opt: int, ema_mode: int = B.PSYNC_EMA_PRE,
+                 alpha: float = 0.0, mu: float = 0.0, rho: float = 0.0, eps: float = 0.0, per_server: bool = False,
+                 clip: float = 0.0, lr=None, track_staleness: bool = False, lag: int = 0):
+        dev = theta.device
+        self.shard_off = np.ascontiguousarray(shard_off, dtype=np.int64)
+        self.M, self.W = self.shard_off.size - 1, W
+        self.theta, self.ema, self.state0, self.state1 = theta, ema, state0, state1
+        self.opt, self.ema_mode = opt, ema_mode
+        self.alpha, self.mu, self.rho, self.eps = alpha, mu, rho, eps
+        self.per_server, self.clip, self.lr, self.lag = bool(per_server), float(clip), lr, int(lag)
+        if track_staleness and per_server:
+            raise ValueError("staleness bookkeeping follows one arrival order (per_server=False)")
+        rows = self.M if per_server else 1
+        self.d_order = torch.full((rows, W), -1, dtype=torch.int32, device=dev)
+        self.d_n_arrived = torch.zeros(rows, dtype=torch.int32, device=dev)
+        self.d_shard_off = torch.from_numpy(self.shard_off).to(dev)
+        self.d_gamma = torch.zeros(W, dtype=torch.float32, device=dev) if lr is not None else None
+        self.d_gscale = torch.ones(W, dtype=torch.float32, device=dev) if clip > 0 else None
+        self._d_clip_work = None
+        self.t0 = 0                       # iterations scheduled so far (host counter: W per batch unless given)
+        self.track_staleness = bool(track_staleness)
+        if track_staleness:
+            self.d_read_iter = torch.zeros(W, dtype=torch.int64, device=dev)
+            self.d_t = torch.zeros(1, dtype=torch.int64, device=dev)
+            self.d_staleness = torch.zeros(W, dtype=torch.int64, device=dev)
+            self.d_stale_stats = torch.zeros(6, dtype=torch.float64, device=dev)
+            self.d_stale_status = torch.zeros(1, dtype=torch.int32, device=dev)
+        self._d_tiles = {}
+        self.layout = B.PSYNC_GRADS_FLAT
+        self.table: Optional[B.GradTable] = None
+        self._retired = deque(maxlen=4)   # tables of batches that may still be in flight (ParameterServerStep's note)
+        self._step = None
+        self._keep = None
+
+    def set_gradients(self, buffers: Sequence[torch.Tensor]) -> None:
+        if len(buffers) != self.W:
+            raise ValueError(f"need W = {self.W} gradient buffers")
+        if self.table is not None:
+            self._retired.append((self.table, self._keep))
+        self.table, self.layout, self._step = B.make_grad_table(buffers), B.PSYNC_GRADS_FLAT, None
+
+    def set_gradient_slices(self, slices: Sequence[Sequence[Optional[torch.Tensor]]]) -> None:
+        if len(slices) != self.W or any(len(row) != self.M for row in slices):
+            raise ValueError(f"need W = {self.W} rows of M = {self.M} slices")
+        if self.clip > 0:
+            raise ValueError("global-norm clipping needs each worker's whole gradient: flat buffers")
+        if self.table is not None:
+            self._retired.append((self.table, self._keep))
+        self.table, self.layout, self._step = B.make_slice_table(slices), B.PSYNC_GRADS_SLICES, None
+
+    def _build(self, gamma_t: float):
+        sharded = self.per_server or self.layout == B.PSYNC_GRADS_SLICES
+        gd = self.table.grad_dtype
+        if sharded and gd not in self._d_tiles:
+            self._d_tiles[gd] = B.psync_shard_worklist(self.d_shard_off, gd)
+        self._step, self._keep = B.make_step(
+            self.shard_off, self.W, self.W, gd, self.theta, self.ema, self.state0, self.state1, opt=self.opt,
+            ema_mode=self.ema_mode, gamma_t=gamma_t, alpha=self.alpha, mu=self.mu, rho=self.rho, eps=self.eps,
+            d_grads=self.table.d_ptrs, d_kept=self.d_order, per_shard=self.per_server,
+            d_shard_off=self.d_shard_off if sharded else None, d_n_kept=self.d_n_arrived, kept_stride=self.W,
+            grad_layout=self.layout, d_tile_start=self._d_tiles[gd] if sharded else None)
+        return self._step
+
+    def apply(self, d_arrival: torch.Tensor, gamma_t: float = 0.0, t0: Optional[int] = None, stream=None) -> None:
+        """One batch: every gradient whose arrival time is finite is one iteration, in arrival order (L85-87)."""
+        if self.table is None:
+            raise RuntimeError("set_gradients() first")
+        if self._step is None or self._step.gamma_t != np.float32(gamma_t):
+            self._build(gamma_t)
+        if stream is not None and hasattr(stream, "cuda_stream"):
+            self.table.d_ptrs.record_stream(stream)
+        if self.per_server:
+            B.psync_order_by_arrival_sharded(d_arrival, self.W, self.M, self.d_order, self.d_n_arrived, stream)
+        else:
+            B.psync_order_by_arrival(d_arrival, self.W, self.d_order, self.d_n_arrived, stream)
+        if self.clip > 0:
+            if self._d_clip_work is None:
+                nbytes = B.psync_clip_workspace_bytes(self.W, self.theta.numel(), self.table.grad_dtype)
+                self._d_clip_work = torch.empty(nbytes // 8, dtype=torch.float64, device=self.theta.device)
+            B.psync_clip_scales(self.table, self.clip, self.d_gscale, self._d_clip_work, stream)
+        if self.lr is not None:
+            gamma0, beta, s = self.lr
+            B.psync_lr_schedule(gamma0, beta, self.t0 if t0 is None else t0, self.W, s, self.d_gamma, stream)
+        B.psync_async_apply(self._step, self.d_gamma, stream, d_gscale=self.d_gscale)
+        if self.track_staleness:
+            B.psync_staleness(self.d_read_iter, self.d_order, self.d_t, self.d_staleness, self.d_stale_stats,
+                              self.d_stale_status, d_n_arrived=self.d_n_arrived, lag=self.lag, stream=stream)
+        self.t0 = (self.t0 if t0 is None else t0) + self.W

@@ -348,3 +348,89 @@ def test_full_size_cfg3_shape_every_element_on_separately_allocated_slices():
                                  gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
     assert rc == oracle.OK
     pair.compare_and_sync("async rows cfg3 (every element)", 106)
+
+
+# ------------------------------------------------------------------ AsyncServerStep: the calls of one batch, chained
+def test_async_server_step_flat_with_clipping_schedule_and_staleness_chained_batches():
+    """Order -> clip factors -> learning rates -> K iterations -> staleness, enqueued without a host sync, two batches;
+    every piece against its own oracle function."""
+    cfg = replace(BASE, P=50_021, M=5, opt=synth.RMSPROP_MOM, grad_dist=("normal", 2e-3), name="aserver_flat")
+    off = synth.shard_offsets(cfg)
+    theta = synth.init_theta(cfg, DEV)
+    s0, s1 = synth.init_state(cfg, DEV)
+    ema = theta.clone()
+    lr = (0.045, 0.94, 1.0 / 40.0)
+    clip = 0.4                                              # ||G|| ~ 2e-3 * sqrt(P) ~ 0.45: some workers are clipped
+    srv = psync.AsyncServerStep(off, cfg.W, theta, ema, s0, s1, cfg.opt, cfg.ema_mode, alpha=cfg.alpha, mu=cfg.mu,
+                                rho=cfg.rho, eps=cfg.eps, clip=clip, lr=lr, track_staleness=True, lag=2)
+    h = {"theta": to_np(theta), "ema": to_np(ema), "state0": to_np(s0), "state1": to_np(s1)}
+    read = np.zeros(cfg.W, np.int64)
+    t_srv = 0
+    for s in range(2):
+        grads = [synth.gradient(cfg, s, k, DEV) for k in range(cfg.W)]
+        for k in range(0, cfg.W, 2):
+            grads[k].mul_(0.5)                              # these workers' norms are within the bound: factor 1
+        a = synth.arrival_times(cfg, s)
+        if s == 1:
+            a[4] = np.inf
+        srv.set_gradients(grads)
+        srv.apply(torch.from_numpy(a).to(DEV))
+        torch.cuda.synchronize()
+        order = oracle.order_by_arrival(a)
+        K = order.size
+        np_g = [synth.as_numpy_grad(g) for g in grads]
+        scales = oracle.clip_scales(np_g, clip)
+        gammas = oracle.lr_schedule(lr[0], lr[1], s * cfg.W, cfg.W, lr[2])
+        assert np.array_equal(srv.d_order.cpu().numpy()[0, :K], order) and int(srv.d_n_arrived.item()) == K
+        assert np.array_equal(srv.d_gscale.cpu().numpy(), scales) and (scales < 1).any() and (scales == 1).any()
+        assert np.array_equal(srv.d_gamma.cpu().numpy(), gammas)
+        rc = oracle.async_apply(off, np_g, order, h["theta"], h["ema"], h["state0"], h["state1"], gammas=gammas[:K].copy(),
+                                gscales=scales[order].copy(), opt=cfg.opt, ema_mode=cfg.ema_mode, alpha=cfg.alpha, mu=cfg.mu,
+                                rho=cfg.rho, eps=cfg.eps)
+        assert rc == oracle.OK
+        for n, t in (("theta", theta), ("ema", ema), ("state0", s0), ("state1", s1)):
+            assert_close(to_np(t), h[n], rtol_async(K), ATOL_STEP, f"aserver batch {s} {n}")
+            h[n] = to_np(t)
+        st, stale, read, stats = oracle.staleness(read, order, t_srv, lag=2)
+        t_srv += K
+        assert st == oracle.OK and int(srv.d_stale_status.item()) == 0 and int(srv.d_t.item()) == t_srv
+        assert np.array_equal(srv.d_staleness.cpu().numpy()[:K], stale)
+        assert np.array_equal(srv.d_read_iter.cpu().numpy(), read)
+        assert np.array_equal(srv.d_stale_stats.cpu().numpy(), stats)
+
+
+def test_async_server_step_per_server_on_slices_chained_batches():
+    cfg = replace(BASE, opt=synth.MOMENTUM, grad_dtype=synth.BF16, name="aserver_rows")
+    off = np.asarray(RAGGED, dtype=np.int64)
+    theta = synth.init_theta(cfg, DEV)
+    s0, _ = synth.init_state(cfg, DEV)
+    ema = theta.clone()
+    lr = (0.045, 0.94, 1.0 / 40.0)
+    srv = psync.AsyncServerStep(off, cfg.W, theta, ema, s0, None, cfg.opt, cfg.ema_mode, alpha=cfg.alpha, mu=cfg.mu,
+                                per_server=True, lr=lr)
+    with pytest.raises(ValueError):
+        psync.AsyncServerStep(off, cfg.W, theta, ema, s0, None, cfg.opt, per_server=True, track_staleness=True)
+    h = {"theta": to_np(theta), "ema": to_np(ema), "state0": to_np(s0)}
+    M = off.size - 1
+    for s in range(2):
+        flat = [synth.gradient(cfg, s, k, DEV) for k in range(cfg.W)]
+        sl = cut_slices(flat, off, lambda k, j: (k + 2 * j) % 8 if s else 0)
+        a = synth.arrival_times_per_server(cfg, s, server_sigma=0.3)
+        a[2, 5] = np.nan
+        srv.set_gradient_slices(sl)
+        srv.apply(torch.from_numpy(a).to(DEV))
+        torch.cuda.synchronize()
+        order = np.zeros((M, cfg.W), dtype=np.int32)
+        n_arr = np.zeros(M, dtype=np.int32)
+        for j in range(M):
+            o = oracle.order_by_arrival(a[j])
+            order[j, :o.size], n_arr[j] = o, o.size
+        assert np.array_equal(srv.d_n_arrived.cpu().numpy(), n_arr) and n_arr[2] == cfg.W - 1
+        gammas = oracle.lr_schedule(lr[0], lr[1], s * cfg.W, cfg.W, lr[2])
+        rc = oracle.async_apply_rows(off, np_slices(sl), order, h["theta"], h["ema"], h["state0"], None, slices=True,
+                                     per_shard=True, n_arrived=n_arr, gammas=gammas, opt=cfg.opt, ema_mode=cfg.ema_mode,
+                                     alpha=cfg.alpha, mu=cfg.mu)
+        assert rc == oracle.OK
+        for n, t in (("theta", theta), ("ema", ema), ("state0", s0)):
+            assert_close(to_np(t), h[n], rtol_async(cfg.W), ATOL_STEP, f"aserver rows batch {s} {n}")
+            h[n] = to_np(t)
