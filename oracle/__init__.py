@@ -86,6 +86,8 @@ def lib() -> ctypes.CDLL:
                                               vp, vp, vp, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int,
                                               f32, f32, f32, f32, f32]
         L.oracle_async_apply_rows.restype = ctypes.c_int
+        L.oracle_clip_scales_slices.argtypes = [vp, i32, i32, vp, ctypes.c_int, f32, vp]
+        L.oracle_clip_scales_slices.restype = ctypes.c_int
         L.oracle_staleness.argtypes = [vp, i32, vp, i32, i64, i32, vp, vp, vp]
         L.oracle_staleness.restype = ctypes.c_int
         L.oracle_order_by_arrival.argtypes = [vp, i32, vp, vp]
@@ -378,6 +380,26 @@ def clip_scales(grads, clip):
     out = np.zeros(W, dtype=np.float32)
     if lib().oracle_clip_scales(ctypes.cast(ptrs, ctypes.c_void_p), W, grads[0].size, gd, clip, _ptr(out)) != OK:
         raise ValueError("oracle_clip_scales: invalid arguments")
+    return out
+
+
+def clip_scales_slices(shard_off, slices, clip):
+    """The same factors for gradients that lie as W x M per-(worker, server) slices: the norm is over all of a worker's
+    slices (PAPER.md:L313, "across all layers") -> float32 [W]."""
+    shard_off = np.ascontiguousarray(shard_off, dtype=np.int64)
+    M, W = shard_off.size - 1, len(slices)
+    first = next(a for row in slices for a in row if a is not None)
+    gd = _grad_dtype([first])
+    for k, row in enumerate(slices):
+        if len(row) != M:
+            raise ValueError("every worker needs M slices")
+        for j, a in enumerate(row):
+            _chk(a, first.dtype, f"slices[{k}][{j}]", int(shard_off[j + 1] - shard_off[j]))
+    ptrs = (ctypes.c_void_p * (W * M))(*[None if a is None else a.ctypes.data for row in slices for a in row])
+    out = np.zeros(W, dtype=np.float32)
+    if lib().oracle_clip_scales_slices(ctypes.cast(ptrs, ctypes.c_void_p), W, M, _ptr(shard_off), gd, clip,
+                                       _ptr(out)) != OK:
+        raise ValueError("oracle_clip_scales_slices: invalid arguments")
     return out
 
 

@@ -32,7 +32,8 @@
 // schedule and clip factors (tests/test_oracle_helpers.py), straggler statistics and the Fig. 5
 // interpolation, the latter against the two values the paper prints (tests/test_oracle_stragglers.py);
 // the per-(worker, server) slice layout (tests/test_oracle_slices.py); the staleness bookkeeping of Alg. 2
-// (tests/test_oracle_staleness.py) and Alg. 2 per server (tests/test_oracle_async.py).
+// (tests/test_oracle_staleness.py), Alg. 2 per server (tests/test_oracle_async.py) and the clip factors
+// of sliced gradients (tests/test_oracle_helpers.py).
 // (The fp32 diagnostic mirror of the GPU's operation list is a SEPARATE library, oracle/psync_mirror_f32.cpp;
 // nothing of it is in this file.)
 // Nothing here is "parity unpinned".
@@ -610,6 +611,37 @@ int oracle_clip_scales(const void* const* grads, int32_t W, int64_t P, int grad_
     for (int64_t i = 0; i < P; ++i) {
       const double g = grad_at(grads[k], grad_dtype, i);
       sumsq += g * g;
+    }
+    const double norm = std::sqrt(sumsq);
+    const double c = static_cast<double>(clip);
+    scales[k] = static_cast<float>(c / std::max(norm, c));
+  }
+  return ORACLE_OK;
+}
+
+// The same factor when worker k's gradient lies as M per-(worker, server) slices (grads is [W*M], entry k*M + j ->
+// the len_j elements of G_k[j]; reading R24).  "Collect the gradient across all layers ... compute the global norm"
+// (L313): the norm is over ALL of worker k's slices -- the squares are added server by server, element by element,
+// i.e. in the order of the flat vector.  Every slice of a non-empty server must be present.
+int oracle_clip_scales_slices(const void* const* grads, int32_t W, int32_t M, const int64_t* shard_off, int grad_dtype,
+                              float clip, float* scales) {
+  if (!grads || !scales || !shard_off || W < 1 || M < 1 || !(clip > 0.0f)) return ORACLE_EINVAL;
+  if (grad_dtype != ORACLE_F32 && grad_dtype != ORACLE_BF16) return ORACLE_EINVAL;
+  if (shard_off[0] != 0) return ORACLE_EINVAL;
+  for (int32_t j = 0; j < M; ++j)
+    if (shard_off[j + 1] < shard_off[j]) return ORACLE_EINVAL;
+  for (int32_t k = 0; k < W; ++k)
+    for (int32_t j = 0; j < M; ++j)
+      if (shard_off[j + 1] > shard_off[j] && !grads[static_cast<int64_t>(k) * M + j]) return ORACLE_EINVAL;
+  for (int32_t k = 0; k < W; ++k) {
+    double sumsq = 0.0;
+    for (int32_t j = 0; j < M; ++j) {  // server j's part of worker k's gradient
+      const void* G = grads[static_cast<int64_t>(k) * M + j];
+      const int64_t len_j = shard_off[j + 1] - shard_off[j];
+      for (int64_t i = 0; i < len_j; ++i) {
+        const double g = grad_at(G, grad_dtype, i);
+        sumsq += g * g;
+      }
     }
     const double norm = std::sqrt(sumsq);
     const double c = static_cast<double>(clip);

@@ -88,6 +88,61 @@ def test_clip_invalid_and_nonfinite():
         oracle.clip_scales(g, 0.0)
 
 
+# ------------------------------------------------------------------ clip factors of sliced gradients
+def test_clip_scales_slices_3_4_12_by_hand():
+    """Worker 0: G[0] = [3], G[1] = [4, 12] on two servers: ||G|| = 13 over BOTH slices (a per-slice norm would give 3
+    and sqrt(160)).  clip 6.5 -> 0.5.  Worker 1: [0], [0, 1]: norm 1 -> 1."""
+    off = [0, 1, 3]
+    sl = [[np.array([3.0], f32), np.array([4.0, 12.0], f32)], [np.array([0.0], f32), np.array([0.0, 1.0], f32)]]
+    assert oracle.clip_scales_slices(off, sl, 6.5).tolist() == [0.5, 1.0]
+    assert oracle.clip_scales_slices(off, sl, 13.0).tolist() == [1.0, 1.0]
+    assert oracle.clip_scales_slices(off, sl, 0.25).tolist() == [float(f32(0.25 / 13.0)), 0.25]
+
+
+@pytest.mark.parametrize("bf16", [False, True])
+def test_clip_scales_slices_equal_the_pinned_flat_factors_and_numpy(bf16):
+    """Slices that are cuts of flat buffers (views, and separately allocated copies at odd offsets, with an empty and a
+    one-element server): bit-equal to the already pinned flat oracle; numpy's norm of the concatenation."""
+    rng = np.random.default_rng(70 + bf16)
+    off = np.array([0, 1, 1, 4_099, 7_000, 10_007], np.int64)
+    P, W = int(off[-1]), 6
+    vals = [(rng.normal(0, 10.0 ** rng.integers(-3, 1), P)).astype(f32) for _ in range(W)]
+    if bf16:
+        grads = [(v.view(np.uint32) >> 16).astype(np.uint16) for v in vals]
+        vals = [(g.astype(np.uint32) << 16).view(np.float32) for g in grads]
+    else:
+        grads = vals
+    clip = 0.5
+    want = oracle.clip_scales(grads, clip)
+    views = [[g[off[j]:off[j + 1]] for j in range(off.size - 1)] for g in grads]
+    assert np.array_equal(oracle.clip_scales_slices(off, views, clip), want)
+    copies = []
+    for k, g in enumerate(grads):
+        row = []
+        for j in range(off.size - 1):
+            buf = np.zeros(int(off[j + 1] - off[j]) + 8, g.dtype)
+            o = (k + j) % 3
+            buf[o:o + int(off[j + 1] - off[j])] = g[off[j]:off[j + 1]]
+            row.append(buf[o:o + int(off[j + 1] - off[j])])
+        copies.append(row)
+    got = oracle.clip_scales_slices(off, copies, clip)
+    assert np.array_equal(got, want)
+    for k in range(W):
+        norm = np.linalg.norm(np.concatenate([vals[k][off[j]:off[j + 1]] for j in range(off.size - 1)]).astype(np.float64))
+        assert ulp_diff(got[k], f32(clip / max(norm, clip))) <= 1
+
+
+def test_clip_scales_slices_invalid():
+    off = [0, 1, 3]
+    sl = [[np.array([3.0], f32), None]]
+    with pytest.raises(ValueError):
+        oracle.clip_scales_slices(off, sl, 1.0)                      # a missing slice of a non-empty server
+    sl = [[np.array([3.0], f32), np.array([4.0, 12.0], f32)]]
+    with pytest.raises(ValueError):
+        oracle.clip_scales_slices(off, sl, 0.0)
+    assert oracle.clip_scales_slices([0, 1, 1, 3], [[sl[0][0], None, sl[0][1]]], 6.5).tolist() == [0.5]   # empty server
+
+
 # ------------------------------------------------------------------ clipped async update
 def test_async_with_clip_by_hand():
     """theta = [1, 1], one arrival G = [3, 4], clip 2.5, gamma 0.5: clipped G = [1.5, 2]; theta' = [0.25, 0.0]."""
