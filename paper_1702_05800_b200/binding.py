@@ -26,7 +26,7 @@ PSYNC_MAX_WORKERS = 1024
 PSYNC_TILE_UNITS = 256
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
-           "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_order_by_arrival_sharded", "psync_async_apply", "psync_staleness", "psync_step_device", "psync_clip_workspace_bytes",
+           "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_order_by_arrival_sharded", "psync_clip_slices_workspace_bytes", "psync_clip_scales_slices", "psync_async_apply", "psync_staleness", "psync_step_device", "psync_clip_workspace_bytes",
            "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_host_ctx_create", "psync_host_ctx_destroy",
            "psync_step_host_ctx", "psync_launch_geometry", "psync_probe_read",
@@ -92,6 +92,10 @@ def lib() -> ctypes.CDLL:
         L.psync_clip_workspace_bytes.restype = ctypes.c_size_t
         L.psync_clip_scales.argtypes = [vp, i32, i64, i32, f32, vp, vp, ctypes.c_size_t, vp]
         L.psync_clip_scales.restype = ctypes.c_int
+        L.psync_clip_slices_workspace_bytes.argtypes = [i32, i32, vp, i32]
+        L.psync_clip_slices_workspace_bytes.restype = ctypes.c_size_t
+        L.psync_clip_scales_slices.argtypes = [vp, i32, i32, vp, vp, i32, f32, vp, vp, ctypes.c_size_t, vp]
+        L.psync_clip_scales_slices.restype = ctypes.c_int
         L.psync_kth_arrival_stats.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, vp]
         L.psync_kth_arrival_stats.restype = ctypes.c_int
         L.psync_interp_iterations.argtypes = [vp, vp, i32, i32, vp, vp]
@@ -386,6 +390,29 @@ def psync_clip_scales(table: "GradTable", clip: float, d_scales: torch.Tensor, d
                                  _stream(stream))
     if check and st != PSYNC_OK:
         raise PsyncError(st, "psync_clip_scales")
+    return st
+
+
+def psync_clip_slices_workspace_bytes(W: int, shard_off, grad_dtype: int) -> int:
+    off = np.ascontiguousarray(shard_off, dtype=np.int64)
+    return lib().psync_clip_slices_workspace_bytes(W, off.size - 1, off.ctypes.data, grad_dtype)
+
+
+def psync_clip_scales_slices(table: "GradTable", shard_off, d_shard_off: torch.Tensor, clip: float, d_scales: torch.Tensor,
+                             d_work: torch.Tensor, stream=None, check: bool = True) -> int:
+    """Global-norm clip factors of W x M per-(worker, server) slices, the norm over all of a worker's slices
+    (include/psync.h: psync_clip_scales_slices; PAPER.md:L313).  `table` comes from make_slice_table."""
+    off = np.ascontiguousarray(shard_off, dtype=np.int64)
+    M = off.size - 1
+    W = table.d_ptrs.numel() // M
+    if d_scales.numel() < W or d_shard_off.numel() < M + 1:
+        raise ValueError("d_scales needs W elements, d_shard_off M + 1")
+    st = lib().psync_clip_scales_slices(_dptr(table.d_ptrs, torch.int64, "d_grads"), W, M, off.ctypes.data,
+                                        _dptr(d_shard_off, torch.int64, "d_shard_off"), table.grad_dtype, clip,
+                                        _dptr(d_scales, torch.float32, "d_scales"), _dptr(d_work, None, "d_work"),
+                                        d_work.numel() * d_work.element_size(), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_clip_scales_slices")
     return st
 
 

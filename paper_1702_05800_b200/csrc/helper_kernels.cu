@@ -90,6 +90,60 @@ __global__ void __launch_bounds__(kClipThreads) sumsq_chunks_kernel(const void* 
   if (threadIdx.x == 0) work[static_cast<int64_t>(blockIdx.y) * gridDim.x + blockIdx.x] = total;
 }
 
+// K5s -- the same sums for gradients that lie as per-(worker, server) slices (grads [W*M], entry k*M + j -> G_k[j]).
+// grid (n_chunks, W): CTA (c, k) finds its (server j, chunk) in chunk_start (the work-list prefix sum for chunks of
+// 8192 16-byte units), sums the squares of that chunk of slice (k, j) and writes work[k * n_chunks + c].  A slice may
+// start at any element: the < 16 bytes before its first 16-byte boundary inside the chunk and the tail go element by
+// element, everything between as 128-bit loads.
+template <bool BF16>
+__global__ void __launch_bounds__(kClipThreads) sumsq_slices_kernel(const void* const* __restrict__ grads, int32_t M,
+                                                                    const int64_t* shard_off, const int64_t* chunk_start,
+                                                                    double* __restrict__ work) {
+  constexpr int E = BF16 ? 8 : 4;
+  constexpr int ESZ = BF16 ? 2 : 4;
+  constexpr int64_t CE = kClipChunkUnits * E;  // elements per chunk
+  __shared__ double s_warp[kClipThreads / 32];
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const int64_t c = blockIdx.x;
+  double acc = 0.0;
+  if (chunk_start[M] == static_cast<int64_t>(gridDim.x)) {  // else: a chunk list of another layout -- sums stay 0
+    const int j = upper_slot_warp(chunk_start, M, c);
+    const int64_t len_j = shard_off[j + 1] - shard_off[j];
+    const int64_t lo = (c - chunk_start[j]) * CE;
+    const int64_t hi = (len_j - lo < CE) ? len_j : lo + CE;
+    const char* g = static_cast<const char*>(grads[static_cast<int64_t>(blockIdx.y) * M + j]);
+    const int mis = static_cast<int>((reinterpret_cast<uintptr_t>(g + lo * ESZ) & 15u) / ESZ);
+    int64_t head = mis ? (16 / ESZ - mis) : 0;
+    if (head > hi - lo) head = hi - lo;
+    const int64_t n_units = (hi - lo - head) / E;
+    const char* base = g + (lo + head) * ESZ;  // 16-byte aligned
+    constexpr int U = 8;
+    for (int b = 0; b < kClipUnitsPerThread; b += U) {
+      uint4 r[U];
+      bool on[U];
+#pragma unroll
+      for (int v = 0; v < U; ++v) {
+        const int64_t u = static_cast<int64_t>(b + v) * kClipThreads + threadIdx.x;
+        on[v] = u < n_units;
+        r[v] = on[v] ? ldg_stream16(base + u * 16) : make_uint4(0u, 0u, 0u, 0u);
+      }
+#pragma unroll
+      for (int v = 0; v < U; ++v)
+        if (on[v]) acc += static_cast<double>(unit_sumsq<BF16>(r[v]));
+    }
+    const int64_t tail0 = lo + head + n_units * E;
+    const int64_t n_peel = head + (hi - tail0);  // < 2 E
+    if (threadIdx.x < n_peel) {
+      const int64_t i = threadIdx.x < head ? lo + threadIdx.x : tail0 + (threadIdx.x - head);
+      const float x = load_grad_scalar<BF16>(g, i);
+      acc += static_cast<double>(x) * static_cast<double>(x);
+    }
+  }
+  const double total = block_sum(acc, s_warp);
+  if (threadIdx.x == 0) work[static_cast<int64_t>(blockIdx.y) * gridDim.x + blockIdx.x] = total;
+}
+
 // one CTA per worker: fixed-order sum of its chunk partials, then the clip factor (`work` comes from the
 // predecessor kernel: a plain pointer, see K7b)
 __global__ void __launch_bounds__(kClipThreads) clip_finalize_kernel(const double* work, int chunks,
@@ -368,6 +422,37 @@ cudaError_t launch_clip_scales(const void* const* d_grads, int32_t W, int64_t P,
   cudaError_t err = dtype == 1 ? cudaLaunchKernelEx(&cfg, sumsq_chunks_kernel<true>, d_grads, P, work)
                                : cudaLaunchKernelEx(&cfg, sumsq_chunks_kernel<false>, d_grads, P, work);
   if (err != cudaSuccess) return err;
+  pdl_config(&cfg, attr, dim3(static_cast<unsigned>(W)), dim3(kClipThreads), stream);
+  return cudaLaunchKernelEx(&cfg, clip_finalize_kernel, static_cast<const double*>(work), chunks, clip, d_scales);
+}
+
+int64_t clip_chunk_elems(int dtype) { return kClipChunkUnits * (dtype == 1 ? 8 : 4); }
+
+size_t clip_slices_workspace_bytes(int32_t W, int32_t M, int64_t n_chunks) {
+  return sizeof(int64_t) * (static_cast<size_t>(M) + 1) +
+         sizeof(double) * static_cast<size_t>(W) * static_cast<size_t>(n_chunks < 1 ? 1 : n_chunks);
+}
+
+cudaError_t launch_clip_scales_slices(const void* const* d_grads, int32_t W, int32_t M, const int64_t* d_shard_off,
+                                      int64_t n_chunks, int dtype, float clip, float* d_scales, void* d_work,
+                                      cudaStream_t stream) {
+  if (n_chunks > 0x7FFFFFFF) return cudaErrorInvalidConfiguration;
+  int64_t* chunk_start = static_cast<int64_t*>(d_work);
+  double* work = reinterpret_cast<double*>(chunk_start + M + 1);
+  cudaError_t err = launch_shard_worklist_elems(d_shard_off, M, static_cast<int32_t>(clip_chunk_elems(dtype)), chunk_start,
+                                                stream);
+  if (err != cudaSuccess) return err;
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute attr[1];
+  const int chunks = static_cast<int>(n_chunks);
+  if (chunks > 0) {
+    pdl_config(&cfg, attr, dim3(static_cast<unsigned>(chunks), static_cast<unsigned>(W)), dim3(kClipThreads), stream);
+    err = dtype == 1 ? cudaLaunchKernelEx(&cfg, sumsq_slices_kernel<true>, d_grads, M, d_shard_off,
+                                          static_cast<const int64_t*>(chunk_start), work)
+                     : cudaLaunchKernelEx(&cfg, sumsq_slices_kernel<false>, d_grads, M, d_shard_off,
+                                          static_cast<const int64_t*>(chunk_start), work);
+    if (err != cudaSuccess) return err;
+  }
   pdl_config(&cfg, attr, dim3(static_cast<unsigned>(W)), dim3(kClipThreads), stream);
   return cudaLaunchKernelEx(&cfg, clip_finalize_kernel, static_cast<const double*>(work), chunks, clip, d_scales);
 }

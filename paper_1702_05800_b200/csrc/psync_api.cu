@@ -307,6 +307,43 @@ PSYNC_API int psync_clip_scales(const void* const* d_grads, int32_t W, int64_t P
              : PSYNC_ECUDA;
 }
 
+namespace {
+// sum_j ceil(len_j / chunk) for a valid host shard table, -1 otherwise
+int64_t clip_slice_chunks(int32_t M, const int64_t* h_shard_off, int32_t grad_dtype) {
+  if (M < 1 || h_shard_off == nullptr || h_shard_off[0] != 0) return -1;
+  if (grad_dtype != PSYNC_F32 && grad_dtype != PSYNC_BF16) return -1;
+  const int64_t ce = psync::clip_chunk_elems(grad_dtype);
+  int64_t n = 0;
+  for (int32_t j = 0; j < M; ++j) {
+    const int64_t len = h_shard_off[j + 1] - h_shard_off[j];
+    if (len < 0) return -1;
+    n += (len + ce - 1) / ce;
+  }
+  return n;
+}
+}  // namespace
+
+PSYNC_API size_t psync_clip_slices_workspace_bytes(int32_t W, int32_t M, const int64_t* h_shard_off, int32_t grad_dtype) {
+  const int64_t n = clip_slice_chunks(M, h_shard_off, grad_dtype);
+  if (W < 1 || W > PSYNC_MAX_WORKERS || n < 0) return 0;
+  return psync::clip_slices_workspace_bytes(W, M, n);
+}
+
+PSYNC_API int psync_clip_scales_slices(const void* const* d_grads, int32_t W, int32_t M, const int64_t* h_shard_off,
+                             const int64_t* d_shard_off, int32_t grad_dtype, float clip, float* d_scales, void* d_work,
+                             size_t work_bytes, void* stream) {
+  if (d_grads == nullptr || d_shard_off == nullptr || d_scales == nullptr || d_work == nullptr) return PSYNC_EINVAL;
+  if (W < 1 || W > PSYNC_MAX_WORKERS || !(clip > 0.0f)) return PSYNC_EINVAL;
+  const int64_t n = clip_slice_chunks(M, h_shard_off, grad_dtype);
+  if (n < 0) return PSYNC_EINVAL;
+  if (work_bytes < psync::clip_slices_workspace_bytes(W, M, n) || (reinterpret_cast<uintptr_t>(d_work) & 7u) != 0)
+    return PSYNC_EINVAL;
+  return psync::launch_clip_scales_slices(d_grads, W, M, d_shard_off, n, grad_dtype, clip, d_scales, d_work,
+                                          static_cast<cudaStream_t>(stream)) == cudaSuccess
+             ? PSYNC_OK
+             : PSYNC_ECUDA;
+}
+
 PSYNC_API int psync_kth_arrival_stats(const float* d_arrival, int32_t T, int32_t W, float* d_sorted, int32_t* d_count,
                             double* d_mean, double* d_median, const double* d_iters, double* d_est_time, void* stream) {
   if (d_arrival == nullptr || d_sorted == nullptr || d_count == nullptr || d_mean == nullptr || d_median == nullptr)

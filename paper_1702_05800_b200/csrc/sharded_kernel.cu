@@ -299,8 +299,8 @@ KernelFn pick_opt(int opt, int ema) {
 
 int sharded_tile_elems(int dtype) { return kThreads * (dtype == 1 ? 8 : 4); }
 
-cudaError_t launch_shard_worklist(const int64_t* d_shard_off, int32_t M, int dtype, int64_t* d_tile_start,
-                                  cudaStream_t stream) {
+cudaError_t launch_shard_worklist_elems(const int64_t* d_shard_off, int32_t M, int32_t tile_elems, int64_t* d_tile_start,
+                                        cudaStream_t stream) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(1);
   cfg.blockDim = dim3(1024);
@@ -310,8 +310,12 @@ cudaError_t launch_shard_worklist(const int64_t* d_shard_off, int32_t M, int dty
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, shard_worklist_kernel, d_shard_off, M, static_cast<int32_t>(sharded_tile_elems(dtype)),
-                            d_tile_start);
+  return cudaLaunchKernelEx(&cfg, shard_worklist_kernel, d_shard_off, M, tile_elems, d_tile_start);
+}
+
+cudaError_t launch_shard_worklist(const int64_t* d_shard_off, int32_t M, int dtype, int64_t* d_tile_start,
+                                  cudaStream_t stream) {
+  return launch_shard_worklist_elems(d_shard_off, M, static_cast<int32_t>(sharded_tile_elems(dtype)), d_tile_start, stream);
 }
 
 cudaError_t launch_sharded(const FusedParams& p, int dtype, int opt, int ema, int64_t n_tiles, cudaStream_t stream) {

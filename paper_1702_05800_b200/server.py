@@ -109,8 +109,8 @@ class AsyncServerStep:
     """The Async-SGD parameter server (Alg. 2, L78-89): device buffers + the calls of one batch of arrivals.
 
     apply(d_arrival) enqueues, with no host synchronisation: the arrival order (per server with per_server=True,
-    d_arrival [M][W]), optionally the global-norm clip factors (clip > 0; flat buffers only: the norm is over the whole
-    gradient of a worker, L313), optionally the learning rates of this batch's iterations (lr = (gamma0, beta, s):
+    d_arrival [M][W]), optionally the global-norm clip factors (clip > 0: the norm is over the whole gradient of a
+    worker, all of its slices, L313), optionally the learning rates of this batch's iterations (lr = (gamma0, beta, s):
     gamma0 * beta^((t0 + i) s), L315), the one-pass application of the arrivals, and with track_staleness=True (one
     order only) Table 1's bookkeeping.  Plumbing only, no arithmetic."""
 
@@ -159,8 +159,9 @@ class AsyncServerStep:
     def set_gradient_slices(self, slices: Sequence[Sequence[Optional[torch.Tensor]]]) -> None:
         if len(slices) != self.W or any(len(row) != self.M for row in slices):
             raise ValueError(f"need W = {self.W} rows of M = {self.M} slices")
-        if self.clip > 0:
-            raise ValueError("global-norm clipping needs each worker's whole gradient: flat buffers")
+        if self.clip > 0 and any(t is None and self.shard_off[j + 1] > self.shard_off[j]
+                                 for row in slices for j, t in enumerate(row)):
+            raise ValueError("global-norm clipping needs every slice of every worker (the norm is over all of them)")
         if self.table is not None:
             self._retired.append((self.table, self._keep))
         self.table, self.layout, self._step = B.make_slice_table(slices), B.PSYNC_GRADS_SLICES, None
@@ -191,10 +192,17 @@ class AsyncServerStep:
         else:
             B.psync_order_by_arrival(d_arrival, self.W, self.d_order, self.d_n_arrived, stream)
         if self.clip > 0:
-            if self._d_clip_work is None:
-                nbytes = B.psync_clip_workspace_bytes(self.W, self.theta.numel(), self.table.grad_dtype)
-                self._d_clip_work = torch.empty(nbytes // 8, dtype=torch.float64, device=self.theta.device)
-            B.psync_clip_scales(self.table, self.clip, self.d_gscale, self._d_clip_work, stream)
+            sliced = self.layout == B.PSYNC_GRADS_SLICES
+            key = (sliced, self.table.grad_dtype)
+            if self._d_clip_work is None or self._d_clip_work[0] != key:
+                nbytes = (B.psync_clip_slices_workspace_bytes(self.W, self.shard_off, self.table.grad_dtype) if sliced
+                          else B.psync_clip_workspace_bytes(self.W, self.theta.numel(), self.table.grad_dtype))
+                self._d_clip_work = (key, torch.empty((nbytes + 7) // 8, dtype=torch.float64, device=self.theta.device))
+            if sliced:
+                B.psync_clip_scales_slices(self.table, self.shard_off, self.d_shard_off, self.clip, self.d_gscale,
+                                           self._d_clip_work[1], stream)
+            else:
+                B.psync_clip_scales(self.table, self.clip, self.d_gscale, self._d_clip_work[1], stream)
         if self.lr is not None:
             gamma0, beta, s = self.lr
             B.psync_lr_schedule(gamma0, beta, self.t0 if t0 is None else t0, self.W, s, self.d_gamma, stream)

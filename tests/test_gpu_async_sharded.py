@@ -434,3 +434,67 @@ def test_async_server_step_per_server_on_slices_chained_batches():
         for n, t in (("theta", theta), ("ema", ema), ("state0", s0)):
             assert_close(to_np(t), h[n], rtol_async(cfg.W), ATOL_STEP, f"aserver rows batch {s} {n}")
             h[n] = to_np(t)
+
+
+# ------------------------------------------------------------------ K5s: clip factors of sliced gradients
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+def test_clip_scales_slices_match_the_oracle_and_the_flat_kernel(dtype):
+    """Norm over ALL of a worker's slices: ragged servers (an empty and a one-element one), slices at odd element offsets,
+    several 8192-unit chunks per server and a partial last chunk."""
+    cfg = replace(BASE, P=300_007, M=5, N=9, grad_dtype=dtype, grad_dist=("normal", 2e-3), name=f"clips_d{dtype}")
+    off = np.array([0, 1, 1, 70_001, 140_000, 300_007], np.int64)
+    flat = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    for k in range(0, cfg.W, 2):
+        flat[k].mul_(0.25)
+    sl = cut_slices(flat, off, lambda k, j: (3 * k + j) % 8)
+    table = psync.make_slice_table(sl)
+    d_off = torch.from_numpy(off).to(DEV)
+    clip = 0.6
+    nbytes = psync.psync_clip_slices_workspace_bytes(cfg.W, off, table.grad_dtype)
+    assert nbytes > 0
+    d_work = torch.empty((nbytes + 7) // 8, dtype=torch.float64, device=DEV)
+    d_scales = torch.full((cfg.W,), -1.0, device=DEV)
+    psync.psync_clip_scales_slices(table, off, d_off, clip, d_scales, d_work)
+    torch.cuda.synchronize()
+    want = oracle.clip_scales_slices(off, np_slices(sl), clip)
+    got = d_scales.cpu().numpy()
+    assert (want < 1).any() and (want == 1).any()
+    assert np.array_equal(got, want)
+    # the flat kernel on the uncut buffers gives the same factors
+    ft = psync.make_grad_table(flat)
+    d_w2 = torch.empty(psync.psync_clip_workspace_bytes(cfg.W, cfg.P, ft.grad_dtype) // 8, dtype=torch.float64, device=DEV)
+    d_s2 = torch.full((cfg.W,), -1.0, device=DEV)
+    psync.psync_clip_scales(ft, clip, d_s2, d_w2)
+    torch.cuda.synchronize()
+    assert np.array_equal(d_s2.cpu().numpy(), got)
+    L = psync.binding.lib()
+    assert L.psync_clip_scales_slices(None, 3, 2, None, None, 0, 1.0, None, None, 0, None) == psync.PSYNC_EINVAL
+    assert psync.psync_clip_scales_slices(table, off, d_off, 0.0, d_scales, d_work, check=False) == psync.PSYNC_EINVAL
+    assert psync.psync_clip_scales_slices(table, off, d_off, clip, d_scales, d_work[:2], check=False) == psync.PSYNC_EINVAL
+
+
+def test_async_server_step_clips_sliced_gradients_per_server():
+    cfg = replace(BASE, P=50_021, M=7, opt=synth.SGD, grad_dist=("normal", 2e-3), name="aserver_clip_slices")
+    off = np.asarray(synth.shard_offsets(cfg), dtype=np.int64)
+    theta = synth.init_theta(cfg, DEV)
+    ema = theta.clone()
+    clip = 0.4
+    srv = psync.AsyncServerStep(off, cfg.W, theta, ema, None, None, cfg.opt, cfg.ema_mode, alpha=cfg.alpha,
+                                per_server=True, clip=clip)
+    h = {"theta": to_np(theta), "ema": to_np(ema)}
+    flat = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    for k in range(1, cfg.W, 2):
+        flat[k].mul_(0.5)
+    sl = cut_slices(flat, off, lambda k, j: (k + j) % 4)
+    a = synth.arrival_times_per_server(cfg, 0, server_sigma=0.3)
+    srv.set_gradient_slices(sl)
+    srv.apply(torch.from_numpy(a).to(DEV), cfg.gamma)
+    torch.cuda.synchronize()
+    scales = oracle.clip_scales_slices(off, np_slices(sl), clip)
+    assert np.array_equal(srv.d_gscale.cpu().numpy(), scales) and (scales < 1).any() and (scales == 1).any()
+    order = np.stack([oracle.order_by_arrival(a[j]) for j in range(cfg.M)])
+    rc = oracle.async_apply_rows(off, np_slices(sl), order, h["theta"], h["ema"], slices=True, per_shard=True,
+                                 gscales=scales, opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha)
+    assert rc == oracle.OK
+    assert_close(to_np(theta), h["theta"], rtol_async(cfg.W), ATOL_STEP, "aserver clip slices theta")
+    assert_close(to_np(ema), h["ema"], rtol_async(cfg.W), ATOL_STEP, "aserver clip slices ema")
