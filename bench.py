@@ -384,7 +384,10 @@ def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist
                                    grad_layout=psync.PSYNC_GRADS_SLICES if slices else psync.PSYNC_GRADS_FLAT,
                                    d_tile_start=wl.d_tiles if use_tiles else None)
         steps_struct.append((st, keep))
-    geo = psync.psync_launch_geometry(steps_struct[0][0])
+    try:
+        geo = psync.psync_launch_geometry(steps_struct[0][0])
+    except psync.PsyncError:        # an A/B shape of Alg. 2's kernel (--mode async --variant N): no K2 geometry
+        geo = {}
     d_scales = d_clip_work = None
     if is_async and clip > 0:
         d_scales = torch.ones(cfg.W, dtype=torch.float32, device=dev)

@@ -498,3 +498,34 @@ def test_async_server_step_clips_sliced_gradients_per_server():
     assert rc == oracle.OK
     assert_close(to_np(theta), h["theta"], rtol_async(cfg.W), ATOL_STEP, "aserver clip slices theta")
     assert_close(to_np(ema), h["ema"], rtol_async(cfg.W), ATOL_STEP, "aserver clip slices ema")
+
+
+def test_every_server_of_a_per_server_pass_has_the_bits_of_the_flat_kernel_run_with_that_servers_order():
+    """K4s with M different orders == for every j, K4 (flat, one order) run with server j's order, restricted to
+    server j's slice: bit for bit, RMSProp + per-iteration rates + clip factors."""
+    cfg = replace(BASE, P=120_007, M=6, N=11, opt=synth.RMSPROP_MOM, name="arows_vs_k4_rows")
+    a = synth.arrival_times_per_server(cfg, 0, server_sigma=0.4)
+    a[3, 7] = np.inf
+    flat = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    rng = np.random.default_rng(5)
+    gam = torch.from_numpy(rng.uniform(0.01, 0.09, cfg.W).astype(np.float32)).to(DEV)
+    gsc = torch.from_numpy(rng.uniform(0.25, 1.0, cfg.W).astype(np.float32)).to(DEV)
+    rows = RowsPair(cfg)
+    sl = cut_slices(flat, rows.off, lambda k, j: (k + j) % 4)
+    psync.psync_order_by_arrival_sharded(torch.from_numpy(a).to(DEV), cfg.W, rows.M, rows.d_order, rows.d_n)
+    st, keep = rows.make_step(psync.make_slice_table(sl))
+    psync.psync_async_apply(st, gam, d_gscale=gsc)
+    torch.cuda.synchronize()
+    t_flat = psync.make_grad_table(flat)
+    assert len({tuple(r) for r in rows.d_order.cpu().numpy().tolist()}) == rows.M
+    for j in range(rows.M):
+        one = RowsPair(cfg)
+        st1, keep1 = psync.make_step(one.off, cfg.W, cfg.W, t_flat.grad_dtype, one.theta, one.ema, one.state0, one.state1,
+                                     opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu,
+                                     rho=cfg.rho, eps=cfg.eps, d_grads=t_flat.d_ptrs, d_kept=rows.d_order[j],
+                                     d_n_kept=rows.d_n[j:j + 1], kept_stride=cfg.W)
+        psync.psync_async_apply(st1, gam, d_gscale=gsc)
+        torch.cuda.synchronize()
+        lo, hi = int(rows.off[j]), int(rows.off[j + 1])
+        for n in STATE_NAMES:
+            assert np.array_equal(to_np(getattr(rows, n))[lo:hi], to_np(getattr(one, n))[lo:hi]), (j, n)
