@@ -268,6 +268,135 @@ __global__ void __launch_bounds__(THREADS, MINB) async_apply_pair_kernel(const F
   }
 }
 
+// K4 with the gradient stream staged through a per-thread ring in SHARED memory (cp.async, LDGSTS): the loads in flight
+// live in shared memory instead of registers, so D arrivals per thread are on their way while one is applied, without the
+// second register buffer of the pipelined form.  Every thread copies and consumes only its own 16-byte slots, so the only
+// synchronisation is cp.async.wait_group -- no barrier.  Selected by psync_step.variant = 3 in psync_async_apply (flat
+// buffers, one order): an A/B shape, bit-identical to the default.
+template <int D, int MINB, bool BF16, int OPT, int EMA, bool SCALED>
+__global__ void __launch_bounds__(256, MINB) async_apply_ring_kernel(const FusedParams p) {
+  constexpr int THREADS = 256;
+  constexpr int E = BF16 ? 8 : 4;
+  constexpr int Q = E / 4;
+  __shared__ const char* s_ptr[kMaxWorkers];
+  __shared__ float s_gamma[kMaxWorkers];
+  __shared__ float s_scale[kMaxWorkers];
+  __shared__ __align__(16) uint4 s_ring[D][THREADS];
+
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+
+  if (p.status != nullptr && *p.status != 0) return;
+  const int K = p.n_kept ? *p.n_kept : p.N;
+  if (K <= 0 || K > kMaxWorkers) return;
+
+  unsigned misalign = 0;
+  for (int i = threadIdx.x; i < K; i += THREADS) {
+    const int k = p.kept[i];
+    const char* g = static_cast<const char*>(p.grads[k]);
+    s_ptr[i] = g;
+    s_scale[i] = p.gscales ? p.gscales[k] : 1.0f;
+    s_gamma[i] = p.gammas ? p.gammas[i] : p.gamma;
+    misalign |= static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 15u;
+  }
+  const bool vec_ok = (__syncthreads_or(static_cast<int>(misalign)) == 0) && (p.base_aligned != 0);
+
+  const PairCoeffs pc = make_pair_coeffs(p);
+  const int64_t n_units = vec_ok ? p.P / E : 0;
+  const uint32_t slot0 = static_cast<uint32_t>(__cvta_generic_to_shared(&s_ring[0][threadIdx.x]));
+  for (int64_t u = static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x; u < n_units;
+       u += static_cast<int64_t>(gridDim.x) * THREADS) {
+    // D arrivals on their way before anything else (one commit group per arrival, empty past K)
+#pragma unroll
+    for (int i = 0; i < D; ++i) {
+      if (i < K)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(slot0 + i * THREADS * 16), "l"(s_ptr[i] + u * 16)
+                     : "memory");
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+    float4 th4[Q], em4[Q], a04[Q], a14[Q];
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const int64_t e = u * E + 4 * q;
+      th4[q] = ld_state16(p.theta + e);
+      if (EMA != EMA_OFF) em4[q] = ld_state16(p.ema + e);
+      if (OPT != OPT_SGD) a04[q] = ld_state16(p.s0 + e);
+      if (OPT == OPT_RMSPROP_MOM) a14[q] = ld_state16(p.s1 + e);
+    }
+    float2* th = reinterpret_cast<float2*>(th4);
+    float2* em = reinterpret_cast<float2*>(em4);
+    float2* a0 = reinterpret_cast<float2*>(a04);
+    float2* a1 = reinterpret_cast<float2*>(a14);
+    unsigned bad = 0;
+    // one arrival: wait for it (groups retire in order), take it from its slot, apply it, refill the slot with
+    // arrival i + D (the slot is free once its value has been consumed by the update)
+    auto one = [&](int i, int slot) {
+      asm volatile("cp.async.wait_group %0;" ::"n"(D - 1) : "memory");
+      const uint4 r = s_ring[slot][threadIdx.x];
+      apply_unit<BF16, OPT, EMA, SCALED>(r, s_scale[i], s_gamma[i], th, em, a0, a1, pc, bad);
+      if (i + D < K)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(slot0 + slot * THREADS * 16),
+                     "l"(s_ptr[i + D] + u * 16)
+                     : "memory");
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    int i0 = 0;
+    for (; i0 + D <= K; i0 += D) {  // unrolled over the ring: static slots
+#pragma unroll
+      for (int v = 0; v < D; ++v) one(i0 + v, v);
+    }
+    for (int i = i0; i < K; ++i) one(i, i - i0);
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (OPT == OPT_RMSPROP_MOM && rsqrt_pair_left_range(bad)) {  // redo from memory with the checked scalar update
+#pragma unroll
+      for (int q = 0; q < Q; ++q) {
+        const int64_t e = u * E + 4 * q;
+        th4[q] = ld_state16(p.theta + e);
+        if (EMA != EMA_OFF) em4[q] = ld_state16(p.ema + e);
+        a04[q] = ld_state16(p.s0 + e);
+        a14[q] = ld_state16(p.s1 + e);
+      }
+      float* ths = reinterpret_cast<float*>(th4);
+      float* ems = reinterpret_cast<float*>(em4);
+      float* a0s = reinterpret_cast<float*>(a04);
+      float* a1s = reinterpret_cast<float*>(a14);
+      for (int n = 0; n < K; ++n) {
+        const uint4 r = ldg_stream16(s_ptr[n] + u * 16);
+#pragma unroll
+        for (int e = 0; e < E; ++e)
+          update_element_g<OPT, EMA>(unit_element<BF16>(r, e), s_scale[n], s_gamma[n], ths[e], ems[e], a0s[e], a1s[e], p);
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const int64_t e = u * E + 4 * q;
+      st_state16(p.theta + e, th4[q]);
+      if (EMA != EMA_OFF) st_state16(p.ema + e, em4[q]);
+      if (OPT != OPT_SGD) st_state16(p.s0 + e, a04[q]);
+      if (OPT == OPT_RMSPROP_MOM) st_state16(p.s1 + e, a14[q]);
+    }
+  }
+
+  const int64_t tail0 = n_units * E;
+  const bool mine = vec_ok ? (blockIdx.x == 0) : true;
+  if (tail0 < p.P && mine) {
+    const int64_t first = vec_ok ? threadIdx.x : static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x;
+    const int64_t stride = vec_ok ? THREADS : static_cast<int64_t>(gridDim.x) * THREADS;
+    for (int64_t e = tail0 + first; e < p.P; e += stride) {
+      float th = p.theta[e];
+      float em = (EMA != EMA_OFF) ? p.ema[e] : 0.f;
+      float a0 = (OPT != OPT_SGD) ? p.s0[e] : 0.f;
+      float a1 = (OPT == OPT_RMSPROP_MOM) ? p.s1[e] : 0.f;
+      for (int i = 0; i < K; ++i)
+        update_element_g<OPT, EMA>(load_grad_scalar<BF16>(s_ptr[i], e), s_scale[i], s_gamma[i], th, em, a0, a1, p);
+      p.theta[e] = th;
+      if (EMA != EMA_OFF) p.ema[e] = em;
+      if (OPT != OPT_SGD) p.s0[e] = a0;
+      if (OPT == OPT_RMSPROP_MOM) p.s1[e] = a1;
+    }
+  }
+}
+
 // K1c: rank sort of <= 1024 keys in one CTA.  Thread i owns worker i: its rank is the number of eligible
 // workers that come before it in (arrival, index) order; -0.0 == +0.0; non-finite = never arrived.
 // One CTA per row: row r of arrival [rows][W] is what parameter server r saw (Alg. 2 is the program of one server j).
@@ -376,6 +505,56 @@ KernelFn pick_pair(int opt, int ema, bool scaled) {
     case OPT_MOMENTUM: return pick_pair_ema<OPT_MOMENTUM>(ema, scaled);
     default: return pick_pair_ema<OPT_RMSPROP_MOM>(ema, scaled);
   }
+}
+
+// the shared-memory ring (cp.async): {ring depth, CTAs per SM}.  Depth 4 / 6 / 8 are within 1 % of one another on
+// every shape (cfg3's: 1.769 / 1.753 / 1.759 ms), 5 or 6 CTAs/SM are slower (profiles/r2_async.md).
+struct RingShape {
+  int depth, minb;
+};
+#ifndef PSYNC_RING_BF16_MINB
+#define PSYNC_RING_BF16_MINB 3
+#endif
+constexpr RingShape ring_shape_for(bool bf16, int opt) {
+  return bf16 ? (opt == OPT_RMSPROP_MOM ? RingShape{6, 3} : RingShape{6, PSYNC_RING_BF16_MINB}) : RingShape{6, 4};
+}
+template <bool BF16, int OPT, int EMA>
+KernelFn pick_ring_scaled(bool scaled) {
+  constexpr RingShape S = ring_shape_for(BF16, OPT);
+  return scaled ? async_apply_ring_kernel<S.depth, S.minb, BF16, OPT, EMA, true>
+                : async_apply_ring_kernel<S.depth, S.minb, BF16, OPT, EMA, false>;
+}
+template <bool BF16, int OPT>
+KernelFn pick_ring_ema(int ema, bool scaled) {
+  switch (ema) {
+    case EMA_POST: return pick_ring_scaled<BF16, OPT, EMA_POST>(scaled);
+    case EMA_PRE: return pick_ring_scaled<BF16, OPT, EMA_PRE>(scaled);
+    default: return pick_ring_scaled<BF16, OPT, EMA_OFF>(scaled);
+  }
+}
+template <bool BF16>
+KernelFn pick_ring(int opt, int ema, bool scaled) {
+  switch (opt) {
+    case OPT_SGD: return pick_ring_ema<BF16, OPT_SGD>(ema, scaled);
+    case OPT_MOMENTUM: return pick_ring_ema<BF16, OPT_MOMENTUM>(ema, scaled);
+    default: return pick_ring_ema<BF16, OPT_RMSPROP_MOM>(ema, scaled);
+  }
+}
+
+cudaError_t launch_async_apply_ring(const FusedParams& p, int dtype, int opt, int ema, int grid_ctas, cudaStream_t stream) {
+  FusedGeometry g;
+  async_geometry(dtype, grid_ctas, p.P, &g);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(static_cast<unsigned>(g.grid));
+  cfg.blockDim = dim3(256);
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  const bool scaled = p.gscales != nullptr;
+  return cudaLaunchKernelEx(&cfg, dtype == 1 ? pick_ring<true>(opt, ema, scaled) : pick_ring<false>(opt, ema, scaled), p);
 }
 
 cudaError_t launch_async_apply_pair(const FusedParams& p, int opt, int ema, int grid_ctas, cudaStream_t stream) {

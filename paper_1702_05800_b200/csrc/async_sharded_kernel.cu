@@ -111,7 +111,7 @@ __device__ __forceinline__ void load_state(const Geom<E>& g, const FusedParams& 
   if (OPT == OPT_RMSPROP_MOM) load_arr<E>(g, p.s1, a14, 0.f);
 }
 
-template <bool BF16, int OPT, int EMA, bool SCALED, int U, int MINB, bool PIPE>
+template <bool BF16, int OPT, int EMA, bool SCALED, int D, int MINB>
 __global__ void __launch_bounds__(kThreads, MINB) async_sharded_kernel(const FusedParams p) {
   constexpr int E = BF16 ? 8 : 4;
   constexpr int ESZ = BF16 ? 2 : 4;
@@ -121,6 +121,7 @@ __global__ void __launch_bounds__(kThreads, MINB) async_sharded_kernel(const Fus
   __shared__ float s_scale[kMaxWorkers];
   __shared__ __align__(16) float s_seg[kThreads * E];
   __shared__ int64_t s_meta[4];  // off_j, len_j, h, tile: what Geom is derived from, re-read after the gradient loop
+  __shared__ __align__(16) uint4 s_ring[D][kThreads];  // per-thread cp.async ring of arrivals on their way (as K4's)
 
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -183,17 +184,21 @@ __global__ void __launch_bounds__(kThreads, MINB) async_sharded_kernel(const Fus
 
   float4 th4[Q], em4[Q], a04[Q], a14[Q];
   int64_t goff;  // byte offset of this thread's unit in every arrival's slice
-  const int n_batches = mixed ? 0 : K / U;  // mixed phases: everything goes through the narrow-load loop below
-  uint4 cur[U], nxt[U];
+  const uint32_t slot0 = static_cast<uint32_t>(__cvta_generic_to_shared(&s_ring[0][threadIdx.x]));
   {
     const Geom<E> g = make_geom<E>(meta[0], meta[1], static_cast<int>(meta[2]), meta[3], p.base_aligned, s_seg);
     if (g.u0 >= g.nu) goto peel;  // CTA-uniform: this tile holds no whole unit (a server shorter than its head)
     goff = g.unit * 16;
-    // the first batch of gradients is requested BEFORE the state: when theta is not co-aligned its loads are followed
-    // by a trip through shared memory, and the gradient stream should not wait for that
-    if (n_batches > 0) {
+    // the first D arrivals are requested BEFORE the state: when theta is not co-aligned its loads are followed by a
+    // trip through shared memory, and the gradient stream should not wait for that (one commit group per arrival)
+    if (!mixed) {
 #pragma unroll
-      for (int v = 0; v < U; ++v) cur[v] = ldg_stream16(s_ptr[v] + goff);
+      for (int i = 0; i < D; ++i) {
+        if (i < K)
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(slot0 + i * kThreads * 16), "l"(s_ptr[i] + goff)
+                       : "memory");
+        asm volatile("cp.async.commit_group;" ::: "memory");
+      }
     }
     load_state<E, OPT, EMA>(g, p, th4, em4, a04, a14);
   }
@@ -206,34 +211,25 @@ __global__ void __launch_bounds__(kThreads, MINB) async_sharded_kernel(const Fus
 
     unsigned bad = 0;  // RMSProp: did any ms + eps leave the range of the unchecked packed rsqrt?
     if (!mixed) {
-      // software-pipelined batches of U arrivals, exactly K4's loop: the loads of batch b+1 fly while batch b is applied
-      for (int bt = 0; bt < n_batches; ++bt) {
-        const int i = bt * U;
-        if (PIPE) {
-          if (bt + 1 < n_batches) {
-#pragma unroll
-            for (int v = 0; v < U; ++v) nxt[v] = ldg_stream16(s_ptr[i + U + v] + goff);
-          }
-          // Scheduling fence.  Without it ptxas predicates the loads above and sinks them below the updates (or, with
-          // the last batch peeled, merges the two buffers): the next batch is then in flight for a few instructions
-          // only and the warp waits for every batch -- 48 % of all stall samples, +8 % kernel time (ncu, r2_async.md).
-          __syncwarp();
-        }
-#pragma unroll
-        for (int v = 0; v < U; ++v)
-          apply_unit<BF16, OPT, EMA, SCALED>(cur[v], s_scale[i + v], s_gamma[i + v], th, em, a0, a1, pc, bad);
-        if (PIPE) {
-#pragma unroll
-          for (int v = 0; v < U; ++v) cur[v] = nxt[v];
-        } else if (bt + 1 < n_batches) {  // one buffer: U independent loads in flight, then U dependent updates
-#pragma unroll
-          for (int v = 0; v < U; ++v) cur[v] = ldg_stream16(s_ptr[i + U + v] + goff);
-        }
-      }
-      for (int i = n_batches * U; i < K; ++i) {
-        const uint4 r = ldg_stream16(s_ptr[i] + goff);
+      // K4's loop: wait for arrival i (groups retire in order), take it from its slot, apply it, refill the slot with
+      // arrival i + D.  Every thread copies and consumes only its own slots: no barrier.
+      auto one = [&](int i, int slot) {
+        asm volatile("cp.async.wait_group %0;" ::"n"(D - 1) : "memory");
+        const uint4 r = s_ring[slot][threadIdx.x];
         apply_unit<BF16, OPT, EMA, SCALED>(r, s_scale[i], s_gamma[i], th, em, a0, a1, pc, bad);
+        if (i + D < K)
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(slot0 + slot * kThreads * 16),
+                       "l"(s_ptr[i + D] + goff)
+                       : "memory");
+        asm volatile("cp.async.commit_group;" ::: "memory");
+      };
+      int i0 = 0;
+      for (; i0 + D <= K; i0 += D) {
+#pragma unroll
+        for (int v = 0; v < D; ++v) one(i0 + v, v);
       }
+      for (int i = i0; i < K; ++i) one(i, i - i0);
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
     } else {
 #pragma unroll 2
       for (int i = 0; i < K; ++i) {
@@ -294,14 +290,13 @@ peel:
   }
 }
 
-// arrivals per batch, CTAs per SM, software-pipelined or not: K4's shapes (async_kernel.cu), measured there
+// ring depth and CTAs per SM (K4's ring shapes; bf16 has a 8 KB transpose buffer, so a shallower ring keeps the CTA
+// within 48 KB of static shared memory)
 struct Shape {
-  int unroll, minb;
-  bool pipe;
+  int depth, minb;
 };
 constexpr Shape shape_for(bool bf16, int opt) {
-  return bf16 ? (opt == OPT_RMSPROP_MOM ? Shape{2, 2, true} : Shape{8, 3, false})
-              : (opt == OPT_RMSPROP_MOM ? Shape{3, 4, true} : Shape{4, 4, true});
+  return bf16 ? (opt == OPT_RMSPROP_MOM ? Shape{4, 3} : Shape{4, 3}) : Shape{6, 4};
 }
 
 using KernelFn = void (*)(const FusedParams);
@@ -309,8 +304,8 @@ using KernelFn = void (*)(const FusedParams);
 template <bool BF16, int OPT, int EMA>
 KernelFn pick_scaled(bool scaled) {
   constexpr Shape S = shape_for(BF16, OPT);
-  return scaled ? async_sharded_kernel<BF16, OPT, EMA, true, S.unroll, S.minb, S.pipe>
-                : async_sharded_kernel<BF16, OPT, EMA, false, S.unroll, S.minb, S.pipe>;
+  return scaled ? async_sharded_kernel<BF16, OPT, EMA, true, S.depth, S.minb>
+                : async_sharded_kernel<BF16, OPT, EMA, false, S.depth, S.minb>;
 }
 template <bool BF16, int OPT>
 KernelFn pick_ema(int ema, bool scaled) {

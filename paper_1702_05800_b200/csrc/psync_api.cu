@@ -272,9 +272,12 @@ PSYNC_API int psync_order_by_arrival_sharded(const float* d_arrival, int32_t W, 
 PSYNC_API int psync_async_apply(const psync_step* step, const float* d_gamma, const float* d_gscale, void* stream) {
   if (step == nullptr) return PSYNC_EINVAL;
   psync_step s = *step;
-  const bool pair_shape = step->variant == 2 && step->grad_dtype == PSYNC_F32 && step->per_shard == 0 &&
-                          step->grad_layout == PSYNC_GRADS_FLAT;  // A/B: 8-byte units (flat fp32 only)
-  s.variant = 0;  // otherwise ignored here: Alg. 2's kernels have one launch shape per instance
+  // launch shapes of the flat single-order kernel: 0 / 3 the shared-memory ring (default), 1 the register-pipelined form,
+  // 2 8-byte units (fp32 only); the sharded kernel has one shape
+  const bool flat_one_order = step->per_shard == 0 && step->grad_layout == PSYNC_GRADS_FLAT;
+  const bool pair_shape = step->variant == 2 && step->grad_dtype == PSYNC_F32 && flat_one_order;
+  const bool ring_shape = (step->variant == 0 || step->variant == 3) && flat_one_order;
+  s.variant = 0;
   const int st = check_step(&s, true);
   if (st != PSYNC_OK) return st;
   // Alg. 2 per server (one order row per server) walks the (server, tile) work list like the slices layout does
@@ -284,6 +287,7 @@ PSYNC_API int psync_async_apply(const psync_step* step, const float* d_gamma, co
   p.gammas = d_gamma;
   p.gscales = d_gscale;
   const cudaError_t err =
+      ring_shape ? psync::launch_async_apply_ring(p, s.grad_dtype, s.opt, s.ema_mode, s.grid_ctas, static_cast<cudaStream_t>(stream)) :
       pair_shape ? psync::launch_async_apply_pair(p, s.opt, s.ema_mode, s.grid_ctas, static_cast<cudaStream_t>(stream)) :
       wants_sharded(&s) ? psync::launch_async_sharded(p, s.grad_dtype, s.opt, s.ema_mode, sharded_tiles(&s),
                                                       static_cast<cudaStream_t>(stream))
