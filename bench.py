@@ -531,6 +531,13 @@ def run_also(psync, args, wl3, stream, peak):
         out.append(short_entry(cfg3, "first_n", "flat", m, peak,
                                "variant 5: cp.async.bulk + mbarrier ring" if v == 5 else "variant 6: 256-bit loads"))
         out[-1]["variant"] = v
+    for v in (1, 2):                     # Alg. 2's other launch shapes, re-measured every run (profiles/r2_async.md)
+        wl3.reset_state()
+        m = measure(psync, args, wl3, "async", K, Wm, stream, variant=v, probe_every=2)
+        out.append(short_entry(cfg3, "async", "flat", m, peak,
+                               "variant 1: two register buffers, software-pipelined (the default is the cp.async ring)"
+                               if v == 1 else "variant 2: 8-byte units, one pair of parameters per thread"))
+        out[-1]["variant"] = v
     sets3 = len(wl3.tables)
     del wl3.tables[1:], wl3.sets[1:]     # keep one flat set for the cpu_baseline leg; make room
     torch.cuda.empty_cache()

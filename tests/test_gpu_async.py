@@ -309,27 +309,32 @@ def test_staleness_round_robin_is_W_minus_1_and_bad_batches_write_nothing():
     assert status == psync.PSYNC_EINVAL and int(d_t.item()) == 3 * W
 
 
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
 @pytest.mark.parametrize("opt", [synth.SGD, synth.MOMENTUM, synth.RMSPROP_MOM])
-def test_async_pair_shape_variant_2_is_bit_identical_to_the_default(opt):
-    """psync_step.variant = 2 in psync_async_apply: 8-byte units, one pair of parameters per thread (an A/B shape)."""
-    cfg = replace(BASE, P=200_003, opt=opt, ema_mode=synth.EMA_POST, name="async_pair")
-    a = synth.arrival_times(cfg, 0)
-    a[3] = np.inf
+def test_async_launch_shapes_are_bit_identical(opt, dtype):
+    """psync_step.variant in psync_async_apply: 0 = the cp.async ring (default), 1 = two register buffers, 2 = 8-byte
+    units (fp32 only).  K = 12 of 13 arrivals: two turns of the 6-deep ring, no remainder; K = 13 on the scaled leg."""
+    cfg = replace(BASE, P=200_003, opt=opt, grad_dtype=dtype, ema_mode=synth.EMA_POST, name="async_shapes")
     grads = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
     table = psync.make_grad_table(grads)
     rng = np.random.default_rng(9)
     gam = torch.from_numpy(rng.uniform(0.01, 0.09, cfg.W).astype(np.float32)).to(DEV)
     gsc = torch.from_numpy(rng.uniform(0.25, 1.0, cfg.W).astype(np.float32)).to(DEV)
-    out = []
-    for variant, scaled in ((0, False), (2, False), (0, True), (2, True)):
-        pair = AsyncPair(cfg)
-        psync.psync_order_by_arrival(torch.from_numpy(a).to(DEV), cfg.W, pair.d_order, pair.d_n)
-        st, keep = pair.make_step(table)
-        st.variant = variant
-        psync.psync_async_apply(st, gam, d_gscale=gsc if scaled else None)
-        torch.cuda.synchronize()
-        out.append({n: to_np(getattr(pair, n)) for n in STATE_NAMES if getattr(pair, n) is not None})
-    for x, y in ((out[0], out[1]), (out[2], out[3])):
-        for n in x:
-            assert np.array_equal(x[n], y[n]), n
-    assert not np.array_equal(out[0]["theta"], out[2]["theta"])
+    variants = (0, 1, 2) if dtype == synth.F32 else (0, 1)
+    results = {}
+    for scaled in (False, True):
+        a = synth.arrival_times(cfg, 0)
+        if not scaled:
+            a[3] = np.inf
+        for variant in variants:
+            pair = AsyncPair(cfg)
+            psync.psync_order_by_arrival(torch.from_numpy(a).to(DEV), cfg.W, pair.d_order, pair.d_n)
+            st, keep = pair.make_step(table)
+            st.variant = variant
+            psync.psync_async_apply(st, gam, d_gscale=gsc if scaled else None)
+            torch.cuda.synchronize()
+            results[(scaled, variant)] = {n: to_np(getattr(pair, n)) for n in STATE_NAMES if getattr(pair, n) is not None}
+        for variant in variants[1:]:
+            for n, x in results[(scaled, 0)].items():
+                assert np.array_equal(x, results[(scaled, variant)][n]), (scaled, variant, n)
+    assert not np.array_equal(results[(False, 0)]["theta"], results[(True, 0)]["theta"])
