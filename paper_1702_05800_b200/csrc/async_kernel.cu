@@ -18,7 +18,11 @@
 // elements with the packed fp32x2 instructions (FFMA2 / FMUL2: half the issue slots, same bits), the
 // step is (gamma G) * rsqrt(ms + eps) with the correctly rounded rsqrt computed by an 8-operation
 // refinement of MUFU.RSQ whose range check is a sticky flag outside the inner loop (psync_device.cuh),
-// and the loads of the next batch of gradients are in flight while the current batch is applied.
+// and the gradients of the next arrivals are on their way while the current one is applied.
+// Three launch shapes of the same arithmetic (psync_step.variant in psync_async_apply; bit-identical, tested):
+//   async_apply_ring_kernel  (0, default) the stream staged through a per-thread cp.async ring in shared memory
+//   async_apply_kernel       (1) two register buffers, software-pipelined batches
+//   async_apply_pair_kernel  (2) 8-byte units, one pair of parameters per thread (fp32 only)
 
 #include "async_common.cuh"
 

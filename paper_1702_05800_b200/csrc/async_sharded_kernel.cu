@@ -15,7 +15,7 @@
 // tile) of the work list, the 128-bit gradient stream aligned to the server's first slice (head peel to its first
 // 128-byte line), narrower loads for a slice with another 16-byte phase, head / tail elements done one by one by the
 // server's first CTA.  Same arithmetic per element as K4 (async_kernel.cu: K dependent optimizer steps + EMAs in
-// registers, packed fp32x2, software-pipelined gradient batches): bit-identical to it and to K launches of the
+// registers, packed fp32x2, the gradient stream staged through a per-thread cp.async ring): bit-identical to it and to K launches of the
 // synchronous step with N = 1 (tested).
 // What differs from K2s: the state cannot wait for the end of the gradient stream -- every arriving gradient is
 // applied to it -- so when theta's slice is not co-aligned with the gradient units (ragged cuts: off[j] + h is not a
@@ -33,10 +33,10 @@ constexpr int kThreads = 256;  // = PSYNC_TILE_UNITS: one 16-byte unit per threa
 
 // Where this thread's unit and its warp's segment lie, derived from four CTA-uniform numbers.  The kernel derives it
 // twice: before the gradient loop from registers, and after it from a copy of the four numbers in shared memory read
-// through a volatile pointer -- so that none of these addresses stays live across the loop.  (With them live, ptxas
-// ran out of the 64 registers that 4 CTAs/SM allow, merged the loop's two gradient buffers into one and loaded the
-// next batch only after the current one was consumed: the warp then waited for every batch, 48 % of all stall
-// samples and 8 % of the kernel; ncu, profiles/r2_async.md.)
+// through a volatile pointer -- so that none of these addresses stays live across the loop, which needs all of the 64
+// registers that 4 CTAs/SM allow for the state, the update's temporaries and the stream's addresses.  (History: in
+// the register-pipelined form of the loop ptxas, short of registers, merged the two gradient buffers into one and the
+// warp waited for every batch -- 48 % of all stall samples; profiles/r2_async.md.)
 template <int E>
 struct Geom {
   int64_t nu, u0, e0, unit, seg_e0, live_in_seg;

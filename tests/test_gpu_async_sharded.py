@@ -529,3 +529,49 @@ def test_every_server_of_a_per_server_pass_has_the_bits_of_the_flat_kernel_run_w
         lo, hi = int(rows.off[j]), int(rows.off[j + 1])
         for n in STATE_NAMES:
             assert np.array_equal(to_np(getattr(rows, n))[lo:hi], to_np(getattr(one, n))[lo:hi]), (j, n)
+
+
+def test_async_server_step_is_capturable_in_a_cuda_graph_and_replays_bit_identically():
+    """One batch of Alg. 2 per server on slices with clipping and a schedule -- order, norms (3 launches), rates, the
+    one-pass application -- makes no synchronising call: captured once, replayed with new arrival times, the result is
+    bit-identical to the same calls made eagerly."""
+    cfg = replace(BASE, P=50_021, M=7, opt=synth.MOMENTUM, grad_dist=("normal", 2e-3), name="aserver_graph")
+    off = np.asarray(synth.shard_offsets(cfg), dtype=np.int64)
+    flat = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    sl = cut_slices(flat, off, lambda k, j: (k + j) % 4)
+
+    def server():
+        theta = synth.init_theta(cfg, DEV)
+        s0, _ = synth.init_state(cfg, DEV)
+        srv = psync.AsyncServerStep(off, cfg.W, theta, theta.clone(), s0, None, cfg.opt, cfg.ema_mode, alpha=cfg.alpha,
+                                    mu=cfg.mu, per_server=True, clip=0.4, lr=(0.045, 0.94, 1.0 / 40.0))
+        srv.set_gradient_slices(sl)
+        return srv
+
+    arrs = [torch.from_numpy(synth.arrival_times_per_server(cfg, s, server_sigma=0.3)).to(DEV) for s in range(3)]
+    eager = server()
+    for s in (1, 2):
+        eager.apply(arrs[s], t0=0)
+    torch.cuda.synchronize()
+
+    cap = server()
+    d_arr = arrs[0].clone()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        snap = {n: getattr(cap, n).clone() for n in ("theta", "ema", "state0")}
+        cap.apply(d_arr, t0=0, stream=side)                      # warm-up outside capture (builds work list, workspace)
+        side.synchronize()
+        for n, v in snap.items():
+            getattr(cap, n).copy_(v)
+        with torch.cuda.graph(graph, stream=side):
+            cap.apply(d_arr, t0=0, stream=side)
+    torch.cuda.synchronize()
+    for s in (1, 2):
+        d_arr.copy_(arrs[s])
+        graph.replay()
+    torch.cuda.synchronize()
+    for n in ("theta", "ema", "state0"):
+        assert np.array_equal(to_np(getattr(cap, n)), to_np(getattr(eager, n))), n
+    assert not np.array_equal(to_np(cap.theta), to_np(snap["theta"]))
