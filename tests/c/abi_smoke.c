@@ -137,6 +137,52 @@ int main(void) {
     for (int i = 0; i < P; ++i) CHECK(h[i] == 0.6875f);
     CHECK(cudaMemcpy(h, d_ema, sizeof(float) * P, cudaMemcpyDeviceToHost) == cudaSuccess);
     for (int i = 0; i < P; ++i) CHECK(h[i] == 0.5f * 0.359375f + 0.34375f);
+    /* Alg. 2 per parameter server on the same slices: every arriving gradient is one iteration, each
+     * server in ITS arrival order; worker 4 never arrives (its slices are NULL).  theta = 1, ema = 0, gamma = 0.5,
+     * alpha = 0.5, EMA_PRE (the literal L87), gradients 0.25 (k+1):
+     *   server 0: order {3,0,2,1}: theta 1 -> .5 -> .375 -> 0 -> -.25;   ema .5 -> .5 -> .4375 -> .21875
+     *   server 1: order {1,0,3,2}: theta 1 -> .75 -> .625 -> .125 -> -.25; ema .5 -> .625 -> .625 -> .375
+     * Clip factors of the sliced gradients with a bound no norm reaches: exactly 1. */
+    {
+      const float arr2[M][W] = {{0.5f, 2.0f, 1.0f, 0.125f, INFINITY}, {1.0f, 0.25f, 4.0f, 2.0f, NAN}};
+      const int32_t want_order[M][4] = {{3, 0, 2, 1}, {1, 0, 3, 2}};
+      float *d_arr2, *d_scales, scales[W];
+      int32_t *d_order, *d_n, order[M][W], n_arr[M];
+      void* d_work;
+      const size_t work_bytes = psync_clip_slices_workspace_bytes(4, M, shard_off, PSYNC_F32);
+      CHECK(work_bytes > 0);
+      CHECK(cudaMalloc((void**)&d_arr2, sizeof(arr2)) == cudaSuccess);
+      CHECK(cudaMalloc((void**)&d_scales, sizeof(scales)) == cudaSuccess);
+      CHECK(cudaMalloc((void**)&d_order, sizeof(order)) == cudaSuccess);
+      CHECK(cudaMalloc((void**)&d_n, sizeof(n_arr)) == cudaSuccess);
+      CHECK(cudaMalloc(&d_work, work_bytes) == cudaSuccess);
+      CHECK(cudaMemcpy(d_arr2, arr2, sizeof(arr2), cudaMemcpyHostToDevice) == cudaSuccess);
+      CHECK(cudaMemset(d_scales, 0xFF, sizeof(scales)) == cudaSuccess);
+      CHECK(psync_clip_scales_slices((const void* const*)d_slices, 4, M, shard_off, d_off, PSYNC_F32, 1.0e6f, d_scales,
+                                     d_work, work_bytes, NULL) == PSYNC_OK);       /* workers 0..3: the first 4 rows */
+      CHECK(psync_clip_scales_slices((const void* const*)d_slices, 4, M, shard_off, d_off, PSYNC_F32, 0.0f, d_scales,
+                                     d_work, work_bytes, NULL) == PSYNC_EINVAL);
+      CHECK(psync_order_by_arrival_sharded(d_arr2, W, M, d_order, d_n, NULL) == PSYNC_OK);
+      for (int i = 0; i < P; ++i) h[i] = 1.0f;
+      CHECK(cudaMemcpy(d_theta, h, sizeof(float) * P, cudaMemcpyHostToDevice) == cudaSuccess);
+      CHECK(cudaMemset(d_ema, 0, sizeof(float) * P) == cudaSuccess);
+      st.N = W; st.d_kept = d_order; st.d_status = NULL; st.d_n_kept = d_n; st.kept_stride = W; st.per_shard = 1;
+      st.ema_mode = PSYNC_EMA_PRE;
+      CHECK(psync_async_apply(&st, NULL, d_scales, NULL) == PSYNC_OK);
+      CHECK(cudaDeviceSynchronize() == cudaSuccess);
+      CHECK(cudaMemcpy(scales, d_scales, sizeof(scales), cudaMemcpyDeviceToHost) == cudaSuccess);
+      for (int k = 0; k < 4; ++k) CHECK(scales[k] == 1.0f);
+      CHECK(cudaMemcpy(order, d_order, sizeof(order), cudaMemcpyDeviceToHost) == cudaSuccess);
+      CHECK(cudaMemcpy(n_arr, d_n, sizeof(n_arr), cudaMemcpyDeviceToHost) == cudaSuccess);
+      for (int j = 0; j < M; ++j) {
+        CHECK(n_arr[j] == 4);
+        for (int i = 0; i < 4; ++i) CHECK(order[j][i] == want_order[j][i]);
+      }
+      CHECK(cudaMemcpy(h, d_theta, sizeof(float) * P, cudaMemcpyDeviceToHost) == cudaSuccess);
+      for (int i = 0; i < P; ++i) CHECK(h[i] == -0.25f);
+      CHECK(cudaMemcpy(h, d_ema, sizeof(float) * P, cudaMemcpyDeviceToHost) == cudaSuccess);
+      for (int i = 0; i < P; ++i) CHECK(h[i] == (i < shard_off[1] ? 0.21875f : 0.375f));
+    }
   }
   printf("abi_smoke ok: %s\n", psync_status_string(PSYNC_OK));
   return 0;
