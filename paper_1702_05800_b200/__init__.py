@@ -6,7 +6,7 @@ buffers of one parameter server, `synth` draws the seeded synthetic workloads, `
 libpsync.so in-tree.  Nothing in this package imports oracle/.
 """
 from . import binding, synth  # noqa: F401
-from .binding import (psync_staleness, HostCtx, PSYNC_GRADS_FLAT, PSYNC_GRADS_SLICES, make_slice_table, psync_shard_worklist, PSYNC_BF16, PSYNC_ECUDA, PSYNC_EINVAL, PSYNC_EMA_OFF, PSYNC_EMA_POST, PSYNC_EMA_PRE,  # noqa: F401
+from .binding import (psync_staleness, psync_staleness_sharded, HostCtx, PSYNC_GRADS_FLAT, PSYNC_GRADS_SLICES, make_slice_table, psync_shard_worklist, PSYNC_BF16, PSYNC_ECUDA, PSYNC_EINVAL, PSYNC_EMA_OFF, PSYNC_EMA_POST, PSYNC_EMA_PRE,  # noqa: F401
                       PSYNC_ETOOFEW, PSYNC_EUNSUPPORTED, PSYNC_F32, PSYNC_MOMENTUM, PSYNC_OK, PSYNC_RMSPROP_MOM, PSYNC_SGD, PsyncError,
                       make_grad_table, make_step, psync_aggregate_update, psync_async_apply, psync_ema,
                       psync_order_by_arrival, psync_order_by_arrival_sharded, psync_step_device, psync_clip_scales, psync_clip_workspace_bytes, psync_clip_scales_slices, psync_clip_slices_workspace_bytes,

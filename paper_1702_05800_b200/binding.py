@@ -26,7 +26,7 @@ PSYNC_MAX_WORKERS = 1024
 PSYNC_TILE_UNITS = 256
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
-           "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_order_by_arrival_sharded", "psync_clip_slices_workspace_bytes", "psync_clip_scales_slices", "psync_async_apply", "psync_staleness", "psync_step_device", "psync_clip_workspace_bytes",
+           "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_order_by_arrival_sharded", "psync_clip_slices_workspace_bytes", "psync_clip_scales_slices", "psync_async_apply", "psync_staleness", "psync_staleness_sharded", "psync_step_device", "psync_clip_workspace_bytes",
            "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_host_ctx_create", "psync_host_ctx_destroy",
            "psync_step_host_ctx", "psync_launch_geometry", "psync_probe_read",
@@ -87,6 +87,8 @@ def lib() -> ctypes.CDLL:
         L.psync_order_by_arrival_sharded.restype = ctypes.c_int
         L.psync_staleness.argtypes = [vp, i32, vp, vp, i32, vp, i32, vp, vp, vp, vp]
         L.psync_staleness.restype = ctypes.c_int
+        L.psync_staleness_sharded.argtypes = [vp, i32, i32, vp, vp, i32, vp, i32, vp, vp, vp, vp]
+        L.psync_staleness_sharded.restype = ctypes.c_int
         L.psync_async_apply.argtypes = [ctypes.POINTER(psync_step), vp, vp, vp]
         L.psync_clip_workspace_bytes.argtypes = [i32, i64, i32]
         L.psync_clip_workspace_bytes.restype = ctypes.c_size_t
@@ -594,4 +596,25 @@ def psync_staleness(d_read_iter: torch.Tensor, d_order: torch.Tensor, d_t: torch
                                _dptr(d_status, torch.int32, "d_status"), _stream(stream))
     if check and st != PSYNC_OK:
         raise PsyncError(st, "psync_staleness")
+    return st
+
+
+def psync_staleness_sharded(d_read_iter: torch.Tensor, d_order: torch.Tensor, d_t: torch.Tensor, d_staleness: torch.Tensor,
+                            d_stats: torch.Tensor, d_status: torch.Tensor, K: int = 0,
+                            d_n_arrived: Optional[torch.Tensor] = None, lag: int = 0, stream=None, check: bool = True) -> int:
+    """Table 1's bookkeeping per parameter server (include/psync.h: psync_staleness_sharded): d_read_iter [M][W]."""
+    if d_read_iter.dim() != 2:
+        raise ValueError("d_read_iter must be [M][W]")
+    M, W = d_read_iter.shape
+    if (d_order.numel() < M * W or d_staleness.numel() < M * W or d_stats.numel() < 6 * M or d_t.numel() < M or
+            d_status.numel() < M or (d_n_arrived is not None and d_n_arrived.numel() < M)):
+        raise ValueError("need d_order [M][W], d_staleness [M][W], d_stats [M][6], d_t [M], d_status [M], d_n_arrived [M]")
+    st = lib().psync_staleness_sharded(_dptr(d_read_iter, torch.int64, "d_read_iter"), W, M,
+                                       _dptr(d_order, torch.int32, "d_order"),
+                                       _dptr(d_n_arrived, torch.int32, "d_n_arrived"), K, _dptr(d_t, torch.int64, "d_t"),
+                                       lag, _dptr(d_staleness, torch.int64, "d_staleness"),
+                                       _dptr(d_stats, torch.float64, "d_stats"), _dptr(d_status, torch.int32, "d_status"),
+                                       _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_staleness_sharded")
     return st

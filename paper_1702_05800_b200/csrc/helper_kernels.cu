@@ -330,9 +330,20 @@ void pdl_config(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* attr, dim3 grid, d
 // read sees t + lag + i + 1.  Validation (a worker twice in one batch, a read from the future) happens before anything
 // is written.  Statistics: min / max by reduction, mean = sum / K (integer sum, exact), the population standard
 // deviation summed by one thread in index order (the order the oracle uses), the median from a rank sort.
-__global__ void __launch_bounds__(1024) staleness_kernel(int64_t* read_iter, int32_t W, const int32_t* order,
-                                                         const int32_t* n_arrived, int32_t K_arg, int64_t* t_counter,
-                                                         int32_t lag, int64_t* staleness, double* stats, int32_t* status) {
+// One CTA per row: row r of every array is parameter server r's own bookkeeping (its counter, what each worker last read
+// from IT, the order its gradients reached IT); rows = 1 is the single-order form.
+__global__ void __launch_bounds__(1024) staleness_kernel(int64_t* read_iter_rows, int32_t W, const int32_t* order_rows,
+                                                         const int32_t* n_arrived_rows, int32_t K_arg,
+                                                         int64_t* t_counter_rows, int32_t lag, int64_t* staleness_rows,
+                                                         double* stats_rows, int32_t* status_rows) {
+  const int64_t row = blockIdx.x;
+  int64_t* read_iter = read_iter_rows + row * W;
+  const int32_t* order = order_rows + row * W;
+  const int32_t* n_arrived = n_arrived_rows ? n_arrived_rows + row : nullptr;
+  int64_t* t_counter = t_counter_rows + row;
+  int64_t* staleness = staleness_rows + row * W;
+  double* stats = stats_rows + row * 6;
+  int32_t* status = status_rows + row;
   __shared__ int s_seen[kMaxWorkers];
   __shared__ long long s_val[kMaxWorkers];
   __shared__ long long s_sorted[kMaxWorkers];
@@ -485,11 +496,11 @@ cudaError_t launch_lr_schedule(float gamma0, float beta, int64_t t0, int32_t K, 
   return cudaLaunchKernelEx(&cfg, lr_schedule_kernel, gamma0, beta, t0, K, s, d_gamma);
 }
 
-cudaError_t launch_staleness(int64_t* d_read_iter, int32_t W, const int32_t* d_order, const int32_t* d_n_arrived,
-                             int32_t K, int64_t* d_t, int32_t lag, int64_t* d_staleness, double* d_stats,
-                             int32_t* d_status, cudaStream_t stream) {
+cudaError_t launch_staleness(int64_t* d_read_iter, int32_t W, int32_t rows, const int32_t* d_order,
+                             const int32_t* d_n_arrived, int32_t K, int64_t* d_t, int32_t lag, int64_t* d_staleness,
+                             double* d_stats, int32_t* d_status, cudaStream_t stream) {
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(1);
+  cfg.gridDim = dim3(static_cast<unsigned>(rows));
   cfg.blockDim = dim3(static_cast<unsigned>((W + 31) / 32 * 32));
   cfg.stream = stream;
   cudaLaunchAttribute attr[1];

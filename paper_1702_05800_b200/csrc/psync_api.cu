@@ -384,7 +384,20 @@ PSYNC_API int psync_staleness(int64_t* d_read_iter, int32_t W, const int32_t* d_
       d_status == nullptr)
     return PSYNC_EINVAL;
   if (W < 1 || W > PSYNC_MAX_WORKERS || K < 0 || K > W || lag < 0) return PSYNC_EINVAL;
-  return psync::launch_staleness(d_read_iter, W, d_order, d_n_arrived, K, d_t, lag, d_staleness, d_stats, d_status,
+  return psync::launch_staleness(d_read_iter, W, 1, d_order, d_n_arrived, K, d_t, lag, d_staleness, d_stats, d_status,
+                                 static_cast<cudaStream_t>(stream)) == cudaSuccess
+             ? PSYNC_OK
+             : PSYNC_ECUDA;
+}
+
+PSYNC_API int psync_staleness_sharded(int64_t* d_read_iter, int32_t W, int32_t M, const int32_t* d_order,
+                            const int32_t* d_n_arrived, int32_t K, int64_t* d_t, int32_t lag, int64_t* d_staleness,
+                            double* d_stats, int32_t* d_status, void* stream) {
+  if (d_read_iter == nullptr || d_order == nullptr || d_t == nullptr || d_staleness == nullptr || d_stats == nullptr ||
+      d_status == nullptr)
+    return PSYNC_EINVAL;
+  if (W < 1 || W > PSYNC_MAX_WORKERS || M < 1 || K < 0 || K > W || lag < 0) return PSYNC_EINVAL;
+  return psync::launch_staleness(d_read_iter, W, M, d_order, d_n_arrived, K, d_t, lag, d_staleness, d_stats, d_status,
                                  static_cast<cudaStream_t>(stream)) == cudaSuccess
              ? PSYNC_OK
              : PSYNC_ECUDA;

@@ -111,8 +111,8 @@ class AsyncServerStep:
     apply(d_arrival) enqueues, with no host synchronisation: the arrival order (per server with per_server=True,
     d_arrival [M][W]), optionally the global-norm clip factors (clip > 0: the norm is over the whole gradient of a
     worker, all of its slices, L313), optionally the learning rates of this batch's iterations (lr = (gamma0, beta, s):
-    gamma0 * beta^((t0 + i) s), L315), the one-pass application of the arrivals, and with track_staleness=True (one
-    order only) Table 1's bookkeeping.  Plumbing only, no arithmetic."""
+    gamma0 * beta^((t0 + i) s), L315), the one-pass application of the arrivals, and with track_staleness=True Table 1's
+    bookkeeping (per server with per_server=True).  Plumbing only, no arithmetic."""
 
     def __init__(self, shard_off, W: int, theta: torch.Tensor, ema: Optional[torch.Tensor],
                  state0: Optional[torch.Tensor], state1: Optional[torch.Tensor], opt: int, ema_mode: int = B.PSYNC_EMA_PRE,
@@ -125,8 +125,6 @@ class AsyncServerStep:
         self.opt, self.ema_mode = opt, ema_mode
         self.alpha, self.mu, self.rho, self.eps = alpha, mu, rho, eps
         self.per_server, self.clip, self.lr, self.lag = bool(per_server), float(clip), lr, int(lag)
-        if track_staleness and per_server:
-            raise ValueError("staleness bookkeeping follows one arrival order (per_server=False)")
         rows = self.M if per_server else 1
         self.d_order = torch.full((rows, W), -1, dtype=torch.int32, device=dev)
         self.d_n_arrived = torch.zeros(rows, dtype=torch.int32, device=dev)
@@ -136,12 +134,12 @@ class AsyncServerStep:
         self._d_clip_work = None
         self.t0 = 0                       # iterations scheduled so far (host counter: W per batch unless given)
         self.track_staleness = bool(track_staleness)
-        if track_staleness:
-            self.d_read_iter = torch.zeros(W, dtype=torch.int64, device=dev)
-            self.d_t = torch.zeros(1, dtype=torch.int64, device=dev)
-            self.d_staleness = torch.zeros(W, dtype=torch.int64, device=dev)
-            self.d_stale_stats = torch.zeros(6, dtype=torch.float64, device=dev)
-            self.d_stale_status = torch.zeros(1, dtype=torch.int32, device=dev)
+        if track_staleness:               # one row per server with per_server=True: every server counts its own updates
+            self.d_read_iter = torch.zeros((rows, W), dtype=torch.int64, device=dev)
+            self.d_t = torch.zeros(rows, dtype=torch.int64, device=dev)
+            self.d_staleness = torch.zeros((rows, W), dtype=torch.int64, device=dev)
+            self.d_stale_stats = torch.zeros((rows, 6), dtype=torch.float64, device=dev)
+            self.d_stale_status = torch.zeros(rows, dtype=torch.int32, device=dev)
         self._d_tiles = {}
         self.layout = B.PSYNC_GRADS_FLAT
         self.table: Optional[B.GradTable] = None
@@ -208,6 +206,6 @@ class AsyncServerStep:
             B.psync_lr_schedule(gamma0, beta, self.t0 if t0 is None else t0, self.W, s, self.d_gamma, stream)
         B.psync_async_apply(self._step, self.d_gamma, stream, d_gscale=self.d_gscale)
         if self.track_staleness:
-            B.psync_staleness(self.d_read_iter, self.d_order, self.d_t, self.d_staleness, self.d_stale_stats,
-                              self.d_stale_status, d_n_arrived=self.d_n_arrived, lag=self.lag, stream=stream)
+            B.psync_staleness_sharded(self.d_read_iter, self.d_order, self.d_t, self.d_staleness, self.d_stale_stats,
+                                      self.d_stale_status, d_n_arrived=self.d_n_arrived, lag=self.lag, stream=stream)
         self.t0 = (self.t0 if t0 is None else t0) + self.W

@@ -394,9 +394,9 @@ def test_async_server_step_flat_with_clipping_schedule_and_staleness_chained_bat
         st, stale, read, stats = oracle.staleness(read, order, t_srv, lag=2)
         t_srv += K
         assert st == oracle.OK and int(srv.d_stale_status.item()) == 0 and int(srv.d_t.item()) == t_srv
-        assert np.array_equal(srv.d_staleness.cpu().numpy()[:K], stale)
-        assert np.array_equal(srv.d_read_iter.cpu().numpy(), read)
-        assert np.array_equal(srv.d_stale_stats.cpu().numpy(), stats)
+        assert np.array_equal(srv.d_staleness.cpu().numpy()[0, :K], stale)
+        assert np.array_equal(srv.d_read_iter.cpu().numpy()[0], read)
+        assert np.array_equal(srv.d_stale_stats.cpu().numpy()[0], stats)
 
 
 def test_async_server_step_per_server_on_slices_chained_batches():
@@ -408,8 +408,6 @@ def test_async_server_step_per_server_on_slices_chained_batches():
     lr = (0.045, 0.94, 1.0 / 40.0)
     srv = psync.AsyncServerStep(off, cfg.W, theta, ema, s0, None, cfg.opt, cfg.ema_mode, alpha=cfg.alpha, mu=cfg.mu,
                                 per_server=True, lr=lr)
-    with pytest.raises(ValueError):
-        psync.AsyncServerStep(off, cfg.W, theta, ema, s0, None, cfg.opt, per_server=True, track_staleness=True)
     h = {"theta": to_np(theta), "ema": to_np(ema), "state0": to_np(s0)}
     M = off.size - 1
     for s in range(2):
@@ -575,3 +573,47 @@ def test_async_server_step_is_capturable_in_a_cuda_graph_and_replays_bit_identic
     for n in ("theta", "ema", "state0"):
         assert np.array_equal(to_np(getattr(cap, n)), to_np(getattr(eager, n))), n
     assert not np.array_equal(to_np(cap.theta), to_np(snap["theta"]))
+
+
+def test_staleness_per_server_chained_batches_match_the_oracle_row_by_row():
+    """psync_staleness_sharded: every server keeps its own counter and its own record of when each worker last read from
+    it; row j is exactly the single-order bookkeeping (the pinned oracle function) on server j's order.  Three chained
+    batches, different counts per server, a fixed lag, one server with a bad batch (a worker listed twice)."""
+    rng = np.random.default_rng(77)
+    M, W, lag = 5, 40, 3
+    d_read = torch.zeros((M, W), dtype=torch.int64, device=DEV)
+    d_t = torch.zeros(M, dtype=torch.int64, device=DEV)
+    d_order = torch.full((M, W), -1, dtype=torch.int32, device=DEV)
+    d_n = torch.zeros(M, dtype=torch.int32, device=DEV)
+    d_st = torch.full((M, W), -7, dtype=torch.int64, device=DEV)
+    d_stats = torch.full((M, 6), -7.0, dtype=torch.float64, device=DEV)
+    d_status = torch.full((M,), -9, dtype=torch.int32, device=DEV)
+    read = np.zeros((M, W), np.int64)
+    t = np.zeros(M, np.int64)
+    for batch in range(3):
+        a = rng.lognormal(0, 0.4, (M, W)).astype(np.float32)
+        a[rng.random((M, W)) < 0.15] = np.inf
+        psync.psync_order_by_arrival_sharded(torch.from_numpy(a).to(DEV), W, M, d_order, d_n)
+        if batch == 1:                                    # server 2's order row is corrupted: a worker appears twice
+            torch.cuda.synchronize()
+            row = d_order[2].clone()
+            row[1] = row[0]
+            d_order[2].copy_(row)
+        psync.psync_staleness_sharded(d_read, d_order, d_t, d_st, d_stats, d_status, d_n_arrived=d_n, lag=lag)
+        torch.cuda.synchronize()
+        got_order, got_n = d_order.cpu().numpy(), d_n.cpu().numpy()
+        for j in range(M):
+            order = got_order[j, :got_n[j]].copy()
+            rc, stale, nxt, stats = oracle.staleness(read[j].copy(), order, int(t[j]), lag=lag)
+            if batch == 1 and j == 2:
+                assert rc != oracle.OK and int(d_status[j].item()) == psync.PSYNC_EINVAL
+                assert np.array_equal(d_read[j].cpu().numpy(), read[j]) and int(d_t[j].item()) == t[j]
+                continue
+            assert rc == oracle.OK and int(d_status[j].item()) == 0
+            read[j], t[j] = nxt, t[j] + order.size
+            assert np.array_equal(d_st[j].cpu().numpy()[:order.size], stale)
+            assert np.array_equal(d_read[j].cpu().numpy(), read[j]) and int(d_t[j].item()) == t[j]
+            assert np.array_equal(d_stats[j].cpu().numpy(), stats)
+    L = psync.binding.lib()
+    assert L.psync_staleness_sharded(None, 4, 2, None, None, 0, None, 0, None, None, None, None) == psync.PSYNC_EINVAL
+    assert L.psync_staleness_sharded(8, 4, 0, 8, None, 0, 8, 0, 8, 8, 8, None) == psync.PSYNC_EINVAL
