@@ -485,7 +485,9 @@ def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist
     return {"total_ms": total_ms, "ms_per_step": total_ms / K, "fused_ms": fused_ms, "select_ms": select_ms,
             "fused_list": fused_list, "n_eff": n_eff, "bytes_per_step": bytes_per_step, "units": n_eff * cfg.P * K,
             "clocks": clocks, "geo": geo, "launches_per_step": launches_per_step,
-            "kernel": ("async_sharded_kernel" if use_tiles else "async_apply_kernel") if is_async else
+            "kernel": ("async_sharded_kernel" if use_tiles else
+                       {1: "async_apply_kernel", 2: "async_apply_pair_kernel"}.get(variant, "async_apply_ring_kernel"))
+                      if is_async else
                       ("sharded_aggregate_update_ema" if use_tiles else "fused_aggregate_update_ema")}
 
 
