@@ -533,10 +533,22 @@ def psync_step_host(step: psync_step, h_arrival: np.ndarray, h_grads: Sequence[t
     W = step.W
     if len(h_grads) != W or h_arrival.size != W or h_arrival.dtype != np.float32:
         raise ValueError("need W host gradient buffers and W fp32 arrival times")
-    for g in h_grads:
-        if g.is_cuda or not g.is_contiguous() or g.numel() != step.P:
-            raise ValueError("h_grads must be contiguous CPU tensors of P elements")
-    ptrs = (ctypes.c_void_p * W)(*[g.data_ptr() for g in h_grads])
+    if step.grad_layout == PSYNC_GRADS_SLICES:      # h_grads[k][j]: worker k's slice for server j (None = missing)
+        M = step.M
+        flat_ptrs = []
+        for row in h_grads:
+            if len(row) != M:
+                raise ValueError("every worker needs M host slices")
+            for g in row:
+                if g is not None and (g.is_cuda or not g.is_contiguous()):
+                    raise ValueError("host slices must be contiguous CPU tensors")
+                flat_ptrs.append(None if g is None else g.data_ptr())
+        ptrs = (ctypes.c_void_p * (W * M))(*flat_ptrs)
+    else:
+        for g in h_grads:
+            if g.is_cuda or not g.is_contiguous() or g.numel() != step.P:
+                raise ValueError("h_grads must be contiguous CPU tensors of P elements")
+        ptrs = (ctypes.c_void_p * W)(*[g.data_ptr() for g in h_grads])
     t_nth = ctypes.c_float(float("nan"))
     if h_theta_out is not None and (h_theta_out.is_cuda or h_theta_out.dtype != torch.float32
                                     or h_theta_out.numel() != step.P):

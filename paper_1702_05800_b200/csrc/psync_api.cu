@@ -500,15 +500,26 @@ PSYNC_API int psync_step_host(const psync_step* st, const float* h_arrival, cons
 PSYNC_API int psync_step_host_ctx(void* ctx, const psync_step* st, const float* h_arrival, const int32_t* h_step_tag,
                         int32_t t, const void* const* h_grads, float* h_theta_out, int32_t* h_kept, float* h_t_nth,
                         void* d_work, size_t work_bytes, int64_t chunk_elems, void* stream) {
-  const int chk = check_step(st, false);
+  if (st == nullptr) return PSYNC_EINVAL;
+  psync_step flat = *st;  // the device side of this path is always the flat stream (see SLICES below)
+  flat.grad_layout = PSYNC_GRADS_FLAT;
+  flat.d_shard_off = nullptr;
+  flat.d_tile_start = nullptr;
+  const int chk = check_step(&flat, false);
   if (chk != PSYNC_OK) return chk;
+  if (st->grad_layout != PSYNC_GRADS_FLAT && st->grad_layout != PSYNC_GRADS_SLICES) return PSYNC_EINVAL;
   if (h_arrival == nullptr || h_grads == nullptr || d_work == nullptr) return PSYNC_EINVAL;
-  if (st->per_shard != 0 || st->d_n_kept != nullptr || st->grad_layout != PSYNC_GRADS_FLAT) return PSYNC_EUNSUPPORTED;
+  if (st->per_shard != 0 || st->d_n_kept != nullptr) return PSYNC_EUNSUPPORTED;
+  // SLICES: h_grads is [W*M] HOST pointers, entry k*M + j -> the len_j elements of G_k[j] as server j received them.  The
+  // kept workers' slices are gathered chunk by chunk into the same flat staging buffers (one copy per (worker, server)
+  // range that intersects the chunk), so the device side is the flat pipeline unchanged.
+  const bool h_slices = st->grad_layout == PSYNC_GRADS_SLICES;
   HostLayout L;
   if (!host_layout(st->N, st->W, st->grad_dtype, chunk_elems, &L)) return PSYNC_EINVAL;
   if (work_bytes < L.total || (reinterpret_cast<uintptr_t>(d_work) & 255u) != 0) return PSYNC_EINVAL;
-  for (int32_t k = 0; k < st->W; ++k)
-    if (h_grads[k] == nullptr) return PSYNC_EINVAL;
+  if (!h_slices)
+    for (int32_t k = 0; k < st->W; ++k)
+      if (h_grads[k] == nullptr) return PSYNC_EINVAL;
 
   const int32_t N = st->N, W = st->W;
   const int64_t esz = st->grad_dtype == PSYNC_BF16 ? 2 : 4;
@@ -553,6 +564,13 @@ PSYNC_API int psync_step_host_ctx(void* ctx, const psync_step* st, const float* 
     PSYNC_CU(psync::launch_fill_stage_table(reinterpret_cast<const void**>(work + L.off_ptrs[i]), d_ident,
                                             work + L.off_stage[i], L.stride_bytes, N, s));
   PSYNC_CU(cudaStreamSynchronize(s));
+  if (h_slices)  // every slice of a KEPT worker must be there (dropped workers' slices are never looked at)
+    for (int32_t n = 0; n < N; ++n)
+      for (int32_t j = 0; j < st->M; ++j)
+        if (st->h_shard_off[j + 1] > st->h_shard_off[j] && h_grads[static_cast<int64_t>(kept[n]) * st->M + j] == nullptr) {
+          result = PSYNC_EINVAL;  // nothing has been updated yet
+          goto cleanup;
+        }
   if (h_kept != nullptr) std::memcpy(h_kept, kept.data(), sizeof(int32_t) * N);
   if (h_t_nth != nullptr) *h_t_nth = t_nth;
 
@@ -567,18 +585,35 @@ PSYNC_API int psync_step_host_ctx(void* ctx, const psync_step* st, const float* 
     cudaEvent_t* consumed = hc->consumed;
     // both streams are idle here: `s` was synchronised above and every call ends with both streams drained
     int64_t c = 0;
+    int32_t j_first = 0;
     for (int64_t first = 0; first < st->P; first += L.chunk, ++c) {
       const int buf = static_cast<int>(c & 1);
       const int64_t count = (st->P - first < L.chunk) ? (st->P - first) : L.chunk;
+      while (h_slices && j_first + 1 < st->M && st->h_shard_off[j_first + 1] <= first) ++j_first;  // first server in chunk
       if (c >= 2) PSYNC_CU(cudaStreamWaitEvent(copy_stream, consumed[buf], 0));
       for (int32_t n = 0; n < N; ++n) {
-        const char* src = static_cast<const char*>(h_grads[kept[n]]) + first * esz;
-        PSYNC_CU(cudaMemcpyAsync(work + L.off_stage[buf] + static_cast<int64_t>(n) * L.stride_bytes, src,
-                                 static_cast<size_t>(count * esz), cudaMemcpyHostToDevice, copy_stream));
+        char* dst = work + L.off_stage[buf] + static_cast<int64_t>(n) * L.stride_bytes;
+        if (!h_slices) {
+          const char* src = static_cast<const char*>(h_grads[kept[n]]) + first * esz;
+          PSYNC_CU(cudaMemcpyAsync(dst, src, static_cast<size_t>(count * esz), cudaMemcpyHostToDevice, copy_stream));
+        } else {
+          for (int32_t j = j_first; j < st->M && st->h_shard_off[j] < first + count; ++j) {  // servers in this chunk
+            const int64_t lo = st->h_shard_off[j] > first ? st->h_shard_off[j] : first;
+            const int64_t hi = st->h_shard_off[j + 1] < first + count ? st->h_shard_off[j + 1] : first + count;
+            if (hi <= lo) continue;
+            const char* slice = static_cast<const char*>(h_grads[static_cast<int64_t>(kept[n]) * st->M + j]);
+            if (slice == nullptr) {  // a kept worker's slice is missing
+              result = PSYNC_EINVAL;
+              goto cleanup;
+            }
+            PSYNC_CU(cudaMemcpyAsync(dst + (lo - first) * esz, slice + (lo - st->h_shard_off[j]) * esz,
+                                     static_cast<size_t>((hi - lo) * esz), cudaMemcpyHostToDevice, copy_stream));
+          }
+        }
       }
       PSYNC_CU(cudaEventRecord(copied[buf], copy_stream));
       PSYNC_CU(cudaStreamWaitEvent(s, copied[buf], 0));
-      const FusedParams p = make_params(st, first, count, reinterpret_cast<const void* const*>(work + L.off_ptrs[buf]),
+      const FusedParams p = make_params(&flat, first, count, reinterpret_cast<const void* const*>(work + L.off_ptrs[buf]),
                                         d_ident, nullptr);
       PSYNC_CU(psync::launch_fused(p, st->grad_dtype, st->opt, st->ema_mode, st->variant, st->grid_ctas, s));
       PSYNC_CU(cudaEventRecord(consumed[buf], s));

@@ -532,3 +532,39 @@ def test_random_shard_layouts_alignments_rows_and_counts(seed):
     pair.oracle(slices, kept, per_shard=per_shard, n_kept=n_kept if mode == 2 else None, status=status)
     pair.compare_and_sync(f"fuzz {seed}: M={M} P={P} W={W} N={N} dtype={dtype} opt={opt} ema={ema_mode} mode={mode}",
                           RTOL_BF16 if dtype == synth.BF16 else RTOL_STEP)
+
+
+# ------------------------------------------------------------------ host-buffer step from per-(worker, server) slices
+@pytest.mark.parametrize("dtype,chunk", [(synth.F32, 4096), (synth.BF16, 0)])
+def test_step_host_from_host_slices_matches_the_oracle(dtype, chunk):
+    """psync_step_host with grad_layout = SLICES: h_grads is W x M host slices (what each server received); the kept
+    workers' slices are gathered chunk by chunk (chunks straddle servers, an empty and a one-element server, slices at odd
+    element offsets in host memory); the dropped workers' slices are not even there."""
+    cfg = replace(BASE, grad_dtype=dtype, opt=synth.RMSPROP_MOM, name=f"host_slices_d{dtype}")
+    pair = SlicesPair(cfg, shard_off=RAGGED)
+    nbytes = psync.psync_step_host_workspace_bytes(cfg.N, cfg.W, cfg.grad_dtype, chunk)
+    d_work = torch.empty(nbytes, dtype=torch.uint8, device=DEV)
+    h_theta = torch.empty(cfg.P, dtype=torch.float32).pin_memory()
+    h_kept = np.full(cfg.N, -1, dtype=np.int32)
+    for s in range(2):
+        flat = [synth.gradient(cfg, s, k, "cpu") for k in range(cfg.W)]
+        arrival = synth.arrival_times(cfg, s)
+        st_o, kept, t_nth_o = oracle.select_first_n(arrival, cfg.N, cfg.b)
+        h_sl = cut_slices(flat, pair.off, lambda k, j: (k + 2 * j) % 5)
+        dropped = sorted(set(range(cfg.W)) - set(kept.tolist()))
+        for k in dropped:
+            h_sl[k] = [None] * pair.M
+        step, keep = psync.make_step(pair.off, cfg.N, cfg.W, cfg.grad_dtype, pair.theta, pair.ema, pair.state0, pair.state1,
+                                     opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu,
+                                     rho=cfg.rho, eps=cfg.eps, grad_layout=psync.PSYNC_GRADS_SLICES)
+        st, t_nth = psync.psync_step_host(step, arrival, h_sl, d_work, h_theta_out=h_theta, h_kept=h_kept,
+                                          chunk_elems=chunk)
+        assert st == st_o == 0 and np.array_equal(h_kept, kept) and t_nth == t_nth_o
+        pair.oracle(h_sl, kept)
+        pair.compare_and_sync(f"host slices step {s}", RTOL_BF16 if dtype == synth.BF16 else RTOL_STEP)
+        assert np.array_equal(h_theta.numpy(), to_np(pair.theta))
+    # a KEPT worker's slice missing: PSYNC_EINVAL before anything is updated
+    before = to_np(pair.theta)
+    h_sl[int(kept[0])][3] = None
+    st, _ = psync.psync_step_host(step, arrival, h_sl, d_work, chunk_elems=chunk, check=False)
+    assert st == psync.PSYNC_EINVAL and np.array_equal(to_np(pair.theta), before)
