@@ -657,7 +657,7 @@ def run_psync(args, cfg, rank, world, dist):
     theta, ema, s0, s1, off = wl.theta, wl.ema, wl.s0, wl.s1, wl.off
     del wl.tables, wl.sets
     torch.cuda.empty_cache()
-    if not args.no_e2e and mode == "first_n" and args.layout == "flat":
+    if not args.no_e2e and mode == "first_n":
         out["e2e"] = run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
@@ -778,9 +778,13 @@ def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist):
     chunk = args.e2e_chunk
     nbytes = psync.psync_step_host_workspace_bytes(cfg.N, cfg.W, cfg.grad_dtype, chunk)
     d_work = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    slices = getattr(args, "layout", "flat") == "slices"
+    if slices:   # what each server received, in host memory: W x M slices (here views of the pinned buffers)
+        h_grads = [[h[int(off[j]):int(off[j + 1])] for j in range(len(off) - 1)] for h in h_grads]
     step, keep = psync.make_step(off, cfg.N, cfg.W, cfg.grad_dtype, theta, ema, s0, s1, opt=cfg.opt,
                                  ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho,
-                                 eps=cfg.eps, grid_ctas=args.grid_ctas, variant=args.variant)
+                                 eps=cfg.eps, grid_ctas=args.grid_ctas, variant=0 if slices else args.variant,
+                                 grad_layout=psync.PSYNC_GRADS_SLICES if slices else psync.PSYNC_GRADS_FLAT)
     arrivals = [synth.arrival_times(cfg, 2000 + s) for s in range(K + 1)]
     ctx = psync.HostCtx()               # the copy stream and events, created once for the loop
     psync.psync_step_host(step, arrivals[K], h_grads, d_work, h_theta_out=h_theta, h_kept=h_kept, chunk_elems=chunk,
@@ -800,7 +804,8 @@ def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist):
     return {"value": units / (max_ms * 1e-3), "unit": UNIT, "steps": K, "ms_per_step": max_ms / K,
             "h2d_bytes_per_step": cfg.N * cfg.P * cfg.grad_bytes + 4 * cfg.W,
             "d2h_bytes_per_step": 4 * cfg.P + 4 * cfg.N + 8,
-            "api": "psync_step_host (C ABI, pinned host gradient buffers; only the N kept buffers cross PCIe)",
+            "api": "psync_step_host (C ABI, pinned host gradient buffers" + (" as W x M per-(worker, server) slices" if slices else "")
+                   + "; only the N kept buffers cross PCIe)",
             "gpu_launches_per_step": 3 + n_chunks,
             "timing": "host wall clock around synchronous calls (the call returns when theta(t+1) is on the host)"}
 
