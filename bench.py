@@ -707,8 +707,10 @@ def run_sweep(args, rank, world, dist):
             continue
         set_bytes = cfg.W * cfg.P * cfg.grad_bytes
         wl = Workload(psync, cfg, dev, 3 if set_bytes < 20e9 else 2, layout=args.layout)
-        m = measure(psync, args, wl, "first_n", K, Wm, stream, dist, variant=args.variant, probe_every=1)
-        e = short_entry(cfg, "first_n", args.layout, m, peak)
+        # --mode async sweeps Alg. 2's one-pass kernel instead: all N+b gradients applied one at a time (K = N+b)
+        sweep_mode = args.mode if args.mode in ("first_n", "async") else "first_n"
+        m = measure(psync, args, wl, sweep_mode, K, Wm, stream, dist, variant=args.variant, probe_every=1)
+        e = short_entry(cfg, sweep_mode, args.layout, m, peak)
         e["grad_sets"] = wl.n_sets
         e["gradient_set_bytes"] = set_bytes
         e["l2"] = ("L2-resident: the whole footprint fits the 126 MB L2" if cfg.footprint_bytes <= L2_BYTES else
@@ -729,13 +731,16 @@ def run_sweep(args, rank, world, dist):
                         "algorithmic_bytes_per_launch": big["algorithmic_bytes_per_launch"]},
            "clocks": big["clocks"], "gpu_launches": 2 * K * len(points), "points": points}
     if args.sweep_md and rank == 0:
-        write_sweep_md(args.sweep_md, points, peak, peak_src)
+        write_sweep_md(args.sweep_md, points, peak, peak_src, mode=points[0]["mode"], layout=args.layout)
     return out
 
 
-def write_sweep_md(path, points, peak, peak_src):
-    lines = ["# cfg5 bandwidth sweep: GB/s of algorithmic bytes (fused kernel, CUDA events) vs P and N+b", "",
-             "Command: `python bench.py --config cfg5 --sweep-md <this file>`; 3 warm-up + 5 timed steps per point, "
+def write_sweep_md(path, points, peak, peak_src, mode="first_n", layout="flat"):
+    what = ("" if mode == "first_n" else ", Alg. 2 (async: all N+b gradients applied one at a time in one pass)") + \
+           ("" if layout == "flat" else ", slices layout")
+    flags = ("" if mode == "first_n" else " --mode async") + ("" if layout == "flat" else " --layout slices")
+    lines = [f"# cfg5 bandwidth sweep{what}: GB/s of algorithmic bytes (fused kernel, CUDA events) vs P and N+b", "",
+             f"Command: `python bench.py --config cfg5{flags} --sweep-md <this file>`; 3 warm-up + 5 timed steps per point, "
              "gradient sets rotated.  Flags: `L2` = whole footprint fits the 126 MB L2, `~L2` = one gradient set is "
              f"smaller than 4 x L2 (partly L2-served); unflagged points stream from HBM.  Peak: {peak} GB/s, {peak_src}.",
              ""]
