@@ -2,7 +2,7 @@
 """bench.py -- whole-job throughput of the parameter-server step (Alg. 4) on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg1..cfg5] [--impl psync|reference]
-                    [--mode first_n|per_server|timeout|async] [--layout flat|slices] [--variant 1..6] [--servers M]
+                    [--mode first_n|per_server|timeout|async] [--layout flat|slices] [--variant 1..7] [--servers M]
 
 The default run is the headline (cfg3, first_n, flat buffers); its JSON line also carries `also`: short
 measurements of cfg2, cfg4, every other mode, the slices layout, many-server cuts and launch variants 5 / 6.
@@ -527,11 +527,12 @@ def run_also(psync, args, wl3, stream, peak):
         wlm.reset_state()
         m = measure(psync, args, wlm, "per_server", K, Wm, stream, probe_every=2)
         out.append(short_entry(wlm.cfg, "per_server", "flat", m, peak, "flat buffers through the (server, tile) work list"))
-    for v in (5, 6):                     # the two rejected designs, re-measured every run (DESIGN.md s.5)
+    for v in (5, 6, 7):                  # the rejected designs, re-measured every run (DESIGN.md s.5)
         wl3.reset_state()
         m = measure(psync, args, wl3, "first_n", K, Wm, stream, variant=v, probe_every=2)
         out.append(short_entry(cfg3, "first_n", "flat", m, peak,
-                               "variant 5: cp.async.bulk + mbarrier ring" if v == 5 else "variant 6: 256-bit loads"))
+                               {5: "variant 5: cp.async.bulk + mbarrier ring", 6: "variant 6: 256-bit loads",
+                                7: "variant 7: per-thread cp.async ring (Alg. 2's staging)"}[v]))
         out[-1]["variant"] = v
     for v in (1, 2):                     # Alg. 2's other launch shapes, re-measured every run (profiles/r2_async.md)
         wl3.reset_state()

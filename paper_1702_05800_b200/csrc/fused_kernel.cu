@@ -475,6 +475,96 @@ __global__ void __launch_bounds__(256 + 32, MINB) fused_aggregate_update_ema_bul
   if (tail0 < p.P && blockIdx.x == 0) scalar_range<BF16, OPT, EMA>(p, s_ptr, tail0, p.P, threadIdx.x, CONSUMERS);
 }
 
+// ---- variant 7: per-thread cp.async ring (the staging Alg. 2's kernels use, async_kernel.cu) --------------------
+// Every thread copies the 16-byte units of its own column of the kept buffers into its own slots of a D-deep ring in
+// shared memory (cp.async.cg, SASS LDGSTS.E.BYPASS.128; one commit group per buffer) and adds them in ascending worker
+// order as they land (cp.async.wait_group): no barrier, no mbarrier, no producer warp, and no registers for loads in
+// flight -- so theta / state / ema are requested right after the ring is filled, not after the gradient stream, for
+// EVERY instance (one dependent round trip less per CTA).  Same adds in the same order: the same bits as variant 1.
+template <int D, int MINB, bool BF16, int OPT, int EMA>
+__global__ void __launch_bounds__(256, MINB) fused_aggregate_update_ema_tring(const FusedParams p) {
+  constexpr int THREADS = 256;
+  constexpr int E = BF16 ? 8 : 4;
+  constexpr int Q = E / 4;
+  __shared__ const char* s_ptr[kMaxWorkers];
+  __shared__ __align__(16) uint4 s_ring[D][THREADS];
+
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+
+  const int64_t n_units = p.P / E;
+  const int64_t n_tiles = (n_units + THREADS - 1) / THREADS;
+  const int64_t tail0 = n_units * E;
+  if (p.status != nullptr && *p.status != 0) return;
+  const unsigned misalign = stage_row<THREADS>(p, s_ptr, 0, p.N);
+  const bool vec_ok = (__syncthreads_or(static_cast<int>(misalign)) == 0) && (p.base_aligned != 0);
+  if (!vec_ok) {
+    scalar_range<BF16, OPT, EMA>(p, s_ptr, 0, p.P, static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x,
+                                 static_cast<int64_t>(gridDim.x) * THREADS);
+    return;
+  }
+  if (blockIdx.x < n_tiles) {
+    const int N = p.N;
+    const int64_t u = static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x;
+    const bool live = u < n_units;
+    const int64_t unit = live ? u : (n_units - 1);  // dead slots re-read a valid unit and store nothing
+    const uint32_t slot0 = static_cast<uint32_t>(__cvta_generic_to_shared(&s_ring[0][threadIdx.x]));
+#pragma unroll
+    for (int i = 0; i < D; ++i) {
+      if (i < N)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(slot0 + i * THREADS * 16), "l"(s_ptr[i] + unit * 16)
+                     : "memory");
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+    float4 th[Q], em[Q], a0[Q], a1[Q];
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const int64_t e = unit * E + 4 * q;
+      th[q] = ld_state16(p.theta + e);
+      if (EMA != EMA_OFF) em[q] = ld_state16(p.ema + e);
+      if (OPT != OPT_SGD) a0[q] = ld_state16(p.s0 + e);
+      if (OPT == OPT_RMSPROP_MOM) a1[q] = ld_state16(p.s1 + e);
+    }
+    float acc[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) acc[e] = 0.f;
+    auto one = [&](int i, int slot) {
+      asm volatile("cp.async.wait_group %0;" ::"n"(D - 1) : "memory");  // buffer i has landed (groups retire in order)
+      const uint4 r = s_ring[slot][threadIdx.x];
+      accumulate_unit<BF16>(acc, r);  // strictly ascending worker order
+      if (i + D < N)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(slot0 + slot * THREADS * 16),
+                     "l"(s_ptr[i + D] + unit * 16)
+                     : "memory");
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    int i0 = 0;
+    for (; i0 + D <= N; i0 += D) {
+#pragma unroll
+      for (int v = 0; v < D; ++v) one(i0 + v, v);
+    }
+    for (int i = i0; i < N; ++i) one(i, i - i0);
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      float* t4 = reinterpret_cast<float*>(&th[q]);
+      float* e4 = reinterpret_cast<float*>(&em[q]);
+      float* x4 = reinterpret_cast<float*>(&a0[q]);
+      float* y4 = reinterpret_cast<float*>(&a1[q]);
+#pragma unroll
+      for (int l = 0; l < 4; ++l) update_element<OPT, EMA>(acc[4 * q + l], p.inv_N, t4[l], e4[l], x4[l], y4[l], p);
+      if (live) {
+        const int64_t e = unit * E + 4 * q;
+        st_state16(p.theta + e, th[q]);
+        if (EMA != EMA_OFF) st_state16(p.ema + e, em[q]);
+        if (OPT != OPT_SGD) st_state16(p.s0 + e, a0[q]);
+        if (OPT == OPT_RMSPROP_MOM) st_state16(p.s1 + e, a1[q]);
+      }
+    }
+  }
+  if (tail0 < p.P && blockIdx.x == 0) scalar_range<BF16, OPT, EMA>(p, s_ptr, tail0, p.P, threadIdx.x, THREADS);
+}
+
 // ---- K3 ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) ema_kernel(float* __restrict__ ema, const float* __restrict__ theta, int64_t P,
                                                   float alpha, float one_minus_alpha, int aligned) {
@@ -494,7 +584,7 @@ __global__ void __launch_bounds__(256) ema_kernel(float* __restrict__ ema, const
 }
 
 // ---- variants and dispatch ---------------------------------------------------------------------
-enum VariantKind { kPlain128 = 0, kBulkRing = 1, kPlain256 = 2 };
+enum VariantKind { kPlain128 = 0, kBulkRing = 1, kPlain256 = 2, kThreadRing = 3 };
 struct Variant {
   int threads, upt, unroll, minb, kind;
 };
@@ -506,6 +596,7 @@ constexpr Variant kVariants[] = {
     {512, 1, 8, 2, kPlain128},    // 4
     {256, 1, 12, 3, kBulkRing},   // 5  cp.async.bulk -> 12-stage shared-memory ring (unroll = stages), 1 producer warp
     {256, 1, 8, 2, kPlain256},    // 6  256-bit loads with L2::evict_first, 8 in flight per thread
+    {256, 1, 8, 4, kThreadRing},  // 7  per-thread cp.async ring in shared memory (unroll = depth), state requested up front
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 constexpr int kRingStages = kVariants[4].unroll;
@@ -524,6 +615,8 @@ template <int V, bool BF16, int OPT, int EMA, bool ROWS = false>
 constexpr KernelFn kernel_for() {
   if constexpr (kVariants[V].kind == kBulkRing)
     return fused_aggregate_update_ema_bulk<kVariants[V].unroll, kVariants[V].minb, BF16, OPT, EMA>;
+  else if constexpr (kVariants[V].kind == kThreadRing)
+    return fused_aggregate_update_ema_tring<kVariants[V].unroll, minb_for(V, BF16, OPT), BF16, OPT, EMA>;
   else if constexpr (kVariants[V].kind == kPlain256)
     return fused_aggregate_update_ema_v256<kVariants[V].threads, kVariants[V].unroll, (BF16 ? 1 : kVariants[V].minb),
                                            BF16, OPT, EMA>;
@@ -580,7 +673,8 @@ KernelFn pick_kernel(int v, int dtype, int opt, int ema) {
     case 2: return pick_dtype<2>(dtype, opt, ema);
     case 3: return pick_dtype<3>(dtype, opt, ema);
     case 4: return pick_dtype<4>(dtype, opt, ema);
-    default: return pick_dtype<5>(dtype, opt, ema);
+    case 5: return pick_dtype<5>(dtype, opt, ema);
+    default: return pick_dtype<6>(dtype, opt, ema);
   }
 }
 
@@ -609,7 +703,8 @@ cudaError_t fused_geometry(int dtype, int opt, int ema, int variant, int grid_ct
   const int E = (dtype == 1 ? 8 : 4) * (vr.kind == kPlain256 ? 2 : 1);  // parameters per 16- or 32-byte unit
   out->block = vr.threads + (vr.kind == kBulkRing ? 32 : 0);           // + the producer warp
   out->tile_elems = vr.threads * vr.upt * E;
-  out->smem_bytes = vr.kind == kBulkRing ? kRingSmemBytes : static_cast<int>(sizeof(const char*)) * kMaxWorkers;
+  out->smem_bytes = vr.kind == kBulkRing ? kRingSmemBytes
+                    : static_cast<int>(sizeof(const char*)) * kMaxWorkers + (vr.kind == kThreadRing ? vr.unroll * 256 * 16 : 0);
   // One tile per CTA, always: the hardware CTA scheduler balances the tiles dynamically over the SMs, which
   // measured 2-3 % faster on B200 than a persistent grid with static striding (DESIGN.md s.5), and a kernel
   // without a tile loop stays inside 64 registers without spilling.  grid_ctas is accepted and ignored.
