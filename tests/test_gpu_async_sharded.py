@@ -617,3 +617,23 @@ def test_staleness_per_server_chained_batches_match_the_oracle_row_by_row():
     L = psync.binding.lib()
     assert L.psync_staleness_sharded(None, 4, 2, None, None, 0, None, 0, None, None, None, None) == psync.PSYNC_EINVAL
     assert L.psync_staleness_sharded(8, 4, 0, 8, None, 0, 8, 0, 8, 8, 8, None) == psync.PSYNC_EINVAL
+
+
+def test_fixed_count_without_a_count_array_applies_exactly_N_per_server():
+    """d_n_kept = NULL: every server applies the first step->N entries of its order row (here N = 9 of 13 arrivals)."""
+    cfg = replace(BASE, opt=synth.MOMENTUM, name="arows_fixedN")
+    pair = RowsPair(cfg, shard_off=RAGGED)
+    a = synth.arrival_times_per_server(cfg, 0, server_sigma=0.3)
+    flat = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    sl = cut_slices(flat, pair.off)
+    psync.psync_order_by_arrival_sharded(torch.from_numpy(a).to(DEV), cfg.W, pair.M, pair.d_order, pair.d_n)
+    st, keep = pair.make_step(psync.make_slice_table(sl), d_n=False, N=9)
+    psync.psync_async_apply(st)
+    torch.cuda.synchronize()
+    order = np.stack([oracle.order_by_arrival(a[j]) for j in range(pair.M)])
+    h = pair.host
+    rc = oracle.async_apply_rows(pair.off, np_slices(sl), order, h["theta"], h["ema"], h["state0"], h["state1"], slices=True,
+                                 per_shard=True, n_arrived=np.full(pair.M, 9, np.int32), opt=cfg.opt, ema_mode=cfg.ema_mode,
+                                 gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
+    assert rc == oracle.OK
+    pair.compare_and_sync("fixed N per server", 9)
