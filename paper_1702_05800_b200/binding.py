@@ -26,7 +26,7 @@ PSYNC_MAX_WORKERS = 1024
 PSYNC_TILE_UNITS = 256
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
-           "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_order_by_arrival_sharded", "psync_clip_slices_workspace_bytes", "psync_clip_scales_slices", "psync_async_apply", "psync_staleness", "psync_staleness_sharded", "psync_step_device", "psync_clip_workspace_bytes",
+           "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_order_by_arrival_sharded", "psync_clip_slices_workspace_bytes", "psync_clip_scales_slices", "psync_async_apply", "psync_async_step_device", "psync_staleness", "psync_staleness_sharded", "psync_step_device", "psync_clip_workspace_bytes",
            "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_host_ctx_create", "psync_host_ctx_destroy",
            "psync_step_host_ctx", "psync_launch_geometry", "psync_probe_read",
@@ -90,6 +90,8 @@ def lib() -> ctypes.CDLL:
         L.psync_staleness_sharded.argtypes = [vp, i32, i32, vp, vp, i32, vp, i32, vp, vp, vp, vp]
         L.psync_staleness_sharded.restype = ctypes.c_int
         L.psync_async_apply.argtypes = [ctypes.POINTER(psync_step), vp, vp, vp]
+        L.psync_async_step_device.argtypes = [ctypes.POINTER(psync_step), vp, vp, vp, vp]
+        L.psync_async_step_device.restype = ctypes.c_int
         L.psync_clip_workspace_bytes.argtypes = [i32, i64, i32]
         L.psync_clip_workspace_bytes.restype = ctypes.c_size_t
         L.psync_clip_scales.argtypes = [vp, i32, i64, i32, f32, vp, vp, ctypes.c_size_t, vp]
@@ -476,6 +478,22 @@ def psync_async_apply(step: psync_step, d_gamma: Optional[torch.Tensor] = None, 
                                  _dptr(d_gscale, torch.float32, "d_gscale"), _stream(stream))
     if check and st != PSYNC_OK:
         raise PsyncError(st, "psync_async_apply")
+    return st
+
+
+def psync_async_step_device(step: psync_step, d_arrival: torch.Tensor, d_gamma: Optional[torch.Tensor] = None, stream=None,
+                            check: bool = True, d_gscale: Optional[torch.Tensor] = None) -> int:
+    """Arrival order + K iterations of Alg. 2 in one C call (include/psync.h: psync_async_step_device)."""
+    rows = step.M if step.per_shard else 1
+    if d_arrival.numel() < rows * step.W:
+        raise ValueError("d_arrival needs [rows][W] elements")
+    if d_gscale is not None and d_gscale.numel() < step.W:
+        raise ValueError("d_gscale needs W elements (indexed by worker)")
+    st = lib().psync_async_step_device(ctypes.byref(step), _dptr(d_arrival, torch.float32, "d_arrival"),
+                                       _dptr(d_gamma, torch.float32, "d_gamma"),
+                                       _dptr(d_gscale, torch.float32, "d_gscale"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_async_step_device")
     return st
 
 

@@ -296,6 +296,22 @@ PSYNC_API int psync_async_apply(const psync_step* step, const float* d_gamma, co
   return err == cudaSuccess ? PSYNC_OK : PSYNC_ECUDA;
 }
 
+PSYNC_API int psync_async_step_device(const psync_step* step, const float* d_arrival, const float* d_gamma,
+                            const float* d_gscale, void* stream) {
+  if (step == nullptr || d_arrival == nullptr) return PSYNC_EINVAL;
+  if (step->d_kept == nullptr || step->d_n_kept == nullptr) return PSYNC_EINVAL;  // the order kernel's outputs
+  if (step->W < 1 || step->W > PSYNC_MAX_WORKERS || step->M < 1) return PSYNC_EINVAL;
+  if (step->kept_stride != 0 && step->kept_stride != step->W) return PSYNC_EINVAL;  // the order kernel writes rows of W
+  psync_step s = *step;
+  s.kept_stride = s.W;
+  s.N = s.W;  // the count comes from the device (d_n_kept); N only has to satisfy 1 <= N <= W
+  const int32_t rows = s.per_shard ? s.M : 1;
+  if (psync::launch_order_by_arrival(d_arrival, s.W, rows, const_cast<int32_t*>(s.d_kept),
+                                     const_cast<int32_t*>(s.d_n_kept), static_cast<cudaStream_t>(stream)) != cudaSuccess)
+    return PSYNC_ECUDA;
+  return psync_async_apply(&s, d_gamma, d_gscale, stream);
+}
+
 PSYNC_API size_t psync_clip_workspace_bytes(int32_t W, int64_t P, int32_t grad_dtype) {
   if (W < 1 || W > PSYNC_MAX_WORKERS || P < 0 || (grad_dtype != PSYNC_F32 && grad_dtype != PSYNC_BF16)) return 0;
   return psync::clip_workspace_bytes(W, P, grad_dtype);

@@ -185,11 +185,7 @@ class AsyncServerStep:
             self._build(gamma_t)
         if stream is not None and hasattr(stream, "cuda_stream"):
             self.table.d_ptrs.record_stream(stream)
-        if self.per_server:
-            B.psync_order_by_arrival_sharded(d_arrival, self.W, self.M, self.d_order, self.d_n_arrived, stream)
-        else:
-            B.psync_order_by_arrival(d_arrival, self.W, self.d_order, self.d_n_arrived, stream)
-        if self.clip > 0:
+        if self.clip > 0:                 # norms and rates do not depend on the order: they are enqueued first
             sliced = self.layout == B.PSYNC_GRADS_SLICES
             key = (sliced, self.table.grad_dtype)
             if self._d_clip_work is None or self._d_clip_work[0] != key:
@@ -204,7 +200,7 @@ class AsyncServerStep:
         if self.lr is not None:
             gamma0, beta, s = self.lr
             B.psync_lr_schedule(gamma0, beta, self.t0 if t0 is None else t0, self.W, s, self.d_gamma, stream)
-        B.psync_async_apply(self._step, self.d_gamma, stream, d_gscale=self.d_gscale)
+        B.psync_async_step_device(self._step, d_arrival, self.d_gamma, stream, d_gscale=self.d_gscale)   # order + K iterations
         if self.track_staleness:
             B.psync_staleness_sharded(self.d_read_iter, self.d_order, self.d_t, self.d_staleness, self.d_stale_stats,
                                       self.d_stale_status, d_n_arrived=self.d_n_arrived, lag=self.lag, stream=stream)

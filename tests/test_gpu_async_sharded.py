@@ -637,3 +637,49 @@ def test_fixed_count_without_a_count_array_applies_exactly_N_per_server():
                                  gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
     assert rc == oracle.OK
     pair.compare_and_sync("fixed N per server", 9)
+
+
+def test_async_step_device_is_the_two_calls_in_one_and_validates_its_outputs():
+    cfg = replace(BASE, opt=synth.RMSPROP_MOM, name="arows_onecall")
+    flat = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    a = synth.arrival_times_per_server(cfg, 0, server_sigma=0.3)
+    a[2, 4] = np.inf
+    d_a = torch.from_numpy(a).to(DEV)
+    two, one = RowsPair(cfg, shard_off=RAGGED), RowsPair(cfg, shard_off=RAGGED)
+    sl = cut_slices(flat, two.off, lambda k, j: (k + j) % 4)
+    table = psync.make_slice_table(sl)
+    psync.psync_order_by_arrival_sharded(d_a, cfg.W, two.M, two.d_order, two.d_n)
+    st2, keep2 = two.make_step(table)
+    psync.psync_async_apply(st2)
+    st1, keep1 = one.make_step(table, N=1)               # N is ignored by the one-call form
+    psync.psync_async_step_device(st1, d_a)
+    torch.cuda.synchronize()
+    assert np.array_equal(one.d_n.cpu().numpy(), two.d_n.cpu().numpy()) and int(one.d_n[2].item()) == cfg.W - 1
+    for n in STATE_NAMES:
+        assert np.array_equal(to_np(getattr(one, n)), to_np(getattr(two, n))), n
+    before = to_np(one.theta)
+    st1.d_n_kept = None
+    assert psync.psync_async_step_device(st1, d_a, check=False) == psync.PSYNC_EINVAL
+    st1, keep1 = one.make_step(table)
+    st1.kept_stride = cfg.W - 1
+    assert psync.psync_async_step_device(st1, d_a, check=False) == psync.PSYNC_EINVAL
+    torch.cuda.synchronize()
+    assert np.array_equal(to_np(one.theta), before)
+    # flat buffers, one order: d_arrival [W]
+    f1, f2 = RowsPair(cfg), RowsPair(cfg)
+    ft = psync.make_grad_table(flat)
+    d_o = torch.full((cfg.W,), -1, dtype=torch.int32, device=DEV)
+    d_n = torch.zeros(1, dtype=torch.int32, device=DEV)
+
+    def flat_step(pair):
+        return psync.make_step(pair.off, cfg.W, cfg.W, ft.grad_dtype, pair.theta, pair.ema, pair.state0, pair.state1,
+                               opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho,
+                               eps=cfg.eps, d_grads=ft.d_ptrs, d_kept=d_o, d_n_kept=d_n, kept_stride=cfg.W)
+    sa, ka = flat_step(f1)
+    psync.psync_order_by_arrival(d_a[0], cfg.W, d_o, d_n)
+    psync.psync_async_apply(sa)
+    sb, kb = flat_step(f2)
+    psync.psync_async_step_device(sb, d_a[0])
+    torch.cuda.synchronize()
+    for n in STATE_NAMES:
+        assert np.array_equal(to_np(getattr(f1, n)), to_np(getattr(f2, n))), n
