@@ -816,6 +816,73 @@ def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist):
             "timing": "host wall clock around synchronous calls (the call returns when theta(t+1) is on the host)"}
 
 
+def run_launch_bound(args):
+    """--launch-bound: the cost of a step when the kernels take ~2 us (cfg1, P = 4096): host calls per step, in us, for the
+    synchronous step (two binding calls; psync_step_device; 100 steps replayed from a CUDA graph) and for one batch of
+    Alg. 2 (psync_async_step_device eager / graph; one order, and one order per server).  Host wall clock over many steps
+    between synchronisations.  One JSON line."""
+    import paper_1702_05800_b200 as psync
+
+    cfg, dev = synth.TINY, torch.device("cuda", env_int("LOCAL_RANK", 0))
+    torch.cuda.set_device(dev)
+    B = psync.binding
+    off = synth.shard_offsets(cfg)
+    grads = [synth.gradient(cfg, 0, k, dev) for k in range(cfg.W)]
+    arr = torch.from_numpy(np.stack([synth.arrival_times(cfg, s) for s in range(100)])).to(dev)
+    arr_rows = arr[:, None, :].repeat(1, cfg.M, 1).contiguous()
+    n_eager, n_replay = 2000, 20
+    st = torch.cuda.Stream(device=dev)
+    st.wait_stream(torch.cuda.current_stream())
+
+    def timed(fn, n):
+        for i in range(20):
+            fn(i)
+        st.synchronize()
+        t0 = time.perf_counter()
+        for i in range(n):
+            fn(i)
+        st.synchronize()
+        return (time.perf_counter() - t0) / n * 1e6
+
+    def graph_of(fn):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            for i in range(100):
+                fn(i)
+        g.replay()
+        st.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(n_replay):
+            g.replay()
+        st.synchronize()
+        return (time.perf_counter() - t0) / (100 * n_replay) * 1e6
+
+    out = {"workload": f"cfg1 {cfg.name}: P={cfg.P}, M={cfg.M}, N={cfg.N}, b={cfg.b}", "unit": "us per step (host wall clock)",
+           "steps_eager": n_eager, "steps_graph": 100 * n_replay}
+    with torch.cuda.stream(st):
+        for per_server in (False, True):
+            theta = synth.init_theta(cfg, dev)
+            ps = psync.ParameterServerStep(off, cfg.N, cfg.b, theta, theta.clone(), None, None, cfg.opt, cfg.ema_mode,
+                                           alpha=cfg.alpha, per_server=per_server)
+            ps.set_gradients(grads)
+            a = arr_rows if per_server else arr
+            key = "sync_per_server" if per_server else "sync"
+            out[key] = {"step_device_eager": timed(lambda i: ps.step(a[i % 100], cfg.gamma, stream=st), n_eager),
+                        "step_device_graph": graph_of(lambda i: ps.step(a[i], cfg.gamma, stream=st))}
+            if not per_server:
+                def two_calls(i):
+                    B.psync_select_first_n(a[i % 100], cfg.N, cfg.b, ps.d_kept, ps.d_status, ps.d_t_nth, None, 0, st)
+                    ps.aggregate_only(cfg.gamma, stream=st)
+                out[key]["two_binding_calls_eager"] = timed(two_calls, n_eager)
+            srv = psync.AsyncServerStep(off, cfg.W, theta, theta.clone(), None, None, cfg.opt, alpha=cfg.alpha,
+                                        per_server=per_server)
+            srv.set_gradients(grads)
+            key = "async_per_server" if per_server else "async"
+            out[key] = {"async_step_device_eager": timed(lambda i: srv.apply(a[i % 100], cfg.gamma, stream=st), n_eager),
+                        "async_step_device_graph": graph_of(lambda i: srv.apply(a[i], cfg.gamma, stream=st))}
+    return out
+
+
 # ------------------------------------------------------------------------------------ main
 def main():
     ap = argparse.ArgumentParser()
@@ -856,6 +923,8 @@ def main():
     ap.add_argument("--cpu-seconds-1thread", type=float, default=3.0)
     ap.add_argument("--clock-period-ms", type=float, default=2.0)
     ap.add_argument("--probe-every", type=int, default=4)
+    ap.add_argument("--launch-bound", action="store_true",
+                    help="cfg1 (P = 4096): us per step of the host calls, eager and replayed from a CUDA graph")
     ap.add_argument("--ref-sample-elems", type=int, default=0,
                     help="--impl reference: run on the first this-many parameters only (0 = the full workload)")
     args = ap.parse_args()
@@ -870,6 +939,11 @@ def main():
         if args.ref_sample_elems <= 0 and args.steps + args.warmup > 400:
             args.ref_sample_elems = 1 << 22  # an unusually long run: keep it within a few minutes of host time
         print(json.dumps(run_reference(args, cfg, rank)), flush=True)
+        return 0
+
+    if args.launch_bound:
+        if rank == 0:
+            print(json.dumps(run_launch_bound(args)), flush=True)
         return 0
 
     dist = None
