@@ -816,6 +816,36 @@ def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist):
             "timing": "host wall clock around synchronous calls (the call returns when theta(t+1) is on the host)"}
 
 
+def run_probe_pipes(args):
+    """--probe-pipes: fp32 lane-operations per clock per SM of the FFMA, packed FFMA2 and MUFU.RSQ pipes (the library's
+    psync_probe_pipe), with the SM clock sampled while the probes run.  One JSON line."""
+    import paper_1702_05800_b200 as psync
+
+    dev = torch.device("cuda", env_int("LOCAL_RANK", 0))
+    torch.cuda.set_device(dev)
+    B = psync.binding
+    st = torch.cuda.Stream(device=dev)
+    sink = torch.zeros(4, dtype=torch.float32, device=dev)
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    out = {"sms": sms, "unit": "fp32 lane-operations per clock per SM", "pipes": {}}
+    sampler = ClockSampler(env_int("LOCAL_RANK", 0), period_s=0.002)
+    sampler.start()
+    for name, mode, iters in (("ffma", 0, 1 << 16), ("ffma2_packed", 1, 1 << 16), ("mufu_rsqrt", 2, 1 << 14)):
+        B.psync_probe_pipe(mode, 256, sink, st)                      # warm-up
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        ops = B.psync_probe_pipe(mode, iters, sink, st)
+        e1.record(st)
+        st.synchronize()
+        out["pipes"][name] = {"lane_ops": ops, "ms": e0.elapsed_time(e1)}
+    clocks = sampler.stop()
+    mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz")
+    for v in out["pipes"].values():
+        v["per_clock_per_sm"] = v["lane_ops"] / (v["ms"] * 1e-3) / (mhz * 1e6) / sms
+    out["clocks"] = clocks
+    return out
+
+
 def run_launch_bound(args):
     """--launch-bound: the cost of a step when the kernels take ~2 us (cfg1, P = 4096): host calls per step, in us, for the
     synchronous step (two binding calls; psync_step_device; 100 steps replayed from a CUDA graph) and for one batch of
@@ -923,6 +953,8 @@ def main():
     ap.add_argument("--cpu-seconds-1thread", type=float, default=3.0)
     ap.add_argument("--clock-period-ms", type=float, default=2.0)
     ap.add_argument("--probe-every", type=int, default=4)
+    ap.add_argument("--probe-pipes", action="store_true",
+                    help="FFMA / packed FFMA2 / MUFU.RSQ lane-operations per clock per SM (psync_probe_pipe)")
     ap.add_argument("--launch-bound", action="store_true",
                     help="cfg1 (P = 4096): us per step of the host calls, eager and replayed from a CUDA graph")
     ap.add_argument("--ref-sample-elems", type=int, default=0,
@@ -944,6 +976,10 @@ def main():
     if args.launch_bound:
         if rank == 0:
             print(json.dumps(run_launch_bound(args)), flush=True)
+        return 0
+    if args.probe_pipes:
+        if rank == 0:
+            print(json.dumps(run_probe_pipes(args)), flush=True)
         return 0
 
     dist = None

@@ -30,7 +30,7 @@ EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psyn
            "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_host_ctx_create", "psync_host_ctx_destroy",
            "psync_step_host_ctx", "psync_launch_geometry", "psync_probe_read",
-           "psync_probe_copy", "psync_selftest_rsqrt")
+           "psync_probe_copy", "psync_probe_pipe", "psync_selftest_rsqrt")
 
 
 class PsyncError(RuntimeError):
@@ -127,6 +127,8 @@ def lib() -> ctypes.CDLL:
         L.psync_probe_read.restype = ctypes.c_int
         L.psync_probe_copy.argtypes = [vp, vp, i64, vp]
         L.psync_probe_copy.restype = ctypes.c_int
+        L.psync_probe_pipe.argtypes = [i32, i64, vp, ctypes.POINTER(ctypes.c_int64), vp]
+        L.psync_probe_pipe.restype = ctypes.c_int
         L.psync_selftest_rsqrt.argtypes = [vp, ctypes.c_uint32, i64, vp, vp, vp]
         L.psync_selftest_rsqrt.restype = ctypes.c_int
         _lib = L
@@ -599,8 +601,17 @@ def psync_probe_copy(d_dst: torch.Tensor, d_src: torch.Tensor, stream=None) -> i
     n = d_src.numel() * d_src.element_size() // 16
     st = lib().psync_probe_copy(_dptr(d_dst), _dptr(d_src), n, _stream(stream))
     if st != PSYNC_OK:
-        raise PsyncError(st, "psync_probe_copy", "psync_selftest_rsqrt")
+        raise PsyncError(st, "psync_probe_copy")
     return n * 32
+
+
+def psync_probe_pipe(mode: int, iters: int, d_sink: torch.Tensor, stream=None) -> int:
+    """Arithmetic-pipe probe (include/psync.h: psync_probe_pipe): returns the fp32 lane-operations of the launch."""
+    ops = ctypes.c_int64(0)
+    st = lib().psync_probe_pipe(mode, iters, _dptr(d_sink, torch.float32), ctypes.byref(ops), _stream(stream))
+    if st != PSYNC_OK:
+        raise PsyncError(st, "psync_probe_pipe")
+    return ops.value
 
 
 def psync_selftest_rsqrt(d_mismatch: torch.Tensor, n: int, first_bits: int = 0, d_x: Optional[torch.Tensor] = None,

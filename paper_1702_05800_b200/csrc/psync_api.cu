@@ -469,6 +469,15 @@ PSYNC_API int psync_probe_copy(void* d_dst, const void* d_src, int64_t n_vec16, 
                                                                                                             : PSYNC_ECUDA;
 }
 
+PSYNC_API int psync_probe_pipe(int32_t mode, int64_t iters, float* d_sink, int64_t* h_lane_ops, void* stream) {
+  if (mode < 0 || mode > 2 || iters < 1 || d_sink == nullptr) return PSYNC_EINVAL;
+  int ctas = 0;
+  if (psync::launch_probe_pipe(mode, iters, d_sink, &ctas, static_cast<cudaStream_t>(stream)) != cudaSuccess)
+    return PSYNC_ECUDA;
+  if (h_lane_ops != nullptr) *h_lane_ops = static_cast<int64_t>(ctas) * 256 * 8 * iters * (mode == 1 ? 2 : 1);
+  return PSYNC_OK;
+}
+
 PSYNC_API int psync_selftest_rsqrt(const float* d_x, uint32_t first_bits, int64_t n, float* d_y,
                          unsigned long long* d_mismatch, void* stream) {
   if (n < 0 || d_mismatch == nullptr) return PSYNC_EINVAL;
