@@ -244,3 +244,18 @@ def test_interp_iterations_and_fig6_estimate_on_the_gpu():
     assert L.psync_interp_iterations(n2.ctypes.data, i2.ctypes.data, 2, W, d_iters.data_ptr(), None) == psync.PSYNC_EINVAL
     assert L.psync_interp_iterations(n2.ctypes.data, i2.ctypes.data, 0, W, d_iters.data_ptr(), None) == psync.PSYNC_EINVAL
     assert L.psync_interp_iterations(None, i2.ctypes.data, 1, W, d_iters.data_ptr(), None) == psync.PSYNC_EINVAL
+
+
+def test_probe_pipe_counts_its_lane_operations_and_validates():
+    """Bench support (psync_probe_pipe): the reported operation count is CTAs x 256 threads x 8 chains x iters (x 2 packed)."""
+    sink = torch.zeros(4, dtype=torch.float32, device=DEV)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    B = psync.binding
+    assert B.psync_probe_pipe(0, 16, sink) == sms * 8 * 256 * 8 * 16
+    assert B.psync_probe_pipe(1, 16, sink) == sms * 8 * 256 * 8 * 16 * 2
+    assert B.psync_probe_pipe(2, 16, sink) == sms * 8 * 256 * 8 * 16
+    torch.cuda.synchronize()
+    L = B.lib()
+    assert L.psync_probe_pipe(3, 16, sink.data_ptr(), None, None) == psync.PSYNC_EINVAL
+    assert L.psync_probe_pipe(0, 0, sink.data_ptr(), None, None) == psync.PSYNC_EINVAL
+    assert L.psync_probe_pipe(0, 16, None, None, None) == psync.PSYNC_EINVAL
