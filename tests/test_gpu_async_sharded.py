@@ -13,7 +13,7 @@ import oracle
 import paper_1702_05800_b200 as psync
 from paper_1702_05800_b200 import synth
 
-from _harness import ATOL_STEP, STATE_NAMES, assert_close, to_np
+from _harness import ATOL_STEP, RTOL_BF16, RTOL_STEP, STATE_NAMES, assert_close, to_np
 from test_gpu_slices import RAGGED, cut_slices, np_slices
 
 pytestmark = pytest.mark.gpu
@@ -683,3 +683,79 @@ def test_async_step_device_is_the_two_calls_in_one_and_validates_its_outputs():
     torch.cuda.synchronize()
     for n in STATE_NAMES:
         assert np.array_equal(to_np(getattr(f1, n)), to_np(getattr(f2, n))), n
+
+
+# ------------------------------------------------------------------ guard bands (compute-sanitizer is closed on this pool)
+@pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
+@pytest.mark.parametrize("kernel", ["K2s", "K4s"])
+def test_guard_bands_around_every_slice_and_around_theta_state_ema(kernel, dtype):
+    """Every (worker, server) slice sits inside its own allocation whose guard bands hold NaN (a USED out-of-bounds read
+    would poison the result and fail parity); theta / state / ema sit inside allocations whose bands hold a sentinel (an
+    out-of-bounds write would change it).  Ragged servers incl. an empty and a one-element one, odd element offsets (head
+    peel, mixed phases), both shard-aware kernels."""
+    cfg = replace(BASE, grad_dtype=dtype, opt=synth.RMSPROP_MOM, name=f"guard_{kernel}_d{dtype}")
+    off = np.asarray(RAGGED, dtype=np.int64)
+    M, P, PAD, SENT = off.size - 1, int(off[-1]), 64, 12345.0
+    tdt = torch.float32 if dtype == synth.F32 else torch.bfloat16
+
+    def banded_state(t):
+        raw = torch.full((P + 2 * PAD,), SENT, dtype=torch.float32, device=DEV)
+        raw[PAD:PAD + P].copy_(t)
+        return raw, raw[PAD:PAD + P]
+
+    th_raw, theta = banded_state(synth.init_theta(cfg, DEV))
+    s0i, s1i = synth.init_state(cfg, DEV)
+    s0_raw, s0 = banded_state(s0i)
+    s1_raw, s1 = banded_state(s1i)
+    em_raw, ema = banded_state(theta.clone())
+    flat = [synth.gradient(cfg, 0, k, DEV) for k in range(cfg.W)]
+    raws, sl = [], []
+    for k, g in enumerate(flat):
+        row = []
+        for j in range(M):
+            lo, hi = int(off[j]), int(off[j + 1])
+            o = PAD + (3 * k + 5 * j) % 8
+            raw = torch.full((hi - lo + o + PAD,), float("nan"), dtype=tdt, device=DEV)
+            raw[o:o + hi - lo].copy_(g[lo:hi])
+            raws.append((raw, o, hi - lo))
+            row.append(raw[o:o + hi - lo])
+        sl.append(row)
+    table = psync.make_slice_table(sl)
+    d_off = torch.from_numpy(off).to(DEV)
+    d_tiles = psync.psync_shard_worklist(d_off, cfg.grad_dtype)
+    host = {"theta": to_np(theta), "ema": to_np(ema), "state0": to_np(s0), "state1": to_np(s1)}
+    a = synth.arrival_times_per_server(cfg, 0, server_sigma=0.3)
+    common = dict(opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
+    if kernel == "K2s":
+        N, b = 10, 3
+        d_kept = torch.full((M, N), -1, dtype=torch.int32, device=DEV)
+        d_status = torch.full((M,), -9, dtype=torch.int32, device=DEV)
+        st, keep = psync.make_step(off, N, cfg.W, table.grad_dtype, theta, ema, s0, s1, d_grads=table.d_ptrs, d_kept=d_kept,
+                                   d_status=d_status, per_shard=True, d_shard_off=d_off,
+                                   grad_layout=psync.PSYNC_GRADS_SLICES, d_tile_start=d_tiles, **common)
+        psync.psync_step_device(st, torch.from_numpy(a).to(DEV))
+        torch.cuda.synchronize()
+        status, kept, _ = oracle.select_first_n_sharded(a, N, b)
+        assert np.array_equal(d_kept.cpu().numpy(), kept)
+        rc = oracle.aggregate_update_slices(off, N, np_slices(sl), kept, host["theta"], host["ema"], host["state0"],
+                                            host["state1"], per_shard=True, status=status, **common)
+        rtol = RTOL_BF16 if dtype == synth.BF16 else RTOL_STEP
+    else:
+        d_order = torch.full((M, cfg.W), -1, dtype=torch.int32, device=DEV)
+        d_n = torch.zeros(M, dtype=torch.int32, device=DEV)
+        st, keep = psync.make_step(off, cfg.W, cfg.W, table.grad_dtype, theta, ema, s0, s1, d_grads=table.d_ptrs,
+                                   d_kept=d_order, d_n_kept=d_n, kept_stride=cfg.W, per_shard=True, d_shard_off=d_off,
+                                   grad_layout=psync.PSYNC_GRADS_SLICES, d_tile_start=d_tiles, **common)
+        psync.psync_async_step_device(st, torch.from_numpy(a).to(DEV))
+        torch.cuda.synchronize()
+        order = np.stack([oracle.order_by_arrival(a[j]) for j in range(M)])
+        rc = oracle.async_apply_rows(off, np_slices(sl), order, host["theta"], host["ema"], host["state0"], host["state1"],
+                                     slices=True, per_shard=True, **common)
+        rtol = rtol_async(cfg.W)
+    assert rc == oracle.OK
+    for n, t in (("theta", theta), ("ema", ema), ("state0", s0), ("state1", s1)):
+        assert_close(to_np(t), host[n], rtol, ATOL_STEP, f"guard {kernel} {n}")
+    for raw in (th_raw, em_raw, s0_raw, s1_raw):
+        assert bool((raw[:PAD] == SENT).all()) and bool((raw[PAD + P:] == SENT).all()), "write outside theta / state / ema"
+    for raw, o, n in raws:
+        assert bool(torch.isnan(raw[:o].float()).all()) and bool(torch.isnan(raw[o + n:].float()).all())
