@@ -816,6 +816,56 @@ def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist):
             "timing": "host wall clock around synchronous calls (the call returns when theta(t+1) is on the host)"}
 
 
+def run_instances(args, base_cfg):
+    """--instances: every template instance of the kernel of --mode (2 gradient dtypes x 3 optimizers x 3 EMA modes) on the
+    shape of --config: kernel ms and GB/s of algorithmic bytes, so that no instance hides behind the three that the
+    configs exercise.  One JSON line; --instances-md writes the table."""
+    from dataclasses import replace
+    import paper_1702_05800_b200 as psync
+
+    dev = torch.device("cuda", env_int("LOCAL_RANK", 0))
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.Stream(device=dev)
+    peak, peak_src = load_peaks()
+    mode = args.mode
+    rows = []
+    for dtype, dname in ((synth.F32, "fp32"), (synth.BF16, "bf16")):
+        wl = None
+        for opt, oname in ((synth.SGD, "sgd"), (synth.MOMENTUM, "momentum"), (synth.RMSPROP_MOM, "rmsprop_momentum")):
+            for ema, ename in ((synth.EMA_POST, "post"), (synth.EMA_PRE, "pre"), (synth.EMA_OFF, "off")):
+                cfg = replace(base_cfg, grad_dtype=dtype, opt=opt, ema_mode=ema, mu=0.9, rho=0.9, eps=1.0,
+                              name=f"{base_cfg.name}_{dname}_{oname}_ema{ename}")
+                if wl is None:                       # one resident gradient set pair per dtype; only the instance changes
+                    wl = Workload(psync, replace(cfg, opt=synth.RMSPROP_MOM, ema_mode=synth.EMA_POST), dev, 2, layout=args.layout)
+                wl.cfg = cfg
+                wl.reset_state()
+                m = measure(psync, args, wl, mode, 6, 3, stream, variant=args.variant, probe_every=1)
+                e = short_entry(cfg, mode, args.layout, m, peak)
+                e.update({"grad_dtype": dname, "optimizer": oname, "ema": ename})
+                rows.append(e)
+        del wl
+        torch.cuda.empty_cache()
+    out = {"workload": f"{base_cfg.name}: P={base_cfg.P}, N={base_cfg.N}, b={base_cfg.b}, M={base_cfg.M}", "mode": mode,
+           "grad_layout": args.layout, "peak": peak, "peak_source": peak_src, "instances": rows}
+    if args.instances_md:
+        lines = [f"# Every template instance on {out['workload']} (`--mode {mode}`, layout {args.layout})", "",
+                 f"Command: `python bench.py --config {args.config} --mode {mode}"
+                 + ("" if args.layout == "flat" else " --layout slices") + (f" --variant {args.variant}" if args.variant else "")
+                 + " --instances --instances-md <this file>`; 3 warm-up + 6 "
+                 "timed steps each, fused-kernel time from CUDA events; GB/s of algorithmic bytes (of nominal 8 TB/s).", "",
+                 "| gradients | optimizer | EMA post | EMA pre | EMA off |", "|---|---|---|---|---|"]
+        for dname in ("fp32", "bf16"):
+            for oname in ("sgd", "momentum", "rmsprop_momentum"):
+                cells = []
+                for ename in ("post", "pre", "off"):
+                    e = next(r for r in rows if (r["grad_dtype"], r["optimizer"], r["ema"]) == (dname, oname, ename))
+                    cells.append(f"{e['kernel_ms']:.4f} ms, {e['gbps']:.0f} ({100 * e['frac_of_nominal_8TBps']:.0f} %)")
+                lines.append(f"| {dname} | {oname} | " + " | ".join(cells) + " |")
+        with open(args.instances_md, "w") as fh:
+            fh.write("\n".join(lines) + "\n")
+    return out
+
+
 def run_probe_pipes(args):
     """--probe-pipes: fp32 lane-operations per clock per SM of the FFMA, packed FFMA2 and MUFU.RSQ pipes (the library's
     psync_probe_pipe), with the SM clock sampled while the probes run.  One JSON line."""
@@ -953,6 +1003,9 @@ def main():
     ap.add_argument("--cpu-seconds-1thread", type=float, default=3.0)
     ap.add_argument("--clock-period-ms", type=float, default=2.0)
     ap.add_argument("--probe-every", type=int, default=4)
+    ap.add_argument("--instances", action="store_true",
+                    help="every template instance (dtype x optimizer x EMA mode) of --mode's kernel on --config's shape")
+    ap.add_argument("--instances-md", default="", help="--instances: also write the table as markdown to this path")
     ap.add_argument("--probe-pipes", action="store_true",
                     help="FFMA / packed FFMA2 / MUFU.RSQ lane-operations per clock per SM (psync_probe_pipe)")
     ap.add_argument("--launch-bound", action="store_true",
@@ -980,6 +1033,10 @@ def main():
     if args.probe_pipes:
         if rank == 0:
             print(json.dumps(run_probe_pipes(args)), flush=True)
+        return 0
+    if args.instances:
+        if rank == 0:
+            print(json.dumps(run_instances(args, cfg)), flush=True)
         return 0
 
     dist = None
