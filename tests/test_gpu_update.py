@@ -10,7 +10,7 @@ import oracle
 import paper_1702_05800_b200 as psync
 from paper_1702_05800_b200 import synth
 
-from _harness import ATOL_STEP, RTOL_BF16, RTOL_FREE_100, RTOL_STEP, Pair, assert_close, to_np
+from _harness import ATOL_STEP, RTOL_BF16, RTOL_STEP, Pair, assert_close, to_np
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda"

@@ -8,7 +8,6 @@ N=1, b=0" onto the already pinned synchronous step.
 import itertools
 import json
 import os
-from fractions import Fraction
 
 import numpy as np
 import pytest

@@ -8,13 +8,12 @@ allocated, odd-offset slices (P <= 64), and from numpy's float64 mean per slice.
 """
 import json
 import os
-from fractions import Fraction
 
 import numpy as np
 import pytest
 
 import oracle
-from test_oracle_update import F, _round_f32, coeffs, exact_step, f32, to_bf16_bits, bf16_bits_to_f32
+from test_oracle_update import exact_step, f32, to_bf16_bits, bf16_bits_to_f32
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "hand_worked_slices.json")
 
