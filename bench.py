@@ -658,8 +658,8 @@ def run_psync(args, cfg, rank, world, dist):
     theta, ema, s0, s1, off = wl.theta, wl.ema, wl.s0, wl.s1, wl.off
     del wl.tables, wl.sets
     torch.cuda.empty_cache()
-    if not args.no_e2e and mode == "first_n":
-        out["e2e"] = run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist)
+    if not args.no_e2e and mode in ("first_n", "async"):
+        out["e2e"] = run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist, mode=mode)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
         if host_grads is None:               # no room in host RAM for one gradient set: bounded sample
@@ -764,7 +764,7 @@ def write_sweep_md(path, points, peak, peak_src, mode="first_n", layout="flat"):
         fh.write("\n".join(lines))
 
 
-def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist):
+def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist, mode="first_n"):
     """The same metric through psync_step_host: gradients and arrival times start in pinned HOST memory
     every step, theta(t+1) is read back to the host every step; all copies are inside the timed region."""
     import paper_1702_05800_b200 as psync
@@ -782,7 +782,9 @@ def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist):
     h_theta = torch.empty(cfg.P, dtype=torch.float32, pin_memory=True)
     h_kept = np.zeros(cfg.N, dtype=np.int32)
     chunk = args.e2e_chunk
-    nbytes = psync.psync_step_host_workspace_bytes(cfg.N, cfg.W, cfg.grad_dtype, chunk)
+    is_async = mode == "async"          # Alg. 2: every gradient that arrived crosses PCIe (nothing is dropped)
+    n_moved = cfg.W if is_async else cfg.N
+    nbytes = psync.psync_step_host_workspace_bytes(n_moved, cfg.W, cfg.grad_dtype, chunk)
     d_work = torch.empty(nbytes, dtype=torch.uint8, device=dev)
     slices = getattr(args, "layout", "flat") == "slices"
     if slices:   # what each server received, in host memory: W x M slices (here views of the pinned buffers)
@@ -793,25 +795,30 @@ def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist):
                                  grad_layout=psync.PSYNC_GRADS_SLICES if slices else psync.PSYNC_GRADS_FLAT)
     arrivals = [synth.arrival_times(cfg, 2000 + s) for s in range(K + 1)]
     ctx = psync.HostCtx()               # the copy stream and events, created once for the loop
-    psync.psync_step_host(step, arrivals[K], h_grads, d_work, h_theta_out=h_theta, h_kept=h_kept, chunk_elems=chunk,
-                          stream=stream, ctx=ctx)                          # warm-up
+    def host_step(a):
+        if is_async:
+            return psync.psync_async_step_host(step, a, h_grads, d_work, h_theta_out=h_theta, chunk_elems=chunk,
+                                               stream=stream, ctx=ctx)
+        return psync.psync_step_host(step, a, h_grads, d_work, h_theta_out=h_theta, h_kept=h_kept, chunk_elems=chunk,
+                                     stream=stream, ctx=ctx)
+    host_step(arrivals[K])                                                 # warm-up
     if dist is not None and dist.is_initialized():
         dist.barrier()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for s in range(K):
-        st, _ = psync.psync_step_host(step, arrivals[s], h_grads, d_work, h_theta_out=h_theta, h_kept=h_kept,
-                                      chunk_elems=chunk, stream=stream, ctx=ctx)
+        st, _ = host_step(arrivals[s])
         assert st == 0
     torch.cuda.synchronize()
     ms = (time.perf_counter() - t0) * 1e3
-    units, max_ms = aggregate_over_ranks(float(cfg.N) * cfg.P * K, ms, dist)
+    units, max_ms = aggregate_over_ranks(float(n_moved) * cfg.P * K, ms, dist)
     n_chunks = -(-cfg.P // (chunk if chunk else 1 << 20))
     return {"value": units / (max_ms * 1e-3), "unit": UNIT, "steps": K, "ms_per_step": max_ms / K,
-            "h2d_bytes_per_step": cfg.N * cfg.P * cfg.grad_bytes + 4 * cfg.W,
+            "h2d_bytes_per_step": n_moved * cfg.P * cfg.grad_bytes + 4 * cfg.W,
             "d2h_bytes_per_step": 4 * cfg.P + 4 * cfg.N + 8,
-            "api": "psync_step_host (C ABI, pinned host gradient buffers" + (" as W x M per-(worker, server) slices" if slices else "")
-                   + "; only the N kept buffers cross PCIe)",
+            "api": ("psync_async_step_host" if is_async else "psync_step_host") + " (C ABI, pinned host gradient buffers"
+                   + (" as W x M per-(worker, server) slices" if slices else "")
+                   + ("; all W arriving buffers cross PCIe)" if is_async else "; only the N kept buffers cross PCIe)"),
             "gpu_launches_per_step": 3 + n_chunks,
             "timing": "host wall clock around synchronous calls (the call returns when theta(t+1) is on the host)"}
 

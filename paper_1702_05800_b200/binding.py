@@ -29,7 +29,7 @@ EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psyn
            "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_order_by_arrival_sharded", "psync_clip_slices_workspace_bytes", "psync_clip_scales_slices", "psync_async_apply", "psync_async_step_device", "psync_staleness", "psync_staleness_sharded", "psync_step_device", "psync_clip_workspace_bytes",
            "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_host_ctx_create", "psync_host_ctx_destroy",
-           "psync_step_host_ctx", "psync_launch_geometry", "psync_probe_read",
+           "psync_step_host_ctx", "psync_async_step_host", "psync_launch_geometry", "psync_probe_read",
            "psync_probe_copy", "psync_probe_pipe", "psync_selftest_rsqrt")
 
 
@@ -121,6 +121,9 @@ def lib() -> ctypes.CDLL:
         L.psync_step_host_ctx.argtypes = [vp, ctypes.POINTER(psync_step), vp, vp, i32, vp, vp, vp, vp, vp,
                                           ctypes.c_size_t, i64, vp]
         L.psync_step_host_ctx.restype = ctypes.c_int
+        L.psync_async_step_host.argtypes = [vp, ctypes.POINTER(psync_step), vp, vp, vp, vp, vp, vp, vp, ctypes.c_size_t,
+                                            i64, vp]
+        L.psync_async_step_host.restype = ctypes.c_int
         L.psync_launch_geometry.argtypes = [ctypes.POINTER(psync_step), vp, vp, vp, vp]
         L.psync_launch_geometry.restype = ctypes.c_int
         L.psync_probe_read.argtypes = [vp, i64, vp, vp]
@@ -587,6 +590,50 @@ def psync_step_host(step: psync_step, h_arrival: np.ndarray, h_grads: Sequence[t
     if check and st not in (PSYNC_OK, PSYNC_ETOOFEW):
         raise PsyncError(st, "psync_step_host")
     return st, t_nth.value
+
+
+def psync_async_step_host(step: psync_step, h_arrival: np.ndarray, h_grads, d_work: torch.Tensor,
+                          h_gamma: Optional[np.ndarray] = None, h_theta_out: Optional[torch.Tensor] = None,
+                          h_order: Optional[np.ndarray] = None, chunk_elems: int = 0, stream=None, check: bool = True,
+                          ctx: Optional[HostCtx] = None):
+    """One batch of Alg. 2 with HOST gradient buffers (include/psync.h: psync_async_step_host).  h_grads: W CPU tensors, or
+    with step.grad_layout = SLICES W lists of M CPU tensors.  Returns (status, n_arrived)."""
+    W = step.W
+    if len(h_grads) != W or h_arrival.size != W or h_arrival.dtype != np.float32:
+        raise ValueError("need W host gradient buffers and W fp32 arrival times")
+    if step.grad_layout == PSYNC_GRADS_SLICES:
+        M = step.M
+        flat_ptrs = []
+        for row in h_grads:
+            if len(row) != M:
+                raise ValueError("every worker needs M host slices")
+            for g in row:
+                if g is not None and (g.is_cuda or not g.is_contiguous()):
+                    raise ValueError("host slices must be contiguous CPU tensors")
+                flat_ptrs.append(None if g is None else g.data_ptr())
+        ptrs = (ctypes.c_void_p * (W * M))(*flat_ptrs)
+    else:
+        for g in h_grads:
+            if g.is_cuda or not g.is_contiguous() or g.numel() != step.P:
+                raise ValueError("h_grads must be contiguous CPU tensors of P elements")
+        ptrs = (ctypes.c_void_p * W)(*[g.data_ptr() for g in h_grads])
+    if h_gamma is not None and (h_gamma.dtype != np.float32 or h_gamma.size < W):
+        raise ValueError("h_gamma must be float32[W]")
+    if h_order is not None and (h_order.dtype != np.int32 or h_order.size < W):
+        raise ValueError("h_order must be int32[W]")
+    if h_theta_out is not None and (h_theta_out.is_cuda or h_theta_out.dtype != torch.float32
+                                    or h_theta_out.numel() != step.P):
+        raise ValueError("h_theta_out must be a CPU float32 tensor of P elements")
+    n = ctypes.c_int32(-1)
+    st = lib().psync_async_step_host(None if ctx is None else ctx.handle, ctypes.byref(step), h_arrival.ctypes.data,
+                                     ctypes.cast(ptrs, ctypes.c_void_p), None if h_gamma is None else h_gamma.ctypes.data,
+                                     None if h_theta_out is None else h_theta_out.data_ptr(),
+                                     None if h_order is None else h_order.ctypes.data, ctypes.byref(n),
+                                     _dptr(d_work, None, "d_work"), d_work.numel() * d_work.element_size(), chunk_elems,
+                                     _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_async_step_host")
+    return st, n.value
 
 
 def psync_probe_read(d_src: torch.Tensor, d_sink: torch.Tensor, stream=None) -> int:

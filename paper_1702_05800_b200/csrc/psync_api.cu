@@ -522,9 +522,16 @@ PSYNC_API int psync_step_host(const psync_step* st, const float* h_arrival, cons
                              work_bytes, chunk_elems, stream);
 }
 
-PSYNC_API int psync_step_host_ctx(void* ctx, const psync_step* st, const float* h_arrival, const int32_t* h_step_tag,
-                        int32_t t, const void* const* h_grads, float* h_theta_out, int32_t* h_kept, float* h_t_nth,
-                        void* d_work, size_t work_bytes, int64_t chunk_elems, void* stream) {
+}  // extern "C"
+
+namespace {
+// The host-buffer pipeline behind psync_step_host_ctx (Alg. 4: selection, then the N kept buffers) and
+// psync_async_step_host (async_mode, Alg. 2: arrival order, then every buffer that arrived, applied one at a time by K4 on
+// each staged chunk; h_kept receives the order, *h_n_arrived the count, h_gamma optional per-iteration rates).
+int host_step_impl(void* ctx, const psync_step* st, const float* h_arrival, const int32_t* h_step_tag, int32_t t,
+                   const void* const* h_grads, float* h_theta_out, int32_t* h_kept, float* h_t_nth, void* d_work,
+                   size_t work_bytes, int64_t chunk_elems, void* stream, bool async_mode, const float* h_gamma,
+                   int32_t* h_n_arrived) {
   if (st == nullptr) return PSYNC_EINVAL;
   psync_step flat = *st;  // the device side of this path is always the flat stream (see SLICES below)
   flat.grad_layout = PSYNC_GRADS_FLAT;
@@ -540,13 +547,14 @@ PSYNC_API int psync_step_host_ctx(void* ctx, const psync_step* st, const float* 
   // range that intersects the chunk), so the device side is the flat pipeline unchanged.
   const bool h_slices = st->grad_layout == PSYNC_GRADS_SLICES;
   HostLayout L;
-  if (!host_layout(st->N, st->W, st->grad_dtype, chunk_elems, &L)) return PSYNC_EINVAL;
+  if (!host_layout(async_mode ? st->W : st->N, st->W, st->grad_dtype, chunk_elems, &L)) return PSYNC_EINVAL;
   if (work_bytes < L.total || (reinterpret_cast<uintptr_t>(d_work) & 255u) != 0) return PSYNC_EINVAL;
   if (!h_slices)
     for (int32_t k = 0; k < st->W; ++k)
       if (h_grads[k] == nullptr) return PSYNC_EINVAL;
 
-  const int32_t N = st->N, W = st->W;
+  const int32_t W = st->W;
+  int32_t N = async_mode ? W : st->N;  // async: replaced by the number of gradients that arrived
   const int64_t esz = st->grad_dtype == PSYNC_BF16 ? 2 : 4;
   char* work = static_cast<char*>(d_work);
   float* d_arrival = reinterpret_cast<float*>(work + L.off_arrival);
@@ -560,7 +568,7 @@ PSYNC_API int psync_step_host_ctx(void* ctx, const psync_step* st, const float* 
   HostCtx local;                                   // used when the caller brought no context
   HostCtx* hc = ctx != nullptr ? static_cast<HostCtx*>(ctx) : &local;
   int result = PSYNC_OK;
-  std::vector<int32_t> kept(N);
+  std::vector<int32_t> kept(N);  // N = W in async mode
   int32_t status = PSYNC_ECUDA;
   float t_nth = 0.f;
 
@@ -572,22 +580,38 @@ PSYNC_API int psync_step_host_ctx(void* ctx, const psync_step* st, const float* 
     }                               \
   } while (0)
 
-  // 1. selection on the device (Alg. 4 l.3-6): the only thing the host learns is kept[] / status
+  // 1. selection on the device (Alg. 4 l.3-6): the only thing the host learns is kept[] / status;
+  //    async: the arrival order (Alg. 2, L85) and how many gradients arrived
   PSYNC_CU(cudaMemcpyAsync(d_arrival, h_arrival, sizeof(float) * W, cudaMemcpyHostToDevice, s));
-  if (h_step_tag != nullptr)
-    PSYNC_CU(cudaMemcpyAsync(d_tags, h_step_tag, sizeof(int32_t) * W, cudaMemcpyHostToDevice, s));
-  PSYNC_CU(psync::launch_select_first_n(d_arrival, h_step_tag ? d_tags : nullptr, t, N, W, 1, d_kept, d_tnth, d_status, s));
-  PSYNC_CU(cudaMemcpyAsync(&status, d_status, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
-  PSYNC_CU(cudaStreamSynchronize(s));
-  if (status != PSYNC_OK) {
-    result = status;
-    goto cleanup;
+  if (async_mode) {
+    PSYNC_CU(psync::launch_order_by_arrival(d_arrival, W, 1, d_kept, d_status, s));  // d_status holds the count here
+    PSYNC_CU(cudaMemcpyAsync(&status, d_status, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    PSYNC_CU(cudaStreamSynchronize(s));
+    N = status;
+    if (h_n_arrived != nullptr) *h_n_arrived = N;
+    if (N < 0 || N > W) {
+      result = PSYNC_ECUDA;
+      goto cleanup;
+    }
+    if (h_gamma != nullptr && N > 0)  // the tag area of the workspace is free in this mode: the rates of this batch
+      PSYNC_CU(cudaMemcpyAsync(d_tags, h_gamma, sizeof(float) * N, cudaMemcpyHostToDevice, s));
+    flat.N = N > 0 ? N : 1;
+  } else {
+    if (h_step_tag != nullptr)
+      PSYNC_CU(cudaMemcpyAsync(d_tags, h_step_tag, sizeof(int32_t) * W, cudaMemcpyHostToDevice, s));
+    PSYNC_CU(psync::launch_select_first_n(d_arrival, h_step_tag ? d_tags : nullptr, t, N, W, 1, d_kept, d_tnth, d_status, s));
+    PSYNC_CU(cudaMemcpyAsync(&status, d_status, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    PSYNC_CU(cudaStreamSynchronize(s));
+    if (status != PSYNC_OK) {
+      result = status;
+      goto cleanup;
+    }
+    PSYNC_CU(cudaMemcpyAsync(&t_nth, d_tnth, sizeof(float), cudaMemcpyDeviceToHost, s));
   }
-  PSYNC_CU(cudaMemcpyAsync(kept.data(), d_kept, sizeof(int32_t) * N, cudaMemcpyDeviceToHost, s));
-  PSYNC_CU(cudaMemcpyAsync(&t_nth, d_tnth, sizeof(float), cudaMemcpyDeviceToHost, s));
+  if (N > 0) PSYNC_CU(cudaMemcpyAsync(kept.data(), d_kept, sizeof(int32_t) * N, cudaMemcpyDeviceToHost, s));
   for (int i = 0; i < 2; ++i)
     PSYNC_CU(psync::launch_fill_stage_table(reinterpret_cast<const void**>(work + L.off_ptrs[i]), d_ident,
-                                            work + L.off_stage[i], L.stride_bytes, N, s));
+                                            work + L.off_stage[i], L.stride_bytes, N > 0 ? N : 1, s));
   PSYNC_CU(cudaStreamSynchronize(s));
   if (h_slices)  // every slice of a KEPT worker must be there (dropped workers' slices are never looked at)
     for (int32_t n = 0; n < N; ++n)
@@ -596,8 +620,15 @@ PSYNC_API int psync_step_host_ctx(void* ctx, const psync_step* st, const float* 
           result = PSYNC_EINVAL;  // nothing has been updated yet
           goto cleanup;
         }
-  if (h_kept != nullptr) std::memcpy(h_kept, kept.data(), sizeof(int32_t) * N);
+  if (h_kept != nullptr && N > 0) std::memcpy(h_kept, kept.data(), sizeof(int32_t) * N);
   if (h_t_nth != nullptr) *h_t_nth = t_nth;
+  if (async_mode && N == 0) {  // nothing arrived: theta is unchanged (and still goes back to the host if asked for)
+    if (h_theta_out != nullptr && st->P > 0) {
+      PSYNC_CU(cudaMemcpyAsync(h_theta_out, st->d_theta, sizeof(float) * static_cast<size_t>(st->P), cudaMemcpyDeviceToHost, s));
+      PSYNC_CU(cudaStreamSynchronize(s));
+    }
+    goto cleanup;
+  }
 
   // 2./3. stream the kept buffers chunk by chunk; copy stream runs one chunk ahead of the kernel
   if (ctx == nullptr && !host_ctx_init(&local)) {
@@ -638,9 +669,14 @@ PSYNC_API int psync_step_host_ctx(void* ctx, const psync_step* st, const float* 
       }
       PSYNC_CU(cudaEventRecord(copied[buf], copy_stream));
       PSYNC_CU(cudaStreamWaitEvent(s, copied[buf], 0));
-      const FusedParams p = make_params(&flat, first, count, reinterpret_cast<const void* const*>(work + L.off_ptrs[buf]),
-                                        d_ident, nullptr);
-      PSYNC_CU(psync::launch_fused(p, st->grad_dtype, st->opt, st->ema_mode, st->variant, st->grid_ctas, s));
+      FusedParams p = make_params(&flat, first, count, reinterpret_cast<const void* const*>(work + L.off_ptrs[buf]),
+                                  d_ident, nullptr);
+      if (async_mode) {  // K4 on the staged chunk: slot i holds the i-th arrival
+        p.gammas = h_gamma != nullptr ? reinterpret_cast<const float*>(d_tags) : nullptr;
+        PSYNC_CU(psync::launch_async_apply_ring(p, st->grad_dtype, st->opt, st->ema_mode, st->grid_ctas, s));
+      } else {
+        PSYNC_CU(psync::launch_fused(p, st->grad_dtype, st->opt, st->ema_mode, st->variant, st->grid_ctas, s));
+      }
       PSYNC_CU(cudaEventRecord(consumed[buf], s));
       if (h_theta_out != nullptr)
         PSYNC_CU(cudaMemcpyAsync(h_theta_out + first, st->d_theta + first, sizeof(float) * static_cast<size_t>(count),
@@ -656,6 +692,23 @@ cleanup:
   if (hc->copy_stream != nullptr) cudaStreamSynchronize(hc->copy_stream);
   if (ctx == nullptr) host_ctx_release(&local);
   return result;
+}
+}  // namespace
+
+extern "C" {
+
+PSYNC_API int psync_step_host_ctx(void* ctx, const psync_step* st, const float* h_arrival, const int32_t* h_step_tag,
+                        int32_t t, const void* const* h_grads, float* h_theta_out, int32_t* h_kept, float* h_t_nth,
+                        void* d_work, size_t work_bytes, int64_t chunk_elems, void* stream) {
+  return host_step_impl(ctx, st, h_arrival, h_step_tag, t, h_grads, h_theta_out, h_kept, h_t_nth, d_work, work_bytes,
+                        chunk_elems, stream, false, nullptr, nullptr);
+}
+
+PSYNC_API int psync_async_step_host(void* ctx, const psync_step* st, const float* h_arrival, const void* const* h_grads,
+                          const float* h_gamma, float* h_theta_out, int32_t* h_order, int32_t* h_n_arrived, void* d_work,
+                          size_t work_bytes, int64_t chunk_elems, void* stream) {
+  return host_step_impl(ctx, st, h_arrival, nullptr, 0, h_grads, h_theta_out, h_order, nullptr, d_work, work_bytes,
+                        chunk_elems, stream, true, h_gamma, h_n_arrived);
 }
 
 }  // extern "C"

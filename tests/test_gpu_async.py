@@ -338,3 +338,54 @@ def test_async_launch_shapes_are_bit_identical(opt, dtype):
             for n, x in results[(scaled, 0)].items():
                 assert np.array_equal(x, results[(scaled, variant)][n]), (scaled, variant, n)
     assert not np.array_equal(results[(False, 0)]["theta"], results[(True, 0)]["theta"])
+
+
+# ------------------------------------------------------------------ host-buffer batch of Alg. 2
+@pytest.mark.parametrize("dtype,opt,chunk,slices", [(synth.F32, synth.RMSPROP_MOM, 8192, False),
+                                                   (synth.BF16, synth.MOMENTUM, 0, False),
+                                                   (synth.F32, synth.SGD, 4096, True)])
+def test_async_step_host_matches_the_oracle(dtype, opt, chunk, slices):
+    """psync_async_step_host: arrival times and gradients in HOST memory, every gradient that arrived crosses PCIe chunk by
+    chunk and is applied one at a time by K4 on the staged chunk; per-iteration rates; theta back on the host.  Two chained
+    batches (two workers never arrive in the second); with slices=True the host gradients are W x M slices."""
+    cfg = replace(BASE, P=60_001, grad_dtype=dtype, opt=opt, name=f"async_host_d{dtype}_o{opt}")
+    pair = AsyncPair(cfg)
+    nbytes = psync.psync_step_host_workspace_bytes(cfg.W, cfg.W, cfg.grad_dtype, chunk)
+    d_work = torch.empty(nbytes, dtype=torch.uint8, device=DEV)
+    h_theta = torch.empty(cfg.P, dtype=torch.float32).pin_memory()
+    h_order = np.full(cfg.W, -1, dtype=np.int32)
+    rng = np.random.default_rng(3)
+    for s in range(2):
+        flat = [synth.gradient(cfg, s, k, "cpu") for k in range(cfg.W)]
+        a = synth.arrival_times(cfg, s)
+        if s == 1:
+            a[[1, 7]] = np.inf
+        gam = rng.uniform(0.01, 0.09, cfg.W).astype(np.float32)
+        h_grads = [[g[int(pair.off[j]):int(pair.off[j + 1])].clone() for j in range(cfg.M)] for g in flat] if slices else flat
+        step, keep = psync.make_step(pair.off, cfg.W, cfg.W, cfg.grad_dtype, pair.theta, pair.ema, pair.state0, pair.state1,
+                                     opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu,
+                                     rho=cfg.rho, eps=cfg.eps,
+                                     grad_layout=psync.PSYNC_GRADS_SLICES if slices else psync.PSYNC_GRADS_FLAT)
+        st, K = psync.psync_async_step_host(step, a, h_grads, d_work, h_gamma=gam, h_theta_out=h_theta, h_order=h_order,
+                                            chunk_elems=chunk)
+        order = oracle.order_by_arrival(a)
+        assert st == 0 and K == order.size == (cfg.W if s == 0 else cfg.W - 2) and np.array_equal(h_order[:K], order)
+        h = pair.host
+        rc = oracle.async_apply(pair.off, [synth.as_numpy_grad(g) for g in flat], order, h["theta"], h["ema"], h["state0"],
+                                h["state1"], gammas=gam[:K].copy(), opt=cfg.opt, ema_mode=cfg.ema_mode, alpha=cfg.alpha,
+                                mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
+        assert rc == oracle.OK
+        for n in STATE_NAMES:
+            g = getattr(pair, n)
+            if g is not None:
+                tol = 2e-3 if dtype == synth.BF16 else rtol_async(K)
+                assert_close(to_np(g), h[n], tol, ATOL_STEP, f"async host batch {s} {n}")
+                h[n] = to_np(g)
+        assert np.array_equal(h_theta.numpy(), to_np(pair.theta))
+    # nobody arrives: OK, theta unchanged and still delivered; a too-small workspace is EINVAL
+    before = to_np(pair.theta)
+    st, K = psync.psync_async_step_host(step, np.full(cfg.W, np.nan, np.float32), h_grads, d_work, h_theta_out=h_theta,
+                                        chunk_elems=chunk)
+    assert st == 0 and K == 0 and np.array_equal(to_np(pair.theta), before) and np.array_equal(h_theta.numpy(), before)
+    st, K = psync.psync_async_step_host(step, a, h_grads, d_work[: nbytes // 2], chunk_elems=chunk, check=False)
+    assert st == psync.PSYNC_EINVAL
