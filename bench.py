@@ -2,7 +2,7 @@
 """bench.py -- whole-job throughput of the parameter-server step (Alg. 4) on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg1..cfg5] [--impl psync|reference]
-                    [--mode first_n|per_server|timeout|async] [--layout flat|slices] [--variant 1..7] [--servers M]
+                    [--mode first_n|per_server|timeout|async] [--layout flat|slices] [--variant 1..8] [--servers M]
 
 The default run is the headline (cfg3, first_n, flat buffers); its JSON line also carries `also`: short
 measurements of cfg2, cfg4, every other mode, the slices layout, many-server cuts and launch variants 5 / 6.

@@ -597,6 +597,7 @@ constexpr Variant kVariants[] = {
     {256, 1, 12, 3, kBulkRing},   // 5  cp.async.bulk -> 12-stage shared-memory ring (unroll = stages), 1 producer warp
     {256, 1, 8, 2, kPlain256},    // 6  256-bit loads with L2::evict_first, 8 in flight per thread
     {256, 1, 8, 4, kThreadRing},  // 7  per-thread cp.async ring in shared memory (unroll = depth), state requested up front
+    {128, 1, 8, 8, kPlain128},    // 8  half-size tiles: 128 threads, 512 fp32 parameters per CTA, 8 CTAs/SM
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 constexpr int kRingStages = kVariants[4].unroll;
@@ -674,7 +675,8 @@ KernelFn pick_kernel(int v, int dtype, int opt, int ema) {
     case 3: return pick_dtype<3>(dtype, opt, ema);
     case 4: return pick_dtype<4>(dtype, opt, ema);
     case 5: return pick_dtype<5>(dtype, opt, ema);
-    default: return pick_dtype<6>(dtype, opt, ema);
+    case 6: return pick_dtype<6>(dtype, opt, ema);
+    default: return pick_dtype<7>(dtype, opt, ema);
   }
 }
 

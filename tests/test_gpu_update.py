@@ -33,7 +33,7 @@ def test_every_template_instance_lockstep(dtype, opt, ema_mode):
     Pair(cfg).run(3, lockstep=True, rtol=RTOL_STEP, atol=ATOL_STEP)
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6, 7])   # 5: cp.async.bulk ring; 6: 256-bit loads; 7: per-thread cp.async ring
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6, 7, 8])   # 5: cp.async.bulk ring; 6: 256-bit loads; 7: per-thread cp.async ring; 8: half-size tiles
 @pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
 def test_every_variant(variant, dtype):
     cfg = replace(BASE, grad_dtype=dtype, opt=synth.RMSPROP_MOM, N=21, b=2, P=200_001, name=f"variant{variant}")
@@ -152,10 +152,10 @@ def test_bitwise_invariance_shard_layout_launch_variant_and_rerun():
     ref = None
     P = cfg.P
     layouts = [None, [0, P], [0, 1, 2, 77_777, 77_777, P]]
-    # the seven launch variants differ in tile size (1024 ... 2048 parameters), load width (128 / 256 bit) and staging
+    # the eight launch variants differ in tile size (512 ... 2048 parameters), load width (128 / 256 bit) and staging
     # (registers / cp.async.bulk ring): the fixed-order fp32 sum must give the same bits in all of them.  (grid_ctas
     # is accepted and ignored by this kernel, so it is not a dimension here.)
-    runs = [(lay, 0, 0) for lay in layouts] + [(None, 0, v) for v in range(1, 8)]
+    runs = [(lay, 0, 0) for lay in layouts] + [(None, 0, v) for v in range(1, 9)]
     runs.append((None, 0, 0))   # the same launch again
     for lay, grid, variant in runs:
         pair = Pair(cfg, shard_off=lay, grid_ctas=grid, variant=variant)
