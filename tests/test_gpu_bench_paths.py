@@ -1,0 +1,46 @@
+"""The side paths of bench.py that profiles/ and DESIGN.md cite must keep running on a GPU box: each is started as the user
+would start it (a subprocess) on a small configuration and its one JSON line is checked for shape, not for speed."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def run_bench(*flags, timeout=600):
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), *flags], capture_output=True, text=True,
+                         timeout=timeout, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    return json.loads(out.stdout.strip().splitlines()[-1])
+
+
+def test_probe_pipes_reports_three_pipe_rates():
+    d = run_bench("--probe-pipes")
+    rates = {k: v["per_clock_per_sm"] for k, v in d["pipes"].items()}
+    assert set(rates) == {"ffma", "ffma2_packed", "mufu_rsqrt"}
+    assert 30 < rates["ffma"] <= 130 and 30 < rates["ffma2_packed"] <= 260 and 4 < rates["mufu_rsqrt"] <= 33
+
+
+def test_launch_bound_reports_eager_and_graph_costs_for_both_algorithms():
+    d = run_bench("--launch-bound")
+    for key, eager, graph in (("sync", "step_device_eager", "step_device_graph"),
+                              ("sync_per_server", "step_device_eager", "step_device_graph"),
+                              ("async", "async_step_device_eager", "async_step_device_graph"),
+                              ("async_per_server", "async_step_device_eager", "async_step_device_graph")):
+        assert 0 < d[key][graph] < d[key][eager] < 1000
+
+
+@pytest.mark.parametrize("flags", [("--mode", "async"), ("--mode", "async_per_server", "--layout", "slices"),
+                                   ("--mode", "per_server", "--layout", "slices"), ("--variant", "7"), ("--variant", "8")])
+def test_small_config_through_every_mode_line_has_the_contract_keys(flags):
+    d = run_bench("--config", "cfg2", "--steps", "3", "--warmup", "3", "--no-cpu-baseline", "--no-e2e", "--no-probe",
+                  "--no-also", *flags)
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "dtype", "data", "config", "roofline", "clocks", "gpu_launches"):
+        assert key in d, key
+    assert d["roofline"]["bound"] == "hbm" and 0.3 < d["roofline"]["frac_of_nominal_8TBps"] < 1.0
+    assert d["gpu_launches"] > 0 and d["value"] > 0
