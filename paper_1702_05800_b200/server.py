@@ -48,6 +48,8 @@ class ParameterServerStep:
         self._retired = deque(maxlen=4)
         self._step = None
         self._keep = None
+        self.d_kept_timeout = None
+        self._tstep = None
 
     def set_gradients(self, buffers: Sequence[torch.Tensor]) -> None:
         if len(buffers) != self.W:
@@ -103,6 +105,35 @@ class ParameterServerStep:
         if self._step is None or self._step.gamma_t != np.float32(gamma_t):
             self._build(gamma_t)
         B.psync_aggregate_update(self._step, stream)
+
+    def step_timeout(self, d_arrival: torch.Tensor, timeout: float, gamma_t: float, min_keep: int = 1,
+                     d_step_tag: Optional[torch.Tensor] = None, t: int = 0, stream=None) -> None:
+        """The time-out rule instead of backup workers: keep every eligible worker that arrived within
+        `timeout` seconds, divide by the number kept (per server with per_server=True).  Kept rows land in
+        self.d_kept_timeout [rows][W] (first self.d_n_kept[r] entries), status in self.d_status."""
+        if self.table is None:
+            raise RuntimeError("set_gradients() first")
+        rows = self.M if self.per_server else 1
+        if getattr(self, "d_kept_timeout", None) is None:
+            dev = self.theta.device
+            self.d_kept_timeout = torch.full((rows, self.W), -1, dtype=torch.int32, device=dev)
+            self.d_n_kept = torch.zeros(rows, dtype=torch.int32, device=dev)
+            self._tstep = None
+        if self._tstep is None or self._tstep[0].gamma_t != np.float32(gamma_t) or self._tstep[2] is not self.table:
+            sharded = self.per_server or self.layout == B.PSYNC_GRADS_SLICES
+            st, keep = B.make_step(
+                self.shard_off, 1, self.W, self.table.grad_dtype, self.theta, self.ema, self.state0, self.state1,
+                opt=self.opt, ema_mode=self.ema_mode, gamma_t=gamma_t, alpha=self.alpha, mu=self.mu, rho=self.rho,
+                eps=self.eps, d_grads=self.table.d_ptrs, d_kept=self.d_kept_timeout, d_status=self.d_status,
+                per_shard=self.per_server, kept_stride=self.W, d_shard_off=self.d_shard_off if sharded else None,
+                d_n_kept=self.d_n_kept, grad_layout=self.layout,
+                d_tile_start=self._tiles(self.table.grad_dtype) if sharded else None)
+            self._tstep = (st, keep, self.table)
+        if stream is not None and hasattr(stream, "cuda_stream"):
+            self.table.d_ptrs.record_stream(stream)
+        B.psync_select_timeout(d_arrival, self.W, timeout, self.d_kept_timeout, self.d_n_kept, self.d_status, rows=rows,
+                               min_keep=min_keep, d_step_tag=d_step_tag, t=t, stream=stream)
+        B.psync_aggregate_update(self._tstep[0], stream)
 
 
 class AsyncServerStep:

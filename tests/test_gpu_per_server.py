@@ -426,3 +426,45 @@ def test_flat_rows_kernel_status_null_zero_count_and_garbage_count_are_failed_ro
     pair.oracle_rows(grads, kept, True, n_kept=n_kept, status=status)
     pair.compare_and_sync("rows kernel, status NULL")
     assert bool(torch.isfinite(pair.theta).all())
+
+
+@pytest.mark.parametrize("per_server,slices", [(False, False), (True, False), (True, True)])
+def test_parameter_server_step_timeout_rule(per_server, slices):
+    """ParameterServerStep.step_timeout: the time-out rule (L259) through the plumbing object -- flat buffers or slices, one
+    kept set or one per server -- against the oracle over three chained steps with different time-outs."""
+    cfg = per_server_cfg(N=1, b=22, P=60_007, opt=synth.MOMENTUM, name=f"ps_timeout_{int(per_server)}{int(slices)}")
+    off = synth.shard_offsets(cfg)
+    M, W = off.size - 1, cfg.W
+    theta = synth.init_theta(cfg, DEV)
+    s0, _ = synth.init_state(cfg, DEV)
+    ema = theta.clone()
+    ps = psync.ParameterServerStep(off, cfg.N, cfg.b, theta, ema, s0, None, cfg.opt, cfg.ema_mode, alpha=cfg.alpha, mu=cfg.mu,
+                                   per_server=per_server)
+    host = {"theta": to_np(theta), "ema": to_np(ema), "state0": to_np(s0)}
+    rows = M if per_server else 1
+    for s, timeout in enumerate((1.0, 1.3, 0.8)):
+        a = synth.arrival_times_per_server(cfg, s, server_sigma=0.3)[:rows].copy()
+        grads = [synth.gradient(cfg, s, k, DEV) for k in range(W)]
+        if slices:
+            sl = [[g[int(off[j]):int(off[j + 1])].clone() for j in range(M)] for g in grads]
+            ps.set_gradient_slices(sl)
+        else:
+            ps.set_gradients(grads)
+        ps.step_timeout(torch.from_numpy(a if per_server else a[0]).to(DEV), timeout, cfg.gamma)
+        torch.cuda.synchronize()
+        kept = np.full((rows, W), -1, np.int32)
+        n_kept = np.ones(rows, np.int32)
+        status = np.zeros(rows, np.int32)
+        for r in range(rows):
+            status[r], k = oracle.select_timeout(a[r], timeout)
+            if status[r] == oracle.OK:
+                kept[r, :k.size], n_kept[r] = k, k.size
+        assert np.array_equal(ps.d_status.cpu().numpy(), status)
+        np_grads = [synth.as_numpy_grad(g) for g in grads]
+        rc = oracle.aggregate_update_rows(off, cfg.N, np_grads, kept, host["theta"], host["ema"], host["state0"], None,
+                                          per_shard=per_server, n_kept=n_kept, status=status, opt=cfg.opt,
+                                          ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu)
+        assert rc == oracle.OK
+        for n, t in (("theta", theta), ("ema", ema), ("state0", s0)):
+            assert_close(to_np(t), host[n], RTOL_STEP, ATOL_STEP, f"ps timeout step {s} {n}")
+            host[n] = to_np(t)
