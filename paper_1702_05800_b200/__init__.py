@@ -10,7 +10,8 @@ from .binding import (  # noqa: F401
     HostCtx, PSYNC_BF16, PSYNC_ECUDA, PSYNC_EINVAL, PSYNC_EMA_OFF, PSYNC_EMA_POST, PSYNC_EMA_PRE, PSYNC_ETOOFEW,
     PSYNC_EUNSUPPORTED, PSYNC_F32, PSYNC_GRADS_FLAT, PSYNC_GRADS_SLICES, PSYNC_MOMENTUM, PSYNC_OK,
     PSYNC_RMSPROP_MOM, PSYNC_SGD, PsyncError, make_grad_table, make_slice_table, make_step,
-    psync_aggregate_update, psync_async_apply, psync_async_step_device, psync_async_step_host, psync_clip_scales, psync_clip_scales_slices,
+    psync_aggregate_update, psync_async_apply, psync_async_step_device, psync_async_step_host, psync_clip_scales, psync_clip_scales_slices, psync_clip_scales_static,
+    PSYNC_CLIP_STATIC_SCRATCH_BYTES,
     psync_clip_slices_workspace_bytes, psync_clip_workspace_bytes, psync_ema, psync_interp_iterations,
     psync_kth_arrival_stats, psync_launch_geometry, psync_lr_schedule, psync_order_by_arrival,
     psync_order_by_arrival_sharded, psync_select_first_n, psync_select_first_n_sharded, psync_select_timeout,

@@ -27,7 +27,7 @@ PSYNC_TILE_UNITS = 256
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
            "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_order_by_arrival_sharded", "psync_clip_slices_workspace_bytes", "psync_clip_scales_slices", "psync_async_apply", "psync_async_step_device", "psync_staleness", "psync_staleness_sharded", "psync_step_device", "psync_clip_workspace_bytes",
-           "psync_clip_scales", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
+           "psync_clip_scales", "psync_clip_scales_static", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_host_ctx_create", "psync_host_ctx_destroy",
            "psync_step_host_ctx", "psync_async_step_host", "psync_launch_geometry", "psync_probe_read",
            "psync_probe_copy", "psync_probe_pipe", "psync_selftest_rsqrt")
@@ -96,6 +96,8 @@ def lib() -> ctypes.CDLL:
         L.psync_clip_workspace_bytes.restype = ctypes.c_size_t
         L.psync_clip_scales.argtypes = [vp, i32, i64, i32, f32, vp, vp, ctypes.c_size_t, vp]
         L.psync_clip_scales.restype = ctypes.c_int
+        L.psync_clip_scales_static.argtypes = [vp, i32, i64, i32, f32, vp, vp]
+        L.psync_clip_scales_static.restype = ctypes.c_int
         L.psync_clip_slices_workspace_bytes.argtypes = [i32, i32, vp, i32]
         L.psync_clip_slices_workspace_bytes.restype = ctypes.c_size_t
         L.psync_clip_scales_slices.argtypes = [vp, i32, i32, vp, vp, i32, f32, vp, vp, ctypes.c_size_t, vp]
@@ -399,6 +401,26 @@ def psync_clip_scales(table: "GradTable", clip: float, d_scales: torch.Tensor, d
                                  _stream(stream))
     if check and st != PSYNC_OK:
         raise PsyncError(st, "psync_clip_scales")
+    return st
+
+
+PSYNC_CLIP_STATIC_SCRATCH_BYTES = 2 << 20
+
+
+def psync_clip_scales_static(table: "GradTable", clip: float, d_scales: torch.Tensor, stream=None, check: bool = True) -> int:
+    """psync_clip_scales without a workspace argument, for callers that cannot allocate device memory (code running
+    under a framework that owns the whole device through its caching allocator, or that must avoid cudaMalloc's
+    device-wide synchronisation mid-step).  The partial sums go to a fixed 2 MiB array inside libpsync.so, so the request
+    must satisfy psync_clip_workspace_bytes(W, P, dtype) <= PSYNC_CLIP_STATIC_SCRATCH_BYTES (else PSYNC_EUNSUPPORTED) and
+    calls that may overlap on the GPU (different streams) race on that array; calls on one stream are safe.  The first
+    call per device looks the array's address up -- make it before any stream capture.  include/psync.h has the contract."""
+    if d_scales.numel() < table.W:
+        raise ValueError("d_scales needs W elements")
+    st = lib().psync_clip_scales_static(_dptr(table.d_ptrs, torch.int64, "d_grads"), table.W, table.buffers[0].numel(),
+                                        table.grad_dtype, clip, _dptr(d_scales, torch.float32, "d_scales"),
+                                        _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_clip_scales_static")
     return st
 
 

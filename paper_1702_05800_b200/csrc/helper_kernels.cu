@@ -513,3 +513,80 @@ cudaError_t launch_staleness(int64_t* d_read_iter, int32_t W, int32_t rows, cons
 }
 
 }  // namespace psync
+
+// ---- K5n: psync_clip_scales_static -- K5 for callers that must not allocate device memory ----------------------------
+// Some users of this library are not allowed to call cudaMalloc where the clip factors are needed: code that runs
+// inside a framework's allocator-owned region (every byte of the device already handed to a caching pool, so a raw
+// cudaMalloc fails or fragments it), a plugin that is given buffers and a stream and nothing else, or a latency-critical
+// loop in which cudaMalloc's implicit device synchronisation is unacceptable.  K5 needs scratch memory for its per-chunk
+// partial sums (double [W][chunks]); the ordinary entry point makes the caller bring it (d_work).  This variant keeps that
+// scratch inside the library image instead: one fixed array in device global memory, reserved on every GPU that loads
+// libpsync.so from the moment the module is loaded until the process exits (kClipStaticBytes = 2 MiB per GPU).
+//
+// What follows from that, and what the header repeats for the caller:
+//  * the problem must fit: W * chunks <= kClipStaticPartials (chunks = ceil(P*sizeof(grad) / 128 KiB), at least 1);
+//    larger requests are refused (PSYNC_EUNSUPPORTED), never truncated;
+//  * every call on a device uses the SAME array.  Two calls whose kernels can be on the GPU at the same time (different
+//    streams, or different host threads on different streams) overwrite each other's partial sums.  Calls on one stream
+//    are ordered by the stream and are safe;
+//  * the array keeps whatever the previous call left in it.  Nothing has to be cleared: sumsq_chunks_kernel stores
+//    (does not accumulate into) every one of the W * chunks slots that clip_finalize_kernel reads, in every call;
+//  * inside host code the name g_clip_static_scratch is only a handle for the runtime, not a device address.  The
+//    address a kernel can use is looked up once per device with cudaGetSymbolAddress while that device is current and
+//    remembered; that look-up (which may also load the module onto the device) happens in the first call made on each
+//    device, so make that first call outside any stream capture.
+namespace psync {
+namespace {
+
+constexpr size_t kClipStaticBytes = size_t{2} << 20;                      // == PSYNC_CLIP_STATIC_SCRATCH_BYTES
+constexpr size_t kClipStaticPartials = kClipStaticBytes / sizeof(double);  // 262,144 partial sums
+static __device__ __align__(256) double g_clip_static_scratch[kClipStaticPartials];
+
+constexpr int kClipStaticMaxDevices = 64;
+double* g_clip_static_addr[kClipStaticMaxDevices] = {};  // device address of the array on device i, once looked up
+
+// Device address of the scratch array on the CURRENT device (nullptr + *err on failure).  Host threads may race here:
+// they all obtain the same address for the same device, and an aligned pointer store is atomic on the hosts CUDA runs on.
+double* clip_static_scratch(cudaError_t* err) {
+  int dev = -1;
+  *err = cudaGetDevice(&dev);
+  if (*err != cudaSuccess) return nullptr;
+  const bool cached = dev >= 0 && dev < kClipStaticMaxDevices;
+  if (cached) {
+    double* p = __atomic_load_n(&g_clip_static_addr[dev], __ATOMIC_ACQUIRE);
+    if (p != nullptr) return p;
+  }
+  double* p = nullptr;
+  *err = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_clip_static_scratch);
+  if (*err != cudaSuccess || p == nullptr) {
+    if (*err == cudaSuccess) *err = cudaErrorInvalidSymbol;
+    return nullptr;
+  }
+  if (cached) __atomic_store_n(&g_clip_static_addr[dev], p, __ATOMIC_RELEASE);
+  return p;
+}
+
+}  // namespace
+}  // namespace psync
+
+#include "../../include/psync.h"
+
+static_assert(PSYNC_CLIP_STATIC_SCRATCH_BYTES == psync::kClipStaticBytes, "psync.h and the scratch array disagree");
+
+// The C entry point lives in this file because the scratch array has file scope (see psync.h for the contract).
+// It calls no cudaMalloc / cudaFree and nothing that allocates: one cudaGetDevice, on the first call per device one
+// cudaGetSymbolAddress, then the two launches of K5.
+extern "C" PSYNC_API int psync_clip_scales_static(const void* const* d_grads, int32_t W, int64_t P, int32_t grad_dtype,
+                                                  float clip, float* d_scales, void* stream) {
+  if (d_grads == nullptr || d_scales == nullptr) return PSYNC_EINVAL;
+  if (W < 1 || W > PSYNC_MAX_WORKERS || P < 0 || !(clip > 0.0f)) return PSYNC_EINVAL;
+  if (grad_dtype != PSYNC_F32 && grad_dtype != PSYNC_BF16) return PSYNC_EINVAL;
+  if (psync::clip_workspace_bytes(W, P, grad_dtype) > psync::kClipStaticBytes) return PSYNC_EUNSUPPORTED;  // does not fit
+  cudaError_t err = cudaSuccess;
+  double* scratch = psync::clip_static_scratch(&err);
+  if (scratch == nullptr) return PSYNC_ECUDA;
+  return psync::launch_clip_scales(d_grads, W, P, grad_dtype, clip, d_scales, scratch, static_cast<cudaStream_t>(stream)) ==
+                 cudaSuccess
+             ? PSYNC_OK
+             : PSYNC_ECUDA;
+}
