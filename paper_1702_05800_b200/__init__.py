@@ -13,7 +13,7 @@ from .binding import (  # noqa: F401
     psync_aggregate_update, psync_async_apply, psync_async_step_device, psync_async_step_host, psync_clip_scales, psync_clip_scales_slices, psync_clip_scales_static,
     PSYNC_CLIP_STATIC_SCRATCH_BYTES,
     psync_clip_slices_workspace_bytes, psync_clip_workspace_bytes, psync_ema, psync_interp_iterations,
-    psync_kth_arrival_stats, psync_launch_geometry, psync_lr_schedule, psync_order_by_arrival,
+    psync_kth_arrival_stats, psync_launch_geometry, psync_lr_schedule, psync_lr_schedule_counted, psync_order_by_arrival,
     psync_order_by_arrival_sharded, psync_select_first_n, psync_select_first_n_sharded, psync_select_timeout,
     psync_shard_worklist, psync_staleness, psync_staleness_sharded, psync_step_device, psync_step_host,
     psync_step_host_workspace_bytes)

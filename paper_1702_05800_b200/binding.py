@@ -108,6 +108,8 @@ def lib() -> ctypes.CDLL:
         L.psync_interp_iterations.restype = ctypes.c_int
         L.psync_lr_schedule.argtypes = [f32, f32, i64, i32, ctypes.c_double, vp, vp]
         L.psync_lr_schedule.restype = ctypes.c_int
+        L.psync_lr_schedule_counted.argtypes = [f32, f32, vp, i64, vp, i32, i32, ctypes.c_double, vp, vp]
+        L.psync_lr_schedule_counted.restype = ctypes.c_int
         L.psync_async_apply.restype = ctypes.c_int
         L.psync_ema.argtypes = [vp, vp, i64, f32, vp]
         L.psync_ema.restype = ctypes.c_int
@@ -493,6 +495,21 @@ def psync_lr_schedule(gamma0: float, beta: float, t0: int, K: int, s: float, d_g
     st = lib().psync_lr_schedule(gamma0, beta, t0, K, s, _dptr(d_gamma, torch.float32, "d_gamma"), _stream(stream))
     if check and st != PSYNC_OK:
         raise PsyncError(st, "psync_lr_schedule")
+    return st
+
+
+def psync_lr_schedule_counted(gamma0: float, beta: float, d_t: torch.Tensor, K: int, s: float, d_gamma: torch.Tensor,
+                              d_n_add: Optional[torch.Tensor] = None, t_set: int = -1, stream=None, check: bool = True) -> int:
+    """The schedule from a device iteration counter: d_t <- t_set if t_set >= 0 else d_t + max(d_n_add); then
+    d_gamma[i] = gamma_0 beta^((d_t+i) s), i < K (include/psync.h: psync_lr_schedule_counted)."""
+    if d_gamma.numel() < K or d_t.numel() < 1:
+        raise ValueError("d_gamma needs K elements and d_t one")
+    st = lib().psync_lr_schedule_counted(gamma0, beta, _dptr(d_t, torch.int64, "d_t"), t_set,
+                                         _dptr(d_n_add, torch.int32, "d_n_add") if d_n_add is not None else None,
+                                         d_n_add.numel() if d_n_add is not None else 0, K, s,
+                                         _dptr(d_gamma, torch.float32, "d_gamma"), _stream(stream))
+    if check and st != PSYNC_OK:
+        raise PsyncError(st, "psync_lr_schedule_counted")
     return st
 
 

@@ -170,6 +170,33 @@ __global__ void lr_schedule_kernel(float gamma0, float beta, int64_t t0, int32_t
                                 pow(static_cast<double>(beta), static_cast<double>(t0 + i) * s));
 }
 
+// K6c -- the same table when the iteration count t lives on the DEVICE (Alg. 2's t, L84, advances by the number of
+// gradients that actually arrived, which only the device knows without a host sync).  One CTA: t0 = t_set >= 0 ? t_set :
+// *t_counter + max_r n_add[r]  (rows = 1: the one order's count; rows = M: the largest count of any server -- every
+// worker gradient that reached a server is one iteration of the schedule); *t_counter <- t0; out[i] = gamma_{t0 + i}.
+__global__ void __launch_bounds__(1024) lr_schedule_counted_kernel(float gamma0, float beta, int64_t* t_counter,
+                                                                   int64_t t_set, const int32_t* n_add, int32_t rows,
+                                                                   int32_t K, double s, float* out) {
+  __shared__ int s_max;
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  if (threadIdx.x == 0) s_max = 0;
+  __syncthreads();
+  if (t_set < 0 && n_add != nullptr) {
+    int m = 0;
+    for (int r = threadIdx.x; r < rows; r += blockDim.x) m = max(m, n_add[r]);
+    if (m > 0) atomicMax(&s_max, m);
+  }
+  const int64_t before = *t_counter;
+  __syncthreads();  // every thread has read the counter before thread 0 replaces it
+  const int64_t t0 = t_set >= 0 ? t_set : before + s_max;
+  if (threadIdx.x == 0) *t_counter = t0;
+  const int i = threadIdx.x;
+  if (i < K)
+    out[i] = static_cast<float>(static_cast<double>(gamma0) *
+                                pow(static_cast<double>(beta), static_cast<double>(t0 + i) * s));
+}
+
 // ---- K7: straggler statistics, the procedure of section 3.1 -----------------------------
 __device__ __forceinline__ uint32_t time_key(float a) {  // order-preserving; 0xFFFFFFFF = never arrived
   uint32_t u = __float_as_uint(a);
@@ -494,6 +521,14 @@ cudaError_t launch_lr_schedule(float gamma0, float beta, int64_t t0, int32_t K, 
   cudaLaunchAttribute attr[1];
   pdl_config(&cfg, attr, dim3(static_cast<unsigned>((K + 127) / 128)), dim3(128), stream);
   return cudaLaunchKernelEx(&cfg, lr_schedule_kernel, gamma0, beta, t0, K, s, d_gamma);
+}
+
+cudaError_t launch_lr_schedule_counted(float gamma0, float beta, int64_t* d_t, int64_t t_set, const int32_t* d_n_add,
+                                       int32_t rows, int32_t K, double s, float* d_gamma, cudaStream_t stream) {
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute attr[1];
+  pdl_config(&cfg, attr, dim3(1), dim3(1024), stream);
+  return cudaLaunchKernelEx(&cfg, lr_schedule_counted_kernel, gamma0, beta, d_t, t_set, d_n_add, rows, K, s, d_gamma);
 }
 
 cudaError_t launch_staleness(int64_t* d_read_iter, int32_t W, int32_t rows, const int32_t* d_order,

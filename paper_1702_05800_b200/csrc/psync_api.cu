@@ -427,6 +427,16 @@ PSYNC_API int psync_lr_schedule(float gamma0, float beta, int64_t t0, int32_t K,
              : PSYNC_ECUDA;
 }
 
+PSYNC_API int psync_lr_schedule_counted(float gamma0, float beta, int64_t* d_t, int64_t t_set, const int32_t* d_n_add,
+                                        int32_t rows, int32_t K, double s, float* d_gamma, void* stream) {
+  if (d_t == nullptr || K < 0 || K > PSYNC_MAX_WORKERS || !(beta > 0.0f) || (K > 0 && d_gamma == nullptr)) return PSYNC_EINVAL;
+  if (t_set < 0 && d_n_add != nullptr && rows < 1) return PSYNC_EINVAL;
+  return psync::launch_lr_schedule_counted(gamma0, beta, d_t, t_set, d_n_add, rows, K, s, d_gamma,
+                                           static_cast<cudaStream_t>(stream)) == cudaSuccess
+             ? PSYNC_OK
+             : PSYNC_ECUDA;
+}
+
 PSYNC_API int psync_ema(float* d_ema, const float* d_theta, int64_t P, float alpha, void* stream) {
   if (d_ema == nullptr || d_theta == nullptr || P < 0) return PSYNC_EINVAL;
   if (P == 0) return PSYNC_OK;

@@ -163,7 +163,9 @@ class AsyncServerStep:
         self.d_gamma = torch.zeros(W, dtype=torch.float32, device=dev) if lr is not None else None
         self.d_gscale = torch.ones(W, dtype=torch.float32, device=dev) if clip > 0 else None
         self._d_clip_work = None
-        self.t0 = 0                       # iterations scheduled so far (host counter: W per batch unless given)
+        # iterations applied so far, for the schedule (L315): a DEVICE counter, advanced before each batch by the number
+        # of gradients the previous batch really applied (d_n_arrived), so a partial batch does not run the schedule ahead
+        self.d_t_sched = torch.zeros(1, dtype=torch.int64, device=dev)
         self.track_staleness = bool(track_staleness)
         if track_staleness:               # one row per server with per_server=True: every server counts its own updates
             self.d_read_iter = torch.zeros((rows, W), dtype=torch.int64, device=dev)
@@ -209,7 +211,8 @@ class AsyncServerStep:
         return self._step
 
     def apply(self, d_arrival: torch.Tensor, gamma_t: float = 0.0, t0: Optional[int] = None, stream=None) -> None:
-        """One batch: every gradient whose arrival time is finite is one iteration, in arrival order (L85-87)."""
+        """One batch: every gradient whose arrival time is finite is one iteration, in arrival order (L85-87).
+        t0 (optional) restarts the schedule's iteration counter at that value for this batch."""
         if self.table is None:
             raise RuntimeError("set_gradients() first")
         if self._step is None or self._step.gamma_t != np.float32(gamma_t):
@@ -230,9 +233,9 @@ class AsyncServerStep:
                 B.psync_clip_scales(self.table, self.clip, self.d_gscale, self._d_clip_work[1], stream)
         if self.lr is not None:
             gamma0, beta, s = self.lr
-            B.psync_lr_schedule(gamma0, beta, self.t0 if t0 is None else t0, self.W, s, self.d_gamma, stream)
+            B.psync_lr_schedule_counted(gamma0, beta, self.d_t_sched, self.W, s, self.d_gamma, d_n_add=self.d_n_arrived,
+                                        t_set=-1 if t0 is None else int(t0), stream=stream)   # before this batch's order
         B.psync_async_step_device(self._step, d_arrival, self.d_gamma, stream, d_gscale=self.d_gscale)   # order + K iterations
         if self.track_staleness:
             B.psync_staleness_sharded(self.d_read_iter, self.d_order, self.d_t, self.d_staleness, self.d_stale_stats,
                                       self.d_stale_status, d_n_arrived=self.d_n_arrived, lag=self.lag, stream=stream)
-        self.t0 = (self.t0 if t0 is None else t0) + self.W

@@ -399,6 +399,48 @@ def test_async_server_step_flat_with_clipping_schedule_and_staleness_chained_bat
         assert np.array_equal(srv.d_stale_stats.cpu().numpy()[0], stats)
 
 
+def test_async_server_step_schedule_follows_the_applied_count_over_partial_batches():
+    """L84-87: every received gradient is one iteration, so after a batch of K < W arrivals the schedule (L315) advances
+    by K, not W.  Three batches, the middle one partial (and the first too), no t0 given: the rates of batch s must be
+    gamma_{t + i} with t = the sum of the K of the batches before it -- the device counter, no host synchronisation."""
+    cfg = replace(BASE, P=9_001, M=3, opt=synth.SGD, name="aserver_partial")
+    off = synth.shard_offsets(cfg)
+    theta = synth.init_theta(cfg, DEV)
+    ema = theta.clone()
+    lr = (0.045, 0.94, 1.0 / 7.0)                           # a steep schedule: an off-by-(W-K) start is far outside 1 ulp
+    srv = psync.AsyncServerStep(off, cfg.W, theta, ema, None, None, cfg.opt, cfg.ema_mode, alpha=cfg.alpha, lr=lr)
+    h = {"theta": to_np(theta), "ema": to_np(ema)}
+    applied = 0
+    missing = [(1,), (0, 3, 4), ()]
+    for s in range(3):
+        grads = [synth.gradient(cfg, s, k, DEV) for k in range(cfg.W)]
+        a = synth.arrival_times(cfg, s)
+        a[list(missing[s])] = np.inf
+        srv.set_gradients(grads)
+        srv.apply(torch.from_numpy(a).to(DEV))              # no synchronisation between the calls of a batch
+        torch.cuda.synchronize()
+        order = oracle.order_by_arrival(a)
+        K = order.size
+        assert K == cfg.W - len(missing[s])
+        gammas = oracle.lr_schedule(lr[0], lr[1], applied, cfg.W, lr[2])
+        assert np.array_equal(srv.d_gamma.cpu().numpy(), gammas), f"batch {s}: schedule does not start at t = {applied}"
+        assert int(srv.d_t_sched.item()) == applied
+        if 0 < applied < s * cfg.W:
+            assert not np.array_equal(gammas, oracle.lr_schedule(lr[0], lr[1], s * cfg.W, cfg.W, lr[2]))
+        rc = oracle.async_apply(off, [synth.as_numpy_grad(g) for g in grads], order, h["theta"], h["ema"], None, None,
+                                gammas=gammas[:K].copy(), opt=cfg.opt, ema_mode=cfg.ema_mode, alpha=cfg.alpha)
+        assert rc == oracle.OK
+        for n, t in (("theta", theta), ("ema", ema)):
+            assert_close(to_np(t), h[n], rtol_async(K), ATOL_STEP, f"aserver partial batch {s} {n}")
+            h[n] = to_np(t)
+        applied += K
+    srv.set_gradients(grads)
+    srv.apply(torch.from_numpy(a).to(DEV), t0=5)            # an explicit t0 restarts the count
+    torch.cuda.synchronize()
+    assert np.array_equal(srv.d_gamma.cpu().numpy(), oracle.lr_schedule(lr[0], lr[1], 5, cfg.W, lr[2]))
+    assert int(srv.d_t_sched.item()) == 5
+
+
 def test_async_server_step_per_server_on_slices_chained_batches():
     cfg = replace(BASE, opt=synth.MOMENTUM, grad_dtype=synth.BF16, name="aserver_rows")
     off = np.asarray(RAGGED, dtype=np.int64)

@@ -39,6 +39,33 @@ def test_lr_schedule_matches_oracle(gamma0, beta, t0, K, s):
     assert L.psync_lr_schedule(0.1, 0.5, 0, 1, 1.0, None, None) == psync.PSYNC_EINVAL
 
 
+def test_lr_schedule_counted_advances_by_the_largest_count_and_restarts():
+    """psync_lr_schedule_counted: *d_t <- t_set or *d_t + max_r d_n_add[r], then the same bits as psync_lr_schedule."""
+    gamma0, beta, s, K = 0.045, 0.94, 1.0 / 11.0, 37
+    d_t = torch.tensor([100], dtype=torch.int64, device=DEV)
+    d_n = torch.tensor([5, 31, 0, 17], dtype=torch.int32, device=DEV)
+    d = torch.zeros(K, dtype=torch.float32, device=DEV)
+    psync.psync_lr_schedule_counted(gamma0, beta, d_t, K, s, d, d_n_add=d_n)
+    assert int(d_t.item()) == 131 and np.array_equal(d.cpu().numpy(), oracle.lr_schedule(gamma0, beta, 131, K, s))
+    psync.psync_lr_schedule_counted(gamma0, beta, d_t, K, s, d, d_n_add=d_n[:1])
+    assert int(d_t.item()) == 136 and np.array_equal(d.cpu().numpy(), oracle.lr_schedule(gamma0, beta, 136, K, s))
+    psync.psync_lr_schedule_counted(gamma0, beta, d_t, K, s, d)                         # no counts: the counter stays
+    assert int(d_t.item()) == 136
+    psync.psync_lr_schedule_counted(gamma0, beta, d_t, K, s, d, d_n_add=d_n, t_set=7)   # restart: counts ignored
+    assert int(d_t.item()) == 7 and np.array_equal(d.cpu().numpy(), oracle.lr_schedule(gamma0, beta, 7, K, s))
+    big = torch.arange(5000, dtype=torch.int32, device=DEV) % 1000                      # more rows than threads
+    psync.psync_lr_schedule_counted(gamma0, beta, d_t, 1, s, d, d_n_add=big)
+    assert int(d_t.item()) == 7 + 999
+    ref = torch.zeros(K, dtype=torch.float32, device=DEV)
+    psync.psync_lr_schedule(gamma0, beta, 7 + 999, 1, s, ref)
+    assert d[0].item() == ref[0].item()
+    L = psync.binding.lib()
+    assert L.psync_lr_schedule_counted(0.1, 0.5, None, -1, None, 0, 1, 1.0, d.data_ptr(), None) == psync.PSYNC_EINVAL
+    assert L.psync_lr_schedule_counted(0.1, 0.5, d_t.data_ptr(), -1, None, 0, 1025, 1.0, d.data_ptr(), None) == psync.PSYNC_EINVAL
+    assert L.psync_lr_schedule_counted(0.1, 0.0, d_t.data_ptr(), -1, None, 0, 1, 1.0, d.data_ptr(), None) == psync.PSYNC_EINVAL
+    assert L.psync_lr_schedule_counted(0.1, 0.5, d_t.data_ptr(), -1, d_n.data_ptr(), 0, 1, 1.0, d.data_ptr(), None) == psync.PSYNC_EINVAL
+
+
 def _clip_gpu(grads, clip):
     table = psync.make_grad_table(grads)
     nbytes = psync.psync_clip_workspace_bytes(table.W, grads[0].numel(), table.grad_dtype)
