@@ -27,7 +27,7 @@ PSYNC_TILE_UNITS = 256
 
 EXPORTS = ("psync_version", "psync_status_string", "psync_select_first_n", "psync_select_first_n_sharded",
            "psync_select_timeout", "psync_aggregate_update", "psync_shard_worklist", "psync_ema", "psync_order_by_arrival", "psync_order_by_arrival_sharded", "psync_clip_slices_workspace_bytes", "psync_clip_scales_slices", "psync_async_apply", "psync_async_step_device", "psync_staleness", "psync_staleness_sharded", "psync_step_device", "psync_clip_workspace_bytes",
-           "psync_clip_scales", "psync_clip_scales_static", "psync_lr_schedule", "psync_kth_arrival_stats", "psync_interp_iterations",
+           "psync_clip_scales", "psync_clip_scales_static", "psync_lr_schedule", "psync_lr_schedule_counted", "psync_kth_arrival_stats", "psync_interp_iterations",
            "psync_step_host_workspace_bytes", "psync_step_host", "psync_host_ctx_create", "psync_host_ctx_destroy",
            "psync_step_host_ctx", "psync_async_step_host", "psync_launch_geometry", "psync_probe_read",
            "psync_probe_copy", "psync_probe_pipe", "psync_selftest_rsqrt")
@@ -233,10 +233,27 @@ class GradTable:
     d_ptrs: torch.Tensor
     buffers: Sequence[torch.Tensor]
     grad_dtype: int
+    n_workers: Optional[int] = None       # set for slice tables, whose `buffers` holds W*M entries
+    _recorded: set = field(default_factory=set, repr=False)   # side streams the tensors were recorded on
+
+    def record_stream(self, stream) -> None:
+        """Tells torch's caching allocator that `stream` (a torch.cuda.Stream other than the one the tensors were
+        allocated on) reads the pointer table AND every gradient tensor, so none of those blocks is handed out again
+        before the work enqueued on `stream` so far has finished -- even if the caller drops its references.  Done
+        once per (table, stream); non-torch stream handles cannot be recorded and are the caller's to order."""
+        if stream is None or not hasattr(stream, "cuda_stream") or stream.cuda_stream in self._recorded:
+            return
+        self.d_ptrs.record_stream(stream)
+        seen = set()
+        for t in self.buffers:
+            if t is not None and t.untyped_storage().data_ptr() not in seen:     # views of one arena: once
+                seen.add(t.untyped_storage().data_ptr())
+                t.record_stream(stream)
+        self._recorded.add(stream.cuda_stream)
 
     @property
     def W(self) -> int:
-        return len(self.buffers)
+        return len(self.buffers) if self.n_workers is None else self.n_workers
 
 
 def make_grad_table(buffers: Sequence[torch.Tensor]) -> GradTable:
@@ -250,24 +267,36 @@ def make_grad_table(buffers: Sequence[torch.Tensor]) -> GradTable:
     return GradTable(ptrs, list(buffers), PSYNC_F32 if dt == torch.float32 else PSYNC_BF16)
 
 
-def make_slice_table(slices: Sequence[Sequence[Optional[torch.Tensor]]]) -> GradTable:
+def make_slice_table(slices: Sequence[Sequence[Optional[torch.Tensor]]], shard_off=None) -> GradTable:
     """Device pointer table [W*M] for PSYNC_GRADS_SLICES: slices[k][j] is worker k's G_k[j], its own CUDA tensor of
-    len_j elements (any element alignment; None -> a NULL entry, legal where server j does not keep worker k)."""
-    W, M = len(slices), len(slices[0])
-    first = next(t for row in slices for t in row if t is not None)
+    len_j elements (any element alignment; None -> a NULL entry, legal where server j does not keep worker k).
+    With shard_off (int64 [M+1]) every present slice is checked to hold exactly len_j = off[j+1] - off[j] elements: the
+    kernels read len_j elements through every kept pointer, so a short slice would be an out-of-bounds device read."""
+    W, M = len(slices), len(slices[0]) if len(slices) else 0
+    first = next((t for row in slices for t in row if t is not None), None)
+    if first is None:
+        raise ValueError("no gradient slice is present (every entry is None)")
     dt = first.dtype
     if dt not in (torch.float32, torch.bfloat16):
         raise TypeError("gradient slices must be float32 or bfloat16")
+    off = None
+    if shard_off is not None:
+        off = np.ascontiguousarray(shard_off, dtype=np.int64)
+        if off.size != M + 1:
+            raise ValueError(f"shard_off has {off.size - 1} servers, the slice rows have {M}")
     ptrs = []
-    for row in slices:
+    for k, row in enumerate(slices):
         if len(row) != M:
             raise ValueError("every worker needs M slices")
-        for t in row:
-            if t is not None and (t.dtype != dt or not t.is_cuda or not t.is_contiguous()):
-                raise ValueError("gradient slices must be contiguous CUDA tensors of one dtype")
+        for j, t in enumerate(row):
+            if t is not None and (t.dtype != dt or not t.is_cuda or not t.is_contiguous() or t.device != first.device):
+                raise ValueError("gradient slices must be contiguous CUDA tensors of one dtype on one device")
+            if t is not None and off is not None and t.numel() != int(off[j + 1] - off[j]):
+                raise ValueError(f"slice of worker {k} for server {j} has {t.numel()} elements, "
+                                 f"the shard table says {int(off[j + 1] - off[j])}")
             ptrs.append(0 if t is None else t.data_ptr())
     d_ptrs = torch.tensor(ptrs, dtype=torch.int64).to(first.device)
-    return GradTable(d_ptrs, [t for row in slices for t in row], PSYNC_F32 if dt == torch.float32 else PSYNC_BF16)
+    return GradTable(d_ptrs, [t for row in slices for t in row], PSYNC_F32 if dt == torch.float32 else PSYNC_BF16, W)
 
 
 def psync_shard_worklist(d_shard_off: torch.Tensor, grad_dtype: int, d_tile_start: Optional[torch.Tensor] = None,

@@ -66,7 +66,7 @@ class ParameterServerStep:
             raise ValueError(f"need W = {self.W} rows of M = {self.M} slices")
         if self.table is not None:
             self._retired.append((self.table, self._keep))
-        self.table = B.make_slice_table(slices)
+        self.table = B.make_slice_table(slices, self.shard_off)
         self.layout = B.PSYNC_GRADS_SLICES
         self._step = None
 
@@ -142,7 +142,8 @@ class AsyncServerStep:
     apply(d_arrival) enqueues, with no host synchronisation: the arrival order (per server with per_server=True,
     d_arrival [M][W]), optionally the global-norm clip factors (clip > 0: the norm is over the whole gradient of a
     worker, all of its slices, L313), optionally the learning rates of this batch's iterations (lr = (gamma0, beta, s):
-    gamma0 * beta^((t0 + i) s), L315), the one-pass application of the arrivals, and with track_staleness=True Table 1's
+    gamma0 * beta^((t + i) s), L315, with t = the number of gradients applied so far, counted on the device in
+    d_t_sched -- a batch in which K < W gradients arrived advances it by K; apply(t0=...) restarts it), the one-pass application of the arrivals, and with track_staleness=True Table 1's
     bookkeeping (per server with per_server=True).  Plumbing only, no arithmetic."""
 
     def __init__(self, shard_off, W: int, theta: torch.Tensor, ema: Optional[torch.Tensor],
@@ -195,7 +196,7 @@ class AsyncServerStep:
             raise ValueError("global-norm clipping needs every slice of every worker (the norm is over all of them)")
         if self.table is not None:
             self._retired.append((self.table, self._keep))
-        self.table, self.layout, self._step = B.make_slice_table(slices), B.PSYNC_GRADS_SLICES, None
+        self.table, self.layout, self._step = B.make_slice_table(slices, self.shard_off), B.PSYNC_GRADS_SLICES, None
 
     def _build(self, gamma_t: float):
         sharded = self.per_server or self.layout == B.PSYNC_GRADS_SLICES
@@ -217,8 +218,7 @@ class AsyncServerStep:
             raise RuntimeError("set_gradients() first")
         if self._step is None or self._step.gamma_t != np.float32(gamma_t):
             self._build(gamma_t)
-        if stream is not None and hasattr(stream, "cuda_stream"):
-            self.table.d_ptrs.record_stream(stream)
+        self.table.record_stream(stream)    # a side stream reads the pointer table and every gradient tensor
         if self.clip > 0:                 # norms and rates do not depend on the order: they are enqueued first
             sliced = self.layout == B.PSYNC_GRADS_SLICES
             key = (sliced, self.table.grad_dtype)

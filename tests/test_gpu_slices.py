@@ -568,3 +568,23 @@ def test_step_host_from_host_slices_matches_the_oracle(dtype, chunk):
     h_sl[int(kept[0])][3] = None
     st, _ = psync.psync_step_host(step, arrival, h_sl, d_work, chunk_elems=chunk, check=False)
     assert st == psync.PSYNC_EINVAL and np.array_equal(to_np(pair.theta), before)
+
+
+def test_slice_table_validates_lengths_presence_and_worker_count():
+    """The kernels read len_j elements through every kept slice pointer: the binding refuses a slice of another length
+    (a short one would be an out-of-bounds device read), a table with no slice at all, and reports W (not W*M)."""
+    off = np.array([0, 5, 5, 12], dtype=np.int64)
+    mk = lambda n: torch.zeros(n, dtype=torch.float32, device=DEV)
+    good = [[mk(5), None, mk(7)], [mk(5), mk(0), mk(7)]]
+    t = psync.make_slice_table(good, off)
+    assert t.W == 2 and t.d_ptrs.numel() == 6
+    assert psync.make_slice_table(good).W == 2                       # without a shard table: no length check
+    with pytest.raises(ValueError, match="worker 1 for server 2"):
+        psync.make_slice_table([[mk(5), None, mk(7)], [mk(5), None, mk(6)]], off)
+    with pytest.raises(ValueError, match="servers"):
+        psync.make_slice_table(good, off[:3])
+    with pytest.raises(ValueError, match="no gradient slice"):
+        psync.make_slice_table([[None, None, None]], off)
+    srv = psync.ParameterServerStep(off, 2, 0, mk(12), mk(12), None, None, psync.PSYNC_SGD, psync.PSYNC_EMA_POST, alpha=0.5)
+    with pytest.raises(ValueError, match="worker 0 for server 0"):
+        srv.set_gradient_slices([[mk(4), mk(0), mk(7)], [mk(5), mk(0), mk(7)]])
