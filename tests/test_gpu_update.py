@@ -338,6 +338,10 @@ def test_device_rsqrt_rn_equals_frsqrt_rn_exhaustively_and_the_mirror_on_a_sampl
     bad = torch.zeros(1, dtype=torch.int64, device=DEV)
     lo, hi = 0x21800000, 0x5D800000                      # 2^-60 ... 2^60: every bit pattern (1.0e9 inputs)
     B.psync_selftest_rsqrt(bad, hi - lo, first_bits=lo)
+    # the packed unchecked form (what Alg. 2's kernels run) is valid on the wider band [2^-63, 2^65): the kernel checks
+    # it against __frsqrt_rn wherever its range flag stays clear -- cover the two bands outside [2^-60, 2^60) entirely
+    B.psync_selftest_rsqrt(bad, lo - 0x20000000 + (1 << 15), first_bits=0x20000000 - (1 << 15))
+    B.psync_selftest_rsqrt(bad, 0x60000000 - hi + (1 << 15), first_bits=hi)
     B.psync_selftest_rsqrt(bad, 1 << 16, first_bits=lo - (1 << 15))          # across the lower edge
     B.psync_selftest_rsqrt(bad, 1 << 16, first_bits=hi - (1 << 15))          # across the upper edge
     B.psync_selftest_rsqrt(bad, 1 << 24, first_bits=0)                       # zero, denormals, tiny normals
