@@ -7,7 +7,7 @@ missing or a tensor is not on a CUDA device the call raises.  This module never 
 from __future__ import annotations
 
 import ctypes
-from dataclasses import dataclass
+from dataclasses import dataclass, field
 from pathlib import Path
 from typing import Optional, Sequence
 

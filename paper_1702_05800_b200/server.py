@@ -44,7 +44,8 @@ class ParameterServerStep:
         # A fused kernel in flight stages its pointers from the table it was launched with for its whole lifetime
         # (each CTA reads it at its own start).  Tables replaced by set_gradients() are therefore kept alive for a few
         # steps instead of going straight back to torch's caching allocator, and step() also records the launch stream
-        # on the table, so a step enqueued on a side stream can never see its table's block reused under it.
+        # on the table AND on every gradient tensor it points to (GradTable.record_stream), so a step enqueued on a
+        # side stream can never see a block reused under it, however many steps are in flight.
         self._retired = deque(maxlen=4)
         self._step = None
         self._keep = None
@@ -97,8 +98,7 @@ class ParameterServerStep:
             raise RuntimeError("set_gradients() first")
         if self._step is None or self._step.gamma_t != np.float32(gamma_t):
             self._build(gamma_t)
-        if stream is not None and hasattr(stream, "cuda_stream"):
-            self.table.d_ptrs.record_stream(stream)
+        self.table.record_stream(stream)    # a side stream reads the pointer table and every gradient tensor
         B.psync_step_device(self._step, d_arrival, self.d_t_nth, d_step_tag, t, stream)   # K1 + K2, one C call
 
     def aggregate_only(self, gamma_t: float, stream=None) -> None:
@@ -129,8 +129,7 @@ class ParameterServerStep:
                 d_n_kept=self.d_n_kept, grad_layout=self.layout,
                 d_tile_start=self._tiles(self.table.grad_dtype) if sharded else None)
             self._tstep = (st, keep, self.table)
-        if stream is not None and hasattr(stream, "cuda_stream"):
-            self.table.d_ptrs.record_stream(stream)
+        self.table.record_stream(stream)    # a side stream reads the pointer table and every gradient tensor
         B.psync_select_timeout(d_arrival, self.W, timeout, self.d_kept_timeout, self.d_n_kept, self.d_status, rows=rows,
                                min_keep=min_keep, d_step_tag=d_step_tag, t=t, stream=stream)
         B.psync_aggregate_update(self._tstep[0], stream)

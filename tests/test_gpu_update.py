@@ -10,7 +10,7 @@ import oracle
 import paper_1702_05800_b200 as psync
 from paper_1702_05800_b200 import synth
 
-from _harness import ATOL_STEP, RTOL_BF16, RTOL_STEP, Pair, assert_close, to_np
+from _harness import ATOL_STEP, RTOL_BF16, RTOL_STEP, STATE_NAMES, Pair, assert_close, to_np
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda"
@@ -358,3 +358,31 @@ def test_device_rsqrt_rn_equals_frsqrt_rn_exhaustively_and_the_mirror_on_a_sampl
     fn = oracle.mirror_lib().mirror_rsqrt_rn
     want = np.array([fn(float(v)) for v in x], dtype=np.float32)
     assert int(bad.item()) == 0 and np.array_equal(d_y.cpu().numpy().view(np.uint32), want.view(np.uint32))
+
+
+def test_steps_in_flight_on_a_side_stream_keep_their_gradients_alive():
+    """Eight set_gradients() / step() pairs enqueued on a side stream with no synchronisation, the caller dropping every
+    reference to the gradient tensors as it goes (more pairs than the plumbing object keeps tables for): the table
+    records the side stream on the pointer table and on every gradient tensor, so torch's allocator cannot hand a block
+    to the next batch while a kernel may still read it.  Same bits as the same steps run one at a time."""
+    cfg = replace(BASE, P=300_007, N=6, b=2, opt=synth.MOMENTUM, name="side_stream")
+    arr = [synth.arrival_times(cfg, s) for s in range(8)]
+    ref = Pair(cfg)
+    for s in range(8):
+        ref.gpu_step(ref.gradients(s), arr[s])
+    pair = Pair(cfg)
+    side = torch.cuda.Stream()
+    d_arr = [torch.from_numpy(a).to(DEV) for a in arr]
+    torch.cuda.synchronize()
+    for s in range(8):
+        grads = pair.gradients(s)                    # allocated and filled on the current stream
+        pair.ps.set_gradients(grads)                 # the pointer table is copied on the current stream too
+        side.wait_stream(torch.cuda.current_stream())
+        pair.ps.step(d_arr[s], cfg.gamma, stream=side)
+        assert side.cuda_stream in pair.ps.table._recorded
+        del grads                                    # the only other reference is the table's
+    torch.cuda.synchronize()
+    for n in STATE_NAMES:
+        a, b_ = getattr(ref.ps, n), getattr(pair.ps, n)
+        if a is not None:
+            assert np.array_equal(to_np(a), to_np(b_)), n
