@@ -2,7 +2,7 @@
 """bench.py -- whole-job throughput of the parameter-server step (Alg. 4) on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg1..cfg5] [--impl psync|reference]
-                    [--mode first_n|per_server|timeout|async] [--layout flat|slices] [--variant 1..8] [--servers M]
+                    [--mode first_n|per_server|timeout|async] [--layout flat|slices] [--variant 1|5|6|7] [--servers M]
 
 The default run is the headline (cfg3, first_n, flat buffers); its JSON line also carries `also`: short
 measurements of cfg2, cfg4, every other mode, the slices layout, many-server cuts and launch variants 5 / 6.
@@ -486,7 +486,7 @@ def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist
             "fused_list": fused_list, "n_eff": n_eff, "bytes_per_step": bytes_per_step, "units": n_eff * cfg.P * K,
             "clocks": clocks, "geo": geo, "launches_per_step": launches_per_step,
             "kernel": ("async_sharded_kernel" if use_tiles else
-                       {1: "async_apply_kernel", 2: "async_apply_pair_kernel"}.get(variant, "async_apply_ring_kernel"))
+                       {1: "async_apply_kernel"}.get(variant, "async_apply_ring_kernel"))
                       if is_async else
                       ("sharded_aggregate_update_ema" if use_tiles else "fused_aggregate_update_ema")}
 
@@ -534,13 +534,11 @@ def run_also(psync, args, wl3, stream, peak):
                                {5: "variant 5: cp.async.bulk + mbarrier ring", 6: "variant 6: 256-bit loads",
                                 7: "variant 7: per-thread cp.async ring (Alg. 2's staging)"}[v]))
         out[-1]["variant"] = v
-    for v in (1, 2):                     # Alg. 2's other launch shapes, re-measured every run (profiles/r2_async.md)
-        wl3.reset_state()
-        m = measure(psync, args, wl3, "async", K, Wm, stream, variant=v, probe_every=2)
-        out.append(short_entry(cfg3, "async", "flat", m, peak,
-                               "variant 1: two register buffers, software-pipelined (the default is the cp.async ring)"
-                               if v == 1 else "variant 2: 8-byte units, one pair of parameters per thread"))
-        out[-1]["variant"] = v
+    wl3.reset_state()                    # Alg. 2's other launch shape, re-measured every run (profiles/r2_async.md)
+    m = measure(psync, args, wl3, "async", K, Wm, stream, variant=1, probe_every=2)
+    out.append(short_entry(cfg3, "async", "flat", m, peak,
+                           "variant 1: two register buffers, software-pipelined (the default is the cp.async ring)"))
+    out[-1]["variant"] = 1
     sets3 = len(wl3.tables)
     del wl3.tables[1:], wl3.sets[1:]     # keep one flat set for the cpu_baseline leg; make room
     torch.cuda.empty_cache()

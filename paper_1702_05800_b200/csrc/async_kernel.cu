@@ -19,10 +19,11 @@
 // step is (gamma G) * rsqrt(ms + eps) with the correctly rounded rsqrt computed by an 8-operation
 // refinement of MUFU.RSQ whose range check is a sticky flag outside the inner loop (psync_device.cuh),
 // and the gradients of the next arrivals are on their way while the current one is applied.
-// Three launch shapes of the same arithmetic (psync_step.variant in psync_async_apply; bit-identical, tested):
+// Two launch shapes of the same arithmetic (psync_step.variant in psync_async_apply; bit-identical, tested):
 //   async_apply_ring_kernel  (0, default) the stream staged through a per-thread cp.async ring in shared memory
 //   async_apply_kernel       (1) two register buffers, software-pipelined batches
-//   async_apply_pair_kernel  (2) 8-byte units, one pair of parameters per thread (fp32 only)
+//   (a third shape, 8-byte units -- one pair of parameters per thread -- measured 3.5 % slower on cfg3's shape,
+//    profiles/r2_async.md, and was removed after round 2)
 
 #include "async_common.cuh"
 
@@ -172,111 +173,11 @@ __global__ void __launch_bounds__(THREADS, MINB) async_apply_kernel(const FusedP
   }
 }
 
-// K4 with 8-BYTE units (fp32 gradients): one PAIR of parameters per thread instead of two pairs.  Same arithmetic per
-// pair (update_pair_g), half the registers for state and gradient buffers -> more resident warps to overlap the FMA pipe
-// with HBM.  Selected by psync_step.variant = 2 in psync_async_apply: an A/B shape kept so that the comparison can be re-run;
-// bit-identical to the 16-byte form (tested) and 3.5 % SLOWER on cfg3's shape, so it is not the default anywhere.
-template <int THREADS, int U, int MINB, int OPT, int EMA, bool SCALED>
-__global__ void __launch_bounds__(THREADS, MINB) async_apply_pair_kernel(const FusedParams p) {
-  __shared__ const char* s_ptr[kMaxWorkers];
-  __shared__ float s_gamma[kMaxWorkers];
-  __shared__ float s_scale[kMaxWorkers];
-
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-
-  if (p.status != nullptr && *p.status != 0) return;
-  const int K = p.n_kept ? *p.n_kept : p.N;
-  if (K <= 0 || K > kMaxWorkers) return;
-
-  unsigned misalign = 0;
-  for (int i = threadIdx.x; i < K; i += THREADS) {
-    const int k = p.kept[i];
-    const char* g = static_cast<const char*>(p.grads[k]);
-    s_ptr[i] = g;
-    s_scale[i] = p.gscales ? p.gscales[k] : 1.0f;
-    s_gamma[i] = p.gammas ? p.gammas[i] : p.gamma;
-    misalign |= static_cast<unsigned>(reinterpret_cast<uintptr_t>(g)) & 7u;
-  }
-  const bool vec_ok = (__syncthreads_or(static_cast<int>(misalign)) == 0) && (p.base_aligned != 0);
-
-  const PairCoeffs pc = make_pair_coeffs(p);
-  const int64_t n_units = vec_ok ? p.P / 2 : 0;
-  for (int64_t u = static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x; u < n_units;
-       u += static_cast<int64_t>(gridDim.x) * THREADS) {
-    const int64_t e = u * 2;
-    float2 th = ld_state8(p.theta + e), em = make_float2(0.f, 0.f), a0 = make_float2(0.f, 0.f), a1 = make_float2(0.f, 0.f);
-    if (EMA != EMA_OFF) em = ld_state8(p.ema + e);
-    if (OPT != OPT_SGD) a0 = ld_state8(p.s0 + e);
-    if (OPT == OPT_RMSPROP_MOM) a1 = ld_state8(p.s1 + e);
-    unsigned bad = 0;
-    const int n_batches = K / U;
-    uint2 cur[U], nxt[U];
-    if (n_batches > 0) {
-#pragma unroll
-      for (int v = 0; v < U; ++v) cur[v] = ldg_stream8(s_ptr[v] + u * 8);
-    }
-    for (int b = 0; b < n_batches; ++b) {
-      const int i = b * U;
-      if (b + 1 < n_batches) {
-#pragma unroll
-        for (int v = 0; v < U; ++v) nxt[v] = ldg_stream8(s_ptr[i + U + v] + u * 8);
-      }
-      __syncwarp();  // scheduling fence: the loads above are issued before the updates below
-#pragma unroll
-      for (int v = 0; v < U; ++v)
-        update_pair_g<OPT, EMA, SCALED>(make_float2(__uint_as_float(cur[v].x), __uint_as_float(cur[v].y)),
-                                        dup2(s_scale[i + v]), dup2(s_gamma[i + v]), th, em, a0, a1, pc, bad);
-#pragma unroll
-      for (int v = 0; v < U; ++v) cur[v] = nxt[v];
-    }
-    for (int i = n_batches * U; i < K; ++i) {
-      const uint2 r = ldg_stream8(s_ptr[i] + u * 8);
-      update_pair_g<OPT, EMA, SCALED>(make_float2(__uint_as_float(r.x), __uint_as_float(r.y)), dup2(s_scale[i]),
-                                      dup2(s_gamma[i]), th, em, a0, a1, pc, bad);
-    }
-    if (OPT == OPT_RMSPROP_MOM && rsqrt_pair_left_range(bad)) {  // redo with the checked scalar update
-      th = ld_state8(p.theta + e);
-      if (EMA != EMA_OFF) em = ld_state8(p.ema + e);
-      a0 = ld_state8(p.s0 + e);
-      a1 = ld_state8(p.s1 + e);
-      for (int n = 0; n < K; ++n) {
-        const uint2 r = ldg_stream8(s_ptr[n] + u * 8);
-        update_element_g<OPT, EMA>(__uint_as_float(r.x), s_scale[n], s_gamma[n], th.x, em.x, a0.x, a1.x, p);
-        update_element_g<OPT, EMA>(__uint_as_float(r.y), s_scale[n], s_gamma[n], th.y, em.y, a0.y, a1.y, p);
-      }
-    }
-    st_state8(p.theta + e, th);
-    if (EMA != EMA_OFF) st_state8(p.ema + e, em);
-    if (OPT != OPT_SGD) st_state8(p.s0 + e, a0);
-    if (OPT == OPT_RMSPROP_MOM) st_state8(p.s1 + e, a1);
-  }
-
-  const int64_t tail0 = n_units * 2;
-  const bool mine = vec_ok ? (blockIdx.x == 0) : true;
-  if (tail0 < p.P && mine) {
-    const int64_t first = vec_ok ? threadIdx.x : static_cast<int64_t>(blockIdx.x) * THREADS + threadIdx.x;
-    const int64_t stride = vec_ok ? THREADS : static_cast<int64_t>(gridDim.x) * THREADS;
-    for (int64_t e = tail0 + first; e < p.P; e += stride) {
-      float th = p.theta[e];
-      float em = (EMA != EMA_OFF) ? p.ema[e] : 0.f;
-      float a0 = (OPT != OPT_SGD) ? p.s0[e] : 0.f;
-      float a1 = (OPT == OPT_RMSPROP_MOM) ? p.s1[e] : 0.f;
-      for (int i = 0; i < K; ++i)
-        update_element_g<OPT, EMA>(load_grad_scalar<false>(s_ptr[i], e), s_scale[i], s_gamma[i], th, em, a0, a1, p);
-      p.theta[e] = th;
-      if (EMA != EMA_OFF) p.ema[e] = em;
-      if (OPT != OPT_SGD) p.s0[e] = a0;
-      if (OPT == OPT_RMSPROP_MOM) p.s1[e] = a1;
-    }
-  }
-}
-
 // K4 with the gradient stream staged through a per-thread ring in SHARED memory (cp.async, LDGSTS): the loads in flight
 // live in shared memory instead of registers, so D arrivals per thread are on their way while one is applied, without the
 // second register buffer of the pipelined form.  Every thread copies and consumes only its own 16-byte slots, so the only
-// synchronisation is cp.async.wait_group -- no barrier.  Selected by psync_step.variant = 3 in psync_async_apply (flat
-// buffers, one order): an A/B shape, bit-identical to the default.
+// synchronisation is cp.async.wait_group -- no barrier.  The default of psync_async_apply (flat buffers,
+// one order); bit-identical to the register-pipelined form.
 template <int D, int MINB, bool BF16, int OPT, int EMA, bool SCALED>
 __global__ void __launch_bounds__(256, MINB) async_apply_ring_kernel(const FusedParams p) {
   constexpr int THREADS = 256;
@@ -488,29 +389,6 @@ cudaError_t async_geometry(int dtype, int grid_ctas, int64_t P, FusedGeometry* o
   return cudaSuccess;
 }
 
-// variant 2: the 8-byte-unit shape (fp32 gradients only), batches of 8 at 4 CTAs/SM -- the best of the five shapes
-// measured ({4,5} 2.124 ms, {3,5} 2.155, {6,4} 1.952, {3,6} 2.019, {8,4} 1.886 on cfg3's shape against 1.822 for the
-// 16-byte default): more resident warps do not help, bytes in flight per thread do (profiles/r2_async.md).
-template <int OPT, int EMA>
-KernelFn pick_pair_scaled(bool scaled) {
-  return scaled ? async_apply_pair_kernel<256, 8, 4, OPT, EMA, true> : async_apply_pair_kernel<256, 8, 4, OPT, EMA, false>;
-}
-template <int OPT>
-KernelFn pick_pair_ema(int ema, bool scaled) {
-  switch (ema) {
-    case EMA_POST: return pick_pair_scaled<OPT, EMA_POST>(scaled);
-    case EMA_PRE: return pick_pair_scaled<OPT, EMA_PRE>(scaled);
-    default: return pick_pair_scaled<OPT, EMA_OFF>(scaled);
-  }
-}
-KernelFn pick_pair(int opt, int ema, bool scaled) {
-  switch (opt) {
-    case OPT_SGD: return pick_pair_ema<OPT_SGD>(ema, scaled);
-    case OPT_MOMENTUM: return pick_pair_ema<OPT_MOMENTUM>(ema, scaled);
-    default: return pick_pair_ema<OPT_RMSPROP_MOM>(ema, scaled);
-  }
-}
-
 // the shared-memory ring (cp.async): {ring depth, CTAs per SM}.  Depth 4 / 6 / 8 are within 1 % of one another on
 // every shape (cfg3's: 1.769 / 1.753 / 1.759 ms), 5 or 6 CTAs/SM are slower (profiles/r2_async.md).
 struct RingShape {
@@ -559,22 +437,6 @@ cudaError_t launch_async_apply_ring(const FusedParams& p, int dtype, int opt, in
   cfg.numAttrs = 1;
   const bool scaled = p.gscales != nullptr;
   return cudaLaunchKernelEx(&cfg, dtype == 1 ? pick_ring<true>(opt, ema, scaled) : pick_ring<false>(opt, ema, scaled), p);
-}
-
-cudaError_t launch_async_apply_pair(const FusedParams& p, int opt, int ema, int grid_ctas, cudaStream_t stream) {
-  int64_t grid = grid_ctas > 0 ? grid_ctas : (p.P / 2 + 255) / 256;
-  if (grid > 0x7FFFFFFF) grid = 0x7FFFFFFF;
-  if (grid < 1) grid = 1;
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(static_cast<unsigned>(grid));
-  cfg.blockDim = dim3(256);
-  cfg.stream = stream;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr;
-  cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, pick_pair(opt, ema, p.gscales != nullptr), p);
 }
 
 cudaError_t launch_async_apply(const FusedParams& p, int dtype, int opt, int ema, int grid_ctas, cudaStream_t stream) {

@@ -584,20 +584,20 @@ __global__ void __launch_bounds__(256) ema_kernel(float* __restrict__ ema, const
 }
 
 // ---- variants and dispatch ---------------------------------------------------------------------
-enum VariantKind { kPlain128 = 0, kBulkRing = 1, kPlain256 = 2, kThreadRing = 3 };
+enum VariantKind { kPlain128 = 0, kBulkRing = 1, kPlain256 = 2, kThreadRing = 3, kRemoved = 4 };
 struct Variant {
   int threads, upt, unroll, minb, kind;
 };
 // variant ids are 1-based in the ABI (0 = default)
 constexpr Variant kVariants[] = {
     {256, 1, 8, 4, kPlain128},    // 1  the default: 128-bit loads, 8 in flight per thread, 4 CTAs/SM
-    {256, 2, 8, 2, kPlain128},    // 2
-    {256, 1, 16, 3, kPlain128},   // 3
-    {512, 1, 8, 2, kPlain128},    // 4
+    {256, 2, 8, 2, kRemoved},     // 2  } other tile shapes of the plain kernel (2 units per thread, 16 loads in flight,
+    {256, 1, 16, 3, kRemoved},    // 3  } 512 threads): "no size at which one wins" (profiles/r2_variants.md), removed
+    {512, 1, 8, 2, kRemoved},     // 4  } after round 2 -- the ids stay reserved and return PSYNC_EUNSUPPORTED
     {256, 1, 12, 3, kBulkRing},   // 5  cp.async.bulk -> 12-stage shared-memory ring (unroll = stages), 1 producer warp
     {256, 1, 8, 2, kPlain256},    // 6  256-bit loads with L2::evict_first, 8 in flight per thread
     {256, 1, 8, 4, kThreadRing},  // 7  per-thread cp.async ring in shared memory (unroll = depth), state requested up front
-    {128, 1, 8, 8, kPlain128},    // 8  half-size tiles: 128 threads, 512 fp32 parameters per CTA, 8 CTAs/SM
+    {128, 1, 8, 8, kRemoved},     // 8  half-size tiles (128 threads, 8 CTAs/SM): no gain (profiles/r2_small_points.md), removed
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 constexpr int kRingStages = kVariants[4].unroll;
@@ -670,13 +670,10 @@ KernelFn pick_dtype(int dtype, int opt, int ema) {
 KernelFn pick_kernel(int v, int dtype, int opt, int ema) {
   switch (v) {
     case 0: return pick_dtype<0>(dtype, opt, ema);
-    case 1: return pick_dtype<1>(dtype, opt, ema);
-    case 2: return pick_dtype<2>(dtype, opt, ema);
-    case 3: return pick_dtype<3>(dtype, opt, ema);
     case 4: return pick_dtype<4>(dtype, opt, ema);
     case 5: return pick_dtype<5>(dtype, opt, ema);
     case 6: return pick_dtype<6>(dtype, opt, ema);
-    default: return pick_dtype<7>(dtype, opt, ema);
+    default: return nullptr;  // a removed variant (the ABI refuses it before it gets here)
   }
 }
 
@@ -688,6 +685,10 @@ int resolve_variant(int variant) {
 }  // namespace
 
 int fused_num_variants() { return kNumVariants; }
+
+bool fused_variant_exists(int variant) {
+  return variant == 0 || (variant >= 1 && variant <= kNumVariants && kVariants[variant - 1].kind != kRemoved);
+}
 
 int sm_count() {
   int dev = 0, sms = 0;
@@ -729,6 +730,7 @@ cudaError_t launch_fused(const FusedParams& p, int dtype, int opt, int ema, int 
   const int v = resolve_variant(variant);
   const bool rows = p.per_shard || p.n_kept != nullptr;
   const KernelFn kernel = rows ? pick_rows_kernel(dtype, opt, ema) : pick_kernel(v, dtype, opt, ema);
+  if (kernel == nullptr) return cudaErrorInvalidValue;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(static_cast<unsigned>(g.grid));
   cfg.blockDim = dim3(static_cast<unsigned>(g.block));

@@ -41,6 +41,7 @@ int check_step(const psync_step* s, bool need_device_tables) {
     return PSYNC_EINVAL;
   if ((s->per_shard || s->d_n_kept != nullptr || s->grad_layout == PSYNC_GRADS_SLICES) && s->variant > 1)
     return PSYNC_EUNSUPPORTED;  // rows / shard-aware kernels: default launch shape only
+  if (!psync::fused_variant_exists(s->variant)) return PSYNC_EUNSUPPORTED;  // an id whose kernel was removed (2, 3, 4, 8)
   return PSYNC_OK;
 }
 
@@ -272,11 +273,13 @@ PSYNC_API int psync_order_by_arrival_sharded(const float* d_arrival, int32_t W, 
 PSYNC_API int psync_async_apply(const psync_step* step, const float* d_gamma, const float* d_gscale, void* stream) {
   if (step == nullptr) return PSYNC_EINVAL;
   psync_step s = *step;
-  // launch shapes of the flat single-order kernel: 0 / 3 the shared-memory ring (default), 1 the register-pipelined form,
-  // 2 8-byte units (fp32 only); the sharded kernel has one shape
+  // launch shapes of the flat single-order kernel: 0 the shared-memory ring (default), 1 the register-pipelined form.
+  // Everything else is refused: the work-list kernel (per server / slices) has one shape, the 8-byte-unit shape (2)
+  // was removed after round 2 (measured slower, profiles/r2_async.md).
   const bool flat_one_order = step->per_shard == 0 && step->grad_layout == PSYNC_GRADS_FLAT;
-  const bool pair_shape = step->variant == 2 && step->grad_dtype == PSYNC_F32 && flat_one_order;
-  const bool ring_shape = (step->variant == 0 || step->variant == 3) && flat_one_order;
+  if (step->variant < 0) return PSYNC_EINVAL;
+  if (step->variant > (flat_one_order ? 1 : 0)) return PSYNC_EUNSUPPORTED;
+  const bool ring_shape = step->variant == 0 && flat_one_order;
   s.variant = 0;
   const int st = check_step(&s, true);
   if (st != PSYNC_OK) return st;
@@ -288,7 +291,6 @@ PSYNC_API int psync_async_apply(const psync_step* step, const float* d_gamma, co
   p.gscales = d_gscale;
   const cudaError_t err =
       ring_shape ? psync::launch_async_apply_ring(p, s.grad_dtype, s.opt, s.ema_mode, s.grid_ctas, static_cast<cudaStream_t>(stream)) :
-      pair_shape ? psync::launch_async_apply_pair(p, s.opt, s.ema_mode, s.grid_ctas, static_cast<cudaStream_t>(stream)) :
       wants_sharded(&s) ? psync::launch_async_sharded(p, s.grad_dtype, s.opt, s.ema_mode, sharded_tiles(&s),
                                                       static_cast<cudaStream_t>(stream))
                         : psync::launch_async_apply(p, s.grad_dtype, s.opt, s.ema_mode, s.grid_ctas,

@@ -35,7 +35,7 @@ def test_launch_bound_reports_eager_and_graph_costs_for_both_algorithms():
 
 
 @pytest.mark.parametrize("flags", [("--mode", "async"), ("--mode", "async_per_server", "--layout", "slices"),
-                                   ("--mode", "per_server", "--layout", "slices"), ("--variant", "7"), ("--variant", "8")])
+                                   ("--mode", "per_server", "--layout", "slices"), ("--variant", "7"), ("--variant", "5")])
 def test_small_config_through_every_mode_line_has_the_contract_keys(flags):
     d = run_bench("--config", "cfg2", "--steps", "3", "--warmup", "3", "--no-cpu-baseline", "--no-e2e", "--no-probe",
                   "--no-also", *flags)

@@ -49,7 +49,7 @@ def test_synchronous_step_every_template_instance(dtype, opt, ema_mode):
             assert_bits(pair.ps, pair.host, f"{cfg.name} step {s}")
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6, 7, 8])   # 5: cp.async.bulk ring; 6: 256-bit loads; 7: per-thread cp.async ring; 8: half-size tiles
+@pytest.mark.parametrize("variant", [1, 5, 6, 7])   # 5: cp.async.bulk ring; 6: 256-bit loads; 7: per-thread cp.async ring (2, 3, 4, 8 were removed)
 def test_every_variant_and_the_scalar_path(variant):
     cfg = replace(BASE, opt=synth.RMSPROP_MOM, N=100, b=6, P=40_001, name=f"bits_variant{variant}")
     pair = Pair(cfg, variant=variant)

@@ -33,7 +33,7 @@ def test_every_template_instance_lockstep(dtype, opt, ema_mode):
     Pair(cfg).run(3, lockstep=True, rtol=RTOL_STEP, atol=ATOL_STEP)
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6, 7, 8])   # 5: cp.async.bulk ring; 6: 256-bit loads; 7: per-thread cp.async ring; 8: half-size tiles
+@pytest.mark.parametrize("variant", [1, 5, 6, 7])   # 5: cp.async.bulk ring; 6: 256-bit loads; 7: per-thread cp.async ring (2, 3, 4, 8 were removed)
 @pytest.mark.parametrize("dtype", [synth.F32, synth.BF16])
 def test_every_variant(variant, dtype):
     cfg = replace(BASE, grad_dtype=dtype, opt=synth.RMSPROP_MOM, N=21, b=2, P=200_001, name=f"variant{variant}")
@@ -152,10 +152,10 @@ def test_bitwise_invariance_shard_layout_launch_variant_and_rerun():
     ref = None
     P = cfg.P
     layouts = [None, [0, P], [0, 1, 2, 77_777, 77_777, P]]
-    # the eight launch variants differ in tile size (512 ... 2048 parameters), load width (128 / 256 bit) and staging
-    # (registers / cp.async.bulk ring): the fixed-order fp32 sum must give the same bits in all of them.  (grid_ctas
+    # the four launch variants differ in load width (128 / 256 bit: 1024 / 2048 parameters per tile) and staging
+    # (registers / cp.async.bulk ring / per-thread cp.async ring): the fixed-order fp32 sum must give the same bits in all of them.  (grid_ctas
     # is accepted and ignored by this kernel, so it is not a dimension here.)
-    runs = [(lay, 0, 0) for lay in layouts] + [(None, 0, v) for v in range(1, 9)]
+    runs = [(lay, 0, 0) for lay in layouts] + [(None, 0, v) for v in (1, 5, 6, 7)]
     runs.append((None, 0, 0))   # the same launch again
     for lay, grid, variant in runs:
         pair = Pair(cfg, shard_off=lay, grid_ctas=grid, variant=variant)
@@ -283,6 +283,9 @@ def test_argument_errors_return_einval_and_touch_nothing():
         kw.update(bad)
         step, keep = psync.make_step(**kw)
         assert psync.psync_aggregate_update(step, check=False) == psync.PSYNC_EINVAL, bad
+    for removed in (2, 3, 4, 8):             # ids of tile shapes whose kernels were removed after their A/B
+        step, keep = psync.make_step(**dict(good, variant=removed))
+        assert psync.psync_aggregate_update(step, check=False) == psync.PSYNC_EUNSUPPORTED, removed
     torch.cuda.synchronize()
     assert np.array_equal(before, to_np(pair.ps.theta))
     assert psync.psync_ema(pair.ps.ema, pair.ps.theta, 0.9) == psync.PSYNC_OK
