@@ -319,12 +319,17 @@ class Workload:
                 self.tables.append(psync.binding.GradTable(torch.from_numpy(ptrs.reshape(-1)).to(dev), arenas,
                                                            psync.PSYNC_F32 if esz == 4 else psync.PSYNC_BF16))
             del tmp, dst
+            self.arena_starts = starts
             self.slices_how = "slices carved at 256-byte boundaries from one arena per worker"
         self.theta = synth.init_theta(cfg, dev)
         self.s0, self.s1 = synth.init_state(cfg, dev)
         self.ema = self.theta.clone()
         self.d_off = torch.from_numpy(self.off).to(dev)
         self.d_tiles = psync.psync_shard_worklist(self.d_off, cfg.grad_dtype)
+
+    def break_worklist(self, psync):
+        """--fault worklist: the list of the OTHER gradient dtype (another tile count): the kernel must refuse it."""
+        self.d_tiles = psync.psync_shard_worklist(self.d_off, 1 - self.cfg.grad_dtype)
 
     def with_servers(self, psync, M):
         """The same resident flat gradient sets and state cut into M ragged servers (only the tables change)."""
@@ -348,6 +353,128 @@ class Workload:
             self.s1.copy_(s1)
 
 
+# ------------------------------------------------------------------------------------ proof of what was timed
+RTOL_STEP, RTOL_BF16, ATOL_STEP = 1e-5, 2e-3, 1e-6      # north_star's per-step tolerances (tests/_harness.py)
+
+
+class VerifyError(AssertionError):
+    pass
+
+
+def sample_columns(cfg, off, n_sample=20_000):
+    """The parameter indices a timed configuration is checked on: the first and last tiles, both sides of every shard
+    cut, and n_sample uniformly drawn ones (sorted, unique) -- the index set of tests/test_gpu_configs.py."""
+    rng = np.random.default_rng(1000 + cfg.cfg_id)
+    tile = min(8192, cfg.P)
+    cuts = np.asarray(off[1:-1], dtype=np.int64)
+    if cuts.size > 4096:                                 # thousands of servers: a seeded subset of the cuts
+        cuts = rng.choice(cuts, 4096, replace=False)
+    idx = np.concatenate([np.arange(0, tile), np.arange(cfg.P - tile, cfg.P), cuts, np.maximum(cuts - 1, 0),
+                          rng.integers(0, cfg.P, n_sample)])
+    return np.unique(idx).astype(np.int64)
+
+
+def gather_gradient_columns(wl, set_id, idx, d_idx):
+    """Columns idx of every worker's gradient of one resident set, as W host arrays (moves data, computes nothing)."""
+    cfg = wl.cfg
+    data = wl.sets[set_id]
+    if wl.layout == "flat":
+        return [synth.as_numpy_grad(g[d_idx]) for g in data]
+    server = np.searchsorted(wl.off, idx, side="right") - 1          # owner j of every sampled parameter
+    local = idx - wl.off[server]
+    if hasattr(wl, "arena_starts"):                                      # slices carved from one arena per worker
+        d_pos = torch.from_numpy(wl.arena_starts[server] + local).to(wl.dev)
+        return [synth.as_numpy_grad(a[d_pos]) for a in data]
+    out = []
+    bounds = np.searchsorted(server, np.arange(cfg.M + 1))               # sampled columns of server j: [b[j], b[j+1])
+    d_local = torch.from_numpy(local).to(wl.dev)
+    for row in data:                                                     # row[j]: worker's own slice for server j
+        parts = [row[j][d_local[bounds[j]:bounds[j + 1]]] for j in range(cfg.M) if bounds[j + 1] > bounds[j]]
+        out.append(synth.as_numpy_grad(torch.cat(parts)))
+    return out
+
+
+def verify_step(cfg, off, mode, timeout, arrival, g_s, before, after, kept_g, n_g, idx, d_idx, gscales=None):
+    """Replays ONE step of what `measure` times through the CPU oracle on the sampled columns and compares: the kept
+    rows / arrival orders bit for bit, theta / state / ema at north_star's tolerance (PAPER.md:L130, L157-162 for Alg. 4,
+    L84-87 for Alg. 2).  `before` holds the sampled state just before the step.  Returns the `verified` object or raises
+    VerifyError.  g_s: the sampled columns of the W gradients (host arrays); after: the device tensors theta / ema /
+    state0 / state1 after the step; kept_g [rows][stride] / n_g [rows]: what the device selected (None: not returned by
+    this path, only the state is checked).  The oracle is on the checking side only: nothing here feeds the timed path."""
+    import oracle
+    W, N, M = cfg.W, cfg.N, cfg.M
+    off_s = np.searchsorted(idx, off).astype(np.int64)                  # the shard table of the sampled columns
+    have_kept = kept_g is not None
+    if not have_kept:
+        kept_g, n_g = np.full((M, W), -2, dtype=np.int32), np.full(M, -2, dtype=np.int32)
+    h = {n: (None if v is None else v.copy()) for n, v in before.items()}
+    kw = dict(opt=cfg.opt, ema_mode=cfg.ema_mode, gamma_t=cfg.gamma, alpha=cfg.alpha, mu=cfg.mu, rho=cfg.rho, eps=cfg.eps)
+    K_applied = N
+    if mode == "first_n":
+        st, kept_o, _ = oracle.select_first_n(arrival, N, cfg.b)
+        same = st == oracle.OK and np.array_equal(kept_g[0, :N], kept_o)
+        rc = oracle.aggregate_update(off_s, N, g_s, kept_o, h["theta"], h["ema"], h["state0"], h["state1"], **kw)
+    elif mode == "per_server":
+        st, kept_o, _ = oracle.select_first_n_sharded(arrival, N, cfg.b)
+        same = bool((st == oracle.OK).all()) and np.array_equal(kept_g[:, :N], kept_o)
+        rc = oracle.aggregate_update_rows(off_s, N, g_s, kept_o, h["theta"], h["ema"], h["state0"], h["state1"],
+                                          per_shard=True, **kw)
+    elif mode == "timeout":
+        st, kept_o = oracle.select_timeout(arrival, timeout)
+        same = st == oracle.OK and int(n_g[0]) == kept_o.size and np.array_equal(kept_g[0, :kept_o.size], kept_o)
+        row = np.full((1, W), -1, dtype=np.int32)
+        row[0, :kept_o.size] = kept_o
+        rc = oracle.aggregate_update_rows(off_s, N, g_s, row, h["theta"], h["ema"], h["state0"], h["state1"],
+                                          per_shard=False, n_kept=np.array([kept_o.size], dtype=np.int32), **kw)
+        K_applied = kept_o.size
+    elif mode == "async":
+        order = oracle.order_by_arrival(arrival)
+        same = int(n_g[0]) == order.size and np.array_equal(kept_g[0, :order.size], order)
+        rc = oracle.async_apply(off_s, g_s, order, h["theta"], h["ema"], h["state0"], h["state1"],
+                                gscales=None if gscales is None else gscales[order].copy(), **kw)
+        K_applied = order.size
+    else:                                                                # async_per_server
+        order = np.full((M, W), -1, dtype=np.int32)
+        n_arr = np.zeros(M, dtype=np.int32)
+        for j in range(M):
+            o = oracle.order_by_arrival(arrival[j])
+            order[j, :o.size], n_arr[j] = o, o.size
+        same = np.array_equal(n_g, n_arr) and all(np.array_equal(kept_g[j, :n_arr[j]], order[j, :n_arr[j]]) for j in range(M))
+        rc = oracle.async_apply_rows(off_s, g_s, order, h["theta"], h["ema"], h["state0"], h["state1"], slices=False,
+                                     per_shard=True, n_arrived=n_arr, gscales=gscales, **kw)
+        K_applied = int(n_arr.max())
+    if have_kept and not same:
+        raise VerifyError(f"{cfg.name} {mode}: kept rows / arrival order differ from the oracle's")
+    if rc != oracle.OK:
+        raise VerifyError(f"{cfg.name} {mode}: oracle returned {rc}")
+    is_async = mode in ("async", "async_per_server")
+    rtol = 1e-6 * max(10, K_applied) if is_async else (RTOL_BF16 if cfg.grad_dtype == synth.BF16 else RTOL_STEP)
+    worst, max_rel, max_abs, moved = 0.0, 0.0, 0.0, 0
+    for n, t in after.items():
+        if t is None or h[n] is None:
+            continue
+        got = t[d_idx].cpu().numpy().astype(np.float64)
+        want = h[n].astype(np.float64)
+        err = np.abs(got - want)
+        if not np.isfinite(got).all():
+            raise VerifyError(f"{cfg.name} {mode}: non-finite {n}")
+        worst = max(worst, float((err / (ATOL_STEP + rtol * np.abs(want))).max()))
+        max_abs = max(max_abs, float(err.max()))
+        big = np.abs(want) >= 1e-3
+        if big.any():
+            max_rel = max(max_rel, float((err[big] / np.abs(want[big])).max()))
+        if n == "theta":
+            moved = int((got != before["theta"].astype(np.float64)).sum())
+    if worst > 1.0:
+        raise VerifyError(f"{cfg.name} {mode}: sampled state differs from the oracle by {worst:.3g} x the tolerance "
+                          f"(rtol {rtol:g}, atol {ATOL_STEP:g}); max abs error {max_abs:.3g}")
+    if cfg.gamma != 0 and moved < idx.size // 2:
+        raise VerifyError(f"{cfg.name} {mode}: only {moved} of {idx.size} sampled parameters changed in the step")
+    return {"elements": int(idx.size), "kept_bit_exact": True if have_kept else None, "max_rel_err": max_rel, "max_abs_err": max_abs,
+            "max_err_over_tolerance": worst, "rtol": rtol, "atol": ATOL_STEP, "theta_changed": moved,
+            "how": "one more step after the timed region, same launch, replayed by the CPU oracle on the sampled columns"}
+
+
 def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist=True, clip=0.0, probe_every=4):
     """W warm-up + K timed steps of one (workload, mode) on `stream`; returns the per-step numbers, the fused kernel's
     own CUDA-event duration (every `probe_every`-th timed step) and the clocks sampled during the timed region.
@@ -362,10 +489,10 @@ def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist
     per_server = mode in ("per_server", "async_per_server")
     is_async = mode in ("async", "async_per_server")
     rows = cfg.M if per_server else 1
-    if per_server:
-        arr_np = np.stack([synth.arrival_times_per_server(cfg, s) for s in range(K + Wm)])
+    if per_server:                       # K + Wm steps, + 1 for the verified step after the timed region
+        arr_np = np.stack([synth.arrival_times_per_server(cfg, s) for s in range(K + Wm + 1)])
     else:
-        arr_np = np.stack([synth.arrival_times(cfg, s) for s in range(K + Wm)])
+        arr_np = np.stack([synth.arrival_times(cfg, s) for s in range(K + Wm + 1)])
     arrivals = torch.from_numpy(arr_np).to(dev)
     stride = cfg.W if (mode == "timeout" or is_async) else cfg.N
     d_kept = torch.full((rows, stride), -1, dtype=torch.int32, device=dev)
@@ -470,6 +597,25 @@ def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist
         print("fused ms per probed step:", [round(x, 4) for x in fused_list], file=sys.stderr)
     assert bool((d_status == 0).all()) and bool(torch.isfinite(wl.theta[:4096]).all())
 
+    # Proof that what was timed computes Alg. 4 / Alg. 2: one more step through exactly the same calls, outside the timed
+    # region, checked against the CPU oracle on sampled columns (kept rows bit for bit, state at north_star's tolerance).
+    verified = None
+    if not getattr(args, "no_verify", False):
+        idx = sample_columns(cfg, wl.off, args.verify_sample)
+        d_idx = torch.from_numpy(idx).to(dev)
+        before = {n: (None if t is None else t[d_idx].cpu().numpy())
+                  for n, t in (("theta", wl.theta), ("ema", wl.ema), ("state0", wl.s0), ("state1", wl.s1))}
+        torch.cuda.synchronize()
+        iv = Wm + K
+        one_step(iv)
+        torch.cuda.synchronize()
+        if not bool((d_status == 0).all()):
+            raise VerifyError(f"{cfg.name} {mode}: device status {d_status.cpu().tolist()[:8]}")
+        verified = verify_step(cfg, wl.off, mode, args.timeout, arr_np[iv], gather_gradient_columns(wl, iv % n_sets, idx, d_idx),
+                               before, {"theta": wl.theta, "ema": wl.ema, "state0": wl.s0, "state1": wl.s1},
+                               d_kept.cpu().numpy(), None if d_n_kept is None else d_n_kept.cpu().numpy(), idx, d_idx,
+                               gscales=None if d_scales is None else d_scales.cpu().numpy())
+
     # gradient elements aggregated per step: N*P, or (workers in time)*P for the time-out rule
     if is_async:
         n_eff = float(cfg.W)                 # every gradient is applied (nothing is dropped in Alg. 2)
@@ -483,6 +629,7 @@ def measure(psync, args, wl, mode, K, Wm, stream, dist=None, variant=0, worklist
         bytes_per_step += cfg.W * cfg.P * cfg.grad_bytes      # the norm pass reads every buffer once more
         launches_per_step = 4                # + sum-of-squares chunks + clip factors
     return {"total_ms": total_ms, "ms_per_step": total_ms / K, "fused_ms": fused_ms, "select_ms": select_ms,
+            "verified": verified,
             "fused_list": fused_list, "n_eff": n_eff, "bytes_per_step": bytes_per_step, "units": n_eff * cfg.P * K,
             "clocks": clocks, "geo": geo, "launches_per_step": launches_per_step,
             "kernel": ("async_sharded_kernel" if use_tiles else
@@ -500,6 +647,9 @@ def short_entry(cfg, mode, layout, m, peak, note=None):
          "frac_of_nominal_8TBps": gbs / 8000.0,
          "value": m["units"] / (m["total_ms"] * 1e-3), "unit": UNIT, "launch": m["geo"],
          "clocks": {k: m["clocks"].get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons")}}
+    if m.get("verified") is not None:
+        v = m["verified"]
+        e["verified"] = {k: v[k] for k in ("elements", "kept_bit_exact", "max_rel_err", "max_err_over_tolerance")}
     if note:
         e["note"] = note
     return e
@@ -580,6 +730,8 @@ def run_psync(args, cfg, rank, world, dist):
         from dataclasses import replace
         cfg = replace(cfg, M=args.servers, name=f"{cfg.name}_M{args.servers}")
     wl = Workload(psync, cfg, dev, args.grad_sets, layout=args.layout)
+    if args.fault == "worklist":
+        wl.break_worklist(psync)
     stream = torch.cuda.Stream(device=dev)
     B = psync.binding
     m = measure(psync, args, wl, mode, K, Wm, stream, dist, variant=args.variant, worklist=not args.no_worklist,
@@ -609,6 +761,7 @@ def run_psync(args, cfg, rank, world, dist):
                      "frac_of_nominal_8TBps": achieved / 8000.0},
         "clocks": m["clocks"],
         "gpu_launches": m["launches_per_step"] * K,
+        "verified": m["verified"],
     }
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_file) and mode == "first_n" and args.layout == "flat" and args.variant in (0, 1):
@@ -645,8 +798,11 @@ def run_psync(args, cfg, rank, world, dist):
 
     headline = (rank == 0 and world == 1 and args.config == "cfg3" and mode == "first_n" and args.layout == "flat"
                 and args.servers <= 0)
+    cfg5_subset = None
     if headline and not args.no_also:
         out["also"], _ = run_also(psync, args, wl, stream, peak)
+        if not args.no_cfg5:
+            cfg5_subset = run_cfg5_subset(psync, args, dev, stream, peak)
 
     # the CPU baseline leg: the exact bytes of gradient set 0, copied D2H before any oracle timing
     host_grads = None
@@ -683,7 +839,48 @@ def run_psync(args, cfg, rank, world, dist):
                 oracle.set_num_threads(threads)
             out["cpu_baseline"]["value_1thread"] = v1
             out["cpu_baseline"]["sample_1thread"] = f"first {sub.P} parameters of every buffer; " + info1["sample"]
+    # compact records, assigned LAST so that they are the tail of the JSON line: BASELINE.json's cfg5 metric ("GB/s vs P
+    # and N+b") on a fixed 10-point subset, and one short row per `also` entry
+    if cfg5_subset is not None:
+        out["cfg5"] = cfg5_subset
+    if "also" in out:
+        out["also_summary"] = {
+            "columns": ["kernel_ms", "GB/s", "frac_of_nominal_8TBps", "verified_elements", "max_err_over_tolerance"],
+            "rows": {f"{e['workload']}|{e['mode']}|{e['grad_layout']}" + (f"|v{e['variant']}" if "variant" in e else ""):
+                     [round(e["kernel_ms"], 4), round(e["gbps"], 1), round(e["frac_of_nominal_8TBps"], 3),
+                      e.get("verified", {}).get("elements"), e.get("verified", {}).get("max_err_over_tolerance")]
+                     for e in out["also"]}}
     return out
+
+
+def run_cfg5_subset(psync, args, dev, stream, peak):
+    """Ten points of BASELINE.json's cfg5 sweep in the default run: every P at (N, b) = (100, 10) over M = 64 ragged
+    servers, and every P at (N, b) = (8, 0) on a single shard -- the two ends of the N+b axis.  3 warm-up + 5 timed steps
+    each, each point checked against the oracle like every other timed configuration.  The full 40-point table is
+    `bench.py --config cfg5` (profiles/)."""
+    rows = {}
+    for cfg in synth.sweep_configs():
+        if not ((cfg.N == 100 and cfg.M == 64) or (cfg.N == 8 and cfg.M == 1)):
+            continue
+        set_bytes = cfg.W * cfg.P * cfg.grad_bytes
+        if torch.cuda.mem_get_info()[0] < 1.05 * (set_bytes + 5 * 4 * cfg.P):
+            rows[cfg.name.replace("cfg5_", "")] = "skipped: not enough free HBM next to the headline workload"
+            continue
+        wl = Workload(psync, cfg, dev, 3 if set_bytes < 20e9 else 2)
+        m = measure(psync, args, wl, "first_n", 5, 3, stream, probe_every=1)
+        e = short_entry(cfg, "first_n", "flat", m, peak)
+        l2 = "L2" if cfg.footprint_bytes <= L2_BYTES else ("~L2" if set_bytes < 4 * L2_BYTES else "HBM")
+        rows[cfg.name.replace("cfg5_", "")] = [round(e["kernel_ms"] * 1e3, 2), round(e["gbps"], 1),
+                                               round(e["frac_of_nominal_8TBps"], 3), l2,
+                                               e.get("verified", {}).get("elements"),
+                                               e.get("verified", {}).get("max_err_over_tolerance")]
+        del wl, m
+        torch.cuda.empty_cache()
+    return {"columns": ["kernel_us", "GB/s of algorithmic bytes", "frac_of_nominal_8TBps",
+                        "served from (HBM / ~L2 = one gradient set < 4 x L2 / L2 = footprint fits L2)",
+                        "verified_elements", "max_err_over_tolerance"],
+            "timing": "3 warm-up + 5 timed steps per point, fused kernel by CUDA events, gradient sets rotated when two fit",
+            "rows": rows}
 
 
 def run_sweep(args, rank, world, dist):
@@ -809,6 +1006,31 @@ def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist, 
         assert st == 0
     torch.cuda.synchronize()
     ms = (time.perf_counter() - t0) * 1e3
+    verified = None
+    if not getattr(args, "no_verify", False):     # one more host step, outside the timed region, against the oracle
+        idx = sample_columns(cfg, off, args.verify_sample)
+        d_idx, h_idx = torch.from_numpy(idx).to(dev), torch.from_numpy(idx)
+        state = {"theta": theta, "ema": ema, "state0": s0, "state1": s1}
+        before = {n: (None if t is None else t[d_idx].cpu().numpy()) for n, t in state.items()}
+        a_v = synth.arrival_times(cfg, 2000 + K + 1)
+        st, _ = host_step(a_v)
+        torch.cuda.synchronize()
+        if st != 0:
+            raise VerifyError(f"{cfg.name} e2e: status {st}")
+        if slices:
+            server = np.searchsorted(off, idx, side="right") - 1
+            local = torch.from_numpy(idx - off[server])
+            bounds = np.searchsorted(server, np.arange(len(off)))
+            g_s = [synth.as_numpy_grad(torch.cat([row[j][local[bounds[j]:bounds[j + 1]]] for j in range(len(off) - 1)
+                                                  if bounds[j + 1] > bounds[j]])) for row in h_grads]
+        else:
+            g_s = [synth.as_numpy_grad(h[h_idx]) for h in h_grads]
+        verified = verify_step(cfg, off, mode, args.timeout, a_v, g_s, before, state,
+                               None if is_async else h_kept[None, :].copy(), None, idx, d_idx)
+        got_host = h_theta[h_idx].numpy()                     # what the user reads back: theta(t+1) in host memory
+        if not np.array_equal(got_host, theta[d_idx].cpu().numpy()):
+            raise VerifyError(f"{cfg.name} e2e: theta read back to the host differs from the device's")
+        verified["theta_readback_bit_exact"] = True
     units, max_ms = aggregate_over_ranks(float(n_moved) * cfg.P * K, ms, dist)
     n_chunks = -(-cfg.P // (chunk if chunk else 1 << 20))
     return {"value": units / (max_ms * 1e-3), "unit": UNIT, "steps": K, "ms_per_step": max_ms / K,
@@ -817,6 +1039,7 @@ def run_e2e(args, cfg, dev, off, theta, ema, s0, s1, stream, rank, world, dist, 
             "api": ("psync_async_step_host" if is_async else "psync_step_host") + " (C ABI, pinned host gradient buffers"
                    + (" as W x M per-(worker, server) slices" if slices else "")
                    + ("; all W arriving buffers cross PCIe)" if is_async else "; only the N kept buffers cross PCIe)"),
+            "verified": verified,
             "gpu_launches_per_step": 3 + n_chunks,
             "timing": "host wall clock around synchronous calls (the call returns when theta(t+1) is on the host)"}
 
@@ -1004,6 +1227,12 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-probe", action="store_true", help="skip the live HBM stream probes")
+    ap.add_argument("--no-cfg5", action="store_true", help="skip the 10-point cfg5 subset of the default run")
+    ap.add_argument("--no-verify", action="store_true", help="skip the oracle check of every timed configuration")
+    ap.add_argument("--verify-sample", type=int, default=20_000, help="random columns checked per configuration "
+                    "(+ first / last tile and every shard cut)")
+    ap.add_argument("--fault", default="", choices=["", "worklist"], help="test hook: break the named input on purpose "
+                    "(worklist: a (server, tile) list built for the other gradient dtype) -- the run must exit non-zero")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--cpu-seconds-1thread", type=float, default=3.0)
     ap.add_argument("--clock-period-ms", type=float, default=2.0)

@@ -43,4 +43,34 @@ def test_small_config_through_every_mode_line_has_the_contract_keys(flags):
                 "dtype", "data", "config", "roofline", "clocks", "gpu_launches"):
         assert key in d, key
     assert d["roofline"]["bound"] == "hbm" and 0.3 < d["roofline"]["frac_of_nominal_8TBps"] < 1.0
+    v = d["verified"]                      # every timed configuration is replayed by the oracle on sampled columns
+    assert v["kept_bit_exact"] is True and v["elements"] > 20_000 and v["max_err_over_tolerance"] <= 1.0
+    assert v["theta_changed"] > v["elements"] // 2
     assert d["gpu_launches"] > 0 and d["value"] > 0
+
+
+@pytest.mark.parametrize("flags", [("--mode", "timeout"), ("--mode", "first_n", "--layout", "slices", "--servers", "3000")])
+def test_timeout_mode_and_arena_slices_are_verified_too(flags):
+    d = run_bench("--config", "cfg2", "--steps", "3", "--warmup", "3", "--no-cpu-baseline", "--no-e2e", "--no-probe",
+                  "--no-also", *flags)
+    assert d["verified"]["kept_bit_exact"] is True and d["verified"]["max_err_over_tolerance"] <= 1.0
+
+
+def test_e2e_leg_is_verified_at_the_timed_size():
+    """psync_step_host at cfg2's full size with bench.py's 4 Mi-element chunks: the extra step after the timed loop is
+    replayed by the oracle on sampled columns, and the theta read back to the host equals the device's."""
+    d = run_bench("--config", "cfg2", "--steps", "3", "--warmup", "3", "--no-cpu-baseline", "--no-probe", "--no-also",
+                  "--e2e-steps", "2")
+    v = d["e2e"]["verified"]
+    assert v["kept_bit_exact"] is True and v["theta_readback_bit_exact"] is True and v["max_err_over_tolerance"] <= 1.0
+
+
+def test_a_wrong_work_list_makes_the_bench_exit_non_zero():
+    """The shard-aware kernels return early (theta untouched) when the (server, tile) list does not match the layout:
+    a fast, wrong run.  bench.py must notice: `--fault worklist` hands it the list of the other gradient dtype."""
+    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--config", "cfg2", "--steps", "3", "--warmup", "3",
+           "--no-cpu-baseline", "--no-e2e", "--no-probe", "--no-also", "--mode", "per_server", "--fault", "worklist"]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert out.returncode != 0 and "VerifyError" in out.stderr
+    ok = subprocess.run(cmd[:-2], capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert ok.returncode == 0, ok.stderr[-2000:]
