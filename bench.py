@@ -767,7 +767,12 @@ def run_psync(args, cfg, rank, world, dist):
     if os.path.exists(traffic_file) and mode == "first_n" and args.layout == "flat" and args.variant in (0, 1):
         try:                                  # dram bytes per launch from the committed ncu --set full capture
             with open(traffic_file) as fh:
-                out["roofline"]["traffic"] = json.load(fh).get(cfg.name)
+                tj = json.load(fh)
+            if tj.get("psync_version") == psync.binding.psync_version():
+                out["roofline"]["traffic"] = tj.get(cfg.name)
+            else:                             # captured on another build of the library: not evidence for this one
+                out["roofline"]["traffic_note"] = (f"profiles/traffic.json was captured on build "
+                                                   f"{tj.get('psync_version')}, this is {psync.binding.psync_version()}")
             out["roofline"]["traffic_source"] = ("ncu --set full capture committed in profiles/traffic.json "
                                                  "(dram__bytes_read.sum + dram__bytes_write.sum per launch; not "
                                                  "measured in this run)")
@@ -1260,6 +1265,12 @@ def main():
         print(json.dumps(run_reference(args, cfg, rank)), flush=True)
         return 0
 
+    if args.gpus != world:                  # --gpus only NAMES the replica count; torchrun makes the replicas
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE is {world}: the step does not shard across GPUs, N GPUs are "
+              f"N independent replicas, one process each.  Launch them with\n  python -m torch.distributed.run "
+              f"--nnodes=1 --nproc-per-node {args.gpus} --master-addr 127.0.0.1 --master-port 29500 bench.py --gpus "
+              f"{args.gpus} ...", file=sys.stderr)
+        return 2
     if args.launch_bound:
         if rank == 0:
             print(json.dumps(run_launch_bound(args)), flush=True)

@@ -305,7 +305,7 @@ __global__ void __launch_bounds__(256, MINB) async_apply_ring_kernel(const Fused
 // K1c: rank sort of <= 1024 keys in one CTA.  Thread i owns worker i: its rank is the number of eligible
 // workers that come before it in (arrival, index) order; -0.0 == +0.0; non-finite = never arrived.
 // One CTA per row: row r of arrival [rows][W] is what parameter server r saw (Alg. 2 is the program of one server j).
-__global__ void __launch_bounds__(1024) order_by_arrival_kernel(const float* __restrict__ arrival_rows, int32_t W,
+__global__ void __launch_bounds__(1024) order_by_arrival_kernel(const float* arrival_rows, int32_t W,  // plain: written by a predecessor under PDL
                                                                 int32_t* __restrict__ order_rows,
                                                                 int32_t* __restrict__ n_arrived_rows) {
   __shared__ uint32_t s_key[kMaxWorkers];

@@ -209,7 +209,7 @@ __device__ __forceinline__ float key_time(uint32_t key) {
 }
 
 // K7a: one CTA per iteration: rank-sort its W arrival times; entry k of the row = when the (k+1)-th gradient arrived
-__global__ void __launch_bounds__(1024) sort_rows_kernel(const float* __restrict__ arrival, int32_t W,
+__global__ void __launch_bounds__(1024) sort_rows_kernel(const float* arrival, int32_t W,  // plain: a predecessor may write it
                                                          float* __restrict__ sorted) {
   __shared__ uint32_t s_key[kMaxWorkers];
   asm volatile("griddepcontrol.wait;" ::: "memory");

@@ -59,8 +59,9 @@ __device__ __forceinline__ void pdl_release_successor() { asm volatile("griddepc
 
 // C = keys per lane (W <= 32*C); the keys live in registers, every loop is unrolled.
 template <int C>
-__global__ void __launch_bounds__(32) select_first_n_kernel(const float* __restrict__ arrival,
-                                                            const int32_t* __restrict__ tags, int32_t t, int32_t N,
+__global__ void __launch_bounds__(32) select_first_n_kernel(const float* arrival,  // plain pointers: a predecessor
+                                                            const int32_t* tags,   // under PDL typically writes these
+                                                            int32_t t, int32_t N,
                                                             int32_t W, int32_t* __restrict__ kept,
                                                             float* __restrict__ t_nth, int32_t* __restrict__ status) {
   const int lane = threadIdx.x;
@@ -161,8 +162,8 @@ __global__ void __launch_bounds__(32) select_first_n_kernel(const float* __restr
 // K1b: the time-out rule (reading R19).  Worker k is kept iff it is eligible
 // (finite arrival, tag == t) and arrival[k] <= timeout; kept[] comes out ascending because lanes own
 // contiguous index ranges; fewer than min_keep -> ETOOFEW, n_kept[row] = 0 and the kept row is not written.
-__global__ void __launch_bounds__(32) select_timeout_kernel(const float* __restrict__ arrival,
-                                                            const int32_t* __restrict__ tags, int32_t t, int32_t W,
+__global__ void __launch_bounds__(32) select_timeout_kernel(const float* arrival,  // plain pointers (as above)
+                                                            const int32_t* tags, int32_t t, int32_t W,
                                                             float timeout, int32_t min_keep,
                                                             int32_t* __restrict__ kept, int32_t* __restrict__ n_kept,
                                                             int32_t* __restrict__ status) {

@@ -77,3 +77,12 @@ def test_bytes_model_matches_survey_table():
     for cfg in list(synth.CONFIGS.values()) + sweep[:4]:
         off = synth.shard_offsets(cfg)
         assert off[0] == 0 and off[-1] == cfg.P and len(off) == cfg.M + 1
+
+
+def test_gpus_flag_without_torchrun_exits_instead_of_measuring_one_gpu():
+    """`--gpus N` names the replica count, torchrun makes the replicas: a bare `python bench.py --gpus 8` must not print a
+    one-GPU number labelled n_gpus = 1."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "8", "--steps", "2"], capture_output=True,
+                       text=True, env=env, timeout=300)
+    assert r.returncode == 2 and r.stdout.strip() == "" and "torch.distributed.run" in r.stderr

@@ -79,6 +79,10 @@ class AsyncPair:
             g = getattr(self, n)
             if g is not None:
                 assert_close(to_np(g), h[n], rtol_async(K), ATOL_STEP, f"{cfg.name} step {s} {n}")
+                # the OBSERVED error beside the budget: worst |gpu - oracle| / (atol + rtol |oracle|) seen so far
+                err = np.abs(to_np(g).astype(np.float64) - h[n].astype(np.float64))
+                self.worst_over_budget = max(getattr(self, "worst_over_budget", 0.0),
+                                             float((err / (ATOL_STEP + rtol_async(K) * np.abs(h[n]))).max()))
                 h[n] = to_np(g)
         return order
 
@@ -239,6 +243,8 @@ def test_full_size_async_cfg3_shape_sampled():
     assert rc == oracle.OK
     for n in STATE_NAMES:
         assert_close(to_np(getattr(pair, n)[d_idx]), host[n], rtol_async(106), ATOL_STEP, f"async cfg3 {n} (sampled)")
+        # observed, beside the K-scaled budget: at K = 106 the result also meets north_star's PER-STEP tolerance
+        assert_close(to_np(getattr(pair, n)[d_idx]), host[n], 1e-5, ATOL_STEP, f"async cfg3 {n} (sampled, per-step tolerance)")
     assert bool(torch.isfinite(pair.theta).all())
 
 
@@ -248,6 +254,10 @@ def test_async_max_workers_1024():
     pair = AsyncPair(cfg)
     order = pair.step(0, synth.arrival_times(cfg, 0))
     assert order.size == 1024
+    # rtol_async(1024) = 1e-3 is a budget (1e-6 per applied gradient, R21); what 1024 iterations really
+    # accumulate is far smaller -- the budget is not the only evidence
+    print(f"async K=1024: observed worst error = {pair.worst_over_budget:.3g} x the tolerance")
+    assert pair.worst_over_budget <= 0.05
 
 
 # ------------------------------------------------------------------ staleness bookkeeping (Table 1)
